@@ -1,0 +1,143 @@
+/* mapl.h -- C ABI of the B200-native MAPL boundary codec (libmapl.so).
+ *
+ * MAPL = Manifold Aware Projection Learning, arxiv/paper_2606_05484.  Citations "P:NN" are line NN
+ * of the paper text; "S#" are the readings listed in DESIGN.md.
+ *
+ * The library implements, as hand-written sm_100a CUDA kernels, the per-token pipeline-stage
+ * boundary codec and the step that keeps its projector on the Stiefel manifold:
+ *
+ *   mapl_encode          z = U^T h                          (Eq. 1, Alg. 1 l.1; centring = S6)
+ *                        + residual VQ of z                 (Sec. 3.5)
+ *   mapl_decode          hhat = U zhat + A[tok] B           (Eq. 2, Alg. 1 l.3, Eq. 3)
+ *   mapl_codec_backward  gz = U^T g, dU, dA, dB, dH         (Alg. 1 l.4; STE = S7)
+ *   mapl_stiefel_step    xi = G - U sym(U^T G); U <- Retr(U - lr xi)   (Eq. 4, Eq. 7)
+ *
+ * Notation (paper -> here): X^{b_p} -> H [N,d]; A_p -> U [d,r]; Z^{b_p} -> Z [N,r];
+ * E^small -> A [V,ra]; P_p -> B [ra,d]; t_ids -> tok [N]; C_p -> codebooks [L,K,r].
+ *
+ * GENERAL CONVENTIONS
+ *  - Layout: every tensor is dense row-major (row stride == row length).  Row-vector form:
+ *    Z = H U, Hhat = Zhat U^T + A[tok] B.
+ *  - Memory: unless a parameter says HOST, every pointer is a DEVICE pointer owned by the caller
+ *    (allocate with torch / cudaMalloc).  The library never allocates, frees or keeps a pointer
+ *    after the call returns.  Descriptors are host structs read during the call only.
+ *  - Alignment: every non-NULL device pointer must be 16-byte aligned.
+ *  - Dtypes: U, codebooks, A, B, dU, dA, dB and everything in mapl_stiefel_step are fp32.
+ *    Activations (H, Hhat, g, dH, Z, gz) have desc.act_dtype (fp32 or bf16).  codes, tok: int32.
+ *  - Execution: all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL =
+ *    the legacy default stream).  No host synchronisation, no host read of device data.
+ *  - Errors: every entry point returns a mapl_status (0 = OK, negative = error).  On an argument
+ *    error nothing is enqueued.  No exception crosses the ABI.  CUDA launch failures map to
+ *    MAPL_ERR_CUDA (mapl_last_cuda_error() gives the cudaError_t).
+ *  - Preconditions the host cannot check without a sync (the caller's responsibility):
+ *    0 <= tok[n] < vocab, 0 <= codes[n,l] < rvq_k, U has orthonormal columns, and for the
+ *    Newton-Schulz retraction sigma_max(U - lr xi) < sqrt(3) (S11).
+ *  - There is no CPU fallback: without a CUDA device every compute call returns MAPL_ERR_CUDA.
+ */
+#ifndef MAPL_H_
+#define MAPL_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  MAPL_OK = 0,
+  MAPL_ERR_INVALID_ARG = -1,   /* NULL required pointer, non-positive size, inconsistent combination */
+  MAPL_ERR_UNSUPPORTED = -2,   /* valid request outside the implemented envelope (see each call)     */
+  MAPL_ERR_ALIGNMENT = -3,     /* a device pointer is not 16-byte aligned                             */
+  MAPL_ERR_WORKSPACE = -4,     /* workspace NULL or smaller than mapl_*_workspace_bytes()             */
+  MAPL_ERR_CUDA = -5           /* CUDA runtime error (no device, launch failure)                      */
+} mapl_status;
+
+typedef enum { MAPL_F32 = 0, MAPL_BF16 = 1 } mapl_dtype;
+typedef enum { MAPL_RETRACT_QR = 0, MAPL_RETRACT_NS = 1 } mapl_retraction;
+
+/* One stage boundary (activation X^{b_p} in R^{B x T x d}, N = B*T tokens). */
+typedef struct {
+  int64_t n_tokens;      /* N >= 0 (N == 0: the call is a no-op apart from zeroing overwrite outputs) */
+  int32_t d;             /* hidden size; d >= 8, d % 8 == 0                                          */
+  int32_t r;             /* projector rank; 8 <= r <= d, r % 8 == 0; U is [d,r]                      */
+  int32_t act_dtype;     /* mapl_dtype of H, Hhat, g, dH, Z, gz                                      */
+  int32_t rvq_levels;    /* L; 0 = RVQ off; L <= 8                                                   */
+  int32_t rvq_k;         /* K codewords per level (>= 1 when L > 0); codebooks are [L,K,r] fp32       */
+  int32_t rvq_group_dim; /* must be r or 0 (one group: full-vector RVQ, S3); grouped MCVQ = next     */
+  int32_t vocab;         /* V; A is [V,ra]                                                           */
+  int32_t anchor_rank;   /* ra; 0 = no anchor term; else ra % 8 == 0; B is [ra,d]                    */
+} mapl_boundary_desc;
+
+/* Static strings for a status code / the library build ("mapl-b200 x.y sm_100a"). */
+const char* mapl_status_string(int status);
+const char* mapl_version(void);
+/* cudaError_t of the most recent MAPL_ERR_CUDA on the calling thread (0 if none). */
+int mapl_last_cuda_error(void);
+
+/* Device scratch the three codec calls need for `desc` (max over the three), in bytes; 0 on an
+ * invalid descriptor.  The same workspace may be reused by consecutive calls on one stream.     */
+size_t mapl_workspace_bytes(const mapl_boundary_desc* desc);
+/* Device scratch for mapl_stiefel_step on `batch` projectors of shape [d,r].                    */
+size_t mapl_stiefel_workspace_bytes(int32_t d, int32_t r, int32_t batch);
+
+/* ENCODE (sender side).  P:73 Eq. 1 with h already centred (S6): z_n = U^T h_n.
+ * If desc.rvq_levels == L > 0 (S3, S4): rho_0 = z_n; for l < L:
+ *   codes[n,l] = argmin_k || rho_l - C[l,k,:] ||^2 (lowest k on ties), rho_{l+1} = rho_l - C[l,codes[n,l],:].
+ * z stays on chip between levels.
+ *   H          [N,d] act dtype, read-only.
+ *   U          [d,r] fp32.
+ *   codebooks  [L,K,r] fp32 (ignored / may be NULL when L == 0).
+ *   Zq_out     [N,r] act dtype.  L == 0: required, receives z (the wire payload, 2r bytes/token in
+ *              bf16).  L > 0: optional, receives zhat_n = sum_l C[l,codes[n,l],:].
+ *   codes_out  [N,L] int32; required when L > 0.
+ * Unsupported: rvq_group_dim not in {0, r}; L > 0 with r > 512.                                */
+int mapl_encode(const mapl_boundary_desc* desc, const void* H, const float* U, const float* codebooks,
+                void* Zq_out, int32_t* codes_out, void* workspace, size_t workspace_bytes,
+                void* cuda_stream);
+
+/* DECODE (receiver side).  P:75 Eq. 2 + P:106 Eq. 3: hhat_n = U zhat_n + B^T A[tok_n,:].
+ *   Z / codes  exactly one non-NULL.  Z [N,r] act dtype is used as zhat; codes [N,L] int32 are
+ *              dequantised (zhat_n = sum_l C[l,codes[n,l],:], needs L > 0 and codebooks).
+ *   tok, A, B  required when desc.anchor_rank > 0 (only token ids cross the wire).
+ *   Hhat_out   [N,d] act dtype.                                                                 */
+int mapl_decode(const mapl_boundary_desc* desc, const void* Z, const int32_t* codes, const float* U,
+                const float* codebooks, const int32_t* tok, const float* A, const float* B,
+                void* Hhat_out, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* BACKWARD of loss(Hhat) through decode and encode, straight-through across the quantiser (S7).
+ * With g = dL/dHhat [N,d] ("route the gradient through the same orthogonal projector"):
+ *   gz   = g U                                   [N,r] act dtype (what crosses the wire backwards)
+ *   dU   = g^T Zhat (+ H^T gz when H != NULL)    [d,r] fp32   (Alg. 1 l.4, S8)
+ *   dA[v,:] = sum_{n: tok_n = v} B g_n           [V,ra] fp32  (E_small is trainable)
+ *   dB   = A[tok]^T g                            [ra,d] fp32  (P_p is frozen in the paper: optional)
+ *   dH   = gz U^T                                [N,d] act dtype (optional; needs H != NULL)
+ *   Z / codes  exactly one non-NULL: the zhat the forward pass decoded (as in mapl_decode).
+ *   H          may be NULL: only the decode-side term of dU is formed and dH_out must be NULL.
+ *   gz_out, dU_out required.  dA_out required when anchor_rank > 0 unless A, B, tok are all NULL
+ *   (anchor ignored).  dB_out, dH_out optional (NULL = skipped).
+ *   accumulate 0: dU, dA, dB are overwritten (rows of dA for absent tokens become 0);
+ *              1: results are added to their current contents (micro-batch accumulation).       */
+int mapl_codec_backward(const mapl_boundary_desc* desc, const void* g_Hhat, const void* H, const void* Z,
+                        const int32_t* codes, const float* U, const float* codebooks, const int32_t* tok,
+                        const float* A, const float* B, void* gz_out, float* dU_out, float* dA_out,
+                        float* dB_out, void* dH_out, int accumulate, void* workspace,
+                        size_t workspace_bytes, void* cuda_stream);
+
+/* STIEFEL STEP on `batch` independent projectors, U_inout and G strided [batch,d,r] fp32.
+ *   S = U^T G;  xi = G - U (S + S^T)/2 (Eq. 4);  Y = U - lr xi;
+ *   MAPL_RETRACT_QR: U <- Q of the thin QR of Y with diag(R) > 0 (unique, S17);
+ *   MAPL_RETRACT_NS: X_0 = Y, X_{j+1} = X_j (3I - X_j^T X_j)/2, U <- X_{ns_iters} (S11; the
+ *                    reported configuration is ns_iters = 5; 1 <= ns_iters <= 16).
+ *   U_inout is updated in place.  fp32 storage, fp32-accurate arithmetic: ||U^T U - I||_F <= 1e-5
+ *   after the call for inputs in the documented regime.
+ *   info_out   optional device [batch,2] fp32: ||xi||_F and ||U^T U - I||_F after the update.
+ * Requires 8 <= r <= d, r % 8 == 0, d % 8 == 0, r <= 1024.                                      */
+int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U_inout, const float* G, float lr,
+                      int32_t retraction, int32_t ns_iters, float* info_out, void* workspace,
+                      size_t workspace_bytes, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MAPL_H_ */

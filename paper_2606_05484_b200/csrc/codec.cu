@@ -1,0 +1,255 @@
+// codec.cu -- C-ABI entry points mapl_encode / mapl_decode / mapl_codec_backward (include/mapl.h):
+// host-side validation, workspace carving and kernel selection.  bf16 boundaries whose shape fits
+// the tensor-core envelope run the tcgen05 kernels (tc_*.cu); everything else (fp32 activations,
+// ragged shapes) runs the fp32 SIMT kernels.  There is no CPU path.
+#include <string.h>
+
+#include "common.cuh"
+#include "tc_codec.cuh"
+
+namespace mapl {
+namespace {
+
+int validate_desc(const mapl_boundary_desc* d) {
+  if (!d) return MAPL_ERR_INVALID_ARG;
+  if (d->n_tokens < 0) return MAPL_ERR_INVALID_ARG;
+  if (d->d < 8 || d->d % 8) return MAPL_ERR_INVALID_ARG;
+  if (d->r < 8 || d->r % 8 || d->r > d->d) return MAPL_ERR_INVALID_ARG;
+  if (d->act_dtype != MAPL_F32 && d->act_dtype != MAPL_BF16) return MAPL_ERR_INVALID_ARG;
+  if (d->rvq_levels < 0 || d->rvq_levels > 8) return MAPL_ERR_INVALID_ARG;
+  if (d->rvq_levels > 0 && d->rvq_k < 1) return MAPL_ERR_INVALID_ARG;
+  if (d->anchor_rank < 0 || d->anchor_rank % 8) return MAPL_ERR_INVALID_ARG;
+  if (d->anchor_rank > 0 && d->vocab < 1) return MAPL_ERR_INVALID_ARG;
+  if (d->rvq_levels > 0 && d->rvq_group_dim != 0 && d->rvq_group_dim != d->r) return MAPL_ERR_UNSUPPORTED;
+  if (d->rvq_levels > 0 && d->r > 512) return MAPL_ERR_UNSUPPORTED;
+  if (d->n_tokens > (1ll << 31) - 256) return MAPL_ERR_UNSUPPORTED;
+  return MAPL_OK;
+}
+
+// workspace layout (256-byte aligned segments)
+struct Ws {
+  size_t half_norm = 0;   // [L*K] fp32
+  size_t zhat = 0;        // [N*r] fp32 (dequantised codes, SIMT path)
+  size_t gA = 0;          // [N*ra] fp32
+  size_t tc = 0;          // tensor-core path scratch (parameter packs, partials)
+  size_t total = 0;
+};
+
+Ws carve(const mapl_boundary_desc& d) {
+  Ws w;
+  size_t off = 0;
+  auto seg = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+  w.half_norm = seg((size_t)d.rvq_levels * (size_t)d.rvq_k * 4);
+  w.zhat = seg(d.rvq_levels > 0 ? (size_t)d.n_tokens * d.r * 4 : 0);
+  w.gA = seg((size_t)d.n_tokens * d.anchor_rank * 4);
+  w.tc = seg(tc_workspace_bytes(d));
+  w.total = off + 256;
+  return w;
+}
+
+bool all16(std::initializer_list<const void*> ps) {
+  for (const void* p : ps) if (p && !aligned16(p)) return false;
+  return true;
+}
+
+}  // namespace
+}  // namespace mapl
+
+using namespace mapl;
+
+extern "C" {
+
+const char* mapl_status_string(int status) {
+  switch (status) {
+    case MAPL_OK: return "MAPL_OK";
+    case MAPL_ERR_INVALID_ARG: return "MAPL_ERR_INVALID_ARG";
+    case MAPL_ERR_UNSUPPORTED: return "MAPL_ERR_UNSUPPORTED";
+    case MAPL_ERR_ALIGNMENT: return "MAPL_ERR_ALIGNMENT";
+    case MAPL_ERR_WORKSPACE: return "MAPL_ERR_WORKSPACE";
+    case MAPL_ERR_CUDA: return "MAPL_ERR_CUDA";
+    default: return "MAPL_ERR_UNKNOWN";
+  }
+}
+
+const char* mapl_version(void) { return "mapl-b200 0.1 sm_100a"; }
+
+int mapl_last_cuda_error(void) { return g_last_cuda_error; }
+
+size_t mapl_workspace_bytes(const mapl_boundary_desc* desc) {
+  if (validate_desc(desc) != MAPL_OK) return 0;
+  return carve(*desc).total;
+}
+
+int mapl_encode(const mapl_boundary_desc* desc, const void* H, const float* U, const float* codebooks,
+                void* Zq_out, int32_t* codes_out, void* workspace, size_t workspace_bytes,
+                void* cuda_stream) {
+  MAPL_RETURN_IF(validate_desc(desc));
+  const mapl_boundary_desc& d = *desc;
+  const int L = d.rvq_levels;
+  if (!H || !U) return MAPL_ERR_INVALID_ARG;
+  if (L == 0 && !Zq_out) return MAPL_ERR_INVALID_ARG;
+  if (L > 0 && (!codes_out || !codebooks)) return MAPL_ERR_INVALID_ARG;
+  if (!all16({H, U, codebooks, Zq_out, codes_out, workspace})) return MAPL_ERR_ALIGNMENT;
+  const Ws w = carve(d);
+  if (!workspace || workspace_bytes < w.total) return MAPL_ERR_WORKSPACE;
+  if (d.n_tokens == 0) return MAPL_OK;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  char* ws = reinterpret_cast<char*>(workspace);
+
+  int s = tc_encode(d, H, U, codebooks, Zq_out, codes_out, ws + w.tc, st);
+  if (s != MAPL_ERR_UNSUPPORTED) return s;
+
+  const int bf = d.act_dtype == MAPL_BF16;
+  if (L == 0) {   // Z = H U
+    GemmArgs g;
+    g.M = (int)d.n_tokens; g.N = d.r; g.K[0] = d.d;
+    g.A[0].p = H; g.A[0].bf16 = bf; g.A[0].so = d.d; g.A[0].sk = 1;
+    g.B[0].p = U; g.B[0].so = 1; g.B[0].sk = d.r;
+    g.C = Zq_out; g.c_bf16 = bf; g.ldc = d.r;
+    return simt_gemm(g, st);
+  }
+  float* hn = reinterpret_cast<float*>(ws + w.half_norm);
+  MAPL_RETURN_IF(simt_half_sqnorm(codebooks, hn, L * d.rvq_k, d.r, st));
+  return simt_encode_rvq(d, H, U, codebooks, hn, Zq_out, codes_out, st);
+}
+
+int mapl_decode(const mapl_boundary_desc* desc, const void* Z, const int32_t* codes, const float* U,
+                const float* codebooks, const int32_t* tok, const float* A, const float* B,
+                void* Hhat_out, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  MAPL_RETURN_IF(validate_desc(desc));
+  const mapl_boundary_desc& d = *desc;
+  if (!U || !Hhat_out) return MAPL_ERR_INVALID_ARG;
+  if ((Z == nullptr) == (codes == nullptr)) return MAPL_ERR_INVALID_ARG;
+  if (codes && (d.rvq_levels == 0 || !codebooks)) return MAPL_ERR_INVALID_ARG;
+  const bool anchor = d.anchor_rank > 0;
+  if (anchor && (!tok || !A || !B)) return MAPL_ERR_INVALID_ARG;
+  if (!all16({Z, codes, U, codebooks, tok, A, B, Hhat_out, workspace})) return MAPL_ERR_ALIGNMENT;
+  const Ws w = carve(d);
+  if (!workspace || workspace_bytes < w.total) return MAPL_ERR_WORKSPACE;
+  if (d.n_tokens == 0) return MAPL_OK;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  char* ws = reinterpret_cast<char*>(workspace);
+
+  int s = tc_decode(d, Z, codes, U, codebooks, tok, A, B, Hhat_out, ws + w.tc, st);
+  if (s != MAPL_ERR_UNSUPPORTED) return s;
+
+  const int bf = d.act_dtype == MAPL_BF16;
+  GemmArgs g;
+  g.M = (int)d.n_tokens; g.N = d.d;
+  if (codes) {
+    float* zh = reinterpret_cast<float*>(ws + w.zhat);
+    MAPL_RETURN_IF(simt_dequant(d, codes, codebooks, zh, st));
+    g.A[0].p = zh; g.A[0].bf16 = 0;
+  } else {
+    g.A[0].p = Z; g.A[0].bf16 = bf;
+  }
+  g.A[0].so = d.r; g.A[0].sk = 1; g.K[0] = d.r;
+  g.B[0].p = U; g.B[0].so = d.r; g.B[0].sk = 1;           // B(k,n) = U[n,k]
+  if (anchor) {
+    g.npairs = 2; g.K[1] = d.anchor_rank;
+    g.A[1].p = A; g.A[1].so = d.anchor_rank; g.A[1].sk = 1; g.A[1].gather = tok; g.A[1].gmode = 1;
+    g.B[1].p = B; g.B[1].so = 1; g.B[1].sk = d.d;          // B(k,n) = B[k,n]
+  }
+  g.C = Hhat_out; g.c_bf16 = bf; g.ldc = d.d;
+  return simt_gemm(g, st);
+}
+
+int mapl_codec_backward(const mapl_boundary_desc* desc, const void* g_Hhat, const void* H, const void* Z,
+                        const int32_t* codes, const float* U, const float* codebooks, const int32_t* tok,
+                        const float* A, const float* B, void* gz_out, float* dU_out, float* dA_out,
+                        float* dB_out, void* dH_out, int accumulate, void* workspace,
+                        size_t workspace_bytes, void* cuda_stream) {
+  MAPL_RETURN_IF(validate_desc(desc));
+  const mapl_boundary_desc& d = *desc;
+  if (!g_Hhat || !U || !gz_out || !dU_out) return MAPL_ERR_INVALID_ARG;
+  if ((Z == nullptr) == (codes == nullptr)) return MAPL_ERR_INVALID_ARG;
+  if (codes && (d.rvq_levels == 0 || !codebooks)) return MAPL_ERR_INVALID_ARG;
+  if (!H && dH_out) return MAPL_ERR_INVALID_ARG;
+  bool anchor = d.anchor_rank > 0;
+  if (anchor && !tok && !A && !B) anchor = false;           // anchor ignored on request
+  if (anchor && (!tok || !A || !B || !dA_out)) return MAPL_ERR_INVALID_ARG;
+  if (!anchor && (dA_out || dB_out)) return MAPL_ERR_INVALID_ARG;
+  if (!all16({g_Hhat, H, Z, codes, U, codebooks, tok, A, B, gz_out, dU_out, dA_out, dB_out, dH_out, workspace}))
+    return MAPL_ERR_ALIGNMENT;
+  const Ws w = carve(d);
+  if (!workspace || workspace_bytes < w.total) return MAPL_ERR_WORKSPACE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  char* ws = reinterpret_cast<char*>(workspace);
+  const long long N = d.n_tokens;
+  const int ra = anchor ? d.anchor_rank : 0;
+
+  if (!accumulate) {
+    MAPL_CUDA_CHECK(cudaMemsetAsync(dU_out, 0, (size_t)d.d * d.r * 4, st));
+    if (anchor) MAPL_CUDA_CHECK(cudaMemsetAsync(dA_out, 0, (size_t)d.vocab * ra * 4, st));
+    if (anchor && dB_out) MAPL_CUDA_CHECK(cudaMemsetAsync(dB_out, 0, (size_t)ra * d.d * 4, st));
+  }
+  if (N == 0) return MAPL_OK;
+
+  int s = tc_backward(d, g_Hhat, H, Z, codes, U, codebooks, anchor ? tok : nullptr, A, B, gz_out, dU_out,
+                      dA_out, dB_out, dH_out, ws + w.tc, reinterpret_cast<float*>(ws + w.gA), st);
+  if (s != MAPL_ERR_UNSUPPORTED) return s;
+
+  const int bf = d.act_dtype == MAPL_BF16;
+  // zhat operand
+  MatRef zh;
+  if (codes) {
+    float* z = reinterpret_cast<float*>(ws + w.zhat);
+    MAPL_RETURN_IF(simt_dequant(d, codes, codebooks, z, st));
+    zh.p = z; zh.bf16 = 0;
+  } else {
+    zh.p = Z; zh.bf16 = bf;
+  }
+  {  // gz = g U
+    GemmArgs g;
+    g.M = (int)N; g.N = d.r; g.K[0] = d.d;
+    g.A[0].p = g_Hhat; g.A[0].bf16 = bf; g.A[0].so = d.d; g.A[0].sk = 1;
+    g.B[0].p = U; g.B[0].so = 1; g.B[0].sk = d.r;
+    g.C = gz_out; g.c_bf16 = bf; g.ldc = d.r;
+    MAPL_RETURN_IF(simt_gemm(g, st));
+  }
+  const int splits = (int)((N + 1023) / 1024);
+  {  // dU += g^T zhat (+ H^T gz)
+    GemmArgs g;
+    g.M = d.d; g.N = d.r; g.K[0] = (int)N;
+    g.A[0].p = g_Hhat; g.A[0].bf16 = bf; g.A[0].so = 1; g.A[0].sk = d.d;
+    g.B[0] = zh; g.B[0].so = 1; g.B[0].sk = d.r;
+    if (H) {
+      g.npairs = 2; g.K[1] = (int)N;
+      g.A[1].p = H; g.A[1].bf16 = bf; g.A[1].so = 1; g.A[1].sk = d.d;
+      g.B[1].p = gz_out; g.B[1].bf16 = bf; g.B[1].so = 1; g.B[1].sk = d.r;
+    }
+    g.C = dU_out; g.ldc = d.r; g.atomic = 1; g.splits = splits;
+    MAPL_RETURN_IF(simt_gemm(g, st));
+  }
+  if (dH_out) {  // dH = gz U^T
+    GemmArgs g;
+    g.M = (int)N; g.N = d.d; g.K[0] = d.r;
+    g.A[0].p = gz_out; g.A[0].bf16 = bf; g.A[0].so = d.r; g.A[0].sk = 1;
+    g.B[0].p = U; g.B[0].so = d.r; g.B[0].sk = 1;
+    g.C = dH_out; g.c_bf16 = bf; g.ldc = d.d;
+    MAPL_RETURN_IF(simt_gemm(g, st));
+  }
+  if (anchor) {
+    float* gA = reinterpret_cast<float*>(ws + w.gA);
+    {  // gA = g B^T
+      GemmArgs g;
+      g.M = (int)N; g.N = ra; g.K[0] = d.d;
+      g.A[0].p = g_Hhat; g.A[0].bf16 = bf; g.A[0].so = d.d; g.A[0].sk = 1;
+      g.B[0].p = B; g.B[0].so = d.d; g.B[0].sk = 1;
+      g.C = gA; g.ldc = ra;
+      MAPL_RETURN_IF(simt_gemm(g, st));
+    }
+    MAPL_RETURN_IF(simt_scatter_add_rows(gA, tok, dA_out, N, ra, st));
+    if (dB_out) {  // dB += A[tok]^T g
+      GemmArgs g;
+      g.M = ra; g.N = d.d; g.K[0] = (int)N;
+      g.A[0].p = A; g.A[0].so = 1; g.A[0].sk = ra; g.A[0].gather = tok; g.A[0].gmode = 2;
+      g.B[0].p = g_Hhat; g.B[0].bf16 = bf; g.B[0].so = 1; g.B[0].sk = d.d;
+      g.C = dB_out; g.ldc = d.d; g.atomic = 1; g.splits = splits;
+      MAPL_RETURN_IF(simt_gemm(g, st));
+    }
+  }
+  return MAPL_OK;
+}
+
+}  // extern "C"

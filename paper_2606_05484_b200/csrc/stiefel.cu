@@ -1,0 +1,299 @@
+// stiefel.cu -- mapl_stiefel_step: tangent projection (Eq. 4), step, and retraction
+// onto St(d,r) by thin QR (CholeskyQR2, diag(R) > 0) or by a fixed number of cubic Newton-Schulz
+// polar iterations (count passed in; 5 in every reported number).  fp32 storage and fp32 FFMA
+// arithmetic throughout: tcgen05 has no fp32 kind and a single TF32 pass cannot hold
+// ||U^T U - I||_F <= 1e-5.
+//
+//   Y = U - lr (G - U sym(U^T G)) = U (I + lr sym(S)) - lr G,   S = U^T G
+#include "common.cuh"
+
+namespace mapl {
+namespace {
+
+constexpr int NB = 32;
+
+__global__ void k_step_matrix(const float* __restrict__ S, float* __restrict__ M1, int r, float lr) {
+  // M1 = I + lr (S + S^T)/2, batched over blockIdx.y
+  const long long off = (long long)blockIdx.y * r * r;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= r * r) return;
+  const int a = idx / r, b = idx % r;
+  M1[off + idx] = (a == b ? 1.f : 0.f) + lr * 0.5f * (S[off + a * r + b] + S[off + b * r + a]);
+}
+
+__global__ void k_ns_poly(const float* __restrict__ Gm, float* __restrict__ M, int r) {
+  // M = (3I - Gm)/2
+  const long long off = (long long)blockIdx.y * r * r;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= r * r) return;
+  const int a = idx / r, b = idx % r;
+  M[off + idx] = 0.5f * ((a == b ? 3.f : 0.f) - Gm[off + idx]);
+}
+
+// out[b*2 + slot] = sqrt(sum_i (scale*(X[i] - Yv[i]))^2)   (Yv may be null: then X - I on an [r,r] matrix)
+__global__ void k_fro_norm(const float* __restrict__ X, const float* __restrict__ Yv, float scale, long long n,
+                           int r_if_identity, float* __restrict__ out, int slot) {
+  __shared__ float red[32];
+  const long long off = (long long)blockIdx.x * n;
+  float s = 0.f;
+  for (long long i = threadIdx.x; i < n; i += blockDim.x) {
+    float v;
+    if (Yv) v = scale * (X[off + i] - Yv[off + i]);
+    else {
+      const int a = (int)(i / r_if_identity), b = (int)(i % r_if_identity);
+      v = X[off + i] - (a == b ? 1.f : 0.f);
+    }
+    s = fmaf(v, v, s);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (threadIdx.x % 32 == 0) red[threadIdx.x / 32] = s;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    s = threadIdx.x < blockDim.x / 32 ? red[threadIdx.x] : 0.f;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (threadIdx.x == 0) out[blockIdx.x * 2 + slot] = sqrtf(s);
+  }
+}
+
+// In-place upper Cholesky G = R^T R of a symmetric positive definite [r,r] matrix (row-major; the
+// strict lower triangle is zeroed).  Right-looking, blocked by NB; one CTA per batch item.
+__global__ void __launch_bounds__(1024) k_chol_upper(float* __restrict__ Gb, int r) {
+  extern __shared__ __align__(16) float sm[];
+  float(*D)[NB + 1] = reinterpret_cast<float(*)[NB + 1]>(sm);
+  float* P = sm + NB * (NB + 1) + 3;                 // panel [NB][ldp]
+  P = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(P) + 15) & ~uintptr_t(15));
+  float* G = Gb + (long long)blockIdx.x * r * r;
+  const int tid = threadIdx.x, lane = tid % 32, warp = tid / 32;
+
+  for (int p = 0; p < r; p += NB) {
+    const int nb = min(NB, r - p);
+    for (int idx = tid; idx < nb * nb; idx += blockDim.x) {
+      const int a = idx / nb, b = idx % nb;
+      D[a][b] = G[(long long)(p + a) * r + p + b];
+    }
+    __syncthreads();
+    if (warp == 0) {
+      for (int j = 0; j < nb; ++j) {
+        const float dj = sqrtf(D[j][j]);
+        __syncwarp();
+        if (lane == j) D[j][j] = dj;
+        if (lane > j && lane < nb) D[j][lane] = D[j][lane] / dj;
+        __syncwarp();
+        if (lane > j && lane < nb) {
+          const float dji = D[j][lane];
+          for (int a = j + 1; a <= lane; ++a) D[a][lane] -= D[j][a] * dji;
+        }
+        __syncwarp();
+      }
+    }
+    __syncthreads();
+    for (int idx = tid; idx < nb * nb; idx += blockDim.x) {
+      const int a = idx / nb, b = idx % nb;
+      G[(long long)(p + a) * r + p + b] = (b >= a) ? D[a][b] : 0.f;
+    }
+    const int ncols = r - p - nb;
+    if (ncols <= 0) break;
+    const int ldp = (ncols + 3) & ~3;
+    // zero the block below the panel rows (strict lower part of R)
+    for (int idx = tid; idx < ncols * nb; idx += blockDim.x) {
+      const int i = idx / nb, b = idx % nb;
+      G[(long long)(p + nb + i) * r + p + b] = 0.f;
+    }
+    // panel: solve D^T x = G[p..p+nb, c]
+    for (int c = tid; c < ldp; c += blockDim.x) {
+      float x[NB];
+      if (c < ncols) {
+#pragma unroll
+        for (int j = 0; j < NB; ++j) {
+          float s = G[(long long)(p + j) * r + p + nb + c];
+#pragma unroll
+          for (int k = 0; k < j; ++k) s = fmaf(-D[k][j], x[k], s);
+          x[j] = s / D[j][j];
+        }
+#pragma unroll
+        for (int j = 0; j < NB; ++j) {
+          G[(long long)(p + j) * r + p + nb + c] = x[j];
+          P[j * ldp + c] = x[j];
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < NB; ++j) P[j * ldp + c] = 0.f;
+      }
+    }
+    __syncthreads();
+    // trailing update of the upper triangle
+    const int nblk = ldp / 4;
+    for (int blk = tid; blk < nblk * nblk; blk += blockDim.x) {
+      const int bi = blk / nblk, bj = blk % nblk;
+      if (bj < bi) continue;
+      float acc[4][4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
+#pragma unroll 8
+      for (int k = 0; k < NB; ++k) {
+        const float4 a = *reinterpret_cast<const float4*>(&P[k * ldp + bi * 4]);
+        const float4 b = *reinterpret_cast<const float4*>(&P[k * ldp + bj * 4]);
+        const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(av[i], bv[j], acc[i][j]);
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const int gi = bi * 4 + i;
+        if (gi >= ncols) continue;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int gj = bj * 4 + j;
+          if (gj < ncols && gj >= gi) G[(long long)(p + nb + gi) * r + p + nb + gj] -= acc[i][j];
+        }
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// Xinv = R^-1 for upper-triangular R (row-major [r,r]); thread c owns column c.
+__global__ void __launch_bounds__(1024) k_tri_inverse_upper(const float* __restrict__ Rb, float* __restrict__ Xb, int r) {
+  const float* R = Rb + (long long)blockIdx.x * r * r;
+  float* X = Xb + (long long)blockIdx.x * r * r;
+  for (int c = threadIdx.x; c < r; c += blockDim.x) {
+    for (int i = r - 1; i >= 0; --i) {
+      float x;
+      if (i > c) x = 0.f;
+      else if (i == c) x = 1.f / R[(long long)i * r + i];
+      else {
+        float s = 0.f;
+        for (int k = i + 1; k <= c; ++k) s = fmaf(R[(long long)i * r + k], X[(long long)k * r + c], s);
+        x = -s / R[(long long)i * r + i];
+      }
+      X[(long long)i * r + c] = x;
+    }
+  }
+}
+
+struct StWs {
+  size_t S, M, Rinv, X0, X1, total;
+};
+StWs st_carve(int d, int r, int batch) {
+  StWs w;
+  size_t off = 0;
+  auto seg = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+  w.S = seg((size_t)batch * r * r * 4);
+  w.M = seg((size_t)batch * r * r * 4);
+  w.Rinv = seg((size_t)batch * r * r * 4);
+  w.X0 = seg((size_t)batch * d * r * 4);
+  w.X1 = seg((size_t)batch * d * r * 4);
+  w.total = off + 256;
+  return w;
+}
+
+// Gm[b] = X[b]^T X2[b]  ([r,r], split-K over d with atomics)
+int gram(const float* X, const float* X2, float* Gm, int d, int r, int batch, cudaStream_t st) {
+  MAPL_CUDA_CHECK(cudaMemsetAsync(Gm, 0, (size_t)batch * r * r * 4, st));
+  GemmArgs g;
+  g.M = r; g.N = r; g.K[0] = d; g.batch = batch;
+  g.A[0].p = X; g.A[0].so = 1; g.A[0].sk = r; g.A[0].sb = (long long)d * r;
+  g.B[0].p = X2; g.B[0].so = 1; g.B[0].sk = r; g.B[0].sb = (long long)d * r;
+  g.C = Gm; g.ldc = r; g.sbc = (long long)r * r;
+  g.atomic = 1; g.splits = (d + 255) / 256;
+  return simt_gemm(g, st);
+}
+
+// C[b] = X[b] M[b] (+ beta E[b])
+int right_mul(const float* X, const float* M, float* C, const float* E, float beta, int d, int r, int batch,
+              cudaStream_t st) {
+  GemmArgs g;
+  g.M = d; g.N = r; g.K[0] = r; g.batch = batch;
+  g.A[0].p = X; g.A[0].so = r; g.A[0].sk = 1; g.A[0].sb = (long long)d * r;
+  g.B[0].p = M; g.B[0].so = 1; g.B[0].sk = r; g.B[0].sb = (long long)r * r;
+  g.C = C; g.ldc = r; g.sbc = (long long)d * r;
+  g.E = E; g.lde = r; g.sbe = (long long)d * r; g.beta = beta;
+  return simt_gemm(g, st);
+}
+
+}  // namespace
+}  // namespace mapl
+
+using namespace mapl;
+
+extern "C" {
+
+size_t mapl_stiefel_workspace_bytes(int32_t d, int32_t r, int32_t batch) {
+  if (d < 8 || r < 8 || r > d || d % 8 || r % 8 || batch < 1 || r > 1024) return 0;
+  return st_carve(d, r, batch).total;
+}
+
+int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float* G, float lr,
+                      int32_t retraction, int32_t ns_iters, float* info_out, void* workspace,
+                      size_t workspace_bytes, void* cuda_stream) {
+  if (d < 8 || r < 8 || r > d || d % 8 || r % 8 || batch < 1) return MAPL_ERR_INVALID_ARG;
+  if (r > 1024) return MAPL_ERR_UNSUPPORTED;
+  if (!U || !G) return MAPL_ERR_INVALID_ARG;
+  if (retraction != MAPL_RETRACT_QR && retraction != MAPL_RETRACT_NS) return MAPL_ERR_INVALID_ARG;
+  if (retraction == MAPL_RETRACT_NS && (ns_iters < 1 || ns_iters > 16)) return MAPL_ERR_INVALID_ARG;
+  if (!aligned16(U) || !aligned16(G) || !aligned16(workspace) || (info_out && !aligned16(info_out)))
+    return MAPL_ERR_ALIGNMENT;
+  const StWs w = st_carve(d, r, batch);
+  if (!workspace || workspace_bytes < w.total) return MAPL_ERR_WORKSPACE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  char* ws = reinterpret_cast<char*>(workspace);
+  float* S = reinterpret_cast<float*>(ws + w.S);
+  float* M = reinterpret_cast<float*>(ws + w.M);
+  float* Rinv = reinterpret_cast<float*>(ws + w.Rinv);
+  float* X0 = reinterpret_cast<float*>(ws + w.X0);
+  float* X1 = reinterpret_cast<float*>(ws + w.X1);
+  const dim3 egrid((r * r + 255) / 256, batch);
+
+  // tangent projection + step:  Y = U (I + lr sym(U^T G)) - lr G   -> X0
+  MAPL_RETURN_IF(gram(U, G, S, d, r, batch, st));
+  k_step_matrix<<<egrid, 256, 0, st>>>(S, M, r, lr);
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  MAPL_RETURN_IF(right_mul(U, M, X0, G, -lr, d, r, batch, st));
+  if (info_out) {   // ||xi||_F = ||U - Y||_F / lr
+    k_fro_norm<<<batch, 1024, 0, st>>>(U, X0, lr != 0.f ? 1.f / lr : 0.f, (long long)d * r, 0, info_out, 0);
+    MAPL_CUDA_CHECK(cudaGetLastError());
+  }
+
+  if (retraction == MAPL_RETRACT_NS) {
+    float* cur = X0;
+    float* nxt = X1;
+    for (int it = 0; it < ns_iters; ++it) {
+      MAPL_RETURN_IF(gram(cur, cur, S, d, r, batch, st));
+      k_ns_poly<<<egrid, 256, 0, st>>>(S, M, r);
+      MAPL_CUDA_CHECK(cudaGetLastError());
+      float* out = (it == ns_iters - 1) ? U : nxt;
+      MAPL_RETURN_IF(right_mul(cur, M, out, nullptr, 0.f, d, r, batch, st));
+      nxt = cur; cur = out;
+    }
+  } else {
+    // CholeskyQR2: Y = Q1 R1, Q1 = Q R2  =>  Y = Q (R2 R1), upper triangular with positive diagonal
+    const int ldp = (r + 3) & ~3;
+    const size_t smem = (size_t)(NB * (NB + 1) + 8 + NB * ldp) * 4;
+    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_chol_upper, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const float* src = X0;
+    for (int pass = 0; pass < 2; ++pass) {
+      MAPL_RETURN_IF(gram(src, src, S, d, r, batch, st));
+      k_chol_upper<<<batch, 1024, smem, st>>>(S, r);
+      MAPL_CUDA_CHECK(cudaGetLastError());
+      k_tri_inverse_upper<<<batch, r <= 1024 ? ((r + 31) / 32 * 32) : 1024, 0, st>>>(S, Rinv, r);
+      MAPL_CUDA_CHECK(cudaGetLastError());
+      float* out = pass == 0 ? X1 : U;
+      MAPL_RETURN_IF(right_mul(src, Rinv, out, nullptr, 0.f, d, r, batch, st));
+      src = out;
+    }
+  }
+  if (info_out) {   // ||U^T U - I||_F
+    MAPL_RETURN_IF(gram(U, U, S, d, r, batch, st));
+    k_fro_norm<<<batch, 1024, 0, st>>>(S, nullptr, 1.f, (long long)r * r, r, info_out, 1);
+    MAPL_CUDA_CHECK(cudaGetLastError());
+  }
+  return MAPL_OK;
+}
+
+}  // extern "C"

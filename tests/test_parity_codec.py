@@ -1,0 +1,122 @@
+"""GPU parity: the CUDA codec (through the C ABI) against the fp64 oracle, element by element on the
+same seeded inputs.  Tolerances are BASELINE.json's: codes bit-exact outside near ties (S5),
+relative Frobenius error <= 1e-5 (fp32) / 2e-2 (bf16)."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import mapl_oracle as o
+from paper_2606_05484_b200 import binding as mb
+from paper_2606_05484_b200 import inputs as I
+
+from _util import TOL, Dev, compare, desc_of, rel_fro, run_gpu, run_oracle, to_dev, to_np
+
+pytestmark = pytest.mark.gpu
+
+
+def _roundtrip(bi, **kw):
+    gpu = run_gpu(bi, **kw)
+    ora, stats = run_oracle(bi, gpu_codes=gpu["codes"], with_H=kw.get("with_H", True))
+    errs = compare(gpu, ora, stats, TOL[bi.cfg.act_dtype])
+    return gpu, ora, stats, errs
+
+
+def test_c0_full():
+    """configs[0]: tiny codec, fp32, N=4096, RVQ 2x256, anchors V=1024 ra=16."""
+    bi = I.make_boundary(I.CONFIGS["c0"], 0)
+    gpu, ora, stats, errs = _roundtrip(bi)
+    assert stats["excepted"] < 0.02 * 4096 * 2
+    print("c0", errs, stats)
+
+
+@pytest.mark.parametrize("name,n", [("c1", 1000), ("c1", 2048 + 77), ("c2", 1024 + 13), ("c3", 512 + 5)])
+def test_reduced_configs(name, n):
+    """configs[1..3] at reduced token counts: several tiles plus a ragged tail."""
+    bi = I.make_boundary(I.CONFIGS[name].with_tokens(n), 0)
+    gpu, ora, stats, errs = _roundtrip(bi)
+    print(name, n, errs, stats)
+
+
+@pytest.mark.parametrize("name,n", [("c1", 700), ("c2", 300), ("c0", 999)])
+def test_anchor_visible(name, n):
+    """A std 1.0 so the anchor term is well above the bf16 spacing of Hhat (S9)."""
+    bi = I.make_boundary(I.CONFIGS[name].with_tokens(n).with_anchor_std(1.0), 1)
+    _roundtrip(bi)
+
+
+@pytest.mark.parametrize("act", ["f32", "bf16"])
+def test_anchor_only(act):
+    """Z = 0 => Hhat rows are A[tok] B (S9 anchor-only case)."""
+    bi = I.make_generic(3, 333, 128, 32, 0, 0, 500, 24, act, a_std=1.0)
+    dev = Dev(bi)
+    desc = desc_of(bi)
+    dt = mb.act_torch_dtype(desc)
+    Z = torch.zeros((333, 32), dtype=dt, device="cuda")
+    Hhat = torch.empty((333, 128), dtype=dt, device="cuda")
+    ws = mb.alloc_workspace(mb.mapl_workspace_bytes(desc))
+    mb.mapl_decode(desc, Z, None, dev.U, None, dev.tok, dev.A, dev.B, Hhat, ws)
+    ref = o.decode(np.zeros((333, 32)), bi.U.f64, bi.tok, bi.A.f64, bi.B.f64)
+    assert rel_fro(to_np(Hhat), ref) <= TOL[act]
+
+
+@pytest.mark.parametrize("act", ["f32", "bf16"])
+@pytest.mark.parametrize("shape", [
+    # (N, d, r, L, K, V, ra)
+    (1, 64, 8, 0, 0, 10, 8),
+    (65, 72, 24, 2, 37, 50, 16),
+    (257, 200, 40, 3, 100, 300, 0),
+    (130, 256, 256, 0, 0, 64, 8),     # r == d
+    (70, 128, 16, 1, 1, 20, 8),       # K == 1: all codes 0
+    (513, 384, 96, 2, 257, 1000, 40),
+])
+def test_ragged_shapes(act, shape):
+    N, d, r, L, K, V, ra = shape
+    bi = I.make_generic(N % 97, N, d, r, L, K, V, ra, act)
+    gpu, ora, stats, errs = _roundtrip(bi)
+    if L and K == 1:
+        assert (gpu["codes"] == 0).all()
+
+
+def test_identity_at_full_rank_no_anchor():
+    """r = d, RVQ off, no anchor: Hhat = H up to rounding."""
+    bi = I.make_generic(5, 200, 64, 64, 0, 0, 1, 0, "f32")
+    gpu = run_gpu(bi)
+    assert rel_fro(gpu["Hhat"], bi.H.f64) <= 1e-5
+
+
+def test_empty_batch():
+    bi = I.make_generic(7, 0, 64, 16, 2, 8, 10, 8, "f32")
+    gpu = run_gpu(bi)
+    assert gpu["Hhat"].shape == (0, 64)
+    assert np.all(gpu["dU"] == 0.0) and np.all(gpu["dA"] == 0.0)
+
+
+@pytest.mark.parametrize("act", ["f32", "bf16"])
+def test_accumulate_and_decode_side_only(act):
+    bi = I.make_generic(11, 300, 128, 32, 2, 64, 100, 16, act)
+    base = run_gpu(bi)
+    acc = run_gpu(bi, accumulate=True)          # outputs pre-filled with 1.0
+    for k in ("dU", "dA", "dB"):
+        assert rel_fro(acc[k] - 1.0, base[k]) <= 5 * TOL[act], k
+    # H = NULL: decode-side term only (S8)
+    gpu = run_gpu(bi, with_H=False)
+    ora, stats = run_oracle(bi, gpu_codes=gpu["codes"], with_H=False)
+    compare(gpu, ora, stats, TOL[act])
+    assert gpu["dH"] is None
+
+
+def test_decode_from_z_equals_decode_from_codes():
+    bi = I.make_generic(13, 400, 256, 64, 3, 128, 200, 32, "bf16")
+    a = run_gpu(bi, use_codes_for_decode=True)
+    b = run_gpu(bi, use_codes_for_decode=False)   # uses the bf16-rounded zhat
+    assert np.array_equal(a["codes"], b["codes"])
+    assert rel_fro(b["Hhat"], a["Hhat"]) <= 2e-2
+
+
+def test_c1_full_size_one_boundary():
+    """configs[1] at full size (N=16384): every output against the oracle."""
+    bi = I.make_boundary(I.CONFIGS["c1"], 0)
+    gpu, ora, stats, errs = _roundtrip(bi, want_dB=False)
+    print("c1 full", errs)

@@ -1,0 +1,89 @@
+"""GPU parity of mapl_stiefel_step against the fp64 oracle: relative Frobenius error <= 1e-5 and
+||U^T U - I||_F <= 1e-5 (evaluated in fp64 on the host) after every GPU step."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import mapl_oracle as o
+from paper_2606_05484_b200 import binding as mb
+from paper_2606_05484_b200 import inputs as I
+
+from _util import rel_fro, to_dev, to_np
+
+pytestmark = pytest.mark.gpu
+
+RETR = {"qr": (mb.MAPL_RETRACT_QR, o.RETRACT_QR), "ns": (mb.MAPL_RETRACT_NS, o.RETRACT_NS)}
+
+
+def _gpu_step(U, G, lr, retr, iters=5, info=True):
+    batch, d, r = U.shape
+    ws = mb.alloc_workspace(mb.mapl_stiefel_workspace_bytes(d, r, batch))
+    inf = torch.zeros((batch, 2), dtype=torch.float32, device="cuda") if info else None
+    mb.mapl_stiefel_step(U, G, lr, retr, iters, inf, ws)
+    torch.cuda.synchronize()
+    return inf
+
+
+def _orth_res(U64):
+    return float(np.linalg.norm(U64.T @ U64 - np.eye(U64.shape[1])))
+
+
+@pytest.mark.parametrize("retr", ["qr", "ns"])
+@pytest.mark.parametrize("d,r,batch", [(64, 8, 1), (256, 32, 2), (200, 40, 3), (512, 104, 1), (2048, 64, 3)])
+def test_single_step_matches_oracle(retr, d, r, batch):
+    s = I.make_stiefel(r, d=d, batch=batch)
+    # Gaussian G has ||xi||_2 ~ sqrt(d)+sqrt(r); keep sigma_max(Y) < sqrt(3) for NS (S11)
+    lr = min(1e-2, 0.5 / (np.sqrt(d) + np.sqrt(r)))
+    U = to_dev(s.U); G = to_dev(s.G)
+    inf = _gpu_step(U, G, lr, RETR[retr][0])
+    Ug = to_np(U)
+    for b in range(batch):
+        Uo, xi = o.stiefel_step(s.U.f64[b], s.G.f64[b], lr, RETR[retr][1], 5)
+        assert rel_fro(Ug[b], Uo) <= 1e-5, (retr, d, r, b, rel_fro(Ug[b], Uo))
+        assert _orth_res(Ug[b]) <= 1e-5
+        info = to_np(inf)[b]
+        assert abs(info[0] - np.linalg.norm(xi)) <= 1e-3 * np.linalg.norm(xi)
+        assert info[1] <= 2e-5
+
+
+@pytest.mark.parametrize("retr", ["qr", "ns"])
+@pytest.mark.parametrize("r", I.STIEFEL_RS)
+def test_config4_shapes_one_step(retr, r):
+    """configs[4]: d=2048, r in {64,128,256,512}, 3 projectors, lr=1e-2, Gaussian G."""
+    s = I.make_stiefel(r)
+    U = to_dev(s.U); G = to_dev(s.G)
+    _gpu_step(U, G, I.STIEFEL_LR, RETR[retr][0], I.STIEFEL_NS_ITERS, info=False)
+    Ug = to_np(U)
+    b = r % 3     # one projector per r against the oracle (fp64 Householder QR of 2048x512 is slow)
+    Uo, _ = o.stiefel_step(s.U.f64[b], s.G.f64[b], I.STIEFEL_LR, RETR[retr][1], I.STIEFEL_NS_ITERS)
+    assert rel_fro(Ug[b], Uo) <= 1e-5, rel_fro(Ug[b], Uo)
+    for bb in range(3):
+        assert _orth_res(Ug[bb]) <= 1e-5, _orth_res(Ug[bb])
+
+
+@pytest.mark.parametrize("retr", ["qr", "ns"])
+def test_many_steps_fresh_gradient_residual_stays_bounded(retr):
+    """fresh seeded G per step (S13): residual <= 1e-5 after every one of 50 steps; one-step parity
+    against the oracle restarted from the GPU state at the end."""
+    r = 128
+    s = I.make_stiefel(r)
+    U = to_dev(s.U)
+    for step in range(50):
+        G = to_dev(I.make_stiefel(r, step=step + 1).G)
+        if step == 49:
+            U_before = to_np(U)
+            G_last = to_np(G)
+        _gpu_step(U, G, I.STIEFEL_LR, RETR[retr][0], 5, info=False)
+        if step % 7 == 0 or step == 49:
+            for b in range(3):
+                assert _orth_res(to_np(U)[b]) <= 1e-5, (step, b)
+    Uo, _ = o.stiefel_step(U_before[0], G_last[0], I.STIEFEL_LR, RETR[retr][1], 5)
+    assert rel_fro(to_np(U)[0], Uo) <= 1e-5
+
+
+def test_zero_gradient_is_fixed_point():
+    s = I.make_stiefel(32, d=128, batch=1)
+    for retr in ("qr", "ns"):
+        U = to_dev(s.U); G = torch.zeros_like(U)
+        _gpu_step(U, G, 0.1, RETR[retr][0])
+        assert rel_fro(to_np(U)[0], s.U.f64[0]) <= 1e-5
