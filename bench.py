@@ -1,0 +1,448 @@
+#!/usr/bin/env python
+"""bench.py -- codec tokens/s of the MAPL boundary codec on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mapl|reference] [--workload c1|c2|c3]
+
+One "step" = one pass of the whole hot path over one batch of synthetic input: for every stage
+boundary of the workload, mapl_encode -> mapl_decode (forward order), then mapl_codec_backward in
+reverse order (full backward: H given, dH and dA produced, dB off as in the paper), plus one
+mapl_stiefel_step per boundary when the workload says so (c3).  A codec token = one token crossing
+one boundary through all three calls; value = N * n_boundaries * n_gpus * K / time.
+
+Timing: W >= 3 warm-up steps, then exactly K steps between barrier + synchronize, CUDA events on
+the launching stream, max over ranks.  The K steps replay one CUDA graph of the step (the calls are
+launch-bound from Python otherwise).  Every boundary has its own buffers; the per-step working set
+(hundreds of MB) exceeds the 126 MB L2, so no flush is needed between iterations.
+
+Prints ONE JSON line (rank 0).  Multi-GPU: one process per GPU under torchrun, independent
+micro-batches per rank (weak scaling), no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import ctypes as C
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "codec tokens/s (enc+dec fwd+bwd, proj+RVQ+anchor)"
+UNIT = "tokens/s"
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        j = json.load(open(p))
+        return dict(hbm=float(j["hbm_gbs"]), bf16=float(j["bf16_tflops"]),
+                    bf16_sustained=float(j.get("bf16_tflops_sustained", j["bf16_tflops"])), src="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, src="fallback")
+
+
+# ---------------------------------------------------------------- workload description
+
+def workload(name: str):
+    from paper_2606_05484_b200 import inputs as I
+    cfg = I.CONFIGS[name]
+    desc = (f"{name}: N={cfg.n_tokens} d={cfg.d} r={cfg.r} L={cfg.rvq_levels} K={cfg.rvq_k} V={cfg.vocab} "
+            f"ra={cfg.anchor_rank} {cfg.act_dtype}, {cfg.n_boundaries} boundaries, enc+dec+bwd(dH,dA; dB off)"
+            + (" + stiefel step/boundary" if name == "c3" else ""))
+    return cfg, desc
+
+
+def alg_bytes_per_token(cfg):
+    """what the method itself must move per token per boundary."""
+    s = 2 if cfg.act_dtype == "bf16" else 4
+    d, r, L = cfg.d, cfg.r, cfg.rvq_levels
+    payload = r * s if L == 0 else 4 * L
+    enc = d * s + payload
+    dec = payload + 4 + d * s
+    bwd = 3 * d * s + 2 * r * s + 4            # g, H read; dH written; payload read; gz written; tok
+    return dict(encode=enc, decode=dec, backward=bwd)
+
+
+def alg_flops_per_token(cfg):
+    d, r, ra, L, K = cfg.d, cfg.r, cfg.anchor_rank, cfg.rvq_levels, cfg.rvq_k
+    return dict(encode=2 * d * r + L * 2 * K * r, decode=2 * (r + ra) * d, backward=8 * d * r + 2 * d * ra)
+
+
+# ---------------------------------------------------------------- clocks sampler
+
+class ClockSampler:
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._t = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        names = {getattr(nv, n): n[len("nvmlClocksEventReason"):] for n in dir(nv)
+                 if n.startswith("nvmlClocksEventReason") and isinstance(getattr(nv, n), int)} or \
+                {getattr(nv, n): n[len("nvmlClocksThrottleReason"):] for n in dir(nv)
+                 if n.startswith("nvmlClocksThrottleReason") and isinstance(getattr(nv, n), int)}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if bit and (mask & bit) and nm not in ("None", "All"):
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def start(self):
+        if self.nv:
+            self._t = threading.Thread(target=self._loop, daemon=True)
+            self._t.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._t:
+            self._t.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": []}
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons)}
+
+
+# ---------------------------------------------------------------- the CUDA arm
+
+class Boundary:
+    """device buffers of one stage boundary (own copies: nothing is shared between boundaries)"""
+
+    def __init__(self, cfg, b, rank, torch, mb, I, host=False):
+        bi = I.make_boundary(cfg, b + 16 * rank)
+        self.cfg = cfg
+        act = torch.bfloat16 if cfg.act_dtype == "bf16" else torch.float32
+
+        def dev(s):
+            if isinstance(s, np.ndarray):
+                return torch.from_numpy(s.copy()).cuda()
+            t = torch.from_numpy(s.data.copy())
+            return (t.view(torch.bfloat16) if s.dtype == "bf16" else t).cuda()
+
+        def pin(s):
+            if isinstance(s, np.ndarray):
+                return torch.from_numpy(s.copy()).pin_memory()
+            t = torch.from_numpy(s.data.copy())
+            return (t.view(torch.bfloat16) if s.dtype == "bf16" else t).pin_memory()
+
+        N, d, r, L = cfg.n_tokens, cfg.d, cfg.r, cfg.rvq_levels
+        self.desc = mb.make_desc(N, d, r, act, L, cfg.rvq_k if L else 0, cfg.vocab, cfg.anchor_rank)
+        self.H, self.g, self.tok = dev(bi.H), dev(bi.g), dev(bi.tok)
+        self.U, self.A, self.B = dev(bi.U), dev(bi.A), dev(bi.B)
+        self.C = dev(bi.C) if bi.C is not None else None
+        e = lambda *shape, dt=act: torch.empty(shape, dtype=dt, device="cuda")
+        self.Zq = e(N, r) if L == 0 else None
+        self.codes = e(N, L, dt=torch.int32) if L > 0 else None
+        self.Hhat, self.gz, self.dH = e(N, d), e(N, r), e(N, d)
+        self.dU = e(d, r, dt=torch.float32)
+        self.dA = e(cfg.vocab, cfg.anchor_rank, dt=torch.float32)
+        self.ws = mb.alloc_workspace(mb.mapl_workspace_bytes(self.desc))
+        if host:
+            self.hH, self.hg, self.htok = pin(bi.H), pin(bi.g), pin(bi.tok)
+            ph = lambda t: torch.empty(t.shape, dtype=t.dtype).pin_memory()
+            self.o_payload = ph(self.Zq if L == 0 else self.codes)
+            self.o_Hhat, self.o_gz, self.o_dH, self.o_dU = ph(self.Hhat), ph(self.gz), ph(self.dH), ph(self.dU)
+
+
+def make_step(bs, mb, stiefel=None):
+    def fwd(b):
+        mb.mapl_encode(b.desc, b.H, b.U, b.C, b.Zq, b.codes, b.ws)
+        mb.mapl_decode(b.desc, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.Hhat, b.ws)
+
+    def bwd(b):
+        mb.mapl_codec_backward(b.desc, b.g, b.H, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.gz, b.dU, b.dA,
+                               None, b.dH, False, b.ws)
+
+    def step():
+        for b in bs:
+            fwd(b)
+        for b in reversed(bs):
+            bwd(b)
+        if stiefel is not None:
+            stiefel()
+    return step
+
+
+def run_mapl(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_05484_b200 import binding as mb
+    from paper_2606_05484_b200 import inputs as I
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: there is no CPU path"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg, wdesc = workload(args.workload)
+    if args.tokens:
+        cfg = cfg.with_tokens(args.tokens)
+    nb = cfg.n_boundaries
+    bs = [Boundary(cfg, b, rank, torch, mb, I, host=True) for b in range(nb)]
+    lib = mb.raw_lib()
+
+    stiefel = None
+    if args.workload == "c3":       # configs[3]: "plus a Stiefel step per boundary" (G = dU / N, S12)
+        st_ws = mb.alloc_workspace(mb.mapl_stiefel_workspace_bytes(cfg.d, cfg.r, 1))
+        Gs = [torch.empty_like(b.dU) for b in bs]
+
+        def stiefel():
+            for b, G in zip(bs, Gs):
+                torch.mul(b.dU, 1.0 / cfg.n_tokens, out=G)
+                mb.mapl_stiefel_step(b.U, G, 1e-2, mb.MAPL_RETRACT_NS, 5, None, st_ws)
+    step = make_step(bs, mb, stiefel)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        for _ in range(max(3, args.warmup)):
+            step()
+        stream.synchronize()
+        # count our launches in one step
+        lib.mapl_profile_reset()
+        step()
+        stream.synchronize()
+        launches_per_step = 0
+        for kid in range(lib.mapl_profile_kernel_count()):
+            n = C.c_longlong(0)
+            lib.mapl_profile_read(kid, C.byref(n), None, None)
+            launches_per_step += n.value
+        # capture the step once, replay K times
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            step()
+        for _ in range(3):
+            graph.replay()
+        stream.synchronize()
+
+        sampler = ClockSampler(local)
+        barrier()
+        sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.steps):
+            graph.replay()
+        e1.record(stream)
+        stream.synchronize()
+        barrier()
+        clocks = sampler.stop()
+        ms = e0.elapsed_time(e1)
+
+        # ---- per-kernel timing pass (same K steps, eager launches, event pair around every kernel)
+        lib.mapl_profile_reset()
+        lib.mapl_profile_enable(1)
+        for _ in range(args.steps):
+            step()
+        stream.synchronize()
+        lib.mapl_profile_enable(0)
+        kern = {}
+        for kid in range(lib.mapl_profile_kernel_count()):
+            n, nt, tms = C.c_longlong(0), C.c_longlong(0), C.c_double(0)
+            lib.mapl_profile_read(kid, C.byref(n), C.byref(nt), C.byref(tms))
+            if nt.value:
+                kern[lib.mapl_profile_kernel_name(kid).decode()] = dict(launches=nt.value, ms=tms.value)
+
+        # ---- end to end: pinned host inputs -> device, the three calls, results -> pinned host
+        def e2e_step():
+            for b in bs:
+                b.H.copy_(b.hH, non_blocking=True)
+                b.tok.copy_(b.htok, non_blocking=True)
+                b.g.copy_(b.hg, non_blocking=True)
+            step()
+            for b in bs:
+                b.o_payload.copy_(b.Zq if b.Zq is not None else b.codes, non_blocking=True)
+                b.o_Hhat.copy_(b.Hhat, non_blocking=True)
+                b.o_gz.copy_(b.gz, non_blocking=True)
+                b.o_dH.copy_(b.dH, non_blocking=True)
+                b.o_dU.copy_(b.dU, non_blocking=True)
+        nbytes = lambda t: t.numel() * t.element_size()
+        h2d = sum(nbytes(b.hH) + nbytes(b.htok) + nbytes(b.hg) for b in bs)
+        d2h = sum(nbytes(b.o_payload) + nbytes(b.o_Hhat) + nbytes(b.o_gz) + nbytes(b.o_dH) + nbytes(b.o_dU) for b in bs)
+        e2e_steps = max(1, min(args.steps, 20))
+        for _ in range(2):
+            e2e_step()
+        barrier()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record(stream)
+        for _ in range(e2e_steps):
+            e2e_step()
+        f1.record(stream)
+        stream.synchronize()
+        barrier()
+        e2e_ms = f0.elapsed_time(f1)
+
+    if world > 1:
+        t = torch.tensor([ms, e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_ms = float(t[0]), float(t[1])
+    tokens_per_step = cfg.n_tokens * nb * world
+    value = tokens_per_step * args.steps / (ms * 1e-3)
+    e2e_value = tokens_per_step * e2e_steps / (e2e_ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (largest share of the timed per-kernel pass)
+    peaks = _peaks()
+    roof = None
+    if kern:
+        top = max(kern, key=lambda k: kern[k]["ms"])
+        total = sum(v["ms"] for v in kern.values())
+        roof = roofline_for(top, kern[top], cfg, peaks, total)
+        roof["kernels"] = {k: {"launches": v["launches"], "avg_us": round(1e3 * v["ms"] / v["launches"], 2),
+                               "share": round(v["ms"] / total, 3)} for k, v in sorted(kern.items(), key=lambda kv: -kv[1]["ms"])}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": cfg.act_dtype, "data": "synthetic",
+        "config": {"workload": wdesc, "l2": "distinct buffers per boundary; per-step working set > 126 MB L2, no flush",
+                   "launch": "one CUDA graph of the step, replayed K times", "parallelism": f"replicas x{world}"},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": e2e_steps, "note": "pinned host H,tok,g -> device; payload,Hhat,gz,dH,dU -> pinned host"},
+        "gpu_launches": launches_per_step * args.steps,
+        "roofline": roof,
+    }
+    if rank == 0:
+        if not args.no_cpu_baseline and world >= 1:
+            out["cpu_baseline"] = cpu_baseline(cfg, budget_s=args.cpu_budget)
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def roofline_for(name, k, cfg, peaks, total_ms):
+    """achieved = algorithmic bytes (or flops) of one launch / its measured average duration."""
+    N = cfg.n_tokens
+    ab, af = alg_bytes_per_token(cfg), alg_flops_per_token(cfg)
+    avg_s = 1e-3 * k["ms"] / k["launches"]
+    # which call the kernel belongs to and the share of that call's algorithmic work it carries
+    call = {"k_tc_encode": "encode", "k_tc_encode_rvq": "encode", "k_simt_encode_rvq": "encode",
+            "k_tc_decode": "decode", "k_tc_bwd_gz": "backward", "k_tc_bwd_du": "backward"}.get(name)
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(name)
+    if call is None:
+        return {"kernel": name, "bound": "hbm", "achieved": None, "peak": peaks["hbm"], "unit": "GB/s", "frac": None,
+                "traffic": traffic, "note": "generic kernel shared by several calls; see kernels"}
+    byt, flo = ab[call] * N, af[call] * N
+    if name == "k_tc_bwd_gz":     # reads g, tok, writes gz, dH  (H and payload are read by k_tc_bwd_du)
+        s = 2 if cfg.act_dtype == "bf16" else 4
+        byt = (2 * cfg.d * s + cfg.r * s + 4) * N
+        flo = (4 * cfg.d * cfg.r + 2 * cfg.d * cfg.anchor_rank) * N
+    if name == "k_tc_bwd_du":
+        s = 2 if cfg.act_dtype == "bf16" else 4
+        byt = (2 * cfg.d * s + 2 * cfg.r * s) * N
+        flo = 4 * cfg.d * cfg.r * N
+    t_hbm, t_tc = byt / (peaks["hbm"] * 1e9), flo / (peaks["bf16"] * 1e12)
+    if t_hbm >= t_tc:
+        ach = byt / avg_s / 1e9
+        return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": peaks["hbm"], "unit": "GB/s",
+                "frac": ach / peaks["hbm"], "traffic": traffic, "peak_source": peaks["src"] + " (burst copy)",
+                "avg_us": avg_s * 1e6, "alg_bytes_per_launch": byt}
+    ach = flo / avg_s / 1e12
+    return {"kernel": name, "bound": "tensor", "achieved": ach, "peak": peaks["bf16"], "unit": "TFLOP/s",
+            "frac": ach / peaks["bf16"], "traffic": traffic, "peak_source": peaks["src"] + " (burst bf16)",
+            "avg_us": avg_s * 1e6, "alg_flops_per_launch": flo}
+
+
+# ---------------------------------------------------------------- the oracle arm (CPU baseline)
+
+def cpu_baseline(cfg, budget_s=20.0, sample_tokens=None):
+    """The fp64 oracle, as it stands, on the host cores: one boundary, a contiguous token sample."""
+    from oracle import mapl_oracle as o
+    from paper_2606_05484_b200 import inputs as I
+    n = sample_tokens or min(cfg.n_tokens, 1024)
+    t_used, tokens = 0.0, 0
+    while True:
+        bi = I.make_boundary(cfg.with_tokens(n), 0)
+        H, U, g = bi.H.f64, bi.U.f64, bi.g.f64
+        t0 = time.perf_counter()
+        enc = o.encode(H, U, bi.C.f64 if bi.C is not None else None)
+        Hhat = o.decode(enc["Zhat"], U, bi.tok, bi.A.f64, bi.B.f64)
+        bw = o.backward(g, H, enc["Zhat"], U, bi.tok, bi.A.f64, bi.B.f64, want_dB=False)
+        dt = time.perf_counter() - t0
+        t_used, tokens = dt, n
+        del Hhat, bw
+        if sample_tokens or dt > budget_s / 4 or n >= cfg.n_tokens:
+            break
+        n = min(cfg.n_tokens, int(n * max(2.0, min(8.0, budget_s / 2 / max(dt, 1e-3)))))
+    return {"value": tokens / t_used, "unit": UNIT, "cores": o.threads(), "kind": "oracle",
+            "sample": f"{tokens} contiguous tokens of boundary 0 (enc+dec+bwd, fp64), {t_used:.1f} s"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores.  Each of the K steps is a
+    bounded contiguous-token sample of the workload, sized from one untimed probe so that the whole
+    run ends within a few minutes."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg, wdesc = workload(args.workload)
+    probe_n = 256
+    probe = cpu_baseline(cfg, sample_tokens=probe_n)
+    rate = probe["value"]
+    n = int(max(64, min(cfg.n_tokens, rate * 90.0 / max(1, args.steps + args.warmup))))
+    for _ in range(args.warmup):
+        cpu_baseline(cfg, sample_tokens=n)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        last = cpu_baseline(cfg, sample_tokens=n)
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    cb = {"value": value, "unit": UNIT, "cores": last["cores"], "kind": "oracle",
+          "sample": f"{n} contiguous tokens of boundary 0 per step (enc+dec+bwd, fp64), {args.steps} steps"}
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+        "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": wdesc}, "cpu_baseline": cb,
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="mapl", choices=["mapl", "reference"])
+    ap.add_argument("--workload", default="c1", choices=["c1", "c2", "c3", "c0"])
+    ap.add_argument("--tokens", type=int, default=0, help="override tokens per boundary (debug only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=20.0)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_mapl(args)
+
+
+if __name__ == "__main__":
+    main()

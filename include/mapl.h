@@ -137,6 +137,22 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U_inout, const
                       int32_t retraction, int32_t ns_iters, float* info_out, void* workspace,
                       size_t workspace_bytes, void* cuda_stream);
 
+/* LAUNCH ACCOUNTING (diagnostics; host-side state, not thread-safe).  Every kernel (and memset)
+ * the library enqueues is counted per kernel id.  With timing switched on each launch is also
+ * bracketed by a CUDA-event pair on its own stream; mapl_profile_read() synchronises on those
+ * events.  Do not switch timing on while a stream is being captured into a CUDA graph.
+ *   mapl_profile_kernel_count()      number of kernel ids
+ *   mapl_profile_kernel_name(kid)    static name of kernel id `kid` ("" if out of range)
+ *   mapl_profile_enable(on)          1: time launches from now on; 0: stop (counting never stops)
+ *   mapl_profile_reset()             zero all counters and timers
+ *   mapl_profile_read(kid, ...)      launches since reset, launches that were timed, their total ms
+ *                                    (any out pointer may be NULL)                                  */
+int mapl_profile_kernel_count(void);
+const char* mapl_profile_kernel_name(int kid);
+void mapl_profile_enable(int timing_on);
+void mapl_profile_reset(void);
+int mapl_profile_read(int kid, long long* launches, long long* timed_launches, double* total_ms);
+
 #ifdef __cplusplus
 }
 #endif

@@ -5,6 +5,7 @@
 #include <string.h>
 
 #include "common.cuh"
+#include "profile.cuh"
 #include "tc_codec.cuh"
 
 namespace mapl {
@@ -86,13 +87,13 @@ int mapl_encode(const mapl_boundary_desc* desc, const void* H, const float* U, c
   MAPL_RETURN_IF(validate_desc(desc));
   const mapl_boundary_desc& d = *desc;
   const int L = d.rvq_levels;
+  if (d.n_tokens == 0) return MAPL_OK;           // nothing to do; empty tensors may be NULL
   if (!H || !U) return MAPL_ERR_INVALID_ARG;
   if (L == 0 && !Zq_out) return MAPL_ERR_INVALID_ARG;
   if (L > 0 && (!codes_out || !codebooks)) return MAPL_ERR_INVALID_ARG;
   if (!all16({H, U, codebooks, Zq_out, codes_out, workspace})) return MAPL_ERR_ALIGNMENT;
   const Ws w = carve(d);
   if (!workspace || workspace_bytes < w.total) return MAPL_ERR_WORKSPACE;
-  if (d.n_tokens == 0) return MAPL_OK;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   char* ws = reinterpret_cast<char*>(workspace);
 
@@ -118,6 +119,7 @@ int mapl_decode(const mapl_boundary_desc* desc, const void* Z, const int32_t* co
                 void* Hhat_out, void* workspace, size_t workspace_bytes, void* cuda_stream) {
   MAPL_RETURN_IF(validate_desc(desc));
   const mapl_boundary_desc& d = *desc;
+  if (d.n_tokens == 0) return MAPL_OK;
   if (!U || !Hhat_out) return MAPL_ERR_INVALID_ARG;
   if ((Z == nullptr) == (codes == nullptr)) return MAPL_ERR_INVALID_ARG;
   if (codes && (d.rvq_levels == 0 || !codebooks)) return MAPL_ERR_INVALID_ARG;
@@ -126,7 +128,6 @@ int mapl_decode(const mapl_boundary_desc* desc, const void* Z, const int32_t* co
   if (!all16({Z, codes, U, codebooks, tok, A, B, Hhat_out, workspace})) return MAPL_ERR_ALIGNMENT;
   const Ws w = carve(d);
   if (!workspace || workspace_bytes < w.total) return MAPL_ERR_WORKSPACE;
-  if (d.n_tokens == 0) return MAPL_OK;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   char* ws = reinterpret_cast<char*>(workspace);
 
@@ -161,6 +162,15 @@ int mapl_codec_backward(const mapl_boundary_desc* desc, const void* g_Hhat, cons
                         size_t workspace_bytes, void* cuda_stream) {
   MAPL_RETURN_IF(validate_desc(desc));
   const mapl_boundary_desc& d = *desc;
+  if (d.n_tokens == 0) {                          // only the overwrite semantics remain
+    cudaStream_t st0 = reinterpret_cast<cudaStream_t>(cuda_stream);
+    if (!accumulate) {
+      if (dU_out) MAPL_CUDA_CHECK(cudaMemsetAsync(dU_out, 0, (size_t)d.d * d.r * 4, st0));
+      if (dA_out) MAPL_CUDA_CHECK(cudaMemsetAsync(dA_out, 0, (size_t)d.vocab * d.anchor_rank * 4, st0));
+      if (dB_out) MAPL_CUDA_CHECK(cudaMemsetAsync(dB_out, 0, (size_t)d.anchor_rank * d.d * 4, st0));
+    }
+    return MAPL_OK;
+  }
   if (!g_Hhat || !U || !gz_out || !dU_out) return MAPL_ERR_INVALID_ARG;
   if ((Z == nullptr) == (codes == nullptr)) return MAPL_ERR_INVALID_ARG;
   if (codes && (d.rvq_levels == 0 || !codebooks)) return MAPL_ERR_INVALID_ARG;
@@ -179,12 +189,10 @@ int mapl_codec_backward(const mapl_boundary_desc* desc, const void* g_Hhat, cons
   const int ra = anchor ? d.anchor_rank : 0;
 
   if (!accumulate) {
-    MAPL_CUDA_CHECK(cudaMemsetAsync(dU_out, 0, (size_t)d.d * d.r * 4, st));
-    if (anchor) MAPL_CUDA_CHECK(cudaMemsetAsync(dA_out, 0, (size_t)d.vocab * ra * 4, st));
-    if (anchor && dB_out) MAPL_CUDA_CHECK(cudaMemsetAsync(dB_out, 0, (size_t)ra * d.d * 4, st));
+    { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(dU_out, 0, (size_t)d.d * d.r * 4, st)); }
+    if (anchor) { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(dA_out, 0, (size_t)d.vocab * ra * 4, st)); }
+    if (anchor && dB_out) { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(dB_out, 0, (size_t)ra * d.d * 4, st)); }
   }
-  if (N == 0) return MAPL_OK;
-
   int s = tc_backward(d, g_Hhat, H, Z, codes, U, codebooks, anchor ? tok : nullptr, A, B, gz_out, dU_out,
                       dA_out, dB_out, dH_out, ws + w.tc, reinterpret_cast<float*>(ws + w.gA), st);
   if (s != MAPL_ERR_UNSUPPORTED) return s;

@@ -3,6 +3,7 @@
 #include <float.h>
 
 #include "common.cuh"
+#include "profile.cuh"
 
 namespace mapl {
 namespace {
@@ -200,6 +201,7 @@ __global__ void k_scatter_add_rows(const float* __restrict__ gA, const int32_t* 
 int simt_half_sqnorm(const float* C, float* out, int rows, int r, cudaStream_t stream) {
   if (rows <= 0) return MAPL_OK;
   const int wpb = 8;
+  KernelScope ks(KID_HALF_SQNORM, stream);
   k_half_sqnorm<<<(rows + wpb - 1) / wpb, wpb * 32, 0, stream>>>(C, out, rows, r);
   MAPL_CUDA_CHECK(cudaGetLastError());
   return MAPL_OK;
@@ -212,11 +214,16 @@ int simt_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* U, 
   const size_t smem = ((size_t)rpad * LD + 2 * BK * LD) * sizeof(float) + TOK * MAXL * sizeof(int);
   if (smem > 227 * 1024) return MAPL_ERR_UNSUPPORTED;
   const long long blocks = (d.n_tokens + TOK - 1) / TOK;
+  KernelScope ks(KID_SIMT_ENCODE_RVQ, stream);
+  static bool attr_done = false;   // once per process (not a stream operation; keeps graph capture clean)
+  if (!attr_done) {
+    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_simt_encode_rvq<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_simt_encode_rvq<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    attr_done = true;
+  }
   if (d.act_dtype == MAPL_BF16) {
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_simt_encode_rvq<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_simt_encode_rvq<true><<<(unsigned)blocks, NT, smem, stream>>>(H, U, C, half_norm, Zq_out, codes, d.n_tokens, d.d, d.r, d.rvq_levels, d.rvq_k);
   } else {
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_simt_encode_rvq<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_simt_encode_rvq<false><<<(unsigned)blocks, NT, smem, stream>>>(H, U, C, half_norm, Zq_out, codes, d.n_tokens, d.d, d.r, d.rvq_levels, d.rvq_k);
   }
   MAPL_CUDA_CHECK(cudaGetLastError());
@@ -227,6 +234,7 @@ int simt_dequant(const mapl_boundary_desc& d, const int32_t* codes, const float*
                  cudaStream_t stream) {
   const long long total = d.n_tokens * d.r;
   if (total <= 0) return MAPL_OK;
+  KernelScope ks(KID_DEQUANT, stream);
   k_dequant<<<(unsigned)((total + 255) / 256), 256, 0, stream>>>(codes, C, Zhat, d.n_tokens, d.r, d.rvq_levels, d.rvq_k);
   MAPL_CUDA_CHECK(cudaGetLastError());
   return MAPL_OK;
@@ -236,6 +244,7 @@ int simt_scatter_add_rows(const float* gA, const int32_t* tok, float* dA, long l
                           cudaStream_t stream) {
   const long long total = N * ra;
   if (total <= 0) return MAPL_OK;
+  KernelScope ks(KID_SCATTER_ROWS, stream);
   k_scatter_add_rows<<<(unsigned)((total + 255) / 256), 256, 0, stream>>>(gA, tok, dA, N, ra);
   MAPL_CUDA_CHECK(cudaGetLastError());
   return MAPL_OK;

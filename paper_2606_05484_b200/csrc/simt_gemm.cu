@@ -3,6 +3,7 @@
 // that meets the 1e-5 fp32 tolerance (tcgen05 has no fp32 MMA kind) and the fallback for shapes
 // the tensor-core kernels do not take.
 #include "common.cuh"
+#include "profile.cuh"
 
 namespace mapl {
 
@@ -139,7 +140,7 @@ int simt_gemm(const GemmArgs& a, cudaStream_t stream) {
   g.alpha = a.alpha; g.E = a.E; g.lde = a.lde; g.sbe = a.sbe; g.beta = a.beta;
   const int tiles = ((a.M + BM - 1) / BM) * ((a.N + BN - 1) / BN);
   dim3 grid(tiles, g.splits, a.batch);
-  k_simt_gemm<<<grid, NT, 0, stream>>>(g);
+  { KernelScope ks(KID_SIMT_GEMM, stream); k_simt_gemm<<<grid, NT, 0, stream>>>(g); }
   MAPL_CUDA_CHECK(cudaGetLastError());
   return MAPL_OK;
 }

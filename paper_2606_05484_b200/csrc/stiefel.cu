@@ -6,6 +6,7 @@
 //
 //   Y = U - lr (G - U sym(U^T G)) = U (I + lr sym(S)) - lr G,   S = U^T G
 #include "common.cuh"
+#include "profile.cuh"
 
 namespace mapl {
 namespace {
@@ -195,7 +196,7 @@ StWs st_carve(int d, int r, int batch) {
 
 // Gm[b] = X[b]^T X2[b]  ([r,r], split-K over d with atomics)
 int gram(const float* X, const float* X2, float* Gm, int d, int r, int batch, cudaStream_t st) {
-  MAPL_CUDA_CHECK(cudaMemsetAsync(Gm, 0, (size_t)batch * r * r * 4, st));
+  { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(Gm, 0, (size_t)batch * r * r * 4, st)); }
   GemmArgs g;
   g.M = r; g.N = r; g.K[0] = d; g.batch = batch;
   g.A[0].p = X; g.A[0].so = 1; g.A[0].sk = r; g.A[0].sb = (long long)d * r;
@@ -252,10 +253,11 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
 
   // tangent projection + step:  Y = U (I + lr sym(U^T G)) - lr G   -> X0
   MAPL_RETURN_IF(gram(U, G, S, d, r, batch, st));
-  k_step_matrix<<<egrid, 256, 0, st>>>(S, M, r, lr);
+  { KernelScope ks(KID_ST_STEP_MATRIX, st); k_step_matrix<<<egrid, 256, 0, st>>>(S, M, r, lr); }
   MAPL_CUDA_CHECK(cudaGetLastError());
   MAPL_RETURN_IF(right_mul(U, M, X0, G, -lr, d, r, batch, st));
   if (info_out) {   // ||xi||_F = ||U - Y||_F / lr
+    KernelScope ks(KID_ST_FRO_NORM, st);
     k_fro_norm<<<batch, 1024, 0, st>>>(U, X0, lr != 0.f ? 1.f / lr : 0.f, (long long)d * r, 0, info_out, 0);
     MAPL_CUDA_CHECK(cudaGetLastError());
   }
@@ -265,7 +267,7 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
     float* nxt = X1;
     for (int it = 0; it < ns_iters; ++it) {
       MAPL_RETURN_IF(gram(cur, cur, S, d, r, batch, st));
-      k_ns_poly<<<egrid, 256, 0, st>>>(S, M, r);
+      { KernelScope ks(KID_ST_NS_POLY, st); k_ns_poly<<<egrid, 256, 0, st>>>(S, M, r); }
       MAPL_CUDA_CHECK(cudaGetLastError());
       float* out = (it == ns_iters - 1) ? U : nxt;
       MAPL_RETURN_IF(right_mul(cur, M, out, nullptr, 0.f, d, r, batch, st));
@@ -275,13 +277,17 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
     // CholeskyQR2: Y = Q1 R1, Q1 = Q R2  =>  Y = Q (R2 R1), upper triangular with positive diagonal
     const int ldp = (r + 3) & ~3;
     const size_t smem = (size_t)(NB * (NB + 1) + 8 + NB * ldp) * 4;
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_chol_upper, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    static bool attr_done = false;
+    if (!attr_done) {
+      MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_chol_upper, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+      attr_done = true;
+    }
     const float* src = X0;
     for (int pass = 0; pass < 2; ++pass) {
       MAPL_RETURN_IF(gram(src, src, S, d, r, batch, st));
-      k_chol_upper<<<batch, 1024, smem, st>>>(S, r);
+      { KernelScope ks(KID_ST_CHOL, st); k_chol_upper<<<batch, 1024, smem, st>>>(S, r); }
       MAPL_CUDA_CHECK(cudaGetLastError());
-      k_tri_inverse_upper<<<batch, r <= 1024 ? ((r + 31) / 32 * 32) : 1024, 0, st>>>(S, Rinv, r);
+      { KernelScope ks(KID_ST_TRI_INV, st); k_tri_inverse_upper<<<batch, (r + 31) / 32 * 32, 0, st>>>(S, Rinv, r); }
       MAPL_CUDA_CHECK(cudaGetLastError());
       float* out = pass == 0 ? X1 : U;
       MAPL_RETURN_IF(right_mul(src, Rinv, out, nullptr, 0.f, d, r, batch, st));
@@ -290,6 +296,7 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
   }
   if (info_out) {   // ||U^T U - I||_F
     MAPL_RETURN_IF(gram(U, U, S, d, r, batch, st));
+    KernelScope ks(KID_ST_FRO_NORM, st);
     k_fro_norm<<<batch, 1024, 0, st>>>(S, nullptr, 1.f, (long long)r * r, r, info_out, 1);
     MAPL_CUDA_CHECK(cudaGetLastError());
   }
