@@ -50,6 +50,15 @@ def _load():
     lib.mapl_decode.argtypes = [dp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.mapl_codec_backward.argtypes = [dp] + [vp] * 14 + [C.c_int, vp, sz, vp]
     lib.mapl_stiefel_step.argtypes = [i32, i32, i32, vp, vp, f32, i32, i32, vp, vp, sz, vp]
+    lib.mapl_profile_kernel_count.restype = C.c_int
+    lib.mapl_profile_kernel_name.restype = C.c_char_p
+    lib.mapl_profile_kernel_name.argtypes = [C.c_int]
+    lib.mapl_profile_enable.restype = None
+    lib.mapl_profile_enable.argtypes = [C.c_int]
+    lib.mapl_profile_reset.restype = None
+    lib.mapl_profile_read.restype = C.c_int
+    lib.mapl_profile_read.argtypes = [C.c_int, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong),
+                                      C.POINTER(C.c_double)]
     for n in ("mapl_encode", "mapl_decode", "mapl_codec_backward", "mapl_stiefel_step"):
         getattr(lib, n).restype = C.c_int
     return lib

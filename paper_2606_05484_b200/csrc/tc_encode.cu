@@ -1,0 +1,138 @@
+// tc_encode.cu -- mapl_encode on the tensor cores (RVQ off): Z = H U  (Eq. 1, centred h).
+//
+// One CTA per 128-token tile.  Warp 0 streams H tiles [128 x 64] (HBM, evict-first) and U^T tiles
+// [r x 64] (L2-resident pack) through a TMA/mbarrier ring; one thread of warp 1 issues
+// tcgen05.mma (M=128, N=r, K=16) into a TMEM accumulator [128 lanes x r columns]; warps 2-5 read
+// their TMEM lane quarter back (one token row per thread), round to bf16 and store the payload.
+// Roofline: HBM (reads d*2 B/token, writes r*2 B/token).
+#include "profile.cuh"
+#include "tc_codec.cuh"
+#include "tc_common.cuh"
+
+namespace mapl {
+namespace {
+using namespace tc;
+
+constexpr int BM = 128, BK = 64, kThreads = 192;
+constexpr int kATile = BM * BK * 2;   // 16 KB
+
+__global__ void __launch_bounds__(kThreads, 1)
+k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmW,
+            __nv_bfloat16* __restrict__ Z, long long N, int d, int r, int stages) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const int b_tile = r * BK * 2;
+  const int stage_bytes = kATile + b_tile;
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)stages * stage_bytes);
+  uint64_t* empty = full + stages;
+  uint64_t* accum_full = empty + stages;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum_full + 1);
+
+  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  const long long m0 = (long long)blockIdx.x * BM;
+  const int nkb = d / BK;
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tmH);
+    tma_prefetch_desc(&tmW);
+    for (int s = 0; s < stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    mbar_init(accum_full, 1);
+    fence_barrier_init();
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"((uint32_t)r) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before_sync();
+  __syncthreads();
+  tc_fence_after_sync();
+  const uint32_t tmem_d = *tmem_slot;
+
+  if (warp == 0) {
+    if (elect_one()) {
+      for (int kb = 0; kb < nkb; ++kb) {
+        const int s = kb % stages;
+        mbar_wait(&empty[s], ((kb / stages) & 1) ^ 1);
+        mbar_arrive_expect_tx(&full[s], (uint32_t)stage_bytes);
+        uint8_t* a = smem + (size_t)s * stage_bytes;
+        tma_load_2d(a, &tmH, &full[s], kb * BK, (int)m0, kEvictFirst);
+        tma_load_2d(a + kATile, &tmW, &full[s], kb * BK, 0, kEvictLast);
+      }
+    }
+  } else if (warp == 1) {
+    if (elect_one()) {
+      const uint32_t idesc = make_idesc_bf16(BM, (uint32_t)r, false, false);
+      for (int kb = 0; kb < nkb; ++kb) {
+        const int s = kb % stages;
+        mbar_wait(&full[s], (kb / stages) & 1);
+        tc_fence_after_sync();
+        const uint32_t a = smem_u32(smem + (size_t)s * stage_bytes);
+        const uint32_t b = a + kATile;
+#pragma unroll
+        for (int k = 0; k < BK / 16; ++k)
+          umma_bf16(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc, (kb | k) != 0);
+        umma_commit(&empty[s]);
+      }
+      umma_commit(accum_full);
+    }
+  } else {
+    const int q = warp & 3;                         // TMEM lane quarter this warp may read
+    const long long m = m0 + q * 32 + lane;
+    mbar_wait(accum_full, 0);
+    tc_fence_after_sync();
+    for (int c = 0; c < r / 32; ++c) {
+      uint32_t v[32];
+      tmem_ld32(tmem_d + ((uint32_t)(q * 32) << 16) + c * 32, v);
+      tmem_ld_wait();
+      if (m < N) {
+        uint4* dst = reinterpret_cast<uint4*>(Z + m * r + c * 32);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          uint4 o;
+          o.x = pack_bf16x2(__uint_as_float(v[8 * i + 0]), __uint_as_float(v[8 * i + 1]));
+          o.y = pack_bf16x2(__uint_as_float(v[8 * i + 2]), __uint_as_float(v[8 * i + 3]));
+          o.z = pack_bf16x2(__uint_as_float(v[8 * i + 4]), __uint_as_float(v[8 * i + 5]));
+          o.w = pack_bf16x2(__uint_as_float(v[8 * i + 6]), __uint_as_float(v[8 * i + 7]));
+          dst[i] = o;
+        }
+      }
+    }
+  }
+  tc_fence_before_sync();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after_sync();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"((uint32_t)r) : "memory");
+  }
+}
+
+}  // namespace
+
+int tc_encode(const mapl_boundary_desc& d, const void* H, const float* U, const float* codebooks, void* Zq_out,
+              int32_t* codes_out, char* tc_ws, cudaStream_t st) {
+  (void)codebooks; (void)codes_out;
+  if (!tc_shape_ok(d) || d.rvq_levels != 0) return MAPL_ERR_UNSUPPORTED;
+  const TcPacks p = tc_packs(d, tc_ws);
+  MAPL_RETURN_IF(tc_pack_params(d, U, nullptr, p, 1, st));
+  CUtensorMap tmH, tmW;
+  if (!make_tmap_bf16_2d(&tmH, H, (uint64_t)d.n_tokens, (uint64_t)d.d, (uint64_t)d.d, BK, BM)) return MAPL_ERR_CUDA;
+  if (!make_tmap_bf16_2d(&tmW, p.WB, (uint64_t)d.r, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)d.r)) return MAPL_ERR_CUDA;
+  const int stage_bytes = kATile + d.r * BK * 2;
+  int stages = (200 * 1024) / stage_bytes;
+  if (stages > 8) stages = 8;
+  if (stages > d.d / BK) stages = d.d / BK;
+  const size_t smem = (size_t)stages * stage_bytes + 1024 + 256;
+  static bool attr_done = false;
+  if (!attr_done) {
+    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_encode, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    attr_done = true;
+  }
+  const unsigned tiles = (unsigned)((d.n_tokens + BM - 1) / BM);
+  KernelScope ks(KID_TC_ENCODE, st);
+  k_tc_encode<<<tiles, kThreads, smem, st>>>(tmH, tmW, reinterpret_cast<__nv_bfloat16*>(Zq_out), d.n_tokens, d.d,
+                                            d.r, stages);
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  return MAPL_OK;
+}
+
+}  // namespace mapl
