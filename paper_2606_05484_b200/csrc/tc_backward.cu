@@ -1,8 +1,379 @@
+// tc_backward.cu -- mapl_codec_backward on the tensor cores (STE = S7).
+//
+// k_tc_bwd_gz   one CTA per token tile, two phases over one read of g:
+//     phase 1   [gz | gA] = g . [U | B^T]         K = d, streamed through a TMA ring
+//               epilogue: gz -> bf16 -> gz_out (the backward wire payload) and -> smem as the A
+//               operand of phase 2; gA rows -> red.global.add.v4.f32 into dA[tok] (scatter-add)
+//     phase 2   dH = gz . U^T                     the chunk pipeline of tc_tile_ops.cuh
+// k_tc_bwd_du   dU[d-tile, :] += sum over a token range of  g^T Zhat + H^T gz.  Both operands are
+//               MN-major (tokens are the contraction index): TMA boxes [64 tokens x 64 cols]
+//               are used as they land.  Split over token ranges; fp32 vector atomics into dU.
+// Roofline: HBM at configs 1-2 (g, H read; dH written), tensor at config 3.
+#include "profile.cuh"
 #include "tc_codec.cuh"
+#include "tc_tile_ops.cuh"
+
 namespace mapl {
-int tc_backward(const mapl_boundary_desc&, const void*, const void*, const void*, const int32_t*, const float*,
-                const float*, const int32_t*, const float*, const float*, void*, float*, float*, float*, void*,
-                char*, float*, cudaStream_t) {
-  return MAPL_ERR_UNSUPPORTED;
+namespace {
+using namespace tc;
+
+constexpr int kThreads = 192;
+
+__device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
+  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
+
+// ---------------------------------------------------------------- gz / dA / dH
+struct BwdGzParams {
+  const int32_t* tok; float* dA; __nv_bfloat16* gz_out;
+  long long N;
+  int d, r, ra, tile_m;
+  int stages1, stage1_bytes, b_stages, do_dh;
+};
+
+__global__ void __launch_bounds__(kThreads, 1)
+k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmWu,
+            const __grid_constant__ CUtensorMap tmWb, const __grid_constant__ CUtensorMap tmWd,
+            const __grid_constant__ CUtensorMap tmO, const BwdGzParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const int kc = p.r + p.ra, nkb1 = p.d / 64;
+  // region R: phase 1 ring  |aliased with|  phase 2 gz operand + W ring
+  const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes;
+  const size_t ring2 = (size_t)(p.r / 64 + p.b_stages) * kTileBytes;
+  const size_t regionR = ring1 > ring2 ? ring1 : ring2;
+  ChunkPipe c;
+  c.nkb = p.r / 64; c.nchunks = p.d / kChunkN; c.b_stages = p.b_stages;
+  c.sA = smem;
+  c.sB = smem + (size_t)(p.r / 64) * kTileBytes;
+  c.sOut = smem + regionR;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(c.sOut + (size_t)kOutBufs * kTileBytes);
+  c.b_full = bars; c.b_empty = c.b_full + p.b_stages;
+  c.acc_full = c.b_empty + p.b_stages; c.acc_empty = c.acc_full + kAccStages;
+  uint64_t* s1_full = c.acc_empty + kAccStages;
+  uint64_t* s1_empty = s1_full + p.stages1;
+  uint64_t* acc1_full = s1_empty + p.stages1;
+  uint64_t* gz_full = acc1_full + 1;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(gz_full + 1);
+
+  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  const long long m0 = (long long)blockIdx.x * p.tile_m;
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tmG); tma_prefetch_desc(&tmWu); tma_prefetch_desc(&tmWb);
+    tma_prefetch_desc(&tmWd); tma_prefetch_desc(&tmO);
+    chunk_init_barriers(c);
+    for (int s = 0; s < p.stages1; ++s) { mbar_init(&s1_full[s], 1); mbar_init(&s1_empty[s], 1); }
+    mbar_init(acc1_full, 1);
+    mbar_init(gz_full, 4);
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc<512>(tmem_slot);
+  tc_fence_before_sync();
+  __syncthreads();
+  tc_fence_after_sync();
+  c.tmem_base = *tmem_slot;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+
+  if (warp == 0) {
+    if (elect_one()) {
+      const uint32_t bytes = (uint32_t)(p.tile_m * 128 + kc * 128);
+      for (int kb = 0; kb < nkb1; ++kb) {
+        const int s = kb % p.stages1;
+        mbar_wait(&s1_empty[s], ((kb / p.stages1) & 1) ^ 1);
+        mbar_arrive_expect_tx(&s1_full[s], bytes);
+        uint8_t* a = smem + (size_t)s * p.stage1_bytes;
+        tma_load_2d(a, &tmG, &s1_full[s], kb * 64, (int)m0, kEvictLast);   // g is read again by k_tc_bwd_du
+        tma_load_2d(a + kTileBytes, &tmWu, &s1_full[s], kb * 64, 0, kEvictLast);
+        if (p.ra) tma_load_2d(a + kTileBytes + p.r * 128, &tmWb, &s1_full[s], kb * 64, p.r, kEvictLast);
+      }
+      if (p.do_dh) {
+        mbar_wait(acc1_full, 0);        // phase 1 MMAs have consumed the ring: region R may be reused
+        chunk_produce(c, &tmWd);
+      }
+    }
+  } else if (warp == 1) {
+    if (elect_one()) {
+      const uint32_t idesc_u = make_idesc_bf16(128, (uint32_t)p.r, false, false);
+      const uint32_t idesc_b = make_idesc_bf16(128, (uint32_t)(p.ra ? p.ra : 64), false, false);
+      for (int kb = 0; kb < nkb1; ++kb) {
+        const int s = kb % p.stages1;
+        mbar_wait(&s1_full[s], (kb / p.stages1) & 1);
+        tc_fence_after_sync();
+        const uint32_t a = smem_u32(smem + (size_t)s * p.stage1_bytes);
+        const uint32_t bu = a + kTileBytes, bb = bu + p.r * 128;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const uint64_t da = desc_kmajor_sw128(a + k * 32);
+          umma_bf16(c.tmem_base, da, desc_kmajor_sw128(bu + k * 32), idesc_u, (kb | k) != 0);
+          if (p.ra) umma_bf16(c.tmem_base + p.r, da, desc_kmajor_sw128(bb + k * 32), idesc_b, (kb | k) != 0);
+        }
+        umma_commit(&s1_empty[s]);
+      }
+      umma_commit(acc1_full);
+      if (p.do_dh) {
+        mbar_wait(gz_full, 0);          // gz operand written and the phase 1 accumulator drained
+        tc_fence_after_sync();
+        chunk_mma(c);
+      }
+    }
+  } else {
+    const int q = warp & 3, row = q * 32 + lane;
+    const long long m = m0 + row;
+    const bool live = row < p.tile_m && m < p.N;
+    const uint32_t tmem_row = c.tmem_base + ((uint32_t)(q * 32) << 16);
+    mbar_wait(acc1_full, 0);
+    tc_fence_after_sync();
+    for (int cc = 0; cc < p.r / 32; ++cc) {
+      uint32_t v[32];
+      tmem_ld32(tmem_row + cc * 32, v);
+      tmem_ld_wait();
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        uint4 o;
+        o.x = pack_bf16x2(__uint_as_float(v[8 * i + 0]), __uint_as_float(v[8 * i + 1]));
+        o.y = pack_bf16x2(__uint_as_float(v[8 * i + 2]), __uint_as_float(v[8 * i + 3]));
+        o.z = pack_bf16x2(__uint_as_float(v[8 * i + 4]), __uint_as_float(v[8 * i + 5]));
+        o.w = pack_bf16x2(__uint_as_float(v[8 * i + 6]), __uint_as_float(v[8 * i + 7]));
+        if (live) *reinterpret_cast<uint4*>(p.gz_out + m * p.r + cc * 32 + i * 8) = o;
+        if (p.do_dh) *reinterpret_cast<uint4*>(c.sA + (size_t)(cc / 2) * kTileBytes + sw128_offset(row, (cc & 1) * 4 + i)) = o;
+      }
+    }
+    if (p.ra) {
+      float* dst = p.dA + (live ? (long long)p.tok[m] : 0) * p.ra;
+      for (int cc = 0; cc < p.ra / 32; ++cc) {
+        uint32_t v[32];
+        tmem_ld32(tmem_row + p.r + cc * 32, v);
+        tmem_ld_wait();
+        if (live) {
+#pragma unroll
+          for (int i = 0; i < 8; ++i)
+            red_add_v4(dst + cc * 32 + i * 4, __uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
+                       __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+        }
+      }
+    }
+    if (p.do_dh) {
+      tc_fence_before_sync();
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(gz_full);
+      chunk_epilogue(c, &tmO, (int)m0);
+    }
+  }
+  tc_fence_before_sync();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after_sync();
+    tmem_dealloc<512>(c.tmem_base);
+  }
+}
+
+// ---------------------------------------------------------------- dU
+struct BwdDuParams {
+  float* dU;
+  long long N;
+  int d, r, n_src, stages, item_bytes, blocks_per_split, n_blocks;
+};
+
+__global__ void __launch_bounds__(kThreads, 1)
+k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmZ,
+            const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmGz, const BwdDuParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)p.stages * p.item_bytes);
+  uint64_t* empty = full + p.stages;
+  uint64_t* acc_full = empty + p.stages;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_full + 1);
+
+  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  const int dt = blockIdx.x;                                   // 128 rows of dU
+  const int tb0 = blockIdx.y * p.blocks_per_split;
+  const int tb1 = min(p.n_blocks, tb0 + p.blocks_per_split);
+  const int n_items = (tb1 > tb0 ? tb1 - tb0 : 0) * p.n_src;
+  constexpr int kBox = 64 * 128;                               // [64 tokens x 64 cols] bf16 = 8 KB
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tmG); tma_prefetch_desc(&tmZ); tma_prefetch_desc(&tmH); tma_prefetch_desc(&tmGz);
+    for (int s = 0; s < p.stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    mbar_init(acc_full, 1);
+    fence_barrier_init();
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"((uint32_t)p.r) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before_sync();
+  __syncthreads();
+  tc_fence_after_sync();
+  const uint32_t tmem_d = *tmem_slot;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+
+  if (n_items > 0) {
+    if (warp == 0) {
+      if (elect_one()) {
+        for (int it = 0; it < n_items; ++it) {
+          const int s = it % p.stages, tb = tb0 + it / p.n_src, src = it % p.n_src;
+          mbar_wait(&empty[s], ((it / p.stages) & 1) ^ 1);
+          mbar_arrive_expect_tx(&full[s], (uint32_t)p.item_bytes);
+          uint8_t* a = smem + (size_t)s * p.item_bytes;
+          const CUtensorMap* ma = src ? &tmH : &tmG;
+          const CUtensorMap* mb = src ? &tmGz : &tmZ;
+          tma_load_2d(a, ma, &full[s], dt * 128, tb * 64, kEvictFirst);
+          tma_load_2d(a + kBox, ma, &full[s], dt * 128 + 64, tb * 64, kEvictFirst);
+          for (int j = 0; j < p.r / 64; ++j) tma_load_2d(a + 2 * kBox + j * kBox, mb, &full[s], j * 64, tb * 64, kEvictLast);
+        }
+      }
+    } else if (warp == 1) {
+      if (elect_one()) {
+        const uint32_t idesc = make_idesc_bf16(128, (uint32_t)p.r, true, true);
+        for (int it = 0; it < n_items; ++it) {
+          const int s = it % p.stages;
+          mbar_wait(&full[s], (it / p.stages) & 1);
+          tc_fence_after_sync();
+          const uint32_t a = smem_u32(smem + (size_t)s * p.item_bytes), b = a + 2 * kBox;
+#pragma unroll
+          for (int k = 0; k < 4; ++k)       // 16 tokens (= 2 swizzle atoms of 8 rows) per UMMA
+            umma_bf16(tmem_d, desc_mnmajor_sw128(a + k * 2048, kBox), desc_mnmajor_sw128(b + k * 2048, kBox), idesc,
+                      (it | k) != 0);
+          umma_commit(&empty[s]);
+        }
+        umma_commit(acc_full);
+      }
+    } else {
+      const int q = warp & 3, row = q * 32 + lane;
+      float* dst = p.dU + ((long long)dt * 128 + row) * p.r;
+      mbar_wait(acc_full, 0);
+      tc_fence_after_sync();
+      for (int cc = 0; cc < p.r / 32; ++cc) {
+        uint32_t v[32];
+        tmem_ld32(tmem_d + ((uint32_t)(q * 32) << 16) + cc * 32, v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+          red_add_v4(dst + cc * 32 + i * 4, __uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
+                     __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+      }
+    }
+  }
+  tc_fence_before_sync();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after_sync();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"((uint32_t)p.r) : "memory");
+  }
+}
+
+// zhat (bf16) from RVQ codes, for the dU operand
+__global__ void k_tc_dequant_bf16(const int32_t* __restrict__ codes, const float* __restrict__ C,
+                                  __nv_bfloat16* __restrict__ Zb, long long N, int r, int L, int K) {
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;   // one 8-column chunk each
+  const int cpr = r / 8;
+  if (idx >= N * cpr) return;
+  const long long n = idx / cpr;
+  const int c = (int)(idx % cpr);
+  float s[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  for (int l = 0; l < L; ++l) {
+    const float4* src = reinterpret_cast<const float4*>(C + ((long long)l * K + codes[n * L + l]) * r + c * 8);
+    const float4 x = __ldg(src), y = __ldg(src + 1);
+    s[0] += x.x; s[1] += x.y; s[2] += x.z; s[3] += x.w; s[4] += y.x; s[5] += y.y; s[6] += y.z; s[7] += y.w;
+  }
+  *reinterpret_cast<uint4*>(Zb + n * r + c * 8) =
+      make_uint4(pack_bf16x2(s[0], s[1]), pack_bf16x2(s[2], s[3]), pack_bf16x2(s[4], s[5]), pack_bf16x2(s[6], s[7]));
+}
+
+}  // namespace
+
+int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const void* Z, const int32_t* codes,
+                const float* U, const float* codebooks, const int32_t* tok, const float* A, const float* B,
+                void* gz_out, float* dU_out, float* dA_out, float* dB_out, void* dH_out, char* tc_ws, float* gA_ws,
+                cudaStream_t st) {
+  (void)gA_ws;
+  if (!tc_shape_ok(d)) return MAPL_ERR_UNSUPPORTED;
+  const int ra = tok ? d.anchor_rank : 0, kc = d.r + ra;
+  const TcPacks pk = tc_packs(d, tc_ws);
+  MAPL_RETURN_IF(tc_pack_params(d, U, B, pk, 1 | (ra ? 2 : 0) | (dH_out ? 4 : 0), st));
+
+  static bool attr_done = false;
+  if (!attr_done) {
+    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_bwd_gz, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_bwd_du, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    attr_done = true;
+  }
+  const uint64_t N = (uint64_t)d.n_tokens, dd = (uint64_t)d.d, rr = (uint64_t)d.r;
+
+  // zhat operand for dU
+  const void* zhat = Z;
+  if (codes) {
+    __nv_bfloat16* zb = reinterpret_cast<__nv_bfloat16*>(tc_ws + 2 * align_up((size_t)(d.r + d.anchor_rank) * d.d * 2, 256));
+    const long long total = d.n_tokens * (d.r / 8);
+    KernelScope ks(KID_DEQUANT, st);
+    k_tc_dequant_bf16<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(codes, codebooks, zb, d.n_tokens, d.r,
+                                                                      d.rvq_levels, d.rvq_k);
+    MAPL_CUDA_CHECK(cudaGetLastError());
+    zhat = zb;
+  }
+
+  {  // ---- gz, dA, dH
+    BwdGzParams p;
+    p.tok = tok; p.dA = dA_out; p.gz_out = reinterpret_cast<__nv_bfloat16*>(gz_out);
+    p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.ra = ra; p.tile_m = tc_tile_m(d.n_tokens);
+    p.do_dh = dH_out ? 1 : 0;
+    p.stage1_bytes = kTileBytes + kc * 128;
+    const size_t budget = 227 * 1024 - (size_t)kOutBufs * kTileBytes - 1024 - 1024;   // region R
+    p.stages1 = (int)(budget / p.stage1_bytes);
+    if (p.stages1 > 8) p.stages1 = 8;
+    if (p.stages1 > d.d / 64) p.stages1 = d.d / 64;
+    if (p.stages1 < 2) return MAPL_ERR_UNSUPPORTED;
+    p.b_stages = (int)(budget / kTileBytes) - d.r / 64;
+    if (p.b_stages > 8) p.b_stages = 8;
+    if (p.b_stages < 2) return MAPL_ERR_UNSUPPORTED;
+    const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes, ring2 = (size_t)(d.r / 64 + p.b_stages) * kTileBytes;
+    const size_t smem = (ring1 > ring2 ? ring1 : ring2) + (size_t)kOutBufs * kTileBytes + 1024 + 1024;
+    CUtensorMap tmG, tmWu, tmWb, tmWd, tmO;
+    if (!make_tmap_bf16_2d(&tmG, g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmWu, pk.WB, (uint64_t)(d.r + d.anchor_rank), dd, dd, 64, (uint32_t)d.r)) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmWb, pk.WB, (uint64_t)(d.r + d.anchor_rank), dd, dd, 64, (uint32_t)(ra ? ra : 64))) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmWd, pk.Wd, dd, (uint64_t)pk.kc, (uint64_t)pk.kc, 64, kChunkN)) return MAPL_ERR_CUDA;
+    // dH map: when dH is skipped the map is unused but must be valid
+    if (!make_tmap_bf16_2d(&tmO, dH_out ? dH_out : g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
+    const unsigned tiles = (unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m);
+    KernelScope ks(KID_TC_BWD_GZ, st);
+    MAPL_CUDA_CHECK(launch_pdl(k_tc_bwd_gz, dim3(tiles), dim3(kThreads), smem, st, tmG, tmWu, tmWb, tmWd, tmO, p));
+  }
+  {  // ---- dU
+    BwdDuParams p;
+    p.dU = dU_out; p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.n_src = H ? 2 : 1;
+    p.item_bytes = 2 * 64 * 128 + (d.r / 64) * 64 * 128;
+    p.stages = (int)((227 * 1024 - 2048) / p.item_bytes);
+    if (p.stages > 8) p.stages = 8;
+    p.n_blocks = (int)((d.n_tokens + 63) / 64);
+    const int n_dt = d.d / 128;
+    int S = 148 / n_dt;
+    if (S < 1) S = 1;
+    if (S > p.n_blocks) S = p.n_blocks;
+    p.blocks_per_split = (p.n_blocks + S - 1) / S;
+    S = (p.n_blocks + p.blocks_per_split - 1) / p.blocks_per_split;
+    const size_t smem = (size_t)p.stages * p.item_bytes + 1024 + 512;
+    CUtensorMap tmG, tmZ, tmH, tmGz;
+    if (!make_tmap_bf16_2d(&tmG, g, N, dd, dd, 64, 64)) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmZ, zhat, N, rr, rr, 64, 64)) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmH, H ? H : g, N, dd, dd, 64, 64)) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmGz, gz_out, N, rr, rr, 64, 64)) return MAPL_ERR_CUDA;
+    KernelScope ks(KID_TC_BWD_DU, st);
+    MAPL_CUDA_CHECK(launch_pdl(k_tc_bwd_du, dim3(n_dt, S), dim3(kThreads), smem, st, tmG, tmZ, tmH, tmGz, p));
+  }
+  if (dB_out && ra) {   // dB += A[tok]^T g  (P_p is frozen in the paper: optional, fp32 SIMT)
+    GemmArgs ga;
+    ga.M = ra; ga.N = d.d; ga.K[0] = (int)d.n_tokens;
+    ga.A[0].p = A; ga.A[0].so = 1; ga.A[0].sk = ra; ga.A[0].gather = tok; ga.A[0].gmode = 2;
+    ga.B[0].p = g; ga.B[0].bf16 = 1; ga.B[0].so = 1; ga.B[0].sk = d.d;
+    ga.C = dB_out; ga.ldc = d.d; ga.atomic = 1; ga.splits = (int)((d.n_tokens + 1023) / 1024);
+    MAPL_RETURN_IF(simt_gemm(ga, st));
+  }
+  return MAPL_OK;
+}
+
 }  // namespace mapl

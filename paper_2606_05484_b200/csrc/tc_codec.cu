@@ -18,7 +18,8 @@ bool tc_shape_ok(const mapl_boundary_desc& d) {
 size_t tc_workspace_bytes(const mapl_boundary_desc& d) {
   if (!tc_shape_ok(d)) return 0;
   const size_t pack = align_up((size_t)(d.r + d.anchor_rank) * d.d * 2, 256);
-  return 2 * pack;
+  // + bf16 zhat [N, r] materialised from RVQ codes for the dU operand of backward
+  return 2 * pack + (d.rvq_levels > 0 ? align_up((size_t)d.n_tokens * d.r * 2, 256) : 0);
 }
 
 TcPacks tc_packs(const mapl_boundary_desc& d, char* tc_ws) {

@@ -20,6 +20,8 @@ struct TcPacks {
   int kc;   // r + ra
 };
 TcPacks tc_packs(const mapl_boundary_desc& d, char* tc_ws);
+// tokens per CTA (<= 128, multiple of 8) such that the grid covers the 148 SMs in whole, even waves
+int tc_tile_m(long long N);
 // which: bit0 = WB rows [0,r) (U^T), bit1 = WB rows [r,r+ra) (B), bit2 = Wd cols [0,r) (U), bit3 = Wd cols [r,..) (B^T)
 int tc_pack_params(const mapl_boundary_desc& d, const float* U, const float* B, const TcPacks& p, int which,
                    cudaStream_t st);
