@@ -67,6 +67,10 @@ typedef struct {
   int32_t rvq_group_dim; /* must be r or 0 (one group: full-vector RVQ, S3); grouped MCVQ = next     */
   int32_t vocab;         /* V; A is [V,ra]                                                           */
   int32_t anchor_rank;   /* ra; 0 = no anchor term; else ra % 8 == 0; B is [ra,d]                    */
+  const void* param_pack; /* optional DEVICE pointer to the prepared parameter pack written by
+                            mapl_pack_params() for these U, B, codebooks (mapl_param_pack_bytes() bytes);
+                            NULL = every call re-derives what it needs in its workspace.  The caller
+                            guarantees the pack is current (re-pack after every parameter update).   */
 } mapl_boundary_desc;
 
 /* Static strings for a status code / the library build ("mapl-b200 x.y sm_100a"). */
@@ -80,6 +84,18 @@ int mapl_last_cuda_error(void);
 size_t mapl_workspace_bytes(const mapl_boundary_desc* desc);
 /* Device scratch for mapl_stiefel_step on `batch` projectors of shape [d,r].                    */
 size_t mapl_stiefel_workspace_bytes(int32_t d, int32_t r, int32_t batch);
+
+/* PARAMETER PACK (optional).  The tensor-core kernels read U, B and the codebooks as bf16 operand
+ * tiles (U additionally as a two-term bf16 split when RVQ follows, so z stays fp32-accurate) plus
+ * per-codeword half squared norms.  mapl_pack_params writes that derived copy into caller-owned
+ * device memory `pack_out` (mapl_param_pack_bytes(desc) bytes, 256-byte aligned; 0 bytes when the
+ * boundary runs on the fp32 kernels: then pack_out may be NULL and the call is a no-op).  In the
+ * paper's schedule the parameters change once per optimizer step while ~128 micro-batches cross
+ * the boundary, so the pack is made once per step and referenced from
+ * desc.param_pack.  B / codebooks may be NULL when anchor_rank / rvq_levels is 0.                 */
+size_t mapl_param_pack_bytes(const mapl_boundary_desc* desc);
+int mapl_pack_params(const mapl_boundary_desc* desc, const float* U, const float* B, const float* codebooks,
+                     void* pack_out, void* cuda_stream);
 
 /* ENCODE (sender side).  P:73 Eq. 1 with h already centred (S6): z_n = U^T h_n.
  * If desc.rvq_levels == L > 0 (S3, S4): rho_0 = z_n; for l < L:

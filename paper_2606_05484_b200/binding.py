@@ -28,7 +28,7 @@ class BoundaryDesc(C.Structure):
     """mapl_boundary_desc (include/mapl.h)."""
     _fields_ = [("n_tokens", C.c_int64), ("d", C.c_int32), ("r", C.c_int32), ("act_dtype", C.c_int32),
                 ("rvq_levels", C.c_int32), ("rvq_k", C.c_int32), ("rvq_group_dim", C.c_int32),
-                ("vocab", C.c_int32), ("anchor_rank", C.c_int32)]
+                ("vocab", C.c_int32), ("anchor_rank", C.c_int32), ("param_pack", C.c_void_p)]
 
 
 def _load():
@@ -46,6 +46,10 @@ def _load():
     lib.mapl_workspace_bytes.argtypes = [dp]
     lib.mapl_stiefel_workspace_bytes.restype = sz
     lib.mapl_stiefel_workspace_bytes.argtypes = [i32, i32, i32]
+    lib.mapl_param_pack_bytes.restype = sz
+    lib.mapl_param_pack_bytes.argtypes = [dp]
+    lib.mapl_pack_params.restype = C.c_int
+    lib.mapl_pack_params.argtypes = [dp, vp, vp, vp, vp, vp]
     lib.mapl_encode.argtypes = [dp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.mapl_decode.argtypes = [dp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.mapl_codec_backward.argtypes = [dp] + [vp] * 14 + [C.c_int, vp, sz, vp]
@@ -97,7 +101,8 @@ def version() -> str:
 def make_desc(n_tokens: int, d: int, r: int, act_dtype: torch.dtype, rvq_levels: int = 0, rvq_k: int = 0,
               vocab: int = 0, anchor_rank: int = 0) -> BoundaryDesc:
     act = {torch.float32: MAPL_F32, torch.bfloat16: MAPL_BF16}[act_dtype]
-    return BoundaryDesc(n_tokens, d, r, act, rvq_levels, rvq_k, r if rvq_levels > 0 else 0, vocab, anchor_rank)
+    return BoundaryDesc(n_tokens, d, r, act, rvq_levels, rvq_k, r if rvq_levels > 0 else 0, vocab, anchor_rank,
+                        None)
 
 
 def act_torch_dtype(desc: BoundaryDesc) -> torch.dtype:
@@ -116,6 +121,18 @@ def mapl_stiefel_workspace_bytes(d: int, r: int, batch: int) -> int:
     if n == 0:
         raise MaplError("mapl_stiefel_workspace_bytes: invalid shape")
     return n
+
+
+def mapl_param_pack_bytes(desc: BoundaryDesc) -> int:
+    return int(_lib.mapl_param_pack_bytes(C.byref(desc)))
+
+
+def mapl_pack_params(desc: BoundaryDesc, U, B, codebooks, pack_out) -> None:
+    """Write the prepared parameter pack for (U, B, codebooks) into `pack_out` (uint8 device tensor of
+    mapl_param_pack_bytes(desc) bytes).  Reference it with `desc.param_pack = pack_out.data_ptr()`."""
+    f = torch.float32
+    _check(_lib.mapl_pack_params(C.byref(desc), _ptr(U, f, "U"), _ptr(B, f, "B"), _ptr(codebooks, f, "codebooks"),
+                                 _ptr(pack_out, None, "pack_out"), _stream()), "mapl_pack_params")
 
 
 def alloc_workspace(nbytes: int, device="cuda") -> torch.Tensor:

@@ -32,7 +32,8 @@ struct Ws {
   size_t half_norm = 0;   // [L*K] fp32
   size_t zhat = 0;        // [N*r] fp32 (dequantised codes, SIMT path)
   size_t gA = 0;          // [N*ra] fp32
-  size_t tc = 0;          // tensor-core path scratch (parameter packs, partials)
+  size_t pack = 0;        // tensor-core parameter pack, used when desc.param_pack == NULL
+  size_t tc = 0;          // tensor-core path scratch (bf16 zhat)
   size_t total = 0;
 };
 
@@ -43,9 +44,21 @@ Ws carve(const mapl_boundary_desc& d) {
   w.half_norm = seg((size_t)d.rvq_levels * (size_t)d.rvq_k * 4);
   w.zhat = seg(d.rvq_levels > 0 ? (size_t)d.n_tokens * d.r * 4 : 0);
   w.gA = seg((size_t)d.n_tokens * d.anchor_rank * 4);
-  w.tc = seg(tc_workspace_bytes(d));
+  w.pack = seg(tc_pack_layout(d, nullptr).bytes);
+  w.tc = seg(tc_scratch_bytes(d));
   w.total = off + 256;
   return w;
+}
+
+// the parameter pack of this call: the caller's (desc.param_pack) or one built now in the workspace
+int resolve_pack(const mapl_boundary_desc& d, const float* U, const float* B, const float* codebooks, char* ws,
+                 const Ws& w, cudaStream_t st, TcPack* out) {
+  if (d.param_pack) {
+    *out = tc_pack_layout(d, const_cast<char*>(reinterpret_cast<const char*>(d.param_pack)));
+    return MAPL_OK;
+  }
+  *out = tc_pack_layout(d, ws + w.pack);
+  return tc_pack_build(d, U, B, codebooks, *out, st);
 }
 
 bool all16(std::initializer_list<const void*> ps) {
@@ -76,6 +89,24 @@ const char* mapl_version(void) { return "mapl-b200 0.1 sm_100a"; }
 
 int mapl_last_cuda_error(void) { return g_last_cuda_error; }
 
+size_t mapl_param_pack_bytes(const mapl_boundary_desc* desc) {
+  if (validate_desc(desc) != MAPL_OK) return 0;
+  return tc_pack_layout(*desc, nullptr).bytes;
+}
+
+int mapl_pack_params(const mapl_boundary_desc* desc, const float* U, const float* B, const float* codebooks,
+                     void* pack_out, void* cuda_stream) {
+  MAPL_RETURN_IF(validate_desc(desc));
+  const mapl_boundary_desc& d = *desc;
+  const TcPack lay = tc_pack_layout(d, reinterpret_cast<char*>(pack_out));
+  if (lay.bytes == 0) return MAPL_OK;                       // fp32 kernels read the masters directly
+  if (!U || !pack_out) return MAPL_ERR_INVALID_ARG;
+  if (d.anchor_rank > 0 && !B) return MAPL_ERR_INVALID_ARG;
+  if (d.rvq_levels > 0 && !codebooks) return MAPL_ERR_INVALID_ARG;
+  if (!all16({U, B, codebooks}) || (reinterpret_cast<uintptr_t>(pack_out) & 255u)) return MAPL_ERR_ALIGNMENT;
+  return tc_pack_build(d, U, B, codebooks, lay, reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
 size_t mapl_workspace_bytes(const mapl_boundary_desc* desc) {
   if (validate_desc(desc) != MAPL_OK) return 0;
   return carve(*desc).total;
@@ -97,8 +128,12 @@ int mapl_encode(const mapl_boundary_desc* desc, const void* H, const float* U, c
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   char* ws = reinterpret_cast<char*>(workspace);
 
-  int s = tc_encode(d, H, U, codebooks, Zq_out, codes_out, ws + w.tc, st);
-  if (s != MAPL_ERR_UNSUPPORTED) return s;
+  if (tc_shape_ok(d) && (L == 0 || tc_rvq_ok(d))) {
+    TcPack pk;
+    MAPL_RETURN_IF(resolve_pack(d, U, nullptr, codebooks, ws, w, st, &pk));
+    int s = tc_encode(d, H, codebooks, pk, Zq_out, codes_out, st);
+    if (s != MAPL_ERR_UNSUPPORTED) return s;
+  }
 
   const int bf = d.act_dtype == MAPL_BF16;
   if (L == 0) {   // Z = H U
@@ -131,8 +166,12 @@ int mapl_decode(const mapl_boundary_desc* desc, const void* Z, const int32_t* co
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   char* ws = reinterpret_cast<char*>(workspace);
 
-  int s = tc_decode(d, Z, codes, U, codebooks, tok, A, B, Hhat_out, ws + w.tc, st);
-  if (s != MAPL_ERR_UNSUPPORTED) return s;
+  if (tc_shape_ok(d)) {
+    TcPack pk;
+    MAPL_RETURN_IF(resolve_pack(d, U, B, codebooks, ws, w, st, &pk));
+    int s = tc_decode(d, Z, codes, codebooks, tok, A, pk, Hhat_out, st);
+    if (s != MAPL_ERR_UNSUPPORTED) return s;
+  }
 
   const int bf = d.act_dtype == MAPL_BF16;
   GemmArgs g;
@@ -188,14 +227,19 @@ int mapl_codec_backward(const mapl_boundary_desc* desc, const void* g_Hhat, cons
   const long long N = d.n_tokens;
   const int ra = anchor ? d.anchor_rank : 0;
 
+  if (tc_shape_ok(d)) {
+    TcPack pk;
+    MAPL_RETURN_IF(resolve_pack(d, U, anchor ? B : nullptr, codebooks, ws, w, st, &pk));
+    int s = tc_backward(d, g_Hhat, H, Z, codes, codebooks, anchor ? tok : nullptr, A, pk, gz_out, dU_out, dA_out,
+                        dB_out, dH_out, accumulate, reinterpret_cast<float*>(ws + w.gA),
+                        reinterpret_cast<__nv_bfloat16*>(ws + w.tc), st);
+    if (s != MAPL_ERR_UNSUPPORTED) return s;
+  }
   if (!accumulate) {
     { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(dU_out, 0, (size_t)d.d * d.r * 4, st)); }
     if (anchor) { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(dA_out, 0, (size_t)d.vocab * ra * 4, st)); }
     if (anchor && dB_out) { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(dB_out, 0, (size_t)ra * d.d * 4, st)); }
   }
-  int s = tc_backward(d, g_Hhat, H, Z, codes, U, codebooks, anchor ? tok : nullptr, A, B, gz_out, dU_out,
-                      dA_out, dB_out, dH_out, ws + w.tc, reinterpret_cast<float*>(ws + w.gA), st);
-  if (s != MAPL_ERR_UNSUPPORTED) return s;
 
   const int bf = d.act_dtype == MAPL_BF16;
   // zhat operand

@@ -3,11 +3,17 @@
 // k_tc_bwd_gz   one CTA per token tile, two phases over one read of g:
 //     phase 1   [gz | gA] = g . [U | B^T]         K = d, streamed through a TMA ring
 //               epilogue: gz -> bf16 -> gz_out (the backward wire payload) and -> smem as the A
-//               operand of phase 2; gA rows -> red.global.add.v4.f32 into dA[tok] (scatter-add)
+//               operand of phase 2; gA rows -> fp32 scratch [N,ra]
 //     phase 2   dH = gz . U^T                     the chunk pipeline of tc_tile_ops.cuh
+//               While phase 1 streams, the epilogue warps zero dU / dA / dB (overwrite mode): no
+//               separate memset launches.
 // k_tc_bwd_du   dU[d-tile, :] += sum over a token range of  g^T Zhat + H^T gz.  Both operands are
 //               MN-major (tokens are the contraction index): TMA boxes [64 tokens x 64 cols]
 //               are used as they land.  Split over token ranges; fp32 vector atomics into dU.
+//               While the MMAs run, the epilogue warps scatter-add the gA rows into dA[tok]:
+//               per 128-token block the rows of equal token id are first summed in shared memory
+//               (Zipf ids: the hottest id owns ~14 % of all rows), then one red.global.add.v4 row
+//               per distinct id leaves the CTA.
 // Roofline: HBM at configs 1-2 (g, H read; dH written), tensor at config 3.
 #include "profile.cuh"
 #include "tc_codec.cuh"
@@ -25,7 +31,10 @@ __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float 
 
 // ---------------------------------------------------------------- gz / dA / dH
 struct BwdGzParams {
-  const int32_t* tok; float* dA; __nv_bfloat16* gz_out;
+  float* gA; __nv_bfloat16* gz_out;
+  float* z0; long long n0;      // overwrite mode: fp32 arrays to zero (element counts, multiples of 4)
+  float* z1; long long n1;
+  float* z2; long long n2;
   long long N;
   int d, r, ra, tile_m;
   int stages1, stage1_bytes, b_stages, do_dh;
@@ -123,6 +132,19 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
     const long long m = m0 + row;
     const bool live = row < p.tile_m && m < p.N;
     const uint32_t tmem_row = c.tmem_base + ((uint32_t)(q * 32) << 16);
+    {   // overwrite mode: this CTA's slice of dU / dA / dB := 0 while phase 1 streams
+      const int et = threadIdx.x - 64;
+      const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+      float* zp[3] = {p.z0, p.z1, p.z2};
+      const long long zn[3] = {p.n0, p.n1, p.n2};
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        if (zp[a] == nullptr) continue;
+        const long long nv = zn[a] / 4, per = (nv + gridDim.x - 1) / gridDim.x;
+        const long long lo = per * blockIdx.x, hi = lo + per < nv ? lo + per : nv;
+        for (long long i = lo + et; i < hi; i += 128) reinterpret_cast<float4*>(zp[a])[i] = zero;
+      }
+    }
     mbar_wait(acc1_full, 0);
     tc_fence_after_sync();
     for (int cc = 0; cc < p.r / 32; ++cc) {
@@ -141,7 +163,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
       }
     }
     if (p.ra) {
-      float* dst = p.dA + (live ? (long long)p.tok[m] : 0) * p.ra;
+      float4* dst = reinterpret_cast<float4*>(p.gA + (live ? m : 0) * p.ra);
       for (int cc = 0; cc < p.ra / 32; ++cc) {
         uint32_t v[32];
         tmem_ld32(tmem_row + p.r + cc * 32, v);
@@ -149,8 +171,8 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         if (live) {
 #pragma unroll
           for (int i = 0; i < 8; ++i)
-            red_add_v4(dst + cc * 32 + i * 4, __uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
-                       __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+            dst[cc * 8 + i] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
+                                          __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
         }
       }
     }
@@ -175,7 +197,38 @@ struct BwdDuParams {
   float* dU;
   long long N;
   int d, r, n_src, stages, item_bytes, blocks_per_split, n_blocks;
+  const int32_t* tok; const float* gA; float* dA;   // anchor-gradient scatter (tok == nullptr: none)
+  int ra;
 };
+
+// dA[tok_n, :] += gA[n, :] for the 128-token blocks this CTA owns; called by the 128 epilogue threads.
+__device__ __forceinline__ void scatter_gA(const BwdDuParams& p, float* sG, int* sTok, int cta, int n_ctas) {
+  const int et = threadIdx.x - 64, pitch = p.ra + 4, vpr = p.ra / 4;
+  for (long long base = (long long)cta * 128; base < p.N; base += (long long)n_ctas * 128) {
+    const int cnt = (int)(p.N - base < 128 ? p.N - base : 128);
+    const float4* src = reinterpret_cast<const float4*>(p.gA + base * p.ra);
+    for (int i = et; i < cnt * vpr; i += 128)
+      *reinterpret_cast<float4*>(sG + (i / vpr) * pitch + (i % vpr) * 4) = __ldg(src + i);
+    const int my = et < cnt ? __ldg(p.tok + base + et) : -1 - et;
+    sTok[et] = my;
+    asm volatile("bar.sync 1, 128;" ::: "memory");
+    int leader = et;
+    for (int j = 0; j < et; ++j)
+      if (sTok[j] == my) { leader = j; break; }
+    if (et < cnt && leader != et) {
+      const float* mine = sG + et * pitch;
+      float* dst = sG + leader * pitch;
+      for (int c = 0; c < p.ra; ++c) atomicAdd(dst + c, mine[c]);
+    }
+    asm volatile("bar.sync 1, 128;" ::: "memory");
+    if (et < cnt && leader == et) {
+      const float4* mine = reinterpret_cast<const float4*>(sG + et * pitch);
+      float* dst = p.dA + (long long)my * p.ra;
+      for (int c = 0; c < vpr; ++c) { const float4 v = mine[c]; red_add_v4(dst + c * 4, v.x, v.y, v.z, v.w); }
+    }
+    asm volatile("bar.sync 1, 128;" ::: "memory");
+  }
+}
 
 __global__ void __launch_bounds__(kThreads, 1)
 k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmZ,
@@ -186,6 +239,8 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   uint64_t* empty = full + p.stages;
   uint64_t* acc_full = empty + p.stages;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_full + 1);
+  float* sG = reinterpret_cast<float*>(smem + (size_t)p.stages * p.item_bytes + 512);   // [128][ra+4]
+  int* sTok = reinterpret_cast<int*>(sG + 128 * (p.ra + 4));
 
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
   const int dt = blockIdx.x;                                   // 128 rows of dU
@@ -211,6 +266,8 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
 
+  if (warp >= 2 && p.tok != nullptr)
+    scatter_gA(p, sG, sTok, blockIdx.y * gridDim.x + blockIdx.x, gridDim.x * gridDim.y);
   if (n_items > 0) {
     if (warp == 0) {
       if (elect_one()) {
@@ -287,14 +344,11 @@ __global__ void k_tc_dequant_bf16(const int32_t* __restrict__ codes, const float
 }  // namespace
 
 int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const void* Z, const int32_t* codes,
-                const float* U, const float* codebooks, const int32_t* tok, const float* A, const float* B,
-                void* gz_out, float* dU_out, float* dA_out, float* dB_out, void* dH_out, char* tc_ws, float* gA_ws,
-                cudaStream_t st) {
-  (void)gA_ws;
+                const float* codebooks, const int32_t* tok, const float* A, const TcPack& pk, void* gz_out,
+                float* dU_out, float* dA_out, float* dB_out, void* dH_out, int accumulate, float* gA_ws,
+                __nv_bfloat16* zhat_ws, cudaStream_t st) {
   if (!tc_shape_ok(d)) return MAPL_ERR_UNSUPPORTED;
   const int ra = tok ? d.anchor_rank : 0, kc = d.r + ra;
-  const TcPacks pk = tc_packs(d, tc_ws);
-  MAPL_RETURN_IF(tc_pack_params(d, U, B, pk, 1 | (ra ? 2 : 0) | (dH_out ? 4 : 0), st));
 
   static bool attr_done = false;
   if (!attr_done) {
@@ -307,18 +361,23 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
   // zhat operand for dU
   const void* zhat = Z;
   if (codes) {
-    __nv_bfloat16* zb = reinterpret_cast<__nv_bfloat16*>(tc_ws + 2 * align_up((size_t)(d.r + d.anchor_rank) * d.d * 2, 256));
     const long long total = d.n_tokens * (d.r / 8);
     KernelScope ks(KID_DEQUANT, st);
-    k_tc_dequant_bf16<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(codes, codebooks, zb, d.n_tokens, d.r,
+    k_tc_dequant_bf16<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(codes, codebooks, zhat_ws, d.n_tokens, d.r,
                                                                       d.rvq_levels, d.rvq_k);
     MAPL_CUDA_CHECK(cudaGetLastError());
-    zhat = zb;
+    zhat = zhat_ws;
   }
 
-  {  // ---- gz, dA, dH
+  {  // ---- gz, gA, dH (+ zero fill of the overwrite outputs)
     BwdGzParams p;
-    p.tok = tok; p.dA = dA_out; p.gz_out = reinterpret_cast<__nv_bfloat16*>(gz_out);
+    p.gA = gA_ws; p.gz_out = reinterpret_cast<__nv_bfloat16*>(gz_out);
+    p.z0 = p.z1 = p.z2 = nullptr; p.n0 = p.n1 = p.n2 = 0;
+    if (!accumulate) {
+      p.z0 = dU_out; p.n0 = (long long)d.d * d.r;
+      if (ra) { p.z1 = dA_out; p.n1 = (long long)d.vocab * ra; }
+      if (ra && dB_out) { p.z2 = dB_out; p.n2 = (long long)ra * d.d; }
+    }
     p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.ra = ra; p.tile_m = tc_tile_m(d.n_tokens);
     p.do_dh = dH_out ? 1 : 0;
     p.stage1_bytes = kTileBytes + kc * 128;
@@ -334,8 +393,8 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     const size_t smem = (ring1 > ring2 ? ring1 : ring2) + (size_t)kOutBufs * kTileBytes + 1024 + 1024;
     CUtensorMap tmG, tmWu, tmWb, tmWd, tmO;
     if (!make_tmap_bf16_2d(&tmG, g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
-    if (!make_tmap_bf16_2d(&tmWu, pk.WB, (uint64_t)(d.r + d.anchor_rank), dd, dd, 64, (uint32_t)d.r)) return MAPL_ERR_CUDA;
-    if (!make_tmap_bf16_2d(&tmWb, pk.WB, (uint64_t)(d.r + d.anchor_rank), dd, dd, 64, (uint32_t)(ra ? ra : 64))) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmWu, pk.WB, (uint64_t)pk.kc, dd, dd, 64, (uint32_t)d.r)) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmWb, pk.WB, (uint64_t)pk.kc, dd, dd, 64, (uint32_t)(ra ? ra : 64))) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmWd, pk.Wd, dd, (uint64_t)pk.kc, (uint64_t)pk.kc, 64, kChunkN)) return MAPL_ERR_CUDA;
     // dH map: when dH is skipped the map is unused but must be valid
     if (!make_tmap_bf16_2d(&tmO, dH_out ? dH_out : g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
@@ -343,12 +402,15 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     KernelScope ks(KID_TC_BWD_GZ, st);
     MAPL_CUDA_CHECK(launch_pdl(k_tc_bwd_gz, dim3(tiles), dim3(kThreads), smem, st, tmG, tmWu, tmWb, tmWd, tmO, p));
   }
-  {  // ---- dU
+  {  // ---- dU (+ dA scatter)
     BwdDuParams p;
     p.dU = dU_out; p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.n_src = H ? 2 : 1;
+    p.tok = ra ? tok : nullptr; p.gA = gA_ws; p.dA = dA_out; p.ra = ra;
     p.item_bytes = 2 * 64 * 128 + (d.r / 64) * 64 * 128;
-    p.stages = (int)((227 * 1024 - 2048) / p.item_bytes);
+    const size_t scatter_bytes = ra ? (size_t)128 * (ra + 4) * 4 + 512 : 0;
+    p.stages = (int)((227 * 1024 - 2048 - scatter_bytes) / p.item_bytes);
     if (p.stages > 8) p.stages = 8;
+    if (p.stages < 2) return MAPL_ERR_UNSUPPORTED;
     p.n_blocks = (int)((d.n_tokens + 63) / 64);
     const int n_dt = d.d / 128;
     int S = 148 / n_dt;
@@ -356,7 +418,7 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     if (S > p.n_blocks) S = p.n_blocks;
     p.blocks_per_split = (p.n_blocks + S - 1) / S;
     S = (p.n_blocks + p.blocks_per_split - 1) / p.blocks_per_split;
-    const size_t smem = (size_t)p.stages * p.item_bytes + 1024 + 512;
+    const size_t smem = (size_t)p.stages * p.item_bytes + 1024 + 512 + scatter_bytes;
     CUtensorMap tmG, tmZ, tmH, tmGz;
     if (!make_tmap_bf16_2d(&tmG, g, N, dd, dd, 64, 64)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmZ, zhat, N, rr, rr, 64, 64)) return MAPL_ERR_CUDA;

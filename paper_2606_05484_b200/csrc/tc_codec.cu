@@ -1,5 +1,5 @@
-// tc_codec.cu -- envelope checks, parameter packing and workspace layout shared by the tcgen05 codec
-// kernels (tc_encode.cu, tc_decode.cu, tc_backward.cu).
+// tc_codec.cu -- envelope checks and the parameter pack shared by the tcgen05 codec kernels
+// (tc_encode.cu, tc_encode_rvq.cu, tc_decode.cu, tc_backward.cu).
 #include "tc_codec.cuh"
 
 #include "profile.cuh"
@@ -15,20 +15,42 @@ bool tc_shape_ok(const mapl_boundary_desc& d) {
   return true;
 }
 
-size_t tc_workspace_bytes(const mapl_boundary_desc& d) {
-  if (!tc_shape_ok(d)) return 0;
-  const size_t pack = align_up((size_t)(d.r + d.anchor_rank) * d.d * 2, 256);
-  // + bf16 zhat [N, r] materialised from RVQ codes for the dU operand of backward
-  return 2 * pack + (d.rvq_levels > 0 ? align_up((size_t)d.n_tokens * d.r * 2, 256) : 0);
+bool tc_rvq_ok(const mapl_boundary_desc& d) {
+  return tc_shape_ok(d) && d.rvq_levels > 0 && d.rvq_k >= 128 && d.rvq_k % 128 == 0;
 }
 
-TcPacks tc_packs(const mapl_boundary_desc& d, char* tc_ws) {
-  const size_t pack = align_up((size_t)(d.r + d.anchor_rank) * d.d * 2, 256);
-  TcPacks p;
-  p.WB = reinterpret_cast<__nv_bfloat16*>(tc_ws);
-  p.Wd = reinterpret_cast<__nv_bfloat16*>(tc_ws + pack);
+TcPack tc_pack_layout(const mapl_boundary_desc& d, char* base) {
+  TcPack p;
+  if (!tc_shape_ok(d)) return p;
+  size_t off = 0;
+  auto seg = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return base ? base + o : nullptr; };
   p.kc = d.r + d.anchor_rank;
+  p.WB = reinterpret_cast<__nv_bfloat16*>(seg((size_t)p.kc * d.d * 2));
+  p.Wd = reinterpret_cast<__nv_bfloat16*>(seg((size_t)p.kc * d.d * 2));
+  if (d.rvq_levels > 0) {
+    const size_t LK = (size_t)d.rvq_levels * d.rvq_k;
+    p.WBlo = reinterpret_cast<__nv_bfloat16*>(seg((size_t)d.r * d.d * 2));
+    p.Cb = reinterpret_cast<__nv_bfloat16*>(seg(LK * d.r * 2));
+    p.hn = reinterpret_cast<float*>(seg(LK * 4));
+    p.cmax = reinterpret_cast<float*>(seg(8 * 4));
+  }
+  p.bytes = off;
   return p;
+}
+
+size_t tc_scratch_bytes(const mapl_boundary_desc& d) {
+  if (!tc_shape_ok(d)) return 0;
+  return d.rvq_levels > 0 ? align_up((size_t)d.n_tokens * d.r * 2, 256) : 0;
+}
+
+int tc_tile_m(long long N) {
+  const long long per_wave = 148ll * 128;
+  const long long waves = (N + per_wave - 1) / per_wave;
+  long long t = (N + 148 * waves - 1) / (148 * waves);
+  t = (t + 7) / 8 * 8;
+  if (t > 128) t = 128;
+  if (t < 8) t = 8;
+  return (int)t;
 }
 
 namespace {
@@ -37,8 +59,14 @@ struct PackJob {
   const float* src; int rows, cols;        // src is [rows, cols] fp32 row-major
   __nv_bfloat16* dst; long long pitch;     // dst element (i,j) -> dst[i*pitch + j] (after optional transpose)
   int transpose;
+  int lo;                                  // 1: store bf16(x - float(bf16(x))), the second split term
 };
-struct PackArgs { PackJob job[4]; int njobs; };
+struct PackArgs { PackJob job[6]; int njobs; };
+
+__device__ __forceinline__ __nv_bfloat16 pack_term(float x, int lo) {
+  const __nv_bfloat16 hi = __float2bfloat16_rn(x);
+  return lo ? __float2bfloat16_rn(x - __bfloat162float(hi)) : hi;
+}
 
 // 32x32 tiles; blockIdx.y = job
 __global__ void __launch_bounds__(256) k_tc_pack(const PackArgs a) {
@@ -56,33 +84,61 @@ __global__ void __launch_bounds__(256) k_tc_pack(const PackArgs a) {
     if (j.transpose) {
       for (int i = ty; i < 32; i += 8) {
         const int c = c0 + i, r = r0 + tx;           // dst row = src col
-        if (c < j.cols && r < j.rows) j.dst[(long long)c * j.pitch + r] = __float2bfloat16_rn(tile[tx][i]);
+        if (c < j.cols && r < j.rows) j.dst[(long long)c * j.pitch + r] = pack_term(tile[tx][i], j.lo);
       }
     } else {
       for (int i = ty; i < 32; i += 8) {
         const int r = r0 + i, c = c0 + tx;
-        if (r < j.rows && c < j.cols) j.dst[(long long)r * j.pitch + c] = __float2bfloat16_rn(tile[i][tx]);
+        if (r < j.rows && c < j.cols) j.dst[(long long)r * j.pitch + c] = pack_term(tile[i][tx], j.lo);
       }
     }
     __syncthreads();
   }
 }
 
+// one block per level: cmax[l] = max_k sqrt(2 hn[l,k])
+__global__ void __launch_bounds__(256) k_tc_cmax(const float* __restrict__ hn, float* __restrict__ cmax, int K) {
+  __shared__ float red[8];
+  float m = 0.f;
+  for (int k = threadIdx.x; k < K; k += 256) m = fmaxf(m, hn[(long long)blockIdx.x * K + k]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if (threadIdx.x % 32 == 0) red[threadIdx.x / 32] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int i = 1; i < 8; ++i) m = fmaxf(m, red[i]);
+    cmax[blockIdx.x] = sqrtf(2.f * m);
+  }
+}
+
 }  // namespace
 
-int tc_pack_params(const mapl_boundary_desc& d, const float* U, const float* B, const TcPacks& p, int which,
-                   cudaStream_t st) {
+int tc_pack_build(const mapl_boundary_desc& d, const float* U, const float* B, const float* codebooks,
+                  const TcPack& p, cudaStream_t st) {
   PackArgs a;
   a.njobs = 0;
   const int ra = d.anchor_rank;
-  if (which & 1) a.job[a.njobs++] = PackJob{U, d.d, d.r, p.WB, d.d, 1};                               // WB[j][i] = U[i][j]
-  if ((which & 2) && ra && B) a.job[a.njobs++] = PackJob{B, ra, d.d, p.WB + (long long)d.r * d.d, d.d, 0};
-  if (which & 4) a.job[a.njobs++] = PackJob{U, d.d, d.r, p.Wd, p.kc, 0};                              // Wd[i][j] = U[i][j]
-  if ((which & 8) && ra && B) a.job[a.njobs++] = PackJob{B, ra, d.d, p.Wd + d.r, p.kc, 1};            // Wd[i][r+q] = B[q][i]
-  if (a.njobs == 0) return MAPL_OK;
-  KernelScope ks(KID_TC_PACK, st);
-  k_tc_pack<<<dim3(128, a.njobs), 256, 0, st>>>(a);
-  MAPL_CUDA_CHECK(cudaGetLastError());
+  a.job[a.njobs++] = PackJob{U, d.d, d.r, p.WB, d.d, 1, 0};                                        // WB[j][i] = U[i][j]
+  a.job[a.njobs++] = PackJob{U, d.d, d.r, p.Wd, p.kc, 0, 0};                                       // Wd[i][j] = U[i][j]
+  if (ra && B) {
+    a.job[a.njobs++] = PackJob{B, ra, d.d, p.WB + (long long)d.r * d.d, d.d, 0, 0};
+    a.job[a.njobs++] = PackJob{B, ra, d.d, p.Wd + d.r, p.kc, 1, 0};                                // Wd[i][r+q] = B[q][i]
+  }
+  if (d.rvq_levels > 0 && p.WBlo) {
+    a.job[a.njobs++] = PackJob{U, d.d, d.r, p.WBlo, d.d, 1, 1};
+    if (codebooks) a.job[a.njobs++] = PackJob{codebooks, d.rvq_levels * d.rvq_k, d.r, p.Cb, d.r, 0, 0};
+  }
+  {
+    KernelScope ks(KID_TC_PACK, st);
+    k_tc_pack<<<dim3(148, a.njobs), 256, 0, st>>>(a);
+    MAPL_CUDA_CHECK(cudaGetLastError());
+  }
+  if (d.rvq_levels > 0 && p.hn && codebooks) {
+    MAPL_RETURN_IF(simt_half_sqnorm(codebooks, p.hn, d.rvq_levels * d.rvq_k, d.r, st));
+    KernelScope ks(KID_TC_PACK, st);
+    k_tc_cmax<<<d.rvq_levels, 256, 0, st>>>(p.hn, p.cmax, d.rvq_k);
+    MAPL_CUDA_CHECK(cudaGetLastError());
+  }
   return MAPL_OK;
 }
 

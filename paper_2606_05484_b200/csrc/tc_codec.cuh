@@ -2,41 +2,54 @@
 // MAPL_ERR_UNSUPPORTED when the boundary is outside its envelope (the caller then runs the fp32
 // SIMT kernels), MAPL_OK once everything is enqueued, or an error.
 //
-// Envelope (v1): bf16 activations, d % 128 == 0, r in {64,128,256}, anchor_rank in {0,64,128}.
-// Parameter packs (bf16, rebuilt by every call from the fp32 masters; a few hundred KB):
-//   WB [(r+ra), d] = [U^T ; B]    K-major over d     (encode / backward-gz B operand)
-//   Wd [d, (r+ra)] = [U | B^T]    K-major over r+ra  (decode / backward-dH B operand)
+// Envelope: bf16 activations, d % 128 == 0, r in {64,128,256}, anchor_rank in {0,64,128};
+// RVQ on the tensor cores additionally needs K % 128 == 0.
+//
+// Parameter pack (bf16 operand copies of the fp32 masters, see mapl_pack_params in mapl.h):
+//   WB   [(r+ra), d] = [U^T ; B]    K-major over d     (encode / backward-gz B operand)
+//   Wd   [d, (r+ra)] = [U | B^T]    K-major over r+ra  (decode / backward-dH B operand)
+//   WBlo [r, d]      = (U - bf16(U))^T                 (second split term: fp32-accurate z for RVQ)
+//   Cb   [L*K, r]    bf16 codebooks;  hn [L*K] = 0.5 ||C_k||^2 (fp32);  cmax [L] = max_k ||C_l,k||
 #pragma once
 #include "common.cuh"
 
 namespace mapl {
 
-size_t tc_workspace_bytes(const mapl_boundary_desc& d);
 bool tc_shape_ok(const mapl_boundary_desc& d);
+bool tc_rvq_ok(const mapl_boundary_desc& d);
 
-struct TcPacks {
-  __nv_bfloat16* WB;
-  __nv_bfloat16* Wd;
-  int kc;   // r + ra
+struct TcPack {
+  __nv_bfloat16* WB = nullptr;
+  __nv_bfloat16* Wd = nullptr;
+  __nv_bfloat16* WBlo = nullptr;
+  __nv_bfloat16* Cb = nullptr;
+  float* hn = nullptr;
+  float* cmax = nullptr;
+  int kc = 0;          // r + ra
+  size_t bytes = 0;
 };
-TcPacks tc_packs(const mapl_boundary_desc& d, char* tc_ws);
+// layout of a pack placed at `base` (base may be nullptr to query `bytes`); bytes == 0 outside the envelope
+TcPack tc_pack_layout(const mapl_boundary_desc& d, char* base);
+int tc_pack_build(const mapl_boundary_desc& d, const float* U, const float* B, const float* codebooks,
+                  const TcPack& p, cudaStream_t st);
+
+// scratch of the tc path besides the pack: bf16 zhat [N,r] (RVQ codes -> dU operand)
+size_t tc_scratch_bytes(const mapl_boundary_desc& d);
+
 // tokens per CTA (<= 128, multiple of 8) such that the grid covers the 148 SMs in whole, even waves
 int tc_tile_m(long long N);
-// which: bit0 = WB rows [0,r) (U^T), bit1 = WB rows [r,r+ra) (B), bit2 = Wd cols [0,r) (U), bit3 = Wd cols [r,..) (B^T)
-int tc_pack_params(const mapl_boundary_desc& d, const float* U, const float* B, const TcPacks& p, int which,
-                   cudaStream_t st);
 
-int tc_encode(const mapl_boundary_desc& d, const void* H, const float* U, const float* codebooks,
-              void* Zq_out, int32_t* codes_out, char* tc_ws, cudaStream_t st);
+int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
+              int32_t* codes_out, cudaStream_t st);
 
-int tc_decode(const mapl_boundary_desc& d, const void* Z, const int32_t* codes, const float* U,
-              const float* codebooks, const int32_t* tok, const float* A, const float* B, void* Hhat_out,
-              char* tc_ws, cudaStream_t st);
+int tc_decode(const mapl_boundary_desc& d, const void* Z, const int32_t* codes, const float* codebooks,
+              const int32_t* tok, const float* A, const TcPack& pk, void* Hhat_out, cudaStream_t st);
 
-// tok == nullptr: anchor ignored.  gA_ws: [N,ra] fp32 scratch.
+// tok == nullptr: anchor ignored.  gA_ws: [N,ra] fp32 scratch; zhat_ws: [N,r] bf16 scratch.
+// Zeroes dU/dA/dB itself when accumulate == 0.
 int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const void* Z, const int32_t* codes,
-                const float* U, const float* codebooks, const int32_t* tok, const float* A, const float* B,
-                void* gz_out, float* dU_out, float* dA_out, float* dB_out, void* dH_out, char* tc_ws,
-                float* gA_ws, cudaStream_t st);
+                const float* codebooks, const int32_t* tok, const float* A, const TcPack& pk, void* gz_out,
+                float* dU_out, float* dA_out, float* dB_out, void* dH_out, int accumulate, float* gA_ws,
+                __nv_bfloat16* zhat_ws, cudaStream_t st);
 
 }  // namespace mapl

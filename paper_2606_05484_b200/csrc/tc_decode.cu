@@ -84,12 +84,17 @@ k_tc_decode(const __grid_constant__ CUtensorMap tmZ, const __grid_constant__ CUt
     const bool live = row < p.tile_m && m < p.N;
     // ---- A operand columns produced by threads: dequantised zhat and gathered anchor rows
     if (!p.z_from_tma) {
+      const float* rowp[8];
+#pragma unroll
+      for (int l = 0; l < 8; ++l)
+        rowp[l] = p.codebooks + ((long long)(l < p.L ? l : 0) * p.K + ((live && l < p.L) ? __ldg(p.codes + m * p.L + l) : 0)) * p.r;
       for (int cc = 0; cc < p.r / 8; ++cc) {            // 8 columns = one 16-byte chunk
         float s[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         if (live) {
-          for (int l = 0; l < p.L; ++l) {
-            const float4* src = reinterpret_cast<const float4*>(
-                p.codebooks + ((long long)l * p.K + p.codes[m * p.L + l]) * p.r + cc * 8);
+#pragma unroll
+          for (int l = 0; l < 8; ++l) {
+            if (l >= p.L) break;
+            const float4* src = reinterpret_cast<const float4*>(rowp[l] + cc * 8);
             const float4 x = __ldg(src), y = __ldg(src + 1);
             s[0] += x.x; s[1] += x.y; s[2] += x.z; s[3] += x.w; s[4] += y.x; s[5] += y.y; s[6] += y.z; s[7] += y.w;
           }
@@ -99,15 +104,19 @@ k_tc_decode(const __grid_constant__ CUtensorMap tmZ, const __grid_constant__ CUt
       }
     }
     if (p.ra > 0) {
-      const long long t = live ? (long long)p.tok[m] : 0;
-      for (int cc = 0; cc < p.ra / 8; ++cc) {
-        uint4 o = make_uint4(0, 0, 0, 0);
-        if (live) {
-          const float4* src = reinterpret_cast<const float4*>(p.A + t * p.ra + cc * 8);
-          const float4 x = __ldg(src), y = __ldg(src + 1);
-          o = make_uint4(pack_bf16x2(x.x, x.y), pack_bf16x2(x.z, x.w), pack_bf16x2(y.x, y.y), pack_bf16x2(y.z, y.w));
+      const long long t = live ? (long long)__ldg(p.tok + m) : 0;
+      const float4* src = reinterpret_cast<const float4*>(p.A + t * p.ra);
+      for (int c0 = 0; c0 < p.ra / 8; c0 += 4) {       // 8 independent 16-byte loads in flight per thread
+        float4 x[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) x[i] = live ? __ldg(src + c0 * 2 + i) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int cc = c0 + i;
+          const uint4 o = make_uint4(pack_bf16x2(x[2 * i].x, x[2 * i].y), pack_bf16x2(x[2 * i].z, x[2 * i].w),
+                                     pack_bf16x2(x[2 * i + 1].x, x[2 * i + 1].y), pack_bf16x2(x[2 * i + 1].z, x[2 * i + 1].w));
+          *reinterpret_cast<uint4*>(c.sA + (size_t)(p.r / 64 + cc / 8) * kTileBytes + sw128_offset(row, cc % 8)) = o;
         }
-        *reinterpret_cast<uint4*>(c.sA + (size_t)(p.r / 64 + cc / 8) * kTileBytes + sw128_offset(row, cc % 8)) = o;
       }
     }
     fence_proxy_async_smem();
@@ -125,22 +134,10 @@ k_tc_decode(const __grid_constant__ CUtensorMap tmZ, const __grid_constant__ CUt
 
 }  // namespace
 
-int tc_tile_m(long long N) {
-  const long long per_wave = 148ll * 128;
-  const long long waves = (N + per_wave - 1) / per_wave;
-  long long t = (N + 148 * waves - 1) / (148 * waves);
-  t = (t + 7) / 8 * 8;
-  if (t > 128) t = 128;
-  if (t < 8) t = 8;
-  return (int)t;
-}
-
-int tc_decode(const mapl_boundary_desc& d, const void* Z, const int32_t* codes, const float* U, const float* codebooks,
-              const int32_t* tok, const float* A, const float* B, void* Hhat_out, char* tc_ws, cudaStream_t st) {
+int tc_decode(const mapl_boundary_desc& d, const void* Z, const int32_t* codes, const float* codebooks,
+              const int32_t* tok, const float* A, const TcPack& pk, void* Hhat_out, cudaStream_t st) {
   if (!tc_shape_ok(d)) return MAPL_ERR_UNSUPPORTED;
   const int ra = d.anchor_rank, kc = d.r + ra, nkb = kc / 64;
-  const TcPacks pk = tc_packs(d, tc_ws);
-  MAPL_RETURN_IF(tc_pack_params(d, U, B, pk, 4 | 8, st));
   DecodeParams p;
   p.codes = codes; p.codebooks = codebooks; p.tok = ra ? tok : nullptr; p.A = A;
   p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.ra = ra; p.L = d.rvq_levels; p.K = d.rvq_k;

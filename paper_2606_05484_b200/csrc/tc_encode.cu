@@ -1,6 +1,6 @@
 // tc_encode.cu -- mapl_encode on the tensor cores (RVQ off): Z = H U  (Eq. 1, centred h).
 //
-// One CTA per 128-token tile.  Warp 0 streams H tiles [128 x 64] (HBM, evict-first) and U^T tiles
+// One CTA per token tile (tile_m <= 128 tokens, sized so the grid fills the 148 SMs evenly).  Warp 0 streams H tiles [128 x 64] (HBM, evict-first) and U^T tiles
 // [r x 64] (L2-resident pack) through a TMA/mbarrier ring; one thread of warp 1 issues
 // tcgen05.mma (M=128, N=r, K=16) into a TMEM accumulator [128 lanes x r columns]; warps 2-5 read
 // their TMEM lane quarter back (one token row per thread), round to bf16 and store the payload.
@@ -8,6 +8,7 @@
 #include "profile.cuh"
 #include "tc_codec.cuh"
 #include "tc_common.cuh"
+#include "tc_tile_ops.cuh"
 
 namespace mapl {
 namespace {
@@ -18,7 +19,7 @@ constexpr int kATile = BM * BK * 2;   // 16 KB
 
 __global__ void __launch_bounds__(kThreads, 1)
 k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmW,
-            __nv_bfloat16* __restrict__ Z, long long N, int d, int r, int stages) {
+            __nv_bfloat16* __restrict__ Z, long long N, int d, int r, int stages, int tile_m) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int b_tile = r * BK * 2;
@@ -29,7 +30,7 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum_full + 1);
 
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
-  const long long m0 = (long long)blockIdx.x * BM;
+  const long long m0 = (long long)blockIdx.x * tile_m;
   const int nkb = d / BK;
 
   if (warp == 0 && lane == 0) {
@@ -47,13 +48,15 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
   __syncthreads();
   tc_fence_after_sync();
   const uint32_t tmem_d = *tmem_slot;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");       // everything below touches global memory
 
   if (warp == 0) {
     if (elect_one()) {
       for (int kb = 0; kb < nkb; ++kb) {
         const int s = kb % stages;
         mbar_wait(&empty[s], ((kb / stages) & 1) ^ 1);
-        mbar_arrive_expect_tx(&full[s], (uint32_t)stage_bytes);
+        mbar_arrive_expect_tx(&full[s], (uint32_t)(tile_m * 128 + b_tile));
         uint8_t* a = smem + (size_t)s * stage_bytes;
         tma_load_2d(a, &tmH, &full[s], kb * BK, (int)m0, kEvictFirst);
         tma_load_2d(a + kATile, &tmW, &full[s], kb * BK, 0, kEvictLast);
@@ -77,14 +80,15 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
     }
   } else {
     const int q = warp & 3;                         // TMEM lane quarter this warp may read
-    const long long m = m0 + q * 32 + lane;
+    const int row = q * 32 + lane;
+    const long long m = m0 + row;
     mbar_wait(accum_full, 0);
     tc_fence_after_sync();
     for (int c = 0; c < r / 32; ++c) {
       uint32_t v[32];
       tmem_ld32(tmem_d + ((uint32_t)(q * 32) << 16) + c * 32, v);
       tmem_ld_wait();
-      if (m < N) {
+      if (row < tile_m && m < N) {
         uint4* dst = reinterpret_cast<uint4*>(Z + m * r + c * 32);
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -108,15 +112,17 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
 
 }  // namespace
 
-int tc_encode(const mapl_boundary_desc& d, const void* H, const float* U, const float* codebooks, void* Zq_out,
-              int32_t* codes_out, char* tc_ws, cudaStream_t st) {
-  (void)codebooks; (void)codes_out;
-  if (!tc_shape_ok(d) || d.rvq_levels != 0) return MAPL_ERR_UNSUPPORTED;
-  const TcPacks p = tc_packs(d, tc_ws);
-  MAPL_RETURN_IF(tc_pack_params(d, U, nullptr, p, 1, st));
+int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
+                  int32_t* codes_out, cudaStream_t st);   // tc_encode_rvq.cu
+
+int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
+              int32_t* codes_out, cudaStream_t st) {
+  if (!tc_shape_ok(d)) return MAPL_ERR_UNSUPPORTED;
+  if (d.rvq_levels != 0) return tc_encode_rvq(d, H, codebooks, pk, Zq_out, codes_out, st);
+  const int tile_m = tc_tile_m(d.n_tokens);
   CUtensorMap tmH, tmW;
-  if (!make_tmap_bf16_2d(&tmH, H, (uint64_t)d.n_tokens, (uint64_t)d.d, (uint64_t)d.d, BK, BM)) return MAPL_ERR_CUDA;
-  if (!make_tmap_bf16_2d(&tmW, p.WB, (uint64_t)d.r, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)d.r)) return MAPL_ERR_CUDA;
+  if (!make_tmap_bf16_2d(&tmH, H, (uint64_t)d.n_tokens, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)tile_m)) return MAPL_ERR_CUDA;
+  if (!make_tmap_bf16_2d(&tmW, pk.WB, (uint64_t)d.r, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)d.r)) return MAPL_ERR_CUDA;
   const int stage_bytes = kATile + d.r * BK * 2;
   int stages = (200 * 1024) / stage_bytes;
   if (stages > 8) stages = 8;
@@ -127,11 +133,10 @@ int tc_encode(const mapl_boundary_desc& d, const void* H, const float* U, const 
     MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_encode, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     attr_done = true;
   }
-  const unsigned tiles = (unsigned)((d.n_tokens + BM - 1) / BM);
+  const unsigned tiles = (unsigned)((d.n_tokens + tile_m - 1) / tile_m);
   KernelScope ks(KID_TC_ENCODE, st);
-  k_tc_encode<<<tiles, kThreads, smem, st>>>(tmH, tmW, reinterpret_cast<__nv_bfloat16*>(Zq_out), d.n_tokens, d.d,
-                                            d.r, stages);
-  MAPL_CUDA_CHECK(cudaGetLastError());
+  MAPL_CUDA_CHECK(launch_pdl(k_tc_encode, dim3(tiles), dim3(kThreads), smem, st, tmH, tmW,
+                             reinterpret_cast<__nv_bfloat16*>(Zq_out), d.n_tokens, d.d, d.r, stages, tile_m));
   return MAPL_OK;
 }
 
