@@ -16,7 +16,7 @@ bool tc_shape_ok(const mapl_boundary_desc& d) {
 }
 
 bool tc_rvq_ok(const mapl_boundary_desc& d) {
-  return tc_shape_ok(d) && d.rvq_levels > 0 && d.rvq_k >= 128 && d.rvq_k % 128 == 0;
+  return tc_shape_ok(d) && d.rvq_levels > 0 && d.rvq_k >= 128 && d.rvq_k % 128 == 0 && d.rvq_k <= 8192;
 }
 
 TcPack tc_pack_layout(const mapl_boundary_desc& d, char* base) {

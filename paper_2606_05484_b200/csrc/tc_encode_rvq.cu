@@ -1,7 +1,420 @@
-// tc_encode_rvq.cu -- placeholder until the fused projection + RVQ tcgen05 kernel lands.
+// tc_encode_rvq.cu -- mapl_encode with residual VQ on the tensor cores: projection and all RVQ
+// levels in ONE kernel, z never leaves the chip (Eq. 1; Sec. 3.5;
+// readings S3-S5 of DESIGN.md).
+//
+// One CTA per token tile (<= 128 tokens; one TMEM lane = one token).
+//   phase 1   z = H (U_hi + U_lo)      H tiles by TMA (HBM, evict-first), the two bf16 split terms
+//             of U^T from the L2-resident pack; fp32 accumulator [128 x r] in TMEM columns [0,r).
+//             bf16 H is exact and U_hi + U_lo carries 16 mantissa bits, so z is fp32-accurate.
+//   level l   rho (fp32) stays in TMEM columns [0,r); its bf16 rounding is the resident A operand.
+//             Codebook tiles [128 codewords x 64] stream through a TMA ring; per 128-codeword
+//             chunk one accumulator stage S = rho_bf16 . C_bf16^T  (2 stages, TMEM cols 256..511).
+//             Epilogue (thread = token): coarse score s_k = 0.5||c_k||^2 - S_k, running minimum,
+//             and every k with  s_k <= running min + margin  is recorded as a candidate, where
+//               margin = 2 E,   E = 2^-7 * 1.01 * ||rho|| * max_k ||c_k||  >=  |s_coarse - s_exact|
+//             (bf16 rounding of both operands, Cauchy-Schwarz).  The true minimiser is therefore
+//             always among the candidates; they are re-scored in exact fp32 (rho from TMEM, the
+//             fp32 codeword from L2), lowest index winning ties (S4).  Then rho -= C[l, k*].
+// Roofline: tensor at config 3 (K r = 1M per level), HBM/ALU at config 2.
+#include <float.h>
+
+#include "profile.cuh"
 #include "tc_codec.cuh"
+#include "tc_tile_ops.cuh"
+
 namespace mapl {
-int tc_encode_rvq(const mapl_boundary_desc&, const void*, const float*, const TcPack&, void*, int32_t*, cudaStream_t) {
-  return MAPL_ERR_UNSUPPORTED;
+namespace {
+using namespace tc;
+
+constexpr int kThreads = 192;
+constexpr int kChunk = 128;        // codewords per accumulator stage (UMMA N)
+constexpr int kAccCol0 = 256;      // TMEM column of score stage 0
+constexpr int kNE = 12;            // candidate-list entries per token (one entry = one 32-codeword piece)
+
+struct RvqParams {
+  const float* C;        // [L,K,r] fp32 codebooks (exact re-scoring, residual update)
+  const float* hn;       // [L*K] 0.5 ||c||^2
+  const float* cmax;     // [L] max_k ||c_k||
+  __nv_bfloat16* Zq;     // optional [N,r]
+  int32_t* codes;        // [N,L]
+  long long N;
+  int d, r, L, K, tile_m;
+  int stages1, stage1_bytes, ring_tiles;
+};
+
+// smem carve-up (after 1024-byte alignment):
+//   region R  = max(phase-1 ring, rho operand tiles + codebook ring)
+//   sHn [K] fp32 | candidate lists [kNE][128] x (m32, piece, mask) | barriers | tmem slot
+struct Smem {
+  uint8_t* ring1; uint8_t* sRho; uint8_t* ringC;
+  float* sHn; float* eM; int* eP; uint32_t* eMask;
+  uint64_t* s1_full; uint64_t* s1_empty; uint64_t* z_full;
+  uint64_t* c_full; uint64_t* c_empty; uint64_t* acc_full; uint64_t* acc_empty; uint64_t* rho_ready;
+  uint32_t* tmem_slot;
+};
+
+__host__ __device__ inline size_t rvq_regionR(const RvqParams& p) {
+  const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes;
+  const size_t lvl = (size_t)(p.r / 64 + p.ring_tiles) * kTileBytes;
+  return ring1 > lvl ? ring1 : lvl;
 }
+__host__ __device__ inline size_t rvq_tail_bytes(const RvqParams& p) {
+  return (size_t)p.K * 4 + (size_t)kNE * 128 * 12 + 1024;
+}
+
+__device__ __forceinline__ Smem carve_smem(uint8_t* base, const RvqParams& p) {
+  Smem s;
+  s.ring1 = base;
+  s.sRho = base;
+  s.ringC = base + (size_t)(p.r / 64) * kTileBytes;
+  uint8_t* t = base + rvq_regionR(p);
+  s.sHn = reinterpret_cast<float*>(t); t += (size_t)p.K * 4;
+  s.eM = reinterpret_cast<float*>(t); t += kNE * 128 * 4;
+  s.eP = reinterpret_cast<int*>(t); t += kNE * 128 * 4;
+  s.eMask = reinterpret_cast<uint32_t*>(t); t += kNE * 128 * 4;
+  uint64_t* b = reinterpret_cast<uint64_t*>(t);
+  s.s1_full = b; b += p.stages1;
+  s.s1_empty = b; b += p.stages1;
+  s.z_full = b; b += 1;
+  s.c_full = b; b += p.ring_tiles;
+  s.c_empty = b; b += p.ring_tiles;
+  s.acc_full = b; b += 2;
+  s.acc_empty = b; b += 2;
+  s.rho_ready = b; b += 1;
+  s.tmem_slot = reinterpret_cast<uint32_t*>(b);
+  return s;
+}
+
+// exact fp32 score of codeword row `crow` against this thread's residual (TMEM columns [0,r)):
+// 0.5||c||^2 - rho.c.  Warp-convergent (tcgen05.ld is .sync.aligned); lanes without work pass any
+// valid row and ignore the result.
+__device__ __forceinline__ float exact_score(uint32_t tmem_row, const float* __restrict__ crow, float hn, int r) {
+  float dot = 0.f;
+  for (int pc = 0; pc < r / 32; ++pc) {
+    uint32_t v[32];
+    tmem_ld32(tmem_row + pc * 32, v);
+    const float4* c4 = reinterpret_cast<const float4*>(crow + pc * 32);
+    float4 c[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) c[i] = __ldg(c4 + i);
+    tmem_ld_wait();
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      dot = fmaf(__uint_as_float(v[4 * i + 0]), c[i].x, dot);
+      dot = fmaf(__uint_as_float(v[4 * i + 1]), c[i].y, dot);
+      dot = fmaf(__uint_as_float(v[4 * i + 2]), c[i].z, dot);
+      dot = fmaf(__uint_as_float(v[4 * i + 3]), c[i].w, dot);
+    }
+  }
+  return hn - dot;
+}
+
+// rho <- rho - sub (sub == nullptr: rho unchanged); returns ||rho||^2; writes bf16(rho) into the
+// swizzled A-operand tiles.  Warp-convergent.
+__device__ __forceinline__ float update_rho(uint32_t tmem_row, const float* __restrict__ sub, uint8_t* sRho, int row, int r) {
+  float n2 = 0.f;
+  for (int pc = 0; pc < r / 32; ++pc) {
+    uint32_t v[32];
+    tmem_ld32(tmem_row + pc * 32, v);
+    tmem_ld_wait();
+    if (sub != nullptr) {
+      const float4* c4 = reinterpret_cast<const float4*>(sub + pc * 32);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const float4 c = __ldg(c4 + i);
+        v[4 * i + 0] = __float_as_uint(__uint_as_float(v[4 * i + 0]) - c.x);
+        v[4 * i + 1] = __float_as_uint(__uint_as_float(v[4 * i + 1]) - c.y);
+        v[4 * i + 2] = __float_as_uint(__uint_as_float(v[4 * i + 2]) - c.z);
+        v[4 * i + 3] = __float_as_uint(__uint_as_float(v[4 * i + 3]) - c.w);
+      }
+      tmem_st32(tmem_row + pc * 32, v);
+    }
+    uint8_t* tile = sRho + (size_t)(pc / 2) * kTileBytes;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      uint4 o;
+      o.x = pack_bf16x2(__uint_as_float(v[8 * i + 0]), __uint_as_float(v[8 * i + 1]));
+      o.y = pack_bf16x2(__uint_as_float(v[8 * i + 2]), __uint_as_float(v[8 * i + 3]));
+      o.z = pack_bf16x2(__uint_as_float(v[8 * i + 4]), __uint_as_float(v[8 * i + 5]));
+      o.w = pack_bf16x2(__uint_as_float(v[8 * i + 6]), __uint_as_float(v[8 * i + 7]));
+      *reinterpret_cast<uint4*>(tile + sw128_offset(row, (pc & 1) * 4 + i)) = o;
+    }
+#pragma unroll
+    for (int i = 0; i < 32; ++i) n2 = fmaf(__uint_as_float(v[i]), __uint_as_float(v[i]), n2);
+  }
+  if (sub != nullptr) tmem_st_wait();
+  return n2;
+}
+
+__global__ void __launch_bounds__(kThreads, 1)
+k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmWhi,
+                const __grid_constant__ CUtensorMap tmWlo, const __grid_constant__ CUtensorMap tmC,
+                const RvqParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const Smem s = carve_smem(smem, p);
+
+  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  const long long m0 = (long long)blockIdx.x * p.tile_m;
+  const int nkb1 = p.d / 64, nkb = p.r / 64, nchunks = p.K / kChunk;
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tmH); tma_prefetch_desc(&tmWhi); tma_prefetch_desc(&tmWlo); tma_prefetch_desc(&tmC);
+    for (int i = 0; i < p.stages1; ++i) { mbar_init(&s.s1_full[i], 1); mbar_init(&s.s1_empty[i], 1); }
+    mbar_init(s.z_full, 1);
+    for (int i = 0; i < p.ring_tiles; ++i) { mbar_init(&s.c_full[i], 1); mbar_init(&s.c_empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&s.acc_full[i], 1); mbar_init(&s.acc_empty[i], 4); }
+    mbar_init(s.rho_ready, 4);
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc<512>(s.tmem_slot);
+  tc_fence_before_sync();
+  __syncthreads();
+  tc_fence_after_sync();
+  const uint32_t tmem_base = *s.tmem_slot;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");       // everything below touches global memory
+
+  if (warp == 0) {
+    // ------------------------------------------------------------ TMA producer
+    if (elect_one()) {
+      const uint32_t w_tile = (uint32_t)p.r * 128;
+      for (int kb = 0; kb < nkb1; ++kb) {
+        const int st = kb % p.stages1;
+        mbar_wait(&s.s1_empty[st], ((kb / p.stages1) & 1) ^ 1);
+        mbar_arrive_expect_tx(&s.s1_full[st], (uint32_t)(p.tile_m * 128) + 2 * w_tile);
+        uint8_t* a = s.ring1 + (size_t)st * p.stage1_bytes;
+        tma_load_2d(a, &tmH, &s.s1_full[st], kb * 64, (int)m0, kEvictFirst);
+        tma_load_2d(a + kTileBytes, &tmWhi, &s.s1_full[st], kb * 64, 0, kEvictLast);
+        tma_load_2d(a + kTileBytes + w_tile, &tmWlo, &s.s1_full[st], kb * 64, 0, kEvictLast);
+      }
+      mbar_wait(s.z_full, 0);             // phase-1 MMAs have consumed region R: it may be reused
+      int it = 0;
+      for (int l = 0; l < p.L; ++l)
+        for (int c = 0; c < nchunks; ++c)
+          for (int kb = 0; kb < nkb; ++kb, ++it) {
+            const int st = it % p.ring_tiles;
+            mbar_wait(&s.c_empty[st], ((it / p.ring_tiles) & 1) ^ 1);
+            mbar_arrive_expect_tx(&s.c_full[st], kTileBytes);
+            tma_load_2d(s.ringC + (size_t)st * kTileBytes, &tmC, &s.c_full[st], kb * 64, l * p.K + c * kChunk, kEvictLast);
+          }
+    }
+  } else if (warp == 1) {
+    // ------------------------------------------------------------ MMA issuer
+    if (elect_one()) {
+      const uint32_t idesc1 = make_idesc_bf16(128, (uint32_t)p.r, false, false);
+      for (int kb = 0; kb < nkb1; ++kb) {
+        const int st = kb % p.stages1;
+        mbar_wait(&s.s1_full[st], (kb / p.stages1) & 1);
+        tc_fence_after_sync();
+        const uint32_t a = smem_u32(s.ring1 + (size_t)st * p.stage1_bytes);
+        const uint32_t bh = a + kTileBytes, bl = bh + p.r * 128;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const uint64_t da = desc_kmajor_sw128(a + k * 32);
+          umma_bf16(tmem_base, da, desc_kmajor_sw128(bh + k * 32), idesc1, (kb | k) != 0);
+          umma_bf16(tmem_base, da, desc_kmajor_sw128(bl + k * 32), idesc1, 1);
+        }
+        umma_commit(&s.s1_empty[st]);
+      }
+      umma_commit(s.z_full);
+      const uint32_t idesc2 = make_idesc_bf16(128, kChunk, false, false);
+      int it = 0, cg = 0;
+      for (int l = 0; l < p.L; ++l) {
+        mbar_wait(s.rho_ready, l & 1);    // bf16 residual of level l is in sRho
+        tc_fence_after_sync();
+        for (int c = 0; c < nchunks; ++c, ++cg) {
+          const int as = cg & 1;
+          mbar_wait(&s.acc_empty[as], ((cg >> 1) & 1) ^ 1);
+          tc_fence_after_sync();
+          const uint32_t tmem_d = tmem_base + kAccCol0 + as * kChunk;
+          for (int kb = 0; kb < nkb; ++kb, ++it) {
+            const int st = it % p.ring_tiles;
+            mbar_wait(&s.c_full[st], (it / p.ring_tiles) & 1);
+            tc_fence_after_sync();
+            const uint32_t a = smem_u32(s.sRho + (size_t)kb * kTileBytes), b = smem_u32(s.ringC + (size_t)st * kTileBytes);
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+              umma_bf16(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc2, (kb | k) != 0);
+            umma_commit(&s.c_empty[st]);
+          }
+          umma_commit(&s.acc_full[as]);
+        }
+      }
+    }
+  } else {
+    // ------------------------------------------------------------ epilogue: thread = token
+    const int q = warp & 3, row = q * 32 + lane, et = threadIdx.x - 64;
+    const long long m = m0 + row;
+    const bool live = row < p.tile_m && m < p.N;
+    const uint32_t tmem_row = tmem_base + ((uint32_t)(q * 32) << 16);
+    const unsigned full = 0xffffffffu;
+
+    mbar_wait(s.z_full, 0);
+    tc_fence_after_sync();
+    float n2 = update_rho(tmem_row, nullptr, s.sRho, row, p.r);
+    fence_proxy_async_smem();
+    tc_fence_before_sync();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(s.rho_ready);
+
+    int cg = 0;
+    for (int l = 0; l < p.L; ++l) {
+      const float* Cl = p.C + (long long)l * p.K * p.r;
+      asm volatile("bar.sync 1, 128;" ::: "memory");        // previous level's sHn no longer read
+      for (int i = et; i < p.K / 4; i += 128)
+        reinterpret_cast<float4*>(s.sHn)[i] = __ldg(reinterpret_cast<const float4*>(p.hn + (long long)l * p.K) + i);
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      const float margin = 0.015625f * 1.02f * sqrtf(n2) * __ldg(p.cmax + l);
+
+      float best = FLT_MAX;
+      int cnt = 0;
+      bool overflow = false;
+      for (int c = 0; c < nchunks; ++c, ++cg) {
+        const int as = cg & 1;
+        mbar_wait(&s.acc_full[as], (cg >> 1) & 1);
+        tc_fence_after_sync();
+#pragma unroll 1
+        for (int pc = 0; pc < kChunk / 32; ++pc) {
+          uint32_t v[32];
+          tmem_ld32(tmem_row + kAccCol0 + as * kChunk + pc * 32, v);
+          const float4* h4 = reinterpret_cast<const float4*>(s.sHn + c * kChunk + pc * 32);
+          float sc[32];
+          tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const float4 h = h4[i];
+            sc[4 * i + 0] = h.x - __uint_as_float(v[4 * i + 0]);
+            sc[4 * i + 1] = h.y - __uint_as_float(v[4 * i + 1]);
+            sc[4 * i + 2] = h.z - __uint_as_float(v[4 * i + 2]);
+            sc[4 * i + 3] = h.w - __uint_as_float(v[4 * i + 3]);
+          }
+          float mn[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) mn[i] = fminf(fminf(sc[4 * i], sc[4 * i + 1]), fminf(sc[4 * i + 2], sc[4 * i + 3]));
+          const float m32 = fminf(fminf(fminf(mn[0], mn[1]), fminf(mn[2], mn[3])), fminf(fminf(mn[4], mn[5]), fminf(mn[6], mn[7])));
+          best = fminf(best, m32);
+          const float thr = best + margin;
+          if (__any_sync(full, m32 <= thr)) {
+            uint32_t mask = 0;
+#pragma unroll
+            for (int i = 0; i < 32; ++i) mask |= (sc[i] <= thr) ? (1u << i) : 0u;
+            if (mask != 0 && !overflow) {
+              if (cnt == kNE) {                 // list full: drop entries the tighter threshold excludes
+                int j = 0;
+                for (int e = 0; e < kNE; ++e) {
+                  const float em = s.eM[e * 128 + row];
+                  if (em <= thr) {
+                    s.eM[j * 128 + row] = em; s.eP[j * 128 + row] = s.eP[e * 128 + row];
+                    s.eMask[j * 128 + row] = s.eMask[e * 128 + row]; ++j;
+                  }
+                }
+                cnt = j;
+              }
+              if (cnt == kNE) {
+                overflow = true;                // pathological (e.g. many duplicate codewords): exhaustive below
+              } else {
+                s.eM[cnt * 128 + row] = m32; s.eP[cnt * 128 + row] = c * (kChunk / 32) + pc;
+                s.eMask[cnt * 128 + row] = mask; ++cnt;
+              }
+            }
+          }
+        }
+        tc_fence_before_sync();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&s.acc_empty[as]);
+      }
+
+      // ---- exact fp32 re-scoring of the candidates, ascending k, strict '<': lowest index wins ties
+      const float thr = best + margin;
+      float bestx = FLT_MAX;
+      int bestk = 0, e = 0, piece = 0;
+      uint32_t mrem = 0;
+      while (true) {
+        while (mrem == 0 && e < cnt) {
+          if (s.eM[e * 128 + row] <= thr) { mrem = s.eMask[e * 128 + row]; piece = s.eP[e * 128 + row]; }
+          ++e;
+        }
+        const bool have = mrem != 0 && !overflow;
+        if (!__any_sync(full, have)) break;
+        int k = 0;
+        if (have) { k = piece * 32 + __ffs(mrem) - 1; mrem &= mrem - 1; }
+        const float sx = exact_score(tmem_row, Cl + (long long)k * p.r, s.sHn[k], p.r);
+        if (have && sx < bestx) { bestx = sx; bestk = k; }
+      }
+      if (__any_sync(full, overflow)) {
+        for (int k = 0; k < p.K; ++k) {
+          const float sx = exact_score(tmem_row, Cl + (long long)k * p.r, s.sHn[k], p.r);
+          if (overflow && sx < bestx) { bestx = sx; bestk = k; }
+        }
+      }
+      if (live) p.codes[m * p.L + l] = bestk;
+      if (l + 1 < p.L) {
+        n2 = update_rho(tmem_row, Cl + (long long)bestk * p.r, s.sRho, row, p.r);
+        fence_proxy_async_smem();
+        tc_fence_before_sync();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(s.rho_ready);
+      }
+    }
+
+    if (p.Zq != nullptr && live) {                          // zhat = sum_l C[l, code_l, :], rounded once
+      for (int cc = 0; cc < p.r / 8; ++cc) {
+        float a[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        for (int l = 0; l < p.L; ++l) {
+          const float4* src = reinterpret_cast<const float4*>(p.C + ((long long)l * p.K + p.codes[m * p.L + l]) * p.r + cc * 8);
+          const float4 x = __ldg(src), y = __ldg(src + 1);
+          a[0] += x.x; a[1] += x.y; a[2] += x.z; a[3] += x.w; a[4] += y.x; a[5] += y.y; a[6] += y.z; a[7] += y.w;
+        }
+        *reinterpret_cast<uint4*>(p.Zq + m * p.r + cc * 8) =
+            make_uint4(pack_bf16x2(a[0], a[1]), pack_bf16x2(a[2], a[3]), pack_bf16x2(a[4], a[5]), pack_bf16x2(a[6], a[7]));
+      }
+    }
+  }
+  tc_fence_before_sync();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after_sync();
+    tmem_dealloc<512>(tmem_base);
+  }
+}
+
+}  // namespace
+
+int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
+                  int32_t* codes_out, cudaStream_t st) {
+  if (!tc_rvq_ok(d) || !pk.WBlo || !pk.Cb) return MAPL_ERR_UNSUPPORTED;
+  RvqParams p;
+  p.C = codebooks; p.hn = pk.hn; p.cmax = pk.cmax;
+  p.Zq = reinterpret_cast<__nv_bfloat16*>(Zq_out); p.codes = codes_out;
+  p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.L = d.rvq_levels; p.K = d.rvq_k;
+  p.tile_m = tc_tile_m(d.n_tokens);
+  p.stage1_bytes = kTileBytes + 2 * d.r * 128;
+  p.stages1 = 2; p.ring_tiles = 2;
+  const size_t avail = (size_t)227 * 1024 - 1024 - rvq_tail_bytes(p);
+  if (avail < (size_t)2 * p.stage1_bytes || avail < (size_t)(d.r / 64 + 2) * kTileBytes) return MAPL_ERR_UNSUPPORTED;
+  p.stages1 = (int)(avail / p.stage1_bytes);
+  if (p.stages1 > 8) p.stages1 = 8;
+  if (p.stages1 > d.d / 64) p.stages1 = d.d / 64;
+  p.ring_tiles = (int)(avail / kTileBytes) - d.r / 64;
+  if (p.ring_tiles > 12) p.ring_tiles = 12;
+  if (p.stages1 < 2 || p.ring_tiles < 2) return MAPL_ERR_UNSUPPORTED;
+  const size_t smem = 1024 + rvq_regionR(p) + rvq_tail_bytes(p);
+  CUtensorMap tmH, tmWhi, tmWlo, tmC;
+  const uint64_t dd = (uint64_t)d.d, rr = (uint64_t)d.r;
+  if (!make_tmap_bf16_2d(&tmH, H, (uint64_t)d.n_tokens, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
+  if (!make_tmap_bf16_2d(&tmWhi, pk.WB, rr, dd, dd, 64, (uint32_t)d.r)) return MAPL_ERR_CUDA;
+  if (!make_tmap_bf16_2d(&tmWlo, pk.WBlo, rr, dd, dd, 64, (uint32_t)d.r)) return MAPL_ERR_CUDA;
+  if (!make_tmap_bf16_2d(&tmC, pk.Cb, (uint64_t)d.rvq_levels * d.rvq_k, rr, rr, 64, kChunk)) return MAPL_ERR_CUDA;
+  static bool attr_done = false;
+  if (!attr_done) {
+    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_encode_rvq, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    attr_done = true;
+  }
+  const unsigned tiles = (unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m);
+  KernelScope ks(KID_TC_ENCODE_RVQ, st);
+  MAPL_CUDA_CHECK(launch_pdl(k_tc_encode_rvq, dim3(tiles), dim3(kThreads), smem, st, tmH, tmWhi, tmWlo, tmC, p));
+  return MAPL_OK;
+}
+
 }  // namespace mapl

@@ -120,3 +120,45 @@ def test_c1_full_size_one_boundary():
     bi = I.make_boundary(I.CONFIGS["c1"], 0)
     gpu, ora, stats, errs = _roundtrip(bi, want_dB=False)
     print("c1 full", errs)
+
+
+# ---------------------------------------------------------------- fused tcgen05 projection + RVQ kernel
+
+def _with_codebook(bi, C64):
+    return dataclasses.replace(bi, C=I.store(C64, "f32"))
+
+
+def test_tc_rvq_duplicate_codewords_take_the_lowest_index():
+    """Tensor-core envelope (bf16, d=256, r=64, K=256).  Level 0: every codeword identical (each k is
+    a candidate: the exhaustive fp32 fallback must return index 0).  Level 1: the codebook holds each
+    codeword twice (k and k+128): the lower copy must win (S4)."""
+    bi = I.make_generic(21, 300, 256, 64, 2, 256, 100, 0, "bf16")
+    C = bi.C.f64.copy()
+    C[0, :, :] = C[0, 0, :]
+    C[1, 128:, :] = C[1, :128, :]
+    bi = _with_codebook(bi, C)
+    gpu = run_gpu(bi)
+    assert (gpu["codes"][:, 0] == 0).all()
+    assert (gpu["codes"][:, 1] < 128).all()
+    ora, stats = run_oracle(bi, gpu_codes=gpu["codes"])
+    compare(gpu, ora, stats, TOL["bf16"])
+
+
+def test_tc_rvq_planted_codewords_are_recovered():
+    """z = C0[k0] + C1[k1] exactly representable on the span of U: codes = (k0, k1), no near ties."""
+    bi = I.make_generic(22, 256, 256, 64, 2, 128, 50, 0, "bf16", cb_std=(4.0, 0.25))
+    rng = np.random.default_rng(5)
+    k0, k1 = rng.integers(0, 128, 256), rng.integers(0, 128, 256)
+    Z = bi.C.f64[0][k0] + bi.C.f64[1][k1]
+    H = I.store(Z @ bi.U.f64.T, "bf16")           # bf16 rounding of H perturbs z by ~2^-9 relative
+    bi = dataclasses.replace(bi, H=H)
+    gpu = run_gpu(bi)
+    assert np.array_equal(gpu["codes"][:, 0], k0)
+    assert np.array_equal(gpu["codes"][:, 1], k1)
+
+
+@pytest.mark.parametrize("r,K,L", [(64, 128, 1), (128, 512, 3), (256, 1024, 2), (64, 4096, 2)])
+def test_tc_rvq_envelope_shapes(r, K, L):
+    bi = I.make_generic(23 + r % 7, 200 + r, 512, r, L, K, 300, 64, "bf16")
+    gpu, ora, stats, errs = _roundtrip(bi)
+    assert stats["forced"] <= stats["excepted"]
