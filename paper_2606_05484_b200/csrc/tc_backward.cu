@@ -11,9 +11,9 @@
 //               MN-major (tokens are the contraction index): TMA boxes [64 tokens x 64 cols]
 //               are used as they land.  Split over token ranges; fp32 vector atomics into dU.
 //               While the MMAs run, the epilogue warps scatter-add the gA rows into dA[tok]:
-//               per 128-token block the rows of equal token id are first summed in shared memory
-//               (Zipf ids: the hottest id owns ~14 % of all rows), then one red.global.add.v4 row
-//               per distinct id leaves the CTA.
+//               per 128-token block the ids are ranked in shared memory and rows of equal id are
+//               summed in registers (Zipf ids: the hottest id owns ~14 % of all rows), then one
+//               red.global.add row per distinct id leaves the CTA.
 // Roofline: HBM at configs 1-2 (g, H read; dH written), tensor at config 3.
 #include "profile.cuh"
 #include "tc_codec.cuh"
@@ -202,29 +202,43 @@ struct BwdDuParams {
 };
 
 // dA[tok_n, :] += gA[n, :] for the 128-token blocks this CTA owns; called by the 128 epilogue threads.
+// Per block: the token ids are ranked (counting sort, 128 broadcast reads per thread), then every
+// thread owns one column and walks a run of the sorted order, summing rows of equal id in a
+// register and issuing one red.global.add per (distinct id, column): no shared-memory atomics, and a
+// hot Zipf id costs one global row per block instead of one per occurrence.
 __device__ __forceinline__ void scatter_gA(const BwdDuParams& p, float* sG, int* sTok, int cta, int n_ctas) {
   const int et = threadIdx.x - 64, pitch = p.ra + 4, vpr = p.ra / 4;
+  int* sSorted = sTok + 128;      // token id at each sorted position
+  int* sOrder = sTok + 256;       // source row of each sorted position
+  const int col = et % p.ra, nseg = 128 / p.ra, seg = et / p.ra, seglen = 128 / nseg;
   for (long long base = (long long)cta * 128; base < p.N; base += (long long)n_ctas * 128) {
     const int cnt = (int)(p.N - base < 128 ? p.N - base : 128);
     const float4* src = reinterpret_cast<const float4*>(p.gA + base * p.ra);
     for (int i = et; i < cnt * vpr; i += 128)
       *reinterpret_cast<float4*>(sG + (i / vpr) * pitch + (i % vpr) * 4) = __ldg(src + i);
-    const int my = et < cnt ? __ldg(p.tok + base + et) : -1 - et;
+    const int my = et < cnt ? __ldg(p.tok + base + et) : 0x7fffffff;
     sTok[et] = my;
     asm volatile("bar.sync 1, 128;" ::: "memory");
-    int leader = et;
-    for (int j = 0; j < et; ++j)
-      if (sTok[j] == my) { leader = j; break; }
-    if (et < cnt && leader != et) {
-      const float* mine = sG + et * pitch;
-      float* dst = sG + leader * pitch;
-      for (int c = 0; c < p.ra; ++c) atomicAdd(dst + c, mine[c]);
+    int rank = 0;
+#pragma unroll 8
+    for (int j = 0; j < 128; ++j) {
+      const int t = sTok[j];
+      rank += (t < my || (t == my && j < et)) ? 1 : 0;
     }
+    sSorted[rank] = my;
+    sOrder[rank] = et;
     asm volatile("bar.sync 1, 128;" ::: "memory");
-    if (et < cnt && leader == et) {
-      const float4* mine = reinterpret_cast<const float4*>(sG + et * pitch);
-      float* dst = p.dA + (long long)my * p.ra;
-      for (int c = 0; c < vpr; ++c) { const float4 v = mine[c]; red_add_v4(dst + c * 4, v.x, v.y, v.z, v.w); }
+    float acc = 0.f;
+    const int p0 = seg * seglen, p1 = p0 + seglen;
+    int cur = sSorted[p0];
+    for (int pos = p0; pos < p1; ++pos) {
+      const int nxt = pos + 1 < p1 ? sSorted[pos + 1] : -1;
+      acc += sG[sOrder[pos] * pitch + col];
+      if (nxt != cur) {
+        if (cur != 0x7fffffff) atomicAdd(p.dA + (long long)cur * p.ra + col, acc);   // result unused: RED
+        acc = 0.f;
+        cur = nxt;
+      }
     }
     asm volatile("bar.sync 1, 128;" ::: "memory");
   }
@@ -240,7 +254,7 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   uint64_t* acc_full = empty + p.stages;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_full + 1);
   float* sG = reinterpret_cast<float*>(smem + (size_t)p.stages * p.item_bytes + 512);   // [128][ra+4]
-  int* sTok = reinterpret_cast<int*>(sG + 128 * (p.ra + 4));
+  int* sTok = reinterpret_cast<int*>(sG + 128 * (p.ra + 4));                           // 3 x [128]
 
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
   const int dt = blockIdx.x;                                   // 128 rows of dU
@@ -407,7 +421,7 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     p.dU = dU_out; p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.n_src = H ? 2 : 1;
     p.tok = ra ? tok : nullptr; p.gA = gA_ws; p.dA = dA_out; p.ra = ra;
     p.item_bytes = 2 * 64 * 128 + (d.r / 64) * 64 * 128;
-    const size_t scatter_bytes = ra ? (size_t)128 * (ra + 4) * 4 + 512 : 0;
+    const size_t scatter_bytes = ra ? (size_t)128 * (ra + 4) * 4 + 3 * 512 : 0;
     p.stages = (int)((227 * 1024 - 2048 - scatter_bytes) / p.item_bytes);
     if (p.stages > 8) p.stages = 8;
     if (p.stages < 2) return MAPL_ERR_UNSUPPORTED;
