@@ -2,6 +2,8 @@
 // (tc_encode.cu, tc_encode_rvq.cu, tc_decode.cu, tc_backward.cu).
 #include "tc_codec.cuh"
 
+#include <cuda_fp16.h>
+
 #include "profile.cuh"
 
 namespace mapl {
@@ -32,7 +34,9 @@ TcPack tc_pack_layout(const mapl_boundary_desc& d, char* base) {
     p.WBlo = reinterpret_cast<__nv_bfloat16*>(seg((size_t)d.r * d.d * 2));
     p.Cb = reinterpret_cast<__nv_bfloat16*>(seg(LK * d.r * 2));
     p.hn = reinterpret_cast<float*>(seg(LK * 4));
+    p.rowamax = reinterpret_cast<float*>(seg(LK * 4));
     p.cmax = reinterpret_cast<float*>(seg(8 * 4));
+    p.cscale = reinterpret_cast<float*>(seg(2 * 8 * 4));
   }
   p.bytes = off;
   return p;
@@ -59,13 +63,19 @@ struct PackJob {
   const float* src; int rows, cols;        // src is [rows, cols] fp32 row-major
   __nv_bfloat16* dst; long long pitch;     // dst element (i,j) -> dst[i*pitch + j] (after optional transpose)
   int transpose;
-  int lo;                                  // 1: store bf16(x - float(bf16(x))), the second split term
+  int mode;                                // 0: bf16(x)   1: bf16(x - float(bf16(x))), the second split term
+                                           // 2: fp16(x * scale[src_row / rows_per_scale])  (16-bit store)
+  const float* scale; int rows_per_scale;
 };
 struct PackArgs { PackJob job[6]; int njobs; };
 
-__device__ __forceinline__ __nv_bfloat16 pack_term(float x, int lo) {
+__device__ __forceinline__ __nv_bfloat16 pack_term(float x, int mode, float sc) {
+  if (mode == 2) {
+    const unsigned short h = __half_as_ushort(__float2half_rn(x * sc));
+    return *reinterpret_cast<const __nv_bfloat16*>(&h);
+  }
   const __nv_bfloat16 hi = __float2bfloat16_rn(x);
-  return lo ? __float2bfloat16_rn(x - __bfloat162float(hi)) : hi;
+  return mode == 1 ? __float2bfloat16_rn(x - __bfloat162float(hi)) : hi;
 }
 
 // 32x32 tiles; blockIdx.y = job
@@ -78,36 +88,59 @@ __global__ void __launch_bounds__(256) k_tc_pack(const PackArgs a) {
     const int tx = threadIdx.x % 32, ty = threadIdx.x / 32;
     for (int i = ty; i < 32; i += 8) {
       const int r = r0 + i, c = c0 + tx;
-      tile[i][tx] = (r < j.rows && c < j.cols) ? j.src[(long long)r * j.cols + c] : 0.f;
+      float x = (r < j.rows && c < j.cols) ? j.src[(long long)r * j.cols + c] : 0.f;
+      tile[i][tx] = x;
     }
     __syncthreads();
     if (j.transpose) {
       for (int i = ty; i < 32; i += 8) {
         const int c = c0 + i, r = r0 + tx;           // dst row = src col
-        if (c < j.cols && r < j.rows) j.dst[(long long)c * j.pitch + r] = pack_term(tile[tx][i], j.lo);
+        if (c < j.cols && r < j.rows) j.dst[(long long)c * j.pitch + r] = pack_term(tile[tx][i], j.mode, 1.f);
       }
     } else {
       for (int i = ty; i < 32; i += 8) {
         const int r = r0 + i, c = c0 + tx;
-        if (r < j.rows && c < j.cols) j.dst[(long long)r * j.pitch + c] = pack_term(tile[i][tx], j.lo);
+        const float sc = (j.mode == 2 && r < j.rows) ? j.scale[r / j.rows_per_scale] : 1.f;
+        if (r < j.rows && c < j.cols) j.dst[(long long)r * j.pitch + c] = pack_term(tile[i][tx], j.mode, sc);
       }
     }
     __syncthreads();
   }
 }
 
-// one block per level: cmax[l] = max_k sqrt(2 hn[l,k])
-__global__ void __launch_bounds__(256) k_tc_cmax(const float* __restrict__ hn, float* __restrict__ cmax, int K) {
-  __shared__ float red[8];
-  float m = 0.f;
-  for (int k = threadIdx.x; k < K; k += 256) m = fmaxf(m, hn[(long long)blockIdx.x * K + k]);
+// one warp per codeword row: hn = 0.5 ||c||^2, rowamax = max_j |c_j|
+__global__ void __launch_bounds__(256) k_tc_cb_stats(const float* __restrict__ C, float* __restrict__ hn,
+                                                     float* __restrict__ rowamax, int rows, int r) {
+  const int row = (blockIdx.x * blockDim.x + threadIdx.x) / 32, lane = threadIdx.x % 32;
+  if (row >= rows) return;
+  float s = 0.f, m = 0.f;
+  for (int j = lane; j < r; j += 32) { const float c = C[(long long)row * r + j]; s = fmaf(c, c, s); m = fmaxf(m, fabsf(c)); }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-  if (threadIdx.x % 32 == 0) red[threadIdx.x / 32] = m;
+  for (int o = 16; o > 0; o >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, o); m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o)); }
+  if (lane == 0) { hn[row] = 0.5f * s; rowamax[row] = m; }
+}
+
+// one block per level: cmax[l] = max_k ||c_k||;  cscale[l] = 2^-e with max|c| * 2^-e in [0.5, 1),
+// cscale[8 + l] = 2^e  (the fp16 codebook copy is C * cscale[l]; powers of two, so exact)
+__global__ void __launch_bounds__(256) k_tc_cmax(const float* __restrict__ hn, const float* __restrict__ rowamax,
+                                                 float* __restrict__ cmax, float* __restrict__ cscale, int K) {
+  __shared__ float red[8], red2[8];
+  float m = 0.f, a = 0.f;
+  for (int k = threadIdx.x; k < K; k += 256) {
+    m = fmaxf(m, hn[(long long)blockIdx.x * K + k]);
+    a = fmaxf(a, rowamax[(long long)blockIdx.x * K + k]);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o)); a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, o)); }
+  if (threadIdx.x % 32 == 0) { red[threadIdx.x / 32] = m; red2[threadIdx.x / 32] = a; }
   __syncthreads();
   if (threadIdx.x == 0) {
-    for (int i = 1; i < 8; ++i) m = fmaxf(m, red[i]);
+    for (int i = 1; i < 8; ++i) { m = fmaxf(m, red[i]); a = fmaxf(a, red2[i]); }
     cmax[blockIdx.x] = sqrtf(2.f * m);
+    int eb = (int)((__float_as_uint(a) >> 23) & 0xffu);
+    eb = eb < 2 ? 126 : (eb > 250 ? 250 : eb);             // all-zero / denormal codebook: scale 1
+    cscale[blockIdx.x] = __uint_as_float((uint32_t)(253 - eb) << 23);
+    cscale[8 + blockIdx.x] = __uint_as_float((uint32_t)(eb + 1) << 23);
   }
 }
 
@@ -115,28 +148,34 @@ __global__ void __launch_bounds__(256) k_tc_cmax(const float* __restrict__ hn, f
 
 int tc_pack_build(const mapl_boundary_desc& d, const float* U, const float* B, const float* codebooks,
                   const TcPack& p, cudaStream_t st) {
+  const bool rvq = d.rvq_levels > 0 && p.hn && codebooks;
+  if (rvq) {
+    const int rows = d.rvq_levels * d.rvq_k;
+    {
+      KernelScope ks(KID_TC_PACK, st);
+      k_tc_cb_stats<<<(rows + 7) / 8, 256, 0, st>>>(codebooks, p.hn, p.rowamax, rows, d.r);
+      MAPL_CUDA_CHECK(cudaGetLastError());
+    }
+    KernelScope ks(KID_TC_PACK, st);
+    k_tc_cmax<<<d.rvq_levels, 256, 0, st>>>(p.hn, p.rowamax, p.cmax, p.cscale, d.rvq_k);
+    MAPL_CUDA_CHECK(cudaGetLastError());
+  }
   PackArgs a;
   a.njobs = 0;
   const int ra = d.anchor_rank;
-  a.job[a.njobs++] = PackJob{U, d.d, d.r, p.WB, d.d, 1, 0};                                        // WB[j][i] = U[i][j]
-  a.job[a.njobs++] = PackJob{U, d.d, d.r, p.Wd, p.kc, 0, 0};                                       // Wd[i][j] = U[i][j]
+  a.job[a.njobs++] = PackJob{U, d.d, d.r, p.WB, d.d, 1, 0, nullptr, 1};                            // WB[j][i] = U[i][j]
+  a.job[a.njobs++] = PackJob{U, d.d, d.r, p.Wd, p.kc, 0, 0, nullptr, 1};                           // Wd[i][j] = U[i][j]
   if (ra && B) {
-    a.job[a.njobs++] = PackJob{B, ra, d.d, p.WB + (long long)d.r * d.d, d.d, 0, 0};
-    a.job[a.njobs++] = PackJob{B, ra, d.d, p.Wd + d.r, p.kc, 1, 0};                                // Wd[i][r+q] = B[q][i]
+    a.job[a.njobs++] = PackJob{B, ra, d.d, p.WB + (long long)d.r * d.d, d.d, 0, 0, nullptr, 1};
+    a.job[a.njobs++] = PackJob{B, ra, d.d, p.Wd + d.r, p.kc, 1, 0, nullptr, 1};                    // Wd[i][r+q] = B[q][i]
   }
   if (d.rvq_levels > 0 && p.WBlo) {
-    a.job[a.njobs++] = PackJob{U, d.d, d.r, p.WBlo, d.d, 1, 1};
-    if (codebooks) a.job[a.njobs++] = PackJob{codebooks, d.rvq_levels * d.rvq_k, d.r, p.Cb, d.r, 0, 0};
+    a.job[a.njobs++] = PackJob{U, d.d, d.r, p.WBlo, d.d, 1, 1, nullptr, 1};
+    if (rvq) a.job[a.njobs++] = PackJob{codebooks, d.rvq_levels * d.rvq_k, d.r, p.Cb, d.r, 0, 2, p.cscale, d.rvq_k};
   }
   {
     KernelScope ks(KID_TC_PACK, st);
     k_tc_pack<<<dim3(148, a.njobs), 256, 0, st>>>(a);
-    MAPL_CUDA_CHECK(cudaGetLastError());
-  }
-  if (d.rvq_levels > 0 && p.hn && codebooks) {
-    MAPL_RETURN_IF(simt_half_sqnorm(codebooks, p.hn, d.rvq_levels * d.rvq_k, d.r, st));
-    KernelScope ks(KID_TC_PACK, st);
-    k_tc_cmax<<<d.rvq_levels, 256, 0, st>>>(p.hn, p.cmax, d.rvq_k);
     MAPL_CUDA_CHECK(cudaGetLastError());
   }
   return MAPL_OK;

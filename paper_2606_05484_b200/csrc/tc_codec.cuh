@@ -9,7 +9,8 @@
 //   WB   [(r+ra), d] = [U^T ; B]    K-major over d     (encode / backward-gz B operand)
 //   Wd   [d, (r+ra)] = [U | B^T]    K-major over r+ra  (decode / backward-dH B operand)
 //   WBlo [r, d]      = (U - bf16(U))^T                 (second split term: fp32-accurate z for RVQ)
-//   Cb   [L*K, r]    bf16 codebooks;  hn [L*K] = 0.5 ||C_k||^2 (fp32);  cmax [L] = max_k ||C_l,k||
+//   Cb   [L*K, r]    fp16 codebooks scaled per level by cscale[l] = 2^-e (max|c| 2^-e in [0.5,1));
+//                    hn [L*K] = 0.5 ||C_k||^2 (fp32);  cmax [L] = max_k ||C_l,k||;  cscale[8+l] = 2^e
 #pragma once
 #include "common.cuh"
 
@@ -24,7 +25,9 @@ struct TcPack {
   __nv_bfloat16* WBlo = nullptr;
   __nv_bfloat16* Cb = nullptr;
   float* hn = nullptr;
+  float* rowamax = nullptr;
   float* cmax = nullptr;
+  float* cscale = nullptr;
   int kc = 0;          // r + ra
   size_t bytes = 0;
 };

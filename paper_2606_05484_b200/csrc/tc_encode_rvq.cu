@@ -6,13 +6,15 @@
 //   phase 1   z = H (U_hi + U_lo)      H tiles by TMA (HBM, evict-first), the two bf16 split terms
 //             of U^T from the L2-resident pack; fp32 accumulator [128 x r] in TMEM columns [0,r).
 //             bf16 H is exact and U_hi + U_lo carries 16 mantissa bits, so z is fp32-accurate.
-//   level l   rho (fp32) stays in TMEM columns [0,r); its bf16 rounding is the resident A operand.
+//   level l   rho (fp32) stays in TMEM columns [0,r); its fp16 rounding, scaled per token by a power
+//             of two so that max|rho_j| lies in [0.5,1), is the resident A operand (the codebook
+//             copy is fp16 too, scaled per level: 11 significant bits instead of bf16's 8).
 //             Codebook tiles [128 codewords x 64] stream through a TMA ring; per 128-codeword
-//             chunk one accumulator stage S = rho_bf16 . C_bf16^T  (2 stages, TMEM cols 256..511).
+//             chunk one accumulator stage S = rho_f16 . C_f16^T  (2 stages, TMEM cols 256..511).
 //             Epilogue (thread = token): coarse score s_k = 0.5||c_k||^2 - S_k, running minimum,
 //             and every k with  s_k <= running min + margin  is recorded as a candidate, where
-//               margin = 2 E,   E = 2^-7 * 1.01 * ||rho|| * max_k ||c_k||  >=  |s_coarse - s_exact|
-//             (bf16 rounding of both operands, Cauchy-Schwarz).  The true minimiser is therefore
+//               margin = 2 E,   E = 2^-10 * 1.05 * ||rho|| * max_k ||c_k||  >=  |s_coarse - s_exact|
+//             (fp16 rounding of both operands, Cauchy-Schwarz).  The true minimiser is therefore
 //             always among the candidates; they are re-scored in exact fp32 (rho from TMEM, the
 //             fp32 codeword from L2), lowest index winning ties (S4).  Then rho -= C[l, k*].
 // Roofline: tensor at config 3 (K r = 1M per level), HBM/ALU at config 2.
@@ -35,6 +37,7 @@ struct RvqParams {
   const float* C;        // [L,K,r] fp32 codebooks (exact re-scoring, residual update)
   const float* hn;       // [L*K] 0.5 ||c||^2
   const float* cmax;     // [L] max_k ||c_k||
+  const float* cscale;   // [8+l] = 2^e_l: the fp16 codebook copy is C * 2^-e_l
   __nv_bfloat16* Zq;     // optional [N,r]
   int32_t* codes;        // [N,L]
   long long N;
@@ -109,10 +112,12 @@ __device__ __forceinline__ float exact_score(uint32_t tmem_row, const float* __r
   return hn - dot;
 }
 
-// rho <- rho - sub (sub == nullptr: rho unchanged); returns ||rho||^2; writes bf16(rho) into the
-// swizzled A-operand tiles.  Warp-convergent.
-__device__ __forceinline__ float update_rho(uint32_t tmem_row, const float* __restrict__ sub, uint8_t* sRho, int row, int r) {
-  float n2 = 0.f;
+// rho <- rho - sub (sub == nullptr: rho unchanged); returns ||rho||^2; writes fp16(rho * 2^-e) into
+// the swizzled A-operand tiles, 2^-e chosen so that max|rho_j| 2^-e lies in [0.5,1); *unscale = 2^e.
+// Warp-convergent.
+__device__ __forceinline__ float update_rho(uint32_t tmem_row, const float* __restrict__ sub, uint8_t* sRho, int row, int r,
+                                            float* unscale) {
+  float n2 = 0.f, amax = 0.f;
   for (int pc = 0; pc < r / 32; ++pc) {
     uint32_t v[32];
     tmem_ld32(tmem_row + pc * 32, v);
@@ -129,20 +134,33 @@ __device__ __forceinline__ float update_rho(uint32_t tmem_row, const float* __re
       }
       tmem_st32(tmem_row + pc * 32, v);
     }
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+      const float x = __uint_as_float(v[i]);
+      n2 = fmaf(x, x, n2);
+      amax = fmaxf(amax, fabsf(x));
+    }
+  }
+  if (sub != nullptr) tmem_st_wait();
+  int eb = (int)((__float_as_uint(amax) >> 23) & 0xffu);
+  eb = eb < 2 ? 126 : (eb > 250 ? 250 : eb);
+  const float inv = __uint_as_float((uint32_t)(253 - eb) << 23);
+  *unscale = __uint_as_float((uint32_t)(eb + 1) << 23);
+  for (int pc = 0; pc < r / 32; ++pc) {
+    uint32_t v[32];
+    tmem_ld32(tmem_row + pc * 32, v);
+    tmem_ld_wait();
     uint8_t* tile = sRho + (size_t)(pc / 2) * kTileBytes;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       uint4 o;
-      o.x = pack_bf16x2(__uint_as_float(v[8 * i + 0]), __uint_as_float(v[8 * i + 1]));
-      o.y = pack_bf16x2(__uint_as_float(v[8 * i + 2]), __uint_as_float(v[8 * i + 3]));
-      o.z = pack_bf16x2(__uint_as_float(v[8 * i + 4]), __uint_as_float(v[8 * i + 5]));
-      o.w = pack_bf16x2(__uint_as_float(v[8 * i + 6]), __uint_as_float(v[8 * i + 7]));
+      o.x = pack_f16x2(__uint_as_float(v[8 * i + 0]) * inv, __uint_as_float(v[8 * i + 1]) * inv);
+      o.y = pack_f16x2(__uint_as_float(v[8 * i + 2]) * inv, __uint_as_float(v[8 * i + 3]) * inv);
+      o.z = pack_f16x2(__uint_as_float(v[8 * i + 4]) * inv, __uint_as_float(v[8 * i + 5]) * inv);
+      o.w = pack_f16x2(__uint_as_float(v[8 * i + 6]) * inv, __uint_as_float(v[8 * i + 7]) * inv);
       *reinterpret_cast<uint4*>(tile + sw128_offset(row, (pc & 1) * 4 + i)) = o;
     }
-#pragma unroll
-    for (int i = 0; i < 32; ++i) n2 = fmaf(__uint_as_float(v[i]), __uint_as_float(v[i]), n2);
   }
-  if (sub != nullptr) tmem_st_wait();
   return n2;
 }
 
@@ -218,7 +236,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         umma_commit(&s.s1_empty[st]);
       }
       umma_commit(s.z_full);
-      const uint32_t idesc2 = make_idesc_bf16(128, kChunk, false, false);
+      const uint32_t idesc2 = make_idesc_f16(128, kChunk);
       int it = 0, cg = 0;
       for (int l = 0; l < p.L; ++l) {
         mbar_wait(s.rho_ready, l & 1);    // bf16 residual of level l is in sRho
@@ -252,7 +270,8 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 
     mbar_wait(s.z_full, 0);
     tc_fence_after_sync();
-    float n2 = update_rho(tmem_row, nullptr, s.sRho, row, p.r);
+    float unscale;
+    float n2 = update_rho(tmem_row, nullptr, s.sRho, row, p.r, &unscale);
     fence_proxy_async_smem();
     tc_fence_before_sync();
     __syncwarp();
@@ -265,7 +284,8 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       for (int i = et; i < p.K / 4; i += 128)
         reinterpret_cast<float4*>(s.sHn)[i] = __ldg(reinterpret_cast<const float4*>(p.hn + (long long)l * p.K) + i);
       asm volatile("bar.sync 1, 128;" ::: "memory");
-      const float margin = 0.015625f * 1.02f * sqrtf(n2) * __ldg(p.cmax + l);
+      const float margin = 0.001953125f * 1.05f * sqrtf(n2) * __ldg(p.cmax + l);
+      const float nsc = -unscale * __ldg(p.cscale + 8 + l);     // coarse S -> rho.c
 
       float best = FLT_MAX;
       int cnt = 0;
@@ -284,10 +304,10 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
             const float4 h = h4[i];
-            sc[4 * i + 0] = h.x - __uint_as_float(v[4 * i + 0]);
-            sc[4 * i + 1] = h.y - __uint_as_float(v[4 * i + 1]);
-            sc[4 * i + 2] = h.z - __uint_as_float(v[4 * i + 2]);
-            sc[4 * i + 3] = h.w - __uint_as_float(v[4 * i + 3]);
+            sc[4 * i + 0] = fmaf(__uint_as_float(v[4 * i + 0]), nsc, h.x);
+            sc[4 * i + 1] = fmaf(__uint_as_float(v[4 * i + 1]), nsc, h.y);
+            sc[4 * i + 2] = fmaf(__uint_as_float(v[4 * i + 2]), nsc, h.z);
+            sc[4 * i + 3] = fmaf(__uint_as_float(v[4 * i + 3]), nsc, h.w);
           }
           float mn[8];
 #pragma unroll
@@ -295,11 +315,11 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
           const float m32 = fminf(fminf(fminf(mn[0], mn[1]), fminf(mn[2], mn[3])), fminf(fminf(mn[4], mn[5]), fminf(mn[6], mn[7])));
           best = fminf(best, m32);
           const float thr = best + margin;
-          if (__any_sync(full, m32 <= thr)) {
+          if (__any_sync(full, live && m32 <= thr)) {      // dead rows hold stale smem: never candidates
             uint32_t mask = 0;
 #pragma unroll
             for (int i = 0; i < 32; ++i) mask |= (sc[i] <= thr) ? (1u << i) : 0u;
-            if (mask != 0 && !overflow) {
+            if (live && mask != 0 && !overflow) {
               if (cnt == kNE) {                 // list full: drop entries the tighter threshold excludes
                 int j = 0;
                 for (int e = 0; e < kNE; ++e) {
@@ -350,7 +370,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       }
       if (live) p.codes[m * p.L + l] = bestk;
       if (l + 1 < p.L) {
-        n2 = update_rho(tmem_row, Cl + (long long)bestk * p.r, s.sRho, row, p.r);
+        n2 = update_rho(tmem_row, Cl + (long long)bestk * p.r, s.sRho, row, p.r, &unscale);
         fence_proxy_async_smem();
         tc_fence_before_sync();
         __syncwarp();
@@ -385,7 +405,7 @@ int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codeb
                   int32_t* codes_out, cudaStream_t st) {
   if (!tc_rvq_ok(d) || !pk.WBlo || !pk.Cb) return MAPL_ERR_UNSUPPORTED;
   RvqParams p;
-  p.C = codebooks; p.hn = pk.hn; p.cmax = pk.cmax;
+  p.C = codebooks; p.hn = pk.hn; p.cmax = pk.cmax; p.cscale = pk.cscale;
   p.Zq = reinterpret_cast<__nv_bfloat16*>(Zq_out); p.codes = codes_out;
   p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.L = d.rvq_levels; p.K = d.rvq_k;
   p.tile_m = tc_tile_m(d.n_tokens);

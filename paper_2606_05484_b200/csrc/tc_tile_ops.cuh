@@ -6,6 +6,8 @@
 //   Out   bf16, through swizzled staging boxes and TMA stores
 // Three roles, each called by the warp(s) that own it.
 #pragma once
+#include <stdlib.h>
+
 #include "tc_common.cuh"
 
 namespace mapl {
@@ -114,9 +116,10 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
                               Args&&... args) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  static const bool pdl = getenv("MAPL_NO_PDL") == nullptr;     // debugging aid: plain stream order
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
   cfg.attrs = attr; cfg.numAttrs = 1;
   return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
 }
