@@ -1,6 +1,7 @@
 // tc_backward.cu -- mapl_codec_backward on the tensor cores (STE = S7).
 //
-// k_tc_bwd_gz   one CTA per token tile, two phases over one read of g:
+// k_tc_bwd_gz   one CTA per token tile, CTAs in pairs (cta_group::2, M = 256: every parameter byte is
+//               read from L2 once per pair); two phases over one read of g:
 //     phase 1   [gz | gA] = g . [U | B^T]         K = d, streamed through a TMA ring
 //               epilogue: gz -> bf16 -> gz_out (the backward wire payload) and -> smem as the A
 //               operand of phase 2; gA rows -> fp32 scratch [N,ra]
@@ -49,17 +50,18 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   const int kc = p.r + p.ra, nkb1 = p.d / 64;
   // region R: phase 1 ring  |aliased with|  phase 2 gz operand + W ring
   const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes;
-  const size_t ring2 = (size_t)(p.r / 64 + p.b_stages) * kTileBytes;
+  const size_t ring2 = (size_t)(p.r / 64) * kTileBytes + (size_t)p.b_stages * kHalfTileBytes;
   const size_t regionR = ring1 > ring2 ? ring1 : ring2;
   ChunkPipe c;
-  c.nkb = p.r / 64; c.nchunks = p.d / kChunkN; c.b_stages = p.b_stages;
+  c.nkb = p.r / 64; c.nchunks = p.d / kChunkN; c.b_stages = p.b_stages; c.acc_stages = 4;
+  c.rank = cluster_ctarank();
   c.sA = smem;
   c.sB = smem + (size_t)(p.r / 64) * kTileBytes;
   c.sOut = smem + regionR;
   uint64_t* bars = reinterpret_cast<uint64_t*>(c.sOut + (size_t)kOutBufs * kTileBytes);
   c.b_full = bars; c.b_empty = c.b_full + p.b_stages;
-  c.acc_full = c.b_empty + p.b_stages; c.acc_empty = c.acc_full + kAccStages;
-  uint64_t* s1_full = c.acc_empty + kAccStages;
+  c.acc_full = c.b_empty + p.b_stages; c.acc_empty = c.acc_full + 4;
+  uint64_t* s1_full = c.acc_empty + 4;
   uint64_t* s1_empty = s1_full + p.stages1;
   uint64_t* acc1_full = s1_empty + p.stages1;
   uint64_t* gz_full = acc1_full + 1;
@@ -74,12 +76,12 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
     chunk_init_barriers(c);
     for (int s = 0; s < p.stages1; ++s) { mbar_init(&s1_full[s], 1); mbar_init(&s1_empty[s], 1); }
     mbar_init(acc1_full, 1);
-    mbar_init(gz_full, 4);
+    mbar_init(gz_full, 8);                    // leader's: the epilogue warps of both CTAs
     fence_barrier_init();
   }
-  if (warp == 1) tmem_alloc<512>(tmem_slot);
+  if (warp == 1) tmem_alloc_pair<512>(tmem_slot);
   tc_fence_before_sync();
-  __syncthreads();
+  cluster_sync_all();
   tc_fence_after_sync();
   c.tmem_base = *tmem_slot;
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -87,15 +89,15 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
 
   if (warp == 0) {
     if (elect_one()) {
-      const uint32_t bytes = (uint32_t)(p.tile_m * 128 + kc * 128);
+      const uint32_t bytes = (uint32_t)(p.tile_m * 128 + kc * 64);   // per CTA: g tile + half of the [U^T;B] rows
       for (int kb = 0; kb < nkb1; ++kb) {
         const int s = kb % p.stages1;
         mbar_wait(&s1_empty[s], ((kb / p.stages1) & 1) ^ 1);
-        mbar_arrive_expect_tx(&s1_full[s], bytes);
+        if (c.rank == 0) mbar_arrive_expect_tx(&s1_full[s], 2 * bytes);
         uint8_t* a = smem + (size_t)s * p.stage1_bytes;
-        tma_load_2d(a, &tmG, &s1_full[s], kb * 64, (int)m0, kEvictLast);   // g is read again by k_tc_bwd_du
-        tma_load_2d(a + kTileBytes, &tmWu, &s1_full[s], kb * 64, 0, kEvictLast);
-        if (p.ra) tma_load_2d(a + kTileBytes + p.r * 128, &tmWb, &s1_full[s], kb * 64, p.r, kEvictLast);
+        tma_load_2d_pair(a, &tmG, &s1_full[s], kb * 64, (int)m0, kEvictLast);   // g is read again by k_tc_bwd_du
+        tma_load_2d_pair(a + kTileBytes, &tmWu, &s1_full[s], kb * 64, (int)c.rank * (p.r / 2), kEvictLast);
+        if (p.ra) tma_load_2d_pair(a + kTileBytes + p.r * 64, &tmWb, &s1_full[s], kb * 64, p.r + (int)c.rank * (p.ra / 2), kEvictLast);
       }
       if (p.do_dh) {
         mbar_wait(acc1_full, 0);        // phase 1 MMAs have consumed the ring: region R may be reused
@@ -103,26 +105,26 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
       }
     }
   } else if (warp == 1) {
-    if (elect_one()) {
-      const uint32_t idesc_u = make_idesc_bf16(128, (uint32_t)p.r, false, false);
-      const uint32_t idesc_b = make_idesc_bf16(128, (uint32_t)(p.ra ? p.ra : 64), false, false);
+    if (c.rank == 0 && elect_one()) {
+      const uint32_t idesc_u = make_idesc_bf16(256, (uint32_t)p.r, false, false);
+      const uint32_t idesc_b = make_idesc_bf16(256, (uint32_t)(p.ra ? p.ra : 64), false, false);
       for (int kb = 0; kb < nkb1; ++kb) {
         const int s = kb % p.stages1;
         mbar_wait(&s1_full[s], (kb / p.stages1) & 1);
         tc_fence_after_sync();
         const uint32_t a = smem_u32(smem + (size_t)s * p.stage1_bytes);
-        const uint32_t bu = a + kTileBytes, bb = bu + p.r * 128;
+        const uint32_t bu = a + kTileBytes, bb = bu + p.r * 64;
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           const uint64_t da = desc_kmajor_sw128(a + k * 32);
-          umma_bf16(c.tmem_base, da, desc_kmajor_sw128(bu + k * 32), idesc_u, (kb | k) != 0);
-          if (p.ra) umma_bf16(c.tmem_base + p.r, da, desc_kmajor_sw128(bb + k * 32), idesc_b, (kb | k) != 0);
+          umma_bf16_pair(c.tmem_base, da, desc_kmajor_sw128(bu + k * 32), idesc_u, (kb | k) != 0);
+          if (p.ra) umma_bf16_pair(c.tmem_base + p.r, da, desc_kmajor_sw128(bb + k * 32), idesc_b, (kb | k) != 0);
         }
-        umma_commit(&s1_empty[s]);
+        umma_commit_pair(&s1_empty[s]);
       }
-      umma_commit(acc1_full);
+      umma_commit_pair(acc1_full);
       if (p.do_dh) {
-        mbar_wait(gz_full, 0);          // gz operand written and the phase 1 accumulator drained
+        mbar_wait_cluster(gz_full, 0);          // gz operand written and the phase 1 accumulator drained
         tc_fence_after_sync();
         chunk_mma(c);
       }
@@ -178,17 +180,17 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
     }
     if (p.do_dh) {
       tc_fence_before_sync();
-      fence_proxy_async_smem();
+      fence_proxy_async_all();
       __syncwarp();
-      if (lane == 0) mbar_arrive(gz_full);
+      if (lane == 0) mbar_arrive_leader(gz_full);
       chunk_epilogue(c, &tmO, (int)m0);
     }
   }
   tc_fence_before_sync();
-  __syncthreads();
+  cluster_sync_all();
   if (warp == 1) {
     tc_fence_after_sync();
-    tmem_dealloc<512>(c.tmem_base);
+    tmem_dealloc_pair<512>(c.tmem_base);
   }
 }
 
@@ -394,27 +396,28 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     }
     p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.ra = ra; p.tile_m = tc_tile_m(d.n_tokens);
     p.do_dh = dH_out ? 1 : 0;
-    p.stage1_bytes = kTileBytes + kc * 128;
+    p.stage1_bytes = kTileBytes + kc * 64;
     const size_t budget = 227 * 1024 - (size_t)kOutBufs * kTileBytes - 1024 - 1024;   // region R
     p.stages1 = (int)(budget / p.stage1_bytes);
     if (p.stages1 > 8) p.stages1 = 8;
     if (p.stages1 > d.d / 64) p.stages1 = d.d / 64;
     if (p.stages1 < 2) return MAPL_ERR_UNSUPPORTED;
-    p.b_stages = (int)(budget / kTileBytes) - d.r / 64;
+    p.b_stages = (int)((budget - (size_t)(d.r / 64) * kTileBytes) / kHalfTileBytes);
     if (p.b_stages > 8) p.b_stages = 8;
     if (p.b_stages < 2) return MAPL_ERR_UNSUPPORTED;
-    const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes, ring2 = (size_t)(d.r / 64 + p.b_stages) * kTileBytes;
+    const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes,
+                 ring2 = (size_t)(d.r / 64) * kTileBytes + (size_t)p.b_stages * kHalfTileBytes;
     const size_t smem = (ring1 > ring2 ? ring1 : ring2) + (size_t)kOutBufs * kTileBytes + 1024 + 1024;
     CUtensorMap tmG, tmWu, tmWb, tmWd, tmO;
     if (!make_tmap_bf16_2d(&tmG, g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
-    if (!make_tmap_bf16_2d(&tmWu, pk.WB, (uint64_t)pk.kc, dd, dd, 64, (uint32_t)d.r)) return MAPL_ERR_CUDA;
-    if (!make_tmap_bf16_2d(&tmWb, pk.WB, (uint64_t)pk.kc, dd, dd, 64, (uint32_t)(ra ? ra : 64))) return MAPL_ERR_CUDA;
-    if (!make_tmap_bf16_2d(&tmWd, pk.Wd, dd, (uint64_t)pk.kc, (uint64_t)pk.kc, 64, kChunkN)) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmWu, pk.WB, (uint64_t)pk.kc, dd, dd, 64, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmWb, pk.WB, (uint64_t)pk.kc, dd, dd, 64, (uint32_t)(ra ? ra : 64) / 2)) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmWd, pk.Wd, dd, (uint64_t)pk.kc, (uint64_t)pk.kc, 64, kChunkN / 2)) return MAPL_ERR_CUDA;
     // dH map: when dH is skipped the map is unused but must be valid
     if (!make_tmap_bf16_2d(&tmO, dH_out ? dH_out : g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
-    const unsigned tiles = (unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m);
+    const unsigned tiles = ((unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m) + 1u) & ~1u;   // whole CTA pairs
     KernelScope ks(KID_TC_BWD_GZ, st);
-    MAPL_CUDA_CHECK(launch_pdl(k_tc_bwd_gz, dim3(tiles), dim3(kThreads), smem, st, tmG, tmWu, tmWb, tmWd, tmO, p));
+    MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_bwd_gz, dim3(tiles), dim3(kThreads), smem, st, tmG, tmWu, tmWb, tmWd, tmO, p));
   }
   {  // ---- dU (+ dA scatter)
     BwdDuParams p;

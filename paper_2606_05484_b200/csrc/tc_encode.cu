@@ -15,14 +15,25 @@ namespace {
 using namespace tc;
 
 constexpr int BM = 128, BK = 64, kThreads = 192;
+#ifdef MAPL_DBG
+__device__ unsigned long long g_dbg[160 * 8];
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define DBG(i) if (lane == 0) g_dbg[blockIdx.x * 8 + (i)] = gtime();
+#else
+#define DBG(i)
+#endif
 constexpr int kATile = BM * BK * 2;   // 16 KB
 
+// CTA pair: the two CTAs of a cluster own consecutive token tiles and run ONE M=256 MMA per k-step
+// (cta_group::2).  Each CTA loads its own H tile and HALF of the U^T tile (r/2 rows), so the
+// parameter stream from L2 is half that of two independent CTAs.  Only the leader (cluster rank 0)
+// issues MMAs; its commits arrive on the barriers of both CTAs.
 __global__ void __launch_bounds__(kThreads, 1)
 k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmW,
             __nv_bfloat16* __restrict__ Z, long long N, int d, int r, int stages, int tile_m) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  const int b_tile = r * BK * 2;
+  const int b_tile = (r / 2) * BK * 2;                 // this CTA's half of the U^T tile
   const int stage_bytes = kATile + b_tile;
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)stages * stage_bytes);
   uint64_t* empty = full + stages;
@@ -30,9 +41,11 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(accum_full + 1);
 
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  const uint32_t rank = cluster_ctarank();
   const long long m0 = (long long)blockIdx.x * tile_m;
   const int nkb = d / BK;
 
+  if (warp == 0) { DBG(0) }
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmH);
     tma_prefetch_desc(&tmW);
@@ -41,48 +54,54 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
     fence_barrier_init();
   }
   if (warp == 1) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"((uint32_t)r) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"((uint32_t)r) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
   }
   tc_fence_before_sync();
-  __syncthreads();
+  cluster_sync_all();                                       // barriers of both CTAs initialised
   tc_fence_after_sync();
   const uint32_t tmem_d = *tmem_slot;
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");       // everything below touches global memory
+  if (warp == 0) { DBG(1) }
 
   if (warp == 0) {
     if (elect_one()) {
       for (int kb = 0; kb < nkb; ++kb) {
         const int s = kb % stages;
         mbar_wait(&empty[s], ((kb / stages) & 1) ^ 1);
-        mbar_arrive_expect_tx(&full[s], (uint32_t)(tile_m * 128 + b_tile));
+        if (rank == 0) mbar_arrive_expect_tx(&full[s], 2u * (uint32_t)(tile_m * 128 + b_tile));
         uint8_t* a = smem + (size_t)s * stage_bytes;
-        tma_load_2d(a, &tmH, &full[s], kb * BK, (int)m0, kEvictFirst);
-        tma_load_2d(a + kATile, &tmW, &full[s], kb * BK, 0, kEvictLast);
+        tma_load_2d_pair(a, &tmH, &full[s], kb * BK, (int)m0, kEvictFirst);
+        tma_load_2d_pair(a + kATile, &tmW, &full[s], kb * BK, (int)rank * (r / 2), kEvictLast);
       }
     }
   } else if (warp == 1) {
-    if (elect_one()) {
-      const uint32_t idesc = make_idesc_bf16(BM, (uint32_t)r, false, false);
+    if (rank == 0 && elect_one()) {
+      const uint32_t idesc = make_idesc_bf16(2 * BM, (uint32_t)r, false, false);
       for (int kb = 0; kb < nkb; ++kb) {
         const int s = kb % stages;
         mbar_wait(&full[s], (kb / stages) & 1);
+#ifdef MAPL_DBG
+        if (kb == 0) g_dbg[blockIdx.x * 8 + 2] = gtime();
+        if (kb == nkb - 1) g_dbg[blockIdx.x * 8 + 3] = gtime();
+#endif
         tc_fence_after_sync();
         const uint32_t a = smem_u32(smem + (size_t)s * stage_bytes);
         const uint32_t b = a + kATile;
 #pragma unroll
         for (int k = 0; k < BK / 16; ++k)
-          umma_bf16(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc, (kb | k) != 0);
-        umma_commit(&empty[s]);
+          umma_bf16_pair(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc, (kb | k) != 0);
+        umma_commit_pair(&empty[s]);
       }
-      umma_commit(accum_full);
+      umma_commit_pair(accum_full);
     }
   } else {
     const int q = warp & 3;                         // TMEM lane quarter this warp may read
     const int row = q * 32 + lane;
     const long long m = m0 + row;
     mbar_wait(accum_full, 0);
+    if (warp == 2) { DBG(4) }
     tc_fence_after_sync();
     for (int c = 0; c < r / 32; ++c) {
       uint32_t v[32];
@@ -102,15 +121,20 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
       }
     }
   }
+  if (warp == 2) { DBG(5) }
   tc_fence_before_sync();
-  __syncthreads();
+  cluster_sync_all();                                       // the peer may still signal our barriers / read our smem
   if (warp == 1) {
     tc_fence_after_sync();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"((uint32_t)r) : "memory");
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"((uint32_t)r) : "memory");
   }
 }
 
 }  // namespace
+
+#ifdef MAPL_DBG
+extern "C" int mapl_debug_read(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, g_dbg, sizeof(g_dbg)); }
+#endif
 
 int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
                   int32_t* codes_out, cudaStream_t st);   // tc_encode_rvq.cu
@@ -122,8 +146,8 @@ int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks
   const int tile_m = tc_tile_m(d.n_tokens);
   CUtensorMap tmH, tmW;
   if (!make_tmap_bf16_2d(&tmH, H, (uint64_t)d.n_tokens, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)tile_m)) return MAPL_ERR_CUDA;
-  if (!make_tmap_bf16_2d(&tmW, pk.WB, (uint64_t)d.r, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)d.r)) return MAPL_ERR_CUDA;
-  const int stage_bytes = kATile + d.r * BK * 2;
+  if (!make_tmap_bf16_2d(&tmW, pk.WB, (uint64_t)d.r, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
+  const int stage_bytes = kATile + (d.r / 2) * BK * 2;
   int stages = (200 * 1024) / stage_bytes;
   if (stages > 8) stages = 8;
   if (stages > d.d / BK) stages = d.d / BK;
@@ -133,9 +157,9 @@ int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks
     MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_encode, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     attr_done = true;
   }
-  const unsigned tiles = (unsigned)((d.n_tokens + tile_m - 1) / tile_m);
+  const unsigned tiles = ((unsigned)((d.n_tokens + tile_m - 1) / tile_m) + 1u) & ~1u;   // whole CTA pairs
   KernelScope ks(KID_TC_ENCODE, st);
-  MAPL_CUDA_CHECK(launch_pdl(k_tc_encode, dim3(tiles), dim3(kThreads), smem, st, tmH, tmW,
+  MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_encode, dim3(tiles), dim3(kThreads), smem, st, tmH, tmW,
                              reinterpret_cast<__nv_bfloat16*>(Zq_out), d.n_tokens, d.d, d.r, stages, tile_m));
   return MAPL_OK;
 }

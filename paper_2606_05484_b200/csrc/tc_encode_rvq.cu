@@ -2,7 +2,8 @@
 // levels in ONE kernel, z never leaves the chip (Eq. 1; Sec. 3.5;
 // readings S3-S5 of DESIGN.md).
 //
-// One CTA per token tile (<= 128 tokens; one TMEM lane = one token).
+// One CTA per token tile (<= 128 tokens; one TMEM lane = one token); CTAs work in pairs (cluster of 2,
+// cta_group::2 MMAs of M = 256): each CTA loads half of every parameter / codebook tile.
 //   phase 1   z = H (U_hi + U_lo)      H tiles by TMA (HBM, evict-first), the two bf16 split terms
 //             of U^T from the L2-resident pack; fp32 accumulator [128 x r] in TMEM columns [0,r).
 //             bf16 H is exact and U_hi + U_lo carries 16 mantissa bits, so z is fp32-accurate.
@@ -58,7 +59,7 @@ struct Smem {
 
 __host__ __device__ inline size_t rvq_regionR(const RvqParams& p) {
   const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes;
-  const size_t lvl = (size_t)(p.r / 64 + p.ring_tiles) * kTileBytes;
+  const size_t lvl = (size_t)(p.r / 64) * kTileBytes + (size_t)p.ring_tiles * kHalfTileBytes;
   return ring1 > lvl ? ring1 : lvl;
 }
 __host__ __device__ inline size_t rvq_tail_bytes(const RvqParams& p) {
@@ -173,6 +174,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
   const Smem s = carve_smem(smem, p);
 
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  const uint32_t rank = cluster_ctarank();
   const long long m0 = (long long)blockIdx.x * p.tile_m;
   const int nkb1 = p.d / 64, nkb = p.r / 64, nchunks = p.K / kChunk;
 
@@ -181,13 +183,13 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
     for (int i = 0; i < p.stages1; ++i) { mbar_init(&s.s1_full[i], 1); mbar_init(&s.s1_empty[i], 1); }
     mbar_init(s.z_full, 1);
     for (int i = 0; i < p.ring_tiles; ++i) { mbar_init(&s.c_full[i], 1); mbar_init(&s.c_empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&s.acc_full[i], 1); mbar_init(&s.acc_empty[i], 4); }
-    mbar_init(s.rho_ready, 4);
+    for (int i = 0; i < 2; ++i) { mbar_init(&s.acc_full[i], 1); mbar_init(&s.acc_empty[i], 8); }
+    mbar_init(s.rho_ready, 8);                // leader's barriers collect the epilogue warps of both CTAs
     fence_barrier_init();
   }
-  if (warp == 1) tmem_alloc<512>(s.tmem_slot);
+  if (warp == 1) tmem_alloc_pair<512>(s.tmem_slot);
   tc_fence_before_sync();
-  __syncthreads();
+  cluster_sync_all();
   tc_fence_after_sync();
   const uint32_t tmem_base = *s.tmem_slot;
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -196,15 +198,15 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
   if (warp == 0) {
     // ------------------------------------------------------------ TMA producer
     if (elect_one()) {
-      const uint32_t w_tile = (uint32_t)p.r * 128;
+      const uint32_t w_tile = (uint32_t)p.r * 64;          // this CTA's half (r/2 rows) of a U^T tile
       for (int kb = 0; kb < nkb1; ++kb) {
         const int st = kb % p.stages1;
         mbar_wait(&s.s1_empty[st], ((kb / p.stages1) & 1) ^ 1);
-        mbar_arrive_expect_tx(&s.s1_full[st], (uint32_t)(p.tile_m * 128) + 2 * w_tile);
+        if (rank == 0) mbar_arrive_expect_tx(&s.s1_full[st], 2u * ((uint32_t)(p.tile_m * 128) + 2 * w_tile));
         uint8_t* a = s.ring1 + (size_t)st * p.stage1_bytes;
-        tma_load_2d(a, &tmH, &s.s1_full[st], kb * 64, (int)m0, kEvictFirst);
-        tma_load_2d(a + kTileBytes, &tmWhi, &s.s1_full[st], kb * 64, 0, kEvictLast);
-        tma_load_2d(a + kTileBytes + w_tile, &tmWlo, &s.s1_full[st], kb * 64, 0, kEvictLast);
+        tma_load_2d_pair(a, &tmH, &s.s1_full[st], kb * 64, (int)m0, kEvictFirst);
+        tma_load_2d_pair(a + kTileBytes, &tmWhi, &s.s1_full[st], kb * 64, (int)rank * (p.r / 2), kEvictLast);
+        tma_load_2d_pair(a + kTileBytes + w_tile, &tmWlo, &s.s1_full[st], kb * 64, (int)rank * (p.r / 2), kEvictLast);
       }
       mbar_wait(s.z_full, 0);             // phase-1 MMAs have consumed region R: it may be reused
       int it = 0;
@@ -213,50 +215,51 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
           for (int kb = 0; kb < nkb; ++kb, ++it) {
             const int st = it % p.ring_tiles;
             mbar_wait(&s.c_empty[st], ((it / p.ring_tiles) & 1) ^ 1);
-            mbar_arrive_expect_tx(&s.c_full[st], kTileBytes);
-            tma_load_2d(s.ringC + (size_t)st * kTileBytes, &tmC, &s.c_full[st], kb * 64, l * p.K + c * kChunk, kEvictLast);
+            if (rank == 0) mbar_arrive_expect_tx(&s.c_full[st], 2 * kHalfTileBytes);
+            tma_load_2d_pair(s.ringC + (size_t)st * kHalfTileBytes, &tmC, &s.c_full[st], kb * 64,
+                             l * p.K + c * kChunk + (int)rank * (kChunk / 2), kEvictLast);
           }
     }
   } else if (warp == 1) {
     // ------------------------------------------------------------ MMA issuer
-    if (elect_one()) {
-      const uint32_t idesc1 = make_idesc_bf16(128, (uint32_t)p.r, false, false);
+    if (rank == 0 && elect_one()) {
+      const uint32_t idesc1 = make_idesc_bf16(256, (uint32_t)p.r, false, false);
       for (int kb = 0; kb < nkb1; ++kb) {
         const int st = kb % p.stages1;
         mbar_wait(&s.s1_full[st], (kb / p.stages1) & 1);
         tc_fence_after_sync();
         const uint32_t a = smem_u32(s.ring1 + (size_t)st * p.stage1_bytes);
-        const uint32_t bh = a + kTileBytes, bl = bh + p.r * 128;
+        const uint32_t bh = a + kTileBytes, bl = bh + p.r * 64;
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           const uint64_t da = desc_kmajor_sw128(a + k * 32);
-          umma_bf16(tmem_base, da, desc_kmajor_sw128(bh + k * 32), idesc1, (kb | k) != 0);
-          umma_bf16(tmem_base, da, desc_kmajor_sw128(bl + k * 32), idesc1, 1);
+          umma_bf16_pair(tmem_base, da, desc_kmajor_sw128(bh + k * 32), idesc1, (kb | k) != 0);
+          umma_bf16_pair(tmem_base, da, desc_kmajor_sw128(bl + k * 32), idesc1, 1);
         }
-        umma_commit(&s.s1_empty[st]);
+        umma_commit_pair(&s.s1_empty[st]);
       }
-      umma_commit(s.z_full);
-      const uint32_t idesc2 = make_idesc_f16(128, kChunk);
+      umma_commit_pair(s.z_full);
+      const uint32_t idesc2 = make_idesc_f16(256, kChunk);
       int it = 0, cg = 0;
       for (int l = 0; l < p.L; ++l) {
-        mbar_wait(s.rho_ready, l & 1);    // bf16 residual of level l is in sRho
+        mbar_wait_cluster(s.rho_ready, l & 1);    // fp16 residuals of level l are in sRho of both CTAs
         tc_fence_after_sync();
         for (int c = 0; c < nchunks; ++c, ++cg) {
           const int as = cg & 1;
-          mbar_wait(&s.acc_empty[as], ((cg >> 1) & 1) ^ 1);
+          mbar_wait_cluster(&s.acc_empty[as], ((cg >> 1) & 1) ^ 1);
           tc_fence_after_sync();
           const uint32_t tmem_d = tmem_base + kAccCol0 + as * kChunk;
           for (int kb = 0; kb < nkb; ++kb, ++it) {
             const int st = it % p.ring_tiles;
             mbar_wait(&s.c_full[st], (it / p.ring_tiles) & 1);
             tc_fence_after_sync();
-            const uint32_t a = smem_u32(s.sRho + (size_t)kb * kTileBytes), b = smem_u32(s.ringC + (size_t)st * kTileBytes);
+            const uint32_t a = smem_u32(s.sRho + (size_t)kb * kTileBytes), b = smem_u32(s.ringC + (size_t)st * kHalfTileBytes);
 #pragma unroll
             for (int k = 0; k < 4; ++k)
-              umma_bf16(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc2, (kb | k) != 0);
-            umma_commit(&s.c_empty[st]);
+              umma_bf16_pair(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc2, (kb | k) != 0);
+            umma_commit_pair(&s.c_empty[st]);
           }
-          umma_commit(&s.acc_full[as]);
+          umma_commit_pair(&s.acc_full[as]);
         }
       }
     }
@@ -272,10 +275,10 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
     tc_fence_after_sync();
     float unscale;
     float n2 = update_rho(tmem_row, nullptr, s.sRho, row, p.r, &unscale);
-    fence_proxy_async_smem();
+    fence_proxy_async_all();
     tc_fence_before_sync();
     __syncwarp();
-    if (lane == 0) mbar_arrive(s.rho_ready);
+    if (lane == 0) mbar_arrive_leader(s.rho_ready);
 
     int cg = 0;
     for (int l = 0; l < p.L; ++l) {
@@ -342,7 +345,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         }
         tc_fence_before_sync();
         __syncwarp();
-        if (lane == 0) mbar_arrive(&s.acc_empty[as]);
+        if (lane == 0) mbar_arrive_leader(&s.acc_empty[as]);
       }
 
       // ---- exact fp32 re-scoring of the candidates, ascending k, strict '<': lowest index wins ties
@@ -371,10 +374,10 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       if (live) p.codes[m * p.L + l] = bestk;
       if (l + 1 < p.L) {
         n2 = update_rho(tmem_row, Cl + (long long)bestk * p.r, s.sRho, row, p.r, &unscale);
-        fence_proxy_async_smem();
+        fence_proxy_async_all();
         tc_fence_before_sync();
         __syncwarp();
-        if (lane == 0) mbar_arrive(s.rho_ready);
+        if (lane == 0) mbar_arrive_leader(s.rho_ready);
       }
     }
 
@@ -392,10 +395,10 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
     }
   }
   tc_fence_before_sync();
-  __syncthreads();
+  cluster_sync_all();
   if (warp == 1) {
     tc_fence_after_sync();
-    tmem_dealloc<512>(tmem_base);
+    tmem_dealloc_pair<512>(tmem_base);
   }
 }
 
@@ -409,31 +412,31 @@ int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codeb
   p.Zq = reinterpret_cast<__nv_bfloat16*>(Zq_out); p.codes = codes_out;
   p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.L = d.rvq_levels; p.K = d.rvq_k;
   p.tile_m = tc_tile_m(d.n_tokens);
-  p.stage1_bytes = kTileBytes + 2 * d.r * 128;
+  p.stage1_bytes = kTileBytes + 2 * d.r * 64;
   p.stages1 = 2; p.ring_tiles = 2;
   const size_t avail = (size_t)227 * 1024 - 1024 - rvq_tail_bytes(p);
-  if (avail < (size_t)2 * p.stage1_bytes || avail < (size_t)(d.r / 64 + 2) * kTileBytes) return MAPL_ERR_UNSUPPORTED;
+  if (avail < (size_t)2 * p.stage1_bytes || avail < (size_t)(d.r / 64 + 1) * kTileBytes) return MAPL_ERR_UNSUPPORTED;
   p.stages1 = (int)(avail / p.stage1_bytes);
   if (p.stages1 > 8) p.stages1 = 8;
   if (p.stages1 > d.d / 64) p.stages1 = d.d / 64;
-  p.ring_tiles = (int)(avail / kTileBytes) - d.r / 64;
-  if (p.ring_tiles > 12) p.ring_tiles = 12;
+  p.ring_tiles = (int)((avail - (size_t)(d.r / 64) * kTileBytes) / kHalfTileBytes);
+  if (p.ring_tiles > 16) p.ring_tiles = 16;
   if (p.stages1 < 2 || p.ring_tiles < 2) return MAPL_ERR_UNSUPPORTED;
   const size_t smem = 1024 + rvq_regionR(p) + rvq_tail_bytes(p);
   CUtensorMap tmH, tmWhi, tmWlo, tmC;
   const uint64_t dd = (uint64_t)d.d, rr = (uint64_t)d.r;
   if (!make_tmap_bf16_2d(&tmH, H, (uint64_t)d.n_tokens, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
-  if (!make_tmap_bf16_2d(&tmWhi, pk.WB, rr, dd, dd, 64, (uint32_t)d.r)) return MAPL_ERR_CUDA;
-  if (!make_tmap_bf16_2d(&tmWlo, pk.WBlo, rr, dd, dd, 64, (uint32_t)d.r)) return MAPL_ERR_CUDA;
-  if (!make_tmap_bf16_2d(&tmC, pk.Cb, (uint64_t)d.rvq_levels * d.rvq_k, rr, rr, 64, kChunk)) return MAPL_ERR_CUDA;
+  if (!make_tmap_bf16_2d(&tmWhi, pk.WB, rr, dd, dd, 64, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
+  if (!make_tmap_bf16_2d(&tmWlo, pk.WBlo, rr, dd, dd, 64, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
+  if (!make_tmap_bf16_2d(&tmC, pk.Cb, (uint64_t)d.rvq_levels * d.rvq_k, rr, rr, 64, kChunk / 2)) return MAPL_ERR_CUDA;
   static bool attr_done = false;
   if (!attr_done) {
     MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_encode_rvq, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     attr_done = true;
   }
-  const unsigned tiles = (unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m);
+  const unsigned tiles = ((unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m) + 1u) & ~1u;   // whole CTA pairs
   KernelScope ks(KID_TC_ENCODE_RVQ, st);
-  MAPL_CUDA_CHECK(launch_pdl(k_tc_encode_rvq, dim3(tiles), dim3(kThreads), smem, st, tmH, tmWhi, tmWlo, tmC, p));
+  MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_encode_rvq, dim3(tiles), dim3(kThreads), smem, st, tmH, tmWhi, tmWlo, tmC, p));
   return MAPL_OK;
 }
 

@@ -1,9 +1,15 @@
 // tc_tile_ops.cuh -- the "token tile x d-chunks" streaming GEMM shared by decode and by the dH phase
-// of backward:   Out[tile_m, d] = Aop[128, nkb*64] . W[d, nkb*64]^T
-//   Aop   resident smem operand, nkb k-blocks of [128 x 64] bf16, K-major SW128
-//   W     streamed by TMA in [128 x 64] tiles through a ring of b_stages
-//   D     kAccStages x [128 lanes x 128 cols] fp32 in TMEM (MMA of chunk j+1 overlaps epilogue of j)
-//   Out   bf16, through swizzled staging boxes and TMA stores
+// of backward, run by a CTA PAIR (cluster of 2, tcgen05 cta_group::2):
+//     Out[2 x 128 tokens, d] = Aop[2 x 128, nkb*64] . W[d, nkb*64]^T
+//   Aop   resident smem operand of EACH CTA (its own 128 token rows), nkb k-blocks of [128 x 64]
+//         bf16, K-major SW128
+//   W     streamed by TMA through a ring of b_stages; per stage each CTA holds HALF of the
+//         [128 x 64] tile (64 rows of W): the pair reads every W byte from L2 once, not twice
+//   D     acc_stages x [128 lanes x 128 cols] fp32 in each CTA's TMEM (MMA of chunk j+1 overlaps the
+//         epilogue of chunk j); one M=256 UMMA per k-step, issued by the leader CTA (rank 0)
+//   Out   bf16, through swizzled staging boxes and TMA stores, each CTA its own rows
+// Barriers: b_full / acc_empty live in the leader (they collect arrivals from both CTAs);
+// b_empty / acc_full exist in both CTAs and are signalled by multicast commits.
 // Three roles, each called by the warp(s) that own it.
 #pragma once
 #include <stdlib.h>
@@ -15,64 +21,65 @@ namespace tc {
 
 constexpr int kChunkN = 128;                 // d-chunk width == UMMA N
 constexpr int kTileBytes = 128 * 64 * 2;     // one [128 x 64] bf16 tile
-constexpr int kAccStages = 4;
+constexpr int kHalfTileBytes = 64 * 64 * 2;  // the half of a W tile one CTA of the pair holds
 constexpr int kOutBufs = 4;
 
 struct ChunkPipe {
   uint8_t* sA;        // resident A operand (nkb tiles)
-  uint8_t* sB;        // ring (b_stages tiles)
+  uint8_t* sB;        // ring (b_stages half tiles)
   uint8_t* sOut;      // kOutBufs staging boxes
   uint64_t* b_full; uint64_t* b_empty;       // [b_stages]
-  uint64_t* acc_full; uint64_t* acc_empty;   // [kAccStages]
-  int nkb, nchunks, b_stages;
-  uint32_t tmem_base;
+  uint64_t* acc_full; uint64_t* acc_empty;   // [acc_stages]
+  int nkb, nchunks, b_stages, acc_stages;
+  uint32_t tmem_base, rank;
 };
 
-// producer: one thread
+// producer: one thread in each CTA; tmW box = [64 rows x 64 cols]
 __device__ __forceinline__ void chunk_produce(const ChunkPipe& c, const CUtensorMap* tmW) {
   int it = 0;
   for (int j = 0; j < c.nchunks; ++j)
     for (int kb = 0; kb < c.nkb; ++kb, ++it) {
       const int s = it % c.b_stages;
       mbar_wait(&c.b_empty[s], ((it / c.b_stages) & 1) ^ 1);
-      mbar_arrive_expect_tx(&c.b_full[s], kTileBytes);
-      tma_load_2d(c.sB + (size_t)s * kTileBytes, tmW, &c.b_full[s], kb * 64, j * kChunkN, kEvictLast);
+      if (c.rank == 0) mbar_arrive_expect_tx(&c.b_full[s], 2 * kHalfTileBytes);
+      tma_load_2d_pair(c.sB + (size_t)s * kHalfTileBytes, tmW, &c.b_full[s], kb * 64, j * kChunkN + (int)c.rank * 64, kEvictLast);
     }
 }
 
-// MMA issuer: one thread; the A operand must already be visible to the async proxy
+// MMA issuer: one thread of the LEADER CTA; the A operands of both CTAs must already be visible to
+// the async proxy
 __device__ __forceinline__ void chunk_mma(const ChunkPipe& c) {
-  const uint32_t idesc = make_idesc_bf16(128, kChunkN, false, false);
+  const uint32_t idesc = make_idesc_bf16(256, kChunkN, false, false);
   int it = 0;
   for (int j = 0; j < c.nchunks; ++j) {
-    const int as = j % kAccStages;
-    mbar_wait(&c.acc_empty[as], ((j / kAccStages) & 1) ^ 1);
+    const int as = j % c.acc_stages;
+    mbar_wait_cluster(&c.acc_empty[as], ((j / c.acc_stages) & 1) ^ 1);
     tc_fence_after_sync();
     const uint32_t tmem_d = c.tmem_base + as * kChunkN;
     for (int kb = 0; kb < c.nkb; ++kb, ++it) {
       const int s = it % c.b_stages;
       mbar_wait(&c.b_full[s], (it / c.b_stages) & 1);
       tc_fence_after_sync();
-      const uint32_t a = smem_u32(c.sA + (size_t)kb * kTileBytes), b = smem_u32(c.sB + (size_t)s * kTileBytes);
+      const uint32_t a = smem_u32(c.sA + (size_t)kb * kTileBytes), b = smem_u32(c.sB + (size_t)s * kHalfTileBytes);
 #pragma unroll
       for (int k = 0; k < 4; ++k)
-        umma_bf16(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc, (kb | k) != 0);
-      umma_commit(&c.b_empty[s]);
+        umma_bf16_pair(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc, (kb | k) != 0);
+      umma_commit_pair(&c.b_empty[s]);
     }
-    umma_commit(&c.acc_full[as]);
+    umma_commit_pair(&c.acc_full[as]);
   }
 }
 
-// epilogue: the 4 warps with threadIdx.x in [64,192); row = TMEM lane = token row in the tile.
-// Uses named barrier 1 (128 threads).  Thread 64 issues the TMA stores.
+// epilogue: the 4 warps with threadIdx.x in [64,192) of each CTA; row = TMEM lane = token row in the
+// tile.  Uses named barrier 1 (128 threads).  Thread 64 issues the TMA stores.
 __device__ __forceinline__ void chunk_epilogue(const ChunkPipe& c, const CUtensorMap* tmO, int m0) {
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32, q = warp & 3, row = q * 32 + lane;
   for (int j = 0; j < c.nchunks; ++j) {
-    const int as = j % kAccStages, ob = (j & 1) * 2;
+    const int as = j % c.acc_stages, ob = (j & 1) * 2;
     // only chunk j-1's store group may still be reading smem: the boxes of chunk j-2 are free
     if (threadIdx.x == 64) tma_store_wait_read<1>();
     asm volatile("bar.sync 1, 128;" ::: "memory");
-    mbar_wait(&c.acc_full[as], (j / kAccStages) & 1);
+    mbar_wait(&c.acc_full[as], (j / c.acc_stages) & 1);
     tc_fence_after_sync();
 #pragma unroll
     for (int cc = 0; cc < kChunkN / 32; ++cc) {
@@ -92,7 +99,7 @@ __device__ __forceinline__ void chunk_epilogue(const ChunkPipe& c, const CUtenso
     }
     tc_fence_before_sync();
     __syncwarp();
-    if (lane == 0) mbar_arrive(&c.acc_empty[as]);     // the TMEM stage may be overwritten
+    if (lane == 0) mbar_arrive_leader(&c.acc_empty[as]);     // the TMEM stage may be overwritten
     fence_proxy_async_smem();
     asm volatile("bar.sync 1, 128;" ::: "memory");
     if (threadIdx.x == 64) {
@@ -106,7 +113,7 @@ __device__ __forceinline__ void chunk_epilogue(const ChunkPipe& c, const CUtenso
 
 __device__ __forceinline__ void chunk_init_barriers(const ChunkPipe& c) {
   for (int s = 0; s < c.b_stages; ++s) { mbar_init(&c.b_full[s], 1); mbar_init(&c.b_empty[s], 1); }
-  for (int s = 0; s < kAccStages; ++s) { mbar_init(&c.acc_full[s], 1); mbar_init(&c.acc_empty[s], 4); }
+  for (int s = 0; s < c.acc_stages; ++s) { mbar_init(&c.acc_full[s], 1); mbar_init(&c.acc_empty[s], 8); }
 }
 
 // host: launch with programmatic dependent launch allowed (the kernels call griddepcontrol.wait
@@ -121,6 +128,22 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
   cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
+// same, as clusters of two CTAs (CTA pairs for cta_group::2); grid.x must be even
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl_pair(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                   Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  static const bool pdl = getenv("MAPL_NO_PDL") == nullptr;
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+  attr[1].id = cudaLaunchAttributeClusterDimension;
+  attr[1].val.clusterDim.x = 2; attr[1].val.clusterDim.y = 1; attr[1].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 2;
   return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
 }
 
