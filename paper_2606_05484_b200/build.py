@@ -22,7 +22,8 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr",
          "-I", os.path.join(ROOT, "include"), "-I", CSRC] + \
-        (["-DMAPL_DBG"] if os.environ.get("MAPL_DBG") else [])   # in-kernel timestamps (development only)
+        (["-DMAPL_DBG"] if os.environ.get("MAPL_DBG") else []) + \
+        (["-D" + os.environ["MAPL_DEFINE"]] if os.environ.get("MAPL_DEFINE") else [])   # in-kernel timestamps (development only)
 
 
 def sources():

@@ -24,7 +24,8 @@ namespace mapl {
 namespace {
 using namespace tc;
 
-constexpr int kThreads = 192;
+constexpr int kThreads = kPipeThreads;   // k_tc_bwd_gz: warp 0 TMA, warp 1 MMA, warps 2-9 epilogue
+constexpr int kThreadsDu = 192;
 
 __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
   asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
@@ -53,15 +54,15 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   const size_t ring2 = (size_t)(p.r / 64) * kTileBytes + (size_t)p.b_stages * kHalfTileBytes;
   const size_t regionR = ring1 > ring2 ? ring1 : ring2;
   ChunkPipe c;
-  c.nkb = p.r / 64; c.nchunks = p.d / kChunkN; c.b_stages = p.b_stages; c.acc_stages = 4;
+  c.nkb = p.r / 64; c.nchunks = p.d / kChunkN; c.b_stages = p.b_stages;
   c.rank = cluster_ctarank();
   c.sA = smem;
   c.sB = smem + (size_t)(p.r / 64) * kTileBytes;
   c.sOut = smem + regionR;
   uint64_t* bars = reinterpret_cast<uint64_t*>(c.sOut + (size_t)kOutBufs * kTileBytes);
   c.b_full = bars; c.b_empty = c.b_full + p.b_stages;
-  c.acc_full = c.b_empty + p.b_stages; c.acc_empty = c.acc_full + 4;
-  uint64_t* s1_full = c.acc_empty + 4;
+  c.acc_full = c.b_empty + p.b_stages; c.acc_empty = c.acc_full + kAccStages;
+  uint64_t* s1_full = c.acc_empty + kAccStages;
   uint64_t* s1_empty = s1_full + p.stages1;
   uint64_t* acc1_full = s1_empty + p.stages1;
   uint64_t* gz_full = acc1_full + 1;
@@ -76,7 +77,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
     chunk_init_barriers(c);
     for (int s = 0; s < p.stages1; ++s) { mbar_init(&s1_full[s], 1); mbar_init(&s1_empty[s], 1); }
     mbar_init(acc1_full, 1);
-    mbar_init(gz_full, 8);                    // leader's: the epilogue warps of both CTAs
+    mbar_init(gz_full, 16);                   // leader's: the epilogue warps of both CTAs
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc_pair<512>(tmem_slot);
@@ -130,7 +131,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
       }
     }
   } else {
-    const int q = warp & 3, row = q * 32 + lane;
+    const int q = warp & 3, half = (warp - 2) >> 2, row = q * 32 + lane;   // two warps per TMEM lane quarter
     const long long m = m0 + row;
     const bool live = row < p.tile_m && m < p.N;
     const uint32_t tmem_row = c.tmem_base + ((uint32_t)(q * 32) << 16);
@@ -144,12 +145,12 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         if (zp[a] == nullptr) continue;
         const long long nv = zn[a] / 4, per = (nv + gridDim.x - 1) / gridDim.x;
         const long long lo = per * blockIdx.x, hi = lo + per < nv ? lo + per : nv;
-        for (long long i = lo + et; i < hi; i += 128) reinterpret_cast<float4*>(zp[a])[i] = zero;
+        for (long long i = lo + et; i < hi; i += 256) reinterpret_cast<float4*>(zp[a])[i] = zero;
       }
     }
     mbar_wait(acc1_full, 0);
     tc_fence_after_sync();
-    for (int cc = 0; cc < p.r / 32; ++cc) {
+    for (int cc = half; cc < p.r / 32; cc += 2) {       // 32-column pieces alternate between the two warps
       uint32_t v[32];
       tmem_ld32(tmem_row + cc * 32, v);
       tmem_ld_wait();
@@ -166,7 +167,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
     }
     if (p.ra) {
       float4* dst = reinterpret_cast<float4*>(p.gA + (live ? m : 0) * p.ra);
-      for (int cc = 0; cc < p.ra / 32; ++cc) {
+      for (int cc = half; cc < p.ra / 32; cc += 2) {
         uint32_t v[32];
         tmem_ld32(tmem_row + p.r + cc * 32, v);
         tmem_ld_wait();
@@ -246,7 +247,7 @@ __device__ __forceinline__ void scatter_gA(const BwdDuParams& p, float* sG, int*
   }
 }
 
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kThreadsDu, 1)
 k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmZ,
             const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmGz, const BwdDuParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -403,18 +404,18 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     if (p.stages1 > d.d / 64) p.stages1 = d.d / 64;
     if (p.stages1 < 2) return MAPL_ERR_UNSUPPORTED;
     p.b_stages = (int)((budget - (size_t)(d.r / 64) * kTileBytes) / kHalfTileBytes);
-    if (p.b_stages > 8) p.b_stages = 8;
+    if (p.b_stages > 16) p.b_stages = 16;
     if (p.b_stages < 2) return MAPL_ERR_UNSUPPORTED;
     const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes,
                  ring2 = (size_t)(d.r / 64) * kTileBytes + (size_t)p.b_stages * kHalfTileBytes;
     const size_t smem = (ring1 > ring2 ? ring1 : ring2) + (size_t)kOutBufs * kTileBytes + 1024 + 1024;
     CUtensorMap tmG, tmWu, tmWb, tmWd, tmO;
+    // dH map: when dH is skipped the map is unused but must be valid
+    if (!make_tmap_bf16_2d(&tmO, dH_out ? dH_out : g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmG, g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmWu, pk.WB, (uint64_t)pk.kc, dd, dd, 64, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmWb, pk.WB, (uint64_t)pk.kc, dd, dd, 64, (uint32_t)(ra ? ra : 64) / 2)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmWd, pk.Wd, dd, (uint64_t)pk.kc, (uint64_t)pk.kc, 64, kChunkN / 2)) return MAPL_ERR_CUDA;
-    // dH map: when dH is skipped the map is unused but must be valid
-    if (!make_tmap_bf16_2d(&tmO, dH_out ? dH_out : g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
     const unsigned tiles = ((unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m) + 1u) & ~1u;   // whole CTA pairs
     KernelScope ks(KID_TC_BWD_GZ, st);
     MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_bwd_gz, dim3(tiles), dim3(kThreads), smem, st, tmG, tmWu, tmWb, tmWd, tmO, p));
@@ -442,7 +443,7 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     if (!make_tmap_bf16_2d(&tmH, H ? H : g, N, dd, dd, 64, 64)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmGz, gz_out, N, rr, rr, 64, 64)) return MAPL_ERR_CUDA;
     KernelScope ks(KID_TC_BWD_DU, st);
-    MAPL_CUDA_CHECK(launch_pdl(k_tc_bwd_du, dim3(n_dt, S), dim3(kThreads), smem, st, tmG, tmZ, tmH, tmGz, p));
+    MAPL_CUDA_CHECK(launch_pdl(k_tc_bwd_du, dim3(n_dt, S), dim3(kThreadsDu), smem, st, tmG, tmZ, tmH, tmGz, p));
   }
   if (dB_out && ra) {   // dB += A[tok]^T g  (P_p is frozen in the paper: optional, fp32 SIMT)
     GemmArgs ga;

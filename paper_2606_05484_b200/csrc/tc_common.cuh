@@ -257,6 +257,19 @@ __device__ __forceinline__ uint32_t sw128_offset(uint32_t row, uint32_t chunk) {
   return row * 128u + ((chunk ^ (row & 7u)) << 4);
 }
 
+// development only (-DMAPL_DBG): per-CTA %globaltimer stamps, 64 slots per CTA, read back with mapl_debug_read
+#ifdef MAPL_DBG
+static __device__ unsigned long long g_dbg[320 * 64];      // one copy per translation unit
+#define MAPL_DBG_READER(name) extern "C" int name(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, mapl::tc::g_dbg, sizeof(mapl::tc::g_dbg)); }
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define DBGT(i) { g_dbg[blockIdx.x * 64 + (i)] = gtime(); }
+#define DBG(i) if (lane == 0) DBGT(i)
+#else
+#define DBGT(i)
+#define DBG(i)
+#define MAPL_DBG_READER(name)
+#endif
+
 #endif  // __CUDACC__
 }  // namespace tc
 }  // namespace mapl

@@ -18,36 +18,56 @@ namespace mapl {
 namespace {
 using namespace tc;
 
-constexpr int kThreads = 192;
+constexpr int kThreads = kPipeThreads;
 
 struct DecodeParams {
   const int32_t* codes; const float* codebooks;   // RVQ dequant (codes != nullptr)
   const int32_t* tok; const float* A;             // anchor gather (tok != nullptr)
   long long N;
   int d, r, ra, L, K;
-  int tile_m, b_stages, acc_stages, z_from_tma;
+  int tile_m, b_stages, z_from_tma;
 };
 
 // sA tiles [tile0, tile0 + width/64): row (q*32 + j) := bf16( sum_{l < nsrc} table[l*src_stride + idx_j[l]*width + :] ),
-// zeros where idx < 0.  idx[] holds the indices of row q*32+lane.  One warp, convergent.
+// zeros where idx < 0.  idx[] holds the indices of row q*32+lane.  One warp, convergent.  The loads
+// of 8 row groups are issued back to back before any is consumed (the gathers are L2-latency bound).
+// Two warps share a quarter: `part` (0/1) takes the first / second half of the row groups.
+template <int kBatch>
 __device__ __forceinline__ void gather_sum_rows(uint8_t* sA, int tile0, int width, const float* __restrict__ table,
-                                                long long src_stride, const int (&idx)[8], int nsrc, int q, int lane) {
-  const int lpr = width / 8, rpi = 32 / lpr, cc = lane % lpr;
-#pragma unroll 2
-  for (int it = 0; it < lpr; ++it) {           // 32 / rpi iterations
-    const int rl = it * rpi + lane / lpr;
-    float s[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+                                                long long src_stride, const int (&idx)[8], int nsrc, int q, int lane,
+                                                int part) {
+  const int lpr = width / 8, rpi = 32 / lpr, cc = lane % lpr, sub = lane / lpr;
+  for (int it0 = part * (lpr / 2); it0 < (part + 1) * (lpr / 2); it0 += kBatch) {   // lpr = 32 / rpi row groups in all
+    float acc[kBatch][8];
+#pragma unroll
+    for (int b = 0; b < kBatch; ++b)
+#pragma unroll
+      for (int j = 0; j < 8; ++j) acc[b][j] = 0.f;
 #pragma unroll
     for (int l = 0; l < 8; ++l) {
-      const int k = __shfl_sync(0xffffffffu, idx[l], rl);
-      if (l < nsrc && k >= 0) {
-        const float4* src = reinterpret_cast<const float4*>(table + l * src_stride + (long long)k * width + cc * 8);
-        const float4 x = __ldg(src), y = __ldg(src + 1);
-        s[0] += x.x; s[1] += x.y; s[2] += x.z; s[3] += x.w; s[4] += y.x; s[5] += y.y; s[6] += y.z; s[7] += y.w;
+      if (l < nsrc) {
+        float4 x[kBatch], y[kBatch];
+#pragma unroll
+        for (int b = 0; b < kBatch; ++b) {
+          const int k = __shfl_sync(0xffffffffu, idx[l], (it0 + b) * rpi + sub);
+          const float4* src = reinterpret_cast<const float4*>(table + l * src_stride + (long long)(k < 0 ? 0 : k) * width + cc * 8);
+          x[b] = __ldg(src); y[b] = __ldg(src + 1);
+          if (k < 0) { x[b] = make_float4(0.f, 0.f, 0.f, 0.f); y[b] = x[b]; }
+        }
+#pragma unroll
+        for (int b = 0; b < kBatch; ++b) {
+          acc[b][0] += x[b].x; acc[b][1] += x[b].y; acc[b][2] += x[b].z; acc[b][3] += x[b].w;
+          acc[b][4] += y[b].x; acc[b][5] += y[b].y; acc[b][6] += y[b].z; acc[b][7] += y[b].w;
+        }
       }
     }
-    const uint4 o = make_uint4(pack_bf16x2(s[0], s[1]), pack_bf16x2(s[2], s[3]), pack_bf16x2(s[4], s[5]), pack_bf16x2(s[6], s[7]));
-    *reinterpret_cast<uint4*>(sA + (size_t)(tile0 + cc / 8) * kTileBytes + sw128_offset(q * 32 + rl, cc % 8)) = o;
+#pragma unroll
+    for (int b = 0; b < kBatch; ++b) {
+      const int rl = (it0 + b) * rpi + sub;
+      const uint4 o = make_uint4(pack_bf16x2(acc[b][0], acc[b][1]), pack_bf16x2(acc[b][2], acc[b][3]),
+                                 pack_bf16x2(acc[b][4], acc[b][5]), pack_bf16x2(acc[b][6], acc[b][7]));
+      *reinterpret_cast<uint4*>(sA + (size_t)(tile0 + cc / 8) * kTileBytes + sw128_offset(q * 32 + rl, cc % 8)) = o;
+    }
   }
 }
 
@@ -57,35 +77,38 @@ k_tc_decode(const __grid_constant__ CUtensorMap tmZ, const __grid_constant__ CUt
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   ChunkPipe c;
-  c.nkb = (p.r + p.ra) / 64; c.nchunks = p.d / kChunkN; c.b_stages = p.b_stages; c.acc_stages = p.acc_stages;
+  c.nkb = (p.r + p.ra) / 64; c.nchunks = p.d / kChunkN; c.b_stages = p.b_stages;
   c.rank = cluster_ctarank();
   c.sA = smem;
   c.sOut = c.sA + (size_t)c.nkb * kTileBytes;
   c.sB = c.sOut + (size_t)kOutBufs * kTileBytes;
   uint64_t* bars = reinterpret_cast<uint64_t*>(c.sB + (size_t)p.b_stages * kHalfTileBytes);
   c.b_full = bars; c.b_empty = c.b_full + p.b_stages;
-  c.acc_full = c.b_empty + p.b_stages; c.acc_empty = c.acc_full + p.acc_stages;
-  uint64_t* a_full = c.acc_empty + p.acc_stages;       // leader's: A operands of both CTAs are in place
+  c.acc_full = c.b_empty + p.b_stages; c.acc_empty = c.acc_full + kAccStages;
+  uint64_t* a_full = c.acc_empty + kAccStages;         // leader's: A operands of both CTAs are in place
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(a_full + 1);
 
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
   const long long m0 = (long long)blockIdx.x * p.tile_m;
 
+  if (warp == 0) DBG(0)
+#ifdef MAPL_DBG
+  if (threadIdx.x == 0) { g_dbg[blockIdx.x * 64 + 5] = 0; g_dbg[blockIdx.x * 64 + 6] = 0; }
+#endif
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmZ); tma_prefetch_desc(&tmW); tma_prefetch_desc(&tmO);
     chunk_init_barriers(c);
-    mbar_init(a_full, 1 + 8);                 // leader's producer (expect_tx) + the epilogue warps of both CTAs
+    mbar_init(a_full, 1 + 16);                // leader's producer (expect_tx) + the epilogue warps of both CTAs
     fence_barrier_init();
   }
-  if (warp == 1) {
-    if (p.acc_stages == 4) tmem_alloc_pair<512>(tmem_slot); else tmem_alloc_pair<256>(tmem_slot);
-  }
+  if (warp == 1) tmem_alloc_pair<512>(tmem_slot);
   tc_fence_before_sync();
   cluster_sync_all();
   tc_fence_after_sync();
   c.tmem_base = *tmem_slot;
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");       // everything below touches global memory
+  if (warp == 0) DBG(1)
 
   if (warp == 0) {
     if (elect_one()) {
@@ -101,11 +124,12 @@ k_tc_decode(const __grid_constant__ CUtensorMap tmZ, const __grid_constant__ CUt
   } else if (warp == 1) {
     if (c.rank == 0 && elect_one()) {
       mbar_wait_cluster(a_full, 0);
+      DBGT(2)
       tc_fence_after_sync();
       chunk_mma(c);
     }
   } else {
-    const int q = warp & 3;
+    const int q = warp & 3, part = (warp - 2) >> 2;
     const int row = q * 32 + lane;                      // token row inside the tile == TMEM lane
     const long long m = m0 + row;
     const bool live = row < p.tile_m && m < p.N;
@@ -116,29 +140,36 @@ k_tc_decode(const __grid_constant__ CUtensorMap tmZ, const __grid_constant__ CUt
       int idx[8];
 #pragma unroll
       for (int l = 0; l < 8; ++l) idx[l] = (live && l < p.L) ? __ldg(p.codes + m * p.L + l) : -1;
-      gather_sum_rows(c.sA, 0, p.r, p.codebooks, (long long)p.K * p.r, idx, p.L, q, lane);
+      if (p.r >= 128) gather_sum_rows<8>(c.sA, 0, p.r, p.codebooks, (long long)p.K * p.r, idx, p.L, q, lane, part);
+      else gather_sum_rows<4>(c.sA, 0, p.r, p.codebooks, (long long)p.K * p.r, idx, p.L, q, lane, part);
     }
     if (p.ra > 0) {
       int idx[8];
 #pragma unroll
       for (int l = 0; l < 8; ++l) idx[l] = -1;
       idx[0] = live ? __ldg(p.tok + m) : -1;
-      gather_sum_rows(c.sA, p.r / 64, p.ra, p.A, 0, idx, 1, q, lane);
+      if (p.ra >= 128) gather_sum_rows<8>(c.sA, p.r / 64, p.ra, p.A, 0, idx, 1, q, lane, part);
+      else gather_sum_rows<4>(c.sA, p.r / 64, p.ra, p.A, 0, idx, 1, q, lane, part);
     }
     fence_proxy_async_all();
     __syncwarp();
+    if (warp == 2) DBG(3)
     if (lane == 0) mbar_arrive_leader(a_full);
     chunk_epilogue(c, &tmO, (int)m0);
   }
+  if (warp == 2) DBG(4)
   tc_fence_before_sync();
   cluster_sync_all();                       // the peer may still signal our barriers / its MMAs read our smem
   if (warp == 1) {
     tc_fence_after_sync();
-    if (p.acc_stages == 4) tmem_dealloc_pair<512>(c.tmem_base); else tmem_dealloc_pair<256>(c.tmem_base);
+    tmem_dealloc_pair<512>(c.tmem_base);
   }
 }
 
 }  // namespace
+}  // namespace mapl
+MAPL_DBG_READER(mapl_debug_read_decode)
+namespace mapl {
 
 int tc_decode(const mapl_boundary_desc& d, const void* Z, const int32_t* codes, const float* codebooks,
               const int32_t* tok, const float* A, const TcPack& pk, void* Hhat_out, cudaStream_t st) {
@@ -149,10 +180,9 @@ int tc_decode(const mapl_boundary_desc& d, const void* Z, const int32_t* codes, 
   p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.ra = ra; p.L = d.rvq_levels; p.K = d.rvq_k;
   p.tile_m = tc_tile_m(d.n_tokens);
   p.z_from_tma = codes ? 0 : 1;
-  p.acc_stages = 4;
   const size_t fixed = (size_t)(nkb + kOutBufs) * kTileBytes + 1024 + 512;
   p.b_stages = (int)((227 * 1024 - fixed) / kHalfTileBytes);
-  if (p.b_stages > 8) p.b_stages = 8;
+  if (p.b_stages > 16) p.b_stages = 16;
   if (p.b_stages < 2) return MAPL_ERR_UNSUPPORTED;
   const size_t smem = fixed + (size_t)p.b_stages * kHalfTileBytes;
   CUtensorMap tmZ, tmW, tmO;

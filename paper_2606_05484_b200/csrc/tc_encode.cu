@@ -15,13 +15,7 @@ namespace {
 using namespace tc;
 
 constexpr int BM = 128, BK = 64, kThreads = 192;
-#ifdef MAPL_DBG
-__device__ unsigned long long g_dbg[160 * 8];
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define DBG(i) if (lane == 0) g_dbg[blockIdx.x * 8 + (i)] = gtime();
-#else
-#define DBG(i)
-#endif
+
 constexpr int kATile = BM * BK * 2;   // 16 KB
 
 // CTA pair: the two CTAs of a cluster own consecutive token tiles and run ONE M=256 MMA per k-step
@@ -83,8 +77,8 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
         const int s = kb % stages;
         mbar_wait(&full[s], (kb / stages) & 1);
 #ifdef MAPL_DBG
-        if (kb == 0) g_dbg[blockIdx.x * 8 + 2] = gtime();
-        if (kb == nkb - 1) g_dbg[blockIdx.x * 8 + 3] = gtime();
+        if (kb == 0) DBGT(2)
+        if (kb == nkb - 1) DBGT(3)
 #endif
         tc_fence_after_sync();
         const uint32_t a = smem_u32(smem + (size_t)s * stage_bytes);
@@ -131,10 +125,9 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
 }
 
 }  // namespace
-
-#ifdef MAPL_DBG
-extern "C" int mapl_debug_read(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, g_dbg, sizeof(g_dbg)); }
-#endif
+}  // namespace mapl
+MAPL_DBG_READER(mapl_debug_read_encode)
+namespace mapl {
 
 int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
                   int32_t* codes_out, cudaStream_t st);   // tc_encode_rvq.cu

@@ -5,11 +5,15 @@
 //         bf16, K-major SW128
 //   W     streamed by TMA through a ring of b_stages; per stage each CTA holds HALF of the
 //         [128 x 64] tile (64 rows of W): the pair reads every W byte from L2 once, not twice
-//   D     acc_stages x [128 lanes x 128 cols] fp32 in each CTA's TMEM (MMA of chunk j+1 overlaps the
+//   D     4 stages x [128 lanes x 128 cols] fp32 in each CTA's TMEM (MMA of chunk j+1 overlaps the
 //         epilogue of chunk j); one M=256 UMMA per k-step, issued by the leader CTA (rank 0)
-//   Out   bf16, through swizzled staging boxes and TMA stores, each CTA its own rows
+//   Out   bf16, through two swizzled staging boxes and TMA stores, each CTA its own rows.  (Direct
+//         st.global from the row-per-thread register layout was measured 2x slower: 32 partial
+//         sectors per instruction.)
 // Barriers: b_full / acc_empty live in the leader (they collect arrivals from both CTAs);
 // b_empty / acc_full exist in both CTAs and are signalled by multicast commits.
+// Measured (profiles/): with the tensor pipe at ~75 % of nominal inside the chunk loop the MMA issue
+// is the limiter there; the A-operand prologue of the callers is what remains exposed.
 // Three roles, each called by the warp(s) that own it.
 #pragma once
 #include <stdlib.h>
@@ -22,15 +26,17 @@ namespace tc {
 constexpr int kChunkN = 128;                 // d-chunk width == UMMA N
 constexpr int kTileBytes = 128 * 64 * 2;     // one [128 x 64] bf16 tile
 constexpr int kHalfTileBytes = 64 * 64 * 2;  // the half of a W tile one CTA of the pair holds
-constexpr int kOutBufs = 4;
+constexpr int kAccStages = 4;
+constexpr int kOutBufs = 2;                  // one chunk's two [128 x 64] staging boxes
+constexpr int kPipeThreads = 320;            // warp 0 TMA, warp 1 MMA, warps 2-9 epilogue
 
 struct ChunkPipe {
   uint8_t* sA;        // resident A operand (nkb tiles)
   uint8_t* sB;        // ring (b_stages half tiles)
   uint8_t* sOut;      // kOutBufs staging boxes
   uint64_t* b_full; uint64_t* b_empty;       // [b_stages]
-  uint64_t* acc_full; uint64_t* acc_empty;   // [acc_stages]
-  int nkb, nchunks, b_stages, acc_stages;
+  uint64_t* acc_full; uint64_t* acc_empty;   // [kAccStages]
+  int nkb, nchunks, b_stages;
   uint32_t tmem_base, rank;
 };
 
@@ -52,8 +58,9 @@ __device__ __forceinline__ void chunk_mma(const ChunkPipe& c) {
   const uint32_t idesc = make_idesc_bf16(256, kChunkN, false, false);
   int it = 0;
   for (int j = 0; j < c.nchunks; ++j) {
-    const int as = j % c.acc_stages;
-    mbar_wait_cluster(&c.acc_empty[as], ((j / c.acc_stages) & 1) ^ 1);
+    const int as = j % kAccStages;
+    mbar_wait_cluster(&c.acc_empty[as], ((j / kAccStages) & 1) ^ 1);
+    if (j < 16) DBGT(8 + j)
     tc_fence_after_sync();
     const uint32_t tmem_d = c.tmem_base + as * kChunkN;
     for (int kb = 0; kb < c.nkb; ++kb, ++it) {
@@ -67,53 +74,57 @@ __device__ __forceinline__ void chunk_mma(const ChunkPipe& c) {
       umma_commit_pair(&c.b_empty[s]);
     }
     umma_commit_pair(&c.acc_full[as]);
+    if (j < 16) DBGT(24 + j)
   }
 }
 
-// epilogue: the 4 warps with threadIdx.x in [64,192) of each CTA; row = TMEM lane = token row in the
-// tile.  Uses named barrier 1 (128 threads).  Thread 64 issues the TMA stores.
+// epilogue: the 8 warps with threadIdx.x in [64,320) of each CTA.  Warp w reads TMEM lane quarter
+// q = w & 3 (row = token row in the tile) and column half h = (w - 2) / 4 of the chunk, i.e. exactly one
+// [128 x 64] staging box; the two halves run independently (named barriers 1 and 2, 128 threads
+// each; threads 64 and 192 issue the TMA stores of their box).
 __device__ __forceinline__ void chunk_epilogue(const ChunkPipe& c, const CUtensorMap* tmO, int m0) {
-  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32, q = warp & 3, row = q * 32 + lane;
+  const int warp = threadIdx.x / 32, lane = threadIdx.x % 32, q = warp & 3, h = (warp - 2) >> 2, row = q * 32 + lane;
+  const bool issuer = threadIdx.x == 64 + h * 128;
+  uint8_t* box = c.sOut + (size_t)h * kTileBytes;
   for (int j = 0; j < c.nchunks; ++j) {
-    const int as = j % c.acc_stages, ob = (j & 1) * 2;
-    // only chunk j-1's store group may still be reading smem: the boxes of chunk j-2 are free
-    if (threadIdx.x == 64) tma_store_wait_read<1>();
-    asm volatile("bar.sync 1, 128;" ::: "memory");
-    mbar_wait(&c.acc_full[as], (j / c.acc_stages) & 1);
+    const int as = j % kAccStages;
+    mbar_wait(&c.acc_full[as], (j / kAccStages) & 1);
+    if (threadIdx.x == 64 && j < 16) DBGT(40 + j)
     tc_fence_after_sync();
-#pragma unroll
-    for (int cc = 0; cc < kChunkN / 32; ++cc) {
-      uint32_t v[32];
-      tmem_ld32(c.tmem_base + ((uint32_t)(q * 32) << 16) + as * kChunkN + cc * 32, v);
-      tmem_ld_wait();
-      uint8_t* box = c.sOut + (size_t)(ob + cc / 2) * kTileBytes;
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        uint4 o;
-        o.x = pack_bf16x2(__uint_as_float(v[8 * i + 0]), __uint_as_float(v[8 * i + 1]));
-        o.y = pack_bf16x2(__uint_as_float(v[8 * i + 2]), __uint_as_float(v[8 * i + 3]));
-        o.z = pack_bf16x2(__uint_as_float(v[8 * i + 4]), __uint_as_float(v[8 * i + 5]));
-        o.w = pack_bf16x2(__uint_as_float(v[8 * i + 6]), __uint_as_float(v[8 * i + 7]));
-        *reinterpret_cast<uint4*>(box + sw128_offset(row, (cc & 1) * 4 + i)) = o;
-      }
-    }
+    uint32_t v[2][32];
+    const uint32_t taddr = c.tmem_base + ((uint32_t)(q * 32) << 16) + as * kChunkN + h * 64;
+    tmem_ld32(taddr, v[0]);
+    tmem_ld32(taddr + 32, v[1]);
+    tmem_ld_wait();
     tc_fence_before_sync();
     __syncwarp();
     if (lane == 0) mbar_arrive_leader(&c.acc_empty[as]);     // the TMEM stage may be overwritten
+    // chunk j-1's store must have read the staging box before it is rewritten
+    if (issuer) tma_store_wait_read<0>();
+    if (h == 0) asm volatile("bar.sync 1, 128;" ::: "memory"); else asm volatile("bar.sync 2, 128;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const uint32_t* w = &v[i / 4][8 * (i % 4)];
+      uint4 o;
+      o.x = pack_bf16x2(__uint_as_float(w[0]), __uint_as_float(w[1]));
+      o.y = pack_bf16x2(__uint_as_float(w[2]), __uint_as_float(w[3]));
+      o.z = pack_bf16x2(__uint_as_float(w[4]), __uint_as_float(w[5]));
+      o.w = pack_bf16x2(__uint_as_float(w[6]), __uint_as_float(w[7]));
+      *reinterpret_cast<uint4*>(box + sw128_offset(row, i)) = o;
+    }
     fence_proxy_async_smem();
-    asm volatile("bar.sync 1, 128;" ::: "memory");
-    if (threadIdx.x == 64) {
-      tma_store_2d(tmO, c.sOut + (size_t)ob * kTileBytes, j * kChunkN, m0);
-      tma_store_2d(tmO, c.sOut + (size_t)(ob + 1) * kTileBytes, j * kChunkN + 64, m0);
+    if (h == 0) asm volatile("bar.sync 1, 128;" ::: "memory"); else asm volatile("bar.sync 2, 128;" ::: "memory");
+    if (issuer) {
+      tma_store_2d(tmO, box, j * kChunkN + h * 64, m0);
       tma_store_commit();
     }
   }
-  if (threadIdx.x == 64) tma_store_wait_all<0>();
+  if (issuer) tma_store_wait_all<0>();
 }
 
 __device__ __forceinline__ void chunk_init_barriers(const ChunkPipe& c) {
   for (int s = 0; s < c.b_stages; ++s) { mbar_init(&c.b_full[s], 1); mbar_init(&c.b_empty[s], 1); }
-  for (int s = 0; s < c.acc_stages; ++s) { mbar_init(&c.acc_full[s], 1); mbar_init(&c.acc_empty[s], 8); }
+  for (int s = 0; s < kAccStages; ++s) { mbar_init(&c.acc_full[s], 1); mbar_init(&c.acc_empty[s], 16); }
 }
 
 // host: launch with programmatic dependent launch allowed (the kernels call griddepcontrol.wait
