@@ -265,8 +265,8 @@ __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; as
 #define DBGT(i) { g_dbg[blockIdx.x * 64 + (i)] = gtime(); }
 #define DBG(i) if (lane == 0) DBGT(i)
 #else
-#define DBGT(i)
-#define DBG(i)
+#define DBGT(i) {}
+#define DBG(i) {}
 #define MAPL_DBG_READER(name)
 #endif
 

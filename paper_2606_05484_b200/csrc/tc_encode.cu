@@ -144,6 +144,7 @@ int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks
   int stages = (200 * 1024) / stage_bytes;
   if (stages > 8) stages = 8;
   if (stages > d.d / BK) stages = d.d / BK;
+  if (const char* e = getenv("MAPL_ENC_STAGES")) { int v = atoi(e); if (v >= 2 && v < stages) stages = v; }   // experiment
   const size_t smem = (size_t)stages * stage_bytes + 1024 + 256;
   static bool attr_done = false;
   if (!attr_done) {

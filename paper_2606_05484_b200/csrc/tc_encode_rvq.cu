@@ -29,10 +29,10 @@ namespace mapl {
 namespace {
 using namespace tc;
 
-constexpr int kThreads = 192;
+constexpr int kThreads = kPipeThreads;   // warp 0 TMA, warp 1 MMA, warps 2-9 scan / re-score (two per TMEM lane quarter)
 constexpr int kChunk = 128;        // codewords per accumulator stage (UMMA N)
 constexpr int kAccCol0 = 256;      // TMEM column of score stage 0
-constexpr int kNE = 12;            // candidate-list entries per token (one entry = one 32-codeword piece)
+constexpr int kNE = 8;             // candidate-list entries per thread (one entry = one 32-codeword piece)
 
 struct RvqParams {
   const float* C;        // [L,K,r] fp32 codebooks (exact re-scoring, residual update)
@@ -48,10 +48,11 @@ struct RvqParams {
 
 // smem carve-up (after 1024-byte alignment):
 //   region R  = max(phase-1 ring, rho operand tiles + codebook ring)
-//   sHn [K] fp32 | candidate lists [kNE][128] x (m32, piece, mask) | barriers | tmem slot
+//   sHn [K] fp32 | candidate lists [kNE][256] x (m32, piece, mask) | exchange [5][2][128] | barriers | tmem slot
 struct Smem {
   uint8_t* ring1; uint8_t* sRho; uint8_t* ringC;
   float* sHn; float* eM; int* eP; uint32_t* eMask;
+  float* xch;            // [5][2][128]: per (half, token) best / score / k / n2 / amax exchanged by the two warps of a quarter
   uint64_t* s1_full; uint64_t* s1_empty; uint64_t* z_full;
   uint64_t* c_full; uint64_t* c_empty; uint64_t* acc_full; uint64_t* acc_empty; uint64_t* rho_ready;
   uint32_t* tmem_slot;
@@ -63,7 +64,7 @@ __host__ __device__ inline size_t rvq_regionR(const RvqParams& p) {
   return ring1 > lvl ? ring1 : lvl;
 }
 __host__ __device__ inline size_t rvq_tail_bytes(const RvqParams& p) {
-  return (size_t)p.K * 4 + (size_t)kNE * 128 * 12 + 1024;
+  return (size_t)p.K * 4 + (size_t)kNE * 256 * 12 + 5 * 2 * 128 * 4 + 1024;
 }
 
 __device__ __forceinline__ Smem carve_smem(uint8_t* base, const RvqParams& p) {
@@ -73,9 +74,10 @@ __device__ __forceinline__ Smem carve_smem(uint8_t* base, const RvqParams& p) {
   s.ringC = base + (size_t)(p.r / 64) * kTileBytes;
   uint8_t* t = base + rvq_regionR(p);
   s.sHn = reinterpret_cast<float*>(t); t += (size_t)p.K * 4;
-  s.eM = reinterpret_cast<float*>(t); t += kNE * 128 * 4;
-  s.eP = reinterpret_cast<int*>(t); t += kNE * 128 * 4;
-  s.eMask = reinterpret_cast<uint32_t*>(t); t += kNE * 128 * 4;
+  s.eM = reinterpret_cast<float*>(t); t += kNE * 256 * 4;
+  s.eP = reinterpret_cast<int*>(t); t += kNE * 256 * 4;
+  s.eMask = reinterpret_cast<uint32_t*>(t); t += kNE * 256 * 4;
+  s.xch = reinterpret_cast<float*>(t); t += 5 * 2 * 128 * 4;
   uint64_t* b = reinterpret_cast<uint64_t*>(t);
   s.s1_full = b; b += p.stages1;
   s.s1_empty = b; b += p.stages1;
@@ -113,13 +115,14 @@ __device__ __forceinline__ float exact_score(uint32_t tmem_row, const float* __r
   return hn - dot;
 }
 
-// rho <- rho - sub (sub == nullptr: rho unchanged); returns ||rho||^2; writes fp16(rho * 2^-e) into
-// the swizzled A-operand tiles, 2^-e chosen so that max|rho_j| 2^-e lies in [0.5,1); *unscale = 2^e.
-// Warp-convergent.
-__device__ __forceinline__ float update_rho(uint32_t tmem_row, const float* __restrict__ sub, uint8_t* sRho, int row, int r,
-                                            float* unscale) {
+// The two warps of a TMEM lane quarter split the residual by 32-column pieces: warp half h owns the
+// pieces pc with (pc & 1) == h.
+// Step 1 of a residual update: rho <- rho - sub on the own pieces (sub == nullptr: rho unchanged);
+// returns the partial ||rho||^2 and max|rho_j| of those pieces.  Warp-convergent.
+__device__ __forceinline__ void rho_subtract(uint32_t tmem_row, const float* __restrict__ sub, int r, int h, float* n2_out,
+                                             float* amax_out) {
   float n2 = 0.f, amax = 0.f;
-  for (int pc = 0; pc < r / 32; ++pc) {
+  for (int pc = h; pc < r / 32; pc += 2) {
     uint32_t v[32];
     tmem_ld32(tmem_row + pc * 32, v);
     tmem_ld_wait();
@@ -143,11 +146,16 @@ __device__ __forceinline__ float update_rho(uint32_t tmem_row, const float* __re
     }
   }
   if (sub != nullptr) tmem_st_wait();
+  *n2_out = n2; *amax_out = amax;
+}
+
+// Step 2: fp16(rho * 2^-e) of the own pieces into the swizzled A-operand tiles, 2^-e chosen from the
+// row's max|rho_j| so that it lands in [0.5,1); returns 2^e.  Warp-convergent.
+__device__ __forceinline__ float rho_to_operand(uint32_t tmem_row, uint8_t* sRho, int row, int r, int h, float amax) {
   int eb = (int)((__float_as_uint(amax) >> 23) & 0xffu);
   eb = eb < 2 ? 126 : (eb > 250 ? 250 : eb);
   const float inv = __uint_as_float((uint32_t)(253 - eb) << 23);
-  *unscale = __uint_as_float((uint32_t)(eb + 1) << 23);
-  for (int pc = 0; pc < r / 32; ++pc) {
+  for (int pc = h; pc < r / 32; pc += 2) {
     uint32_t v[32];
     tmem_ld32(tmem_row + pc * 32, v);
     tmem_ld_wait();
@@ -162,7 +170,7 @@ __device__ __forceinline__ float update_rho(uint32_t tmem_row, const float* __re
       *reinterpret_cast<uint4*>(tile + sw128_offset(row, (pc & 1) * 4 + i)) = o;
     }
   }
-  return n2;
+  return __uint_as_float((uint32_t)(eb + 1) << 23);
 }
 
 __global__ void __launch_bounds__(kThreads, 1)
@@ -183,8 +191,8 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
     for (int i = 0; i < p.stages1; ++i) { mbar_init(&s.s1_full[i], 1); mbar_init(&s.s1_empty[i], 1); }
     mbar_init(s.z_full, 1);
     for (int i = 0; i < p.ring_tiles; ++i) { mbar_init(&s.c_full[i], 1); mbar_init(&s.c_empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&s.acc_full[i], 1); mbar_init(&s.acc_empty[i], 8); }
-    mbar_init(s.rho_ready, 8);                // leader's barriers collect the epilogue warps of both CTAs
+    for (int i = 0; i < 2; ++i) { mbar_init(&s.acc_full[i], 1); mbar_init(&s.acc_empty[i], 16); }
+    mbar_init(s.rho_ready, 16);               // leader's barriers collect the epilogue warps of both CTAs
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc_pair<512>(s.tmem_slot);
@@ -194,6 +202,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
   const uint32_t tmem_base = *s.tmem_slot;
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");       // everything below touches global memory
+  if (warp == 0) { DBG(0) }
 
   if (warp == 0) {
     // ------------------------------------------------------------ TMA producer
@@ -247,6 +256,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         for (int c = 0; c < nchunks; ++c, ++cg) {
           const int as = cg & 1;
           mbar_wait_cluster(&s.acc_empty[as], ((cg >> 1) & 1) ^ 1);
+          if (cg < 8) DBGT(24 + cg)
           tc_fence_after_sync();
           const uint32_t tmem_d = tmem_base + kAccCol0 + as * kChunk;
           for (int kb = 0; kb < nkb; ++kb, ++it) {
@@ -260,33 +270,48 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
             umma_commit_pair(&s.c_empty[st]);
           }
           umma_commit_pair(&s.acc_full[as]);
+          if (cg < 8) DBGT(32 + cg)
         }
       }
     }
   } else {
-    // ------------------------------------------------------------ epilogue: thread = token
-    const int q = warp & 3, row = q * 32 + lane, et = threadIdx.x - 64;
+    // ------------------------------------------------------------ epilogue: 8 warps, two threads per token
+    // q = TMEM lane quarter, h = which half of the 32-codeword pieces / 32-column pieces this warp owns
+    const int q = warp & 3, h = (warp - 2) >> 2, row = q * 32 + lane, et = threadIdx.x - 64;
     const long long m = m0 + row;
     const bool live = row < p.tile_m && m < p.N;
     const uint32_t tmem_row = tmem_base + ((uint32_t)(q * 32) << 16);
     const unsigned full = 0xffffffffu;
+    float* xBest = s.xch; float* xScore = s.xch + 256; int* xK = reinterpret_cast<int*>(s.xch + 512);
+    float* xN2 = s.xch + 768; float* xAmax = s.xch + 1024;
+    const int mine = h * 128 + row, other = (1 - h) * 128 + row;
+    float* eM = s.eM + mine; int* eP = s.eP + mine; uint32_t* eMask = s.eMask + mine;   // entry e at [e * 256]
+    int code_l[8];
+#pragma unroll
+    for (int l = 0; l < 8; ++l) code_l[l] = 0;
 
     mbar_wait(s.z_full, 0);
+    if (warp == 2) { DBG(1) }
     tc_fence_after_sync();
-    float unscale;
-    float n2 = update_rho(tmem_row, nullptr, s.sRho, row, p.r, &unscale);
+    float n2, amax;
+    rho_subtract(tmem_row, nullptr, p.r, h, &n2, &amax);
+    xN2[mine] = n2; xAmax[mine] = amax;
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    n2 += xN2[other]; amax = fmaxf(amax, xAmax[other]);
+    float unscale = rho_to_operand(tmem_row, s.sRho, row, p.r, h, amax);
     fence_proxy_async_all();
     tc_fence_before_sync();
     __syncwarp();
     if (lane == 0) mbar_arrive_leader(s.rho_ready);
 
     int cg = 0;
+#pragma unroll 1
     for (int l = 0; l < p.L; ++l) {
       const float* Cl = p.C + (long long)l * p.K * p.r;
-      asm volatile("bar.sync 1, 128;" ::: "memory");        // previous level's sHn no longer read
-      for (int i = et; i < p.K / 4; i += 128)
+      for (int i = et; i < p.K / 4; i += 256)
         reinterpret_cast<float4*>(s.sHn)[i] = __ldg(reinterpret_cast<const float4*>(p.hn + (long long)l * p.K) + i);
-      asm volatile("bar.sync 1, 128;" ::: "memory");
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      if (warp == 2 && l < 4) { DBG(4 + l * 4) }
       const float margin = 0.001953125f * 1.05f * sqrtf(n2) * __ldg(p.cmax + l);
       const float nsc = -unscale * __ldg(p.cscale + 8 + l);     // coarse S -> rho.c
 
@@ -296,21 +321,28 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       for (int c = 0; c < nchunks; ++c, ++cg) {
         const int as = cg & 1;
         mbar_wait(&s.acc_full[as], (cg >> 1) & 1);
+        if (threadIdx.x == 64 && cg < 8) DBGT(40 + cg)
         tc_fence_after_sync();
-#pragma unroll 1
-        for (int pc = 0; pc < kChunk / 32; ++pc) {
-          uint32_t v[32];
-          tmem_ld32(tmem_row + kAccCol0 + as * kChunk + pc * 32, v);
-          const float4* h4 = reinterpret_cast<const float4*>(s.sHn + c * kChunk + pc * 32);
+        uint32_t v[2][32];                     // this warp's two pieces of the chunk: h and h + 2
+        tmem_ld32(tmem_row + kAccCol0 + as * kChunk + h * 32, v[0]);
+        tmem_ld32(tmem_row + kAccCol0 + as * kChunk + (h + 2) * 32, v[1]);
+        tmem_ld_wait();
+        tc_fence_before_sync();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_leader(&s.acc_empty[as]);     // scores are in registers: the stage is free
+        if (threadIdx.x == 64 && cg < 8) DBGT(48 + cg)
+#pragma unroll
+        for (int pp = 0; pp < 2; ++pp) {
+          const int piece = c * (kChunk / 32) + h + 2 * pp;
+          const float4* h4 = reinterpret_cast<const float4*>(s.sHn + piece * 32);
           float sc[32];
-          tmem_ld_wait();
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
-            const float4 h = h4[i];
-            sc[4 * i + 0] = fmaf(__uint_as_float(v[4 * i + 0]), nsc, h.x);
-            sc[4 * i + 1] = fmaf(__uint_as_float(v[4 * i + 1]), nsc, h.y);
-            sc[4 * i + 2] = fmaf(__uint_as_float(v[4 * i + 2]), nsc, h.z);
-            sc[4 * i + 3] = fmaf(__uint_as_float(v[4 * i + 3]), nsc, h.w);
+            const float4 hh = h4[i];
+            sc[4 * i + 0] = fmaf(__uint_as_float(v[pp][4 * i + 0]), nsc, hh.x);
+            sc[4 * i + 1] = fmaf(__uint_as_float(v[pp][4 * i + 1]), nsc, hh.y);
+            sc[4 * i + 2] = fmaf(__uint_as_float(v[pp][4 * i + 2]), nsc, hh.z);
+            sc[4 * i + 3] = fmaf(__uint_as_float(v[pp][4 * i + 3]), nsc, hh.w);
           }
           float mn[8];
 #pragma unroll
@@ -326,36 +358,33 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
               if (cnt == kNE) {                 // list full: drop entries the tighter threshold excludes
                 int j = 0;
                 for (int e = 0; e < kNE; ++e) {
-                  const float em = s.eM[e * 128 + row];
-                  if (em <= thr) {
-                    s.eM[j * 128 + row] = em; s.eP[j * 128 + row] = s.eP[e * 128 + row];
-                    s.eMask[j * 128 + row] = s.eMask[e * 128 + row]; ++j;
-                  }
+                  const float em = eM[e * 256];
+                  if (em <= thr) { eM[j * 256] = em; eP[j * 256] = eP[e * 256]; eMask[j * 256] = eMask[e * 256]; ++j; }
                 }
                 cnt = j;
               }
               if (cnt == kNE) {
                 overflow = true;                // pathological (e.g. many duplicate codewords): exhaustive below
               } else {
-                s.eM[cnt * 128 + row] = m32; s.eP[cnt * 128 + row] = c * (kChunk / 32) + pc;
-                s.eMask[cnt * 128 + row] = mask; ++cnt;
+                eM[cnt * 256] = m32; eP[cnt * 256] = piece; eMask[cnt * 256] = mask; ++cnt;
               }
             }
           }
         }
-        tc_fence_before_sync();
-        __syncwarp();
-        if (lane == 0) mbar_arrive_leader(&s.acc_empty[as]);
       }
+      xBest[mine] = best;
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      best = fminf(best, xBest[other]);
+      if (warp == 2 && l < 4) { DBG(5 + l * 4) }
 
-      // ---- exact fp32 re-scoring of the candidates, ascending k, strict '<': lowest index wins ties
+      // ---- exact fp32 re-scoring of this thread's candidates, ascending k, strict '<': lowest index wins ties
       const float thr = best + margin;
       float bestx = FLT_MAX;
-      int bestk = 0, e = 0, piece = 0;
+      int bestk = 0x7fffffff, e = 0, piece = 0;
       uint32_t mrem = 0;
       while (true) {
         while (mrem == 0 && e < cnt) {
-          if (s.eM[e * 128 + row] <= thr) { mrem = s.eMask[e * 128 + row]; piece = s.eP[e * 128 + row]; }
+          if (eM[e * 256] <= thr) { mrem = eMask[e * 256]; piece = eP[e * 256]; }
           ++e;
         }
         const bool have = mrem != 0 && !overflow;
@@ -365,15 +394,32 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         const float sx = exact_score(tmem_row, Cl + (long long)k * p.r, s.sHn[k], p.r);
         if (have && sx < bestx) { bestx = sx; bestk = k; }
       }
-      if (__any_sync(full, overflow)) {
-        for (int k = 0; k < p.K; ++k) {
-          const float sx = exact_score(tmem_row, Cl + (long long)k * p.r, s.sHn[k], p.r);
-          if (overflow && sx < bestx) { bestx = sx; bestk = k; }
-        }
+      if (__any_sync(full, overflow)) {         // exhaustive over the pieces this warp owns
+        for (int pc = h; pc < p.K / 32; pc += 2)
+          for (int i = 0; i < 32; ++i) {
+            const int k = pc * 32 + i;
+            const float sx = exact_score(tmem_row, Cl + (long long)k * p.r, s.sHn[k], p.r);
+            if (overflow && sx < bestx) { bestx = sx; bestk = k; }
+          }
       }
-      if (live) p.codes[m * p.L + l] = bestk;
+      xScore[mine] = bestx; xK[mine] = bestk;
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      {
+        const float ox = xScore[other];
+        const int ok = xK[other];
+        if (ox < bestx || (ox == bestx && ok < bestk)) { bestx = ox; bestk = ok; }
+      }
+      if (bestk == 0x7fffffff) bestk = 0;       // dead rows
+#pragma unroll
+      for (int ll = 0; ll < 8; ++ll) if (ll == l) code_l[ll] = bestk;
+      if (warp == 2 && l < 4) { DBG(6 + l * 4) }
+      if (live && h == 0) p.codes[m * p.L + l] = bestk;
       if (l + 1 < p.L) {
-        n2 = update_rho(tmem_row, Cl + (long long)bestk * p.r, s.sRho, row, p.r, &unscale);
+        rho_subtract(tmem_row, Cl + (long long)bestk * p.r, p.r, h, &n2, &amax);
+        xN2[mine] = n2; xAmax[mine] = amax;
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        n2 += xN2[other]; amax = fmaxf(amax, xAmax[other]);
+        unscale = rho_to_operand(tmem_row, s.sRho, row, p.r, h, amax);
         fence_proxy_async_all();
         tc_fence_before_sync();
         __syncwarp();
@@ -381,13 +427,17 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       }
     }
 
+    if (warp == 2) { DBG(2) }
     if (p.Zq != nullptr && live) {                          // zhat = sum_l C[l, code_l, :], rounded once
-      for (int cc = 0; cc < p.r / 8; ++cc) {
+      for (int cc = h; cc < p.r / 8; cc += 2) {
         float a[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-        for (int l = 0; l < p.L; ++l) {
-          const float4* src = reinterpret_cast<const float4*>(p.C + ((long long)l * p.K + p.codes[m * p.L + l]) * p.r + cc * 8);
-          const float4 x = __ldg(src), y = __ldg(src + 1);
-          a[0] += x.x; a[1] += x.y; a[2] += x.z; a[3] += x.w; a[4] += y.x; a[5] += y.y; a[6] += y.z; a[7] += y.w;
+#pragma unroll
+        for (int l = 0; l < 8; ++l) {
+          if (l < p.L) {
+            const float4* src = reinterpret_cast<const float4*>(p.C + ((long long)l * p.K + code_l[l]) * p.r + cc * 8);
+            const float4 x = __ldg(src), y = __ldg(src + 1);
+            a[0] += x.x; a[1] += x.y; a[2] += x.z; a[3] += x.w; a[4] += y.x; a[5] += y.y; a[6] += y.z; a[7] += y.w;
+          }
         }
         *reinterpret_cast<uint4*>(p.Zq + m * p.r + cc * 8) =
             make_uint4(pack_bf16x2(a[0], a[1]), pack_bf16x2(a[2], a[3]), pack_bf16x2(a[4], a[5]), pack_bf16x2(a[6], a[7]));
@@ -403,6 +453,9 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 }
 
 }  // namespace
+}  // namespace mapl
+MAPL_DBG_READER(mapl_debug_read_rvq)
+namespace mapl {
 
 int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
                   int32_t* codes_out, cudaStream_t st) {
