@@ -71,6 +71,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
   const long long m0 = (long long)blockIdx.x * p.tile_m;
 
+  if (warp == 0) DBG(56)
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmG); tma_prefetch_desc(&tmWu); tma_prefetch_desc(&tmWb);
     tma_prefetch_desc(&tmWd); tma_prefetch_desc(&tmO);
@@ -87,6 +88,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   c.tmem_base = *tmem_slot;
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
+  if (warp == 0) DBG(57)
 
   if (warp == 0) {
     if (elect_one()) {
@@ -149,6 +151,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
       }
     }
     mbar_wait(acc1_full, 0);
+    if (warp == 2) DBG(58)
     tc_fence_after_sync();
     for (int cc = half; cc < p.r / 32; cc += 2) {       // 32-column pieces alternate between the two warps
       uint32_t v[32];
@@ -183,9 +186,11 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
       tc_fence_before_sync();
       fence_proxy_async_all();
       __syncwarp();
+      if (warp == 2) DBG(59)
       if (lane == 0) mbar_arrive_leader(gz_full);
       chunk_epilogue(c, &tmO, (int)m0);
     }
+    if (warp == 2) DBG(60)
   }
   tc_fence_before_sync();
   cluster_sync_all();
@@ -205,22 +210,33 @@ struct BwdDuParams {
 };
 
 // dA[tok_n, :] += gA[n, :] for the 128-token blocks this CTA owns; called by the 128 epilogue threads.
-// Per block: the token ids are ranked (counting sort, 128 broadcast reads per thread), then every
-// thread owns one column and walks a run of the sorted order, summing rows of equal id in a
-// register and issuing one red.global.add per (distinct id, column): no shared-memory atomics, and a
-// hot Zipf id costs one global row per block instead of one per occurrence.
-__device__ __forceinline__ void scatter_gA(const BwdDuParams& p, float* sG, int* sTok, int cta, int n_ctas) {
-  const int et = threadIdx.x - 64, pitch = p.ra + 4, vpr = p.ra / 4;
+// Per block: all gA rows are staged in shared memory (every load in flight before the first store),
+// the token ids are ranked (counting sort, 128 broadcast reads per thread), then the thread that holds
+// the FIRST sorted position of an id sums the rows of that id in registers and issues one
+// red.global.add.v4 row: no shared-memory atomics, and a hot Zipf id costs one global row per
+// block instead of one per occurrence.
+template <int kRa>
+__device__ __forceinline__ void scatter_gA_t(const BwdDuParams& p, float* sG, int* sTok, int cta, int n_ctas) {
+  constexpr int kPitch = kRa + 4, kVpr = kRa / 4, kLoads = kVpr;      // 128 rows * kVpr float4 / 128 threads
+  const int et = threadIdx.x - 64;
   int* sSorted = sTok + 128;      // token id at each sorted position
   int* sOrder = sTok + 256;       // source row of each sorted position
-  const int col = et % p.ra, nseg = 128 / p.ra, seg = et / p.ra, seglen = 128 / nseg;
   for (long long base = (long long)cta * 128; base < p.N; base += (long long)n_ctas * 128) {
     const int cnt = (int)(p.N - base < 128 ? p.N - base : 128);
-    const float4* src = reinterpret_cast<const float4*>(p.gA + base * p.ra);
-    for (int i = et; i < cnt * vpr; i += 128)
-      *reinterpret_cast<float4*>(sG + (i / vpr) * pitch + (i % vpr) * 4) = __ldg(src + i);
+    const float4* src = reinterpret_cast<const float4*>(p.gA + base * kRa);
     const int my = et < cnt ? __ldg(p.tok + base + et) : 0x7fffffff;
+    float4 x[kLoads];
+#pragma unroll
+    for (int i = 0; i < kLoads; ++i) {
+      const int f = et + i * 128;                     // float4 index inside the block
+      x[i] = f < cnt * kVpr ? __ldg(src + f) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
     sTok[et] = my;
+#pragma unroll
+    for (int i = 0; i < kLoads; ++i) {
+      const int f = et + i * 128;
+      *reinterpret_cast<float4*>(sG + (f / kVpr) * kPitch + (f % kVpr) * 4) = x[i];
+    }
     asm volatile("bar.sync 1, 128;" ::: "memory");
     int rank = 0;
 #pragma unroll 8
@@ -231,20 +247,28 @@ __device__ __forceinline__ void scatter_gA(const BwdDuParams& p, float* sG, int*
     sSorted[rank] = my;
     sOrder[rank] = et;
     asm volatile("bar.sync 1, 128;" ::: "memory");
-    float acc = 0.f;
-    const int p0 = seg * seglen, p1 = p0 + seglen;
-    int cur = sSorted[p0];
-    for (int pos = p0; pos < p1; ++pos) {
-      const int nxt = pos + 1 < p1 ? sSorted[pos + 1] : -1;
-      acc += sG[sOrder[pos] * pitch + col];
-      if (nxt != cur) {
-        if (cur != 0x7fffffff) atomicAdd(p.dA + (long long)cur * p.ra + col, acc);   // result unused: RED
-        acc = 0.f;
-        cur = nxt;
+    // thread et owns sorted position et
+    const int id = sSorted[et];
+    const bool head = id != 0x7fffffff && (et == 0 || sSorted[et - 1] != id);
+    if (head) {
+      float4 acc[kVpr];
+      const float4* r0 = reinterpret_cast<const float4*>(sG + sOrder[et] * kPitch);
+#pragma unroll
+      for (int c = 0; c < kVpr; ++c) acc[c] = r0[c];
+      for (int pos = et + 1; pos < 128 && sSorted[pos] == id; ++pos) {
+        const float4* rr = reinterpret_cast<const float4*>(sG + sOrder[pos] * kPitch);
+#pragma unroll
+        for (int c = 0; c < kVpr; ++c) { const float4 v = rr[c]; acc[c].x += v.x; acc[c].y += v.y; acc[c].z += v.z; acc[c].w += v.w; }
       }
+      float* dst = p.dA + (long long)id * kRa;
+#pragma unroll
+      for (int c = 0; c < kVpr; ++c) red_add_v4(dst + c * 4, acc[c].x, acc[c].y, acc[c].z, acc[c].w);
     }
     asm volatile("bar.sync 1, 128;" ::: "memory");
   }
+}
+__device__ __forceinline__ void scatter_gA(const BwdDuParams& p, float* sG, int* sTok, int cta, int n_ctas) {
+  if (p.ra == 64) scatter_gA_t<64>(p, sG, sTok, cta, n_ctas); else scatter_gA_t<128>(p, sG, sTok, cta, n_ctas);
 }
 
 __global__ void __launch_bounds__(kThreadsDu, 1)
@@ -283,8 +307,16 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
 
+#ifdef MAPL_DBG
+  const int dbg_cta = blockIdx.y * gridDim.x + blockIdx.x;
+#define DU_DBG(i) { if (dbg_cta < 320) g_dbg[dbg_cta * 64 + (i)] = gtime(); }
+#else
+#define DU_DBG(i) {}
+#endif
+  if (threadIdx.x == 0) DU_DBG(0)
   if (warp >= 2 && p.tok != nullptr)
     scatter_gA(p, sG, sTok, blockIdx.y * gridDim.x + blockIdx.x, gridDim.x * gridDim.y);
+  if (threadIdx.x == 64) DU_DBG(1)
   if (n_items > 0) {
     if (warp == 0) {
       if (elect_one()) {
@@ -306,6 +338,8 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         for (int it = 0; it < n_items; ++it) {
           const int s = it % p.stages;
           mbar_wait(&full[s], (it / p.stages) & 1);
+          if (it == 0) DU_DBG(2)
+          if (it == n_items - 1) DU_DBG(3)
           tc_fence_after_sync();
           const uint32_t a = smem_u32(smem + (size_t)s * p.item_bytes), b = a + 2 * kBox;
 #pragma unroll
@@ -320,6 +354,7 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
       const int q = warp & 3, row = q * 32 + lane;
       float* dst = p.dU + ((long long)dt * 128 + row) * p.r;
       mbar_wait(acc_full, 0);
+      if (threadIdx.x == 64) DU_DBG(4)
       tc_fence_after_sync();
       for (int cc = 0; cc < p.r / 32; ++cc) {
         uint32_t v[32];
@@ -332,6 +367,7 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
       }
     }
   }
+  if (threadIdx.x == 64) DU_DBG(5)
   tc_fence_before_sync();
   __syncthreads();
   if (warp == 1) {
@@ -359,6 +395,9 @@ __global__ void k_tc_dequant_bf16(const int32_t* __restrict__ codes, const float
 }
 
 }  // namespace
+}  // namespace mapl
+MAPL_DBG_READER(mapl_debug_read_bwd)
+namespace mapl {
 
 int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const void* Z, const int32_t* codes,
                 const float* codebooks, const int32_t* tok, const float* A, const TcPack& pk, void* gz_out,
