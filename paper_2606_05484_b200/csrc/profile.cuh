@@ -25,6 +25,7 @@ enum KernelId {
   KID_TC_BWD_DU,
   KID_TC_ENCODE_RVQ,
   KID_TC_SCATTER,
+  KID_ST_GEMM,
   KID_COUNT
 };
 

@@ -194,28 +194,122 @@ StWs st_carve(int d, int r, int batch) {
   return w;
 }
 
-// Gm[b] = X[b]^T X2[b]  ([r,r], split-K over d with atomics)
+// ---------------------------------------------------------------- fp32 FFMA GEMMs of the step
+// 64x64 output tile, BK = 16, 256 threads x (4x4), register-prefetched double buffering, 128-bit
+// global and shared accesses.  Two shapes:
+//   kGram : C[r,r] (+)= X[k0:k1, :]^T Y[k0:k1, :]   X, Y row-major [d,r]; split over d, vector reds
+//   !kGram: C[d,r]  = A[d,r] M[r,r] (+ beta E)       A row-major (k contiguous), M row-major
+// Sizes need only r % 4 == 0 (the ABI asks r % 8 == 0); edges are zero-filled / guarded.
+constexpr int TM = 64, TN = 64, TK = 16, TPAD = 4;
+
+template <bool kGram>
+__global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, const float* __restrict__ B, float* __restrict__ C,
+                                                 const float* __restrict__ E, float beta, int M, int N, int K, int kper,
+                                                 long long sA, long long sB, long long sC) {
+  __shared__ __align__(16) float As[2][TK][TM + TPAD];
+  __shared__ __align__(16) float Bs[2][TK][TN + TPAD];
+  const int t = threadIdx.x, tx = t % 16, ty = t / 16;
+  const int tiles_n = (N + TN - 1) / TN;
+  const int m0 = (blockIdx.x / tiles_n) * TM, n0 = (blockIdx.x % tiles_n) * TN;
+  const int kbeg = blockIdx.y * kper, kend = min(K, kbeg + kper);
+  A += (long long)blockIdx.z * sA; B += (long long)blockIdx.z * sB; C += (long long)blockIdx.z * sC;
+  if (E) E += (long long)blockIdx.z * sC;
+  const int lda = kGram ? M : K;                 // gram: A is [K(d), M(r)];  rmul: A is [M(d), K(r)]
+  float acc[4][4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
+
+  float4 ra, rb;
+  auto gload = [&](int k0) {
+    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+    {   // B tile [TK][TN]: row k, 4 consecutive n
+      const int k = k0 + t / 16, n = n0 + (t % 16) * 4;
+      rb = (k < kend && n < N) ? __ldg(reinterpret_cast<const float4*>(B + (long long)k * N + n)) : z;
+    }
+    if (kGram) {
+      const int k = k0 + t / 16, m = m0 + (t % 16) * 4;
+      ra = (k < kend && m < M) ? __ldg(reinterpret_cast<const float4*>(A + (long long)k * lda + m)) : z;
+    } else {   // A tile [TM][TK]: row m, 4 consecutive k
+      const int m = m0 + t / 4, k = k0 + (t % 4) * 4;
+      ra = (m < M && k < kend) ? __ldg(reinterpret_cast<const float4*>(A + (long long)m * lda + k)) : z;
+    }
+  };
+  auto sstore = [&](int buf) {
+    *reinterpret_cast<float4*>(&Bs[buf][t / 16][(t % 16) * 4]) = rb;
+    if (kGram) {
+      *reinterpret_cast<float4*>(&As[buf][t / 16][(t % 16) * 4]) = ra;
+    } else {
+      const int m = t / 4, k = (t % 4) * 4;
+      As[buf][k + 0][m] = ra.x; As[buf][k + 1][m] = ra.y; As[buf][k + 2][m] = ra.z; As[buf][k + 3][m] = ra.w;
+    }
+  };
+  if (kbeg < kend) {
+    gload(kbeg);
+    sstore(0);
+    __syncthreads();
+    int buf = 0;
+    for (int k0 = kbeg; k0 < kend; k0 += TK) {
+      const bool more = k0 + TK < kend;
+      if (more) gload(k0 + TK);
+#pragma unroll
+      for (int k = 0; k < TK; ++k) {
+        const float4 a = *reinterpret_cast<const float4*>(&As[buf][k][ty * 4]);
+        const float4 bb = *reinterpret_cast<const float4*>(&Bs[buf][k][tx * 4]);
+        const float av[4] = {a.x, a.y, a.z, a.w};
+        const float bv[4] = {bb.x, bb.y, bb.z, bb.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(av[i], bv[j], acc[i][j]);
+      }
+      if (more) { sstore(buf ^ 1); __syncthreads(); buf ^= 1; }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int m = m0 + ty * 4 + i, n = n0 + tx * 4;
+    if (m >= M || n >= N) continue;
+    float* dst = C + (long long)m * N + n;
+    if (kGram) {
+      asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(acc[i][0]), "f"(acc[i][1]),
+                   "f"(acc[i][2]), "f"(acc[i][3]) : "memory");
+    } else {
+      float4 v = make_float4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]);
+      if (E) {
+        const float4 e = __ldg(reinterpret_cast<const float4*>(E + (long long)m * N + n));
+        v.x = fmaf(beta, e.x, v.x); v.y = fmaf(beta, e.y, v.y); v.z = fmaf(beta, e.z, v.z); v.w = fmaf(beta, e.w, v.w);
+      }
+      *reinterpret_cast<float4*>(dst) = v;
+    }
+  }
+}
+
+// Gm[b] = X[b]^T X2[b]  ([r,r], split over d with vector reds)
 int gram(const float* X, const float* X2, float* Gm, int d, int r, int batch, cudaStream_t st) {
   { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(Gm, 0, (size_t)batch * r * r * 4, st)); }
-  GemmArgs g;
-  g.M = r; g.N = r; g.K[0] = d; g.batch = batch;
-  g.A[0].p = X; g.A[0].so = 1; g.A[0].sk = r; g.A[0].sb = (long long)d * r;
-  g.B[0].p = X2; g.B[0].so = 1; g.B[0].sk = r; g.B[0].sb = (long long)d * r;
-  g.C = Gm; g.ldc = r; g.sbc = (long long)r * r;
-  g.atomic = 1; g.splits = (d + 255) / 256;
-  return simt_gemm(g, st);
+  const int tiles = ((r + TM - 1) / TM) * ((r + TN - 1) / TN);
+  int splits = (2 * 148 + tiles * batch - 1) / (tiles * batch);          // about two waves of CTAs
+  int kper = ((d + splits - 1) / splits + TK - 1) / TK * TK;
+  if (kper < 4 * TK) kper = 4 * TK;
+  splits = (d + kper - 1) / kper;
+  KernelScope ks(KID_ST_GEMM, st);
+  k_st_gemm<true><<<dim3(tiles, splits, batch), 256, 0, st>>>(X, X2, Gm, nullptr, 0.f, r, r, d, kper, (long long)d * r,
+                                                            (long long)d * r, (long long)r * r);
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  return MAPL_OK;
 }
 
 // C[b] = X[b] M[b] (+ beta E[b])
 int right_mul(const float* X, const float* M, float* C, const float* E, float beta, int d, int r, int batch,
               cudaStream_t st) {
-  GemmArgs g;
-  g.M = d; g.N = r; g.K[0] = r; g.batch = batch;
-  g.A[0].p = X; g.A[0].so = r; g.A[0].sk = 1; g.A[0].sb = (long long)d * r;
-  g.B[0].p = M; g.B[0].so = 1; g.B[0].sk = r; g.B[0].sb = (long long)r * r;
-  g.C = C; g.ldc = r; g.sbc = (long long)d * r;
-  g.E = E; g.lde = r; g.sbe = (long long)d * r; g.beta = beta;
-  return simt_gemm(g, st);
+  const int tiles = ((d + TM - 1) / TM) * ((r + TN - 1) / TN);
+  KernelScope ks(KID_ST_GEMM, st);
+  k_st_gemm<false><<<dim3(tiles, 1, batch), 256, 0, st>>>(X, M, C, E, beta, d, r, r, r, (long long)d * r, (long long)r * r,
+                                                         (long long)d * r);
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  return MAPL_OK;
 }
 
 }  // namespace
