@@ -39,13 +39,14 @@ struct BwdGzParams {
   float* z2; long long n2;
   long long N;
   int d, r, ra, tile_m;
-  int stages1, stage1_bytes, b_stages, do_dh;
+  int stages1, stage1_bytes, b_stages, do_dh, ga_tma;
 };
 
 __global__ void __launch_bounds__(kThreads, 1)
 k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmWu,
             const __grid_constant__ CUtensorMap tmWb, const __grid_constant__ CUtensorMap tmWd,
-            const __grid_constant__ CUtensorMap tmO, const BwdGzParams p) {
+            const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUtensorMap tmGz,
+            const __grid_constant__ CUtensorMap tmGA, const BwdGzParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int kc = p.r + p.ra, nkb1 = p.d / 64;
@@ -74,7 +75,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   if (warp == 0) DBG(56)
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmG); tma_prefetch_desc(&tmWu); tma_prefetch_desc(&tmWb);
-    tma_prefetch_desc(&tmWd); tma_prefetch_desc(&tmO);
+    tma_prefetch_desc(&tmWd); tma_prefetch_desc(&tmO); tma_prefetch_desc(&tmGz); tma_prefetch_desc(&tmGA);
     chunk_init_barriers(c);
     for (int s = 0; s < p.stages1; ++s) { mbar_init(&s1_full[s], 1); mbar_init(&s1_empty[s], 1); }
     mbar_init(acc1_full, 1);
@@ -164,8 +165,8 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         o.y = pack_bf16x2(__uint_as_float(v[8 * i + 2]), __uint_as_float(v[8 * i + 3]));
         o.z = pack_bf16x2(__uint_as_float(v[8 * i + 4]), __uint_as_float(v[8 * i + 5]));
         o.w = pack_bf16x2(__uint_as_float(v[8 * i + 6]), __uint_as_float(v[8 * i + 7]));
-        if (live) *reinterpret_cast<uint4*>(p.gz_out + m * p.r + cc * 32 + i * 8) = o;
-        if (p.do_dh) *reinterpret_cast<uint4*>(c.sA + (size_t)(cc / 2) * kTileBytes + sw128_offset(row, (cc & 1) * 4 + i)) = o;
+        // the bf16 gz tile is both the A operand of phase 2 and the source of the TMA store to gz_out
+        *reinterpret_cast<uint4*>(c.sA + (size_t)(cc / 2) * kTileBytes + sw128_offset(row, (cc & 1) * 4 + i)) = o;
       }
     }
     if (p.ra) {
@@ -174,13 +175,32 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         uint32_t v[32];
         tmem_ld32(tmem_row + p.r + cc * 32, v);
         tmem_ld_wait();
-        if (live) {
+        if (p.ga_tma) {          // ra == 64: box cc = [128 rows x 32 floats], swizzled, stored by TMA below
+#pragma unroll
+          for (int i = 0; i < 8; ++i)
+            *reinterpret_cast<float4*>(c.sOut + (size_t)cc * kTileBytes + sw128_offset(row, i)) =
+                make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]), __uint_as_float(v[4 * i + 2]),
+                            __uint_as_float(v[4 * i + 3]));
+        } else if (live) {
 #pragma unroll
           for (int i = 0; i < 8; ++i)
             dst[cc * 8 + i] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
                                           __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
         }
       }
+    }
+    fence_proxy_async_smem();
+    asm volatile("bar.sync 3, 256;" ::: "memory");
+    if (threadIdx.x == 64) {
+      for (int kb = 0; kb < p.r / 64; ++kb) tma_store_2d(&tmGz, c.sA + (size_t)kb * kTileBytes, kb * 64, (int)m0);
+      if (p.ga_tma) tma_store_2d(&tmGA, c.sOut, 0, (int)m0);
+      tma_store_commit();
+      if (!p.do_dh) tma_store_wait_all<0>();
+    }
+    if (threadIdx.x == 192 && p.ga_tma) {
+      tma_store_2d(&tmGA, c.sOut + kTileBytes, 32, (int)m0);
+      tma_store_commit();
+      if (!p.do_dh) tma_store_wait_all<0>();
     }
     if (p.do_dh) {
       tc_fence_before_sync();
@@ -448,7 +468,12 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes,
                  ring2 = (size_t)(d.r / 64) * kTileBytes + (size_t)p.b_stages * kHalfTileBytes;
     const size_t smem = (ring1 > ring2 ? ring1 : ring2) + (size_t)kOutBufs * kTileBytes + 1024 + 1024;
-    CUtensorMap tmG, tmWu, tmWb, tmWd, tmO;
+    p.ga_tma = ra == 64 ? 1 : 0;
+    CUtensorMap tmG, tmWu, tmWb, tmWd, tmO, tmGz, tmGA;
+    if (!make_tmap_bf16_2d(&tmGz, gz_out, N, rr, rr, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
+    // gA map: unused unless ga_tma, but must be valid
+    if (p.ga_tma) { if (!make_tmap_f32_2d(&tmGA, gA_ws, N, (uint64_t)ra, (uint64_t)ra, 32, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA; }
+    else tmGA = tmGz;
     // dH map: when dH is skipped the map is unused but must be valid
     if (!make_tmap_bf16_2d(&tmO, dH_out ? dH_out : g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmG, g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
@@ -457,7 +482,7 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     if (!make_tmap_bf16_2d(&tmWd, pk.Wd, dd, (uint64_t)pk.kc, (uint64_t)pk.kc, 64, kChunkN / 2)) return MAPL_ERR_CUDA;
     const unsigned tiles = ((unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m) + 1u) & ~1u;   // whole CTA pairs
     KernelScope ks(KID_TC_BWD_GZ, st);
-    MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_bwd_gz, dim3(tiles), dim3(kThreads), smem, st, tmG, tmWu, tmWb, tmWd, tmO, p));
+    MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_bwd_gz, dim3(tiles), dim3(kThreads), smem, st, tmG, tmWu, tmWb, tmWd, tmO, tmGz, tmGA, p));
   }
   {  // ---- dU (+ dA scatter)
     BwdDuParams p;

@@ -23,6 +23,10 @@ namespace tc {
 bool make_tmap_bf16_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols,
                        uint64_t pitch_elems, uint32_t box_cols, uint32_t box_rows);
 
+// same for fp32 (box_cols * 4 bytes <= 128)
+bool make_tmap_f32_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols, uint64_t pitch_elems,
+                      uint32_t box_cols, uint32_t box_rows);
+
 #ifdef __CUDACC__
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
