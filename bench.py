@@ -362,9 +362,12 @@ def roofline_for(name, k, cfg, peaks, total_ms):
     call = {"k_tc_encode": "encode", "k_tc_encode_rvq": "encode", "k_simt_encode_rvq": "encode",
             "k_tc_decode": "decode", "k_tc_bwd_gz": "backward", "k_tc_bwd_du": "backward"}.get(name)
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(name)
+        for line in open(tpath).read().splitlines()[1:]:
+            wl, kern_name, nbytes = line.split(",")
+            if wl == cfg.name and kern_name == name:
+                traffic = int(nbytes)
     if call is None:
         return {"kernel": name, "bound": "hbm", "achieved": None, "peak": peaks["hbm"], "unit": "GB/s", "frac": None,
                 "traffic": traffic, "note": "generic kernel shared by several calls; see kernels"}
