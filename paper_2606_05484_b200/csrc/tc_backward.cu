@@ -291,6 +291,11 @@ __device__ __forceinline__ void scatter_gA(const BwdDuParams& p, float* sG, int*
   if (p.ra == 64) scatter_gA_t<64>(p, sG, sTok, cta, n_ctas); else scatter_gA_t<128>(p, sG, sTok, cta, n_ctas);
 }
 
+// kPair: two CTAs of a cluster own adjacent 128-row tiles of dU and the same token range; one M=256
+// cta_group::2 MMA per 16 tokens, each CTA loading its own g/H boxes and HALF of the Zhat/gz columns
+// (r >= 128).  !kPair: one CTA per d-tile (r == 64, where half an operand row is below the 128-byte
+// swizzle span).
+template <bool kPair>
 __global__ void __launch_bounds__(kThreadsDu, 1)
 k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmZ,
             const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmGz, const BwdDuParams p) {
@@ -304,11 +309,13 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   int* sTok = reinterpret_cast<int*>(sG + 128 * (p.ra + 4));                           // 3 x [128]
 
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+  const uint32_t rank = kPair ? cluster_ctarank() : 0u;
   const int dt = blockIdx.x;                                   // 128 rows of dU
   const int tb0 = blockIdx.y * p.blocks_per_split;
   const int tb1 = min(p.n_blocks, tb0 + p.blocks_per_split);
   const int n_items = (tb1 > tb0 ? tb1 - tb0 : 0) * p.n_src;
   constexpr int kBox = 64 * 128;                               // [64 tokens x 64 cols] bf16 = 8 KB
+  const int nb_boxes = kPair ? p.r / 128 : p.r / 64;           // Zhat/gz boxes this CTA loads per item
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmG); tma_prefetch_desc(&tmZ); tma_prefetch_desc(&tmH); tma_prefetch_desc(&tmGz);
@@ -317,11 +324,16 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
     fence_barrier_init();
   }
   if (warp == 1) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"((uint32_t)p.r) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    if (kPair) {
+      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"((uint32_t)p.r) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    } else {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"((uint32_t)p.r) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
   }
   tc_fence_before_sync();
-  __syncthreads();
+  if (kPair) cluster_sync_all(); else __syncthreads();
   tc_fence_after_sync();
   const uint32_t tmem_d = *tmem_slot;
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -343,18 +355,26 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         for (int it = 0; it < n_items; ++it) {
           const int s = it % p.stages, tb = tb0 + it / p.n_src, src = it % p.n_src;
           mbar_wait(&empty[s], ((it / p.stages) & 1) ^ 1);
-          mbar_arrive_expect_tx(&full[s], (uint32_t)p.item_bytes);
           uint8_t* a = smem + (size_t)s * p.item_bytes;
           const CUtensorMap* ma = src ? &tmH : &tmG;
           const CUtensorMap* mb = src ? &tmGz : &tmZ;
-          tma_load_2d(a, ma, &full[s], dt * 128, tb * 64, kEvictFirst);
-          tma_load_2d(a + kBox, ma, &full[s], dt * 128 + 64, tb * 64, kEvictFirst);
-          for (int j = 0; j < p.r / 64; ++j) tma_load_2d(a + 2 * kBox + j * kBox, mb, &full[s], j * 64, tb * 64, kEvictLast);
+          if (kPair) {
+            if (rank == 0) mbar_arrive_expect_tx(&full[s], 2u * (uint32_t)p.item_bytes);
+            tma_load_2d_pair(a, ma, &full[s], dt * 128, tb * 64, kEvictFirst);
+            tma_load_2d_pair(a + kBox, ma, &full[s], dt * 128 + 64, tb * 64, kEvictFirst);
+            for (int j = 0; j < nb_boxes; ++j)
+              tma_load_2d_pair(a + 2 * kBox + j * kBox, mb, &full[s], (int)rank * (p.r / 2) + j * 64, tb * 64, kEvictLast);
+          } else {
+            mbar_arrive_expect_tx(&full[s], (uint32_t)p.item_bytes);
+            tma_load_2d(a, ma, &full[s], dt * 128, tb * 64, kEvictFirst);
+            tma_load_2d(a + kBox, ma, &full[s], dt * 128 + 64, tb * 64, kEvictFirst);
+            for (int j = 0; j < nb_boxes; ++j) tma_load_2d(a + 2 * kBox + j * kBox, mb, &full[s], j * 64, tb * 64, kEvictLast);
+          }
         }
       }
     } else if (warp == 1) {
-      if (elect_one()) {
-        const uint32_t idesc = make_idesc_bf16(128, (uint32_t)p.r, true, true);
+      if (rank == 0 && elect_one()) {
+        const uint32_t idesc = make_idesc_bf16(kPair ? 256 : 128, (uint32_t)p.r, true, true);
         for (int it = 0; it < n_items; ++it) {
           const int s = it % p.stages;
           mbar_wait(&full[s], (it / p.stages) & 1);
@@ -363,12 +383,14 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
           tc_fence_after_sync();
           const uint32_t a = smem_u32(smem + (size_t)s * p.item_bytes), b = a + 2 * kBox;
 #pragma unroll
-          for (int k = 0; k < 4; ++k)       // 16 tokens (= 2 swizzle atoms of 8 rows) per UMMA
-            umma_bf16(tmem_d, desc_mnmajor_sw128(a + k * 2048, kBox), desc_mnmajor_sw128(b + k * 2048, kBox), idesc,
-                      (it | k) != 0);
-          umma_commit(&empty[s]);
+          for (int k = 0; k < 4; ++k) {     // 16 tokens (= 2 swizzle atoms of 8 rows) per UMMA
+            const uint64_t da = desc_mnmajor_sw128(a + k * 2048, kBox), db = desc_mnmajor_sw128(b + k * 2048, kBox);
+            if (kPair) umma_bf16_pair(tmem_d, da, db, idesc, (it | k) != 0);
+            else umma_bf16(tmem_d, da, db, idesc, (it | k) != 0);
+          }
+          if (kPair) umma_commit_pair(&empty[s]); else umma_commit(&empty[s]);
         }
-        umma_commit(acc_full);
+        if (kPair) umma_commit_pair(acc_full); else umma_commit(acc_full);
       }
     } else {
       const int q = warp & 3, row = q * 32 + lane;
@@ -389,10 +411,11 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   }
   if (threadIdx.x == 64) DU_DBG(5)
   tc_fence_before_sync();
-  __syncthreads();
+  if (kPair) cluster_sync_all(); else __syncthreads();
   if (warp == 1) {
     tc_fence_after_sync();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"((uint32_t)p.r) : "memory");
+    if (kPair) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"((uint32_t)p.r) : "memory");
+    else asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"((uint32_t)p.r) : "memory");
   }
 }
 
@@ -429,7 +452,8 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
   static bool attr_done = false;
   if (!attr_done) {
     MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_bwd_gz, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_bwd_du, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_bwd_du<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_bwd_du<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     attr_done = true;
   }
   const uint64_t N = (uint64_t)d.n_tokens, dd = (uint64_t)d.d, rr = (uint64_t)d.r;
@@ -488,13 +512,14 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     BwdDuParams p;
     p.dU = dU_out; p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.n_src = H ? 2 : 1;
     p.tok = ra ? tok : nullptr; p.gA = gA_ws; p.dA = dA_out; p.ra = ra;
-    p.item_bytes = 2 * 64 * 128 + (d.r / 64) * 64 * 128;
+    const int n_dt = d.d / 128;
+    const bool pair = d.r >= 128 && n_dt % 2 == 0;
+    p.item_bytes = 2 * 64 * 128 + (pair ? d.r / 128 : d.r / 64) * 64 * 128;      // per CTA
     const size_t scatter_bytes = ra ? (size_t)128 * (ra + 4) * 4 + 3 * 512 : 0;
     p.stages = (int)((227 * 1024 - 2048 - scatter_bytes) / p.item_bytes);
     if (p.stages > 8) p.stages = 8;
     if (p.stages < 2) return MAPL_ERR_UNSUPPORTED;
     p.n_blocks = (int)((d.n_tokens + 63) / 64);
-    const int n_dt = d.d / 128;
     int S = 148 / n_dt;
     if (S < 1) S = 1;
     if (S > p.n_blocks) S = p.n_blocks;
@@ -507,7 +532,8 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     if (!make_tmap_bf16_2d(&tmH, H ? H : g, N, dd, dd, 64, 64)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmGz, gz_out, N, rr, rr, 64, 64)) return MAPL_ERR_CUDA;
     KernelScope ks(KID_TC_BWD_DU, st);
-    MAPL_CUDA_CHECK(launch_pdl(k_tc_bwd_du, dim3(n_dt, S), dim3(kThreadsDu), smem, st, tmG, tmZ, tmH, tmGz, p));
+    if (pair) MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_bwd_du<true>, dim3(n_dt, S), dim3(kThreadsDu), smem, st, tmG, tmZ, tmH, tmGz, p));
+    else MAPL_CUDA_CHECK(launch_pdl(k_tc_bwd_du<false>, dim3(n_dt, S), dim3(kThreadsDu), smem, st, tmG, tmZ, tmH, tmGz, p));
   }
   if (dB_out && ra) {   // dB += A[tok]^T g  (P_p is frozen in the paper: optional, fp32 SIMT)
     GemmArgs ga;

@@ -136,7 +136,8 @@ int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks
               int32_t* codes_out, cudaStream_t st) {
   if (!tc_shape_ok(d)) return MAPL_ERR_UNSUPPORTED;
   if (d.rvq_levels != 0) return tc_encode_rvq(d, H, codebooks, pk, Zq_out, codes_out, st);
-  const int tile_m = tc_tile_m(d.n_tokens);
+  int tile_m = tc_tile_m(d.n_tokens);
+  if (const char* e = getenv("MAPL_ENC_SPLIT")) { if (atoi(e) == 2) tile_m = (tile_m / 2 + 7) / 8 * 8; }   // experiment
   CUtensorMap tmH, tmW;
   if (!make_tmap_bf16_2d(&tmH, H, (uint64_t)d.n_tokens, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)tile_m)) return MAPL_ERR_CUDA;
   if (!make_tmap_bf16_2d(&tmW, pk.WB, (uint64_t)d.r, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
