@@ -125,13 +125,37 @@ class ClockSampler:
                 "reasons": sorted(self.reasons)}
 
 
+# ---------------------------------------------------------------- multi-rank host logic (replicas only)
+
+def boundary_stream(b: int, rank: int) -> int:
+    """Seed stream of boundary b on rank `rank`: every rank draws its own micro-batches (weak scaling,
+    no data-path collective)."""
+    return b + 16 * rank
+
+
+def max_over_ranks(values, world: int, device):
+    """Element-wise MAX over the ranks of device-measured times (the job is as slow as its slowest
+    replica).  The only collective of the multi-GPU run; covered on CPU by the gloo test."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), device=device, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def job_tokens_per_second(tokens_per_rank_step: int, world: int, steps: int, ms: float) -> float:
+    """Whole-job aggregate: all ranks' tokens over the slowest rank's time."""
+    return tokens_per_rank_step * world * steps / (ms * 1e-3)
+
+
 # ---------------------------------------------------------------- the CUDA arm
 
 class Boundary:
     """device buffers of one stage boundary (own copies: nothing is shared between boundaries)"""
 
     def __init__(self, cfg, b, rank, torch, mb, I, host=False):
-        bi = I.make_boundary(cfg, b + 16 * rank)
+        bi = I.make_boundary(cfg, boundary_stream(b, rank))
         self.cfg = cfg
         act = torch.bfloat16 if cfg.act_dtype == "bf16" else torch.float32
 
@@ -313,13 +337,9 @@ def run_mapl(args):
         barrier()
         e2e_ms = f0.elapsed_time(f1)
 
-    if world > 1:
-        t = torch.tensor([ms, e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_ms = float(t[0]), float(t[1])
-    tokens_per_step = cfg.n_tokens * nb * world
-    value = tokens_per_step * args.steps / (ms * 1e-3)
-    e2e_value = tokens_per_step * e2e_steps / (e2e_ms * 1e-3)
+    ms, e2e_ms = max_over_ranks([ms, e2e_ms], world, "cuda")
+    value = job_tokens_per_second(cfg.n_tokens * nb, world, args.steps, ms)
+    e2e_value = job_tokens_per_second(cfg.n_tokens * nb, world, e2e_steps, e2e_ms)
 
     # ---- roofline of the dominant kernel (largest share of the timed per-kernel pass)
     peaks = _peaks()

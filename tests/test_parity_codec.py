@@ -162,3 +162,41 @@ def test_tc_rvq_envelope_shapes(r, K, L):
     bi = I.make_generic(23 + r % 7, 200 + r, 512, r, L, K, 300, 64, "bf16")
     gpu, ora, stats, errs = _roundtrip(bi)
     assert stats["forced"] <= stats["excepted"]
+
+
+def test_c2_full_size_one_boundary():
+    """configs[2] at full size (N=16384, the launch configuration bench.py times): every output
+    against the oracle, RVQ codes under the near-tie rule S5."""
+    bi = I.make_boundary(I.CONFIGS["c2"], 0)
+    gpu, ora, stats, errs = _roundtrip(bi, want_dB=False)
+    print("c2 full", errs, stats)
+
+
+def test_c3_full_size_sampled_tokens():
+    """configs[3] at full size (N=32768: two waves of CTA pairs, as bench.py launches it).  The fp64
+    oracle cannot run 32768 tokens of K=4096 RVQ in seconds, so the per-token outputs (codes, Zhat,
+    Hhat, gz, dH), which depend on their own token only, are compared on a sample of tokens that
+    covers the first and last tile, tile borders and a random spread."""
+    cfg = I.CONFIGS["c3"]
+    bi = I.make_boundary(cfg, 0)
+    gpu = run_gpu(bi, want_dB=False)
+    N = cfg.n_tokens
+    rng = np.random.default_rng(7)
+    idx = np.unique(np.concatenate([np.arange(0, 40), np.arange(N - 40, N), np.arange(100, 130), np.arange(16380, 16420),
+                                    rng.integers(0, N, 150)]))
+    H, U, g = bi.H.f64[idx], bi.U.f64, bi.g.f64[idx]
+    Z = o.project(H, U)
+    res, n_exc, n_forced, bad = o.follow_codes(Z, bi.C.f64, gpu["codes"][idx])
+    assert int(bad.sum()) == 0, f"non-admissible RVQ codes: {int(bad.sum())} (excepted {n_exc}, forced {n_forced})"
+    assert np.array_equal(gpu["codes"][idx], res["codes"])
+    Hhat = o.decode(res["Zhat"], U, bi.tok[idx], bi.A.f64, bi.B.f64)
+    bw = o.backward(g, H, res["Zhat"], U, bi.tok[idx], bi.A.f64, bi.B.f64, want_dB=False)
+    tol = TOL["bf16"]
+    for k, ref in (("Zq", res["Zhat"]), ("Hhat", Hhat), ("gz", bw["gz"]), ("dH", bw["dH"])):
+        e = rel_fro(gpu[k][idx], ref)
+        assert np.isfinite(gpu[k]).all() and e <= tol, f"{k}: {e:.3e}"
+    for k in ("dU", "dA"):
+        assert np.isfinite(gpu[k]).all()
+    # tokens absent from tok have zero dA rows, at any size
+    absent = np.setdiff1d(np.arange(cfg.vocab), bi.tok)
+    assert not gpu["dA"][absent].any()
