@@ -365,12 +365,49 @@ def run_mapl(args):
         "gpu_launches": launches_per_step * args.steps,
         "roofline": roof,
     }
+    if rank == 0 and world == 1 and not args.no_stiefel:
+        out["stiefel"] = stiefel_sweep(torch, mb, I, stream)
     if rank == 0:
         if not args.no_cpu_baseline and world >= 1:
             out["cpu_baseline"] = cpu_baseline(cfg, budget_s=args.cpu_budget)
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+def stiefel_sweep(torch, mb, I, stream, reps=10):
+    """BASELINE.json configs[4] beside the codec metric: Stiefel steps/s for the 3 projectors of d=2048,
+    r in {64,128,256,512}, QR (CholeskyQR2) and 5 Newton-Schulz iterations; one CUDA graph per variant.
+    A step = one mapl_stiefel_step call over the batch of 3; projector-steps/s = 3 x that."""
+    out = {}
+    with torch.cuda.stream(stream):
+        for r in (64, 128, 256, 512):
+            s = I.make_stiefel(r)
+            ws = mb.alloc_workspace(mb.mapl_stiefel_workspace_bytes(s.d, r, s.batch))
+            for retr, tag in ((mb.MAPL_RETRACT_NS, "ns5"), (mb.MAPL_RETRACT_QR, "qr")):
+                U = torch.from_numpy(s.U.data.copy()).cuda()
+                G = torch.from_numpy(s.G.data.copy()).cuda()
+                f = lambda: mb.mapl_stiefel_step(U, G, 1e-2, retr, 5, None, ws)
+                f()
+                stream.synchronize()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=stream):
+                    f()
+                g.replay()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                for _ in range(reps):
+                    g.replay()
+                e1.record(stream)
+                stream.synchronize()
+                us = 1e3 * e0.elapsed_time(e1) / reps
+                Uh = U.double()
+                res = float(max(torch.linalg.matrix_norm(Uh[b].T @ Uh[b] - torch.eye(r, device="cuda", dtype=torch.float64))
+                                for b in range(s.batch)))
+                out[f"r{r}_{tag}"] = {"us_per_step": round(us, 1), "projector_steps_per_s": round(s.batch * 1e6 / us),
+                                      "orth_residual_after": float(f"{res:.2e}")}
+    out["config"] = "d=2048, 3 projectors per call, fixed G, lr=1e-2, fp32"
+    return out
 
 
 def roofline_for(name, k, cfg, peaks, total_ms):
@@ -414,27 +451,40 @@ def roofline_for(name, k, cfg, peaks, total_ms):
 
 # ---------------------------------------------------------------- the oracle arm (CPU baseline)
 
-def cpu_baseline(cfg, budget_s=20.0, sample_tokens=None):
-    """The fp64 oracle, as it stands, on the host cores: one boundary, a contiguous token sample."""
+def _oracle_pass(cfg, n, boundary):
+    """One enc + dec + full bwd of `n` contiguous tokens of one boundary through the fp64 oracle."""
     from oracle import mapl_oracle as o
     from paper_2606_05484_b200 import inputs as I
-    n = sample_tokens or min(cfg.n_tokens, 1024)
-    t_used, tokens = 0.0, 0
-    while True:
-        bi = I.make_boundary(cfg.with_tokens(n), 0)
-        H, U, g = bi.H.f64, bi.U.f64, bi.g.f64
-        t0 = time.perf_counter()
-        enc = o.encode(H, U, bi.C.f64 if bi.C is not None else None)
-        Hhat = o.decode(enc["Zhat"], U, bi.tok, bi.A.f64, bi.B.f64)
-        bw = o.backward(g, H, enc["Zhat"], U, bi.tok, bi.A.f64, bi.B.f64, want_dB=False)
-        dt = time.perf_counter() - t0
-        t_used, tokens = dt, n
-        del Hhat, bw
-        if sample_tokens or dt > budget_s / 4 or n >= cfg.n_tokens:
-            break
-        n = min(cfg.n_tokens, int(n * max(2.0, min(8.0, budget_s / 2 / max(dt, 1e-3)))))
+    bi = I.make_boundary(cfg.with_tokens(n), boundary)
+    H, U, g = bi.H.f64, bi.U.f64, bi.g.f64
+    t0 = time.perf_counter()
+    enc = o.encode(H, U, bi.C.f64 if bi.C is not None else None)
+    Hhat = o.decode(enc["Zhat"], U, bi.tok, bi.A.f64, bi.B.f64)
+    bw = o.backward(g, H, enc["Zhat"], U, bi.tok, bi.A.f64, bi.B.f64, want_dB=False)
+    dt = time.perf_counter() - t0
+    del Hhat, bw
+    return dt
+
+
+def cpu_baseline(cfg, budget_s=20.0, sample_tokens=None):
+    """The fp64 oracle, as it stands, on the host cores: contiguous token samples of the workload's
+    boundaries, sized and repeated until about budget_s / 2 seconds of oracle work have been timed."""
+    from oracle import mapl_oracle as o
+    if sample_tokens:
+        dt = _oracle_pass(cfg, sample_tokens, 0)
+        return {"value": sample_tokens / dt, "unit": UNIT, "cores": o.threads(), "kind": "oracle",
+                "sample": f"{sample_tokens} contiguous tokens of boundary 0 (enc+dec+bwd, fp64), {dt:.1f} s"}
+    n = min(cfg.n_tokens, 512)
+    dt = _oracle_pass(cfg, n, 0)                                   # sizing probe, not counted
+    n = int(min(cfg.n_tokens, max(n, n * (budget_s / 4) / max(dt, 1e-3))))
+    t_used, tokens, passes = 0.0, 0, 0
+    while t_used < budget_s / 2 and passes < 64:
+        t_used += _oracle_pass(cfg, n, passes % max(1, cfg.n_boundaries))
+        tokens += n
+        passes += 1
     return {"value": tokens / t_used, "unit": UNIT, "cores": o.threads(), "kind": "oracle",
-            "sample": f"{tokens} contiguous tokens of boundary 0 (enc+dec+bwd, fp64), {t_used:.1f} s"}
+            "sample": f"{passes} passes of {n} contiguous tokens over the workload's boundaries (enc+dec+bwd, fp64), "
+                      f"{t_used:.1f} s of oracle time"}
 
 
 def run_reference(args):
@@ -475,6 +525,7 @@ def main():
     ap.add_argument("--workload", default="c1", choices=["c1", "c2", "c3", "c0"])
     ap.add_argument("--tokens", type=int, default=0, help="override tokens per boundary (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-stiefel", action="store_true", help="skip the configs[4] Stiefel-step sweep")
     ap.add_argument("--cpu-budget", type=float, default=20.0)
     args = ap.parse_args()
     if args.impl == "reference":
