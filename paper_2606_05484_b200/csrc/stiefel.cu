@@ -159,27 +159,8 @@ __global__ void __launch_bounds__(1024) k_chol_upper(float* __restrict__ Gb, int
   }
 }
 
-// Xinv = R^-1 for upper-triangular R (row-major [r,r]); thread c owns column c.
-__global__ void __launch_bounds__(1024) k_tri_inverse_upper(const float* __restrict__ Rb, float* __restrict__ Xb, int r) {
-  const float* R = Rb + (long long)blockIdx.x * r * r;
-  float* X = Xb + (long long)blockIdx.x * r * r;
-  for (int c = threadIdx.x; c < r; c += blockDim.x) {
-    for (int i = r - 1; i >= 0; --i) {
-      float x;
-      if (i > c) x = 0.f;
-      else if (i == c) x = 1.f / R[(long long)i * r + i];
-      else {
-        float s = 0.f;
-        for (int k = i + 1; k <= c; ++k) s = fmaf(R[(long long)i * r + k], X[(long long)k * r + c], s);
-        x = -s / R[(long long)i * r + i];
-      }
-      X[(long long)i * r + c] = x;
-    }
-  }
-}
-
 struct StWs {
-  size_t S, M, Rinv, X0, X1, total;
+  size_t S, M, Rinv, Rinv2, X0, X1, total;
 };
 StWs st_carve(int d, int r, int batch) {
   StWs w;
@@ -188,6 +169,7 @@ StWs st_carve(int d, int r, int batch) {
   w.S = seg((size_t)batch * r * r * 4);
   w.M = seg((size_t)batch * r * r * 4);
   w.Rinv = seg((size_t)batch * r * r * 4);
+  w.Rinv2 = seg((size_t)batch * r * r * 4);
   w.X0 = seg((size_t)batch * d * r * 4);
   w.X1 = seg((size_t)batch * d * r * 4);
   w.total = off + 256;
@@ -198,13 +180,13 @@ StWs st_carve(int d, int r, int batch) {
 // 64x64 output tile, BK = 16, 256 threads x (4x4), register-prefetched double buffering, 128-bit
 // global and shared accesses.  Two shapes:
 //   kGram : C[r,r] (+)= X[k0:k1, :]^T Y[k0:k1, :]   X, Y row-major [d,r]; split over d, vector reds
-//   !kGram: C[d,r]  = A[d,r] M[r,r] (+ beta E)       A row-major (k contiguous), M row-major
+//   !kGram: C[d,r]  = alpha A[d,r] M[r,r] (+ beta E)  A row-major (k contiguous), M row-major
 // Sizes need only r % 4 == 0 (the ABI asks r % 8 == 0); edges are zero-filled / guarded.
 constexpr int TM = 64, TN = 64, TK = 16, TPAD = 4;
 
 template <bool kGram>
 __global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, const float* __restrict__ B, float* __restrict__ C,
-                                                 const float* __restrict__ E, float beta, int M, int N, int K, int kper,
+                                                 const float* __restrict__ E, float alpha, float beta, int M, int N, int K, int kper,
                                                  long long sA, long long sB, long long sC) {
   __shared__ __align__(16) float As[2][TK][TM + TPAD];
   __shared__ __align__(16) float Bs[2][TK][TN + TPAD];
@@ -276,7 +258,7 @@ __global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, co
       asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(acc[i][0]), "f"(acc[i][1]),
                    "f"(acc[i][2]), "f"(acc[i][3]) : "memory");
     } else {
-      float4 v = make_float4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]);
+      float4 v = make_float4(alpha * acc[i][0], alpha * acc[i][1], alpha * acc[i][2], alpha * acc[i][3]);
       if (E) {
         const float4 e = __ldg(reinterpret_cast<const float4*>(E + (long long)m * N + n));
         v.x = fmaf(beta, e.x, v.x); v.y = fmaf(beta, e.y, v.y); v.z = fmaf(beta, e.z, v.z); v.w = fmaf(beta, e.w, v.w);
@@ -295,20 +277,53 @@ int gram(const float* X, const float* X2, float* Gm, int d, int r, int batch, cu
   if (kper < 4 * TK) kper = 4 * TK;
   splits = (d + kper - 1) / kper;
   KernelScope ks(KID_ST_GEMM, st);
-  k_st_gemm<true><<<dim3(tiles, splits, batch), 256, 0, st>>>(X, X2, Gm, nullptr, 0.f, r, r, d, kper, (long long)d * r,
+  k_st_gemm<true><<<dim3(tiles, splits, batch), 256, 0, st>>>(X, X2, Gm, nullptr, 1.f, 0.f, r, r, d, kper, (long long)d * r,
                                                             (long long)d * r, (long long)r * r);
   MAPL_CUDA_CHECK(cudaGetLastError());
   return MAPL_OK;
 }
 
-// C[b] = X[b] M[b] (+ beta E[b])
-int right_mul(const float* X, const float* M, float* C, const float* E, float beta, int d, int r, int batch,
-              cudaStream_t st) {
-  const int tiles = ((d + TM - 1) / TM) * ((r + TN - 1) / TN);
+// C[b] = alpha X[b] M[b] (+ beta E[b]);  X, C, E are [rows, r], M is [r, r]
+int right_mul(const float* X, const float* M, float* C, const float* E, float beta, int rows, int r, int batch,
+              cudaStream_t st, float alpha = 1.f) {
+  const int tiles = ((rows + TM - 1) / TM) * ((r + TN - 1) / TN);
   KernelScope ks(KID_ST_GEMM, st);
-  k_st_gemm<false><<<dim3(tiles, 1, batch), 256, 0, st>>>(X, M, C, E, beta, d, r, r, r, (long long)d * r, (long long)r * r,
-                                                         (long long)d * r);
+  k_st_gemm<false><<<dim3(tiles, 1, batch), 256, 0, st>>>(X, M, C, E, alpha, beta, rows, r, r, r, (long long)rows * r,
+                                                         (long long)r * r, (long long)rows * r);
   MAPL_CUDA_CHECK(cudaGetLastError());
+  return MAPL_OK;
+}
+
+// X0 = diag(R)^-1 (batched [r,r])
+__global__ void k_diag_inverse(const float* __restrict__ R, float* __restrict__ X, int r) {
+  const long long off = (long long)blockIdx.y * r * r;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= r * r) return;
+  const int a = idx / r, b = idx % r;
+  X[off + idx] = a == b ? 1.f / R[off + (long long)a * r + a] : 0.f;
+}
+
+// Xinv = R^-1 for upper-triangular R by Newton's iteration X <- X (2I - R X) from X0 = diag(R)^-1.
+// I - R X0 is strictly upper triangular, hence nilpotent: the error after k steps is its 2^k-th power,
+// which is exactly zero once 2^k >= r.  ceil(log2 r) iterations of two [r,r,r] GEMMs replace a
+// column-serial back substitution; every iterate stays upper triangular.
+// Result in *out (one of Xa, Xb); T is [r,r] scratch.
+int tri_inverse_newton(const float* R, float* Xa, float* Xb, float* T, float** out, int r, int batch, cudaStream_t st) {
+  {
+    KernelScope ks(KID_ST_TRI_INV, st);
+    k_diag_inverse<<<dim3((r * r + 255) / 256, batch), 256, 0, st>>>(R, Xa, r);
+    MAPL_CUDA_CHECK(cudaGetLastError());
+  }
+  int iters = 0;
+  while ((1 << iters) < r) ++iters;
+  float* cur = Xa;
+  float* nxt = Xb;
+  for (int it = 0; it < iters; ++it) {
+    MAPL_RETURN_IF(right_mul(R, cur, T, nullptr, 0.f, r, r, batch, st));            // T = R X
+    MAPL_RETURN_IF(right_mul(cur, T, nxt, cur, 2.f, r, r, batch, st, -1.f));        // X' = 2 X - X T
+    float* t = cur; cur = nxt; nxt = t;
+  }
+  *out = cur;
   return MAPL_OK;
 }
 
@@ -341,6 +356,7 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
   float* S = reinterpret_cast<float*>(ws + w.S);
   float* M = reinterpret_cast<float*>(ws + w.M);
   float* Rinv = reinterpret_cast<float*>(ws + w.Rinv);
+  float* Rinv2 = reinterpret_cast<float*>(ws + w.Rinv2);
   float* X0 = reinterpret_cast<float*>(ws + w.X0);
   float* X1 = reinterpret_cast<float*>(ws + w.X1);
   const dim3 egrid((r * r + 255) / 256, batch);
@@ -381,10 +397,10 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
       MAPL_RETURN_IF(gram(src, src, S, d, r, batch, st));
       { KernelScope ks(KID_ST_CHOL, st); k_chol_upper<<<batch, 1024, smem, st>>>(S, r); }
       MAPL_CUDA_CHECK(cudaGetLastError());
-      { KernelScope ks(KID_ST_TRI_INV, st); k_tri_inverse_upper<<<batch, (r + 31) / 32 * 32, 0, st>>>(S, Rinv, r); }
-      MAPL_CUDA_CHECK(cudaGetLastError());
+      float* Xinv = nullptr;
+      MAPL_RETURN_IF(tri_inverse_newton(S, Rinv, Rinv2, M, &Xinv, r, batch, st));
       float* out = pass == 0 ? X1 : U;
-      MAPL_RETURN_IF(right_mul(src, Rinv, out, nullptr, 0.f, d, r, batch, st));
+      MAPL_RETURN_IF(right_mul(src, Xinv, out, nullptr, 0.f, d, r, batch, st));
       src = out;
     }
   }
