@@ -245,13 +245,18 @@ def run_mapl(args):
 
     stiefel = None
     if args.workload == "c3":       # configs[3]: "plus a Stiefel step per boundary" (G = dU / N, S12)
-        st_ws = mb.alloc_workspace(mb.mapl_stiefel_workspace_bytes(cfg.d, cfg.r, 1))
-        Gs = [torch.empty_like(b.dU) for b in bs]
+        # the nb projectors live in one [nb, d, r] tensor (and their gradients likewise), so the per-boundary
+        # Stiefel steps of a training step are ONE batched mapl_stiefel_step call (batch = nb)
+        st_ws = mb.alloc_workspace(mb.mapl_stiefel_workspace_bytes(cfg.d, cfg.r, nb))
+        Uall = torch.stack([b.U for b in bs]).contiguous()
+        dUall = torch.empty_like(Uall)
+        Gall = torch.empty_like(Uall)
+        for i, b in enumerate(bs):
+            b.U, b.dU = Uall[i], dUall[i]
 
         def stiefel():
-            for b, G in zip(bs, Gs):
-                torch.mul(b.dU, 1.0 / cfg.n_tokens, out=G)
-                mb.mapl_stiefel_step(b.U, G, 1e-2, mb.MAPL_RETRACT_NS, 5, None, st_ws)
+            torch.mul(dUall, 1.0 / cfg.n_tokens, out=Gall)
+            mb.mapl_stiefel_step(Uall, Gall, 1e-2, mb.MAPL_RETRACT_NS, 5, None, st_ws)
     step = make_step(bs, mb, stiefel)
 
     def barrier():

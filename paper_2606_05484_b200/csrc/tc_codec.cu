@@ -175,7 +175,7 @@ int tc_pack_build(const mapl_boundary_desc& d, const float* U, const float* B, c
   }
   {
     KernelScope ks(KID_TC_PACK, st);
-    k_tc_pack<<<dim3(148, a.njobs), 256, 0, st>>>(a);
+    k_tc_pack<<<dim3(1024, a.njobs), 256, 0, st>>>(a);      // 32x32 tiles; blocks beyond a job's tile count exit at once
     MAPL_CUDA_CHECK(cudaGetLastError());
   }
   return MAPL_OK;
