@@ -177,12 +177,20 @@ StWs st_carve(int d, int r, int batch) {
 }
 
 // ---------------------------------------------------------------- fp32 FFMA GEMMs of the step
-// 64x64 output tile, BK = 16, 256 threads x (4x4), register-prefetched double buffering, 128-bit
+// 128x64 output tile, BK = 16, 256 threads x (8x4), register-prefetched double buffering, 128-bit
 // global and shared accesses.  Two shapes:
 //   kGram : C[r,r] (+)= X[k0:k1, :]^T Y[k0:k1, :]   X, Y row-major [d,r]; split over d, vector reds
 //   !kGram: C[d,r]  = alpha A[d,r] M[r,r] (+ beta E)  A row-major (k contiguous), M row-major
 // Sizes need only r % 4 == 0 (the ABI asks r % 8 == 0); edges are zero-filled / guarded.
-constexpr int TM = 64, TN = 64, TK = 16, TPAD = 4;
+#ifndef MAPL_ST_TM
+#define MAPL_ST_TM 64
+#endif
+#ifndef MAPL_ST_TK
+#define MAPL_ST_TK 16
+#endif
+constexpr int TM = MAPL_ST_TM, TN = 64, TK = MAPL_ST_TK, TPAD = 4;
+constexpr int RM = TM / 16;                         // rows per thread (4 or 8); 4 columns per thread
+constexpr int LA = TM * TK / 4 / 256, LB = TN * TK / 4 / 256;   // float4 loads per thread per k-step tile
 
 template <bool kGram>
 __global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, const float* __restrict__ B, float* __restrict__ C,
@@ -190,41 +198,57 @@ __global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, co
                                                  long long sA, long long sB, long long sC) {
   __shared__ __align__(16) float As[2][TK][TM + TPAD];
   __shared__ __align__(16) float Bs[2][TK][TN + TPAD];
-  const int t = threadIdx.x, tx = t % 16, ty = t / 16;
+  const int t = threadIdx.x, tx = t % 16, ty = t / 16;      // thread tile: rows ty*RM..+RM-1, cols tx*4..+3
   const int tiles_n = (N + TN - 1) / TN;
   const int m0 = (blockIdx.x / tiles_n) * TM, n0 = (blockIdx.x % tiles_n) * TN;
   const int kbeg = blockIdx.y * kper, kend = min(K, kbeg + kper);
   A += (long long)blockIdx.z * sA; B += (long long)blockIdx.z * sB; C += (long long)blockIdx.z * sC;
   if (E) E += (long long)blockIdx.z * sC;
   const int lda = kGram ? M : K;                 // gram: A is [K(d), M(r)];  rmul: A is [M(d), K(r)]
-  float acc[4][4];
+  float acc[RM][4];
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
+  for (int i = 0; i < RM; ++i)
 #pragma unroll
     for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
 
-  float4 ra, rb;
+  // one k-step tile (TK rows of k) is fetched into registers while the previous one is multiplied.
+  // Measured (ncu): 128x64 tiles or TK = 32 change nothing -- the kernel is limited by occupancy
+  // (the step's GEMMs are ~0.3 GFLOP each: 1-3 CTAs per SM) and shared-memory scoreboard stalls.
+  float4 ra[LA], rb[LB];
   auto gload = [&](int k0) {
     const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-    {   // B tile [TK][TN]: row k, 4 consecutive n
-      const int k = k0 + t / 16, n = n0 + (t % 16) * 4;
-      rb = (k < kend && n < N) ? __ldg(reinterpret_cast<const float4*>(B + (long long)k * N + n)) : z;
+#pragma unroll
+    for (int i = 0; i < LB; ++i) {   // B tile [TK][TN]: row k, 4 consecutive n
+      const int f = t + i * 256, k = k0 + f / (TN / 4), n = n0 + (f % (TN / 4)) * 4;
+      rb[i] = (k < kend && n < N) ? __ldg(reinterpret_cast<const float4*>(B + (long long)k * N + n)) : z;
     }
-    if (kGram) {
-      const int k = k0 + t / 16, m = m0 + (t % 16) * 4;
-      ra = (k < kend && m < M) ? __ldg(reinterpret_cast<const float4*>(A + (long long)k * lda + m)) : z;
-    } else {   // A tile [TM][TK]: row m, 4 consecutive k
-      const int m = m0 + t / 4, k = k0 + (t % 4) * 4;
-      ra = (m < M && k < kend) ? __ldg(reinterpret_cast<const float4*>(A + (long long)m * lda + k)) : z;
+#pragma unroll
+    for (int i = 0; i < LA; ++i) {
+      const int f = t + i * 256;
+      if (kGram) {   // A tile [TK][TM]: row k, 4 consecutive m
+        const int k = k0 + f / (TM / 4), m = m0 + (f % (TM / 4)) * 4;
+        ra[i] = (k < kend && m < M) ? __ldg(reinterpret_cast<const float4*>(A + (long long)k * lda + m)) : z;
+      } else {       // A tile [TM][TK]: row m, 4 consecutive k
+        const int m = m0 + f / (TK / 4), k = k0 + (f % (TK / 4)) * 4;
+        ra[i] = (m < M && k < kend) ? __ldg(reinterpret_cast<const float4*>(A + (long long)m * lda + k)) : z;
+      }
     }
   };
   auto sstore = [&](int buf) {
-    *reinterpret_cast<float4*>(&Bs[buf][t / 16][(t % 16) * 4]) = rb;
-    if (kGram) {
-      *reinterpret_cast<float4*>(&As[buf][t / 16][(t % 16) * 4]) = ra;
-    } else {
-      const int m = t / 4, k = (t % 4) * 4;
-      As[buf][k + 0][m] = ra.x; As[buf][k + 1][m] = ra.y; As[buf][k + 2][m] = ra.z; As[buf][k + 3][m] = ra.w;
+#pragma unroll
+    for (int i = 0; i < LB; ++i) {
+      const int f = t + i * 256;
+      *reinterpret_cast<float4*>(&Bs[buf][f / (TN / 4)][(f % (TN / 4)) * 4]) = rb[i];
+    }
+#pragma unroll
+    for (int i = 0; i < LA; ++i) {
+      const int f = t + i * 256;
+      if (kGram) {
+        *reinterpret_cast<float4*>(&As[buf][f / (TM / 4)][(f % (TM / 4)) * 4]) = ra[i];
+      } else {
+        const int m = f / (TK / 4), k = (f % (TK / 4)) * 4;
+        As[buf][k + 0][m] = ra[i].x; As[buf][k + 1][m] = ra[i].y; As[buf][k + 2][m] = ra[i].z; As[buf][k + 3][m] = ra[i].w;
+      }
     }
   };
   if (kbeg < kend) {
@@ -237,12 +261,16 @@ __global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, co
       if (more) gload(k0 + TK);
 #pragma unroll
       for (int k = 0; k < TK; ++k) {
-        const float4 a = *reinterpret_cast<const float4*>(&As[buf][k][ty * 4]);
+        float av[RM];
+#pragma unroll
+        for (int i = 0; i < RM / 4; ++i) {
+          const float4 a = *reinterpret_cast<const float4*>(&As[buf][k][ty * RM + 4 * i]);
+          av[4 * i] = a.x; av[4 * i + 1] = a.y; av[4 * i + 2] = a.z; av[4 * i + 3] = a.w;
+        }
         const float4 bb = *reinterpret_cast<const float4*>(&Bs[buf][k][tx * 4]);
-        const float av[4] = {a.x, a.y, a.z, a.w};
         const float bv[4] = {bb.x, bb.y, bb.z, bb.w};
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < RM; ++i)
 #pragma unroll
           for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(av[i], bv[j], acc[i][j]);
       }
@@ -250,8 +278,8 @@ __global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, co
     }
   }
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int m = m0 + ty * 4 + i, n = n0 + tx * 4;
+  for (int i = 0; i < RM; ++i) {
+    const int m = m0 + ty * RM + i, n = n0 + tx * 4;
     if (m >= M || n >= N) continue;
     float* dst = C + (long long)m * N + n;
     if (kGram) {
