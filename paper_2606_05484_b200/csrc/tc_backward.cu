@@ -40,6 +40,7 @@ struct BwdGzParams {
   long long N;
   int d, r, ra, tile_m;
   int stages1, stage1_bytes, b_stages, do_dh, ga_tma;
+  const int32_t* codes; const float* codebooks; __nv_bfloat16* zhat_out; int L, K;   // RVQ: zhat for k_tc_bwd_du
 };
 
 __global__ void __launch_bounds__(kThreads, 1)
@@ -150,6 +151,14 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         const long long lo = per * blockIdx.x, hi = lo + per < nv ? lo + per : nv;
         for (long long i = lo + et; i < hi; i += 256) reinterpret_cast<float4*>(zp[a])[i] = zero;
       }
+    }
+    if (p.codes != nullptr) {   // RVQ: dequantise this tile's codes into the bf16 zhat operand of k_tc_bwd_du while g streams
+      int idx[8];
+#pragma unroll
+      for (int l = 0; l < 8; ++l) idx[l] = (live && l < p.L) ? __ldg(p.codes + m * p.L + l) : -1;
+      __nv_bfloat16* gout = p.zhat_out + m0 * p.r;
+      if (p.r >= 128) gather_sum_rows<8>(nullptr, 0, p.r, p.codebooks, (long long)p.K * p.r, idx, p.L, q, lane, half, gout);
+      else gather_sum_rows<4>(nullptr, 0, p.r, p.codebooks, (long long)p.K * p.r, idx, p.L, q, lane, half, gout);
     }
     mbar_wait(acc1_full, 0);
     if (warp == 2) DBG(58)
@@ -419,24 +428,6 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   }
 }
 
-// zhat (bf16) from RVQ codes, for the dU operand
-__global__ void k_tc_dequant_bf16(const int32_t* __restrict__ codes, const float* __restrict__ C,
-                                  __nv_bfloat16* __restrict__ Zb, long long N, int r, int L, int K) {
-  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;   // one 8-column chunk each
-  const int cpr = r / 8;
-  if (idx >= N * cpr) return;
-  const long long n = idx / cpr;
-  const int c = (int)(idx % cpr);
-  float s[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  for (int l = 0; l < L; ++l) {
-    const float4* src = reinterpret_cast<const float4*>(C + ((long long)l * K + codes[n * L + l]) * r + c * 8);
-    const float4 x = __ldg(src), y = __ldg(src + 1);
-    s[0] += x.x; s[1] += x.y; s[2] += x.z; s[3] += x.w; s[4] += y.x; s[5] += y.y; s[6] += y.z; s[7] += y.w;
-  }
-  *reinterpret_cast<uint4*>(Zb + n * r + c * 8) =
-      make_uint4(pack_bf16x2(s[0], s[1]), pack_bf16x2(s[2], s[3]), pack_bf16x2(s[4], s[5]), pack_bf16x2(s[6], s[7]));
-}
-
 }  // namespace
 }  // namespace mapl
 MAPL_DBG_READER(mapl_debug_read_bwd)
@@ -460,14 +451,7 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
 
   // zhat operand for dU
   const void* zhat = Z;
-  if (codes) {
-    const long long total = d.n_tokens * (d.r / 8);
-    KernelScope ks(KID_DEQUANT, st);
-    k_tc_dequant_bf16<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(codes, codebooks, zhat_ws, d.n_tokens, d.r,
-                                                                      d.rvq_levels, d.rvq_k);
-    MAPL_CUDA_CHECK(cudaGetLastError());
-    zhat = zhat_ws;
-  }
+  if (codes) zhat = zhat_ws;        // written by k_tc_bwd_gz (dequantisation fused under its g stream)
 
   {  // ---- gz, gA, dH (+ zero fill of the overwrite outputs)
     BwdGzParams p;
@@ -493,6 +477,7 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
                  ring2 = (size_t)(d.r / 64) * kTileBytes + (size_t)p.b_stages * kHalfTileBytes;
     const size_t smem = (ring1 > ring2 ? ring1 : ring2) + (size_t)kOutBufs * kTileBytes + 1024 + 1024;
     p.ga_tma = ra == 64 ? 1 : 0;
+    p.codes = codes; p.codebooks = codebooks; p.zhat_out = zhat_ws; p.L = d.rvq_levels; p.K = d.rvq_k;
     CUtensorMap tmG, tmWu, tmWb, tmWd, tmO, tmGz, tmGA;
     if (!make_tmap_bf16_2d(&tmGz, gz_out, N, rr, rr, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
     // gA map: unused unless ga_tma, but must be valid

@@ -28,49 +28,6 @@ struct DecodeParams {
   int tile_m, b_stages, z_from_tma;
 };
 
-// sA tiles [tile0, tile0 + width/64): row (q*32 + j) := bf16( sum_{l < nsrc} table[l*src_stride + idx_j[l]*width + :] ),
-// zeros where idx < 0.  idx[] holds the indices of row q*32+lane.  One warp, convergent.  The loads
-// of 8 row groups are issued back to back before any is consumed (the gathers are L2-latency bound).
-// Two warps share a quarter: `part` (0/1) takes the first / second half of the row groups.
-template <int kBatch>
-__device__ __forceinline__ void gather_sum_rows(uint8_t* sA, int tile0, int width, const float* __restrict__ table,
-                                                long long src_stride, const int (&idx)[8], int nsrc, int q, int lane,
-                                                int part) {
-  const int lpr = width / 8, rpi = 32 / lpr, cc = lane % lpr, sub = lane / lpr;
-  for (int it0 = part * (lpr / 2); it0 < (part + 1) * (lpr / 2); it0 += kBatch) {   // lpr = 32 / rpi row groups in all
-    float acc[kBatch][8];
-#pragma unroll
-    for (int b = 0; b < kBatch; ++b)
-#pragma unroll
-      for (int j = 0; j < 8; ++j) acc[b][j] = 0.f;
-#pragma unroll
-    for (int l = 0; l < 8; ++l) {
-      if (l < nsrc) {
-        float4 x[kBatch], y[kBatch];
-#pragma unroll
-        for (int b = 0; b < kBatch; ++b) {
-          const int k = __shfl_sync(0xffffffffu, idx[l], (it0 + b) * rpi + sub);
-          const float4* src = reinterpret_cast<const float4*>(table + l * src_stride + (long long)(k < 0 ? 0 : k) * width + cc * 8);
-          x[b] = __ldg(src); y[b] = __ldg(src + 1);
-          if (k < 0) { x[b] = make_float4(0.f, 0.f, 0.f, 0.f); y[b] = x[b]; }
-        }
-#pragma unroll
-        for (int b = 0; b < kBatch; ++b) {
-          acc[b][0] += x[b].x; acc[b][1] += x[b].y; acc[b][2] += x[b].z; acc[b][3] += x[b].w;
-          acc[b][4] += y[b].x; acc[b][5] += y[b].y; acc[b][6] += y[b].z; acc[b][7] += y[b].w;
-        }
-      }
-    }
-#pragma unroll
-    for (int b = 0; b < kBatch; ++b) {
-      const int rl = (it0 + b) * rpi + sub;
-      const uint4 o = make_uint4(pack_bf16x2(acc[b][0], acc[b][1]), pack_bf16x2(acc[b][2], acc[b][3]),
-                                 pack_bf16x2(acc[b][4], acc[b][5]), pack_bf16x2(acc[b][6], acc[b][7]));
-      *reinterpret_cast<uint4*>(sA + (size_t)(tile0 + cc / 8) * kTileBytes + sw128_offset(q * 32 + rl, cc % 8)) = o;
-    }
-  }
-}
-
 __global__ void __launch_bounds__(kThreads, 1)
 k_tc_decode(const __grid_constant__ CUtensorMap tmZ, const __grid_constant__ CUtensorMap tmW,
             const __grid_constant__ CUtensorMap tmO, const DecodeParams p) {
