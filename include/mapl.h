@@ -86,13 +86,16 @@ size_t mapl_workspace_bytes(const mapl_boundary_desc* desc);
 size_t mapl_stiefel_workspace_bytes(int32_t d, int32_t r, int32_t batch);
 
 /* PARAMETER PACK (optional).  The tensor-core kernels read U, B and the codebooks as bf16 operand
- * tiles (U additionally as a two-term bf16 split when RVQ follows, so z stays fp32-accurate) plus
- * per-codeword half squared norms.  mapl_pack_params writes that derived copy into caller-owned
+ * tiles (U additionally as a two-term bf16 split when RVQ follows, so z stays fp32-accurate; the
+ * codebooks as fp16 scaled per level by a power of two) plus per-codeword half squared norms.  mapl_pack_params writes that derived copy into caller-owned
  * device memory `pack_out` (mapl_param_pack_bytes(desc) bytes, 256-byte aligned; 0 bytes when the
  * boundary runs on the fp32 kernels: then pack_out may be NULL and the call is a no-op).  In the
  * paper's schedule the parameters change once per optimizer step while ~128 micro-batches cross
  * the boundary, so the pack is made once per step and referenced from
- * desc.param_pack.  B / codebooks may be NULL when anchor_rank / rvq_levels is 0.                 */
+ * desc.param_pack.  B / codebooks may be NULL when anchor_rank / rvq_levels is 0.  With
+ * rvq_levels > 0, codebooks == NULL re-packs U (and B) only and leaves the codebook section of an
+ * existing pack as it is: the call to make after a projector update (mapl_stiefel_step), since
+ * the codebooks did not change.  The first pack of a buffer must pass the codebooks.               */
 size_t mapl_param_pack_bytes(const mapl_boundary_desc* desc);
 int mapl_pack_params(const mapl_boundary_desc* desc, const float* U, const float* B, const float* codebooks,
                      void* pack_out, void* cuda_stream);

@@ -200,3 +200,37 @@ def test_c3_full_size_sampled_tokens():
     # tokens absent from tok have zero dA rows, at any size
     absent = np.setdiff1d(np.arange(cfg.vocab), bi.tok)
     assert not gpu["dA"][absent].any()
+
+
+def test_projector_only_repack_equals_full_repack():
+    """mapl_pack_params with codebooks == NULL re-packs U/B only and keeps the codebook section: after a
+    projector update the encode / decode results equal those of a complete re-pack, bit for bit."""
+    bi = I.make_generic(31, 700, 512, 128, 2, 512, 300, 64, "bf16")
+    dev = Dev(bi)
+    desc = desc_of(bi)
+    pack = mb.alloc_workspace(mb.mapl_param_pack_bytes(desc))
+    desc.param_pack = pack.data_ptr()
+    ws = mb.alloc_workspace(mb.mapl_workspace_bytes(desc))
+    N, d, r, L = bi.cfg.n_tokens, bi.cfg.d, bi.cfg.r, bi.cfg.rvq_levels
+    mb.mapl_pack_params(desc, dev.U, dev.B, dev.C, pack)
+    U2 = to_dev(I.make_generic(32, 8, 512, 128, 0, 0, 10, 0, "bf16").U)      # another orthonormal projector
+
+    def run():
+        codes = torch.empty((N, L), dtype=torch.int32, device="cuda")
+        Hhat = torch.empty((N, d), dtype=torch.bfloat16, device="cuda")
+        mb.mapl_encode(desc, dev.H, U2, dev.C, None, codes, ws)
+        mb.mapl_decode(desc, None, codes, U2, dev.C, dev.tok, dev.A, dev.B, Hhat, ws)
+        torch.cuda.synchronize()
+        return codes.cpu().numpy(), Hhat.float().cpu().numpy()
+
+    mb.mapl_pack_params(desc, U2, dev.B, None, pack)          # projector-only re-pack
+    a = run()
+    mb.mapl_pack_params(desc, U2, dev.B, dev.C, pack)         # complete re-pack
+    b = run()
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    # and the projector did change the result
+    mb.mapl_pack_params(desc, dev.U, dev.B, dev.C, pack)
+    codes0 = torch.empty((N, L), dtype=torch.int32, device="cuda")
+    mb.mapl_encode(desc, dev.H, dev.U, dev.C, None, codes0, ws)
+    torch.cuda.synchronize()
+    assert not np.array_equal(codes0.cpu().numpy(), a[0])
