@@ -22,13 +22,18 @@ __global__ void k_step_matrix(const float* __restrict__ S, float* __restrict__ M
   M1[off + idx] = (a == b ? 1.f : 0.f) + lr * 0.5f * (S[off + a * r + b] + S[off + b * r + a]);
 }
 
+// element (a,b) of a symmetric [r,r] matrix of which only the 64x64 tiles on or above the diagonal are stored
+__device__ __forceinline__ float sym_at(const float* __restrict__ G, int r, int a, int b) {
+  return (a / 64 <= b / 64) ? G[(long long)a * r + b] : G[(long long)b * r + a];
+}
+
 __global__ void k_ns_poly(const float* __restrict__ Gm, float* __restrict__ M, int r) {
-  // M = (3I - Gm)/2
+  // M = (3I - Gm)/2, Gm = X^T X stored as upper tiles
   const long long off = (long long)blockIdx.y * r * r;
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= r * r) return;
   const int a = idx / r, b = idx % r;
-  M[off + idx] = 0.5f * ((a == b ? 3.f : 0.f) - Gm[off + idx]);
+  M[off + idx] = 0.5f * ((a == b ? 3.f : 0.f) - sym_at(Gm + off, r, a, b));
 }
 
 // out[b*2 + slot] = sqrt(sum_i (scale*(X[i] - Yv[i]))^2)   (Yv may be null: then X - I on an [r,r] matrix)
@@ -195,12 +200,19 @@ constexpr int LA = TM * TK / 4 / 256, LB = TN * TK / 4 / 256;   // float4 loads 
 template <bool kGram>
 __global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, const float* __restrict__ B, float* __restrict__ C,
                                                  const float* __restrict__ E, float alpha, float beta, int M, int N, int K, int kper,
-                                                 long long sA, long long sB, long long sC) {
+                                                 long long sA, long long sB, long long sC, int upper_only) {
   __shared__ __align__(16) float As[2][TK][TM + TPAD];
   __shared__ __align__(16) float Bs[2][TK][TN + TPAD];
   const int t = threadIdx.x, tx = t % 16, ty = t / 16;      // thread tile: rows ty*RM..+RM-1, cols tx*4..+3
   const int tiles_n = (N + TN - 1) / TN;
-  const int m0 = (blockIdx.x / tiles_n) * TM, n0 = (blockIdx.x % tiles_n) * TN;
+  int tm = blockIdx.x / tiles_n, tn = blockIdx.x % tiles_n;
+  if (upper_only) {            // symmetric product (TM == TN): blockIdx.x enumerates the tiles with tn >= tm
+    int rem = blockIdx.x;
+    tm = 0;
+    while (rem >= tiles_n - tm) { rem -= tiles_n - tm; ++tm; }
+    tn = tm + rem;
+  }
+  const int m0 = tm * TM, n0 = tn * TN;
   const int kbeg = blockIdx.y * kper, kend = min(K, kbeg + kper);
   A += (long long)blockIdx.z * sA; B += (long long)blockIdx.z * sB; C += (long long)blockIdx.z * sC;
   if (E) E += (long long)blockIdx.z * sC;
@@ -296,17 +308,20 @@ __global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, co
   }
 }
 
-// Gm[b] = X[b]^T X2[b]  ([r,r], split over d with vector reds)
-int gram(const float* X, const float* X2, float* Gm, int d, int r, int batch, cudaStream_t st) {
+// Gm[b] = X[b]^T X2[b]  ([r,r], split over d with vector reds).  upper_only (X2 == X, TM == TN): only the
+// 64x64 tiles on or above the diagonal are computed; readers use sym_at().
+int gram(const float* X, const float* X2, float* Gm, int d, int r, int batch, cudaStream_t st, bool upper_only = false) {
   { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(Gm, 0, (size_t)batch * r * r * 4, st)); }
-  const int tiles = ((r + TM - 1) / TM) * ((r + TN - 1) / TN);
+  const int nt = (r + TN - 1) / TN;
+  upper_only = upper_only && TM == TN;
+  const int tiles = upper_only ? nt * (nt + 1) / 2 : ((r + TM - 1) / TM) * nt;
   int splits = (2 * 148 + tiles * batch - 1) / (tiles * batch);          // about two waves of CTAs
   int kper = ((d + splits - 1) / splits + TK - 1) / TK * TK;
   if (kper < 4 * TK) kper = 4 * TK;
   splits = (d + kper - 1) / kper;
   KernelScope ks(KID_ST_GEMM, st);
   k_st_gemm<true><<<dim3(tiles, splits, batch), 256, 0, st>>>(X, X2, Gm, nullptr, 1.f, 0.f, r, r, d, kper, (long long)d * r,
-                                                            (long long)d * r, (long long)r * r);
+                                                            (long long)d * r, (long long)r * r, upper_only ? 1 : 0);
   MAPL_CUDA_CHECK(cudaGetLastError());
   return MAPL_OK;
 }
@@ -317,7 +332,7 @@ int right_mul(const float* X, const float* M, float* C, const float* E, float be
   const int tiles = ((rows + TM - 1) / TM) * ((r + TN - 1) / TN);
   KernelScope ks(KID_ST_GEMM, st);
   k_st_gemm<false><<<dim3(tiles, 1, batch), 256, 0, st>>>(X, M, C, E, alpha, beta, rows, r, r, r, (long long)rows * r,
-                                                         (long long)r * r, (long long)rows * r);
+                                                         (long long)r * r, (long long)rows * r, 0);
   MAPL_CUDA_CHECK(cudaGetLastError());
   return MAPL_OK;
 }
@@ -404,7 +419,7 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
     float* cur = X0;
     float* nxt = X1;
     for (int it = 0; it < ns_iters; ++it) {
-      MAPL_RETURN_IF(gram(cur, cur, S, d, r, batch, st));
+      MAPL_RETURN_IF(gram(cur, cur, S, d, r, batch, st, true));
       { KernelScope ks(KID_ST_NS_POLY, st); k_ns_poly<<<egrid, 256, 0, st>>>(S, M, r); }
       MAPL_CUDA_CHECK(cudaGetLastError());
       float* out = (it == ns_iters - 1) ? U : nxt;
@@ -422,7 +437,7 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
     }
     const float* src = X0;
     for (int pass = 0; pass < 2; ++pass) {
-      MAPL_RETURN_IF(gram(src, src, S, d, r, batch, st));
+      MAPL_RETURN_IF(gram(src, src, S, d, r, batch, st, true));   // k_chol_upper reads the upper triangle only
       { KernelScope ks(KID_ST_CHOL, st); k_chol_upper<<<batch, 1024, smem, st>>>(S, r); }
       MAPL_CUDA_CHECK(cudaGetLastError());
       float* Xinv = nullptr;
