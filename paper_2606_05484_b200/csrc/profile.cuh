@@ -26,6 +26,8 @@ enum KernelId {
   KID_TC_ENCODE_RVQ,
   KID_TC_SCATTER,
   KID_ST_GEMM,
+  KID_ST_SPLIT,
+  KID_ST_GEMM3,
   KID_COUNT
 };
 

@@ -6,7 +6,10 @@
 //
 //   Y = U - lr (G - U sym(U^T G)) = U (I + lr sym(S)) - lr G,   S = U^T G
 #include "common.cuh"
+#include <stdlib.h>
+
 #include "profile.cuh"
+#include "tc_stiefel.cuh"
 
 namespace mapl {
 namespace {
@@ -165,7 +168,7 @@ __global__ void __launch_bounds__(1024) k_chol_upper(float* __restrict__ Gb, int
 }
 
 struct StWs {
-  size_t S, M, Rinv, Rinv2, X0, X1, total;
+  size_t S, M, Rinv, Rinv2, X0, X1, Prow, Ptr, Ptr2, Pm, total;   // P*: bf16 planes of the tensor-core path
 };
 StWs st_carve(int d, int r, int batch) {
   StWs w;
@@ -177,6 +180,11 @@ StWs st_carve(int d, int r, int batch) {
   w.Rinv2 = seg((size_t)batch * r * r * 4);
   w.X0 = seg((size_t)batch * d * r * 4);
   w.X1 = seg((size_t)batch * d * r * 4);
+  const bool tcp = tc_st_ok(d, r);
+  w.Prow = seg(tcp ? tc_st_plane_bytes(d, r, batch) : 0);
+  w.Ptr = seg(tcp ? tc_st_plane_bytes(d, r, batch) : 0);
+  w.Ptr2 = seg(tcp ? tc_st_plane_bytes(d, r, batch) : 0);
+  w.Pm = seg(tcp ? tc_st_plane_bytes(r, r, batch) : 0);
   w.total = off + 256;
   return w;
 }
@@ -403,6 +411,53 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
   float* X0 = reinterpret_cast<float*>(ws + w.X0);
   float* X1 = reinterpret_cast<float*>(ws + w.X1);
   const dim3 egrid((r * r + 255) / 256, batch);
+
+  // ---- tensor-core path (Newton-Schulz retraction, d and r multiples of 128, r >= 256): every GEMM of the step
+  // as six bf16-plane MMAs (tc_stiefel.cu); MAPL_ST_TC=0 forces the FFMA kernels (debugging aid)
+  static const bool tc_enabled = !(getenv("MAPL_ST_TC") && getenv("MAPL_ST_TC")[0] == '0');
+  if (retraction == MAPL_RETRACT_NS && tc_st_ok(d, r) && tc_enabled) {
+    __nv_bfloat16* Prow = reinterpret_cast<__nv_bfloat16*>(ws + w.Prow);   // [b][3][d][r]
+    __nv_bfloat16* Ptr = reinterpret_cast<__nv_bfloat16*>(ws + w.Ptr);     // [b][3][r][d]
+    __nv_bfloat16* Ptr2 = reinterpret_cast<__nv_bfloat16*>(ws + w.Ptr2);   // [b][3][r][d]
+    __nv_bfloat16* Pm = reinterpret_cast<__nv_bfloat16*>(ws + w.Pm);       // [b][3][r][r]
+    int ksplit = d / 256 > 0 ? d / 256 : 1;                                 // Gram products: 4 k-blocks (one per TMEM accumulator) per CTA
+    if (const char* e = getenv("MAPL_ST_KSPLIT")) ksplit = atoi(e);
+    auto zero_S = [&]() -> int {
+      KernelScope ks(KID_MEMSET, st);
+      MAPL_CUDA_CHECK(cudaMemsetAsync(S, 0, (size_t)batch * r * r * 4, st));
+      return MAPL_OK;
+    };
+    // S = U^T G ;  M1 = I + lr sym(S) ;  Y = U M1 - lr G  -> X0
+    MAPL_RETURN_IF(tc_st_split(U, d, r, batch, 0, 0.f, Prow, Ptr, st));
+    MAPL_RETURN_IF(tc_st_split(G, d, r, batch, 0, 0.f, nullptr, Ptr2, st));
+    MAPL_RETURN_IF(zero_S());
+    MAPL_RETURN_IF(tc_st_gemm3(Ptr, Ptr2, r, r, d, batch, S, nullptr, 0.f, ksplit, st));
+    MAPL_RETURN_IF(tc_st_split(S, r, r, batch, 2, lr, Pm, nullptr, st));     // M1 is symmetric: its planes are B^T too
+    MAPL_RETURN_IF(tc_st_gemm3(Prow, Pm, d, r, r, batch, X0, G, -lr, 1, st));
+    if (info_out) {
+      KernelScope ks(KID_ST_FRO_NORM, st);
+      k_fro_norm<<<batch, 1024, 0, st>>>(U, X0, lr != 0.f ? 1.f / lr : 0.f, (long long)d * r, 0, info_out, 0);
+      MAPL_CUDA_CHECK(cudaGetLastError());
+    }
+    float* cur = X0;
+    float* nxt = X1;
+    for (int it = 0; it < ns_iters; ++it) {
+      MAPL_RETURN_IF(tc_st_split(cur, d, r, batch, 0, 0.f, Prow, Ptr, st));
+      MAPL_RETURN_IF(zero_S());
+      MAPL_RETURN_IF(tc_st_gemm3(Ptr, Ptr, r, r, d, batch, S, nullptr, 0.f, ksplit, st));   // X^T X
+      MAPL_RETURN_IF(tc_st_split(S, r, r, batch, 1, 0.f, Pm, nullptr, st));                 // (3I - X^T X)/2, symmetric
+      float* out = (it == ns_iters - 1) ? U : nxt;
+      MAPL_RETURN_IF(tc_st_gemm3(Prow, Pm, d, r, r, batch, out, nullptr, 0.f, 1, st));
+      nxt = cur; cur = out;
+    }
+    if (info_out) {
+      MAPL_RETURN_IF(gram(U, U, S, d, r, batch, st));
+      KernelScope ks(KID_ST_FRO_NORM, st);
+      k_fro_norm<<<batch, 1024, 0, st>>>(S, nullptr, 1.f, (long long)r * r, r, info_out, 1);
+      MAPL_CUDA_CHECK(cudaGetLastError());
+    }
+    return MAPL_OK;
+  }
 
   // tangent projection + step:  Y = U (I + lr sym(U^T G)) - lr G   -> X0
   MAPL_RETURN_IF(gram(U, G, S, d, r, batch, st));
