@@ -428,9 +428,9 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
       return MAPL_OK;
     };
     // S = U^T G ;  M1 = I + lr sym(S) ;  Y = U M1 - lr G  -> X0
+    MAPL_RETURN_IF(zero_S());
     MAPL_RETURN_IF(tc_st_split(U, d, r, batch, 0, 0.f, Prow, Ptr, st));
     MAPL_RETURN_IF(tc_st_split(G, d, r, batch, 0, 0.f, nullptr, Ptr2, st));
-    MAPL_RETURN_IF(zero_S());
     MAPL_RETURN_IF(tc_st_gemm3(Ptr, Ptr2, r, r, d, batch, S, nullptr, 0.f, ksplit, st));
     MAPL_RETURN_IF(tc_st_split(S, r, r, batch, 2, lr, Pm, nullptr, st));     // M1 is symmetric: its planes are B^T too
     MAPL_RETURN_IF(tc_st_gemm3(Prow, Pm, d, r, r, batch, X0, G, -lr, 1, st));
@@ -442,8 +442,7 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
     float* cur = X0;
     float* nxt = X1;
     for (int it = 0; it < ns_iters; ++it) {
-      MAPL_RETURN_IF(tc_st_split(cur, d, r, batch, 0, 0.f, Prow, Ptr, st));
-      MAPL_RETURN_IF(zero_S());
+      MAPL_RETURN_IF(tc_st_split(cur, d, r, batch, 0, 0.f, Prow, Ptr, st, S, (long long)r * r));   // also clears S
       MAPL_RETURN_IF(tc_st_gemm3(Ptr, Ptr, r, r, d, batch, S, nullptr, 0.f, ksplit, st));   // X^T X
       MAPL_RETURN_IF(tc_st_split(S, r, r, batch, 1, 0.f, Pm, nullptr, st));                 // (3I - X^T X)/2, symmetric
       float* out = (it == ns_iters - 1) ? U : nxt;

@@ -22,9 +22,12 @@
 // retraction inherits (measured: ||U^T U - I||_F 2.8e-5).  The k-blocks of a CTA therefore rotate over
 // FOUR TMEM accumulators (24 MMAs each per visit) that the epilogue sums in registers with
 // round-to-nearest; measured bias 7e-9, residual 2e-6, as the FFMA path.
+#include <stdlib.h>
+
 #include "profile.cuh"
 #include "tc_common.cuh"
 #include "tc_stiefel.cuh"
+#include "tc_tile_ops.cuh"
 
 namespace mapl {
 namespace {
@@ -43,9 +46,16 @@ __device__ __forceinline__ void split3(float x, __nv_bfloat16* p0, __nv_bfloat16
 }
 
 // 32 x 32 tiles; blockIdx.y = batch item.  src [rows, cols] fp32; prow / ptr may be null.
+// zero / nzero4: optional fp32 buffer (float4 count per batch item) cleared on the way (the next split-K target).
 __global__ void __launch_bounds__(256) k_st_split(const float* __restrict__ src, int rows, int cols, int mode, float lr,
-                                                  __nv_bfloat16* __restrict__ prow, __nv_bfloat16* __restrict__ ptr) {
+                                                  __nv_bfloat16* __restrict__ prow, __nv_bfloat16* __restrict__ ptr,
+                                                  float4* __restrict__ zero, long long nzero4) {
   __shared__ float tile[32][33];
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  if (zero != nullptr)
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < nzero4; i += (long long)gridDim.x * 256)
+      zero[(long long)blockIdx.y * nzero4 + i] = make_float4(0.f, 0.f, 0.f, 0.f);
   const long long plane = (long long)rows * cols;
   src += (long long)blockIdx.y * plane;
   if (prow) prow += (long long)blockIdx.y * 3 * plane;
@@ -208,18 +218,21 @@ k_tc_gemm3(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
 
 }  // namespace
 
-bool tc_st_ok(int d, int r) { return d % 128 == 0 && r % 128 == 0 && r >= 256 && r <= 1024; }
+bool tc_st_ok(int d, int r) {
+  static const int rmin = getenv("MAPL_ST_RMIN") ? atoi(getenv("MAPL_ST_RMIN")) : 256;   // experiment knob
+  return d % 128 == 0 && r % 128 == 0 && r >= rmin && r <= 1024;
+}
 
 size_t tc_st_plane_bytes(int d, int r, int batch) {   // one set of planes of a [d,r] matrix
   return align_up((size_t)batch * 3 * d * r * 2, 256);
 }
 
 int tc_st_split(const float* src, int rows, int cols, int batch, int mode, float lr, __nv_bfloat16* prow,
-                __nv_bfloat16* ptr, cudaStream_t st) {
+                __nv_bfloat16* ptr, cudaStream_t st, float* zero, long long nzero) {
   const int tiles = ((rows + 31) / 32) * ((cols + 31) / 32);
   KernelScope ks(KID_ST_SPLIT, st);
-  k_st_split<<<dim3(tiles < 1024 ? tiles : 1024, batch), 256, 0, st>>>(src, rows, cols, mode, lr, prow, ptr);
-  MAPL_CUDA_CHECK(cudaGetLastError());
+  MAPL_CUDA_CHECK(tc::launch_pdl(k_st_split, dim3(tiles < 1024 ? tiles : 1024, batch), dim3(256), 0, st, src, rows, cols, mode, lr,
+                                 prow, ptr, reinterpret_cast<float4*>(zero), nzero / 4));
   return MAPL_OK;
 }
 
@@ -247,8 +260,7 @@ int tc_st_gemm3(const __nv_bfloat16* Ap, const __nv_bfloat16* Bp, int M, int N, 
     attr_done = true;
   }
   KernelScope ks(KID_ST_GEMM3, st);
-  k_tc_gemm3<<<dim3(M / 128, N / 128, batch * p.nsplit), 192, smem, st>>>(tmA, tmB, p);
-  MAPL_CUDA_CHECK(cudaGetLastError());
+  MAPL_CUDA_CHECK(tc::launch_pdl(k_tc_gemm3, dim3(M / 128, N / 128, batch * p.nsplit), dim3(192), smem, st, tmA, tmB, p));
   return MAPL_OK;
 }
 
