@@ -420,8 +420,7 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
     __nv_bfloat16* Ptr = reinterpret_cast<__nv_bfloat16*>(ws + w.Ptr);     // [b][3][r][d]
     __nv_bfloat16* Ptr2 = reinterpret_cast<__nv_bfloat16*>(ws + w.Ptr2);   // [b][3][r][d]
     __nv_bfloat16* Pm = reinterpret_cast<__nv_bfloat16*>(ws + w.Pm);       // [b][3][r][r]
-    int ksplit = d / 256 > 0 ? d / 256 : 1;                                 // Gram products: 4 k-blocks (one per TMEM accumulator) per CTA
-    if (const char* e = getenv("MAPL_ST_KSPLIT")) ksplit = atoi(e);
+    const int ksplit = d / 256 > 0 ? d / 256 : 1;                           // Gram products: 4 k-blocks (one per TMEM accumulator) per CTA
     auto zero_S = [&]() -> int {
       KernelScope ks(KID_MEMSET, st);
       MAPL_CUDA_CHECK(cudaMemsetAsync(S, 0, (size_t)batch * r * r * 4, st));

@@ -136,8 +136,7 @@ int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks
               int32_t* codes_out, cudaStream_t st) {
   if (!tc_shape_ok(d)) return MAPL_ERR_UNSUPPORTED;
   if (d.rvq_levels != 0) return tc_encode_rvq(d, H, codebooks, pk, Zq_out, codes_out, st);
-  int tile_m = tc_tile_m(d.n_tokens);
-  if (const char* e = getenv("MAPL_ENC_SPLIT")) { if (atoi(e) == 2) tile_m = (tile_m / 2 + 7) / 8 * 8; }   // experiment
+  const int tile_m = tc_tile_m(d.n_tokens);
   CUtensorMap tmH, tmW;
   if (!make_tmap_bf16_2d(&tmH, H, (uint64_t)d.n_tokens, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)tile_m)) return MAPL_ERR_CUDA;
   if (!make_tmap_bf16_2d(&tmW, pk.WB, (uint64_t)d.r, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
@@ -145,7 +144,6 @@ int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks
   int stages = (200 * 1024) / stage_bytes;
   if (stages > 8) stages = 8;
   if (stages > d.d / BK) stages = d.d / BK;
-  if (const char* e = getenv("MAPL_ENC_STAGES")) { int v = atoi(e); if (v >= 2 && v < stages) stages = v; }   // experiment
   const size_t smem = (size_t)stages * stage_bytes + 1024 + 256;
   static bool attr_done = false;
   if (!attr_done) {
