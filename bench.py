@@ -299,6 +299,34 @@ def run_mapl(args):
         clocks = sampler.stop()
         ms = e0.elapsed_time(e1)
 
+        # ---- per-call times: one CUDA graph per entry point (all boundaries, 4 repetitions), replayed 10 times.
+        # Graph replay keeps the programmatic-dependent-launch overlap the step has, unlike the
+        # event-bracketed eager pass below, whose per-kernel times include launch latency.
+        def graph_us(fn, reps=4, replays=10):
+            for b in bs:
+                fn(b)
+            stream.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                for _ in range(reps):
+                    for b in bs:
+                        fn(b)
+            g.replay()
+            stream.synchronize()
+            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            c0.record(stream)
+            for _ in range(replays):
+                g.replay()
+            c1.record(stream)
+            stream.synchronize()
+            return 1e3 * c0.elapsed_time(c1) / (replays * reps * len(bs))
+        calls_us = {
+            "mapl_encode": graph_us(lambda b: mb.mapl_encode(b.desc, b.H, b.U, b.C, b.Zq, b.codes, b.ws)),
+            "mapl_decode": graph_us(lambda b: mb.mapl_decode(b.desc, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.Hhat, b.ws)),
+            "mapl_codec_backward": graph_us(lambda b: mb.mapl_codec_backward(
+                b.desc, b.g, b.H, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.gz, b.dU, b.dA, None, b.dH, False, b.ws)),
+        }
+
         # ---- per-kernel timing pass (same K steps, eager launches, event pair around every kernel)
         lib.mapl_profile_reset()
         lib.mapl_profile_enable(1)
@@ -386,7 +414,9 @@ def run_mapl(args):
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "note": "pinned host H,tok,g -> device; payload,Hhat,gz,dH,dU -> pinned host; uploads of step i+1 overlap downloads of step i (3 streams)"},
+        "roofline_step": roofline_step(cfg, peaks, ms / args.steps, nb, calls_us),
         "gpu_launches": launches_per_step * args.steps,
+        "calls_us": {k: round(v, 2) for k, v in calls_us.items()},
         "roofline": roof,
     }
     if rank == 0 and world == 1 and not args.no_stiefel:
@@ -432,6 +462,20 @@ def stiefel_sweep(torch, mb, I, stream, reps=10):
                                       "orth_residual_after": float(f"{res:.2e}")}
     out["config"] = "d=2048, 3 projectors per call, fixed G, lr=1e-2, fp32"
     return out
+
+
+def roofline_step(cfg, peaks, ms_per_step, nb, calls_us):
+    """Whole-config roofline: t_roof = sum over the three calls of max(bytes/peak_HBM, flops/peak_bf16),
+    per boundary; `frac` compares it with the graph-timed codec time of a boundary (Stiefel step excluded)."""
+    ab, af = alg_bytes_per_token(cfg), alg_flops_per_token(cfg)
+    N = cfg.n_tokens
+    t = {}
+    for call in ("encode", "decode", "backward"):
+        t[call] = 1e6 * max(ab[call] * N / (peaks["hbm"] * 1e9), af[call] * N / (peaks["bf16"] * 1e12))
+    codec_us = sum(calls_us.values())
+    return {"t_roof_us_per_boundary": round(sum(t.values()), 2), "per_call_us": {k: round(v, 2) for k, v in t.items()},
+            "measured_us_per_boundary": round(codec_us, 2), "frac": round(sum(t.values()) / codec_us, 3),
+            "peaks": {"hbm_gbs": peaks["hbm"], "bf16_tflops": peaks["bf16"], "source": peaks["src"]}}
 
 
 def roofline_for(name, k, cfg, peaks, total_ms):
