@@ -242,8 +242,12 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           const uint64_t da = desc_kmajor_sw128(a + k * 32);
-          umma_bf16_pair(tmem_base, da, desc_kmajor_sw128(bh + k * 32), idesc1, (kb | k) != 0);
-          umma_bf16_pair(tmem_base, da, desc_kmajor_sw128(bl + k * 32), idesc1, 1);
+          // even / odd k-blocks accumulate into two TMEM regions ([0,r) and the still unused score stages at
+          // [256,256+r)): the tensor core truncates when it adds into its accumulator, and halving the chain of
+          // MMAs halves that one-sided error of z (tc_stiefel.cu measures it); the epilogue adds the two halves
+          const uint32_t acc = tmem_base + (uint32_t)(kb & 1) * kAccCol0;
+          umma_bf16_pair(acc, da, desc_kmajor_sw128(bh + k * 32), idesc1, (kb >= 2) || k != 0);
+          umma_bf16_pair(acc, da, desc_kmajor_sw128(bl + k * 32), idesc1, 1);
         }
         umma_commit_pair(&s.s1_empty[st]);
       }
@@ -294,6 +298,18 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
     if (warp == 2) { DBG(1) }
     tc_fence_after_sync();
     float n2, amax;
+    if (nkb1 >= 2) {                     // z = even-k-block half + odd-k-block half (see the MMA issuer)
+      for (int pc = h; pc < p.r / 32; pc += 2) {
+        uint32_t v[32], w[32];
+        tmem_ld32(tmem_row + pc * 32, v);
+        tmem_ld32(tmem_row + kAccCol0 + pc * 32, w);
+        tmem_ld_wait();
+#pragma unroll
+        for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(__uint_as_float(v[i]) + __uint_as_float(w[i]));
+        tmem_st32(tmem_row + pc * 32, v);
+      }
+      tmem_st_wait();
+    }
     rho_subtract(tmem_row, nullptr, p.r, h, &n2, &amax);
     xN2[mine] = n2; xAmax[mine] = amax;
     asm volatile("bar.sync 1, 256;" ::: "memory");
