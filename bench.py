@@ -510,11 +510,15 @@ def roofline_for(name, k, cfg, peaks, total_ms):
         ach = byt / avg_s / 1e9
         return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": peaks["hbm"], "unit": "GB/s",
                 "frac": ach / peaks["hbm"], "traffic": traffic, "peak_source": peaks["src"] + " (burst copy)",
-                "avg_us": avg_s * 1e6, "alg_bytes_per_launch": byt}
+                "avg_us": avg_s * 1e6, "alg_bytes_per_launch": byt,
+                "note": "avg_us is event-bracketed per launch (no dependent-launch overlap, ~5 us of launch latency "
+                        "inside the pair): a lower bound on frac; calls_us / roofline_step are graph-timed"}
     ach = flo / avg_s / 1e12
     return {"kernel": name, "bound": "tensor", "achieved": ach, "peak": peaks["bf16"], "unit": "TFLOP/s",
             "frac": ach / peaks["bf16"], "traffic": traffic, "peak_source": peaks["src"] + " (burst bf16)",
-            "avg_us": avg_s * 1e6, "alg_flops_per_launch": flo}
+            "avg_us": avg_s * 1e6, "alg_flops_per_launch": flo,
+            "note": "avg_us is event-bracketed per launch (no dependent-launch overlap): a lower bound on frac; "
+                    "calls_us / roofline_step are graph-timed"}
 
 
 # ---------------------------------------------------------------- the oracle arm (CPU baseline)
