@@ -3,14 +3,19 @@
 // k_tc_bwd_gz   one CTA per token tile, CTAs in pairs (cta_group::2, M = 256: every parameter byte is
 //               read from L2 once per pair); two phases over one read of g:
 //     phase 1   [gz | gA] = g . [U | B^T]         K = d, streamed through a TMA ring
-//               epilogue: gz -> bf16 -> gz_out (the backward wire payload) and -> smem as the A
-//               operand of phase 2; gA rows -> fp32 scratch [N,ra]
+//               epilogue (8 warps): gz -> bf16 -> swizzled smem tiles that are both the A operand of
+//               phase 2 and the source of the TMA store to gz_out (the backward wire payload);
+//               gA rows -> fp32 scratch [N,ra] (TMA store from staging boxes when ra = 64).
+//               With RVQ the same warps first dequantise the tile's codes into the bf16 Zhat
+//               operand of k_tc_bwd_du (hidden under the g stream).
 //     phase 2   dH = gz . U^T                     the chunk pipeline of tc_tile_ops.cuh
 //               While phase 1 streams, the epilogue warps zero dU / dA / dB (overwrite mode): no
 //               separate memset launches.
 // k_tc_bwd_du   dU[d-tile, :] += sum over a token range of  g^T Zhat + H^T gz.  Both operands are
 //               MN-major (tokens are the contraction index): TMA boxes [64 tokens x 64 cols]
 //               are used as they land.  Split over token ranges; fp32 vector atomics into dU.
+//               r >= 128: CTA pairs (two d-tiles, M = 256, half of the Zhat / gz columns per CTA).
+//               Its main loop streams g and H at 6.2 TB/s (measured, c1).
 //               While the MMAs run, the epilogue warps scatter-add the gA rows into dA[tok]:
 //               per 128-token block the ids are ranked in shared memory and rows of equal id are
 //               summed in registers (Zipf ids: the hottest id owns ~14 % of all rows), then one
