@@ -66,104 +66,66 @@ __global__ void k_fro_norm(const float* __restrict__ X, const float* __restrict_
   }
 }
 
-// In-place upper Cholesky G = R^T R of a symmetric positive definite [r,r] matrix (row-major; the
-// strict lower triangle is zeroed).  Right-looking, blocked by NB; one CTA per batch item.
-__global__ void __launch_bounds__(1024) k_chol_upper(float* __restrict__ Gb, int r) {
-  extern __shared__ __align__(16) float sm[];
-  float(*D)[NB + 1] = reinterpret_cast<float(*)[NB + 1]>(sm);
-  float* P = sm + NB * (NB + 1) + 3;                 // panel [NB][ldp]
-  P = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(P) + 15) & ~uintptr_t(15));
+// One panel step of the in-place upper Cholesky G = R^T R (row-major [r,r], right-looking, blocked by NB;
+// one CTA per batch item): factor the diagonal block at p, zero the strict lower part of its columns,
+// solve the panel rows R[p:p+nb, p+nb:].  The trailing update G[p+nb:, p+nb:] -= R_panel^T R_panel is a
+// multi-CTA launch of k_st_gemm (chol_upper below).
+__global__ void __launch_bounds__(256) k_chol_panel(float* __restrict__ Gb, int r, int p) {
+  __shared__ float D[NB][NB + 1];
   float* G = Gb + (long long)blockIdx.x * r * r;
   const int tid = threadIdx.x, lane = tid % 32, warp = tid / 32;
-
-  for (int p = 0; p < r; p += NB) {
-    const int nb = min(NB, r - p);
-    for (int idx = tid; idx < nb * nb; idx += blockDim.x) {
-      const int a = idx / nb, b = idx % nb;
-      D[a][b] = G[(long long)(p + a) * r + p + b];
-    }
-    __syncthreads();
-    if (warp == 0) {
-      for (int j = 0; j < nb; ++j) {
-        const float dj = sqrtf(D[j][j]);
-        __syncwarp();
-        if (lane == j) D[j][j] = dj;
-        if (lane > j && lane < nb) D[j][lane] = D[j][lane] / dj;
-        __syncwarp();
-        if (lane > j && lane < nb) {
-          const float dji = D[j][lane];
-          for (int a = j + 1; a <= lane; ++a) D[a][lane] -= D[j][a] * dji;
-        }
-        __syncwarp();
+  const int nb = min(NB, r - p);
+  for (int idx = tid; idx < nb * nb; idx += blockDim.x) {
+    const int a = idx / nb, b = idx % nb;
+    D[a][b] = G[(long long)(p + a) * r + p + b];
+  }
+  __syncthreads();
+  if (warp == 0) {
+    // the 32 x 32 block lives in registers, lane = column (col[a] = D[a][lane]); row j is exchanged by shuffles.
+    // Rows / columns past nb are padded with the identity.
+    float col[NB];
+#pragma unroll
+    for (int a = 0; a < NB; ++a) col[a] = (a < nb && lane < nb) ? D[a][lane] : (a == lane ? 1.f : 0.f);
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {
+      const float dj = sqrtf(__shfl_sync(0xffffffffu, col[j], j));
+      const float rowj = lane == j ? dj : (lane > j ? col[j] / dj : col[j]);     // R[j][lane]
+      col[j] = rowj;
+#pragma unroll
+      for (int a = j + 1; a < NB; ++a) {
+        const float dja = __shfl_sync(0xffffffffu, rowj, a);                      // R[j][a]
+        if (a <= lane) col[a] = fmaf(-dja, rowj, col[a]);
       }
     }
-    __syncthreads();
-    for (int idx = tid; idx < nb * nb; idx += blockDim.x) {
-      const int a = idx / nb, b = idx % nb;
-      G[(long long)(p + a) * r + p + b] = (b >= a) ? D[a][b] : 0.f;
+#pragma unroll
+    for (int a = 0; a < NB; ++a)
+      if (a < nb && lane < nb) D[a][lane] = col[a];
+  }
+  __syncthreads();
+  for (int idx = tid; idx < nb * nb; idx += blockDim.x) {
+    const int a = idx / nb, b = idx % nb;
+    G[(long long)(p + a) * r + p + b] = (b >= a) ? D[a][b] : 0.f;
+  }
+  const int ncols = r - p - nb;
+  if (ncols <= 0) return;
+  // zero the block below the panel rows (strict lower part of R)
+  for (int idx = tid; idx < ncols * nb; idx += blockDim.x) {
+    const int i = idx / nb, b = idx % nb;
+    G[(long long)(p + nb + i) * r + p + b] = 0.f;
+  }
+  // panel: solve D^T x = G[p..p+nb, c]
+  for (int c = tid; c < ncols; c += blockDim.x) {
+    float x[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {
+      float s = j < nb ? G[(long long)(p + j) * r + p + nb + c] : 0.f;
+#pragma unroll
+      for (int k = 0; k < j; ++k) s = fmaf(-D[k][j], x[k], s);
+      x[j] = j < nb ? s / D[j][j] : 0.f;
     }
-    const int ncols = r - p - nb;
-    if (ncols <= 0) break;
-    const int ldp = (ncols + 3) & ~3;
-    // zero the block below the panel rows (strict lower part of R)
-    for (int idx = tid; idx < ncols * nb; idx += blockDim.x) {
-      const int i = idx / nb, b = idx % nb;
-      G[(long long)(p + nb + i) * r + p + b] = 0.f;
-    }
-    // panel: solve D^T x = G[p..p+nb, c]
-    for (int c = tid; c < ldp; c += blockDim.x) {
-      float x[NB];
-      if (c < ncols) {
 #pragma unroll
-        for (int j = 0; j < NB; ++j) {
-          float s = G[(long long)(p + j) * r + p + nb + c];
-#pragma unroll
-          for (int k = 0; k < j; ++k) s = fmaf(-D[k][j], x[k], s);
-          x[j] = s / D[j][j];
-        }
-#pragma unroll
-        for (int j = 0; j < NB; ++j) {
-          G[(long long)(p + j) * r + p + nb + c] = x[j];
-          P[j * ldp + c] = x[j];
-        }
-      } else {
-#pragma unroll
-        for (int j = 0; j < NB; ++j) P[j * ldp + c] = 0.f;
-      }
-    }
-    __syncthreads();
-    // trailing update of the upper triangle
-    const int nblk = ldp / 4;
-    for (int blk = tid; blk < nblk * nblk; blk += blockDim.x) {
-      const int bi = blk / nblk, bj = blk % nblk;
-      if (bj < bi) continue;
-      float acc[4][4];
-#pragma unroll
-      for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
-#pragma unroll 8
-      for (int k = 0; k < NB; ++k) {
-        const float4 a = *reinterpret_cast<const float4*>(&P[k * ldp + bi * 4]);
-        const float4 b = *reinterpret_cast<const float4*>(&P[k * ldp + bj * 4]);
-        const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {b.x, b.y, b.z, b.w};
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-          for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(av[i], bv[j], acc[i][j]);
-      }
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const int gi = bi * 4 + i;
-        if (gi >= ncols) continue;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int gj = bj * 4 + j;
-          if (gj < ncols && gj >= gi) G[(long long)(p + nb + gi) * r + p + nb + gj] -= acc[i][j];
-        }
-      }
-    }
-    __syncthreads();
+    for (int j = 0; j < NB; ++j)
+      if (j < nb) G[(long long)(p + j) * r + p + nb + c] = x[j];
   }
 }
 
@@ -208,7 +170,8 @@ constexpr int LA = TM * TK / 4 / 256, LB = TN * TK / 4 / 256;   // float4 loads 
 template <bool kGram>
 __global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, const float* __restrict__ B, float* __restrict__ C,
                                                  const float* __restrict__ E, float alpha, float beta, int M, int N, int K, int kper,
-                                                 long long sA, long long sB, long long sC, int upper_only) {
+                                                 long long sA, long long sB, long long sC, int upper_only,
+                                                 int lda, int ldb, int ldc) {      // row pitches (elements) of A, B, C / E
   __shared__ __align__(16) float As[2][TK][TM + TPAD];
   __shared__ __align__(16) float Bs[2][TK][TN + TPAD];
   const int t = threadIdx.x, tx = t % 16, ty = t / 16;      // thread tile: rows ty*RM..+RM-1, cols tx*4..+3
@@ -224,7 +187,6 @@ __global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, co
   const int kbeg = blockIdx.y * kper, kend = min(K, kbeg + kper);
   A += (long long)blockIdx.z * sA; B += (long long)blockIdx.z * sB; C += (long long)blockIdx.z * sC;
   if (E) E += (long long)blockIdx.z * sC;
-  const int lda = kGram ? M : K;                 // gram: A is [K(d), M(r)];  rmul: A is [M(d), K(r)]
   float acc[RM][4];
 #pragma unroll
   for (int i = 0; i < RM; ++i)
@@ -240,7 +202,7 @@ __global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, co
 #pragma unroll
     for (int i = 0; i < LB; ++i) {   // B tile [TK][TN]: row k, 4 consecutive n
       const int f = t + i * 256, k = k0 + f / (TN / 4), n = n0 + (f % (TN / 4)) * 4;
-      rb[i] = (k < kend && n < N) ? __ldg(reinterpret_cast<const float4*>(B + (long long)k * N + n)) : z;
+      rb[i] = (k < kend && n < N) ? __ldg(reinterpret_cast<const float4*>(B + (long long)k * ldb + n)) : z;
     }
 #pragma unroll
     for (int i = 0; i < LA; ++i) {
@@ -301,14 +263,14 @@ __global__ void __launch_bounds__(256) k_st_gemm(const float* __restrict__ A, co
   for (int i = 0; i < RM; ++i) {
     const int m = m0 + ty * RM + i, n = n0 + tx * 4;
     if (m >= M || n >= N) continue;
-    float* dst = C + (long long)m * N + n;
+    float* dst = C + (long long)m * ldc + n;
     if (kGram) {
-      asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(acc[i][0]), "f"(acc[i][1]),
-                   "f"(acc[i][2]), "f"(acc[i][3]) : "memory");
+      asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(alpha * acc[i][0]), "f"(alpha * acc[i][1]),
+                   "f"(alpha * acc[i][2]), "f"(alpha * acc[i][3]) : "memory");
     } else {
       float4 v = make_float4(alpha * acc[i][0], alpha * acc[i][1], alpha * acc[i][2], alpha * acc[i][3]);
       if (E) {
-        const float4 e = __ldg(reinterpret_cast<const float4*>(E + (long long)m * N + n));
+        const float4 e = __ldg(reinterpret_cast<const float4*>(E + (long long)m * ldc + n));
         v.x = fmaf(beta, e.x, v.x); v.y = fmaf(beta, e.y, v.y); v.z = fmaf(beta, e.z, v.z); v.w = fmaf(beta, e.w, v.w);
       }
       *reinterpret_cast<float4*>(dst) = v;
@@ -329,7 +291,7 @@ int gram(const float* X, const float* X2, float* Gm, int d, int r, int batch, cu
   splits = (d + kper - 1) / kper;
   KernelScope ks(KID_ST_GEMM, st);
   k_st_gemm<true><<<dim3(tiles, splits, batch), 256, 0, st>>>(X, X2, Gm, nullptr, 1.f, 0.f, r, r, d, kper, (long long)d * r,
-                                                            (long long)d * r, (long long)r * r, upper_only ? 1 : 0);
+                                                            (long long)d * r, (long long)r * r, upper_only ? 1 : 0, r, r, r);
   MAPL_CUDA_CHECK(cudaGetLastError());
   return MAPL_OK;
 }
@@ -340,8 +302,31 @@ int right_mul(const float* X, const float* M, float* C, const float* E, float be
   const int tiles = ((rows + TM - 1) / TM) * ((r + TN - 1) / TN);
   KernelScope ks(KID_ST_GEMM, st);
   k_st_gemm<false><<<dim3(tiles, 1, batch), 256, 0, st>>>(X, M, C, E, alpha, beta, rows, r, r, r, (long long)rows * r,
-                                                         (long long)r * r, (long long)rows * r, 0);
+                                                         (long long)r * r, (long long)rows * r, 0, r, r, r);
   MAPL_CUDA_CHECK(cudaGetLastError());
+  return MAPL_OK;
+}
+
+// In-place upper Cholesky of `batch` SPD [r,r] matrices (upper triangle read; strict lower part zeroed):
+// per 32-column panel one single-CTA panel kernel and one multi-CTA trailing update.
+int chol_upper(float* G, int r, int batch, cudaStream_t st) {
+  for (int p = 0; p < r; p += NB) {
+    const int nb = r - p < NB ? r - p : NB;
+    {
+      KernelScope ks(KID_ST_CHOL, st);
+      k_chol_panel<<<batch, 256, 0, st>>>(G, r, p);      // 256 threads: the register-resident block needs > 64 registers
+      MAPL_CUDA_CHECK(cudaGetLastError());
+    }
+    const int ncols = r - p - nb;
+    if (ncols <= 0) break;
+    const int nt = (ncols + TN - 1) / TN;
+    const float* P = G + (long long)p * r + p + nb;                 // panel rows [nb, ncols], pitch r
+    float* T = G + (long long)(p + nb) * r + p + nb;                // trailing block, pitch r
+    KernelScope ks(KID_ST_GEMM, st);
+    k_st_gemm<true><<<dim3(nt * (nt + 1) / 2, 1, batch), 256, 0, st>>>(P, P, T, nullptr, -1.f, 0.f, ncols, ncols, nb, nb,
+                                                                      (long long)r * r, (long long)r * r, (long long)r * r, 1, r, r, r);
+    MAPL_CUDA_CHECK(cudaGetLastError());
+  }
   return MAPL_OK;
 }
 
@@ -481,18 +466,10 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
     }
   } else {
     // CholeskyQR2: Y = Q1 R1, Q1 = Q R2  =>  Y = Q (R2 R1), upper triangular with positive diagonal
-    const int ldp = (r + 3) & ~3;
-    const size_t smem = (size_t)(NB * (NB + 1) + 8 + NB * ldp) * 4;
-    static bool attr_done = false;
-    if (!attr_done) {
-      MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_chol_upper, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-      attr_done = true;
-    }
     const float* src = X0;
     for (int pass = 0; pass < 2; ++pass) {
-      MAPL_RETURN_IF(gram(src, src, S, d, r, batch, st, true));   // k_chol_upper reads the upper triangle only
-      { KernelScope ks(KID_ST_CHOL, st); k_chol_upper<<<batch, 1024, smem, st>>>(S, r); }
-      MAPL_CUDA_CHECK(cudaGetLastError());
+      MAPL_RETURN_IF(gram(src, src, S, d, r, batch, st, true));   // chol_upper reads the upper triangle only
+      MAPL_RETURN_IF(chol_upper(S, r, batch, st));
       float* Xinv = nullptr;
       MAPL_RETURN_IF(tri_inverse_newton(S, Rinv, Rinv2, M, &Xinv, r, batch, st));
       float* out = pass == 0 ? X1 : U;
