@@ -205,7 +205,7 @@ def make_step(bs, mb, stiefel=None):
 
     def fwd(b):
         if b.pack is not None and stiefel is not None:
-            mb.mapl_pack_params(b.desc, b.U, b.B, None, b.pack)     # U changed (Stiefel step); codebooks did not
+            mb.mapl_pack_params(b.desc, b.U, None, None, b.pack)    # U changed (Stiefel step); B and the codebooks did not
         mb.mapl_encode(b.desc, b.H, b.U, b.C, b.Zq, b.codes, b.ws)
         mb.mapl_decode(b.desc, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.Hhat, b.ws)
 

@@ -92,10 +92,10 @@ size_t mapl_stiefel_workspace_bytes(int32_t d, int32_t r, int32_t batch);
  * boundary runs on the fp32 kernels: then pack_out may be NULL and the call is a no-op).  In the
  * paper's schedule the parameters change once per optimizer step while ~128 micro-batches cross
  * the boundary, so the pack is made once per step and referenced from
- * desc.param_pack.  B / codebooks may be NULL when anchor_rank / rvq_levels is 0.  With
- * rvq_levels > 0, codebooks == NULL re-packs U (and B) only and leaves the codebook section of an
- * existing pack as it is: the call to make after a projector update (mapl_stiefel_step), since
- * the codebooks did not change.  The first pack of a buffer must pass the codebooks.               */
+ * desc.param_pack.  B / codebooks may be NULL when anchor_rank / rvq_levels is 0.  Otherwise a
+ * NULL B or NULL codebooks leaves that section of an existing pack as it is: after a projector
+ * update (mapl_stiefel_step) call it with U alone, since B and the codebooks did not change.  The
+ * first pack of a buffer must pass everything the descriptor uses.                                */
 size_t mapl_param_pack_bytes(const mapl_boundary_desc* desc);
 int mapl_pack_params(const mapl_boundary_desc* desc, const float* U, const float* B, const float* codebooks,
                      void* pack_out, void* cuda_stream);

@@ -101,9 +101,8 @@ int mapl_pack_params(const mapl_boundary_desc* desc, const float* U, const float
   const TcPack lay = tc_pack_layout(d, reinterpret_cast<char*>(pack_out));
   if (lay.bytes == 0) return MAPL_OK;                       // fp32 kernels read the masters directly
   if (!U || !pack_out) return MAPL_ERR_INVALID_ARG;
-  if (d.anchor_rank > 0 && !B) return MAPL_ERR_INVALID_ARG;
-  // codebooks == NULL with rvq_levels > 0: the codebook section of an existing pack is left as it is
-  // (re-pack after a projector update only)
+  // B == NULL with anchor_rank > 0 / codebooks == NULL with rvq_levels > 0: that section of an existing pack is
+  // left as it is (re-pack after a projector update only)
   if (!all16({U, B, codebooks}) || (reinterpret_cast<uintptr_t>(pack_out) & 255u)) return MAPL_ERR_ALIGNMENT;
   return tc_pack_build(d, U, B, codebooks, lay, reinterpret_cast<cudaStream_t>(cuda_stream));
 }

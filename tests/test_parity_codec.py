@@ -223,7 +223,7 @@ def test_projector_only_repack_equals_full_repack():
         torch.cuda.synchronize()
         return codes.cpu().numpy(), Hhat.float().cpu().numpy()
 
-    mb.mapl_pack_params(desc, U2, dev.B, None, pack)          # projector-only re-pack
+    mb.mapl_pack_params(desc, U2, None, None, pack)           # projector-only re-pack
     a = run()
     mb.mapl_pack_params(desc, U2, dev.B, dev.C, pack)         # complete re-pack
     b = run()
