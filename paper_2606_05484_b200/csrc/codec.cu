@@ -259,7 +259,14 @@ int mapl_codec_backward(const mapl_boundary_desc* desc, const void* g_Hhat, cons
     g.C = gz_out; g.c_bf16 = bf; g.ldc = d.r;
     MAPL_RETURN_IF(simt_gemm(g, st));
   }
-  const int splits = (int)((N + 1023) / 1024);
+  // split the token contraction so that tiles x splits covers about two waves of the 148 SMs (>= 64 tokens each)
+  auto splits_for = [&](int m, int n) {
+    const long long tiles = (long long)((m + 63) / 64) * ((n + 63) / 64);
+    long long sp = (2 * 148 + tiles - 1) / tiles;
+    const long long max_sp = (N + 63) / 64;
+    if (sp > max_sp) sp = max_sp;
+    return (int)(sp < 1 ? 1 : sp);
+  };
   {  // dU += g^T zhat (+ H^T gz)
     GemmArgs g;
     g.M = d.d; g.N = d.r; g.K[0] = (int)N;
@@ -270,7 +277,7 @@ int mapl_codec_backward(const mapl_boundary_desc* desc, const void* g_Hhat, cons
       g.A[1].p = H; g.A[1].bf16 = bf; g.A[1].so = 1; g.A[1].sk = d.d;
       g.B[1].p = gz_out; g.B[1].bf16 = bf; g.B[1].so = 1; g.B[1].sk = d.r;
     }
-    g.C = dU_out; g.ldc = d.r; g.atomic = 1; g.splits = splits;
+    g.C = dU_out; g.ldc = d.r; g.atomic = 1; g.splits = splits_for(d.d, d.r);
     MAPL_RETURN_IF(simt_gemm(g, st));
   }
   if (dH_out) {  // dH = gz U^T
@@ -297,7 +304,7 @@ int mapl_codec_backward(const mapl_boundary_desc* desc, const void* g_Hhat, cons
       g.M = ra; g.N = d.d; g.K[0] = (int)N;
       g.A[0].p = A; g.A[0].so = 1; g.A[0].sk = ra; g.A[0].gather = tok; g.A[0].gmode = 2;
       g.B[0].p = g_Hhat; g.B[0].bf16 = bf; g.B[0].so = 1; g.B[0].sk = d.d;
-      g.C = dB_out; g.ldc = d.d; g.atomic = 1; g.splits = splits;
+      g.C = dB_out; g.ldc = d.d; g.atomic = 1; g.splits = splits_for(ra, d.d);
       MAPL_RETURN_IF(simt_gemm(g, st));
     }
   }
