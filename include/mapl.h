@@ -143,6 +143,24 @@ int mapl_codec_backward(const mapl_boundary_desc* desc, const void* g_Hhat, cons
                         float* dB_out, void* dH_out, int accumulate, void* workspace,
                         size_t workspace_bytes, void* cuda_stream);
 
+/* SENDER-SIDE ANCHOR CENTRING (Eq. 1 in full; SURVEY 8f "next" row 1, reading S6).  The hot path
+ * takes h as the already centred residual; these two calls add the subtraction of the sender's own
+ * factorised anchor (Eq. 3):
+ *     z = U^T (h - A_s[tok] B_s)  =  U^T h - T[tok],      T = A_s (B_s U)   [V,r] fp32.
+ * mapl_center_table forms T once per parameter update (two small fp32 GEMMs; `workspace` of
+ * mapl_center_workspace_bytes(desc) bytes holds B_s U); mapl_encode_centered is mapl_encode with the row
+ * T[tok_n] subtracted from the fp32 accumulator of token n before anything is rounded or quantised, so
+ * the RVQ codes are those of the centred z.  Arguments as mapl_encode, plus tok [N] int32 (0 <= tok < V)
+ * and center_table [V,r] fp32.  A_s [V,ra], B_s [ra,d] (the sender's anchor factors; desc.vocab and
+ * desc.anchor_rank describe them).  The backward of the centring term (dA_s, and -B_s^T A_s[tok]^T gz in dU)
+ * is not built yet.                                                                                  */
+size_t mapl_center_workspace_bytes(const mapl_boundary_desc* desc);
+int mapl_center_table(const mapl_boundary_desc* desc, const float* A_s, const float* B_s, const float* U,
+                      float* table_out, void* workspace, size_t workspace_bytes, void* cuda_stream);
+int mapl_encode_centered(const mapl_boundary_desc* desc, const void* H, const int32_t* tok, const float* center_table,
+                         const float* U, const float* codebooks, void* Zq_out, int32_t* codes_out, void* workspace,
+                         size_t workspace_bytes, void* cuda_stream);
+
 /* STIEFEL STEP on `batch` independent projectors, U_inout and G strided [batch,d,r] fp32.
  *   S = U^T G;  xi = G - U (S + S^T)/2 (Eq. 4);  Y = U - lr xi;
  *   MAPL_RETRACT_QR: U <- Q of the thin QR of Y with diag(R) > 0 (unique, S17);

@@ -51,6 +51,12 @@ def _load():
     lib.mapl_pack_params.restype = C.c_int
     lib.mapl_pack_params.argtypes = [dp, vp, vp, vp, vp, vp]
     lib.mapl_encode.argtypes = [dp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.mapl_center_workspace_bytes.restype = sz
+    lib.mapl_center_workspace_bytes.argtypes = [dp]
+    lib.mapl_center_table.restype = C.c_int
+    lib.mapl_center_table.argtypes = [dp, vp, vp, vp, vp, vp, sz, vp]
+    lib.mapl_encode_centered.restype = C.c_int
+    lib.mapl_encode_centered.argtypes = [dp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.mapl_decode.argtypes = [dp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.mapl_codec_backward.argtypes = [dp] + [vp] * 14 + [C.c_int, vp, sz, vp]
     lib.mapl_stiefel_step.argtypes = [i32, i32, i32, vp, vp, f32, i32, i32, vp, vp, sz, vp]
@@ -145,6 +151,27 @@ def mapl_encode(desc: BoundaryDesc, H, U, codebooks, Zq_out, codes_out, workspac
                             _ptr(codebooks, torch.float32, "codebooks"), _ptr(Zq_out, act, "Zq_out"),
                             _ptr(codes_out, torch.int32, "codes_out"), _ptr(workspace, None, "workspace"),
                             workspace.numel() * workspace.element_size(), _stream()), "mapl_encode")
+
+
+def mapl_center_workspace_bytes(desc: BoundaryDesc) -> int:
+    return int(_lib.mapl_center_workspace_bytes(C.byref(desc)))
+
+
+def mapl_center_table(desc: BoundaryDesc, A_s, B_s, U, table_out, workspace) -> None:
+    """T = A_s (B_s U), [V,r] fp32: the per-token-id centring rows of mapl_encode_centered (Eq. 1)."""
+    f = torch.float32
+    _check(_lib.mapl_center_table(C.byref(desc), _ptr(A_s, f, "A_s"), _ptr(B_s, f, "B_s"), _ptr(U, f, "U"),
+                                  _ptr(table_out, f, "table_out"), _ptr(workspace, None, "workspace"),
+                                  workspace.numel() * workspace.element_size(), _stream()), "mapl_center_table")
+
+
+def mapl_encode_centered(desc: BoundaryDesc, H, tok, center_table, U, codebooks, Zq_out, codes_out, workspace) -> None:
+    act = act_torch_dtype(desc)
+    _check(_lib.mapl_encode_centered(
+        C.byref(desc), _ptr(H, act, "H"), _ptr(tok, torch.int32, "tok"), _ptr(center_table, torch.float32, "center_table"),
+        _ptr(U, torch.float32, "U"), _ptr(codebooks, torch.float32, "codebooks"), _ptr(Zq_out, act, "Zq_out"),
+        _ptr(codes_out, torch.int32, "codes_out"), _ptr(workspace, None, "workspace"),
+        workspace.numel() * workspace.element_size(), _stream()), "mapl_encode_centered")
 
 
 def mapl_decode(desc: BoundaryDesc, Z, codes, U, codebooks, tok, A, B, Hhat_out, workspace) -> None:

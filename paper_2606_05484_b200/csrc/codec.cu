@@ -112,17 +112,19 @@ size_t mapl_workspace_bytes(const mapl_boundary_desc* desc) {
   return carve(*desc).total;
 }
 
-int mapl_encode(const mapl_boundary_desc* desc, const void* H, const float* U, const float* codebooks,
-                void* Zq_out, int32_t* codes_out, void* workspace, size_t workspace_bytes,
-                void* cuda_stream) {
+// shared by mapl_encode (tok == Tc == NULL) and mapl_encode_centered
+static int encode_impl(const mapl_boundary_desc* desc, const void* H, const float* U, const float* codebooks,
+                       const int32_t* tok, const float* Tc, void* Zq_out, int32_t* codes_out, void* workspace,
+                       size_t workspace_bytes, void* cuda_stream) {
   MAPL_RETURN_IF(validate_desc(desc));
   const mapl_boundary_desc& d = *desc;
   const int L = d.rvq_levels;
   if (d.n_tokens == 0) return MAPL_OK;           // nothing to do; empty tensors may be NULL
   if (!H || !U) return MAPL_ERR_INVALID_ARG;
+  if ((tok == nullptr) != (Tc == nullptr)) return MAPL_ERR_INVALID_ARG;
   if (L == 0 && !Zq_out) return MAPL_ERR_INVALID_ARG;
   if (L > 0 && (!codes_out || !codebooks)) return MAPL_ERR_INVALID_ARG;
-  if (!all16({H, U, codebooks, Zq_out, codes_out, workspace})) return MAPL_ERR_ALIGNMENT;
+  if (!all16({H, U, codebooks, Zq_out, codes_out, workspace, tok, Tc})) return MAPL_ERR_ALIGNMENT;
   const Ws w = carve(d);
   if (!workspace || workspace_bytes < w.total) return MAPL_ERR_WORKSPACE;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
@@ -131,22 +133,56 @@ int mapl_encode(const mapl_boundary_desc* desc, const void* H, const float* U, c
   if (tc_shape_ok(d) && (L == 0 || tc_rvq_ok(d))) {
     TcPack pk;
     MAPL_RETURN_IF(resolve_pack(d, U, nullptr, codebooks, ws, w, st, &pk));
-    int s = tc_encode(d, H, codebooks, pk, Zq_out, codes_out, st);
+    int s = tc_encode(d, H, codebooks, pk, Zq_out, codes_out, st, tok, Tc);
     if (s != MAPL_ERR_UNSUPPORTED) return s;
   }
 
   const int bf = d.act_dtype == MAPL_BF16;
-  if (L == 0) {   // Z = H U
+  if (L == 0) {   // Z = H U (- Tc[tok])
     GemmArgs g;
     g.M = (int)d.n_tokens; g.N = d.r; g.K[0] = d.d;
     g.A[0].p = H; g.A[0].bf16 = bf; g.A[0].so = d.d; g.A[0].sk = 1;
     g.B[0].p = U; g.B[0].so = 1; g.B[0].sk = d.r;
     g.C = Zq_out; g.c_bf16 = bf; g.ldc = d.r;
-    return simt_gemm(g, st);
+    MAPL_RETURN_IF(simt_gemm(g, st));
+    if (Tc) MAPL_RETURN_IF(simt_center_rows(Zq_out, bf, tok, Tc, d.n_tokens, d.r, st));
+    return MAPL_OK;
   }
   float* hn = reinterpret_cast<float*>(ws + w.half_norm);
   MAPL_RETURN_IF(simt_half_sqnorm(codebooks, hn, L * d.rvq_k, d.r, st));
-  return simt_encode_rvq(d, H, U, codebooks, hn, Zq_out, codes_out, st);
+  return simt_encode_rvq(d, H, U, codebooks, hn, Zq_out, codes_out, st, tok, Tc);
+}
+
+int mapl_encode(const mapl_boundary_desc* desc, const void* H, const float* U, const float* codebooks,
+                void* Zq_out, int32_t* codes_out, void* workspace, size_t workspace_bytes,
+                void* cuda_stream) {
+  return encode_impl(desc, H, U, codebooks, nullptr, nullptr, Zq_out, codes_out, workspace, workspace_bytes, cuda_stream);
+}
+
+int mapl_encode_centered(const mapl_boundary_desc* desc, const void* H, const int32_t* tok, const float* center_table,
+                         const float* U, const float* codebooks, void* Zq_out, int32_t* codes_out, void* workspace,
+                         size_t workspace_bytes, void* cuda_stream) {
+  if (!tok || !center_table) return MAPL_ERR_INVALID_ARG;
+  return encode_impl(desc, H, U, codebooks, tok, center_table, Zq_out, codes_out, workspace, workspace_bytes, cuda_stream);
+}
+
+size_t mapl_center_workspace_bytes(const mapl_boundary_desc* desc) {
+  if (validate_desc(desc) != MAPL_OK || desc->anchor_rank <= 0) return 0;
+  return align_up((size_t)desc->anchor_rank * desc->r * 4, 256) + 256;
+}
+
+int mapl_center_table(const mapl_boundary_desc* desc, const float* A_s, const float* B_s, const float* U,
+                      float* table_out, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  MAPL_RETURN_IF(validate_desc(desc));
+  const mapl_boundary_desc& d = *desc;
+  if (d.anchor_rank <= 0 || d.vocab < 1) return MAPL_ERR_INVALID_ARG;
+  if (!A_s || !B_s || !U || !table_out) return MAPL_ERR_INVALID_ARG;
+  if (!all16({A_s, B_s, U, table_out, workspace})) return MAPL_ERR_ALIGNMENT;
+  if (!workspace || workspace_bytes < mapl_center_workspace_bytes(desc)) return MAPL_ERR_WORKSPACE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  float* Wc = reinterpret_cast<float*>(workspace);                       // [ra, r] = B_s U
+  MAPL_RETURN_IF(st_gemm_nn(B_s, U, Wc, d.anchor_rank, d.r, d.d, st));
+  return st_gemm_nn(A_s, Wc, table_out, d.vocab, d.r, d.anchor_rank, st);   // T = A_s (B_s U)   [V, r]
 }
 
 int mapl_decode(const mapl_boundary_desc* desc, const void* Z, const int32_t* codes, const float* U,

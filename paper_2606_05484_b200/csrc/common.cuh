@@ -61,10 +61,15 @@ struct GemmArgs {
 
 int simt_gemm(const GemmArgs& g, cudaStream_t stream);
 
+// C[M,N] = A[M,K] B[K,N], all dense row-major fp32 (the 64x64-tile FFMA kernel of stiefel.cu); N, K % 4 == 0
+int st_gemm_nn(const float* A, const float* B, float* C, int M, int N, int K, cudaStream_t stream);
+
 // ---------------------------------------------------------------- SIMT codec pieces (simt_codec.cu)
 int simt_half_sqnorm(const float* C, float* out, int rows, int r, cudaStream_t stream);
 int simt_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* U, const float* C,
-                    const float* half_norm, void* Zq_out, int32_t* codes, cudaStream_t stream);
+                    const float* half_norm, void* Zq_out, int32_t* codes, cudaStream_t stream,
+                    const int32_t* tok = nullptr, const float* Tc = nullptr);     // Tc: centring table (Eq. 1)
+int simt_center_rows(void* Z, int bf16, const int32_t* tok, const float* Tc, long long N, int r, cudaStream_t stream);
 int simt_dequant(const mapl_boundary_desc& d, const int32_t* codes, const float* C, float* Zhat,
                  cudaStream_t stream);
 int simt_scatter_add_rows(const float* gA, const int32_t* tok, float* dA, long long N, int ra,

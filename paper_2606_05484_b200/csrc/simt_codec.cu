@@ -30,7 +30,7 @@ template <bool kActBf16>
 __global__ void __launch_bounds__(NT) k_simt_encode_rvq(
     const void* __restrict__ Hv, const float* __restrict__ U, const float* __restrict__ C,
     const float* __restrict__ half_norm, void* __restrict__ Zq, int32_t* __restrict__ codes,
-    long long N, int d, int r, int L, int K) {
+    long long N, int d, int r, int L, int K, const int32_t* __restrict__ tok, const float* __restrict__ Tc) {
   extern __shared__ __align__(16) float smem[];
   const int rpad = (r + BK - 1) / BK * BK;
   float(*rhoT)[LD] = reinterpret_cast<float(*)[LD]>(smem);                 // [rpad][LD]
@@ -93,6 +93,14 @@ __global__ void __launch_bounds__(NT) k_simt_encode_rvq(
     }
   }
   __syncthreads();
+  if (Tc != nullptr) {   // sender-side centring (Eq. 1): z -= T[tok], T = A_s (B_s U) per vocabulary entry
+    for (int i = t; i < r * TOK; i += NT) {
+      const int k = i % r, tt = i / r;
+      const long long m = m0 + tt;
+      if (m < N) rhoT[k][tt] -= Tc[(long long)tok[m] * r + k];
+    }
+    __syncthreads();
+  }
 
   // ---- levels
   for (int l = 0; l < L; ++l) {
@@ -198,6 +206,32 @@ __global__ void k_scatter_add_rows(const float* __restrict__ gA, const int32_t* 
 
 }  // namespace
 
+// Z[n,:] -= T[tok_n,:]  (sender-side centring after a plain projection; Z in the activation dtype)
+template <bool kBf16>
+__global__ void k_center_rows(void* __restrict__ Zv, const int32_t* __restrict__ tok, const float* __restrict__ Tc, long long N, int r) {
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= N * r) return;
+  const long long n = idx / r;
+  const int j = (int)(idx % r);
+  const float t = Tc[(long long)tok[n] * r + j];
+  if (kBf16) {
+    __nv_bfloat16* Z = reinterpret_cast<__nv_bfloat16*>(Zv);
+    Z[idx] = __float2bfloat16_rn(__bfloat162float(Z[idx]) - t);
+  } else {
+    reinterpret_cast<float*>(Zv)[idx] -= t;
+  }
+}
+
+int simt_center_rows(void* Z, int bf16, const int32_t* tok, const float* Tc, long long N, int r, cudaStream_t stream) {
+  if (N <= 0) return MAPL_OK;
+  KernelScope ks(KID_SCATTER_ROWS, stream);
+  const unsigned blocks = (unsigned)((N * r + 255) / 256);
+  if (bf16) k_center_rows<true><<<blocks, 256, 0, stream>>>(Z, tok, Tc, N, r);
+  else k_center_rows<false><<<blocks, 256, 0, stream>>>(Z, tok, Tc, N, r);
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  return MAPL_OK;
+}
+
 int simt_half_sqnorm(const float* C, float* out, int rows, int r, cudaStream_t stream) {
   if (rows <= 0) return MAPL_OK;
   const int wpb = 8;
@@ -208,7 +242,8 @@ int simt_half_sqnorm(const float* C, float* out, int rows, int r, cudaStream_t s
 }
 
 int simt_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* U, const float* C,
-                    const float* half_norm, void* Zq_out, int32_t* codes, cudaStream_t stream) {
+                    const float* half_norm, void* Zq_out, int32_t* codes, cudaStream_t stream, const int32_t* tok,
+                    const float* Tc) {
   if (d.n_tokens <= 0) return MAPL_OK;
   const int rpad = (d.r + BK - 1) / BK * BK;
   const size_t smem = ((size_t)rpad * LD + 2 * BK * LD) * sizeof(float) + TOK * MAXL * sizeof(int);
@@ -222,9 +257,9 @@ int simt_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* U, 
     attr_done = true;
   }
   if (d.act_dtype == MAPL_BF16) {
-    k_simt_encode_rvq<true><<<(unsigned)blocks, NT, smem, stream>>>(H, U, C, half_norm, Zq_out, codes, d.n_tokens, d.d, d.r, d.rvq_levels, d.rvq_k);
+    k_simt_encode_rvq<true><<<(unsigned)blocks, NT, smem, stream>>>(H, U, C, half_norm, Zq_out, codes, d.n_tokens, d.d, d.r, d.rvq_levels, d.rvq_k, tok, Tc);
   } else {
-    k_simt_encode_rvq<false><<<(unsigned)blocks, NT, smem, stream>>>(H, U, C, half_norm, Zq_out, codes, d.n_tokens, d.d, d.r, d.rvq_levels, d.rvq_k);
+    k_simt_encode_rvq<false><<<(unsigned)blocks, NT, smem, stream>>>(H, U, C, half_norm, Zq_out, codes, d.n_tokens, d.d, d.r, d.rvq_levels, d.rvq_k, tok, Tc);
   }
   MAPL_CUDA_CHECK(cudaGetLastError());
   return MAPL_OK;

@@ -364,6 +364,17 @@ int tri_inverse_newton(const float* R, float* Xa, float* Xb, float* T, float** o
 }
 
 }  // namespace
+
+int st_gemm_nn(const float* A, const float* B, float* C, int M, int N, int K, cudaStream_t st) {
+  if (M <= 0 || N <= 0 || K <= 0) return MAPL_OK;
+  if (N % 4 || K % 4) return MAPL_ERR_UNSUPPORTED;
+  const int tiles = ((M + TM - 1) / TM) * ((N + TN - 1) / TN);
+  KernelScope ks(KID_ST_GEMM, st);
+  k_st_gemm<false><<<dim3(tiles, 1, 1), 256, 0, st>>>(A, B, C, nullptr, 1.f, 0.f, M, N, K, K, 0, 0, 0, 0, K, N, N);
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  return MAPL_OK;
+}
+
 }  // namespace mapl
 
 using namespace mapl;

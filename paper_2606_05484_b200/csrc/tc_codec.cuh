@@ -42,8 +42,9 @@ size_t tc_scratch_bytes(const mapl_boundary_desc& d);
 // tokens per CTA (<= 128, multiple of 8) such that the grid covers the 148 SMs in whole, even waves
 int tc_tile_m(long long N);
 
+// tok / Tc (both or neither): sender-side centring z -= Tc[tok], Tc [V,r] fp32 (mapl_center_table)
 int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
-              int32_t* codes_out, cudaStream_t st);
+              int32_t* codes_out, cudaStream_t st, const int32_t* tok = nullptr, const float* Tc = nullptr);
 
 int tc_decode(const mapl_boundary_desc& d, const void* Z, const int32_t* codes, const float* codebooks,
               const int32_t* tok, const float* A, const TcPack& pk, void* Hhat_out, cudaStream_t st);

@@ -27,7 +27,8 @@ constexpr int kATile = BM * BK * 2;   // 16 KB
 // issues MMAs; its commits arrive on the barriers of both CTAs.
 __global__ void __launch_bounds__(kThreads, 1)
 k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmW,
-            __nv_bfloat16* __restrict__ Z, long long N, int d, int r, int stages, int tile_m) {
+            __nv_bfloat16* __restrict__ Z, long long N, int d, int r, int stages, int tile_m,
+            const int32_t* __restrict__ tok, const float* __restrict__ Tc) {   // Tc != NULL: z -= Tc[tok] (Eq. 1 centring)
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int b_tile = (r / 2) * BK * 2;                 // this CTA's half of the U^T tile
@@ -97,6 +98,8 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
     const int q = warp & 3;                         // TMEM lane quarter this warp may read
     const int row = q * 32 + lane;
     const long long m = m0 + row;
+    const bool live = row < tile_m && m < N;
+    const float* trow = (Tc != nullptr && live) ? Tc + (long long)__ldg(tok + m) * r : nullptr;
     mbar_wait(accum_full, 0);
     if (warp == 2) { DBG(4) }
     tc_fence_after_sync();
@@ -104,7 +107,17 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
       uint32_t v[32];
       tmem_ld32(tmem_d + ((uint32_t)(q * 32) << 16) + c * 32, v);
       tmem_ld_wait();
-      if (row < tile_m && m < N) {
+      if (trow != nullptr) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          const float4 t4 = __ldg(reinterpret_cast<const float4*>(trow + c * 32) + i);
+          v[4 * i + 0] = __float_as_uint(__uint_as_float(v[4 * i + 0]) - t4.x);
+          v[4 * i + 1] = __float_as_uint(__uint_as_float(v[4 * i + 1]) - t4.y);
+          v[4 * i + 2] = __float_as_uint(__uint_as_float(v[4 * i + 2]) - t4.z);
+          v[4 * i + 3] = __float_as_uint(__uint_as_float(v[4 * i + 3]) - t4.w);
+        }
+      }
+      if (live) {
         uint4* dst = reinterpret_cast<uint4*>(Z + m * r + c * 32);
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -133,12 +146,12 @@ MAPL_DBG_READER(mapl_debug_read_encode)
 namespace mapl {
 
 int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
-                  int32_t* codes_out, cudaStream_t st);   // tc_encode_rvq.cu
+                  int32_t* codes_out, cudaStream_t st, const int32_t* tok, const float* Tc);   // tc_encode_rvq.cu
 
 int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
-              int32_t* codes_out, cudaStream_t st) {
+              int32_t* codes_out, cudaStream_t st, const int32_t* tok, const float* Tc) {
   if (!tc_shape_ok(d)) return MAPL_ERR_UNSUPPORTED;
-  if (d.rvq_levels != 0) return tc_encode_rvq(d, H, codebooks, pk, Zq_out, codes_out, st);
+  if (d.rvq_levels != 0) return tc_encode_rvq(d, H, codebooks, pk, Zq_out, codes_out, st, tok, Tc);
   const int tile_m = tc_tile_m(d.n_tokens);
   CUtensorMap tmH, tmW;
   if (!make_tmap_bf16_2d(&tmH, H, (uint64_t)d.n_tokens, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)tile_m)) return MAPL_ERR_CUDA;
@@ -156,7 +169,7 @@ int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks
   const unsigned tiles = ((unsigned)((d.n_tokens + tile_m - 1) / tile_m) + 1u) & ~1u;   // whole CTA pairs
   KernelScope ks(KID_TC_ENCODE, st);
   MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_encode, dim3(tiles), dim3(kThreads), smem, st, tmH, tmW,
-                             reinterpret_cast<__nv_bfloat16*>(Zq_out), d.n_tokens, d.d, d.r, stages, tile_m));
+                             reinterpret_cast<__nv_bfloat16*>(Zq_out), d.n_tokens, d.d, d.r, stages, tile_m, tok, Tc));
   return MAPL_OK;
 }
 

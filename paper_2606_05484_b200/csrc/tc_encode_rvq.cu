@@ -39,6 +39,7 @@ struct RvqParams {
   const float* hn;       // [L*K] 0.5 ||c||^2
   const float* cmax;     // [L] max_k ||c_k||
   const float* cscale;   // [8+l] = 2^e_l: the fp16 codebook copy is C * 2^-e_l
+  const int32_t* tok; const float* Tc;   // optional sender-side centring (Eq. 1): z -= Tc[tok], Tc [V,r] fp32
   __nv_bfloat16* Zq;     // optional [N,r]
   int32_t* codes;        // [N,L]
   long long N;
@@ -310,7 +311,9 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       }
       tmem_st_wait();
     }
-    rho_subtract(tmem_row, nullptr, p.r, h, &n2, &amax);
+    // centring: the first residual is z - Tc[tok] (dead rows subtract row 0: any valid row keeps the warp convergent)
+    const float* csub = p.Tc != nullptr ? p.Tc + (live ? (long long)__ldg(p.tok + m) * p.r : 0) : nullptr;
+    rho_subtract(tmem_row, csub, p.r, h, &n2, &amax);
     xN2[mine] = n2; xAmax[mine] = amax;
     asm volatile("bar.sync 1, 256;" ::: "memory");
     n2 += xN2[other]; amax = fmaxf(amax, xAmax[other]);
@@ -474,10 +477,10 @@ MAPL_DBG_READER(mapl_debug_read_rvq)
 namespace mapl {
 
 int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
-                  int32_t* codes_out, cudaStream_t st) {
+                  int32_t* codes_out, cudaStream_t st, const int32_t* tok, const float* Tc) {
   if (!tc_rvq_ok(d) || !pk.WBlo || !pk.Cb) return MAPL_ERR_UNSUPPORTED;
   RvqParams p;
-  p.C = codebooks; p.hn = pk.hn; p.cmax = pk.cmax; p.cscale = pk.cscale;
+  p.C = codebooks; p.hn = pk.hn; p.cmax = pk.cmax; p.cscale = pk.cscale; p.tok = tok; p.Tc = Tc;
   p.Zq = reinterpret_cast<__nv_bfloat16*>(Zq_out); p.codes = codes_out;
   p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.L = d.rvq_levels; p.K = d.rvq_k;
   p.tile_m = tc_tile_m(d.n_tokens);

@@ -92,3 +92,20 @@ def test_no_cpu_fallback():
     with pytest.raises(mb.MaplError):
         t = torch.zeros(64, 64)
         mb.mapl_encode(d, t, t, None, t, None, torch.zeros(n, dtype=torch.uint8))
+
+
+def test_centering_entry_points_check_arguments():
+    lib = mb.raw_lib()
+    d = mb.make_desc(64, 64, 16, torch.float32, 0, 0, 100, 8)
+    assert mb.mapl_center_workspace_bytes(d) >= 8 * 16 * 4
+    no_anchor = mb.make_desc(64, 64, 16, torch.float32, 0, 0, 0, 0)
+    assert mb.mapl_center_workspace_bytes(no_anchor) == 0
+    buf = (C.c_char * 8192)()
+    p = (C.addressof(buf) + 15) & ~15
+    # tok / table missing
+    assert lib.mapl_encode_centered(C.byref(d), p, None, p, p, None, p, None, p, 8192, None) == -1
+    assert lib.mapl_encode_centered(C.byref(d), p, p, None, p, None, p, None, p, 8192, None) == -1
+    # table_out NULL
+    assert lib.mapl_center_table(C.byref(d), p, p, p, None, p, 8192, None) == -1
+    # workspace too small
+    assert lib.mapl_center_table(C.byref(d), p, p, p, p, p, 16, None) == -4

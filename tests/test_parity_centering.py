@@ -1,0 +1,71 @@
+"""Sender-side anchor centring (Eq. 1 in full): mapl_center_table +
+mapl_encode_centered through the C ABI against the fp64 oracle (oracle.project with A_s, B_s, then the
+same RVQ / near-tie rule as the hot path)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import mapl_oracle as o
+from paper_2606_05484_b200 import binding as mb
+from paper_2606_05484_b200 import inputs as I
+
+from _util import TOL, desc_of, rel_fro, to_dev, to_np
+
+pytestmark = pytest.mark.gpu
+
+
+def _centered_encode(bi, a_std=1.0):
+    """GPU: T = A_s (B_s U), then encode_centered.  The sender's anchor factors are the boundary's A, B
+    rescaled so that the centring term is comparable to h (an error in it cannot hide)."""
+    c = bi.cfg
+    desc = desc_of(bi)
+    act = mb.act_torch_dtype(desc)
+    A_s = (bi.A.f64 * (a_std / max(bi.A.f64.std(), 1e-30))).astype(np.float32)
+    B_s = bi.B.f64.astype(np.float32)
+    dA, dB, dU, dH, dtok = to_dev(A_s), to_dev(B_s), to_dev(bi.U), to_dev(bi.H), to_dev(bi.tok)
+    dC = to_dev(bi.C) if bi.C is not None else None
+    T = torch.empty((c.vocab, c.r), dtype=torch.float32, device="cuda")
+    cws = mb.alloc_workspace(mb.mapl_center_workspace_bytes(desc))
+    mb.mapl_center_table(desc, dA, dB, dU, T, cws)
+    ws = mb.alloc_workspace(mb.mapl_workspace_bytes(desc))
+    N, r, L = c.n_tokens, c.r, c.rvq_levels
+    Zq = torch.empty((N, r), dtype=act, device="cuda")
+    codes = torch.empty((N, L), dtype=torch.int32, device="cuda") if L > 0 else None
+    mb.mapl_encode_centered(desc, dH, dtok, T, dU, dC, Zq, codes, ws)
+    torch.cuda.synchronize()
+    return A_s.astype(np.float64), B_s.astype(np.float64), to_np(T), to_np(Zq), (to_np(codes) if L > 0 else None)
+
+
+@pytest.mark.parametrize("name,n", [("c0", 999), ("c1", 1500), ("c2", 1037), ("c3", 517)])
+def test_centered_encode_matches_oracle(name, n):
+    bi = I.make_boundary(I.CONFIGS[name].with_tokens(n), 3)
+    A_s, B_s, T, Zq, codes = _centered_encode(bi)
+    U = bi.U.f64
+    # the table itself: T = A_s (B_s U) (fp32 GEMMs)
+    assert rel_fro(T, A_s @ (B_s @ U)) <= 1e-5
+    Z = o.project(bi.H.f64, U, bi.tok, A_s, B_s)
+    # centring really changes z
+    assert rel_fro(o.project(bi.H.f64, U), Z) > 1e-2
+    tol = TOL[bi.cfg.act_dtype]
+    if bi.cfg.rvq_levels == 0:
+        assert rel_fro(Zq, Z) <= tol
+        return
+    res, n_exc, n_forced, bad = o.follow_codes(Z, bi.C.f64, codes)
+    assert int(bad.sum()) == 0, f"non-admissible codes: {int(bad.sum())} (excepted {n_exc}, forced {n_forced})"
+    assert np.array_equal(codes, res["codes"])
+    assert rel_fro(Zq, res["Zhat"]) <= tol
+
+
+def test_zero_anchor_reduces_to_plain_encode():
+    bi = I.make_boundary(I.CONFIGS["c2"].with_tokens(700), 4)
+    desc = desc_of(bi)
+    c = bi.cfg
+    dU, dH, dtok, dC = to_dev(bi.U), to_dev(bi.H), to_dev(bi.tok), to_dev(bi.C)
+    T = torch.zeros((c.vocab, c.r), dtype=torch.float32, device="cuda")
+    ws = mb.alloc_workspace(mb.mapl_workspace_bytes(desc))
+    a = torch.empty((c.n_tokens, c.rvq_levels), dtype=torch.int32, device="cuda")
+    b = torch.empty_like(a)
+    mb.mapl_encode_centered(desc, dH, dtok, T, dU, dC, None, a, ws)
+    mb.mapl_encode(desc, dH, dU, dC, None, b, ws)
+    torch.cuda.synchronize()
+    assert torch.equal(a, b)
