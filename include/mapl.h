@@ -152,14 +152,24 @@ int mapl_codec_backward(const mapl_boundary_desc* desc, const void* g_Hhat, cons
  * T[tok_n] subtracted from the fp32 accumulator of token n before anything is rounded or quantised, so
  * the RVQ codes are those of the centred z.  Arguments as mapl_encode, plus tok [N] int32 (0 <= tok < V)
  * and center_table [V,r] fp32.  A_s [V,ra], B_s [ra,d] (the sender's anchor factors; desc.vocab and
- * desc.anchor_rank describe them).  The backward of the centring term (dA_s, and -B_s^T A_s[tok]^T gz in dU)
- * is not built yet.                                                                                  */
+ * desc.anchor_rank describe them).
+ * mapl_center_backward is the backward of the centring term for gz = dL/dz ([N,r], activation dtype: the gz_out
+ * of mapl_codec_backward):  with D[v,:] = sum_{n: tok_n = v} gz_n and Q = A_s^T D,
+ *     dA_s = - D (B_s U)^T   [V,ra];    dB_s = - Q U^T   [ra,d] (optional, NULL = skipped);
+ *     dU  += - B_s^T Q       [d,r]      (always ADDED: it completes the H^T gz that mapl_codec_backward formed
+ *                                        with the uncentred H to (H - A_s[tok] B_s)^T gz).
+ * accumulate 0 / 1 applies to dA_s and dB_s as in mapl_codec_backward.  fp32 arithmetic; work is O(V r ra),
+ * independent of N apart from the scatter.  workspace: mapl_center_backward_workspace_bytes(desc).   */
 size_t mapl_center_workspace_bytes(const mapl_boundary_desc* desc);
+size_t mapl_center_backward_workspace_bytes(const mapl_boundary_desc* desc);
 int mapl_center_table(const mapl_boundary_desc* desc, const float* A_s, const float* B_s, const float* U,
                       float* table_out, void* workspace, size_t workspace_bytes, void* cuda_stream);
 int mapl_encode_centered(const mapl_boundary_desc* desc, const void* H, const int32_t* tok, const float* center_table,
                          const float* U, const float* codebooks, void* Zq_out, int32_t* codes_out, void* workspace,
                          size_t workspace_bytes, void* cuda_stream);
+int mapl_center_backward(const mapl_boundary_desc* desc, const void* gz, const int32_t* tok, const float* A_s,
+                         const float* B_s, const float* U, float* dA_s_out, float* dB_s_out, float* dU_inout,
+                         int accumulate, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* STIEFEL STEP on `batch` independent projectors, U_inout and G strided [batch,d,r] fp32.
  *   S = U^T G;  xi = G - U (S + S^T)/2 (Eq. 4);  Y = U - lr xi;

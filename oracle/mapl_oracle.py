@@ -147,6 +147,28 @@ def backward(g, H, Zhat, U, tok=None, A=None, B=None, want_dB=True, want_dH=True
     return dict(gz=gz, dU=dU, dA=dA, dB=dB, dH=dH)
 
 
+def center_backward(gz, tok, A_s, B_s, U, want_dB=True):
+    """Backward of the sender-side centring term of PAPER.md:73 Eq. 1, Z = (H - A_s[tok] B_s) U, for an
+    upstream gradient gz = dL/dZ (plain loops over the definition; library matmuls as steps):
+        dL/dA_s[v,:] = - sum_{n: tok_n = v} (B_s U) gz_n           [V,ra]
+        dL/dB_s      = - (sum_n A_s[tok_n]^T gz_n^T) U^T           [ra,d]
+        dU_corr      = - B_s^T (sum_n A_s[tok_n] gz_n^T)           [d,r]   (added to H^T gz: the U-gradient of Eq. 1
+                                                                           is (H - A_s[tok] B_s)^T gz)"""
+    gz, A_s, B_s, U = _f64(gz), _f64(A_s), _f64(B_s), _f64(U)
+    tok = _i32(tok)
+    V, ra = A_s.shape
+    N, r = gz.shape
+    Wc = B_s @ U                                   # [ra,r]
+    dA = np.zeros((V, ra), np.float64)
+    Q = np.zeros((ra, r), np.float64)              # sum_n A_s[tok_n] (outer) gz_n
+    for n in range(N):
+        dA[tok[n], :] -= Wc @ gz[n]
+        Q += np.outer(A_s[tok[n]], gz[n])
+    dU = -(B_s.T @ Q)
+    dB = -(Q @ U.T) if want_dB else None
+    return dict(dA_s=dA, dB_s=dB, dU_corr=dU)
+
+
 def tangent(U, G) -> np.ndarray:
     """xi = G - U sym(U^T G)  (Eq. 4)."""
     U, G = _f64(U), _f64(G)

@@ -55,6 +55,10 @@ def _load():
     lib.mapl_center_workspace_bytes.argtypes = [dp]
     lib.mapl_center_table.restype = C.c_int
     lib.mapl_center_table.argtypes = [dp, vp, vp, vp, vp, vp, sz, vp]
+    lib.mapl_center_backward_workspace_bytes.restype = sz
+    lib.mapl_center_backward_workspace_bytes.argtypes = [dp]
+    lib.mapl_center_backward.restype = C.c_int
+    lib.mapl_center_backward.argtypes = [dp, vp, vp, vp, vp, vp, vp, vp, vp, C.c_int, vp, sz, vp]
     lib.mapl_encode_centered.restype = C.c_int
     lib.mapl_encode_centered.argtypes = [dp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.mapl_decode.argtypes = [dp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -172,6 +176,22 @@ def mapl_encode_centered(desc: BoundaryDesc, H, tok, center_table, U, codebooks,
         _ptr(U, torch.float32, "U"), _ptr(codebooks, torch.float32, "codebooks"), _ptr(Zq_out, act, "Zq_out"),
         _ptr(codes_out, torch.int32, "codes_out"), _ptr(workspace, None, "workspace"),
         workspace.numel() * workspace.element_size(), _stream()), "mapl_encode_centered")
+
+
+def mapl_center_backward_workspace_bytes(desc: BoundaryDesc) -> int:
+    return int(_lib.mapl_center_backward_workspace_bytes(C.byref(desc)))
+
+
+def mapl_center_backward(desc: BoundaryDesc, gz, tok, A_s, B_s, U, dA_s_out, dB_s_out, dU_inout, accumulate: bool,
+                         workspace) -> None:
+    """Backward of the centring term (include/mapl.h): dA_s, optional dB_s, and dU += -B_s^T A_s[tok]^T gz."""
+    act = act_torch_dtype(desc)
+    f = torch.float32
+    _check(_lib.mapl_center_backward(
+        C.byref(desc), _ptr(gz, act, "gz"), _ptr(tok, torch.int32, "tok"), _ptr(A_s, f, "A_s"), _ptr(B_s, f, "B_s"),
+        _ptr(U, f, "U"), _ptr(dA_s_out, f, "dA_s_out"), _ptr(dB_s_out, f, "dB_s_out"), _ptr(dU_inout, f, "dU_inout"),
+        int(bool(accumulate)), _ptr(workspace, None, "workspace"), workspace.numel() * workspace.element_size(),
+        _stream()), "mapl_center_backward")
 
 
 def mapl_decode(desc: BoundaryDesc, Z, codes, U, codebooks, tok, A, B, Hhat_out, workspace) -> None:

@@ -185,6 +185,61 @@ int mapl_center_table(const mapl_boundary_desc* desc, const float* A_s, const fl
   return st_gemm_nn(A_s, Wc, table_out, d.vocab, d.r, d.anchor_rank, st);   // T = A_s (B_s U)   [V, r]
 }
 
+namespace {
+struct CenterWs { size_t D, Q, Wc, Wct, Ut, total; };
+CenterWs center_carve(const mapl_boundary_desc& d) {
+  CenterWs w;
+  size_t off = 0;
+  auto seg = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+  w.D = seg((size_t)d.vocab * d.r * 4);
+  w.Q = seg((size_t)d.anchor_rank * d.r * 4);
+  w.Wc = seg((size_t)d.anchor_rank * d.r * 4);
+  w.Wct = seg((size_t)d.anchor_rank * d.r * 4);
+  w.Ut = seg((size_t)d.d * d.r * 4);
+  w.total = off + 256;
+  return w;
+}
+}  // namespace
+
+size_t mapl_center_backward_workspace_bytes(const mapl_boundary_desc* desc) {
+  if (validate_desc(desc) != MAPL_OK || desc->anchor_rank <= 0 || desc->vocab < 1) return 0;
+  return center_carve(*desc).total;
+}
+
+int mapl_center_backward(const mapl_boundary_desc* desc, const void* gz, const int32_t* tok, const float* A_s,
+                         const float* B_s, const float* U, float* dA_s_out, float* dB_s_out, float* dU_inout,
+                         int accumulate, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  MAPL_RETURN_IF(validate_desc(desc));
+  const mapl_boundary_desc& d = *desc;
+  if (d.anchor_rank <= 0 || d.vocab < 1) return MAPL_ERR_INVALID_ARG;
+  if (!A_s || !B_s || !U || !dA_s_out || !dU_inout) return MAPL_ERR_INVALID_ARG;
+  if (d.n_tokens > 0 && (!gz || !tok)) return MAPL_ERR_INVALID_ARG;
+  if (!all16({gz, tok, A_s, B_s, U, dA_s_out, dB_s_out, dU_inout, workspace})) return MAPL_ERR_ALIGNMENT;
+  const CenterWs w = center_carve(d);
+  if (!workspace || workspace_bytes < w.total) return MAPL_ERR_WORKSPACE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  char* ws = reinterpret_cast<char*>(workspace);
+  float* D = reinterpret_cast<float*>(ws + w.D);       // [V,r]  D[v] = sum_{n: tok_n = v} gz_n
+  float* Q = reinterpret_cast<float*>(ws + w.Q);       // [ra,r] A_s^T D = sum_n A_s[tok_n] (outer) gz_n
+  float* Wc = reinterpret_cast<float*>(ws + w.Wc);     // [ra,r] B_s U
+  float* Wct = reinterpret_cast<float*>(ws + w.Wct);   // [r,ra]
+  float* Ut = reinterpret_cast<float*>(ws + w.Ut);     // [r,d]
+  const int V = d.vocab, ra = d.anchor_rank, r = d.r, dd = d.d;
+  { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(D, 0, (size_t)V * r * 4, st)); }
+  { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(Q, 0, (size_t)ra * r * 4, st)); }
+  MAPL_RETURN_IF(simt_scatter_add_act_rows(gz, d.act_dtype == MAPL_BF16, tok, D, d.n_tokens, r, st));
+  MAPL_RETURN_IF(st_gemm_nn(B_s, U, Wc, ra, r, dd, st));
+  MAPL_RETURN_IF(simt_transpose(Wc, Wct, ra, r, st));
+  MAPL_RETURN_IF(st_gemm_tn(A_s, D, Q, ra, r, V, st));                                        // Q = A_s^T D
+  MAPL_RETURN_IF(st_gemm_nn(D, Wct, dA_s_out, V, ra, r, st, -1.f, accumulate ? dA_s_out : nullptr, 1.f));   // dA_s = -D Wc^T
+  MAPL_RETURN_IF(st_gemm_tn(B_s, Q, dU_inout, dd, r, ra, st, -1.f));                         // dU += -B_s^T Q
+  if (dB_s_out) {
+    MAPL_RETURN_IF(simt_transpose(U, Ut, dd, r, st));
+    MAPL_RETURN_IF(st_gemm_nn(Q, Ut, dB_s_out, ra, dd, r, st, -1.f, accumulate ? dB_s_out : nullptr, 1.f));   // dB_s = -Q U^T
+  }
+  return MAPL_OK;
+}
+
 int mapl_decode(const mapl_boundary_desc* desc, const void* Z, const int32_t* codes, const float* U,
                 const float* codebooks, const int32_t* tok, const float* A, const float* B,
                 void* Hhat_out, void* workspace, size_t workspace_bytes, void* cuda_stream) {

@@ -62,7 +62,13 @@ struct GemmArgs {
 int simt_gemm(const GemmArgs& g, cudaStream_t stream);
 
 // C[M,N] = A[M,K] B[K,N], all dense row-major fp32 (the 64x64-tile FFMA kernel of stiefel.cu); N, K % 4 == 0
-int st_gemm_nn(const float* A, const float* B, float* C, int M, int N, int K, cudaStream_t stream);
+int st_gemm_nn(const float* A, const float* B, float* C, int M, int N, int K, cudaStream_t stream, float alpha = 1.f,
+               const float* E = nullptr, float beta = 0.f);       // C = alpha A B + beta E (E may be C)
+// C[M,N] += alpha X[K,M]^T Y[K,N] (split over K, red.global.add: C must hold the value to add to); M, N % 4 == 0
+int st_gemm_tn(const float* X, const float* Y, float* C, int M, int N, int K, cudaStream_t stream, float alpha = 1.f);
+// D[tok_n, :] += X[n, :] (X in the activation dtype, D fp32 [V,w]);  dst[c, r] = src[r, c] (fp32)
+int simt_scatter_add_act_rows(const void* X, int bf16, const int32_t* tok, float* D, long long N, int w, cudaStream_t stream);
+int simt_transpose(const float* src, float* dst, int rows, int cols, cudaStream_t stream);
 
 // ---------------------------------------------------------------- SIMT codec pieces (simt_codec.cu)
 int simt_half_sqnorm(const float* C, float* out, int rows, int r, cudaStream_t stream);

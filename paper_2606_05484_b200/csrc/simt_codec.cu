@@ -232,6 +232,48 @@ int simt_center_rows(void* Z, int bf16, const int32_t* tok, const float* Tc, lon
   return MAPL_OK;
 }
 
+// D[tok_n, :] += X[n, :]: one warp per token row, fp32 atomics (reds)
+template <bool kBf16>
+__global__ void k_scatter_act_rows(const void* __restrict__ Xv, const int32_t* __restrict__ tok, float* __restrict__ D,
+                                   long long N, int w) {
+  const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) / 32;
+  const int lane = threadIdx.x % 32;
+  if (n >= N) return;
+  float* dst = D + (long long)tok[n] * w;
+  for (int j = lane; j < w; j += 32) {
+    const float x = kBf16 ? __bfloat162float(reinterpret_cast<const __nv_bfloat16*>(Xv)[n * w + j])
+                          : reinterpret_cast<const float*>(Xv)[n * w + j];
+    atomicAdd(dst + j, x);
+  }
+}
+
+int simt_scatter_add_act_rows(const void* X, int bf16, const int32_t* tok, float* D, long long N, int w, cudaStream_t stream) {
+  if (N <= 0) return MAPL_OK;
+  KernelScope ks(KID_SCATTER_ROWS, stream);
+  const unsigned blocks = (unsigned)((N * 32 + 255) / 256);
+  if (bf16) k_scatter_act_rows<true><<<blocks, 256, 0, stream>>>(X, tok, D, N, w);
+  else k_scatter_act_rows<false><<<blocks, 256, 0, stream>>>(X, tok, D, N, w);
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  return MAPL_OK;
+}
+
+__global__ void k_transpose(const float* __restrict__ src, float* __restrict__ dst, int rows, int cols) {
+  __shared__ float tile[32][33];
+  const int r0 = blockIdx.y * 32, c0 = blockIdx.x * 32, tx = threadIdx.x % 32, ty = threadIdx.x / 32;
+  for (int i = ty; i < 32; i += 8)
+    tile[i][tx] = (r0 + i < rows && c0 + tx < cols) ? src[(long long)(r0 + i) * cols + c0 + tx] : 0.f;
+  __syncthreads();
+  for (int i = ty; i < 32; i += 8)
+    if (c0 + i < cols && r0 + tx < rows) dst[(long long)(c0 + i) * rows + r0 + tx] = tile[tx][i];
+}
+
+int simt_transpose(const float* src, float* dst, int rows, int cols, cudaStream_t stream) {
+  KernelScope ks(KID_SCATTER_ROWS, stream);
+  k_transpose<<<dim3((cols + 31) / 32, (rows + 31) / 32), 256, 0, stream>>>(src, dst, rows, cols);
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  return MAPL_OK;
+}
+
 int simt_half_sqnorm(const float* C, float* out, int rows, int r, cudaStream_t stream) {
   if (rows <= 0) return MAPL_OK;
   const int wpb = 8;

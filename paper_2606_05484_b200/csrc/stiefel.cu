@@ -365,12 +365,27 @@ int tri_inverse_newton(const float* R, float* Xa, float* Xb, float* T, float** o
 
 }  // namespace
 
-int st_gemm_nn(const float* A, const float* B, float* C, int M, int N, int K, cudaStream_t st) {
+int st_gemm_nn(const float* A, const float* B, float* C, int M, int N, int K, cudaStream_t st, float alpha, const float* E,
+               float beta) {
   if (M <= 0 || N <= 0 || K <= 0) return MAPL_OK;
   if (N % 4 || K % 4) return MAPL_ERR_UNSUPPORTED;
   const int tiles = ((M + TM - 1) / TM) * ((N + TN - 1) / TN);
   KernelScope ks(KID_ST_GEMM, st);
-  k_st_gemm<false><<<dim3(tiles, 1, 1), 256, 0, st>>>(A, B, C, nullptr, 1.f, 0.f, M, N, K, K, 0, 0, 0, 0, K, N, N);
+  k_st_gemm<false><<<dim3(tiles, 1, 1), 256, 0, st>>>(A, B, C, E, alpha, beta, M, N, K, K, 0, 0, 0, 0, K, N, N);
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  return MAPL_OK;
+}
+
+int st_gemm_tn(const float* X, const float* Y, float* C, int M, int N, int K, cudaStream_t st, float alpha) {
+  if (M <= 0 || N <= 0 || K <= 0) return MAPL_OK;
+  if (M % 4 || N % 4) return MAPL_ERR_UNSUPPORTED;
+  const int tiles = ((M + TM - 1) / TM) * ((N + TN - 1) / TN);
+  int splits = (2 * 148 + tiles - 1) / tiles;
+  int kper = ((K + splits - 1) / splits + TK - 1) / TK * TK;
+  if (kper < 4 * TK) kper = 4 * TK;
+  splits = (K + kper - 1) / kper;
+  KernelScope ks(KID_ST_GEMM, st);
+  k_st_gemm<true><<<dim3(tiles, splits, 1), 256, 0, st>>>(X, Y, C, nullptr, alpha, 0.f, M, N, K, kper, 0, 0, 0, 0, M, N, N);
   MAPL_CUDA_CHECK(cudaGetLastError());
   return MAPL_OK;
 }

@@ -295,3 +295,33 @@ def test_backward_adjoint_identities_and_split():
     # no anchor
     na = o.backward(g, H, Zhat, U)
     assert na["dA"] is None and np.abs(na["dU"] - out["dU"]).max() == 0.0
+
+
+def test_centring_backward_matches_finite_differences():
+    """center_backward is the gradient of L = <gz, (H - A_s[tok] B_s) U> w.r.t. A_s, B_s, and its dU_corr completes
+    H^T gz to the U-gradient of Eq. 1 (central differences in fp64 on every entry class)."""
+    rng = np.random.default_rng(16)
+    N, d, r, V, ra = 23, 10, 4, 6, 3
+    H = rng.standard_normal((N, d)); U = _orth(rng, d, r)
+    A = rng.standard_normal((V, ra)); B = rng.standard_normal((ra, d))
+    tok = rng.integers(0, V - 1, N).astype(np.int32)          # id V-1 never occurs
+    gz = rng.standard_normal((N, r))
+    L = lambda A_, B_, U_: float((gz * o.project(H, U_, tok, A_, B_)).sum())
+    bw = o.center_backward(gz, tok, A, B, U)
+    eps = 1e-6
+
+    def fd(X, which):
+        G = np.zeros_like(X)
+        for idx in np.ndindex(*X.shape):
+            Xp, Xm = X.copy(), X.copy()
+            Xp[idx] += eps; Xm[idx] -= eps
+            args = {"A": (Xp, B, U), "B": (A, Xp, U), "U": (A, B, Xp)}[which], {"A": (Xm, B, U), "B": (A, Xm, U), "U": (A, B, Xm)}[which]
+            G[idx] = (L(*args[0]) - L(*args[1])) / (2 * eps)
+        return G
+
+    assert np.abs(bw["dA_s"] - fd(A, "A")).max() < 1e-7
+    assert np.abs(bw["dB_s"] - fd(B, "B")).max() < 1e-7
+    assert np.abs((H.T @ gz + bw["dU_corr"]) - fd(U, "U")).max() < 1e-7
+    assert not bw["dA_s"][V - 1].any()                          # absent id: zero row
+    # closed form of the U term: (H - A_s[tok] B_s)^T gz
+    assert np.abs((H - A[tok] @ B).T @ gz - (H.T @ gz + bw["dU_corr"])).max() < 1e-12

@@ -69,3 +69,40 @@ def test_zero_anchor_reduces_to_plain_encode():
     mb.mapl_encode(desc, dH, dU, dC, None, b, ws)
     torch.cuda.synchronize()
     assert torch.equal(a, b)
+
+
+@pytest.mark.parametrize("name,n", [("c0", 999), ("c1", 1500), ("c3", 517)])
+def test_center_backward_matches_oracle(name, n):
+    """dA_s, dB_s and the dU correction of the centring term against oracle.center_backward, for a Gaussian
+    gz in the activation dtype; then the accumulate variant."""
+    bi = I.make_boundary(I.CONFIGS[name].with_tokens(n), 5)
+    c = bi.cfg
+    desc = desc_of(bi)
+    act = mb.act_torch_dtype(desc)
+    rng = np.random.default_rng(99)
+    gz64 = rng.standard_normal((n, c.r))
+    gz = torch.from_numpy(gz64).to(act).cuda()
+    gz64 = gz.double().cpu().numpy()                       # the stored (rounded) values
+    A_s = (bi.A.f64 / max(bi.A.f64.std(), 1e-30)).astype(np.float32)
+    B_s = bi.B.f64.astype(np.float32)
+    dA_s, dB_s = to_dev(A_s), to_dev(B_s)
+    dU_t, dtok = to_dev(bi.U), to_dev(bi.tok)
+    ws = mb.alloc_workspace(mb.mapl_center_backward_workspace_bytes(desc))
+    dA = torch.full((c.vocab, c.anchor_rank), float("nan"), dtype=torch.float32, device="cuda")
+    dB = torch.full((c.anchor_rank, c.d), float("nan"), dtype=torch.float32, device="cuda")
+    dU0 = torch.from_numpy(rng.standard_normal((c.d, c.r)).astype(np.float32)).cuda()
+    dU = dU0.clone()
+    mb.mapl_center_backward(desc, gz, dtok, dA_s, dB_s, dU_t, dA, dB, dU, False, ws)
+    torch.cuda.synchronize()
+    ref = o.center_backward(gz64, bi.tok, A_s.astype(np.float64), B_s.astype(np.float64), bi.U.f64)
+    tol = 1e-5                                             # fp32 arithmetic whatever the activation dtype
+    assert rel_fro(to_np(dA), ref["dA_s"]) <= tol
+    assert rel_fro(to_np(dB), ref["dB_s"]) <= tol
+    assert rel_fro(to_np(dU) - to_np(dU0), ref["dU_corr"]) <= 1e-4   # difference of fp32 numbers of size ~1
+    absent = np.setdiff1d(np.arange(c.vocab), bi.tok)
+    assert not to_np(dA)[absent].any()
+    # accumulate: a second call adds the same amounts
+    mb.mapl_center_backward(desc, gz, dtok, dA_s, dB_s, dU_t, dA, dB, dU, True, ws)
+    torch.cuda.synchronize()
+    assert rel_fro(to_np(dA), 2 * ref["dA_s"]) <= tol
+    assert rel_fro(to_np(dB), 2 * ref["dB_s"]) <= tol
