@@ -421,6 +421,8 @@ def run_mapl(args):
     }
     if rank == 0 and world == 1 and not args.no_stiefel:
         out["stiefel"] = stiefel_sweep(torch, mb, I, stream)
+    if rank == 0 and world == 1 and not args.no_stiefel:
+        out["centering"] = centering_times(torch, mb, bs[0], cfg, stream)
     if rank == 0:
         if not args.no_cpu_baseline and world >= 1:
             out["cpu_baseline"] = cpu_baseline(cfg, budget_s=args.cpu_budget)
@@ -461,6 +463,40 @@ def stiefel_sweep(torch, mb, I, stream, reps=10):
                 out[f"r{r}_{tag}"] = {"us_per_step": round(us, 1), "projector_steps_per_s": round(s.batch * 1e6 / us),
                                       "orth_residual_after": float(f"{res:.2e}")}
     out["config"] = "d=2048, 3 projectors per call, fixed G, lr=1e-2, fp32"
+    return out
+
+
+def centering_times(torch, mb, b, cfg, stream, reps=10):
+    """SURVEY 8f next row 1 (Eq. 1 in full), measured beside the hot path on boundary 0 of the workload:
+    mapl_center_table (once per parameter update), mapl_encode_centered (per micro-batch; compare calls_us.mapl_encode)
+    and mapl_center_backward.  The sender's anchor factors are the boundary's A, B.  Graph-timed, us per call."""
+    T = torch.empty((cfg.vocab, cfg.r), dtype=torch.float32, device="cuda")
+    cws = mb.alloc_workspace(mb.mapl_center_workspace_bytes(b.desc))
+    bws = mb.alloc_workspace(mb.mapl_center_backward_workspace_bytes(b.desc))
+    dA = torch.empty_like(b.A)
+    dU = torch.zeros_like(b.dU)
+    fns = {
+        "mapl_center_table": lambda: mb.mapl_center_table(b.desc, b.A, b.B, b.U, T, cws),
+        "mapl_encode_centered": lambda: mb.mapl_encode_centered(b.desc, b.H, b.tok, T, b.U, b.C, b.Zq, b.codes, b.ws),
+        "mapl_center_backward": lambda: mb.mapl_center_backward(b.desc, b.gz, b.tok, b.A, b.B, b.U, dA, None, dU, False, bws),
+    }
+    out = {}
+    with torch.cuda.stream(stream):
+        for name, f in fns.items():
+            f()
+            stream.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                f()
+            g.replay()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                g.replay()
+            e1.record(stream)
+            stream.synchronize()
+            out[name] = round(1e3 * e0.elapsed_time(e1) / reps, 2)
+    out["note"] = "us per call, boundary 0; not part of the codec metric"
     return out
 
 
