@@ -203,6 +203,21 @@ void mapl_profile_enable(int timing_on);
 void mapl_profile_reset(void);
 int mapl_profile_read(int kid, long long* launches, long long* timed_launches, double* total_ms);
 
+/* FULL SPEL STEP (Eq. 4-7; SURVEY 8f "next" row 2) on `batch` projectors, U, G, M strided [batch,d,r] fp32:
+ *     xi = G - U sym(U^T G)                      (Eq. 4, tangent projection)
+ *     m  <- beta m + (1 - beta) xi               (Eq. 5, heavy-ball momentum; M_inout updated in place)
+ *     d  = NS_{lmo_iters}( m / ||m||_F )         (Eq. 6, spectral LMO direction)
+ *     U  <- NS_{retr_iters}( U - lr d )          (Eq. 7, retraction)
+ * The paper's PolarExpress [2] is not printed in it; here both polar steps are the cubic Newton-Schulz iteration
+ * X <- X (3I - X^T X)/2 (reading S11), for Eq. 6 from the Frobenius-normalised momentum (all singular values <= 1; with
+ * the paper's 5 iterations the small ones are only partly lifted towards 1, as in Muon), for Eq. 7 with the paper's 7.
+ * ||m||_F == 0 gives d = 0.  1 <= lmo_iters, retr_iters <= 16; 0 <= beta <= 1.  Same shapes, arithmetic paths and
+ * workspace as mapl_stiefel_step (mapl_spel_workspace_bytes).                                                        */
+size_t mapl_spel_workspace_bytes(int32_t d, int32_t r, int32_t batch);
+int mapl_spel_step(int32_t d, int32_t r, int32_t batch, float* U_inout, const float* G, float* M_inout, float lr,
+                   float beta, int32_t lmo_iters, int32_t retr_iters, void* workspace, size_t workspace_bytes,
+                   void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -211,6 +211,19 @@ def stiefel_step(U, G, lr: float, retraction: int, ns_iters: int = 5):
 REL_GAP = 1e-4
 
 
+def spel_step(U, G, m, lr: float, beta: float, lmo_iters: int = 5, retr_iters: int = 7):
+    """Full SPEL update, Eq. 4-7, step by step in the paper's order; PolarExpress is read as the
+    cubic Newton-Schulz iteration (reading S11), for Eq. 6 from m / ||m||_F.  Returns (U_new, m_new, d)."""
+    U, G, m = _f64(U), _f64(G), _f64(m)
+    xi = tangent(U, G)                                    # Eq. 4
+    m_new = beta * m + (1.0 - beta) * xi                  # Eq. 5
+    nrm = float(np.sqrt((m_new * m_new).sum()))
+    X0 = m_new / nrm if nrm > 0 else np.zeros_like(m_new)
+    d = newton_schulz(X0, lmo_iters)                      # Eq. 6
+    U_new = newton_schulz(U - lr * d, retr_iters)         # Eq. 7
+    return U_new, m_new, d
+
+
 def near_tie_mask(d1: np.ndarray, d2: np.ndarray, rel: float = REL_GAP) -> np.ndarray:
     """(token, level) pairs whose top-2 squared-distance gap is below `rel` relative:
     (D2 - D1)/D1 < rel  (north_star: codes bit-exact "except where the oracle's top-2 distance gap is

@@ -64,6 +64,10 @@ def _load():
     lib.mapl_decode.argtypes = [dp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.mapl_codec_backward.argtypes = [dp] + [vp] * 14 + [C.c_int, vp, sz, vp]
     lib.mapl_stiefel_step.argtypes = [i32, i32, i32, vp, vp, f32, i32, i32, vp, vp, sz, vp]
+    lib.mapl_spel_workspace_bytes.restype = sz
+    lib.mapl_spel_workspace_bytes.argtypes = [i32, i32, i32]
+    lib.mapl_spel_step.restype = C.c_int
+    lib.mapl_spel_step.argtypes = [i32, i32, i32, vp, vp, vp, f32, f32, i32, i32, vp, sz, vp]
     lib.mapl_profile_kernel_count.restype = C.c_int
     lib.mapl_profile_kernel_name.restype = C.c_char_p
     lib.mapl_profile_kernel_name.argtypes = [C.c_int]
@@ -228,6 +232,24 @@ def mapl_stiefel_step(U_inout, G, lr: float, retraction: int, ns_iters: int, inf
                                   int(retraction), int(ns_iters), _ptr(info_out, f, "info_out"),
                                   _ptr(workspace, None, "workspace"),
                                   workspace.numel() * workspace.element_size(), _stream()), "mapl_stiefel_step")
+
+
+def mapl_spel_workspace_bytes(d: int, r: int, batch: int) -> int:
+    return int(_lib.mapl_spel_workspace_bytes(d, r, batch))
+
+
+def mapl_spel_step(U_inout, G, M_inout, lr: float, beta: float, lmo_iters: int, retr_iters: int, workspace) -> None:
+    """Full SPEL update (include/mapl.h): tangent projection, momentum, LMO direction, retraction."""
+    f = torch.float32
+    if U_inout.dim() == 2:
+        batch, (d, r) = 1, U_inout.shape
+    else:
+        batch, d, r = U_inout.shape
+    if tuple(G.shape) != tuple(U_inout.shape) or tuple(M_inout.shape) != tuple(U_inout.shape):
+        raise MaplError("mapl_spel_step: G and M must have the shape of U")
+    _check(_lib.mapl_spel_step(d, r, batch, _ptr(U_inout, f, "U_inout"), _ptr(G, f, "G"), _ptr(M_inout, f, "M_inout"),
+                               float(lr), float(beta), int(lmo_iters), int(retr_iters), _ptr(workspace, None, "workspace"),
+                               workspace.numel() * workspace.element_size(), _stream()), "mapl_spel_step")
 
 
 def raw_lib():

@@ -130,7 +130,7 @@ __global__ void __launch_bounds__(256) k_chol_panel(float* __restrict__ Gb, int 
 }
 
 struct StWs {
-  size_t S, M, Rinv, Rinv2, X0, X1, Prow, Ptr, Ptr2, Pm, total;   // P*: bf16 planes of the tensor-core path
+  size_t S, M, Rinv, Rinv2, X0, X1, X2, norm2, Prow, Ptr, Ptr2, Pm, total;   // P*: bf16 planes of the tensor-core path
 };
 StWs st_carve(int d, int r, int batch) {
   StWs w;
@@ -142,6 +142,8 @@ StWs st_carve(int d, int r, int batch) {
   w.Rinv2 = seg((size_t)batch * r * r * 4);
   w.X0 = seg((size_t)batch * d * r * 4);
   w.X1 = seg((size_t)batch * d * r * 4);
+  w.X2 = seg((size_t)batch * d * r * 4);          // mapl_spel_step: the LMO direction
+  w.norm2 = seg((size_t)batch * 4);
   const bool tcp = tc_st_ok(d, r);
   w.Prow = seg(tcp ? tc_st_plane_bytes(d, r, batch) : 0);
   w.Ptr = seg(tcp ? tc_st_plane_bytes(d, r, batch) : 0);
@@ -363,6 +365,92 @@ int tri_inverse_newton(const float* R, float* Xa, float* Xb, float* T, float** o
   return MAPL_OK;
 }
 
+// ---------------------------------------------------------------- full SPEL step (Eq. 4-7)
+// M = -(S + S^T)/2 (batched [r,r])
+__global__ void k_neg_sym(const float* __restrict__ S, float* __restrict__ M, int r) {
+  const long long off = (long long)blockIdx.y * r * r;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= r * r) return;
+  const int a = idx / r, b = idx % r;
+  M[off + idx] = -0.5f * (S[off + a * r + b] + S[off + b * r + a]);
+}
+
+// m <- beta m + (1 - beta) xi ;  norm2[b] += sum m^2   (norm2 zeroed before)
+__global__ void __launch_bounds__(256) k_momentum(float* __restrict__ Mom, const float* __restrict__ xi, float beta, long long n,
+                                                  float* __restrict__ norm2) {
+  __shared__ float red[8];
+  const long long off = (long long)blockIdx.y * n;
+  float s = 0.f;
+  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256) {
+    const float m = fmaf(beta, Mom[off + i], (1.f - beta) * xi[off + i]);
+    Mom[off + i] = m;
+    s = fmaf(m, m, s);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (threadIdx.x % 32 == 0) red[threadIdx.x / 32] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int k = 1; k < 8; ++k) s += red[k];
+    atomicAdd(norm2 + blockIdx.y, s);
+  }
+}
+
+// out = a X + c Y / sqrt(norm2[b])   (norm2 == nullptr: plain a X + c Y;  norm2[b] == 0: the Y term is 0)
+__global__ void k_axpby_scaled(float* __restrict__ out, const float* __restrict__ X, float a, const float* __restrict__ Y, float c,
+                               const float* __restrict__ norm2, long long n) {
+  const long long off = (long long)blockIdx.y * n;
+  float cs = c;
+  if (norm2 != nullptr) { const float q = norm2[blockIdx.y]; cs = q > 0.f ? c / sqrtf(q) : 0.f; }
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+    out[off + i] = (X != nullptr ? a * X[off + i] : 0.f) + cs * Y[off + i];
+}
+
+struct StCtx {
+  int d, r, batch; cudaStream_t st; bool tc;
+  float *S, *M;
+  __nv_bfloat16 *Prow, *Ptr, *Ptr2, *Pm;
+};
+
+// xi = G - U sym(U^T G)  (Eq. 4) into `out`
+int ctx_tangent(const StCtx& c, const float* U, const float* G, float* out) {
+  const int d = c.d, r = c.r, batch = c.batch;
+  if (c.tc) {
+    { KernelScope ks(KID_MEMSET, c.st); MAPL_CUDA_CHECK(cudaMemsetAsync(c.S, 0, (size_t)batch * r * r * 4, c.st)); }
+    MAPL_RETURN_IF(tc_st_split(U, d, r, batch, 0, 0.f, c.Prow, c.Ptr, c.st));
+    MAPL_RETURN_IF(tc_st_split(G, d, r, batch, 0, 0.f, nullptr, c.Ptr2, c.st));
+    MAPL_RETURN_IF(tc_st_gemm3(c.Ptr, c.Ptr2, r, r, d, batch, c.S, nullptr, 0.f, d / 256 > 0 ? d / 256 : 1, c.st));
+    MAPL_RETURN_IF(tc_st_split(c.S, r, r, batch, 3, 0.f, c.Pm, nullptr, c.st));
+    return tc_st_gemm3(c.Prow, c.Pm, d, r, r, batch, out, G, 1.f, 1, c.st);
+  }
+  MAPL_RETURN_IF(gram(U, G, c.S, d, r, batch, c.st));
+  { KernelScope ks(KID_ST_STEP_MATRIX, c.st); k_neg_sym<<<dim3((r * r + 255) / 256, batch), 256, 0, c.st>>>(c.S, c.M, r); }
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  return right_mul(U, c.M, out, G, 1.f, d, r, batch, c.st);
+}
+
+// `iters` cubic Newton-Schulz iterations X <- X (3I - X^T X)/2 from `cur` (overwritten) with scratch `nxt`; the last
+// iterate is written to `final_out` (which may be neither cur nor nxt)
+int ctx_ns(const StCtx& c, float* cur, float* nxt, float* final_out, int iters) {
+  const int d = c.d, r = c.r, batch = c.batch;
+  for (int it = 0; it < iters; ++it) {
+    float* out = (it == iters - 1) ? final_out : nxt;
+    if (c.tc) {
+      MAPL_RETURN_IF(tc_st_split(cur, d, r, batch, 0, 0.f, c.Prow, c.Ptr, c.st, c.S, (long long)r * r));
+      MAPL_RETURN_IF(tc_st_gemm3(c.Ptr, c.Ptr, r, r, d, batch, c.S, nullptr, 0.f, d / 256 > 0 ? d / 256 : 1, c.st));
+      MAPL_RETURN_IF(tc_st_split(c.S, r, r, batch, 1, 0.f, c.Pm, nullptr, c.st));
+      MAPL_RETURN_IF(tc_st_gemm3(c.Prow, c.Pm, d, r, r, batch, out, nullptr, 0.f, 1, c.st));
+    } else {
+      MAPL_RETURN_IF(gram(cur, cur, c.S, d, r, batch, c.st, true));
+      { KernelScope ks(KID_ST_NS_POLY, c.st); k_ns_poly<<<dim3((r * r + 255) / 256, batch), 256, 0, c.st>>>(c.S, c.M, r); }
+      MAPL_CUDA_CHECK(cudaGetLastError());
+      MAPL_RETURN_IF(right_mul(cur, c.M, out, nullptr, 0.f, d, r, batch, c.st));
+    }
+    nxt = cur; cur = out;
+  }
+  return MAPL_OK;
+}
+
 }  // namespace
 
 int st_gemm_nn(const float* A, const float* B, float* C, int M, int N, int K, cudaStream_t st, float alpha, const float* E,
@@ -510,6 +598,45 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
     MAPL_CUDA_CHECK(cudaGetLastError());
   }
   return MAPL_OK;
+}
+
+size_t mapl_spel_workspace_bytes(int32_t d, int32_t r, int32_t batch) { return mapl_stiefel_workspace_bytes(d, r, batch); }
+
+int mapl_spel_step(int32_t d, int32_t r, int32_t batch, float* U, const float* G, float* Mom, float lr, float beta,
+                   int32_t lmo_iters, int32_t retr_iters, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (d < 8 || r < 8 || r > d || d % 8 || r % 8 || batch < 1) return MAPL_ERR_INVALID_ARG;
+  if (r > 1024) return MAPL_ERR_UNSUPPORTED;
+  if (!U || !G || !Mom) return MAPL_ERR_INVALID_ARG;
+  if (lmo_iters < 1 || lmo_iters > 16 || retr_iters < 1 || retr_iters > 16) return MAPL_ERR_INVALID_ARG;
+  if (!(beta >= 0.f && beta <= 1.f)) return MAPL_ERR_INVALID_ARG;
+  if (!aligned16(U) || !aligned16(G) || !aligned16(Mom) || !aligned16(workspace)) return MAPL_ERR_ALIGNMENT;
+  const StWs w = st_carve(d, r, batch);
+  if (!workspace || workspace_bytes < w.total) return MAPL_ERR_WORKSPACE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  char* ws = reinterpret_cast<char*>(workspace);
+  float* X0 = reinterpret_cast<float*>(ws + w.X0);
+  float* X1 = reinterpret_cast<float*>(ws + w.X1);
+  float* X2 = reinterpret_cast<float*>(ws + w.X2);
+  float* norm2 = reinterpret_cast<float*>(ws + w.norm2);
+  static const bool tc_enabled = !(getenv("MAPL_ST_TC") && getenv("MAPL_ST_TC")[0] == '0');
+  StCtx c;
+  c.d = d; c.r = r; c.batch = batch; c.st = st; c.tc = tc_st_ok(d, r) && tc_enabled;
+  c.S = reinterpret_cast<float*>(ws + w.S); c.M = reinterpret_cast<float*>(ws + w.M);
+  c.Prow = reinterpret_cast<__nv_bfloat16*>(ws + w.Prow); c.Ptr = reinterpret_cast<__nv_bfloat16*>(ws + w.Ptr);
+  c.Ptr2 = reinterpret_cast<__nv_bfloat16*>(ws + w.Ptr2); c.Pm = reinterpret_cast<__nv_bfloat16*>(ws + w.Pm);
+  const long long n = (long long)d * r;
+  const dim3 eg(148, batch);
+
+  MAPL_RETURN_IF(ctx_tangent(c, U, G, X0));                                                   // Eq. 4: xi -> X0
+  { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(norm2, 0, (size_t)batch * 4, st)); }
+  { KernelScope ks(KID_ST_STEP_MATRIX, st); k_momentum<<<eg, 256, 0, st>>>(Mom, X0, beta, n, norm2); }     // Eq. 5
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  { KernelScope ks(KID_ST_STEP_MATRIX, st); k_axpby_scaled<<<eg, 256, 0, st>>>(X1, nullptr, 0.f, Mom, 1.f, norm2, n); }   // m / ||m||_F
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  MAPL_RETURN_IF(ctx_ns(c, X1, X0, X2, lmo_iters));                                           // Eq. 6: d_t -> X2
+  { KernelScope ks(KID_ST_STEP_MATRIX, st); k_axpby_scaled<<<eg, 256, 0, st>>>(X0, U, 1.f, X2, -lr, nullptr, n); }        // U - lr d_t
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  return ctx_ns(c, X0, X1, U, retr_iters);                                                    // Eq. 7
 }
 
 }  // extern "C"

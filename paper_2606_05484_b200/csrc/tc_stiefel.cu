@@ -14,6 +14,7 @@
 //                optionally applies the r x r maps of the step on the fly:
 //                  mode 1  M  = (3 I - G) / 2                       (Newton-Schulz polynomial)
 //                  mode 2  M1 = I + lr (S + S^T) / 2                (tangent projection + step, Eq. 4)
+//                  mode 3  -(S + S^T) / 2                           (tangent projection alone: xi = G + U (-sym S))
 //   k_tc_gemm3   C[M,N] (+)= sum_pairs A_i[M,K] B_j[N,K]^T, both K-major, 128 x 128 tile per CTA,
 //                TMA-fed 2-stage ring of six [128 x 64] tiles; epilogue either C = acc + beta E (fp32
 //                stores) or red.global.add (split over K).
@@ -71,6 +72,7 @@ __global__ void __launch_bounds__(256) k_st_split(const float* __restrict__ src,
         x = src[(long long)r * cols + c];
         if (mode == 1) x = 0.5f * ((r == c ? 3.f : 0.f) - x);
         if (mode == 2) x = (r == c ? 1.f : 0.f) + lr * 0.5f * (x + src[(long long)c * cols + r]);
+        if (mode == 3) x = -0.5f * (x + src[(long long)c * cols + r]);
       }
       tile[i][tx] = x;
       if (prow && r < rows && c < cols) {

@@ -123,3 +123,50 @@ def test_orthonormal_after_every_step_1e12():
             G = rng.standard_normal((d, r))
             Uc, _ = o.stiefel_step(Uc, G, 1e-2, retr, 5)
             assert np.linalg.norm(Uc.T @ Uc - np.eye(r)) < 1e-12
+
+
+# ------------------------------------------------------------------ full SPEL step (Eq. 4-7)
+
+def _scalar_ns(s, iters):
+    for _ in range(iters):
+        s = 0.5 * s * (3.0 - s * s)
+    return s
+
+
+def test_spel_lmo_direction_matches_svd_with_scalar_iteration():
+    """The cubic Newton-Schulz map acts on singular values only: with m_new = P diag(s) Q^T, d = P diag(f(s/||s||)) Q^T where
+    f is the scalar iteration s <- s (3 - s^2)/2 applied lmo_iters times (independent computation by numpy SVD)."""
+    rng = np.random.default_rng(40)
+    d_, r = 40, 6
+    U = np.linalg.qr(rng.standard_normal((d_, r)))[0]
+    G = rng.standard_normal((d_, r)); m = rng.standard_normal((d_, r))
+    beta, lr = 0.9, 0.05
+    U2, m2, dirn = o.spel_step(U, G, m, lr, beta, 5, 7)
+    xi = o.tangent(U, G)
+    assert np.abs(m2 - (beta * m + (1 - beta) * xi)).max() < 1e-13
+    P, s, Qt = np.linalg.svd(m2, full_matrices=False)
+    f = np.array([_scalar_ns(x, 5) for x in s / np.linalg.norm(s)])
+    assert np.abs(dirn - (P * f) @ Qt).max() < 1e-12
+    # retraction: orthonormal to 1e-10 (sigma(U - lr d) within [1 - lr, 1 + lr]) and equal to the polar factor
+    assert np.linalg.norm(U2.T @ U2 - np.eye(r)) < 1e-10
+    Y = U - lr * dirn
+    Py, sy, Qyt = np.linalg.svd(Y, full_matrices=False)
+    assert np.abs(U2 - Py @ Qyt).max() < 1e-9
+
+
+def test_spel_special_cases():
+    rng = np.random.default_rng(41)
+    d_, r = 24, 4
+    U = np.linalg.qr(rng.standard_normal((d_, r)))[0]
+    G = rng.standard_normal((d_, r))
+    # beta = 1: the momentum is untouched, whatever G is
+    m = rng.standard_normal((d_, r))
+    _, m2, _ = o.spel_step(U, G, m, 0.1, 1.0)
+    assert np.array_equal(m2, m)
+    # no gradient, no momentum: nothing moves
+    U2, m2, dirn = o.spel_step(U, np.zeros_like(G), np.zeros_like(G), 0.1, 0.9)
+    assert not dirn.any() and not m2.any() and np.abs(U2 - U).max() < 1e-12
+    # momentum with orthonormal columns times a scalar: the direction is f(1/sqrt(r)) times those columns
+    W = np.linalg.qr(rng.standard_normal((d_, r)))[0]
+    _, _, dirn = o.spel_step(U, np.zeros_like(G), 3.7 * W, 0.1, 1.0, 5, 7)
+    assert np.abs(dirn - _scalar_ns(1.0 / np.sqrt(r), 5) * W).max() < 1e-12

@@ -87,3 +87,26 @@ def test_zero_gradient_is_fixed_point():
         U = to_dev(s.U); G = torch.zeros_like(U)
         _gpu_step(U, G, 0.1, RETR[retr][0])
         assert rel_fro(to_np(U)[0], s.U.f64[0]) <= 1e-5
+
+
+@pytest.mark.parametrize("d,r,batch", [(256, 32, 2), (512, 104, 1), (2048, 128, 2), (2048, 256, 3), (1024, 512, 1)])
+def test_spel_step_matches_oracle(d, r, batch):
+    """Full SPEL update (Eq. 4-7: tangent projection, momentum, LMO direction by 5 NS iterations, retraction by 7)
+    through the C ABI against oracle.spel_step, two consecutive steps (the second starts from the GPU's momentum)."""
+    s = I.make_stiefel(r, d=d, batch=batch)
+    rng = np.random.default_rng(7)
+    m0 = rng.standard_normal((batch, d, r)).astype(np.float32)
+    U = to_dev(s.U); G = to_dev(s.G); M = torch.from_numpy(m0.copy()).cuda()
+    ws = mb.alloc_workspace(mb.mapl_spel_workspace_bytes(d, r, batch))
+    lr, beta = 2e-3, 0.95
+    Uo = [s.U.f64[b] for b in range(batch)]
+    Mo = [m0[b].astype(np.float64) for b in range(batch)]
+    for step in range(2):
+        mb.mapl_spel_step(U, G, M, lr, beta, 5, 7, ws)
+        torch.cuda.synchronize()
+        Ug, Mg = to_np(U), to_np(M)
+        for b in range(batch):
+            Uo[b], Mo[b], _ = o.spel_step(Uo[b], s.G.f64[b], Mo[b], lr, beta, 5, 7)
+            assert rel_fro(Mg[b], Mo[b]) <= 1e-5
+            assert rel_fro(Ug[b], Uo[b]) <= 1e-5
+            assert np.linalg.norm(Ug[b].T @ Ug[b] - np.eye(r)) <= 1e-5
