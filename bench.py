@@ -462,6 +462,33 @@ def stiefel_sweep(torch, mb, I, stream, reps=10):
                                 for b in range(s.batch)))
                 out[f"r{r}_{tag}"] = {"us_per_step": round(us, 1), "projector_steps_per_s": round(s.batch * 1e6 / us),
                                       "orth_residual_after": float(f"{res:.2e}")}
+    # full SPEL update (Eq. 4-7: tangent projection, momentum 0.95, 5 + 7 Newton-Schulz iterations), SURVEY 8f next row 2
+    with torch.cuda.stream(stream):
+        for r in (64, 128, 256, 512):
+            s = I.make_stiefel(r)
+            ws = mb.alloc_workspace(mb.mapl_spel_workspace_bytes(s.d, r, s.batch))
+            U = torch.from_numpy(s.U.data.copy()).cuda()
+            G = torch.from_numpy(s.G.data.copy()).cuda()
+            Mom = torch.zeros_like(U)
+            f = lambda: mb.mapl_spel_step(U, G, Mom, 2e-3, 0.95, 5, 7, ws)
+            f()
+            stream.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                f()
+            g.replay()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                g.replay()
+            e1.record(stream)
+            stream.synchronize()
+            us = 1e3 * e0.elapsed_time(e1) / reps
+            Uh = U.double()
+            res = float(max(torch.linalg.matrix_norm(Uh[b].T @ Uh[b] - torch.eye(r, device="cuda", dtype=torch.float64))
+                            for b in range(s.batch)))
+            out[f"r{r}_spel"] = {"us_per_step": round(us, 1), "projector_steps_per_s": round(s.batch * 1e6 / us),
+                                 "orth_residual_after": float(f"{res:.2e}")}
     out["config"] = "d=2048, 3 projectors per call, fixed G, lr=1e-2, fp32"
     return out
 
