@@ -100,22 +100,34 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
     const long long m = m0 + row;
     const bool live = row < tile_m && m < N;
     const float* trow = (Tc != nullptr && live) ? Tc + (long long)__ldg(tok + m) * r : nullptr;
+    // centring rows are gathered (L2 latency): piece c+1 is in flight while piece c is consumed, piece 0 while the
+    // MMAs still run
+    float4 tcur[8], tnext[8];
+    if (trow != nullptr) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) tcur[i] = __ldg(reinterpret_cast<const float4*>(trow) + i);
+    }
     mbar_wait(accum_full, 0);
     if (warp == 2) { DBG(4) }
     tc_fence_after_sync();
     for (int c = 0; c < r / 32; ++c) {
       uint32_t v[32];
       tmem_ld32(tmem_d + ((uint32_t)(q * 32) << 16) + c * 32, v);
+      if (trow != nullptr && c + 1 < r / 32) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) tnext[i] = __ldg(reinterpret_cast<const float4*>(trow + (c + 1) * 32) + i);
+      }
       tmem_ld_wait();
       if (trow != nullptr) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
-          const float4 t4 = __ldg(reinterpret_cast<const float4*>(trow + c * 32) + i);
-          v[4 * i + 0] = __float_as_uint(__uint_as_float(v[4 * i + 0]) - t4.x);
-          v[4 * i + 1] = __float_as_uint(__uint_as_float(v[4 * i + 1]) - t4.y);
-          v[4 * i + 2] = __float_as_uint(__uint_as_float(v[4 * i + 2]) - t4.z);
-          v[4 * i + 3] = __float_as_uint(__uint_as_float(v[4 * i + 3]) - t4.w);
+          v[4 * i + 0] = __float_as_uint(__uint_as_float(v[4 * i + 0]) - tcur[i].x);
+          v[4 * i + 1] = __float_as_uint(__uint_as_float(v[4 * i + 1]) - tcur[i].y);
+          v[4 * i + 2] = __float_as_uint(__uint_as_float(v[4 * i + 2]) - tcur[i].z);
+          v[4 * i + 3] = __float_as_uint(__uint_as_float(v[4 * i + 3]) - tcur[i].w);
         }
+#pragma unroll
+        for (int i = 0; i < 8; ++i) tcur[i] = tnext[i];
       }
       if (live) {
         uint4* dst = reinterpret_cast<uint4*>(Z + m * r + c * 32);
