@@ -203,6 +203,20 @@ void mapl_profile_enable(int timing_on);
 void mapl_profile_reset(void);
 int mapl_profile_read(int kid, long long* launches, long long* timed_launches, double* total_ms);
 
+/* GROUPED MULTI-CODEBOOK VQ of a wire payload (Sec. 3.5; reading S3; SURVEY 8f "next" row 3).
+ * X [N,r] in the activation dtype is a stored payload: the Z written by mapl_encode (RVQ off) or the gz written by
+ * mapl_codec_backward.  Its r channels are cut into r/2 groups of G = 2 consecutive channels; group g is residual-
+ * vector-quantised on its own over `levels` rounds with the 2-d codewords codebooks[l, k, 2g:2g+2] (codebooks
+ * [levels,k,r] fp32, the layout of the full-vector RVQ), squared Euclidean distance, lowest index on ties (S4).
+ *   codes_out [N, levels, r/2] uint8 (k <= 256): (r/2) levels bytes per token -- 256 B at r = 256, levels = 2.
+ *   Xq_out    optional [N,r] activation dtype: the dequantised payload (sum of the chosen codewords, rounded once).
+ * mapl_mcvq_dequantize rebuilds Xq from the codes on the receiving side (feed it to mapl_decode as Z, or use it as
+ * gz).  r % 8 == 0, 1 <= levels <= 8, levels * k <= 2048.  No workspace.                                          */
+int mapl_mcvq_quantize(int64_t n_tokens, int32_t r, int32_t act_dtype, int32_t levels, int32_t k, const void* X,
+                       const float* codebooks, uint8_t* codes_out, void* Xq_out, void* cuda_stream);
+int mapl_mcvq_dequantize(int64_t n_tokens, int32_t r, int32_t act_dtype, int32_t levels, int32_t k, const uint8_t* codes,
+                         const float* codebooks, void* Xq_out, void* cuda_stream);
+
 /* FULL SPEL STEP (Eq. 4-7; SURVEY 8f "next" row 2) on `batch` projectors, U, G, M strided [batch,d,r] fp32:
  *     xi = G - U sym(U^T G)                      (Eq. 4, tangent projection)
  *     m  <- beta m + (1 - beta) xi               (Eq. 5, heavy-ball momentum; M_inout updated in place)

@@ -211,6 +211,45 @@ def stiefel_step(U, G, lr: float, retraction: int, ns_iters: int = 5):
 REL_GAP = 1e-4
 
 
+def mcvq(X, Cb, G: int, other_codes=None, rel: float = REL_GAP):
+    """Grouped multi-codebook VQ (reading S3): the r channels are cut into r/G groups
+    of G consecutive channels; group g is residual-vector-quantised on its own, over L rounds, with the G-dimensional
+    codewords Cb[l, k, gG:(g+1)G].  Every group is exactly the full-vector RVQ of this module applied to that slice.
+    other_codes [N,L,r/G] (optional): follow admissible near-tie choices of another implementation (rule S5, per group).
+    Returns dict(codes [N,L,r/G] int32, Xq [N,r], excepted, forced, bad)."""
+    X, Cb = _f64(X), _f64(Cb)
+    N, r = X.shape
+    L, K, _ = Cb.shape
+    assert r % G == 0
+    ng = r // G
+    codes = np.empty((N, L, ng), np.int32)
+    Xq = np.empty((N, r), np.float64)
+    n_exc = n_forced = n_bad = 0
+    for g in range(ng):
+        sl = slice(g * G, (g + 1) * G)
+        Xg = np.ascontiguousarray(X[:, sl])
+        Cg = np.ascontiguousarray(Cb[:, :, sl])
+        if other_codes is None:
+            res = rvq(Xg, Cg)
+        else:
+            res, e, f, bad = follow_codes(Xg, Cg, np.ascontiguousarray(other_codes[:, :, g]), rel)
+            n_exc += e; n_forced += f; n_bad += int(bad.sum())
+        codes[:, :, g] = res["codes"]
+        Xq[:, sl] = res["Zhat"]
+    return dict(codes=codes, Xq=Xq, excepted=n_exc, forced=n_forced, bad=n_bad)
+
+
+def mcvq_dequant(codes, Cb, G: int) -> np.ndarray:
+    """Xq[n, gG:(g+1)G] = sum_l Cb[l, codes[n,l,g], gG:(g+1)G]."""
+    codes, Cb = np.asarray(codes), _f64(Cb)
+    N, L, ng = codes.shape
+    Xq = np.zeros((N, ng * G), np.float64)
+    for g in range(ng):
+        for l in range(L):
+            Xq[:, g * G:(g + 1) * G] += Cb[l, codes[:, l, g], g * G:(g + 1) * G]
+    return Xq
+
+
 def spel_step(U, G, m, lr: float, beta: float, lmo_iters: int = 5, retr_iters: int = 7):
     """Full SPEL update, Eq. 4-7, step by step in the paper's order; PolarExpress is read as the
     cubic Newton-Schulz iteration (reading S11), for Eq. 6 from m / ||m||_F.  Returns (U_new, m_new, d)."""

@@ -64,6 +64,10 @@ def _load():
     lib.mapl_decode.argtypes = [dp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.mapl_codec_backward.argtypes = [dp] + [vp] * 14 + [C.c_int, vp, sz, vp]
     lib.mapl_stiefel_step.argtypes = [i32, i32, i32, vp, vp, f32, i32, i32, vp, vp, sz, vp]
+    lib.mapl_mcvq_quantize.restype = C.c_int
+    lib.mapl_mcvq_quantize.argtypes = [C.c_int64, i32, i32, i32, i32, vp, vp, vp, vp, vp]
+    lib.mapl_mcvq_dequantize.restype = C.c_int
+    lib.mapl_mcvq_dequantize.argtypes = [C.c_int64, i32, i32, i32, i32, vp, vp, vp, vp]
     lib.mapl_spel_workspace_bytes.restype = sz
     lib.mapl_spel_workspace_bytes.argtypes = [i32, i32, i32]
     lib.mapl_spel_step.restype = C.c_int
@@ -232,6 +236,27 @@ def mapl_stiefel_step(U_inout, G, lr: float, retraction: int, ns_iters: int, inf
                                   int(retraction), int(ns_iters), _ptr(info_out, f, "info_out"),
                                   _ptr(workspace, None, "workspace"),
                                   workspace.numel() * workspace.element_size(), _stream()), "mapl_stiefel_step")
+
+
+def _act_code(t: torch.Tensor) -> int:
+    return {torch.float32: MAPL_F32, torch.bfloat16: MAPL_BF16}[t.dtype]
+
+
+def mapl_mcvq_quantize(X, codebooks, codes_out, Xq_out=None) -> None:
+    """Grouped (G = 2) multi-codebook VQ of a payload X [N,r]; codebooks [L,K,r] fp32; codes_out [N,L,r/2] uint8."""
+    N, r = X.shape
+    L, K, _ = codebooks.shape
+    _check(_lib.mapl_mcvq_quantize(N, r, _act_code(X), L, K, _ptr(X, None, "X"), _ptr(codebooks, torch.float32, "codebooks"),
+                                   _ptr(codes_out, torch.uint8, "codes_out"), _ptr(Xq_out, X.dtype, "Xq_out"), _stream()),
+           "mapl_mcvq_quantize")
+
+
+def mapl_mcvq_dequantize(codes, codebooks, Xq_out) -> None:
+    N, r = Xq_out.shape
+    L, K, _ = codebooks.shape
+    _check(_lib.mapl_mcvq_dequantize(N, r, _act_code(Xq_out), L, K, _ptr(codes, torch.uint8, "codes"),
+                                     _ptr(codebooks, torch.float32, "codebooks"), _ptr(Xq_out, None, "Xq_out"), _stream()),
+           "mapl_mcvq_dequantize")
 
 
 def mapl_spel_workspace_bytes(d: int, r: int, batch: int) -> int:

@@ -1,0 +1,146 @@
+// mcvq.cu -- grouped multi-codebook VQ of a wire payload (Sec. 3.5; reading S3;
+// SURVEY 8f "next" row 3): the r channels of every token are cut into r/G groups of G = 2 consecutive channels, each
+// group is residual-vector-quantised on its own over L rounds with the 2-dimensional codewords C[l, k, 2g:2g+2], and
+// the index is one byte (K <= 256): (r/G) L bytes per token -- 256 B at the paper's r = 256, G = 2, K = 256, R = 2.
+// It quantises a stored payload tensor ([N,r] in the activation dtype): the forward payload Z written by mapl_encode,
+// or the backward payload gz of mapl_codec_backward ("compressing both forward activations and backward gradients").
+//
+// N (r/G) L K two-dimensional distance evaluations: CUDA-core work (no contraction worth a tensor core: K = 2 would be
+// padded 8x, and the arg-min scan stays on the ALUs anyway), bound by FP32 issue rate.
+//   k_mcvq_quantize   CTA = 64 tokens x 4 group lanes (256 threads).  Per step the 4 groups' codeword slices of all
+//                     rounds (L K float2 each) are staged in shared memory; a warp holds 32 tokens of ONE group, so
+//                     every codeword read is a broadcast.  Distances in the direct form (x - c)^2, fp32; lowest index
+//                     wins ties (S4).
+//   k_mcvq_dequantize thread = (token, group): sum of the chosen 2-d codewords, rounded once to the activation dtype.
+#include <float.h>
+
+#include "common.cuh"
+#include "profile.cuh"
+
+namespace mapl {
+namespace {
+
+constexpr int kTok = 64, kLanes = 4, kMaxLK = 8 * 256;      // L K <= 2048 codewords per group in shared memory
+
+template <bool kBf16>
+__global__ void __launch_bounds__(kTok* kLanes) k_mcvq_quantize(const void* __restrict__ Xv, const float* __restrict__ C,
+                                                               uint8_t* __restrict__ codes, void* __restrict__ Xqv, long long N,
+                                                               int r, int L, int K) {
+  extern __shared__ float2 sC[];                 // [kLanes][L*K]
+  const int t = threadIdx.x, tok_l = t % kTok, gl = t / kTok, ng = r / 2;
+  const long long n = (long long)blockIdx.x * kTok + tok_l;
+  const bool live = n < N;
+  for (int g0 = 0; g0 < ng; g0 += kLanes) {
+    // stage the slices of groups g0 .. g0+3: C[l, k, 2g : 2g+2]
+    for (int i = t; i < kLanes * L * K; i += kTok * kLanes) {
+      const int lane_g = i / (L * K), lk = i % (L * K), g = g0 + lane_g;
+      sC[i] = g < ng ? *reinterpret_cast<const float2*>(C + (long long)lk * r + 2 * g) : make_float2(0.f, 0.f);
+    }
+    __syncthreads();
+    const int g = g0 + gl;
+    if (g < ng && live) {
+      float x0, x1;
+      if (kBf16) {
+        const __nv_bfloat162 v = *reinterpret_cast<const __nv_bfloat162*>(reinterpret_cast<const __nv_bfloat16*>(Xv) + n * r + 2 * g);
+        x0 = __bfloat162float(v.x); x1 = __bfloat162float(v.y);
+      } else {
+        const float2 v = *reinterpret_cast<const float2*>(reinterpret_cast<const float*>(Xv) + n * r + 2 * g);
+        x0 = v.x; x1 = v.y;
+      }
+      float q0 = 0.f, q1 = 0.f;
+      const float2* cg = sC + (size_t)gl * L * K;
+      for (int l = 0; l < L; ++l) {
+        float best = FLT_MAX;
+        int bk = 0;
+        const float2* cl = cg + l * K;
+#pragma unroll 8
+        for (int k = 0; k < K; ++k) {
+          const float2 c = cl[k];
+          const float d0 = x0 - c.x, d1 = x1 - c.y;
+          const float dist = fmaf(d1, d1, d0 * d0);
+          if (dist < best) { best = dist; bk = k; }           // strict: lowest index on ties
+        }
+        const float2 c = cl[bk];
+        x0 -= c.x; x1 -= c.y;
+        q0 += c.x; q1 += c.y;
+        codes[(n * L + l) * ng + g] = (uint8_t)bk;
+      }
+      if (Xqv != nullptr) {
+        if (kBf16) *reinterpret_cast<__nv_bfloat162*>(reinterpret_cast<__nv_bfloat16*>(Xqv) + n * r + 2 * g) = __floats2bfloat162_rn(q0, q1);
+        else *reinterpret_cast<float2*>(reinterpret_cast<float*>(Xqv) + n * r + 2 * g) = make_float2(q0, q1);
+      }
+    }
+    __syncthreads();
+  }
+}
+
+template <bool kBf16>
+__global__ void k_mcvq_dequantize(const uint8_t* __restrict__ codes, const float* __restrict__ C, void* __restrict__ Xqv,
+                                  long long N, int r, int L, int K) {
+  const int ng = r / 2;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= N * ng) return;
+  const long long n = idx / ng;
+  const int g = (int)(idx % ng);
+  float q0 = 0.f, q1 = 0.f;
+  for (int l = 0; l < L; ++l) {
+    const int k = codes[(n * L + l) * ng + g];
+    const float2 c = *reinterpret_cast<const float2*>(C + ((long long)l * K + k) * r + 2 * g);
+    q0 += c.x; q1 += c.y;
+  }
+  if (kBf16) *reinterpret_cast<__nv_bfloat162*>(reinterpret_cast<__nv_bfloat16*>(Xqv) + n * r + 2 * g) = __floats2bfloat162_rn(q0, q1);
+  else *reinterpret_cast<float2*>(reinterpret_cast<float*>(Xqv) + n * r + 2 * g) = make_float2(q0, q1);
+}
+
+int check(int64_t N, int r, int L, int K, int act_dtype) {
+  if (N < 0 || r < 2 || r % 8 || L < 1 || L > 8 || K < 1 || K > 256) return MAPL_ERR_INVALID_ARG;
+  if (L * K > kMaxLK) return MAPL_ERR_UNSUPPORTED;
+  if (act_dtype != MAPL_F32 && act_dtype != MAPL_BF16) return MAPL_ERR_INVALID_ARG;
+  return MAPL_OK;
+}
+
+}  // namespace
+}  // namespace mapl
+
+using namespace mapl;
+
+extern "C" {
+
+int mapl_mcvq_quantize(int64_t n_tokens, int32_t r, int32_t act_dtype, int32_t levels, int32_t k, const void* X,
+                       const float* codebooks, uint8_t* codes_out, void* Xq_out, void* cuda_stream) {
+  MAPL_RETURN_IF(check(n_tokens, r, levels, k, act_dtype));
+  if (n_tokens == 0) return MAPL_OK;
+  if (!X || !codebooks || !codes_out) return MAPL_ERR_INVALID_ARG;
+  if (!aligned16(X) || !aligned16(codebooks) || !aligned16(codes_out) || (Xq_out && !aligned16(Xq_out))) return MAPL_ERR_ALIGNMENT;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const size_t smem = (size_t)kLanes * levels * k * sizeof(float2);
+  static bool attr_done = false;
+  if (!attr_done) {
+    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_mcvq_quantize<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLanes * kMaxLK * 8));
+    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_mcvq_quantize<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLanes * kMaxLK * 8));
+    attr_done = true;
+  }
+  const unsigned blocks = (unsigned)((n_tokens + kTok - 1) / kTok);
+  KernelScope ks(KID_MCVQ, st);
+  if (act_dtype == MAPL_BF16) k_mcvq_quantize<true><<<blocks, kTok * kLanes, smem, st>>>(X, codebooks, codes_out, Xq_out, n_tokens, r, levels, k);
+  else k_mcvq_quantize<false><<<blocks, kTok * kLanes, smem, st>>>(X, codebooks, codes_out, Xq_out, n_tokens, r, levels, k);
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  return MAPL_OK;
+}
+
+int mapl_mcvq_dequantize(int64_t n_tokens, int32_t r, int32_t act_dtype, int32_t levels, int32_t k, const uint8_t* codes,
+                         const float* codebooks, void* Xq_out, void* cuda_stream) {
+  MAPL_RETURN_IF(check(n_tokens, r, levels, k, act_dtype));
+  if (n_tokens == 0) return MAPL_OK;
+  if (!codes || !codebooks || !Xq_out) return MAPL_ERR_INVALID_ARG;
+  if (!aligned16(codes) || !aligned16(codebooks) || !aligned16(Xq_out)) return MAPL_ERR_ALIGNMENT;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const long long total = n_tokens * (r / 2);
+  KernelScope ks(KID_MCVQ, st);
+  if (act_dtype == MAPL_BF16) k_mcvq_dequantize<true><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(codes, codebooks, Xq_out, n_tokens, r, levels, k);
+  else k_mcvq_dequantize<false><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(codes, codebooks, Xq_out, n_tokens, r, levels, k);
+  MAPL_CUDA_CHECK(cudaGetLastError());
+  return MAPL_OK;
+}
+
+}  // extern "C"

@@ -28,6 +28,7 @@ enum KernelId {
   KID_ST_GEMM,
   KID_ST_SPLIT,
   KID_ST_GEMM3,
+  KID_MCVQ,
   KID_COUNT
 };
 

@@ -109,3 +109,14 @@ def test_centering_entry_points_check_arguments():
     assert lib.mapl_center_table(C.byref(d), p, p, p, None, p, 8192, None) == -1
     # workspace too small
     assert lib.mapl_center_table(C.byref(d), p, p, p, p, p, 16, None) == -4
+
+
+def test_mcvq_entry_points_check_arguments():
+    lib = mb.raw_lib()
+    buf = (C.c_char * 8192)()
+    p = (C.addressof(buf) + 15) & ~15
+    assert lib.mapl_mcvq_quantize(16, 64, 1, 2, 300, p, p, p, None, None) == -1       # K > 256: no byte index
+    assert lib.mapl_mcvq_quantize(16, 64, 1, 2, 256, None, p, p, None, None) == -1    # X NULL
+    assert lib.mapl_mcvq_quantize(16, 12, 1, 2, 256, p, p, p, None, None) == -1       # r % 8 != 0
+    assert lib.mapl_mcvq_dequantize(16, 64, 1, 2, 256, p, p, None, None) == -1        # Xq_out NULL
+    assert lib.mapl_mcvq_quantize(0, 64, 1, 2, 256, None, None, None, None, None) == 0  # empty batch: no-op

@@ -325,3 +325,38 @@ def test_centring_backward_matches_finite_differences():
     assert not bw["dA_s"][V - 1].any()                          # absent id: zero row
     # closed form of the U term: (H - A_s[tok] B_s)^T gz
     assert np.abs((H - A[tok] @ B).T @ gz - (H.T @ gz + bw["dU_corr"])).max() < 1e-12
+
+
+# ------------------------------------------------------------------ grouped MCVQ (reading S3)
+
+def test_mcvq_groups_match_brute_force_and_reduce_to_rvq():
+    rng = np.random.default_rng(50)
+    N, r, G, K, L = 37, 8, 2, 9, 3
+    X = rng.standard_normal((N, r))
+    Cb = rng.standard_normal((L, K, r)) * (0.5 ** np.arange(L))[:, None, None]
+    out = o.mcvq(X, Cb, G)
+    # independent brute force: per token, per group, per round, every codeword, direct distances
+    for n in range(N):
+        for g in range(r // G):
+            rho = X[n, g * G:(g + 1) * G].copy()
+            for l in range(L):
+                D = [float(((rho - Cb[l, k, g * G:(g + 1) * G]) ** 2).sum()) for k in range(K)]
+                k_star = int(np.argmin(D))
+                assert out["codes"][n, l, g] == k_star
+                rho -= Cb[l, k_star, g * G:(g + 1) * G]
+    assert np.abs(out["Xq"] - o.mcvq_dequant(out["codes"], Cb, G)).max() < 1e-12
+    # one group of r channels is the full-vector RVQ
+    full = o.mcvq(X, Cb, r)
+    ref = o.rvq(X, Cb)
+    assert np.array_equal(full["codes"][:, :, 0], ref["codes"]) and np.abs(full["Xq"] - ref["Zhat"]).max() < 1e-12
+    # groups do not talk to each other: changing the channels of one group changes that group's codes only
+    X2 = X.copy(); X2[:, 2:4] += 5.0
+    out2 = o.mcvq(X2, Cb, G)
+    assert np.array_equal(np.delete(out2["codes"], 1, axis=2), np.delete(out["codes"], 1, axis=2))
+
+
+def test_mcvq_payload_is_256_bytes_at_the_papers_setting():
+    """P:181 / P:403: r=256, G=2, K=256, R=2 -> 128 groups x 2 rounds x 1 byte."""
+    r, G, R, K = 256, 2, 2, 256
+    codes_per_token = (r // G) * R
+    assert codes_per_token * int(np.ceil(np.log2(K) / 8)) == 256
