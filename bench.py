@@ -523,6 +523,31 @@ def centering_times(torch, mb, b, cfg, stream, reps=10):
             e1.record(stream)
             stream.synchronize()
             out[name] = round(1e3 * e0.elapsed_time(e1) / reps, 2)
+    # grouped MCVQ (G=2, K=256, R=2) of the workload's [N,r] payload (gz of boundary 0)
+    gen = torch.Generator(device="cuda").manual_seed(3)
+    Cb = torch.randn((2, 256, cfg.r), device="cuda", generator=gen) * torch.tensor([1.0, 0.4], device="cuda")[:, None, None]
+    codes8 = torch.empty((cfg.n_tokens, 2, cfg.r // 2), dtype=torch.uint8, device="cuda")
+    Xq = torch.empty_like(b.gz)
+    fns2 = {
+        "mapl_mcvq_quantize": lambda: mb.mapl_mcvq_quantize(b.gz, Cb, codes8, None),
+        "mapl_mcvq_dequantize": lambda: mb.mapl_mcvq_dequantize(codes8, Cb, Xq),
+    }
+    with torch.cuda.stream(stream):
+        for name, f in fns2.items():
+            f()
+            stream.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                f()
+            g.replay()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                g.replay()
+            e1.record(stream)
+            stream.synchronize()
+            out[name] = round(1e3 * e0.elapsed_time(e1) / reps, 2)
+    out["mcvq_bytes_per_token"] = cfg.r  # (r/2) groups x 2 rounds x 1 byte
     out["note"] = "us per call, boundary 0; not part of the codec metric"
     return out
 
