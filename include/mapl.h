@@ -211,7 +211,7 @@ int mapl_profile_read(int kid, long long* launches, long long* timed_launches, d
  *   codes_out [N, levels, r/2] uint8 (k <= 256): (r/2) levels bytes per token -- 256 B at r = 256, levels = 2.
  *   Xq_out    optional [N,r] activation dtype: the dequantised payload (sum of the chosen codewords, rounded once).
  * mapl_mcvq_dequantize rebuilds Xq from the codes on the receiving side (feed it to mapl_decode as Z, or use it as
- * gz).  r % 8 == 0, 1 <= levels <= 8, levels * k <= 2048.  No workspace.                                          */
+ * gz).  r % 8 == 0, 1 <= levels <= 4.  No workspace.                                                            */
 int mapl_mcvq_quantize(int64_t n_tokens, int32_t r, int32_t act_dtype, int32_t levels, int32_t k, const void* X,
                        const float* codebooks, uint8_t* codes_out, void* Xq_out, void* cuda_stream);
 int mapl_mcvq_dequantize(int64_t n_tokens, int32_t r, int32_t act_dtype, int32_t levels, int32_t k, const uint8_t* codes,
