@@ -548,6 +548,30 @@ def centering_times(torch, mb, b, cfg, stream, reps=10):
             stream.synchronize()
             out[name] = round(1e3 * e0.elapsed_time(e1) / reps, 2)
     out["mcvq_bytes_per_token"] = cfg.r  # (r/2) groups x 2 rounds x 1 byte
+    # retained-energy diagnostic (Fig. 4b) and one micro-batch's codebook delta (a fifth of 2 x 256 rows)
+    sums = torch.zeros(2, dtype=torch.float64, device="cuda")
+    Zp = b.Zq if b.Zq is not None else b.gz
+    idx = torch.arange(0, 512, 5, dtype=torch.int32, device="cuda")
+    rows = torch.empty((idx.numel(), cfg.r), dtype=torch.float32, device="cuda")
+    fns3 = {
+        "mapl_energy_retained": lambda: mb.mapl_energy_retained(b.H, Zp, sums),
+        "mapl_codebook_delta_pack+apply": lambda: (mb.mapl_codebook_delta_pack(Cb, idx, rows), mb.mapl_codebook_delta_apply(Cb, idx, rows)),
+    }
+    with torch.cuda.stream(stream):
+        for name, f in fns3.items():
+            f()
+            stream.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                f()
+            g.replay()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                g.replay()
+            e1.record(stream)
+            stream.synchronize()
+            out[name] = round(1e3 * e0.elapsed_time(e1) / reps, 2)
     out["note"] = "us per call, boundary 0; not part of the codec metric"
     return out
 

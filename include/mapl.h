@@ -217,6 +217,24 @@ int mapl_mcvq_quantize(int64_t n_tokens, int32_t r, int32_t act_dtype, int32_t l
 int mapl_mcvq_dequantize(int64_t n_tokens, int32_t r, int32_t act_dtype, int32_t levels, int32_t k, const uint8_t* codes,
                          const float* codebooks, void* Xq_out, void* cuda_stream);
 
+/* STREAMING CODEBOOK SYNCHRONISATION, device side, and the retained-energy diagnostic (SURVEY 8f "next" row 4).
+ * P:151-153 / P:405-411: sender and receiver keep identical codebooks by shipping a random subset of the codewords
+ * with every micro-batch instead of the whole table.  The codebooks are viewed as a table [L*K, r] fp32:
+ *   mapl_codebook_delta_pack   rows_out[i,:] = codebooks[idx[i],:]   (sender: the m rows this micro-batch carries)
+ *   mapl_codebook_delta_apply  codebooks[idx[i],:] = rows[i,:]       (receiver: patch its copy; idx without duplicates)
+ * idx [m] int32 device, flat row numbers in [0, L*K).  WHICH rows travel when is host protocol logic (reading S15: a
+ * seeded permutation of the rows cut into `interval` = 5 parts, part t mod 5 with micro-batch t: after 5 micro-batches
+ * every row has been refreshed).  r % 4 == 0.
+ *   mapl_energy_retained   sums_inout[0] += ||Z||_F^2, sums_inout[1] += ||H||_F^2  (device double[2], caller-zeroed):
+ *   E = sums[0] / sums[1] is the energy of the activations retained under projection, ||X A||_F^2 / ||X||_F^2 of
+ *   Fig. 4(b).  H [N,d], Z [N,r] in the activation dtype (Z as written by mapl_encode, RVQ off).          */
+int mapl_codebook_delta_pack(const float* codebooks, int32_t r, const int32_t* idx, int32_t m, float* rows_out,
+                             void* cuda_stream);
+int mapl_codebook_delta_apply(float* codebooks_inout, int32_t r, const int32_t* idx, int32_t m, const float* rows,
+                              void* cuda_stream);
+int mapl_energy_retained(int64_t n_tokens, int32_t d, int32_t r, int32_t act_dtype, const void* H, const void* Z,
+                         double* sums_inout, void* cuda_stream);
+
 /* FULL SPEL STEP (Eq. 4-7; SURVEY 8f "next" row 2) on `batch` projectors, U, G, M strided [batch,d,r] fp32:
  *     xi = G - U sym(U^T G)                      (Eq. 4, tangent projection)
  *     m  <- beta m + (1 - beta) xi               (Eq. 5, heavy-ball momentum; M_inout updated in place)

@@ -250,6 +250,21 @@ def mcvq_dequant(codes, Cb, G: int) -> np.ndarray:
     return Xq
 
 
+def energy_retained(H, Z) -> float:
+    """Fig. 4(b): ||X A||_F^2 / ||X||_F^2 with Z = X A."""
+    H, Z = _f64(H), _f64(Z)
+    return float((Z * Z).sum() / (H * H).sum())
+
+
+def codebook_delta_apply(Cb, idx, rows) -> np.ndarray:
+    """Receiver side of the streaming codebook synchronisation: the rows idx of the [L*K, r] table are
+    replaced by `rows`; returns the patched copy."""
+    Cb = _f64(Cb).copy()
+    flat = Cb.reshape(-1, Cb.shape[-1])
+    flat[np.asarray(idx)] = _f64(rows)
+    return Cb
+
+
 def spel_step(U, G, m, lr: float, beta: float, lmo_iters: int = 5, retr_iters: int = 7):
     """Full SPEL update, Eq. 4-7, step by step in the paper's order; PolarExpress is read as the
     cubic Newton-Schulz iteration (reading S11), for Eq. 6 from m / ||m||_F.  Returns (U_new, m_new, d)."""

@@ -68,6 +68,12 @@ def _load():
     lib.mapl_mcvq_quantize.argtypes = [C.c_int64, i32, i32, i32, i32, vp, vp, vp, vp, vp]
     lib.mapl_mcvq_dequantize.restype = C.c_int
     lib.mapl_mcvq_dequantize.argtypes = [C.c_int64, i32, i32, i32, i32, vp, vp, vp, vp]
+    lib.mapl_codebook_delta_pack.restype = C.c_int
+    lib.mapl_codebook_delta_pack.argtypes = [vp, i32, vp, i32, vp, vp]
+    lib.mapl_codebook_delta_apply.restype = C.c_int
+    lib.mapl_codebook_delta_apply.argtypes = [vp, i32, vp, i32, vp, vp]
+    lib.mapl_energy_retained.restype = C.c_int
+    lib.mapl_energy_retained.argtypes = [C.c_int64, i32, i32, i32, vp, vp, vp, vp]
     lib.mapl_spel_workspace_bytes.restype = sz
     lib.mapl_spel_workspace_bytes.argtypes = [i32, i32, i32]
     lib.mapl_spel_step.restype = C.c_int
@@ -257,6 +263,28 @@ def mapl_mcvq_dequantize(codes, codebooks, Xq_out) -> None:
     _check(_lib.mapl_mcvq_dequantize(N, r, _act_code(Xq_out), L, K, _ptr(codes, torch.uint8, "codes"),
                                      _ptr(codebooks, torch.float32, "codebooks"), _ptr(Xq_out, None, "Xq_out"), _stream()),
            "mapl_mcvq_dequantize")
+
+
+def mapl_codebook_delta_pack(codebooks, idx, rows_out) -> None:
+    """rows_out[i] = codebooks.view(-1, r)[idx[i]]: the codewords a micro-batch carries (streaming sync)."""
+    r = codebooks.shape[-1]
+    _check(_lib.mapl_codebook_delta_pack(_ptr(codebooks, torch.float32, "codebooks"), r, _ptr(idx, torch.int32, "idx"),
+                                         idx.numel(), _ptr(rows_out, torch.float32, "rows_out"), _stream()),
+           "mapl_codebook_delta_pack")
+
+
+def mapl_codebook_delta_apply(codebooks_inout, idx, rows) -> None:
+    r = codebooks_inout.shape[-1]
+    _check(_lib.mapl_codebook_delta_apply(_ptr(codebooks_inout, torch.float32, "codebooks"), r, _ptr(idx, torch.int32, "idx"),
+                                          idx.numel(), _ptr(rows, torch.float32, "rows"), _stream()),
+           "mapl_codebook_delta_apply")
+
+
+def mapl_energy_retained(H, Z, sums_inout) -> None:
+    """sums_inout (float64[2], zeroed by the caller) += (||Z||_F^2, ||H||_F^2); E = sums[0] / sums[1] (Fig. 4b)."""
+    N, d = H.shape
+    _check(_lib.mapl_energy_retained(N, d, Z.shape[1], _act_code(H), _ptr(H, None, "H"), _ptr(Z, H.dtype, "Z"),
+                                     _ptr(sums_inout, torch.float64, "sums_inout"), _stream()), "mapl_energy_retained")
 
 
 def mapl_spel_workspace_bytes(d: int, r: int, batch: int) -> int:

@@ -11,7 +11,7 @@ const char* kNames[KID_COUNT] = {
     "k_simt_gemm", "k_half_sqnorm", "k_simt_encode_rvq", "k_dequant", "k_scatter_add_rows",
     "k_step_matrix", "k_ns_poly", "k_fro_norm", "k_chol_upper", "k_tri_inverse_upper", "memset",
     "k_tc_pack", "k_tc_encode", "k_tc_decode", "k_tc_bwd_gz", "k_tc_bwd_du", "k_tc_encode_rvq",
-    "k_tc_scatter", "k_st_gemm", "k_st_split", "k_tc_gemm3", "k_mcvq"};
+    "k_tc_scatter", "k_st_gemm", "k_st_split", "k_tc_gemm3", "k_mcvq", "k_stream_diag"};
 
 struct Pair { cudaEvent_t a, b; int kid; };
 bool g_timing = false;

@@ -29,6 +29,7 @@ enum KernelId {
   KID_ST_SPLIT,
   KID_ST_GEMM3,
   KID_MCVQ,
+  KID_STREAM_DIAG,
   KID_COUNT
 };
 

@@ -210,3 +210,11 @@ def make_stiefel(r: int, d: int = STIEFEL_D, batch: int = STIEFEL_BATCH, step: i
     Gs = np.stack([g_scale * _rng(4, i, _T_GSTIEFEL, r * 100003 + step).standard_normal((d, r))
                    for i in range(batch)])
     return StiefelInputs(d, r, batch, store(Us, "f32"), store(Gs, "f32"))
+
+
+def codebook_stream_parts(n_rows: int, interval: int = 5, seed: int = 0):
+    """Streaming codebook synchronisation schedule ("streaming interval 5"; reading S15): a seeded
+    permutation of the n_rows = L*K codeword rows cut into `interval` parts; micro-batch t carries part t % interval.
+    Protocol bookkeeping only (no arithmetic of the method); returns a list of int32 index arrays."""
+    perm = np.random.default_rng(np.random.SeedSequence([260605484, 15, seed])).permutation(n_rows).astype(np.int32)
+    return [np.ascontiguousarray(p) for p in np.array_split(perm, interval)]

@@ -8,6 +8,7 @@ import numpy as np
 import pytest
 
 from oracle import mapl_oracle as o
+from paper_2606_05484_b200 import inputs as I
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 
@@ -360,3 +361,31 @@ def test_mcvq_payload_is_256_bytes_at_the_papers_setting():
     r, G, R, K = 256, 2, 2, 256
     codes_per_token = (r // G) * R
     assert codes_per_token * int(np.ceil(np.log2(K) / 8)) == 256
+
+
+# ------------------------------------------------------------------ streaming codebook sync + retained energy (row 4)
+
+def test_energy_retained_closed_forms():
+    """E = ||X A||^2 / ||X||^2: 1 when the rows of X lie in span(A); sum of the top-r squared singular values over all of them
+    when A holds the top-r right singular vectors (P:55 energy formula); at most 1 for any orthonormal A."""
+    rng = np.random.default_rng(80)
+    X = rng.standard_normal((50, 12)) * np.linspace(3, 0.1, 12)
+    A = _orth(rng, 12, 4)
+    assert o.energy_retained(X, o.project(X, A)) <= 1.0 + 1e-12
+    Xin = rng.standard_normal((50, 4)) @ A.T
+    assert abs(o.energy_retained(Xin, o.project(Xin, A)) - 1.0) < 1e-12
+    _, s, Vt = np.linalg.svd(X, full_matrices=False)
+    assert abs(o.energy_retained(X, o.project(X, Vt[:4].T)) - (s[:4] ** 2).sum() / (s ** 2).sum()) < 1e-12
+
+
+def test_codebook_stream_schedule_refreshes_every_row_once_per_interval():
+    parts = I.codebook_stream_parts(2 * 256, interval=5, seed=3)
+    allidx = np.concatenate(parts)
+    assert len(parts) == 5 and sorted(allidx.tolist()) == list(range(512))        # a partition of the rows
+    assert max(len(p) for p in parts) - min(len(p) for p in parts) <= 1             # a fifth each
+    rng = np.random.default_rng(81)
+    sender = rng.standard_normal((2, 256, 8)); receiver = np.zeros_like(sender)
+    for t in range(5):                                                              # static sender: converged after 5
+        rows = sender.reshape(-1, 8)[parts[t]]
+        receiver = o.codebook_delta_apply(receiver, parts[t], rows)
+    assert np.array_equal(receiver, sender)
