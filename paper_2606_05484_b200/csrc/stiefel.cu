@@ -66,66 +66,215 @@ __global__ void k_fro_norm(const float* __restrict__ X, const float* __restrict_
   }
 }
 
-// One panel step of the in-place upper Cholesky G = R^T R (row-major [r,r], right-looking, blocked by NB;
-// one CTA per batch item): factor the diagonal block at p, zero the strict lower part of its columns,
-// solve the panel rows R[p:p+nb, p+nb:].  The trailing update G[p+nb:, p+nb:] -= R_panel^T R_panel is a
-// multi-CTA launch of k_st_gemm (chol_upper below).
-__global__ void __launch_bounds__(256) k_chol_panel(float* __restrict__ Gb, int r, int p) {
-  __shared__ float D[NB][NB + 1];
-  float* G = Gb + (long long)blockIdx.x * r * r;
-  const int tid = threadIdx.x, lane = tid % 32, warp = tid / 32;
-  const int nb = min(NB, r - p);
-  for (int idx = tid; idx < nb * nb; idx += blockDim.x) {
-    const int a = idx / nb, b = idx % nb;
-    D[a][b] = G[(long long)(p + a) * r + p + b];
-  }
-  __syncthreads();
-  if (warp == 0) {
-    // the 32 x 32 block lives in registers, lane = column (col[a] = D[a][lane]); row j is exchanged by shuffles.
-    // Rows / columns past nb are padded with the identity.
-    float col[NB];
+// ---------------------------------------------------------------- blocked upper Cholesky G = R^T R with look-ahead
+// Right-looking, NB = 32 columns per panel, ONE launch per panel (k_chol_step).  A panel's diagonal block D is
+// factored by the launch BEFORE the one that uses it: the CTA that updates the leading trailing tile factors the
+// next diagonal block from its own result (look-ahead).  The panel rows D^-T G[p:p+NB, cols] are a forward
+// substitution (one thread per column) that every CTA redoes for the two column ranges its tile needs, instead of a
+// single CTA solving the whole panel.  The critical path of a launch is load -> solve -> update -> factor; the
+// inverses of the diagonal blocks (seed of the blocked triangular inverse below) are computed off that path by one
+// extra CTA per launch and land in the diagonal blocks of Xinv.
+
+// warp-level: factor the NB x NB block in Dn (upper triangle read; rows / columns past nb padded with the identity),
+// write R (strict lower part zeroed) to Gd (pitch r).  lane = column.
+__device__ __forceinline__ void diag_factor(float (*Dn)[NB + 1], int nb, float* __restrict__ Gd, int r, int lane) {
+  float col[NB];                     // col[a] = D[a][lane]; row j is exchanged by shuffles
 #pragma unroll
-    for (int a = 0; a < NB; ++a) col[a] = (a < nb && lane < nb) ? D[a][lane] : (a == lane ? 1.f : 0.f);
+  for (int a = 0; a < NB; ++a) col[a] = (a < nb && lane < nb) ? Dn[a][lane] : (a == lane ? 1.f : 0.f);
 #pragma unroll
-    for (int j = 0; j < NB; ++j) {
-      const float dj = sqrtf(__shfl_sync(0xffffffffu, col[j], j));
-      const float rowj = lane == j ? dj : (lane > j ? col[j] / dj : col[j]);     // R[j][lane]
-      col[j] = rowj;
+  for (int j = 0; j < NB; ++j) {
+    const float c = __shfl_sync(0xffffffffu, col[j], j);
+    float y = rsqrtf(c);
+    y = y * fmaf(-0.5f * c * y, y, 1.5f);                                      // one Newton step: 1/sqrt(c) to ~1 ulp
+    const float rowj = lane == j ? c * y : (lane > j ? col[j] * y : col[j]);   // R[j][lane]
+    col[j] = rowj;
 #pragma unroll
-      for (int a = j + 1; a < NB; ++a) {
-        const float dja = __shfl_sync(0xffffffffu, rowj, a);                      // R[j][a]
-        if (a <= lane) col[a] = fmaf(-dja, rowj, col[a]);
-      }
+    for (int a = j + 1; a < NB; ++a) {
+      const float dja = __shfl_sync(0xffffffffu, rowj, a);                      // R[j][a]
+      if (a <= lane) col[a] = fmaf(-dja, rowj, col[a]);
     }
+  }
 #pragma unroll
-    for (int a = 0; a < NB; ++a)
-      if (a < nb && lane < nb) D[a][lane] = col[a];
+  for (int a = 0; a < NB; ++a)
+    if (a < nb && lane < nb) Gd[(long long)a * r + lane] = a <= lane ? col[a] : 0.f;
+}
+
+// warp-level: Xd = R^-1 for the upper-triangular block in Dn (padded with the identity past nb).  lane = column:
+// back substitution with x[k] = 0 for k > lane, so the loops are uniform and every Dn read is a broadcast.
+__device__ __forceinline__ void diag_invert(float (*Dn)[NB + 1], int nb, float* __restrict__ Xd, int r, int lane) {
+  float x[NB];
+#pragma unroll
+  for (int a = NB - 1; a >= 0; --a) {
+    float s = a == lane ? 1.f : 0.f;
+#pragma unroll
+    for (int k = a + 1; k < NB; ++k) s = fmaf(-Dn[a][k], x[k], s);
+    x[a] = a <= lane ? s / Dn[a][a] : 0.f;
+  }
+#pragma unroll
+  for (int a = 0; a < NB; ++a)
+    if (a < nb && lane < nb) Xd[(long long)a * r + lane] = x[a];
+}
+
+// first diagonal block (one warp per batch item)
+__global__ void __launch_bounds__(32) k_chol_first(float* __restrict__ Gb, int r) {
+  __shared__ float Dn[NB][NB + 1];
+  float* G = Gb + (long long)blockIdx.x * r * r;
+  const int lane = threadIdx.x, nb = min(NB, r);
+  for (int a = 0; a < nb; ++a) Dn[a][lane] = lane < nb ? G[(long long)a * r + lane] : 0.f;
+  __syncwarp();
+  diag_factor(Dn, nb, G, r, lane);
+}
+
+// Panel p (diagonal block already factored); q = p + NB.  grid = (64x64 tiles on or above the diagonal of the trailing
+// block G[q:, q:]  +  1, batch).  Tile CTAs: P = D^-T G[p:p+NB, cols] for the tile's row range and column range,
+// tile -= P_r^T P_c; diagonal tiles store P (= rows p..p+NB of R) into the SEPARATE matrix Pb (other CTAs of the
+// launch still read the raw panel rows of G); tile (0,0) then factors the next diagonal block.  The extra CTA inverts
+// D into Xinv[p:p+NB, p:p+NB].  R is thus held in two matrices: its diagonal NB-blocks in G, the rest in Pb.
+__global__ void __launch_bounds__(256) k_chol_step(float* __restrict__ Gb, float* __restrict__ Xb, float* __restrict__ Pb, int r, int p) {
+  constexpr int TS = 64, PAD = 4;
+  __shared__ float Di[NB][NB + 1];
+  __shared__ float rd[NB];
+  __shared__ __align__(16) float Pr[NB][TS + PAD], Pc[NB][TS + PAD];
+  float* G = Gb + (long long)blockIdx.y * r * r;
+  float* X = Xb + (long long)blockIdx.y * r * r;
+  float* P = Pb + (long long)blockIdx.y * r * r;
+  const int t = threadIdx.x, q = p + NB, nt = q < r ? (r - q + TS - 1) / TS : 0;
+  if ((int)blockIdx.x == nt * (nt + 1) / 2) {                 // the inverse CTA
+    if (t < 32) {
+      const int nb = min(NB, r - p);
+      for (int a = 0; a < NB; ++a) Di[a][t] = (a < nb && t < nb) ? G[(long long)(p + a) * r + p + t] : (a == t ? 1.f : 0.f);
+      __syncwarp();
+      diag_invert(Di, nb, X + (long long)p * r + p, r, t);
+    }
+    return;
+  }
+  int rem = blockIdx.x, tm = 0;
+  while (rem >= nt - tm) { rem -= nt - tm; ++tm; }
+  const int tn = tm + rem, m0 = q + tm * TS, n0 = q + tn * TS;
+  for (int i = t; i < NB * NB; i += 256) Di[i / NB][i % NB] = G[(long long)(p + i / NB) * r + p + i % NB];
+  // raw panel rows over the tile's row range (-> Pr) and column range (-> Pc)
+  for (int i = t; i < NB * TS / 4; i += 256) {
+    const int j = i / (TS / 4), c = (i % (TS / 4)) * 4;
+    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+    *reinterpret_cast<float4*>(&Pr[j][c]) = m0 + c < r ? *reinterpret_cast<const float4*>(G + (long long)(p + j) * r + m0 + c) : z;
+    *reinterpret_cast<float4*>(&Pc[j][c]) = n0 + c < r ? *reinterpret_cast<const float4*>(G + (long long)(p + j) * r + n0 + c) : z;
+  }
+  // this thread's part of the trailing tile, in flight during the solve
+  const int tx = t % 16, ty = t / 16;
+  float4 tv[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int m = m0 + ty * 4 + i, n = n0 + tx * 4;
+    tv[i] = (m < r && n < r) ? *reinterpret_cast<const float4*>(G + (long long)m * r + n) : make_float4(0.f, 0.f, 0.f, 0.f);
   }
   __syncthreads();
-  for (int idx = tid; idx < nb * nb; idx += blockDim.x) {
-    const int a = idx / nb, b = idx % nb;
-    G[(long long)(p + a) * r + p + b] = (b >= a) ? D[a][b] : 0.f;
-  }
-  const int ncols = r - p - nb;
-  if (ncols <= 0) return;
-  // zero the block below the panel rows (strict lower part of R)
-  for (int idx = tid; idx < ncols * nb; idx += blockDim.x) {
-    const int i = idx / nb, b = idx % nb;
-    G[(long long)(p + nb + i) * r + p + b] = 0.f;
-  }
-  // panel: solve D^T x = G[p..p+nb, c]
-  for (int c = tid; c < ncols; c += blockDim.x) {
+  if (t < NB) rd[t] = 1.f / Di[t][t];
+  __syncthreads();
+  if (t < 2 * TS) {   // forward substitution D^T x = g, in place: thread = one column of Pr (t < 64) or Pc
+    float (*Pm)[TS + PAD] = t < TS ? Pr : Pc;
+    const int c = t % TS;
     float x[NB];
 #pragma unroll
     for (int j = 0; j < NB; ++j) {
-      float s = j < nb ? G[(long long)(p + j) * r + p + nb + c] : 0.f;
+      float sacc = Pm[j][c];
 #pragma unroll
-      for (int k = 0; k < j; ++k) s = fmaf(-D[k][j], x[k], s);
-      x[j] = j < nb ? s / D[j][j] : 0.f;
+      for (int k = 0; k < j; ++k) sacc = fmaf(-Di[k][j], x[k], sacc);
+      x[j] = sacc * rd[j];
     }
 #pragma unroll
-    for (int j = 0; j < NB; ++j)
-      if (j < nb) G[(long long)(p + j) * r + p + nb + c] = x[j];
+    for (int j = 0; j < NB; ++j) Pm[j][c] = x[j];
+    if (t >= TS && tm == tn && n0 + c < r) {
+#pragma unroll
+      for (int j = 0; j < NB; ++j) P[(long long)(p + j) * r + n0 + c] = x[j];
+    }
+  }
+  __syncthreads();
+  float acc[4][4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
+#pragma unroll 8
+  for (int k = 0; k < NB; ++k) {
+    const float4 a = *reinterpret_cast<const float4*>(&Pr[k][ty * 4]);
+    const float4 b = *reinterpret_cast<const float4*>(&Pc[k][tx * 4]);
+    const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(av[i], bv[j], acc[i][j]);
+  }
+  const bool lead = tm == 0 && tn == 0;
+  float (*Dn)[NB + 1] = Di;                       // the next diagonal block reuses Di (every thread is past the solve)
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int m = m0 + ty * 4 + i, n = n0 + tx * 4;
+    if (m >= r || n >= r) continue;
+    float4 v = tv[i];
+    v.x -= acc[i][0]; v.y -= acc[i][1]; v.z -= acc[i][2]; v.w -= acc[i][3];
+    *reinterpret_cast<float4*>(G + (long long)m * r + n) = v;
+    if (lead && ty * 4 + i < NB && tx * 4 < NB) {
+      Dn[ty * 4 + i][tx * 4] = v.x; Dn[ty * 4 + i][tx * 4 + 1] = v.y; Dn[ty * 4 + i][tx * 4 + 2] = v.z; Dn[ty * 4 + i][tx * 4 + 3] = v.w;
+    }
+  }
+  if (lead) {
+    __syncthreads();
+    if (t < 32) diag_factor(Dn, min(NB, r - q), G + (long long)q * r + q, r, t);
+  }
+}
+
+// One half of a level of the blocked triangular inverse: block size b, pair j covers [o, o+2b), o = 2 b j.
+//   phase 0:  T12 = R12 X22      phase 1:  X12 = -X11 T12       (all [r,r] row-major, pitch r)
+// grid = (64x64 tiles of a [b,b] block, pairs, batch)
+__global__ void __launch_bounds__(256) k_tri_level(const float* __restrict__ Rb, float* __restrict__ Xb, float* __restrict__ Tb,
+                                                   int r, int b, int phase) {
+  constexpr int TS = 64, KS = 16, PAD = 4;
+  __shared__ __align__(16) float As[KS][TS + PAD], Bs[KS][TS + PAD];
+  const long long off = (long long)blockIdx.z * r * r;
+  const int o = 2 * b * blockIdx.y, o2 = o + b;
+  const int M = b, N = min(b, r - o2), K = phase == 0 ? N : M;
+  const int tiles_n = (b + TS - 1) / TS;
+  const int m0 = (blockIdx.x / tiles_n) * TS, n0 = (blockIdx.x % tiles_n) * TS;
+  if (n0 >= N) return;
+  const float* A = (phase == 0 ? Rb + off + (long long)o * r + o2 : Xb + off + (long long)o * r + o);
+  const float* B = (phase == 0 ? Xb + off + (long long)o2 * r + o2 : Tb + off + (long long)o * r + o2);
+  float* C = (phase == 0 ? Tb : Xb) + off + (long long)o * r + o2;
+  const int t = threadIdx.x, tx = t % 16, ty = t / 16;
+  float acc[4][4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
+  const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int k0 = 0; k0 < K; k0 += KS) {
+    {   // A tile [TS][KS]: row m, 4 consecutive k (stored transposed);  B tile [KS][TS]: row k, 4 consecutive n
+      const int m = m0 + t / (KS / 4), k = k0 + (t % (KS / 4)) * 4;
+      const float4 a = (m < M && k < K) ? *reinterpret_cast<const float4*>(A + (long long)m * r + k) : z;
+      const int ml = t / (KS / 4), kl = (t % (KS / 4)) * 4;
+      As[kl][ml] = a.x; As[kl + 1][ml] = a.y; As[kl + 2][ml] = a.z; As[kl + 3][ml] = a.w;
+      const int kb = k0 + t / (TS / 4), n = n0 + (t % (TS / 4)) * 4;
+      *reinterpret_cast<float4*>(&Bs[t / (TS / 4)][(t % (TS / 4)) * 4]) =
+          (kb < K && n < N) ? *reinterpret_cast<const float4*>(B + (long long)kb * r + n) : z;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < KS; ++k) {
+      const float4 a = *reinterpret_cast<const float4*>(&As[k][ty * 4]);
+      const float4 bb = *reinterpret_cast<const float4*>(&Bs[k][tx * 4]);
+      const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {bb.x, bb.y, bb.z, bb.w};
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(av[i], bv[j], acc[i][j]);
+    }
+    __syncthreads();
+  }
+  const float sgn = phase == 0 ? 1.f : -1.f;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int m = m0 + ty * 4 + i, n = n0 + tx * 4;
+    if (m >= M || n >= N) continue;
+    *reinterpret_cast<float4*>(C + (long long)m * r + n) = make_float4(sgn * acc[i][0], sgn * acc[i][1], sgn * acc[i][2], sgn * acc[i][3]);
   }
 }
 
@@ -309,59 +458,31 @@ int right_mul(const float* X, const float* M, float* C, const float* E, float be
   return MAPL_OK;
 }
 
-// In-place upper Cholesky of `batch` SPD [r,r] matrices (upper triangle read; strict lower part zeroed):
-// per 32-column panel one single-CTA panel kernel and one multi-CTA trailing update.
-int chol_upper(float* G, int r, int batch, cudaStream_t st) {
-  for (int p = 0; p < r; p += NB) {
-    const int nb = r - p < NB ? r - p : NB;
-    {
-      KernelScope ks(KID_ST_CHOL, st);
-      k_chol_panel<<<batch, 256, 0, st>>>(G, r, p);      // 256 threads: the register-resident block needs > 64 registers
+// Upper Cholesky G = R^T R of `batch` SPD [r,r] matrices (upper triangle read) and Xinv = R^-1.
+// Launches: 1 + r/NB for the factorisation (k_chol_first, k_chol_step per panel), then per doubling level b = NB,
+// 2 NB, ... two block products (R^-1 of [[R11, R12], [0, R22]] is [[X11, -X11 R12 X22], [0, X22]]): ~r^3/3 flops
+// in 2 log2(r/NB) launches.  Rp receives the off-diagonal part of R, T is scratch (all [batch][r][r]).
+int chol_inverse_blocked(float* G, float* Xinv, float* Rp, float* T, int r, int batch, cudaStream_t st) {
+  { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(Xinv, 0, (size_t)batch * r * r * 4, st)); }
+  {
+    KernelScope ks(KID_ST_CHOL, st);
+    k_chol_first<<<batch, 32, 0, st>>>(G, r);
+    MAPL_CUDA_CHECK(cudaGetLastError());
+  }
+  for (int p = 0; p < r; p += NB) {        // the last launch has no trailing block: only the inverse CTA
+    const int nt = p + NB < r ? (r - p - NB + 63) / 64 : 0;
+    KernelScope ks(KID_ST_CHOL, st);
+    k_chol_step<<<dim3(nt * (nt + 1) / 2 + 1, batch), 256, 0, st>>>(G, Xinv, Rp, r, p);
+    MAPL_CUDA_CHECK(cudaGetLastError());
+  }
+  for (int b = NB; b < r; b *= 2) {
+    const int pairs = (r - b + 2 * b - 1) / (2 * b), tiles = ((b + 63) / 64) * ((b + 63) / 64);
+    for (int phase = 0; phase < 2; ++phase) {
+      KernelScope ks(KID_ST_TRI_INV, st);
+      k_tri_level<<<dim3(tiles, pairs, batch), 256, 0, st>>>(Rp, Xinv, T, r, b, phase);
       MAPL_CUDA_CHECK(cudaGetLastError());
     }
-    const int ncols = r - p - nb;
-    if (ncols <= 0) break;
-    const int nt = (ncols + TN - 1) / TN;
-    const float* P = G + (long long)p * r + p + nb;                 // panel rows [nb, ncols], pitch r
-    float* T = G + (long long)(p + nb) * r + p + nb;                // trailing block, pitch r
-    KernelScope ks(KID_ST_GEMM, st);
-    k_st_gemm<true><<<dim3(nt * (nt + 1) / 2, 1, batch), 256, 0, st>>>(P, P, T, nullptr, -1.f, 0.f, ncols, ncols, nb, nb,
-                                                                      (long long)r * r, (long long)r * r, (long long)r * r, 1, r, r, r);
-    MAPL_CUDA_CHECK(cudaGetLastError());
   }
-  return MAPL_OK;
-}
-
-// X0 = diag(R)^-1 (batched [r,r])
-__global__ void k_diag_inverse(const float* __restrict__ R, float* __restrict__ X, int r) {
-  const long long off = (long long)blockIdx.y * r * r;
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= r * r) return;
-  const int a = idx / r, b = idx % r;
-  X[off + idx] = a == b ? 1.f / R[off + (long long)a * r + a] : 0.f;
-}
-
-// Xinv = R^-1 for upper-triangular R by Newton's iteration X <- X (2I - R X) from X0 = diag(R)^-1.
-// I - R X0 is strictly upper triangular, hence nilpotent: the error after k steps is its 2^k-th power,
-// which is exactly zero once 2^k >= r.  ceil(log2 r) iterations of two [r,r,r] GEMMs replace a
-// column-serial back substitution; every iterate stays upper triangular.
-// Result in *out (one of Xa, Xb); T is [r,r] scratch.
-int tri_inverse_newton(const float* R, float* Xa, float* Xb, float* T, float** out, int r, int batch, cudaStream_t st) {
-  {
-    KernelScope ks(KID_ST_TRI_INV, st);
-    k_diag_inverse<<<dim3((r * r + 255) / 256, batch), 256, 0, st>>>(R, Xa, r);
-    MAPL_CUDA_CHECK(cudaGetLastError());
-  }
-  int iters = 0;
-  while ((1 << iters) < r) ++iters;
-  float* cur = Xa;
-  float* nxt = Xb;
-  for (int it = 0; it < iters; ++it) {
-    MAPL_RETURN_IF(right_mul(R, cur, T, nullptr, 0.f, r, r, batch, st));            // T = R X
-    MAPL_RETURN_IF(right_mul(cur, T, nxt, cur, 2.f, r, r, batch, st, -1.f));        // X' = 2 X - X T
-    float* t = cur; cur = nxt; nxt = t;
-  }
-  *out = cur;
   return MAPL_OK;
 }
 
@@ -511,10 +632,10 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
   float* X1 = reinterpret_cast<float*>(ws + w.X1);
   const dim3 egrid((r * r + 255) / 256, batch);
 
-  // ---- tensor-core path (Newton-Schulz retraction, d and r multiples of 128, r >= 256): every GEMM of the step
-  // as six bf16-plane MMAs (tc_stiefel.cu); MAPL_ST_TC=0 forces the FFMA kernels (debugging aid)
+  // ---- tensor-core path (d and r multiples of 128, r >= 256): every [d,r]-sized GEMM of the step as six bf16-plane
+  // MMAs (tc_stiefel.cu); MAPL_ST_TC=0 forces the FFMA kernels (debugging aid)
   static const bool tc_enabled = !(getenv("MAPL_ST_TC") && getenv("MAPL_ST_TC")[0] == '0');
-  if (retraction == MAPL_RETRACT_NS && tc_st_ok(d, r) && tc_enabled) {
+  if (tc_st_ok(d, r) && tc_enabled) {
     __nv_bfloat16* Prow = reinterpret_cast<__nv_bfloat16*>(ws + w.Prow);   // [b][3][d][r]
     __nv_bfloat16* Ptr = reinterpret_cast<__nv_bfloat16*>(ws + w.Ptr);     // [b][3][r][d]
     __nv_bfloat16* Ptr2 = reinterpret_cast<__nv_bfloat16*>(ws + w.Ptr2);   // [b][3][r][d]
@@ -537,9 +658,21 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
       k_fro_norm<<<batch, 1024, 0, st>>>(U, X0, lr != 0.f ? 1.f / lr : 0.f, (long long)d * r, 0, info_out, 0);
       MAPL_CUDA_CHECK(cudaGetLastError());
     }
+    if (retraction == MAPL_RETRACT_QR) {     // CholeskyQR2 (see the FFMA path below); Gram and X R^-1 on the tensor cores
+      const float* src = X0;
+      for (int pass = 0; pass < 2; ++pass) {
+        MAPL_RETURN_IF(tc_st_split(src, d, r, batch, 0, 0.f, Prow, Ptr, st, S, (long long)r * r));   // also clears S
+        MAPL_RETURN_IF(tc_st_gemm3(Ptr, Ptr, r, r, d, batch, S, nullptr, 0.f, ksplit, st));           // X^T X
+        MAPL_RETURN_IF(chol_inverse_blocked(S, Rinv, M, Rinv2, r, batch, st));
+        MAPL_RETURN_IF(tc_st_split(Rinv, r, r, batch, 0, 0.f, nullptr, Pm, st));                      // planes of (R^-1)^T
+        float* out = pass == 0 ? X1 : U;
+        MAPL_RETURN_IF(tc_st_gemm3(Prow, Pm, d, r, r, batch, out, nullptr, 0.f, 1, st));
+        src = out;
+      }
+    }
     float* cur = X0;
     float* nxt = X1;
-    for (int it = 0; it < ns_iters; ++it) {
+    for (int it = 0; it < (retraction == MAPL_RETRACT_NS ? ns_iters : 0); ++it) {
       MAPL_RETURN_IF(tc_st_split(cur, d, r, batch, 0, 0.f, Prow, Ptr, st, S, (long long)r * r));   // also clears S
       MAPL_RETURN_IF(tc_st_gemm3(Ptr, Ptr, r, r, d, batch, S, nullptr, 0.f, ksplit, st));   // X^T X
       MAPL_RETURN_IF(tc_st_split(S, r, r, batch, 1, 0.f, Pm, nullptr, st));                 // (3I - X^T X)/2, symmetric
@@ -582,10 +715,9 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
     // CholeskyQR2: Y = Q1 R1, Q1 = Q R2  =>  Y = Q (R2 R1), upper triangular with positive diagonal
     const float* src = X0;
     for (int pass = 0; pass < 2; ++pass) {
-      MAPL_RETURN_IF(gram(src, src, S, d, r, batch, st, true));   // chol_upper reads the upper triangle only
-      MAPL_RETURN_IF(chol_upper(S, r, batch, st));
-      float* Xinv = nullptr;
-      MAPL_RETURN_IF(tri_inverse_newton(S, Rinv, Rinv2, M, &Xinv, r, batch, st));
+      MAPL_RETURN_IF(gram(src, src, S, d, r, batch, st, true));   // the factorisation reads the upper triangle only
+      MAPL_RETURN_IF(chol_inverse_blocked(S, Rinv, M, Rinv2, r, batch, st));
+      float* Xinv = Rinv;
       float* out = pass == 0 ? X1 : U;
       MAPL_RETURN_IF(right_mul(src, Xinv, out, nullptr, 0.f, d, r, batch, st));
       src = out;
