@@ -177,10 +177,11 @@ int mapl_center_backward(const mapl_boundary_desc* desc, const void* gz, const i
  *   MAPL_RETRACT_NS: X_0 = Y, X_{j+1} = X_j (3I - X_j^T X_j)/2, U <- X_{ns_iters} (S11; the
  *                    reported configuration is ns_iters = 5; 1 <= ns_iters <= 16).
  *   U_inout is updated in place.  fp32 storage, fp32-accurate arithmetic: ||U^T U - I||_F <= 1e-5
- *   after the call for inputs in the documented regime.  (NS with d % 128 == 0, r % 128 == 0,
- *   r >= 256: the products run on the tensor cores as exact three-plane bf16 splits, six MMAs per
- *   product; otherwise fp32 FFMA kernels.  QR: CholeskyQR2 in fp32; it needs cond(Y) well below
- *   1e3, which holds for a step from an orthonormal U.)
+ *   after the call for inputs in the documented regime.  (With d % 128 == 0, r % 128 == 0,
+ *   r >= 256 the [d,r]-sized products run on the tensor cores as exact three-plane bf16 splits,
+ *   six MMAs per product; otherwise fp32 FFMA kernels.  QR: CholeskyQR2 in fp32 -- blocked
+ *   Cholesky of the Gram matrix and a blocked triangular inverse, twice; it needs cond(Y) well
+ *   below 1e3, which holds for a step from an orthonormal U.)
  *   info_out   optional device [batch,2] fp32: ||xi||_F and ||U^T U - I||_F after the update.
  * Requires 8 <= r <= d, r % 8 == 0, d % 8 == 0, r <= 1024.                                      */
 int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U_inout, const float* G, float lr,

@@ -1,8 +1,9 @@
 // stiefel.cu -- mapl_stiefel_step: tangent projection (Eq. 4), step, and retraction
 // onto St(d,r) by thin QR (CholeskyQR2, diag(R) > 0) or by a fixed number of cubic Newton-Schulz
-// polar iterations (count passed in; 5 in every reported number).  fp32 storage and fp32 FFMA
+// polar iterations (count passed in; 5 in every reported number).  fp32 storage and fp32-accurate
 // arithmetic throughout: tcgen05 has no fp32 kind and a single TF32 pass cannot hold
-// ||U^T U - I||_F <= 1e-5.
+// ||U^T U - I||_F <= 1e-5, so the products are fp32 FFMA kernels here or,
+// for d, r multiples of 128 and r >= 256, exact three-plane bf16 splits on the tensor cores (tc_stiefel.cu).
 //
 //   Y = U - lr (G - U sym(U^T G)) = U (I + lr sym(S)) - lr G,   S = U^T G
 #include "common.cuh"
