@@ -325,6 +325,9 @@ def run_mapl(args):
             "mapl_decode": graph_us(lambda b: mb.mapl_decode(b.desc, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.Hhat, b.ws)),
             "mapl_codec_backward": graph_us(lambda b: mb.mapl_codec_backward(
                 b.desc, b.g, b.H, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.gz, b.dU, b.dA, None, b.dH, False, b.ws)),
+            # the receiver's share alone (H == NULL: gz, dA and the decode-side term of dU; no dH), reported beside the headline
+            "mapl_codec_backward_decode_side": graph_us(lambda b: mb.mapl_codec_backward(
+                b.desc, b.g, None, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.gz, b.dU, b.dA, None, None, False, b.ws)),
         }
 
         # ---- per-kernel timing pass (same K steps, eager launches, event pair around every kernel)
@@ -420,7 +423,7 @@ def run_mapl(args):
         "roofline": roof,
     }
     if rank == 0 and world == 1 and not args.no_stiefel:
-        out["stiefel"] = stiefel_sweep(torch, mb, I, stream)
+        out["stiefel"] = stiefel_sweep(torch, mb, I, stream, track_steps=args.track_steps)
     if rank == 0 and world == 1 and not args.no_stiefel:
         out["centering"] = centering_times(torch, mb, bs[0], cfg, stream)
     if rank == 0:
@@ -431,10 +434,48 @@ def run_mapl(args):
         dist.destroy_process_group()
 
 
-def stiefel_sweep(torch, mb, I, stream, reps=10):
+def _stiefel_track(torch, mb, s, r, retr, ws, stream, n_steps):
+    """configs[4]: `n_steps` consecutive steps with ||U^T U - I||_F tracked -- on the device by the library every step
+    (info_out, fp32 Gram: its maximum over the run) and in fp64 (torch) at steps 1, 2, 10, 100, 500, 1000 -- for the
+    fixed seeded gradient and for a fresh Gaussian gradient every step (reading S13; drawn by torch's seeded device
+    generator: an input, not part of the method).  Maximum over the 3 projectors."""
+    marks = [m for m in (1, 2, 10, 100, 500, 1000) if m <= n_steps]
+    eye = torch.eye(r, device="cuda", dtype=torch.float64)
+    res = {}
+    for variant in ("fixed_G", "fresh_G"):
+        U = torch.from_numpy(s.U.data.copy()).cuda()
+        G = torch.from_numpy(s.G.data.copy()).cuda()
+        info = torch.zeros(s.batch, 2, device="cuda", dtype=torch.float32)
+        log = torch.zeros(n_steps, device="cuda", dtype=torch.float32)
+        gen = torch.Generator(device="cuda")
+        gen.manual_seed(260605484 + r)
+        mb.mapl_stiefel_step(U, G, 1e-2, retr, 5, info, ws)
+        stream.synchronize()
+        U.copy_(torch.from_numpy(s.U.data.copy()))
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=stream):
+            mb.mapl_stiefel_step(U, G, 1e-2, retr, 5, info, ws)
+        U.copy_(torch.from_numpy(s.U.data.copy()))
+        at = {}
+        for t in range(1, n_steps + 1):
+            if variant == "fresh_G":
+                G.normal_(generator=gen)
+            g.replay()
+            log[t - 1] = info[:, 1].max()
+            if t in marks:
+                Uh = U.double()
+                at[str(t)] = float(f"{float(max(torch.linalg.matrix_norm(Uh[b].T @ Uh[b] - eye) for b in range(s.batch))):.2e}")
+        stream.synchronize()
+        res[variant] = {"residual_fp64_at_step": at, "max_device_residual": float(f"{float(log.max()):.2e}"), "steps": n_steps}
+    return res
+
+
+def stiefel_sweep(torch, mb, I, stream, reps=10, track_steps=1000):
     """BASELINE.json configs[4] beside the codec metric: Stiefel steps/s for the 3 projectors of d=2048,
     r in {64,128,256,512}, QR (CholeskyQR2) and 5 Newton-Schulz iterations; one CUDA graph per variant.
-    A step = one mapl_stiefel_step call over the batch of 3; projector-steps/s = 3 x that."""
+    A step = one mapl_stiefel_step call over the batch of 3; projector-steps/s = 3 x that.
+    `track`: the variant repeated for track_steps steps from the seeded start, with the orthogonality residual
+    tracked (see _stiefel_track)."""
     out = {}
     with torch.cuda.stream(stream):
         for r in (64, 128, 256, 512):
@@ -462,6 +503,8 @@ def stiefel_sweep(torch, mb, I, stream, reps=10):
                                 for b in range(s.batch)))
                 out[f"r{r}_{tag}"] = {"us_per_step": round(us, 1), "projector_steps_per_s": round(s.batch * 1e6 / us),
                                       "orth_residual_after": float(f"{res:.2e}")}
+                if track_steps:
+                    out[f"r{r}_{tag}"]["track"] = _stiefel_track(torch, mb, s, r, retr, ws, stream, track_steps)
     # full SPEL update (Eq. 4-7: tangent projection, momentum 0.95, 5 + 7 Newton-Schulz iterations), SURVEY 8f next row 2
     with torch.cuda.stream(stream):
         for r in (64, 128, 256, 512):
@@ -489,7 +532,9 @@ def stiefel_sweep(torch, mb, I, stream, reps=10):
                             for b in range(s.batch)))
             out[f"r{r}_spel"] = {"us_per_step": round(us, 1), "projector_steps_per_s": round(s.batch * 1e6 / us),
                                  "orth_residual_after": float(f"{res:.2e}")}
-    out["config"] = "d=2048, 3 projectors per call, fixed G, lr=1e-2, fp32"
+    out["config"] = ("d=2048, 3 projectors per call, fixed G, lr=1e-2, fp32; track: 1000 consecutive steps per variant, "
+                     "residual in fp64 at the listed steps and max over all steps of the library's own per-step check "
+                     "(info_out: an fp32 Gram of U, whose rounding floor is ~2e-8 r -- it reads high at r = 512)")
     return out
 
 
@@ -584,10 +629,14 @@ def roofline_step(cfg, peaks, ms_per_step, nb, calls_us):
     t = {}
     for call in ("encode", "decode", "backward"):
         t[call] = 1e6 * max(ab[call] * N / (peaks["hbm"] * 1e9), af[call] * N / (peaks["bf16"] * 1e12))
-    codec_us = sum(calls_us.values())
+    codec_us = sum(calls_us[k] for k in ("mapl_encode", "mapl_decode", "mapl_codec_backward"))
+    # the same sum against the vendor's nominal peaks (8 TB/s HBM3e, 2.25 PFLOP/s dense bf16): context, SURVEY 8(d)
+    t_nom = sum(1e6 * max(ab[c] * N / 8000e9, af[c] * N / 2250e12) for c in ("encode", "decode", "backward"))
     return {"t_roof_us_per_boundary": round(sum(t.values()), 2), "per_call_us": {k: round(v, 2) for k, v in t.items()},
             "measured_us_per_boundary": round(codec_us, 2), "frac": round(sum(t.values()) / codec_us, 3),
-            "peaks": {"hbm_gbs": peaks["hbm"], "bf16_tflops": peaks["bf16"], "source": peaks["src"]}}
+            "peaks": {"hbm_gbs": peaks["hbm"], "bf16_tflops": peaks["bf16"], "source": peaks["src"]},
+            "nominal": {"t_roof_us_per_boundary": round(t_nom, 2), "frac": round(t_nom / codec_us, 3),
+                        "hbm_gbs": 8000, "bf16_tflops": 2250}}
 
 
 def roofline_for(name, k, cfg, peaks, total_ms):
@@ -710,6 +759,8 @@ def main():
     ap.add_argument("--tokens", type=int, default=0, help="override tokens per boundary (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stiefel", action="store_true", help="skip the configs[4] Stiefel-step sweep")
+    ap.add_argument("--track-steps", type=int, default=1000,
+                    help="configs[4]: consecutive Stiefel steps per variant with the orthogonality residual tracked (0 = off)")
     ap.add_argument("--cpu-budget", type=float, default=20.0)
     args = ap.parse_args()
     if args.impl == "reference":
