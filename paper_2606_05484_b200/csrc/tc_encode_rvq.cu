@@ -29,7 +29,15 @@ namespace mapl {
 namespace {
 using namespace tc;
 
-constexpr int kThreads = kPipeThreads;   // warp 0 TMA, warp 1 MMA, warps 2-9 scan / re-score (two per TMEM lane quarter)
+// scan / re-score threads per token (warps per TMEM lane quarter): 2 or 4.  Measured: 4 (16 scan warps, 96 registers)
+// is SLOWER -- c2 encode 59.7 -> 62.2 us, c3 239 -> 271 us: the per-warp cost of a chunk (TMEM load, wait, barrier
+// arrive, list bookkeeping) does not shrink with the piece count and the 512-thread exchanges cost more.
+#ifndef MAPL_RVQ_PARTS
+#define MAPL_RVQ_PARTS 2
+#endif
+constexpr int kParts = MAPL_RVQ_PARTS;
+constexpr int kEpi = 128 * kParts;       // epilogue threads
+constexpr int kThreads = 64 + kEpi;      // warp 0 TMA, warp 1 MMA, then kParts x 4 scan / re-score warps
 constexpr int kChunk = 128;        // codewords per accumulator stage (UMMA N)
 constexpr int kAccCol0 = 256;      // TMEM column of score stage 0
 constexpr int kNE = 8;             // candidate-list entries per thread (one entry = one 32-codeword piece)
@@ -49,11 +57,11 @@ struct RvqParams {
 
 // smem carve-up (after 1024-byte alignment):
 //   region R  = max(phase-1 ring, rho operand tiles + codebook ring)
-//   sHn [K] fp32 | candidate lists [kNE][256] x (m32, piece, mask) | exchange [5][2][128] | barriers | tmem slot
+//   sHn [K] fp32 | candidate lists [kNE][kEpi] x (m32, piece, mask) | exchange [5][kParts][128] | barriers | tmem slot
 struct Smem {
   uint8_t* ring1; uint8_t* sRho; uint8_t* ringC;
   float* sHn; float* eM; int* eP; uint32_t* eMask;
-  float* xch;            // [5][2][128]: per (half, token) best / score / k / n2 / amax exchanged by the two warps of a quarter
+  float* xch;            // [5][kParts][128]: per (part, token) best / score / k / n2 / amax exchanged by the warps of a quarter
   uint64_t* s1_full; uint64_t* s1_empty; uint64_t* z_full;
   uint64_t* c_full; uint64_t* c_empty; uint64_t* acc_full; uint64_t* acc_empty; uint64_t* rho_ready;
   uint32_t* tmem_slot;
@@ -65,7 +73,7 @@ __host__ __device__ inline size_t rvq_regionR(const RvqParams& p) {
   return ring1 > lvl ? ring1 : lvl;
 }
 __host__ __device__ inline size_t rvq_tail_bytes(const RvqParams& p) {
-  return (size_t)p.K * 4 + (size_t)kNE * 256 * 12 + 5 * 2 * 128 * 4 + 1024;
+  return (size_t)p.K * 4 + (size_t)kNE * kEpi * 12 + 5 * kEpi * 4 + 1024;
 }
 
 __device__ __forceinline__ Smem carve_smem(uint8_t* base, const RvqParams& p) {
@@ -75,10 +83,10 @@ __device__ __forceinline__ Smem carve_smem(uint8_t* base, const RvqParams& p) {
   s.ringC = base + (size_t)(p.r / 64) * kTileBytes;
   uint8_t* t = base + rvq_regionR(p);
   s.sHn = reinterpret_cast<float*>(t); t += (size_t)p.K * 4;
-  s.eM = reinterpret_cast<float*>(t); t += kNE * 256 * 4;
-  s.eP = reinterpret_cast<int*>(t); t += kNE * 256 * 4;
-  s.eMask = reinterpret_cast<uint32_t*>(t); t += kNE * 256 * 4;
-  s.xch = reinterpret_cast<float*>(t); t += 5 * 2 * 128 * 4;
+  s.eM = reinterpret_cast<float*>(t); t += kNE * kEpi * 4;
+  s.eP = reinterpret_cast<int*>(t); t += kNE * kEpi * 4;
+  s.eMask = reinterpret_cast<uint32_t*>(t); t += kNE * kEpi * 4;
+  s.xch = reinterpret_cast<float*>(t); t += 5 * kEpi * 4;
   uint64_t* b = reinterpret_cast<uint64_t*>(t);
   s.s1_full = b; b += p.stages1;
   s.s1_empty = b; b += p.stages1;
@@ -116,14 +124,14 @@ __device__ __forceinline__ float exact_score(uint32_t tmem_row, const float* __r
   return hn - dot;
 }
 
-// The two warps of a TMEM lane quarter split the residual by 32-column pieces: warp half h owns the
-// pieces pc with (pc & 1) == h.
+// The kParts warps of a TMEM lane quarter split the residual by 32-column pieces: part h owns the
+// pieces pc with pc % kParts == h.
 // Step 1 of a residual update: rho <- rho - sub on the own pieces (sub == nullptr: rho unchanged);
 // returns the partial ||rho||^2 and max|rho_j| of those pieces.  Warp-convergent.
 __device__ __forceinline__ void rho_subtract(uint32_t tmem_row, const float* __restrict__ sub, int r, int h, float* n2_out,
                                              float* amax_out) {
   float n2 = 0.f, amax = 0.f;
-  for (int pc = h; pc < r / 32; pc += 2) {
+  for (int pc = h; pc < r / 32; pc += kParts) {
     uint32_t v[32];
     tmem_ld32(tmem_row + pc * 32, v);
     tmem_ld_wait();
@@ -156,7 +164,7 @@ __device__ __forceinline__ float rho_to_operand(uint32_t tmem_row, uint8_t* sRho
   int eb = (int)((__float_as_uint(amax) >> 23) & 0xffu);
   eb = eb < 2 ? 126 : (eb > 250 ? 250 : eb);
   const float inv = __uint_as_float((uint32_t)(253 - eb) << 23);
-  for (int pc = h; pc < r / 32; pc += 2) {
+  for (int pc = h; pc < r / 32; pc += kParts) {
     uint32_t v[32];
     tmem_ld32(tmem_row + pc * 32, v);
     tmem_ld_wait();
@@ -173,6 +181,9 @@ __device__ __forceinline__ float rho_to_operand(uint32_t tmem_row, uint8_t* sRho
   }
   return __uint_as_float((uint32_t)(eb + 1) << 23);
 }
+
+// named barrier 1 over the epilogue warps
+__device__ __forceinline__ void epi_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kEpi) : "memory"); }
 
 __global__ void __launch_bounds__(kThreads, 1)
 k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmWhi,
@@ -192,8 +203,8 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
     for (int i = 0; i < p.stages1; ++i) { mbar_init(&s.s1_full[i], 1); mbar_init(&s.s1_empty[i], 1); }
     mbar_init(s.z_full, 1);
     for (int i = 0; i < p.ring_tiles; ++i) { mbar_init(&s.c_full[i], 1); mbar_init(&s.c_empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&s.acc_full[i], 1); mbar_init(&s.acc_empty[i], 16); }
-    mbar_init(s.rho_ready, 16);               // leader's barriers collect the epilogue warps of both CTAs
+    for (int i = 0; i < 2; ++i) { mbar_init(&s.acc_full[i], 1); mbar_init(&s.acc_empty[i], 8 * kParts); }
+    mbar_init(s.rho_ready, 8 * kParts);               // leader's barriers collect the epilogue warps of both CTAs
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc_pair<512>(s.tmem_slot);
@@ -280,17 +291,17 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       }
     }
   } else {
-    // ------------------------------------------------------------ epilogue: 8 warps, two threads per token
-    // q = TMEM lane quarter, h = which half of the 32-codeword pieces / 32-column pieces this warp owns
+    // ------------------------------------------------------------ epilogue: 4 kParts warps, kParts threads per token
+    // q = TMEM lane quarter, h = which part of the 32-codeword pieces / 32-column pieces this warp owns
     const int q = warp & 3, h = (warp - 2) >> 2, row = q * 32 + lane, et = threadIdx.x - 64;
     const long long m = m0 + row;
     const bool live = row < p.tile_m && m < p.N;
     const uint32_t tmem_row = tmem_base + ((uint32_t)(q * 32) << 16);
     const unsigned full = 0xffffffffu;
-    float* xBest = s.xch; float* xScore = s.xch + 256; int* xK = reinterpret_cast<int*>(s.xch + 512);
-    float* xN2 = s.xch + 768; float* xAmax = s.xch + 1024;
-    const int mine = h * 128 + row, other = (1 - h) * 128 + row;
-    float* eM = s.eM + mine; int* eP = s.eP + mine; uint32_t* eMask = s.eMask + mine;   // entry e at [e * 256]
+    float* xBest = s.xch; float* xScore = s.xch + kEpi; int* xK = reinterpret_cast<int*>(s.xch + 2 * kEpi);
+    float* xN2 = s.xch + 3 * kEpi; float* xAmax = s.xch + 4 * kEpi;
+    const int mine = h * 128 + row;
+    float* eM = s.eM + mine; int* eP = s.eP + mine; uint32_t* eMask = s.eMask + mine;   // entry e at [e * kEpi]
     int code_l[8];
 #pragma unroll
     for (int l = 0; l < 8; ++l) code_l[l] = 0;
@@ -300,7 +311,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
     tc_fence_after_sync();
     float n2, amax;
     if (nkb1 >= 2) {                     // z = even-k-block half + odd-k-block half (see the MMA issuer)
-      for (int pc = h; pc < p.r / 32; pc += 2) {
+      for (int pc = h; pc < p.r / 32; pc += kParts) {
         uint32_t v[32], w[32];
         tmem_ld32(tmem_row + pc * 32, v);
         tmem_ld32(tmem_row + kAccCol0 + pc * 32, w);
@@ -315,8 +326,10 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
     const float* csub = p.Tc != nullptr ? p.Tc + (live ? (long long)__ldg(p.tok + m) * p.r : 0) : nullptr;
     rho_subtract(tmem_row, csub, p.r, h, &n2, &amax);
     xN2[mine] = n2; xAmax[mine] = amax;
-    asm volatile("bar.sync 1, 256;" ::: "memory");
-    n2 += xN2[other]; amax = fmaxf(amax, xAmax[other]);
+    epi_sync();
+    n2 = 0.f; amax = 0.f;
+#pragma unroll
+    for (int hh = 0; hh < kParts; ++hh) { n2 += xN2[hh * 128 + row]; amax = fmaxf(amax, xAmax[hh * 128 + row]); }
     float unscale = rho_to_operand(tmem_row, s.sRho, row, p.r, h, amax);
     fence_proxy_async_all();
     tc_fence_before_sync();
@@ -327,9 +340,9 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 #pragma unroll 1
     for (int l = 0; l < p.L; ++l) {
       const float* Cl = p.C + (long long)l * p.K * p.r;
-      for (int i = et; i < p.K / 4; i += 256)
+      for (int i = et; i < p.K / 4; i += kEpi)
         reinterpret_cast<float4*>(s.sHn)[i] = __ldg(reinterpret_cast<const float4*>(p.hn + (long long)l * p.K) + i);
-      asm volatile("bar.sync 1, 256;" ::: "memory");
+      epi_sync();
       if (warp == 2 && l < 4) { DBG(4 + l * 4) }
       const float margin = 0.001953125f * 1.05f * sqrtf(n2) * __ldg(p.cmax + l);
       const float nsc = -unscale * __ldg(p.cscale + 8 + l);     // coarse S -> rho.c
@@ -342,17 +355,17 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         mbar_wait(&s.acc_full[as], (cg >> 1) & 1);
         if (threadIdx.x == 64 && cg < 8) DBGT(40 + cg)
         tc_fence_after_sync();
-        uint32_t v[2][32];                     // this warp's two pieces of the chunk: h and h + 2
-        tmem_ld32(tmem_row + kAccCol0 + as * kChunk + h * 32, v[0]);
-        tmem_ld32(tmem_row + kAccCol0 + as * kChunk + (h + 2) * 32, v[1]);
+        uint32_t v[4 / kParts][32];            // this warp's pieces of the chunk: h, h + kParts, ...
+#pragma unroll
+        for (int pp = 0; pp < 4 / kParts; ++pp) tmem_ld32(tmem_row + kAccCol0 + as * kChunk + (h + kParts * pp) * 32, v[pp]);
         tmem_ld_wait();
         tc_fence_before_sync();
         __syncwarp();
         if (lane == 0) mbar_arrive_leader(&s.acc_empty[as]);     // scores are in registers: the stage is free
         if (threadIdx.x == 64 && cg < 8) DBGT(48 + cg)
 #pragma unroll
-        for (int pp = 0; pp < 2; ++pp) {
-          const int piece = c * (kChunk / 32) + h + 2 * pp;
+        for (int pp = 0; pp < 4 / kParts; ++pp) {
+          const int piece = c * (kChunk / 32) + h + kParts * pp;
           const float4* h4 = reinterpret_cast<const float4*>(s.sHn + piece * 32);
           float sc[32];
 #pragma unroll
@@ -377,23 +390,24 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
               if (cnt == kNE) {                 // list full: drop entries the tighter threshold excludes
                 int j = 0;
                 for (int e = 0; e < kNE; ++e) {
-                  const float em = eM[e * 256];
-                  if (em <= thr) { eM[j * 256] = em; eP[j * 256] = eP[e * 256]; eMask[j * 256] = eMask[e * 256]; ++j; }
+                  const float em = eM[e * kEpi];
+                  if (em <= thr) { eM[j * kEpi] = em; eP[j * kEpi] = eP[e * kEpi]; eMask[j * kEpi] = eMask[e * kEpi]; ++j; }
                 }
                 cnt = j;
               }
               if (cnt == kNE) {
                 overflow = true;                // pathological (e.g. many duplicate codewords): exhaustive below
               } else {
-                eM[cnt * 256] = m32; eP[cnt * 256] = piece; eMask[cnt * 256] = mask; ++cnt;
+                eM[cnt * kEpi] = m32; eP[cnt * kEpi] = piece; eMask[cnt * kEpi] = mask; ++cnt;
               }
             }
           }
         }
       }
       xBest[mine] = best;
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-      best = fminf(best, xBest[other]);
+      epi_sync();
+#pragma unroll
+      for (int hh = 0; hh < kParts; ++hh) best = fminf(best, xBest[hh * 128 + row]);
       if (warp == 2 && l < 4) { DBG(5 + l * 4) }
 
       // ---- exact fp32 re-scoring of this thread's candidates, ascending k, strict '<': lowest index wins ties
@@ -403,7 +417,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       uint32_t mrem = 0;
       while (true) {
         while (mrem == 0 && e < cnt) {
-          if (eM[e * 256] <= thr) { mrem = eMask[e * 256]; piece = eP[e * 256]; }
+          if (eM[e * kEpi] <= thr) { mrem = eMask[e * kEpi]; piece = eP[e * kEpi]; }
           ++e;
         }
         const bool have = mrem != 0 && !overflow;
@@ -414,7 +428,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         if (have && sx < bestx) { bestx = sx; bestk = k; }
       }
       if (__any_sync(full, overflow)) {         // exhaustive over the pieces this warp owns
-        for (int pc = h; pc < p.K / 32; pc += 2)
+        for (int pc = h; pc < p.K / 32; pc += kParts)
           for (int i = 0; i < 32; ++i) {
             const int k = pc * 32 + i;
             const float sx = exact_score(tmem_row, Cl + (long long)k * p.r, s.sHn[k], p.r);
@@ -422,10 +436,11 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
           }
       }
       xScore[mine] = bestx; xK[mine] = bestk;
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-      {
-        const float ox = xScore[other];
-        const int ok = xK[other];
+      epi_sync();
+#pragma unroll
+      for (int hh = 0; hh < kParts; ++hh) {
+        const float ox = xScore[hh * 128 + row];
+        const int ok = xK[hh * 128 + row];
         if (ox < bestx || (ox == bestx && ok < bestk)) { bestx = ox; bestk = ok; }
       }
       if (bestk == 0x7fffffff) bestk = 0;       // dead rows
@@ -436,8 +451,10 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       if (l + 1 < p.L) {
         rho_subtract(tmem_row, Cl + (long long)bestk * p.r, p.r, h, &n2, &amax);
         xN2[mine] = n2; xAmax[mine] = amax;
-        asm volatile("bar.sync 1, 256;" ::: "memory");
-        n2 += xN2[other]; amax = fmaxf(amax, xAmax[other]);
+        epi_sync();
+        n2 = 0.f; amax = 0.f;
+#pragma unroll
+        for (int hh = 0; hh < kParts; ++hh) { n2 += xN2[hh * 128 + row]; amax = fmaxf(amax, xAmax[hh * 128 + row]); }
         unscale = rho_to_operand(tmem_row, s.sRho, row, p.r, h, amax);
         fence_proxy_async_all();
         tc_fence_before_sync();
@@ -448,7 +465,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 
     if (warp == 2) { DBG(2) }
     if (p.Zq != nullptr && live) {                          // zhat = sum_l C[l, code_l, :], rounded once
-      for (int cc = h; cc < p.r / 8; cc += 2) {
+      for (int cc = h; cc < p.r / 8; cc += kParts) {
         float a[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
         for (int l = 0; l < 8; ++l) {

@@ -115,7 +115,7 @@ __device__ __forceinline__ void chunk_epilogue(const ChunkPipe& c, const CUtenso
     fence_proxy_async_smem();
     if (h == 0) asm volatile("bar.sync 1, 128;" ::: "memory"); else asm volatile("bar.sync 2, 128;" ::: "memory");
     if (issuer) {
-      tma_store_2d(tmO, box, j * kChunkN + h * 64, m0);
+      tma_store_2d_hint(tmO, box, j * kChunkN + h * 64, m0, kEvictFirst);     // Hhat / dH: not read again by the codec
       tma_store_commit();
     }
   }
