@@ -305,6 +305,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
     int code_l[8];
 #pragma unroll
     for (int l = 0; l < 8; ++l) code_l[l] = 0;
+    const uint32_t sHn_u32 = smem_u32(s.sHn);
 
     mbar_wait(s.z_full, 0);
     if (warp == 2) { DBG(1) }
@@ -366,26 +367,38 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 #pragma unroll
         for (int pp = 0; pp < 4 / kParts; ++pp) {
           const int piece = c * (kChunk / 32) + h + kParts * pp;
-          const float4* h4 = reinterpret_cast<const float4*>(s.sHn + piece * 32);
+          const uint32_t h4 = sHn_u32 + piece * 128;      // explicit ld.shared: the carved pointers compile to generic loads
           float sc[32];
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
-            const float4 hh = h4[i];
+            float4 hh;
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(hh.x), "=f"(hh.y), "=f"(hh.z), "=f"(hh.w) : "r"(h4 + 16 * i));
             sc[4 * i + 0] = fmaf(__uint_as_float(v[pp][4 * i + 0]), nsc, hh.x);
             sc[4 * i + 1] = fmaf(__uint_as_float(v[pp][4 * i + 1]), nsc, hh.y);
             sc[4 * i + 2] = fmaf(__uint_as_float(v[pp][4 * i + 2]), nsc, hh.z);
             sc[4 * i + 3] = fmaf(__uint_as_float(v[pp][4 * i + 3]), nsc, hh.w);
           }
-          float mn[8];
+          // The min / compare instructions run on the half-rate ALU pipe, which bounds this loop at r = 64: three-input
+          // minima, and the candidate mask from the sign bits of thr - sc (an FADD on the FMA pipe and one funnel
+          // shift per codeword instead of FSETP + SEL + OR).
+          float mn[4];
 #pragma unroll
-          for (int i = 0; i < 8; ++i) mn[i] = fminf(fminf(sc[4 * i], sc[4 * i + 1]), fminf(sc[4 * i + 2], sc[4 * i + 3]));
-          const float m32 = fminf(fminf(fminf(mn[0], mn[1]), fminf(mn[2], mn[3])), fminf(fminf(mn[4], mn[5]), fminf(mn[6], mn[7])));
+          for (int g = 0; g < 4; ++g) {
+            const float a = fminf(fminf(sc[8 * g], sc[8 * g + 1]), sc[8 * g + 2]);
+            const float b = fminf(fminf(sc[8 * g + 3], sc[8 * g + 4]), sc[8 * g + 5]);
+            mn[g] = fminf(fminf(a, b), fminf(sc[8 * g + 6], sc[8 * g + 7]));
+          }
+          const float m32 = fminf(fminf(mn[0], mn[1]), fminf(mn[2], mn[3]));
           best = fminf(best, m32);
           const float thr = best + margin;
           if (__any_sync(full, live && m32 <= thr)) {      // dead rows hold stale smem: never candidates
-            uint32_t mask = 0;
+            // bit i of mask <=> sc[i] <= thr <=> sign(thr - sc[i]) clear (thr - sc == +0 when equal)
+            uint32_t mk[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
-            for (int i = 0; i < 32; ++i) mask |= (sc[i] <= thr) ? (1u << i) : 0u;
+            for (int g = 0; g < 4; ++g)
+#pragma unroll
+              for (int i = 7; i >= 0; --i) mk[g] = __funnelshift_l(__float_as_uint(thr - sc[8 * g + i]), mk[g], 1);
+            const uint32_t mask = ~(mk[0] | (mk[1] << 8) | (mk[2] << 16) | (mk[3] << 24));
             if (live && mask != 0 && !overflow) {
               if (cnt == kNE) {                 // list full: drop entries the tighter threshold excludes
                 int j = 0;
