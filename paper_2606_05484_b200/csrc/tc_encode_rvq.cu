@@ -367,6 +367,9 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 #pragma unroll
         for (int pp = 0; pp < 4 / kParts; ++pp) {
           const int piece = c * (kChunk / 32) + h + kParts * pp;
+#ifdef MAPL_DBG
+          if (threadIdx.x == 64 && cg < 8 && pp == 1) DBGT(56 + cg)      // piece 0 of the chunk done
+#endif
           const uint32_t h4 = sHn_u32 + piece * 128;      // explicit ld.shared: the carved pointers compile to generic loads
           float sc[32];
 #pragma unroll
