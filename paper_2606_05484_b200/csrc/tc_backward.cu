@@ -168,10 +168,9 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
     mbar_wait(acc1_full, 0);
     if (warp == 2) DBG(58)
     tc_fence_after_sync();
-    for (int cc = half; cc < p.r / 32; cc += 2) {       // 32-column pieces alternate between the two warps
-      uint32_t v[32];
-      tmem_ld32(tmem_row + cc * 32, v);
-      tmem_ld_wait();
+    // 32-column pieces alternate between the two warps; r >= 128: two pieces per TMEM wait.
+    // The bf16 gz tile is both the A operand of phase 2 and the source of the TMA store to gz_out.
+    auto put_piece = [&](const uint32_t (&v)[32], int cc) {
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
         uint4 o;
@@ -179,8 +178,22 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         o.y = pack_bf16x2(__uint_as_float(v[8 * i + 2]), __uint_as_float(v[8 * i + 3]));
         o.z = pack_bf16x2(__uint_as_float(v[8 * i + 4]), __uint_as_float(v[8 * i + 5]));
         o.w = pack_bf16x2(__uint_as_float(v[8 * i + 6]), __uint_as_float(v[8 * i + 7]));
-        // the bf16 gz tile is both the A operand of phase 2 and the source of the TMA store to gz_out
         *reinterpret_cast<uint4*>(c.sA + (size_t)(cc / 2) * kTileBytes + sw128_offset(row, (cc & 1) * 4 + i)) = o;
+      }
+    };
+    if (p.r == 64) {
+      uint32_t v[32];
+      tmem_ld32(tmem_row + half * 32, v);
+      tmem_ld_wait();
+      put_piece(v, half);
+    } else {
+      for (int cc = half; cc < p.r / 32; cc += 4) {       // r is 128 or 256 here (tc_shape_ok)
+        uint32_t v0[32], v1[32];
+        tmem_ld32(tmem_row + cc * 32, v0);
+        tmem_ld32(tmem_row + (cc + 2) * 32, v1);
+        tmem_ld_wait();
+        put_piece(v0, cc);
+        put_piece(v1, cc + 2);
       }
     }
     if (p.ra) {
@@ -203,8 +216,16 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         }
       }
     }
+    if (warp == 2) DBG(61)
     fence_proxy_async_smem();
+    if (p.do_dh) {                    // release the phase-2 MMAs first: the TMA stores below only read the same tiles
+      tc_fence_before_sync();
+      __syncwarp();
+      if (warp == 2) DBG(59)
+      if (lane == 0) mbar_arrive_leader(gz_full);
+    }
     asm volatile("bar.sync 3, 256;" ::: "memory");
+    if (warp == 2) DBG(62)
     if (threadIdx.x == 64) {
       for (int kb = 0; kb < p.r / 64; ++kb) tma_store_2d(&tmGz, c.sA + (size_t)kb * kTileBytes, kb * 64, (int)m0);
       if (p.ga_tma) tma_store_2d(&tmGA, c.sOut, 0, (int)m0);
@@ -217,11 +238,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
       if (!p.do_dh) tma_store_wait_all<0>();
     }
     if (p.do_dh) {
-      tc_fence_before_sync();
-      fence_proxy_async_all();
-      __syncwarp();
-      if (warp == 2) DBG(59)
-      if (lane == 0) mbar_arrive_leader(gz_full);
+      if (warp == 2) DBG(63)
       chunk_epilogue(c, &tmO, (int)m0);
     }
     if (warp == 2) DBG(60)

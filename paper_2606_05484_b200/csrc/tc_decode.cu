@@ -108,7 +108,7 @@ k_tc_decode(const __grid_constant__ CUtensorMap tmZ, const __grid_constant__ CUt
       if (p.ra >= 128) gather_sum_rows<8>(c.sA, p.r / 64, p.ra, p.A, 0, idx, 1, q, lane, part);
       else gather_sum_rows<4>(c.sA, p.r / 64, p.ra, p.A, 0, idx, 1, q, lane, part);
     }
-    fence_proxy_async_all();
+    fence_proxy_async_smem();
     __syncwarp();
     if (warp == 2) DBG(3)
     if (lane == 0) mbar_arrive_leader(a_full);

@@ -332,7 +332,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 #pragma unroll
     for (int hh = 0; hh < kParts; ++hh) { n2 += xN2[hh * 128 + row]; amax = fmaxf(amax, xAmax[hh * 128 + row]); }
     float unscale = rho_to_operand(tmem_row, s.sRho, row, p.r, h, amax);
-    fence_proxy_async_all();
+    fence_proxy_async_smem();
     tc_fence_before_sync();
     __syncwarp();
     if (lane == 0) mbar_arrive_leader(s.rho_ready);
@@ -472,7 +472,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 #pragma unroll
         for (int hh = 0; hh < kParts; ++hh) { n2 += xN2[hh * 128 + row]; amax = fmaxf(amax, xAmax[hh * 128 + row]); }
         unscale = rho_to_operand(tmem_row, s.sRho, row, p.r, h, amax);
-        fence_proxy_async_all();
+        fence_proxy_async_smem();
         tc_fence_before_sync();
         __syncwarp();
         if (lane == 0) mbar_arrive_leader(s.rho_ready);
