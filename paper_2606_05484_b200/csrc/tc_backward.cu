@@ -205,7 +205,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         if (p.ga_tma) {          // ra == 64: box cc = [128 rows x 32 floats], swizzled, stored by TMA below
 #pragma unroll
           for (int i = 0; i < 8; ++i)
-            *reinterpret_cast<float4*>(c.sOut + (size_t)cc * kTileBytes + sw128_offset(row, i)) =
+            *reinterpret_cast<float4*>(c.sOut + (size_t)cc * kBoxesPerHalf * kTileBytes + sw128_offset(row, i)) =
                 make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]), __uint_as_float(v[4 * i + 2]),
                             __uint_as_float(v[4 * i + 3]));
         } else if (live) {
@@ -233,7 +233,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
       if (!p.do_dh) tma_store_wait_all<0>();
     }
     if (threadIdx.x == 192 && p.ga_tma) {
-      tma_store_2d(&tmGA, c.sOut + kTileBytes, 32, (int)m0);
+      tma_store_2d(&tmGA, c.sOut + (size_t)kBoxesPerHalf * kTileBytes, 32, (int)m0);     // thread 192's own first box
       tma_store_commit();
       if (!p.do_dh) tma_store_wait_all<0>();
     }

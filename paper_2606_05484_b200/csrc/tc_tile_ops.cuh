@@ -27,7 +27,11 @@ constexpr int kChunkN = 128;                 // d-chunk width == UMMA N
 constexpr int kTileBytes = 128 * 64 * 2;     // one [128 x 64] bf16 tile
 constexpr int kHalfTileBytes = 64 * 64 * 2;  // the half of a W tile one CTA of the pair holds
 constexpr int kAccStages = 4;
-constexpr int kOutBufs = 2;                  // one chunk's two [128 x 64] staging boxes
+#ifndef MAPL_OUT_BUFS
+#define MAPL_OUT_BUFS 4
+#endif
+constexpr int kOutBufs = MAPL_OUT_BUFS;      // [128 x 64] staging boxes: kOutBufs / 2 per column half of a chunk, used in turn
+constexpr int kBoxesPerHalf = kOutBufs / 2;
 constexpr int kPipeThreads = 320;            // warp 0 TMA, warp 1 MMA, warps 2-9 epilogue
 
 struct ChunkPipe {
@@ -85,8 +89,8 @@ __device__ __forceinline__ void chunk_mma(const ChunkPipe& c) {
 __device__ __forceinline__ void chunk_epilogue(const ChunkPipe& c, const CUtensorMap* tmO, int m0) {
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32, q = warp & 3, h = (warp - 2) >> 2, row = q * 32 + lane;
   const bool issuer = threadIdx.x == 64 + h * 128;
-  uint8_t* box = c.sOut + (size_t)h * kTileBytes;
   for (int j = 0; j < c.nchunks; ++j) {
+    uint8_t* box = c.sOut + (size_t)(h * kBoxesPerHalf + j % kBoxesPerHalf) * kTileBytes;
     const int as = j % kAccStages;
     mbar_wait(&c.acc_full[as], (j / kAccStages) & 1);
     if (threadIdx.x == 64 && j < 16) DBGT(40 + j)
@@ -99,8 +103,9 @@ __device__ __forceinline__ void chunk_epilogue(const ChunkPipe& c, const CUtenso
     tc_fence_before_sync();
     __syncwarp();
     if (lane == 0) mbar_arrive_leader(&c.acc_empty[as]);     // the TMEM stage may be overwritten
-    // chunk j-1's store must have read the staging box before it is rewritten
-    if (issuer) tma_store_wait_read<0>();
+    // the store that last used this box (chunk j - kBoxesPerHalf; in the first round whatever the caller staged
+    // there) must have read it before it is rewritten
+    if (issuer) { if (j < kBoxesPerHalf) tma_store_wait_read<0>(); else tma_store_wait_read<kBoxesPerHalf - 1>(); }
     if (h == 0) asm volatile("bar.sync 1, 128;" ::: "memory"); else asm volatile("bar.sync 2, 128;" ::: "memory");
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
