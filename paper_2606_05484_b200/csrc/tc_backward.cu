@@ -5,7 +5,7 @@
 //     phase 1   [gz | gA] = g . [U | B^T]         K = d, streamed through a TMA ring
 //               epilogue (8 warps): gz -> bf16 -> swizzled smem tiles that are both the A operand of
 //               phase 2 and the source of the TMA store to gz_out (the backward wire payload);
-//               gA rows -> fp32 scratch [N,ra] (TMA store from staging boxes when ra = 64).
+//               gA rows -> fp32 scratch [N,ra] (TMA stores from the staging boxes).
 //               With RVQ the same warps first dequantise the tile's codes into the bf16 Zhat
 //               operand of k_tc_bwd_du (hidden under the g stream).
 //     phase 2   dH = gz . U^T                     the chunk pipeline of tc_tile_ops.cuh
@@ -196,16 +196,19 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         put_piece(v1, cc + 2);
       }
     }
+    // gA staging: the ra / 32 pieces spread over the kOutBufs boxes (ra = 64: boxes 0 and 2, ra = 128: all four), so that
+    // thread 64 stores from its own boxes [0, kBoxesPerHalf) and thread 192 from the rest (chunk_epilogue reuses them)
+    const int ga_step = p.ra ? kOutBufs / (p.ra / 32) : 1;
     if (p.ra) {
       float4* dst = reinterpret_cast<float4*>(p.gA + (live ? m : 0) * p.ra);
       for (int cc = half; cc < p.ra / 32; cc += 2) {
         uint32_t v[32];
         tmem_ld32(tmem_row + p.r + cc * 32, v);
         tmem_ld_wait();
-        if (p.ga_tma) {          // ra == 64: box cc = [128 rows x 32 floats], swizzled, stored by TMA below
+        if (p.ga_tma) {          // piece cc = [128 rows x 32 floats] -> staging box cc * ga_step, swizzled, stored by TMA below
 #pragma unroll
           for (int i = 0; i < 8; ++i)
-            *reinterpret_cast<float4*>(c.sOut + (size_t)cc * kBoxesPerHalf * kTileBytes + sw128_offset(row, i)) =
+            *reinterpret_cast<float4*>(c.sOut + (size_t)cc * ga_step * kTileBytes + sw128_offset(row, i)) =
                 make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]), __uint_as_float(v[4 * i + 2]),
                             __uint_as_float(v[4 * i + 3]));
         } else if (live) {
@@ -228,12 +231,15 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
     if (warp == 2) DBG(62)
     if (threadIdx.x == 64) {
       for (int kb = 0; kb < p.r / 64; ++kb) tma_store_2d(&tmGz, c.sA + (size_t)kb * kTileBytes, kb * 64, (int)m0);
-      if (p.ga_tma) tma_store_2d(&tmGA, c.sOut, 0, (int)m0);
+      if (p.ga_tma)
+        for (int cc = 0; cc * ga_step < kBoxesPerHalf; ++cc)
+          tma_store_2d(&tmGA, c.sOut + (size_t)cc * ga_step * kTileBytes, cc * 32, (int)m0);
       tma_store_commit();
       if (!p.do_dh) tma_store_wait_all<0>();
     }
     if (threadIdx.x == 192 && p.ga_tma) {
-      tma_store_2d(&tmGA, c.sOut + (size_t)kBoxesPerHalf * kTileBytes, 32, (int)m0);     // thread 192's own first box
+      for (int cc = 0; cc < p.ra / 32; ++cc)
+        if (cc * ga_step >= kBoxesPerHalf) tma_store_2d(&tmGA, c.sOut + (size_t)cc * ga_step * kTileBytes, cc * 32, (int)m0);
       tma_store_commit();
       if (!p.do_dh) tma_store_wait_all<0>();
     }
@@ -498,7 +504,8 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes,
                  ring2 = (size_t)(d.r / 64) * kTileBytes + (size_t)p.b_stages * kHalfTileBytes;
     const size_t smem = (ring1 > ring2 ? ring1 : ring2) + (size_t)kOutBufs * kTileBytes + 1024 + 1024;
-    p.ga_tma = ra == 64 ? 1 : 0;
+    static_assert(kOutBufs == 4, "gA staging: ra / 32 pieces over four boxes");
+    p.ga_tma = (ra == 64 || ra == 128) ? 1 : 0;
     p.codes = codes; p.codebooks = codebooks; p.zhat_out = zhat_ws; p.L = d.rvq_levels; p.K = d.rvq_k;
     CUtensorMap tmG, tmWu, tmWb, tmWd, tmO, tmGz, tmGA;
     if (!make_tmap_bf16_2d(&tmGz, gz_out, N, rr, rr, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
