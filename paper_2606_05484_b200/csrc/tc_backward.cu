@@ -335,7 +335,8 @@ __device__ __forceinline__ void scatter_gA(const BwdDuParams& p, float* sG, int*
 template <bool kPair>
 __global__ void __launch_bounds__(kThreadsDu, 1)
 k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmZ,
-            const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmGz, const BwdDuParams p) {
+            const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmGz,
+            const __grid_constant__ CUtensorMap tmDU, const BwdDuParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)p.stages * p.item_bytes);
@@ -356,6 +357,7 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmG); tma_prefetch_desc(&tmZ); tma_prefetch_desc(&tmH); tma_prefetch_desc(&tmGz);
+    tma_prefetch_desc(&tmDU);
     for (int s = 0; s < p.stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
     mbar_init(acc_full, 1);
     fence_barrier_init();
@@ -430,8 +432,10 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         if (kPair) umma_commit_pair(acc_full); else umma_commit(acc_full);
       }
     } else {
+      // dU tile += accumulator: staged in the (now idle) ring as swizzled [128 rows x 32 floats] boxes and added by
+      // TMA reductions -- whole 128-byte lines, where a row-per-thread red.global.add.v4 from the TMEM layout
+      // sends 32 separate 16-byte reductions per instruction
       const int q = warp & 3, row = q * 32 + lane;
-      float* dst = p.dU + ((long long)dt * 128 + row) * p.r;
       mbar_wait(acc_full, 0);
       if (threadIdx.x == 64) DU_DBG(4)
       tc_fence_after_sync();
@@ -441,8 +445,16 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         tmem_ld_wait();
 #pragma unroll
         for (int i = 0; i < 8; ++i)
-          red_add_v4(dst + cc * 32 + i * 4, __uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
-                     __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+          *reinterpret_cast<float4*>(smem + (size_t)cc * kTileBytes + sw128_offset(row, i)) =
+              make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]), __uint_as_float(v[4 * i + 2]),
+                          __uint_as_float(v[4 * i + 3]));
+      }
+      fence_proxy_async_smem();
+      asm volatile("bar.sync 2, 128;" ::: "memory");
+      if (threadIdx.x == 64) {
+        for (int cc = 0; cc < p.r / 32; ++cc) tma_reduce_add_2d(&tmDU, smem + (size_t)cc * kTileBytes, cc * 32, dt * 128);
+        tma_store_commit();
+        tma_store_wait_all<0>();
       }
     }
   }
@@ -532,7 +544,7 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     const size_t scatter_bytes = ra ? (size_t)128 * (ra + 4) * 4 + 3 * 512 : 0;
     p.stages = (int)((227 * 1024 - 2048 - scatter_bytes) / p.item_bytes);
     if (p.stages > 8) p.stages = 8;
-    if (p.stages < 2) return MAPL_ERR_UNSUPPORTED;
+    if (p.stages < 2 || (size_t)p.stages * p.item_bytes < (size_t)(d.r / 32) * kTileBytes) return MAPL_ERR_UNSUPPORTED;   // ring doubles as the dU staging
     p.n_blocks = (int)((d.n_tokens + 63) / 64);
     int S = 148 / n_dt;
     if (S < 1) S = 1;
@@ -540,14 +552,15 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     p.blocks_per_split = (p.n_blocks + S - 1) / S;
     S = (p.n_blocks + p.blocks_per_split - 1) / p.blocks_per_split;
     const size_t smem = (size_t)p.stages * p.item_bytes + 1024 + 512 + scatter_bytes;
-    CUtensorMap tmG, tmZ, tmH, tmGz;
+    CUtensorMap tmG, tmZ, tmH, tmGz, tmDU;
+    if (!make_tmap_f32_2d(&tmDU, dU_out, dd, rr, rr, 32, 128)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmG, g, N, dd, dd, 64, 64)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmZ, zhat, N, rr, rr, 64, 64)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmH, H ? H : g, N, dd, dd, 64, 64)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmGz, gz_out, N, rr, rr, 64, 64)) return MAPL_ERR_CUDA;
     KernelScope ks(KID_TC_BWD_DU, st);
-    if (pair) MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_bwd_du<true>, dim3(n_dt, S), dim3(kThreadsDu), smem, st, tmG, tmZ, tmH, tmGz, p));
-    else MAPL_CUDA_CHECK(launch_pdl(k_tc_bwd_du<false>, dim3(n_dt, S), dim3(kThreadsDu), smem, st, tmG, tmZ, tmH, tmGz, p));
+    if (pair) MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_bwd_du<true>, dim3(n_dt, S), dim3(kThreadsDu), smem, st, tmG, tmZ, tmH, tmGz, tmDU, p));
+    else MAPL_CUDA_CHECK(launch_pdl(k_tc_bwd_du<false>, dim3(n_dt, S), dim3(kThreadsDu), smem, st, tmG, tmZ, tmH, tmGz, tmDU, p));
   }
   if (dB_out && ra) {   // dB += A[tok]^T g  (P_p is frozen in the paper: optional, fp32 SIMT)
     GemmArgs ga;
