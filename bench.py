@@ -65,7 +65,7 @@ def alg_bytes_per_token(cfg):
     payload = r * s if L == 0 else 4 * L
     enc = d * s + payload
     dec = payload + 4 + d * s
-    bwd = 3 * d * s + 2 * r * s + 4            # g, H read; dH written; payload read; gz written; tok
+    bwd = 3 * d * s + payload + r * s + 4      # g, H read; dH written; payload (Z or codes) read; gz written; tok
     return dict(encode=enc, decode=dec, backward=bwd)
 
 
