@@ -104,21 +104,26 @@ __device__ __forceinline__ Smem carve_smem(uint8_t* base, const RvqParams& p) {
 // 0.5||c||^2 - rho.c.  Warp-convergent (tcgen05.ld is .sync.aligned); lanes without work pass any
 // valid row and ignore the result.
 __device__ __forceinline__ float exact_score(uint32_t tmem_row, const float* __restrict__ crow, float hn, int r) {
+  // the row loads (L2 latency) of TWO 32-column pieces are in flight together (r is a multiple of 64); the residual
+  // pieces are read from TMEM one at a time to keep the register count down
   float dot = 0.f;
-  for (int pc = 0; pc < r / 32; ++pc) {
-    uint32_t v[32];
-    tmem_ld32(tmem_row + pc * 32, v);
+  for (int pc = 0; pc < r / 32; pc += 2) {
     const float4* c4 = reinterpret_cast<const float4*>(crow + pc * 32);
-    float4 c[8];
+    float4 c[16];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) c[i] = __ldg(c4 + i);
-    tmem_ld_wait();
+    for (int i = 0; i < 16; ++i) c[i] = __ldg(c4 + i);
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      dot = fmaf(__uint_as_float(v[4 * i + 0]), c[i].x, dot);
-      dot = fmaf(__uint_as_float(v[4 * i + 1]), c[i].y, dot);
-      dot = fmaf(__uint_as_float(v[4 * i + 2]), c[i].z, dot);
-      dot = fmaf(__uint_as_float(v[4 * i + 3]), c[i].w, dot);
+    for (int u = 0; u < 2; ++u) {
+      uint32_t v[32];
+      tmem_ld32(tmem_row + (pc + u) * 32, v);
+      tmem_ld_wait();
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        dot = fmaf(__uint_as_float(v[4 * i + 0]), c[8 * u + i].x, dot);
+        dot = fmaf(__uint_as_float(v[4 * i + 1]), c[8 * u + i].y, dot);
+        dot = fmaf(__uint_as_float(v[4 * i + 2]), c[8 * u + i].z, dot);
+        dot = fmaf(__uint_as_float(v[4 * i + 3]), c[8 * u + i].w, dot);
+      }
     }
   }
   return hn - dot;
