@@ -13,7 +13,7 @@
 //               separate memset launches.
 // k_tc_bwd_du   dU[d-tile, :] += sum over a token range of  g^T Zhat + H^T gz.  Both operands are
 //               MN-major (tokens are the contraction index): TMA boxes [64 tokens x 64 cols]
-//               are used as they land.  Split over token ranges; fp32 vector atomics into dU.
+//               are used as they land.  Split over token ranges; the fp32 tile is added to dU by TMA reductions.
 //               r >= 128: CTA pairs (two d-tiles, M = 256, half of the Zhat / gz columns per CTA).
 //               Its main loop streams g and H at 6.2 TB/s (measured, c1).
 //               While the MMAs run, the epilogue warps scatter-add the gA rows into dA[tok]:
