@@ -94,6 +94,72 @@ __global__ void __launch_bounds__(256) k_st_split(const float* __restrict__ src,
   }
 }
 
+// Same for rows, cols multiples of 64 and modes 0 / 1, vectorised: 64 x 64 tiles, every thread converts 8 consecutive
+// elements and stores 16 bytes per plane; the transposed planes go through shared memory so that 8 lanes write one
+// whole 128-byte segment (the scalar kernel above writes 2 bytes per store instruction and lane).
+__device__ __forceinline__ void split3x8(const float (&x)[8], __nv_bfloat16* o, long long plane) {
+  uint32_t w[3][4];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    __nv_bfloat16 a[2], b[2], c[2];
+    split3(x[2 * j], &a[0], &b[0], &c[0]);
+    split3(x[2 * j + 1], &a[1], &b[1], &c[1]);
+    w[0][j] = (uint32_t)__bfloat16_as_ushort(a[0]) | ((uint32_t)__bfloat16_as_ushort(a[1]) << 16);
+    w[1][j] = (uint32_t)__bfloat16_as_ushort(b[0]) | ((uint32_t)__bfloat16_as_ushort(b[1]) << 16);
+    w[2][j] = (uint32_t)__bfloat16_as_ushort(c[0]) | ((uint32_t)__bfloat16_as_ushort(c[1]) << 16);
+  }
+#pragma unroll
+  for (int pl = 0; pl < 3; ++pl) *reinterpret_cast<uint4*>(o + pl * plane) = make_uint4(w[pl][0], w[pl][1], w[pl][2], w[pl][3]);
+}
+
+__global__ void __launch_bounds__(256) k_st_split64(const float* __restrict__ src, int rows, int cols, int mode,
+                                                    __nv_bfloat16* __restrict__ prow, __nv_bfloat16* __restrict__ ptr,
+                                                    float4* __restrict__ zero, long long nzero4) {
+  __shared__ float tile[64][65];
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  if (zero != nullptr)
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < nzero4; i += (long long)gridDim.x * 256)
+      zero[(long long)blockIdx.y * nzero4 + i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  const long long plane = (long long)rows * cols;
+  src += (long long)blockIdx.y * plane;
+  if (prow) prow += (long long)blockIdx.y * 3 * plane;
+  if (ptr) ptr += (long long)blockIdx.y * 3 * plane;
+  const int tiles_c = cols / 64, tiles_r = rows / 64, t = threadIdx.x;
+  for (int tl = blockIdx.x; tl < tiles_c * tiles_r; tl += gridDim.x) {
+    const int r0 = (tl / tiles_c) * 64, c0 = (tl % tiles_c) * 64;
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      const int idx = t + 256 * u, i = idx / 8, c8 = (idx % 8) * 8;         // row i of the tile, columns c8 .. c8+7
+      const int r = r0 + i, c = c0 + c8;
+      const float4 lo = *reinterpret_cast<const float4*>(src + (long long)r * cols + c);
+      const float4 hi = *reinterpret_cast<const float4*>(src + (long long)r * cols + c + 4);
+      float x[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+      if (mode == 1) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) x[j] = 0.5f * ((r == c + j ? 3.f : 0.f) - x[j]);
+      }
+      if (ptr) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) tile[i][c8 + j] = x[j];
+      }
+      if (prow) split3x8(x, prow + (long long)r * cols + c, plane);
+    }
+    if (ptr) {
+      __syncthreads();
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int idx = t + 256 * u, cc = idx / 8, r8 = (idx % 8) * 8;      // transposed row cc, elements r8 .. r8+7
+        float x[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) x[j] = tile[r8 + j][cc];
+        split3x8(x, ptr + (long long)(c0 + cc) * rows + r0 + r8, plane);
+      }
+      __syncthreads();
+    }
+  }
+}
+
 struct Gemm3Params {
   float* C; const float* E;
   float beta;
@@ -229,8 +295,14 @@ size_t tc_st_plane_bytes(int d, int r, int batch) {   // one set of planes of a 
 
 int tc_st_split(const float* src, int rows, int cols, int batch, int mode, float lr, __nv_bfloat16* prow,
                 __nv_bfloat16* ptr, cudaStream_t st, float* zero, long long nzero) {
-  const int tiles = ((rows + 31) / 32) * ((cols + 31) / 32);
   KernelScope ks(KID_ST_SPLIT, st);
+  if (mode <= 1 && rows % 64 == 0 && cols % 64 == 0) {
+    const int tiles64 = (rows / 64) * (cols / 64);
+    MAPL_CUDA_CHECK(tc::launch_pdl(k_st_split64, dim3(tiles64 < 1024 ? tiles64 : 1024, batch), dim3(256), 0, st, src, rows, cols, mode,
+                                   prow, ptr, reinterpret_cast<float4*>(zero), nzero / 4));
+    return MAPL_OK;
+  }
+  const int tiles = ((rows + 31) / 32) * ((cols + 31) / 32);
   MAPL_CUDA_CHECK(tc::launch_pdl(k_st_split, dim3(tiles < 1024 ? tiles : 1024, batch), dim3(256), 0, st, src, rows, cols, mode, lr,
                                  prow, ptr, reinterpret_cast<float4*>(zero), nzero / 4));
   return MAPL_OK;
