@@ -181,7 +181,9 @@ int mapl_center_backward(const mapl_boundary_desc* desc, const void* gz, const i
  *   r >= 256 the [d,r]-sized products run on the tensor cores as exact three-plane bf16 splits,
  *   six MMAs per product; otherwise fp32 FFMA kernels.  QR: CholeskyQR2 in fp32 -- blocked
  *   Cholesky of the Gram matrix and a blocked triangular inverse, twice; it needs cond(Y) well
- *   below 1e3, which holds for a step from an orthonormal U.)
+ *   below 1e3, which holds for a step from an orthonormal U.  Measured residuals: <= 5e-6 on the
+ *   tensor-core shapes up to r = 1024; the FFMA kernels stay below 1e-5 for r <= 768 at
+ *   d <= 2048 and reach 1.1e-5 at d = r = 1024 -- plain fp32 sums over d.)
  *   info_out   optional device [batch,2] fp32: ||xi||_F and ||U^T U - I||_F after the update.
  * Requires 8 <= r <= d, r % 8 == 0, d % 8 == 0, r <= 1024.                                      */
 int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U_inout, const float* G, float lr,

@@ -541,7 +541,7 @@ int ctx_tangent(const StCtx& c, const float* U, const float* G, float* out) {
     { KernelScope ks(KID_MEMSET, c.st); MAPL_CUDA_CHECK(cudaMemsetAsync(c.S, 0, (size_t)batch * r * r * 4, c.st)); }
     MAPL_RETURN_IF(tc_st_split(U, d, r, batch, 0, 0.f, c.Prow, c.Ptr, c.st));
     MAPL_RETURN_IF(tc_st_split(G, d, r, batch, 0, 0.f, nullptr, c.Ptr2, c.st));
-    MAPL_RETURN_IF(tc_st_gemm3(c.Ptr, c.Ptr2, r, r, d, batch, c.S, nullptr, 0.f, d / 256 > 0 ? d / 256 : 1, c.st));
+    MAPL_RETURN_IF(tc_st_gemm3(c.Ptr, c.Ptr2, r, r, d, batch, c.S, nullptr, 0.f, (d / 64 + 3) / 4, c.st));
     MAPL_RETURN_IF(tc_st_split(c.S, r, r, batch, 3, 0.f, c.Pm, nullptr, c.st));
     return tc_st_gemm3(c.Prow, c.Pm, d, r, r, batch, out, G, 1.f, 1, c.st);
   }
@@ -559,7 +559,7 @@ int ctx_ns(const StCtx& c, float* cur, float* nxt, float* final_out, int iters) 
     float* out = (it == iters - 1) ? final_out : nxt;
     if (c.tc) {
       MAPL_RETURN_IF(tc_st_split(cur, d, r, batch, 0, 0.f, c.Prow, c.Ptr, c.st, c.S, (long long)r * r));
-      MAPL_RETURN_IF(tc_st_gemm3(c.Ptr, c.Ptr, r, r, d, batch, c.S, nullptr, 0.f, d / 256 > 0 ? d / 256 : 1, c.st));
+      MAPL_RETURN_IF(tc_st_gemm3(c.Ptr, c.Ptr, r, r, d, batch, c.S, nullptr, 0.f, (d / 64 + 3) / 4, c.st));
       MAPL_RETURN_IF(tc_st_split(c.S, r, r, batch, 1, 0.f, c.Pm, nullptr, c.st));
       MAPL_RETURN_IF(tc_st_gemm3(c.Prow, c.Pm, d, r, r, batch, out, nullptr, 0.f, 1, c.st));
     } else {
@@ -641,7 +641,10 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
     __nv_bfloat16* Ptr = reinterpret_cast<__nv_bfloat16*>(ws + w.Ptr);     // [b][3][r][d]
     __nv_bfloat16* Ptr2 = reinterpret_cast<__nv_bfloat16*>(ws + w.Ptr2);   // [b][3][r][d]
     __nv_bfloat16* Pm = reinterpret_cast<__nv_bfloat16*>(ws + w.Pm);       // [b][3][r][r]
-    const int ksplit = d / 256 > 0 ? d / 256 : 1;                           // Gram products: 4 k-blocks (one per TMEM accumulator) per CTA
+    // Gram products: at most 4 k-blocks of 64 per CTA, one per TMEM accumulator.  A longer chain of MMAs into one
+    // accumulator shows the tensor core's truncating accumulate on diag(X^T X): d = 384 with d / 256 = 1 split ran 6
+    // k-blocks in one CTA and left ||U^T U - I||_F = 1.3e-5 (3.4e-6 with two splits of 3).
+    const int ksplit = (d / 64 + 3) / 4;
     auto zero_S = [&]() -> int {
       KernelScope ks(KID_MEMSET, st);
       MAPL_CUDA_CHECK(cudaMemsetAsync(S, 0, (size_t)batch * r * r * 4, st));

@@ -47,6 +47,23 @@ def test_single_step_matches_oracle(retr, d, r, batch):
 
 
 @pytest.mark.parametrize("retr", ["qr", "ns"])
+@pytest.mark.parametrize("d,r,batch", [(1024, 1024, 1), (384, 384, 2), (640, 256, 1), (1536, 768, 1), (1024, 72, 2)])
+def test_extreme_shapes_one_step(retr, d, r, batch):
+    """The largest supported r (square U: 32 Cholesky panels, 5 doubling levels of the triangular inverse), tensor-core
+    shapes that are not powers of two (r/32 = 12, 24: partial pairs in the inverse; d/64 = 6, 10: uneven Gram splits -- d = 384
+    once ran 6 k-blocks into one TMEM accumulator and left a residual of 1.3e-5), and a ragged last panel (r = 72)."""
+    s = I.make_stiefel(r, d=d, batch=batch)
+    lr = min(1e-2, 0.5 / (np.sqrt(d) + np.sqrt(r)))
+    U = to_dev(s.U); G = to_dev(s.G)
+    _gpu_step(U, G, lr, RETR[retr][0], info=False)
+    Ug = to_np(U)
+    for b in range(batch):
+        Uo, _ = o.stiefel_step(s.U.f64[b], s.G.f64[b], lr, RETR[retr][1], 5)
+        assert rel_fro(Ug[b], Uo) <= 1e-5, (retr, d, r, b, rel_fro(Ug[b], Uo))
+        assert _orth_res(Ug[b]) <= 1e-5, _orth_res(Ug[b])
+
+
+@pytest.mark.parametrize("retr", ["qr", "ns"])
 @pytest.mark.parametrize("r", I.STIEFEL_RS)
 def test_config4_shapes_one_step(retr, r):
     """configs[4]: d=2048, r in {64,128,256,512}, 3 projectors, lr=1e-2, Gaussian G."""
