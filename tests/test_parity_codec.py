@@ -79,6 +79,20 @@ def test_ragged_shapes(act, shape):
         assert (gpu["codes"] == 0).all()
 
 
+@pytest.mark.parametrize("shape", [
+    # (N, d, r, L, K, V, ra) -- corners of the tensor-core envelope (bf16, d % 128 == 0, r in {64,128,256}, ra in {0,64,128})
+    (600, 8192, 256, 2, 8192, 1000, 128),   # longest projection chain, largest codebook
+    (300, 128, 64, 0, 0, 100, 0),           # smallest d, no anchor, no RVQ
+    (1000, 4096, 128, 4, 128, 500, 64),     # smallest codebook the path takes, four levels
+    (150, 1024, 64, 8, 256, 200, 128),      # eight levels (the maximum), anchor wider than the payload
+    (259, 2048, 256, 0, 0, 300, 64),        # two ragged tiles, RVQ off at r = 256
+])
+def test_tc_envelope_corners(shape):
+    N, d, r, L, K, V, ra = shape
+    bi = I.make_generic(40 + N % 13, N, d, r, L, K, V, ra, "bf16")
+    _roundtrip(bi)
+
+
 def test_identity_at_full_rank_no_anchor():
     """r = d, RVQ off, no anchor: Hhat = H up to rounding."""
     bi = I.make_generic(5, 200, 64, 64, 0, 0, 1, 0, "f32")
