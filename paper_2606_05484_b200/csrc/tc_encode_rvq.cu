@@ -18,6 +18,10 @@
 //             (fp16 rounding of both operands, Cauchy-Schwarz).  The true minimiser is therefore
 //             always among the candidates; they are re-scored in exact fp32 (rho from TMEM, the
 //             fp32 codeword from L2), lowest index winning ties (S4).  Then rho -= C[l, k*].
+//             A thread's candidate list holds kNE 32-codeword pieces; when it is full it keeps the
+//             pieces with the lowest minima, and only a left-out piece whose minimum is within the
+//             FINAL threshold (the threshold only tightens during the scan) sends the warp to the
+//             exhaustive fp32 pass over all K codewords (duplicate-heavy codebooks).
 // Roofline: tensor at config 3 (K r = 1M per level), HBM/ALU at config 2.
 #include <float.h>
 
@@ -355,7 +359,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 
       float best = FLT_MAX;
       int cnt = 0;
-      bool overflow = false;
+      float dropped = FLT_MAX;           // lowest piece minimum that found no room in the list
       for (int c = 0; c < nchunks; ++c, ++cg) {
         const int as = cg & 1;
         mbar_wait(&s.acc_full[as], (cg >> 1) & 1);
@@ -407,7 +411,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 #pragma unroll
               for (int i = 7; i >= 0; --i) mk[g] = __funnelshift_l(__float_as_uint(thr - sc[8 * g + i]), mk[g], 1);
             const uint32_t mask = ~(mk[0] | (mk[1] << 8) | (mk[2] << 16) | (mk[3] << 24));
-            if (live && mask != 0 && !overflow) {
+            if (live && mask != 0) {
               if (cnt == kNE) {                 // list full: drop entries the tighter threshold excludes
                 int j = 0;
                 for (int e = 0; e < kNE; ++e) {
@@ -417,7 +421,21 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
                 cnt = j;
               }
               if (cnt == kNE) {
-                overflow = true;                // pathological (e.g. many duplicate codewords): exhaustive below
+                // still full: the list keeps the kNE pieces with the lowest minima.  A piece left out matters only if
+                // its minimum is within the FINAL threshold (checked after the scan; the threshold only tightens), so a
+                // list that is full for a moment under the early, loose threshold no longer forces the exhaustive pass.
+                int w = 0;
+                float wm = eM[0];
+                for (int e = 1; e < kNE; ++e) {
+                  const float em = eM[e * kEpi];
+                  if (em > wm) { wm = em; w = e; }
+                }
+                if (m32 < wm) {
+                  dropped = fminf(dropped, wm);
+                  eM[w * kEpi] = m32; eP[w * kEpi] = piece; eMask[w * kEpi] = mask;     // entries no longer ascend in k
+                } else {
+                  dropped = fminf(dropped, m32);
+                }
               } else {
                 eM[cnt * kEpi] = m32; eP[cnt * kEpi] = piece; eMask[cnt * kEpi] = mask; ++cnt;
               }
@@ -431,8 +449,9 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       for (int hh = 0; hh < kParts; ++hh) best = fminf(best, xBest[hh * 128 + row]);
       if (warp == 2 && l < 4) { DBG(5 + l * 4) }
 
-      // ---- exact fp32 re-scoring of this thread's candidates, ascending k, strict '<': lowest index wins ties
+      // ---- exact fp32 re-scoring of this thread's candidates: lowest score, lowest index on ties
       const float thr = best + margin;
+      const bool overflow = live && dropped <= thr;     // pathological (e.g. many duplicate codewords): exhaustive below
       float bestx = FLT_MAX;
       int bestk = 0x7fffffff, e = 0, piece = 0;
       uint32_t mrem = 0;
@@ -446,7 +465,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         int k = 0;
         if (have) { k = piece * 32 + __ffs(mrem) - 1; mrem &= mrem - 1; }
         const float sx = exact_score(tmem_row, Cl + (long long)k * p.r, s.sHn[k], p.r);
-        if (have && sx < bestx) { bestx = sx; bestk = k; }
+        if (have && (sx < bestx || (sx == bestx && k < bestk))) { bestx = sx; bestk = k; }
       }
       if (__any_sync(full, overflow)) {         // exhaustive over the pieces this warp owns
         for (int pc = h; pc < p.K / 32; pc += kParts)

@@ -171,6 +171,32 @@ def test_tc_rvq_planted_codewords_are_recovered():
     assert np.array_equal(gpu["codes"][:, 1], k1)
 
 
+def test_tc_rvq_candidate_list_full_only_under_the_early_threshold():
+    """One near-copy of a vector w + 2u in every 32-codeword piece (64 pieces, so every scan warp sees more
+    pieces within the margin of the running minimum than its candidate list holds), and w itself in the
+    LAST piece.  Tokens near w: the list is full until the last piece tightens the threshold, the pieces
+    left out lie above the final threshold, and the answer is K-5 without the exhaustive pass.  Tokens
+    near w + 2u: the near-copies really are within the final margin (exhaustive pass).  Both against the
+    oracle under the near-tie rule S5.  Found at c3: one such token after 8 Stiefel steps made one warp
+    re-score all K=4096 codewords (encode 260 -> 2990 us)."""
+    K, r, n = 2048, 64, 336
+    bi = I.make_generic(29, n, 256, r, 1, K, 100, 0, "bf16", cb_std=(1.0,))
+    rng = np.random.default_rng(11)
+    C = bi.C.f64.copy()
+    w = rng.standard_normal(r)
+    u = rng.standard_normal(r)
+    u /= np.linalg.norm(u)
+    for j in range(K // 32):
+        C[0, 32 * j + 3] = w + 2.0 * u + 2e-2 * rng.standard_normal(r)   # score spread ~1e-2: far above fp32 noise, far below the margin (~0.15)
+    C[0, K - 5] = w
+    Z = np.where((np.arange(n) % 3 == 0)[:, None], w + 2.0 * u, w)[:, :] + 0.02 * rng.standard_normal((n, r))
+    bi = dataclasses.replace(_with_codebook(bi, C), H=I.store(Z @ bi.U.f64.T, "bf16"))
+    gpu, ora, stats, errs = _roundtrip(bi)
+    near_w = np.arange(n) % 3 != 0
+    assert (gpu["codes"][near_w, 0] == K - 5).all()
+    assert (gpu["codes"][~near_w, 0] % 32 == 3).all()
+
+
 @pytest.mark.parametrize("r,K,L", [(64, 128, 1), (128, 512, 3), (256, 1024, 2), (64, 4096, 2)])
 def test_tc_rvq_envelope_shapes(r, K, L):
     bi = I.make_generic(23 + r % 7, 200 + r, 512, r, L, K, 300, 64, "bf16")
