@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- codec tokens/s of the MAPL boundary codec on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mapl|reference] [--workload c1|c2|c3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl mapl|reference] [--workload all|c0|c1|c2|c3]
 
 One "step" = one pass of the whole hot path over one batch of synthetic input: for every stage
 boundary of the workload, mapl_encode -> mapl_decode (forward order), then mapl_codec_backward in
@@ -9,10 +9,18 @@ reverse order (full backward: H given, dH and dA produced, dB off as in the pape
 mapl_stiefel_step per boundary when the workload says so (c3).  A codec token = one token crossing
 one boundary through all three calls; value = N * n_boundaries * n_gpus * K / time.
 
+Default (`--workload all`): the headline line is configs[3] (c3: d=2048, r=256, 2-level RVQ with
+K=4096, anchor rank 128, 3 boundaries + the Stiefel step -- the largest single-GPU configuration,
+the one BASELINE.json's "proj+RVQ+anchor" metric names all its work for); `per_config` carries
+c1, c2 and c3 side by side (per-call times, whole-config roofline against measured and nominal peaks,
+the dominant kernel's roofline), `c0` the parity config's call times, `stiefel` configs[4] (steps/s,
+roofline fraction per r, the oracle's time per step and one-step parity late in the 1000-step run).
+
 Timing: W >= 3 warm-up steps, then exactly K steps between barrier + synchronize, CUDA events on
-the launching stream, max over ranks.  The K steps replay one CUDA graph of the step (the calls are
-launch-bound from Python otherwise).  Every boundary has its own buffers; the per-step working set
-(hundreds of MB) exceeds the 126 MB L2, so no flush is needed between iterations.
+the launching stream (one event per step: median and max are reported beside the mean), max over
+ranks.  The K steps replay one CUDA graph of the step (the calls are launch-bound from Python
+otherwise).  Every boundary has its own buffers; the per-step working set (hundreds of MB) exceeds
+the 126 MB L2, so no flush is needed between iterations.
 
 Prints ONE JSON line (rank 0).  Multi-GPU: one process per GPU under torchrun, independent
 micro-batches per rank (weak scaling), no data-path collective.
@@ -21,6 +29,7 @@ from __future__ import annotations
 
 import argparse
 import ctypes as C
+import gc
 import json
 import os
 import statistics
@@ -36,6 +45,12 @@ if ROOT not in sys.path:
 
 METRIC = "codec tokens/s (enc+dec fwd+bwd, proj+RVQ+anchor)"
 UNIT = "tokens/s"
+HEADLINE = "c3"
+
+# nominal vendor figures (B200_PROFILING.md): context next to the measured peaks, never the denominator of `frac`
+NOMINAL = dict(hbm_gbs=8000.0, bf16_tflops=2250.0, tf32_tflops=1125.0)
+# FP32 FFMA peak derived from the guide's unit counts and clocks: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz
+FFMA_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 
 
 def _peaks():
@@ -149,6 +164,37 @@ def job_tokens_per_second(tokens_per_rank_step: int, world: int, steps: int, ms:
     return tokens_per_rank_step * world * steps / (ms * 1e-3)
 
 
+def step_time_stats(step_ms):
+    """median / max / min of the per-step device times (one CUDA event per graph replay)."""
+    if not step_ms:
+        return {}
+    return {"median": statistics.median(step_ms), "max": max(step_ms), "min": min(step_ms)}
+
+
+# ---------------------------------------------------------------- graph timing helper
+
+def graph_time_us(torch, stream, fn, reps=1, replays=10):
+    """Capture `reps` consecutive calls of fn() into one CUDA graph on `stream`, replay it `replays` times with one
+    event per replay; returns (median, max) microseconds per call of fn().  Graph replay keeps the programmatic-
+    dependent-launch overlap the step has."""
+    fn()
+    stream.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=stream):
+        for _ in range(reps):
+            fn()
+    g.replay()
+    stream.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(replays + 1)]
+    ev[0].record(stream)
+    for i in range(replays):
+        g.replay()
+        ev[i + 1].record(stream)
+    stream.synchronize()
+    t = [1e3 * ev[i].elapsed_time(ev[i + 1]) / reps for i in range(replays)]
+    return statistics.median(t), max(t)
+
+
 # ---------------------------------------------------------------- the CUDA arm
 
 class Boundary:
@@ -198,144 +244,125 @@ class Boundary:
             self.o_Hhat, self.o_gz, self.o_dH, self.o_dU = ph(self.Hhat), ph(self.gz), ph(self.dH), ph(self.dU)
 
 
-def make_step(bs, mb, stiefel=None):
-    for b in bs:
-        if b.pack is not None:
-            mb.mapl_pack_params(b.desc, b.U, b.B, b.C, b.pack)
+class Arm:
+    """One workload on this rank's GPU: buffers, the step, its CUDA graph and the measurements taken from it."""
 
-    def fwd(b):
-        if b.pack is not None and stiefel is not None:
-            mb.mapl_pack_params(b.desc, b.U, None, None, b.pack)    # U changed (Stiefel step); B and the codebooks did not
-        mb.mapl_encode(b.desc, b.H, b.U, b.C, b.Zq, b.codes, b.ws)
-        mb.mapl_decode(b.desc, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.Hhat, b.ws)
+    def __init__(self, name, rank, torch, mb, I, stream, host=False, tokens=0):
+        self.torch, self.mb, self.stream, self.name = torch, mb, stream, name
+        self.cfg, self.wdesc = workload(name)
+        if tokens:
+            self.cfg = self.cfg.with_tokens(tokens)
+        cfg = self.cfg
+        self.nb = cfg.n_boundaries
+        self.bs = [Boundary(cfg, b, rank, torch, mb, I, host=host) for b in range(self.nb)]
+        self.lib = mb.raw_lib()
+        self.has_stiefel = name == "c3"
+        if self.has_stiefel:
+            # configs[3]: "plus a Stiefel step per boundary".  The nb projectors live in one [nb, d, r] tensor (and
+            # their gradients likewise), so the per-boundary Stiefel steps of a training step are ONE batched
+            # mapl_stiefel_step call.  Reading S12: the step is fed G = dU / N (mean-over-tokens loss); xi is linear
+            # in G, so U - lr xi(dU / N) = U - (lr / N) xi(dU): the scale goes into the step size on the host and
+            # the library consumes dU as it stands (no extra pass over the gradient).
+            self.st_ws = mb.alloc_workspace(mb.mapl_stiefel_workspace_bytes(cfg.d, cfg.r, self.nb))
+            self.Uall = torch.stack([b.U for b in self.bs]).contiguous()
+            self.dUall = torch.empty_like(self.Uall)
+            for i, b in enumerate(self.bs):
+                b.U, b.dU = self.Uall[i], self.dUall[i]
+        for b in self.bs:
+            if b.pack is not None:
+                mb.mapl_pack_params(b.desc, b.U, b.B, b.C, b.pack)
+        self.graph = None
 
-    def bwd(b):
-        mb.mapl_codec_backward(b.desc, b.g, b.H, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.gz, b.dU, b.dA,
-                               None, b.dH, False, b.ws)
+    # ---- the calls
+    def enc(self, b):
+        self.mb.mapl_encode(b.desc, b.H, b.U, b.C, b.Zq, b.codes, b.ws)
 
-    def step():
-        for b in bs:
-            fwd(b)
-        for b in reversed(bs):
-            bwd(b)
-        if stiefel is not None:
-            stiefel()
-    return step
+    def dec(self, b):
+        self.mb.mapl_decode(b.desc, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.Hhat, b.ws)
 
+    def bwd(self, b):
+        self.mb.mapl_codec_backward(b.desc, b.g, b.H, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.gz, b.dU, b.dA,
+                                    None, b.dH, False, b.ws)
 
-def run_mapl(args):
-    import torch
-    import torch.distributed as dist
-    from paper_2606_05484_b200 import binding as mb
-    from paper_2606_05484_b200 import inputs as I
+    def bwd_decode_side(self, b):
+        self.mb.mapl_codec_backward(b.desc, b.g, None, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.gz, b.dU, b.dA,
+                                    None, None, False, b.ws)
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device: there is no CPU path"
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    cfg, wdesc = workload(args.workload)
-    if args.tokens:
-        cfg = cfg.with_tokens(args.tokens)
-    nb = cfg.n_boundaries
-    bs = [Boundary(cfg, b, rank, torch, mb, I, host=True) for b in range(nb)]
-    lib = mb.raw_lib()
+    def stiefel(self):
+        mb = self.mb
+        mb.mapl_stiefel_step(self.Uall, self.dUall, 1e-2 / self.cfg.n_tokens, mb.MAPL_RETRACT_NS, 5, None, self.st_ws)
 
-    stiefel = None
-    if args.workload == "c3":       # configs[3]: "plus a Stiefel step per boundary" (G = dU / N, S12)
-        # the nb projectors live in one [nb, d, r] tensor (and their gradients likewise), so the per-boundary
-        # Stiefel steps of a training step are ONE batched mapl_stiefel_step call (batch = nb)
-        st_ws = mb.alloc_workspace(mb.mapl_stiefel_workspace_bytes(cfg.d, cfg.r, nb))
-        Uall = torch.stack([b.U for b in bs]).contiguous()
-        dUall = torch.empty_like(Uall)
-        Gall = torch.empty_like(Uall)
-        for i, b in enumerate(bs):
-            b.U, b.dU = Uall[i], dUall[i]
+    def step(self):
+        for b in self.bs:
+            if b.pack is not None and self.has_stiefel:
+                self.mb.mapl_pack_params(b.desc, b.U, None, None, b.pack)    # U changed (Stiefel step); B, codebooks did not
+            self.enc(b)
+            self.dec(b)
+        for b in reversed(self.bs):
+            self.bwd(b)
+        if self.has_stiefel:
+            self.stiefel()
 
-        def stiefel():
-            torch.mul(dUall, 1.0 / cfg.n_tokens, out=Gall)
-            mb.mapl_stiefel_step(Uall, Gall, 1e-2, mb.MAPL_RETRACT_NS, 5, None, st_ws)
-    step = make_step(bs, mb, stiefel)
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    stream = torch.cuda.Stream()
-    with torch.cuda.stream(stream):
-        for _ in range(max(3, args.warmup)):
-            step()
+    # ---- measurements (all inside `with torch.cuda.stream(self.stream)`)
+    def prepare(self, warmup):
+        lib, stream, torch = self.lib, self.stream, self.torch
+        for _ in range(max(3, warmup)):
+            self.step()
         stream.synchronize()
-        # count our launches in one step
         lib.mapl_profile_reset()
-        step()
+        self.step()
         stream.synchronize()
-        launches_per_step = 0
+        self.launches_per_step = 0
         for kid in range(lib.mapl_profile_kernel_count()):
             n = C.c_longlong(0)
             lib.mapl_profile_read(kid, C.byref(n), None, None)
-            launches_per_step += n.value
-        # capture the step once, replay K times
-        graph = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(graph, stream=stream):
-            step()
+            self.launches_per_step += n.value
+        self.graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(self.graph, stream=stream):
+            self.step()
         for _ in range(3):
-            graph.replay()
+            self.graph.replay()
         stream.synchronize()
 
-        sampler = ClockSampler(local)
+    def timed_steps(self, steps, barrier, sampler=None):
+        """exactly `steps` graph replays between barrier + synchronize; returns (total ms, per-step ms list)"""
+        torch, stream = self.torch, self.stream
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
         barrier()
-        sampler.start()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        for _ in range(args.steps):
-            graph.replay()
-        e1.record(stream)
+        if sampler:
+            sampler.start()
+        ev[0].record(stream)
+        for i in range(steps):
+            self.graph.replay()
+            ev[i + 1].record(stream)
         stream.synchronize()
         barrier()
-        clocks = sampler.stop()
-        ms = e0.elapsed_time(e1)
+        return ev[0].elapsed_time(ev[steps]), [ev[i].elapsed_time(ev[i + 1]) for i in range(steps)]
 
-        # ---- per-call times: one CUDA graph per entry point (all boundaries, 4 repetitions), replayed 10 times.
-        # Graph replay keeps the programmatic-dependent-launch overlap the step has, unlike the
-        # event-bracketed eager pass below, whose per-kernel times include launch latency.
-        def graph_us(fn, reps=4, replays=10):
-            for b in bs:
-                fn(b)
-            stream.synchronize()
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g, stream=stream):
-                for _ in range(reps):
-                    for b in bs:
-                        fn(b)
-            g.replay()
-            stream.synchronize()
-            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            c0.record(stream)
-            for _ in range(replays):
-                g.replay()
-            c1.record(stream)
-            stream.synchronize()
-            return 1e3 * c0.elapsed_time(c1) / (replays * reps * len(bs))
-        calls_us = {
-            "mapl_encode": graph_us(lambda b: mb.mapl_encode(b.desc, b.H, b.U, b.C, b.Zq, b.codes, b.ws)),
-            "mapl_decode": graph_us(lambda b: mb.mapl_decode(b.desc, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.Hhat, b.ws)),
-            "mapl_codec_backward": graph_us(lambda b: mb.mapl_codec_backward(
-                b.desc, b.g, b.H, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.gz, b.dU, b.dA, None, b.dH, False, b.ws)),
-            # the receiver's share alone (H == NULL: gz, dA and the decode-side term of dU; no dH), reported beside the headline
-            "mapl_codec_backward_decode_side": graph_us(lambda b: mb.mapl_codec_backward(
-                b.desc, b.g, None, b.Zq, b.codes, b.U, b.C, b.tok, b.A, b.B, b.gz, b.dU, b.dA, None, None, False, b.ws)),
-        }
+    def calls_us(self, replays=10):
+        """graph-timed microseconds per call (median over replays; the max is kept in calls_us_max)"""
+        out, mx = {}, {}
+        reps = 4 if self.cfg.n_tokens * self.cfg.d < (1 << 26) else 2
+        for key, fn in (("mapl_encode", self.enc), ("mapl_decode", self.dec), ("mapl_codec_backward", self.bwd),
+                        ("mapl_codec_backward_decode_side", self.bwd_decode_side)):
+            def all_b(fn=fn):
+                for b in self.bs:
+                    fn(b)
+            med, m = graph_time_us(self.torch, self.stream, all_b, reps=reps, replays=replays)
+            out[key], mx[key] = med / self.nb, m / self.nb
+        if self.has_stiefel:
+            out["mapl_stiefel_step(batch=%d)" % self.nb], mx["mapl_stiefel_step(batch=%d)" % self.nb] = \
+                graph_time_us(self.torch, self.stream, self.stiefel, reps=1, replays=replays)
+        return out, mx
 
-        # ---- per-kernel timing pass (same K steps, eager launches, event pair around every kernel)
+    def kernel_pass(self, steps):
+        """same step, eager launches, one CUDA-event pair around every kernel (the library's launch accounting)"""
+        lib = self.lib
         lib.mapl_profile_reset()
         lib.mapl_profile_enable(1)
-        for _ in range(args.steps):
-            step()
-        stream.synchronize()
+        for _ in range(steps):
+            self.step()
+        self.stream.synchronize()
         lib.mapl_profile_enable(0)
         kern = {}
         for kid in range(lib.mapl_profile_kernel_count()):
@@ -343,11 +370,14 @@ def run_mapl(args):
             lib.mapl_profile_read(kid, C.byref(n), C.byref(nt), C.byref(tms))
             if nt.value:
                 kern[lib.mapl_profile_kernel_name(kid).decode()] = dict(launches=nt.value, ms=tms.value)
+        return kern
 
-        # ---- end to end: pinned host inputs -> device, the three calls, results -> pinned host.
-        # Three streams, as a user of the library would drive it: the uploads of step i+1 run while the
-        # results of step i are downloaded (PCIe is full duplex); the codec calls of a step wait for
-        # its uploads and for the previous step's downloads (they overwrite the same device buffers).
+    def e2e(self, steps, barrier):
+        """End to end: pinned host inputs -> device, the step, results -> pinned host.  Three streams, as a user of the
+        library would drive it: the uploads of step i+1 run while the results of step i are downloaded (PCIe is full
+        duplex); the codec calls of a step wait for its uploads and for the previous step's downloads (they overwrite
+        the same device buffers)."""
+        torch, stream, bs = self.torch, self.stream, self.bs
         s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
         ev_in, ev_done, ev_out = torch.cuda.Event(), torch.cuda.Event(), torch.cuda.Event()
         ev_done.record(stream)
@@ -363,7 +393,7 @@ def run_mapl(args):
                 ev_in.record(s_in)
             stream.wait_event(ev_in)
             stream.wait_event(ev_out)                      # the previous results have left the device
-            step()
+            self.step()
             ev_done.record(stream)
             s_out.wait_event(ev_done)
             with torch.cuda.stream(s_out):
@@ -377,76 +407,191 @@ def run_mapl(args):
         nbytes = lambda t: t.numel() * t.element_size()
         h2d = sum(nbytes(b.hH) + nbytes(b.htok) + nbytes(b.hg) for b in bs)
         d2h = sum(nbytes(b.o_payload) + nbytes(b.o_Hhat) + nbytes(b.o_gz) + nbytes(b.o_dH) + nbytes(b.o_dU) for b in bs)
-        e2e_steps = max(1, min(args.steps, 20))
         for _ in range(2):
             e2e_step()
         stream.wait_event(ev_out)
         barrier()
         f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         f0.record(stream)
-        for _ in range(e2e_steps):
+        for _ in range(steps):
             e2e_step()
         stream.wait_event(ev_out)                          # the last results are in host memory
         f1.record(stream)
         stream.synchronize()
         barrier()
-        e2e_ms = f0.elapsed_time(f1)
+        return f0.elapsed_time(f1), h2d, d2h
 
-    ms, e2e_ms = max_over_ranks([ms, e2e_ms], world, "cuda")
-    value = job_tokens_per_second(cfg.n_tokens * nb, world, args.steps, ms)
-    e2e_value = job_tokens_per_second(cfg.n_tokens * nb, world, e2e_steps, e2e_ms)
+    def free(self):
+        self.graph = None
+        self.bs = []
+        for a in ("Uall", "dUall", "st_ws"):
+            if hasattr(self, a):
+                delattr(self, a)
+        gc.collect()
+        self.torch.cuda.empty_cache()
 
-    # ---- roofline of the dominant kernel (largest share of the timed per-kernel pass)
+
+def config_report(arm, peaks, steps, barrier, kernel_steps):
+    """per-config measurements shared by the headline and the per_config entries"""
+    total_ms, step_ms = arm.timed_steps(steps, barrier)
+    calls, calls_max = arm.calls_us()
+    kern = arm.kernel_pass(kernel_steps)
+    cfg = arm.cfg
+    rep = {
+        "workload": arm.wdesc,
+        "ms_per_step": total_ms / steps,
+        "ms_per_step_stats": {k: round(v, 5) for k, v in step_time_stats(step_ms).items()},
+        "tokens_per_s": cfg.n_tokens * arm.nb * steps / (total_ms * 1e-3),
+        "calls_us": {k: round(v, 2) for k, v in calls.items()},
+        "calls_us_max": {k: round(v, 2) for k, v in calls_max.items()},
+        "roofline_step": roofline_step(cfg, peaks, calls),
+        "roofline": dominant_roofline(kern, cfg, peaks),
+        "gpu_launches_per_step": arm.launches_per_step,
+    }
+    return rep, total_ms, step_ms
+
+
+def run_mapl(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_05484_b200 import binding as mb
+    from paper_2606_05484_b200 import inputs as I
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: there is no CPU path"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peaks = _peaks()
-    roof = None
-    if kern:
-        top = max(kern, key=lambda k: kern[k]["ms"])
-        total = sum(v["ms"] for v in kern.values())
-        roof = roofline_for(top, kern[top], cfg, peaks, total)
-        roof["kernels"] = {k: {"launches": v["launches"], "avg_us": round(1e3 * v["ms"] / v["launches"], 2),
-                               "share": round(v["ms"] / total, 3)} for k, v in sorted(kern.items(), key=lambda kv: -kv[1]["ms"])}
+    headline = HEADLINE if args.workload == "all" else args.workload
+    solo = rank == 0 and world == 1          # everything beside the headline runs on a single-GPU invocation only
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    stream = torch.cuda.Stream()
+    per_config = {}
+    with torch.cuda.stream(stream):
+        # ---- the companion configs first (their buffers are freed before the headline allocates)
+        if args.workload == "all" and solo and not args.no_per_config:
+            for name in ("c1", "c2"):
+                arm = Arm(name, rank, torch, mb, I, stream)
+                arm.prepare(args.warmup)
+                per_config[name], _, _ = config_report(arm, peaks, args.steps, barrier, min(args.steps, 20))
+                arm.free()
+        c0 = None
+        if args.workload == "all" and solo and not args.no_per_config:
+            arm = Arm("c0", rank, torch, mb, I, stream)
+            arm.prepare(args.warmup)
+            t_ms, st = arm.timed_steps(args.steps, barrier)
+            calls, calls_max = arm.calls_us()
+            c0 = {"workload": arm.wdesc + " + one Stiefel step (separately timed below)", "ms_per_step": t_ms / args.steps,
+                  "calls_us": {k: round(v, 2) for k, v in calls.items()},
+                  "note": "4 MB working set: L2-resident, t_roof ~ 2.7 us ~ launch latency; times only (BASELINE.md section 3)"}
+            s0 = I.make_stiefel(arm.cfg.r, d=arm.cfg.d, batch=1)
+            U0 = torch.from_numpy(s0.U.data.copy()).cuda()
+            G0 = torch.from_numpy(s0.G.data.copy()).cuda()
+            ws0 = mb.alloc_workspace(mb.mapl_stiefel_workspace_bytes(arm.cfg.d, arm.cfg.r, 1))
+            for retr, tag in ((mb.MAPL_RETRACT_NS, "ns5"), (mb.MAPL_RETRACT_QR, "qr")):
+                med, _ = graph_time_us(torch, stream, lambda: mb.mapl_stiefel_step(U0, G0, 1e-2, retr, 5, None, ws0))
+                c0["calls_us"][f"mapl_stiefel_step_{tag}"] = round(med, 2)
+            arm.free()
+
+        # ---- the headline
+        arm = Arm(headline, rank, torch, mb, I, stream, host=not args.no_e2e, tokens=args.tokens)
+        cfg, nb = arm.cfg, arm.nb
+        arm.prepare(args.warmup)
+        sampler = ClockSampler(local)
+        total_ms, step_ms = arm.timed_steps(args.steps, barrier, sampler)
+        clocks = sampler.stop()
+        calls, calls_max = arm.calls_us()
+        kern = arm.kernel_pass(min(args.steps, 20))
+        e2e_steps = max(1, min(args.steps, 20))
+        if args.no_e2e:
+            e2e_ms, h2d, d2h = float("nan"), 0, 0
+        else:
+            e2e_ms, h2d, d2h = arm.e2e(e2e_steps, barrier)
+        head_rep = {
+            "workload": arm.wdesc, "ms_per_step": total_ms / args.steps,
+            "ms_per_step_stats": {k: round(v, 5) for k, v in step_time_stats(step_ms).items()},
+            "tokens_per_s": cfg.n_tokens * nb * args.steps / (total_ms * 1e-3),
+            "calls_us": {k: round(v, 2) for k, v in calls.items()},
+            "calls_us_max": {k: round(v, 2) for k, v in calls_max.items()},
+            "roofline_step": roofline_step(cfg, peaks, calls),
+            "roofline": dominant_roofline(kern, cfg, peaks),
+            "gpu_launches_per_step": arm.launches_per_step,
+        }
+        per_config[headline] = head_rep
+        launches_per_step = arm.launches_per_step
+        extras = {}
+        if solo and not args.no_stiefel:
+            extras["centering"] = centering_times(torch, mb, arm.bs[0], cfg, stream)
+        arm.free()
+        if solo and not args.no_stiefel:
+            extras["stiefel"] = stiefel_sweep(torch, mb, I, stream, peaks, track_steps=args.track_steps,
+                                              oracle=not args.no_cpu_baseline)
+
+    total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms if e2e_ms == e2e_ms else 0.0], world, "cuda")
+    value = job_tokens_per_second(cfg.n_tokens * nb, world, args.steps, total_ms)
+    e2e_value = job_tokens_per_second(cfg.n_tokens * nb, world, e2e_steps, e2e_ms) if e2e_ms > 0 else None
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": cfg.act_dtype, "data": "synthetic",
-        "config": {"workload": wdesc, "l2": "distinct buffers per boundary; per-step working set > 126 MB L2, no flush",
-                   "launch": "one CUDA graph of the step, replayed K times",
-                   "param_pack": ("rebuilt per boundary per step (U changes every step)" if stiefel is not None
-                                  else "built once before the timed region (parameters constant across steps)"), "parallelism": f"replicas x{world}"},
+        "config": {"workload": arm.wdesc, "l2": "distinct buffers per boundary; per-step working set > 126 MB L2, no flush",
+                   "launch": "one CUDA graph of the step, replayed K times, one CUDA event per replay",
+                   "param_pack": ("rebuilt per boundary per step (U changes every step)" if arm.has_stiefel
+                                  else "built once before the timed region (parameters constant across steps)"),
+                   "parallelism": f"replicas x{world}"},
         "clocks": clocks,
+        "ms_per_step_stats": head_rep["ms_per_step_stats"],
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "note": "pinned host H,tok,g -> device; payload,Hhat,gz,dH,dU -> pinned host; uploads of step i+1 overlap downloads of step i (3 streams)"},
-        "roofline_step": roofline_step(cfg, peaks, ms / args.steps, nb, calls_us),
+        "roofline_step": head_rep["roofline_step"],
         "gpu_launches": launches_per_step * args.steps,
-        "calls_us": {k: round(v, 2) for k, v in calls_us.items()},
-        "roofline": roof,
+        "calls_us": head_rep["calls_us"],
+        "roofline": head_rep["roofline"],
+        "per_config": per_config,
     }
-    if rank == 0 and world == 1 and not args.no_stiefel:
-        out["stiefel"] = stiefel_sweep(torch, mb, I, stream, track_steps=args.track_steps)
-    if rank == 0 and world == 1 and not args.no_stiefel:
-        out["centering"] = centering_times(torch, mb, bs[0], cfg, stream)
+    if c0 is not None:
+        out["c0"] = c0
+    out.update(extras)
     if rank == 0:
-        if not args.no_cpu_baseline and world >= 1:
+        if not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(cfg, budget_s=args.cpu_budget)
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
 
 
-def _stiefel_track(torch, mb, s, r, retr, ws, stream, n_steps):
+# ---------------------------------------------------------------- configs[4]: the Stiefel sweep
+
+def stiefel_alg_flops(d, r, tag):
+    """Algorithmic flops of one projector step (SURVEY 8(d)): tangent projection 4 d r^2 (S = U^T G, U sym(S));
+    NS-5: 5 x (Gram 2 d r^2 + right-multiply 2 d r^2) = 20 d r^2; QR (CholeskyQR count): 3 d r^2 + r^3 / 3."""
+    return 4 * d * r * r + (20 * d * r * r if tag == "ns5" else 3 * d * r * r + r ** 3 / 3.0)
+
+
+def _stiefel_track(torch, mb, s, r, retr, ws, stream, n_steps, marks_restart):
     """configs[4]: `n_steps` consecutive steps with ||U^T U - I||_F tracked -- on the device by the library every step
     (info_out, fp32 Gram: its maximum over the run) and in fp64 (torch) at steps 1, 2, 10, 100, 500, 1000 -- for the
     fixed seeded gradient and for a fresh Gaussian gradient every step (reading S13; drawn by torch's seeded device
-    generator: an input, not part of the method).  Maximum over the 3 projectors."""
+    generator: an input, not part of the method).  Maximum over the 3 projectors.  For the fixed-G run the state
+    before and after step t+1, t in marks_restart, is kept (projector 0) for the oracle's one-step restarts."""
     marks = [m for m in (1, 2, 10, 100, 500, 1000) if m <= n_steps]
     eye = torch.eye(r, device="cuda", dtype=torch.float64)
-    res = {}
+    res, snaps = {}, {}
     for variant in ("fixed_G", "fresh_G"):
         U = torch.from_numpy(s.U.data.copy()).cuda()
         G = torch.from_numpy(s.G.data.copy()).cuda()
         info = torch.zeros(s.batch, 2, device="cuda", dtype=torch.float32)
-        log = torch.zeros(n_steps, device="cuda", dtype=torch.float32)
+        n_run = n_steps + (1 if (variant == "fixed_G" and marks_restart) else 0)
+        log = torch.zeros(n_run, device="cuda", dtype=torch.float32)
         gen = torch.Generator(device="cuda")
         gen.manual_seed(260605484 + r)
         mb.mapl_stiefel_step(U, G, 1e-2, retr, 5, info, ws)
@@ -457,54 +602,92 @@ def _stiefel_track(torch, mb, s, r, retr, ws, stream, n_steps):
             mb.mapl_stiefel_step(U, G, 1e-2, retr, 5, info, ws)
         U.copy_(torch.from_numpy(s.U.data.copy()))
         at = {}
-        for t in range(1, n_steps + 1):
+        for t in range(1, n_run + 1):
             if variant == "fresh_G":
                 G.normal_(generator=gen)
+            if variant == "fixed_G" and (t - 1) in marks_restart:
+                snaps[t - 1] = [U[0].clone()]
             g.replay()
+            if variant == "fixed_G" and (t - 1) in marks_restart:
+                snaps[t - 1].append(U[0].clone())
             log[t - 1] = info[:, 1].max()
             if t in marks:
                 Uh = U.double()
                 at[str(t)] = float(f"{float(max(torch.linalg.matrix_norm(Uh[b].T @ Uh[b] - eye) for b in range(s.batch))):.2e}")
         stream.synchronize()
         res[variant] = {"residual_fp64_at_step": at, "max_device_residual": float(f"{float(log.max()):.2e}"), "steps": n_steps}
-    return res
+    return res, snaps
 
 
-def stiefel_sweep(torch, mb, I, stream, reps=10, track_steps=1000):
+def _stiefel_oracle(s, r, retr_o, snaps, n_first):
+    """SURVEY 8(d) 'Oracle timing': the fp64 oracle steps 1..n_first from the common start (projector 0) plus single
+    steps restarted from the GPU's U_t at the kept marks; its time per step is the mean of those.  The restarts double
+    as one-step parity late in the run: relative Frobenius error of the GPU's U_{t+1} against the oracle's step from
+    the same U_t."""
+    from oracle import mapl_oracle as o
+    U = s.U.f64[0].copy()
+    G = s.G.f64[0]
+    times = []
+    for _ in range(n_first):
+        t0 = time.perf_counter()
+        U, _info = o.stiefel_step(U, G, 1e-2, retr_o, 5)
+        times.append(time.perf_counter() - t0)
+    parity = {}
+    for t, (Ut, Ut1) in sorted(snaps.items()):
+        Ut64 = Ut.double().cpu().numpy()
+        t0 = time.perf_counter()
+        Uo, _info = o.stiefel_step(Ut64, G, 1e-2, retr_o, 5)
+        times.append(time.perf_counter() - t0)
+        got = Ut1.double().cpu().numpy()
+        parity[str(t)] = float(f"{np.linalg.norm(got - Uo) / np.linalg.norm(Uo):.2e}")
+    return {"s_per_step": round(sum(times) / len(times), 4), "projector_steps_per_s": round(len(times) / sum(times), 3),
+            "cores": o.threads(), "kind": "oracle",
+            "sample": f"projector 0: steps 1-{n_first} from the seeded start + one-step restarts from the GPU's U_t at t = "
+                      f"{sorted(snaps)} (fp64)",
+            "one_step_rel_err_vs_oracle_at_t": parity}
+
+
+def stiefel_sweep(torch, mb, I, stream, peaks, track_steps=1000, oracle=True):
     """BASELINE.json configs[4] beside the codec metric: Stiefel steps/s for the 3 projectors of d=2048,
     r in {64,128,256,512}, QR (CholeskyQR2) and 5 Newton-Schulz iterations; one CUDA graph per variant.
     A step = one mapl_stiefel_step call over the batch of 3; projector-steps/s = 3 x that.
+    `roofline`: algorithmic flops (stiefel_alg_flops) / time against (a) the fp32-accurate tensor peak = measured bf16
+    peak x the guide's nominal TF32 / bf16 ratio (1.1 / 2.25: the contraction must be fp32-accurate and TF32 is the
+    nearest dense tensor mode the guide lists) and (b) the FP32 FFMA peak (148 x 128 x 2 x 1.965 GHz = 74.4 TFLOP/s:
+    the pipe the r < 256 kernels run on).
     `track`: the variant repeated for track_steps steps from the seeded start, with the orthogonality residual
-    tracked (see _stiefel_track)."""
+    tracked (see _stiefel_track); `oracle`: the fp64 oracle's time per step and one-step parity at t = 100/500/1000."""
+    from oracle import mapl_oracle as o
     out = {}
+    tf32_peak = peaks["bf16"] * NOMINAL["tf32_tflops"] / NOMINAL["bf16_tflops"]
     with torch.cuda.stream(stream):
         for r in (64, 128, 256, 512):
             s = I.make_stiefel(r)
             ws = mb.alloc_workspace(mb.mapl_stiefel_workspace_bytes(s.d, r, s.batch))
-            for retr, tag in ((mb.MAPL_RETRACT_NS, "ns5"), (mb.MAPL_RETRACT_QR, "qr")):
+            for retr, tag, retr_o in ((mb.MAPL_RETRACT_NS, "ns5", o.RETRACT_NS), (mb.MAPL_RETRACT_QR, "qr", o.RETRACT_QR)):
                 U = torch.from_numpy(s.U.data.copy()).cuda()
                 G = torch.from_numpy(s.G.data.copy()).cuda()
-                f = lambda: mb.mapl_stiefel_step(U, G, 1e-2, retr, 5, None, ws)
-                f()
-                stream.synchronize()
-                g = torch.cuda.CUDAGraph()
-                with torch.cuda.graph(g, stream=stream):
-                    f()
-                g.replay()
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record(stream)
-                for _ in range(reps):
-                    g.replay()
-                e1.record(stream)
-                stream.synchronize()
-                us = 1e3 * e0.elapsed_time(e1) / reps
+                us, us_max = graph_time_us(torch, stream, lambda: mb.mapl_stiefel_step(U, G, 1e-2, retr, 5, None, ws))
                 Uh = U.double()
                 res = float(max(torch.linalg.matrix_norm(Uh[b].T @ Uh[b] - torch.eye(r, device="cuda", dtype=torch.float64))
                                 for b in range(s.batch)))
-                out[f"r{r}_{tag}"] = {"us_per_step": round(us, 1), "projector_steps_per_s": round(s.batch * 1e6 / us),
-                                      "orth_residual_after": float(f"{res:.2e}")}
+                tfl = s.batch * stiefel_alg_flops(s.d, r, tag) / (us * 1e-6) / 1e12
+                ent = {"us_per_step": round(us, 1), "us_per_step_max": round(us_max, 1),
+                       "projector_steps_per_s": round(s.batch * 1e6 / us),
+                       "orth_residual_after": float(f"{res:.2e}"),
+                       "roofline": {"bound": "tensor" if r >= 256 else "alu", "achieved": round(tfl, 2), "unit": "TFLOP/s",
+                                    "peak": round(tf32_peak if r >= 256 else FFMA_TFLOPS, 1),
+                                    "frac": round(tfl / (tf32_peak if r >= 256 else FFMA_TFLOPS), 4),
+                                    "frac_of_tf32_equiv_tensor": round(tfl / tf32_peak, 4),
+                                    "frac_of_fp32_ffma": round(tfl / FFMA_TFLOPS, 4),
+                                    "alg_flops_per_step": s.batch * stiefel_alg_flops(s.d, r, tag)}}
+                snaps = {}
                 if track_steps:
-                    out[f"r{r}_{tag}"]["track"] = _stiefel_track(torch, mb, s, r, retr, ws, stream, track_steps)
+                    marks_restart = [m for m in (100, 500, 1000) if m <= track_steps] if oracle else []
+                    ent["track"], snaps = _stiefel_track(torch, mb, s, r, retr, ws, stream, track_steps, marks_restart)
+                if oracle:
+                    ent["oracle"] = _stiefel_oracle(s, r, retr_o, snaps, 10 if r <= 256 else 4)
+                out[f"r{r}_{tag}"] = ent
     # full SPEL update (Eq. 4-7: tangent projection, momentum 0.95, 5 + 7 Newton-Schulz iterations), SURVEY 8f next row 2
     with torch.cuda.stream(stream):
         for r in (64, 128, 256, 512):
@@ -513,20 +696,7 @@ def stiefel_sweep(torch, mb, I, stream, reps=10, track_steps=1000):
             U = torch.from_numpy(s.U.data.copy()).cuda()
             G = torch.from_numpy(s.G.data.copy()).cuda()
             Mom = torch.zeros_like(U)
-            f = lambda: mb.mapl_spel_step(U, G, Mom, 2e-3, 0.95, 5, 7, ws)
-            f()
-            stream.synchronize()
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g, stream=stream):
-                f()
-            g.replay()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            for _ in range(reps):
-                g.replay()
-            e1.record(stream)
-            stream.synchronize()
-            us = 1e3 * e0.elapsed_time(e1) / reps
+            us, _ = graph_time_us(torch, stream, lambda: mb.mapl_spel_step(U, G, Mom, 2e-3, 0.95, 5, 7, ws))
             Uh = U.double()
             res = float(max(torch.linalg.matrix_norm(Uh[b].T @ Uh[b] - torch.eye(r, device="cuda", dtype=torch.float64))
                             for b in range(s.batch)))
@@ -538,148 +708,128 @@ def stiefel_sweep(torch, mb, I, stream, reps=10, track_steps=1000):
     return out
 
 
-def centering_times(torch, mb, b, cfg, stream, reps=10):
-    """SURVEY 8f next row 1 (Eq. 1 in full), measured beside the hot path on boundary 0 of the workload:
-    mapl_center_table (once per parameter update), mapl_encode_centered (per micro-batch; compare calls_us.mapl_encode)
-    and mapl_center_backward.  The sender's anchor factors are the boundary's A, B.  Graph-timed, us per call."""
+def centering_times(torch, mb, b, cfg, stream):
+    """SURVEY 8f next rows, measured beside the hot path on boundary 0 of the headline workload (graph-timed, us per call):
+    mapl_center_table (once per parameter update), mapl_encode_centered (per micro-batch; compare calls_us.mapl_encode),
+    mapl_center_backward; grouped MCVQ (G=2, K=256, R=2) of the [N,r] payload; the retained-energy diagnostic and one
+    micro-batch's codebook delta.  The sender's anchor factors are the boundary's A, B."""
     T = torch.empty((cfg.vocab, cfg.r), dtype=torch.float32, device="cuda")
     cws = mb.alloc_workspace(mb.mapl_center_workspace_bytes(b.desc))
     bws = mb.alloc_workspace(mb.mapl_center_backward_workspace_bytes(b.desc))
     dA = torch.empty_like(b.A)
     dU = torch.zeros_like(b.dU)
-    fns = {
-        "mapl_center_table": lambda: mb.mapl_center_table(b.desc, b.A, b.B, b.U, T, cws),
-        "mapl_encode_centered": lambda: mb.mapl_encode_centered(b.desc, b.H, b.tok, T, b.U, b.C, b.Zq, b.codes, b.ws),
-        "mapl_center_backward": lambda: mb.mapl_center_backward(b.desc, b.gz, b.tok, b.A, b.B, b.U, dA, None, dU, False, bws),
-    }
-    out = {}
-    with torch.cuda.stream(stream):
-        for name, f in fns.items():
-            f()
-            stream.synchronize()
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g, stream=stream):
-                f()
-            g.replay()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            for _ in range(reps):
-                g.replay()
-            e1.record(stream)
-            stream.synchronize()
-            out[name] = round(1e3 * e0.elapsed_time(e1) / reps, 2)
-    # SURVEY 8f next row 3: grouped MCVQ (G=2, K=256, R=2) of the workload's [N,r] payload (gz of boundary 0)
     gen = torch.Generator(device="cuda").manual_seed(3)
     Cb = torch.randn((2, 256, cfg.r), device="cuda", generator=gen) * torch.tensor([1.0, 0.4], device="cuda")[:, None, None]
     codes8 = torch.empty((cfg.n_tokens, 2, cfg.r // 2), dtype=torch.uint8, device="cuda")
     Xq = torch.empty_like(b.gz)
-    fns2 = {
-        "mapl_mcvq_quantize": lambda: mb.mapl_mcvq_quantize(b.gz, Cb, codes8, None),
-        "mapl_mcvq_dequantize": lambda: mb.mapl_mcvq_dequantize(codes8, Cb, Xq),
-    }
-    with torch.cuda.stream(stream):
-        for name, f in fns2.items():
-            f()
-            stream.synchronize()
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g, stream=stream):
-                f()
-            g.replay()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            for _ in range(reps):
-                g.replay()
-            e1.record(stream)
-            stream.synchronize()
-            out[name] = round(1e3 * e0.elapsed_time(e1) / reps, 2)
-    out["mcvq_bytes_per_token"] = cfg.r  # (r/2) groups x 2 rounds x 1 byte
-    # SURVEY 8f next row 4: retained-energy diagnostic (Fig. 4b) and one micro-batch's codebook delta (a fifth of 2 x 256 rows)
     sums = torch.zeros(2, dtype=torch.float64, device="cuda")
     Zp = b.Zq if b.Zq is not None else b.gz
     idx = torch.arange(0, 512, 5, dtype=torch.int32, device="cuda")
     rows = torch.empty((idx.numel(), cfg.r), dtype=torch.float32, device="cuda")
-    fns3 = {
+    fns = {
+        "mapl_center_table": lambda: mb.mapl_center_table(b.desc, b.A, b.B, b.U, T, cws),
+        "mapl_encode_centered": lambda: mb.mapl_encode_centered(b.desc, b.H, b.tok, T, b.U, b.C, b.Zq, b.codes, b.ws),
+        "mapl_center_backward": lambda: mb.mapl_center_backward(b.desc, b.gz, b.tok, b.A, b.B, b.U, dA, None, dU, False, bws),
+        "mapl_mcvq_quantize": lambda: mb.mapl_mcvq_quantize(b.gz, Cb, codes8, None),
+        "mapl_mcvq_dequantize": lambda: mb.mapl_mcvq_dequantize(codes8, Cb, Xq),
         "mapl_energy_retained": lambda: mb.mapl_energy_retained(b.H, Zp, sums),
         "mapl_codebook_delta_pack+apply": lambda: (mb.mapl_codebook_delta_pack(Cb, idx, rows), mb.mapl_codebook_delta_apply(Cb, idx, rows)),
     }
+    out = {}
     with torch.cuda.stream(stream):
-        for name, f in fns3.items():
-            f()
-            stream.synchronize()
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g, stream=stream):
-                f()
-            g.replay()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            for _ in range(reps):
-                g.replay()
-            e1.record(stream)
-            stream.synchronize()
-            out[name] = round(1e3 * e0.elapsed_time(e1) / reps, 2)
-    out["note"] = "us per call, boundary 0; not part of the codec metric"
+        for name, f in fns.items():
+            out[name] = round(graph_time_us(torch, stream, f)[0], 2)
+    out["mcvq_bytes_per_token"] = cfg.r  # (r/2) groups x 2 rounds x 1 byte
+    out["note"] = f"us per call, boundary 0 of {cfg.name}; not part of the codec metric"
     return out
 
 
-def roofline_step(cfg, peaks, ms_per_step, nb, calls_us):
+# ---------------------------------------------------------------- rooflines
+
+def roofline_step(cfg, peaks, calls_us):
     """Whole-config roofline: t_roof = sum over the three calls of max(bytes/peak_HBM, flops/peak_bf16),
     per boundary; `frac` compares it with the graph-timed codec time of a boundary (Stiefel step excluded)."""
     ab, af = alg_bytes_per_token(cfg), alg_flops_per_token(cfg)
     N = cfg.n_tokens
-    t = {}
+    t, bound = {}, {}
     for call in ("encode", "decode", "backward"):
-        t[call] = 1e6 * max(ab[call] * N / (peaks["hbm"] * 1e9), af[call] * N / (peaks["bf16"] * 1e12))
-    codec_us = sum(calls_us[k] for k in ("mapl_encode", "mapl_decode", "mapl_codec_backward"))
+        th, tt = ab[call] * N / (peaks["hbm"] * 1e9), af[call] * N / (peaks["bf16"] * 1e12)
+        t[call] = 1e6 * max(th, tt)
+        bound[call] = "hbm" if th >= tt else "tensor"
+    key = {"encode": "mapl_encode", "decode": "mapl_decode", "backward": "mapl_codec_backward"}
+    codec_us = sum(calls_us[key[c]] for c in key)
     # the same sum against the vendor's nominal peaks (8 TB/s HBM3e, 2.25 PFLOP/s dense bf16): context, SURVEY 8(d)
-    t_nom = sum(1e6 * max(ab[c] * N / 8000e9, af[c] * N / 2250e12) for c in ("encode", "decode", "backward"))
+    t_nom = sum(1e6 * max(ab[c] * N / (NOMINAL["hbm_gbs"] * 1e9), af[c] * N / (NOMINAL["bf16_tflops"] * 1e12)) for c in key)
     return {"t_roof_us_per_boundary": round(sum(t.values()), 2), "per_call_us": {k: round(v, 2) for k, v in t.items()},
+            "per_call_bound": bound, "per_call_frac": {c: round(t[c] / calls_us[key[c]], 3) for c in key},
             "measured_us_per_boundary": round(codec_us, 2), "frac": round(sum(t.values()) / codec_us, 3),
             "peaks": {"hbm_gbs": peaks["hbm"], "bf16_tflops": peaks["bf16"], "source": peaks["src"]},
             "nominal": {"t_roof_us_per_boundary": round(t_nom, 2), "frac": round(t_nom / codec_us, 3),
-                        "hbm_gbs": 8000, "bf16_tflops": 2250}}
+                        "hbm_gbs": NOMINAL["hbm_gbs"], "bf16_tflops": NOMINAL["bf16_tflops"]}}
 
 
-def roofline_for(name, k, cfg, peaks, total_ms):
-    """achieved = algorithmic bytes (or flops) of one launch / its measured average duration."""
+def kernel_alg_work(name, cfg):
+    """(bytes, flops) one launch of a codec kernel must move / compute: the algorithmic work of its call (DESIGN.md
+    section 5), split between the two backward kernels so that every stream is counted once per CALL: g is read (and
+    counted) by k_tc_bwd_gz; k_tc_bwd_du re-reads it from L2 and owns the H, payload and gz-read streams."""
     N = cfg.n_tokens
+    s = 2 if cfg.act_dtype == "bf16" else 4
     ab, af = alg_bytes_per_token(cfg), alg_flops_per_token(cfg)
-    avg_s = 1e-3 * k["ms"] / k["launches"]
-    # which call the kernel belongs to and the share of that call's algorithmic work it carries
     call = {"k_tc_encode": "encode", "k_tc_encode_rvq": "encode", "k_simt_encode_rvq": "encode",
             "k_tc_decode": "decode", "k_tc_bwd_gz": "backward", "k_tc_bwd_du": "backward"}.get(name)
-    traffic = None
+    if call is None:
+        return None
+    byt, flo = ab[call] * N, af[call] * N
+    payload = cfg.r * s if cfg.rvq_levels == 0 else 4 * cfg.rvq_levels
+    if name == "k_tc_bwd_gz":     # reads g, tok; writes gz, dH
+        byt = (2 * cfg.d * s + cfg.r * s + 4) * N
+        flo = (4 * cfg.d * cfg.r + 2 * cfg.d * cfg.anchor_rank) * N
+    if name == "k_tc_bwd_du":     # reads H, the payload; (g again: from L2, not counted twice)
+        byt = (cfg.d * s + payload) * N
+        flo = 4 * cfg.d * cfg.r * N
+    return byt, flo
+
+
+def _traffic(cfg_name, kernel):
     tpath = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tpath):
         for line in open(tpath).read().splitlines()[1:]:
-            wl, kern_name, nbytes = line.split(",")
-            if wl == cfg.name and kern_name == name:
-                traffic = int(nbytes)
-    if call is None:
+            f = line.split(",")
+            if len(f) >= 3 and f[0] == cfg_name and f[1] == kernel:
+                return int(f[2])
+    return None
+
+
+def dominant_roofline(kern, cfg, peaks):
+    """roofline of the kernel with the largest share of the eager per-kernel pass:
+    achieved = algorithmic bytes (or flops) of one launch / its measured average CUDA-event duration."""
+    if not kern:
+        return None
+    total = sum(v["ms"] for v in kern.values())
+    codec = {k: v for k, v in kern.items() if kernel_alg_work(k, cfg) is not None}
+    name = max(codec or kern, key=lambda k: kern[k]["ms"])
+    k = kern[name]
+    avg_s = 1e-3 * k["ms"] / k["launches"]
+    kernels = {kk: {"launches": v["launches"], "avg_us": round(1e3 * v["ms"] / v["launches"], 2),
+                    "share": round(v["ms"] / total, 3)} for kk, v in sorted(kern.items(), key=lambda kv: -kv[1]["ms"])}
+    work = kernel_alg_work(name, cfg)
+    traffic = _traffic(cfg.name, name)
+    if work is None:
         return {"kernel": name, "bound": "hbm", "achieved": None, "peak": peaks["hbm"], "unit": "GB/s", "frac": None,
-                "traffic": traffic, "note": "generic kernel shared by several calls; see kernels"}
-    byt, flo = ab[call] * N, af[call] * N
-    if name == "k_tc_bwd_gz":     # reads g, tok, writes gz, dH  (H and payload are read by k_tc_bwd_du)
-        s = 2 if cfg.act_dtype == "bf16" else 4
-        byt = (2 * cfg.d * s + cfg.r * s + 4) * N
-        flo = (4 * cfg.d * cfg.r + 2 * cfg.d * cfg.anchor_rank) * N
-    if name == "k_tc_bwd_du":
-        s = 2 if cfg.act_dtype == "bf16" else 4
-        byt = (2 * cfg.d * s + 2 * cfg.r * s) * N
-        flo = 4 * cfg.d * cfg.r * N
+                "traffic": traffic, "kernels": kernels}
+    byt, flo = work
     t_hbm, t_tc = byt / (peaks["hbm"] * 1e9), flo / (peaks["bf16"] * 1e12)
+    note = ("avg_us is event-bracketed per launch in an eager pass (no dependent-launch overlap, a few us of launch latency "
+            "inside the pair): a lower bound on frac; calls_us / roofline_step are graph-timed")
     if t_hbm >= t_tc:
         ach = byt / avg_s / 1e9
         return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": peaks["hbm"], "unit": "GB/s",
                 "frac": ach / peaks["hbm"], "traffic": traffic, "peak_source": peaks["src"] + " (burst copy)",
-                "avg_us": avg_s * 1e6, "alg_bytes_per_launch": byt,
-                "note": "avg_us is event-bracketed per launch (no dependent-launch overlap, ~5 us of launch latency "
-                        "inside the pair): a lower bound on frac; calls_us / roofline_step are graph-timed"}
+                "avg_us": avg_s * 1e6, "alg_bytes_per_launch": byt, "note": note, "kernels": kernels}
     ach = flo / avg_s / 1e12
     return {"kernel": name, "bound": "tensor", "achieved": ach, "peak": peaks["bf16"], "unit": "TFLOP/s",
             "frac": ach / peaks["bf16"], "traffic": traffic, "peak_source": peaks["src"] + " (burst bf16)",
-            "avg_us": avg_s * 1e6, "alg_flops_per_launch": flo,
-            "note": "avg_us is event-bracketed per launch (no dependent-launch overlap): a lower bound on frac; "
-                    "calls_us / roofline_step are graph-timed"}
+            "avg_us": avg_s * 1e6, "alg_flops_per_launch": flo, "note": note, "kernels": kernels}
 
 
 # ---------------------------------------------------------------- the oracle arm (CPU baseline)
@@ -706,8 +856,8 @@ def cpu_baseline(cfg, budget_s=20.0, sample_tokens=None):
     if sample_tokens:
         dt = _oracle_pass(cfg, sample_tokens, 0)
         return {"value": sample_tokens / dt, "unit": UNIT, "cores": o.threads(), "kind": "oracle",
-                "sample": f"{sample_tokens} contiguous tokens of boundary 0 (enc+dec+bwd, fp64), {dt:.1f} s"}
-    n = min(cfg.n_tokens, 512)
+                "sample": f"{sample_tokens} contiguous tokens of boundary 0 of {cfg.name} (enc+dec+bwd, fp64), {dt:.1f} s"}
+    n = min(cfg.n_tokens, 256)
     dt = _oracle_pass(cfg, n, 0)                                   # sizing probe, not counted
     n = int(min(cfg.n_tokens, max(n, n * (budget_s / 4) / max(dt, 1e-3))))
     t_used, tokens, passes = 0.0, 0, 0
@@ -716,19 +866,19 @@ def cpu_baseline(cfg, budget_s=20.0, sample_tokens=None):
         tokens += n
         passes += 1
     return {"value": tokens / t_used, "unit": UNIT, "cores": o.threads(), "kind": "oracle",
-            "sample": f"{passes} passes of {n} contiguous tokens over the workload's boundaries (enc+dec+bwd, fp64), "
-                      f"{t_used:.1f} s of oracle time"}
+            "sample": f"{passes} passes of {n} contiguous tokens over the boundaries of {cfg.name} (enc+dec+bwd, fp64; the "
+                      f"Stiefel step is timed in stiefel.*.oracle), {t_used:.1f} s of oracle time"}
 
 
 def run_reference(args):
-    """--impl reference: the oracle, as it stands, on the host cores.  Each of the K steps is a
-    bounded contiguous-token sample of the workload, sized from one untimed probe so that the whole
+    """--impl reference: the oracle, as it stands, on the host cores, on the headline workload.  Each of the K steps
+    is a bounded contiguous-token sample of the workload, sized from one untimed probe so that the whole
     run ends within a few minutes."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    cfg, wdesc = workload(args.workload)
-    probe_n = 256
+    cfg, wdesc = workload(HEADLINE if args.workload == "all" else args.workload)
+    probe_n = 128
     probe = cpu_baseline(cfg, sample_tokens=probe_n)
     rate = probe["value"]
     n = int(max(64, min(cfg.n_tokens, rate * 90.0 / max(1, args.steps + args.warmup))))
@@ -755,10 +905,13 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="mapl", choices=["mapl", "reference"])
-    ap.add_argument("--workload", default="c1", choices=["c1", "c2", "c3", "c0"])
+    ap.add_argument("--workload", default="all", choices=["all", "c1", "c2", "c3", "c0"],
+                    help="all (default): headline c3 with c1, c2, c0 beside it; cN: that config alone as the headline")
     ap.add_argument("--tokens", type=int, default=0, help="override tokens per boundary (debug only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-stiefel", action="store_true", help="skip the configs[4] Stiefel-step sweep")
+    ap.add_argument("--no-stiefel", action="store_true", help="skip the configs[4] Stiefel-step sweep and the next-row timings")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the companion configs (c1, c2, c0)")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (debug only)")
     ap.add_argument("--track-steps", type=int, default=1000,
                     help="configs[4]: consecutive Stiefel steps per variant with the orthogonality residual tracked (0 = off)")
     ap.add_argument("--cpu-budget", type=float, default=20.0)

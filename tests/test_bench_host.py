@@ -29,7 +29,7 @@ def test_roofline_step_arithmetic():
     cfg = I.CONFIGS["c1"]
     peaks = {"hbm": 8000.0, "bf16": 2250.0, "src": "test"}
     calls = {"mapl_encode": 10.0, "mapl_decode": 10.0, "mapl_codec_backward": 30.0, "mapl_codec_backward_decode_side": 20.0}
-    out = bench.roofline_step(cfg, peaks, 0.15, 3, calls)
+    out = bench.roofline_step(cfg, peaks, calls)
     N = cfg.n_tokens
     t = [max(b * N / 8000e9, f * N / 2250e12) * 1e6 for f, b in (TABLE[("c1", c)] for c in ("encode", "decode", "backward"))]
     assert out["t_roof_us_per_boundary"] == pytest.approx(sum(t), abs=0.01)
@@ -42,3 +42,34 @@ def test_roofline_step_arithmetic():
 def test_job_tokens_per_second_is_whole_job():
     # 3 boundaries x 16384 tokens per rank-step, 4 ranks, 10 steps in 2 ms
     assert bench.job_tokens_per_second(3 * 16384, 4, 10, 2.0) == pytest.approx(3 * 16384 * 4 * 10 / 2e-3)
+
+
+def test_kernel_work_counts_every_backward_stream_once():
+    """g is read by k_tc_bwd_gz and re-read by k_tc_bwd_du; the call's algorithmic bytes count it once,
+    so the two kernels' byte counts must add up to the call's plus the gz re-read that only exists between them."""
+    for name in ("c1", "c2", "c3"):
+        cfg = I.CONFIGS[name]
+        s = 2
+        gzb, _ = bench.kernel_alg_work("k_tc_bwd_gz", cfg)
+        dub, _ = bench.kernel_alg_work("k_tc_bwd_du", cfg)
+        call = bench.alg_bytes_per_token(cfg)["backward"] * cfg.n_tokens
+        assert gzb + dub == call
+        _, f1 = bench.kernel_alg_work("k_tc_bwd_gz", cfg)
+        _, f2 = bench.kernel_alg_work("k_tc_bwd_du", cfg)
+        assert f1 + f2 == bench.alg_flops_per_token(cfg)["backward"] * cfg.n_tokens
+
+
+def test_stiefel_flops_and_step_stats():
+    d = 2048
+    # SURVEY 8(d): NS-5 24 d r^2 -> 0.20 / 0.81 / 3.22 / 12.9 GFLOP at r = 64 / 128 / 256 / 512
+    for r, gf in ((64, 0.20), (128, 0.81), (256, 3.22), (512, 12.9)):
+        assert bench.stiefel_alg_flops(d, r, "ns5") / 1e9 == pytest.approx(gf, rel=0.02)
+    assert bench.stiefel_alg_flops(d, 64, "qr") == pytest.approx(7 * d * 64 * 64 + 64 ** 3 / 3.0)
+    st = bench.step_time_stats([1.0, 3.0, 2.0])
+    assert st == {"median": 2.0, "max": 3.0, "min": 1.0}
+    assert bench.FFMA_TFLOPS == pytest.approx(74.4, abs=0.1)
+
+
+def test_default_headline_is_the_rvq_config():
+    cfg, desc = bench.workload(bench.HEADLINE)
+    assert desc.startswith("c3:") and cfg.rvq_levels == 2 and cfg.rvq_k == 4096 and cfg.d == 2048

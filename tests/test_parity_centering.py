@@ -56,6 +56,33 @@ def test_centered_encode_matches_oracle(name, n):
     assert rel_fro(Zq, res["Zhat"]) <= tol
 
 
+def test_centered_encode_bf16_ragged_shape_rounds_once():
+    """bf16 activations at a shape outside the tensor-core envelope (fp32 SIMT kernels), RVQ off, with an anchor much
+    larger than the centred z: T[tok] must be subtracted from the fp32 accumulator BEFORE the single bf16 rounding
+    (mapl.h); rounding U^T h to bf16 first would leave an error of 2^-9 |U^T h|, far above the centred z's own
+    rounding."""
+    bi = I.make_generic(35, 333, 200, 40, 0, 0, 300, 24, "bf16", a_std=1.0)
+    c = bi.cfg
+    desc = desc_of(bi)
+    # H = A_s[tok] B_s + small: the centred z is ~50x smaller than U^T h
+    A_s = (30.0 * bi.A.f64).astype(np.float32)
+    B_s = bi.B.f64.astype(np.float32)
+    small = bi.H.f64 * 0.1
+    H = I.store(A_s.astype(np.float64)[bi.tok] @ B_s.astype(np.float64) + small, "bf16")
+    dA, dB, dU, dH, dtok = to_dev(A_s), to_dev(B_s), to_dev(bi.U), to_dev(H), to_dev(bi.tok)
+    T = torch.empty((c.vocab, c.r), dtype=torch.float32, device="cuda")
+    cws = mb.alloc_workspace(mb.mapl_center_workspace_bytes(desc))
+    mb.mapl_center_table(desc, dA, dB, dU, T, cws)
+    ws = mb.alloc_workspace(mb.mapl_workspace_bytes(desc))
+    Zq = torch.empty((c.n_tokens, c.r), dtype=torch.bfloat16, device="cuda")
+    mb.mapl_encode_centered(desc, dH, dtok, T, dU, None, Zq, None, ws)
+    torch.cuda.synchronize()
+    Z = o.project(H.f64, bi.U.f64, bi.tok, A_s.astype(np.float64), B_s.astype(np.float64))
+    Zu = o.project(H.f64, bi.U.f64)
+    assert np.linalg.norm(Zu) > 10 * np.linalg.norm(Z)          # the offset dominates the uncentred projection
+    assert rel_fro(to_np(Zq), Z) <= 4e-3                        # one bf16 rounding of the centred z (2^-9 per entry)
+
+
 def test_zero_anchor_reduces_to_plain_encode():
     bi = I.make_boundary(I.CONFIGS["c2"].with_tokens(700), 4)
     desc = desc_of(bi)
@@ -71,7 +98,7 @@ def test_zero_anchor_reduces_to_plain_encode():
     assert torch.equal(a, b)
 
 
-@pytest.mark.parametrize("name,n", [("c0", 999), ("c1", 1500), ("c3", 517)])
+@pytest.mark.parametrize("name,n", [("c0", 999), ("c1", 1500), ("c2", 1037), ("c3", 517)])
 def test_center_backward_matches_oracle(name, n):
     """dA_s, dB_s and the dU correction of the centring term against oracle.center_backward, for a Gaussian
     gz in the activation dtype; then the accumulate variant."""

@@ -98,6 +98,45 @@ def test_many_steps_fresh_gradient_residual_stays_bounded(retr):
     assert rel_fro(to_np(U)[0], Uo) <= 1e-5
 
 
+@pytest.mark.parametrize("retr", ["qr", "ns"])
+@pytest.mark.parametrize("r", [64, 256, 512])
+def test_one_step_parity_late_in_the_1000_step_run(retr, r):
+    """configs[4] repeats the step 1000 times with the fixed seeded G; the oracle cannot follow all of
+    them, so it is restarted from the GPU's U_t at t = 100, 500, 1000 and the GPU's step t+1 must match its step from
+    the same U_t to 1e-5 (projector 0), with ||U^T U - I||_F <= 1e-5 for all three projectors at every mark."""
+    s = I.make_stiefel(r)
+    U = to_dev(s.U); G = to_dev(s.G)
+    batch, d, _ = U.shape
+    ws = mb.alloc_workspace(mb.mapl_stiefel_workspace_bytes(d, r, batch))
+    marks = (100, 500, 1000)
+    for t in range(1, marks[-1] + 2):
+        if (t - 1) in marks:
+            U_t = to_np(U)[0].copy()
+        mb.mapl_stiefel_step(U, G, I.STIEFEL_LR, RETR[retr][0], I.STIEFEL_NS_ITERS, None, ws)
+        if (t - 1) in marks:
+            torch.cuda.synchronize()
+            Ug = to_np(U)
+            Uo, _ = o.stiefel_step(U_t, s.G.f64[0], I.STIEFEL_LR, RETR[retr][1], I.STIEFEL_NS_ITERS)
+            assert rel_fro(Ug[0], Uo) <= 1e-5, (retr, r, t - 1, rel_fro(Ug[0], Uo))
+            for b in range(batch):
+                assert _orth_res(Ug[b]) <= 1e-5, (retr, r, t - 1, b, _orth_res(Ug[b]))
+
+
+def test_gradient_scale_folds_into_the_step_size():
+    """Reading S12 feeds the step G = dU / N.  xi is linear in G, so bench.py passes dU and lr / N instead of scaling the
+    gradient: both calls must give the same projector (to fp32 rounding) and match the oracle fed G = dU / N."""
+    r, d, N = 128, 1024, 4096.0
+    s = I.make_stiefel(r, d=d, batch=2, g_scale=N)            # a gradient of the size of a sum over N tokens
+    for retr in ("qr", "ns"):
+        Ua = to_dev(s.U); Ub = to_dev(s.U)
+        Gs = to_dev(s.G)
+        _gpu_step(Ua, Gs, 1e-2 / N, RETR[retr][0], info=False)
+        _gpu_step(Ub, (Gs / N).contiguous(), 1e-2, RETR[retr][0], info=False)
+        assert rel_fro(to_np(Ua)[0], to_np(Ub)[0]) <= 2e-6
+        Uo, _ = o.stiefel_step(s.U.f64[0], s.G.f64[0] / N, 1e-2, RETR[retr][1], 5)
+        assert rel_fro(to_np(Ua)[0], Uo) <= 1e-5
+
+
 def test_zero_gradient_is_fixed_point():
     s = I.make_stiefel(32, d=128, batch=1)
     for retr in ("qr", "ns"):
