@@ -144,9 +144,10 @@ static int encode_impl(const mapl_boundary_desc* desc, const void* H, const floa
     g.A[0].p = H; g.A[0].bf16 = bf; g.A[0].so = d.d; g.A[0].sk = 1;
     g.B[0].p = U; g.B[0].so = 1; g.B[0].sk = d.r;
     g.C = Zq_out; g.c_bf16 = bf; g.ldc = d.r;
-    MAPL_RETURN_IF(simt_gemm(g, st));
-    if (Tc) MAPL_RETURN_IF(simt_center_rows(Zq_out, bf, tok, Tc, d.n_tokens, d.r, st));
-    return MAPL_OK;
+    // centring: T[tok_n] leaves the fp32 accumulator of row n in the GEMM's epilogue, before the one rounding to the
+    // activation dtype (mapl.h); a separate pass over a bf16 Z would round U^T h first and lose 2^-9 |U^T h|
+    if (Tc) { g.E = Tc; g.lde = d.r; g.beta = -1.f; g.e_gather = tok; }
+    return simt_gemm(g, st);
   }
   float* hn = reinterpret_cast<float*>(ws + w.half_norm);
   MAPL_RETURN_IF(simt_half_sqnorm(codebooks, hn, L * d.rvq_k, d.r, st));

@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <mutex>
+
 #include "mapl.h"
 
 namespace mapl {
@@ -24,6 +26,23 @@ extern thread_local int g_last_cuda_error;
     int s_ = (expr);                \
     if (s_ != MAPL_OK) return s_;   \
   } while (0)
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is a per-DEVICE property of a kernel: set it once per device the
+// process drives, under a lock (two host threads may make their first call together).  Usage:
+//   MAPL_SMEM_OPT_IN(k_tc_decode, 227 * 1024);
+#define MAPL_SMEM_OPT_IN(kernel, bytes)                                                                    \
+  do {                                                                                                     \
+    static std::mutex mu_;                                                                                 \
+    static bool done_[::mapl::kMaxDevices] = {};                                                           \
+    int dev_ = 0;                                                                                          \
+    MAPL_CUDA_CHECK(cudaGetDevice(&dev_));                                                                 \
+    std::lock_guard<std::mutex> lk_(mu_);                                                                  \
+    if (dev_ < 0 || dev_ >= ::mapl::kMaxDevices || !done_[dev_]) {                                         \
+      MAPL_CUDA_CHECK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (bytes))); \
+      if (dev_ >= 0 && dev_ < ::mapl::kMaxDevices) done_[dev_] = true;                                     \
+    }                                                                                                      \
+  } while (0)
+constexpr int kMaxDevices = 64;
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -56,6 +75,7 @@ struct GemmArgs {
   const float* E = nullptr; // optional epilogue matrix (fp32, same indexing as C), only when !atomic
   long long lde = 0, sbe = 0;
   float beta = 0.f;
+  const int32_t* e_gather = nullptr;  // optional: row m of E is E[e_gather[m]] (the centring rows T[tok_n] of Eq. 1)
   int batch = 1;
 };
 
@@ -75,7 +95,6 @@ int simt_half_sqnorm(const float* C, float* out, int rows, int r, cudaStream_t s
 int simt_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* U, const float* C,
                     const float* half_norm, void* Zq_out, int32_t* codes, cudaStream_t stream,
                     const int32_t* tok = nullptr, const float* Tc = nullptr);     // Tc: centring table (Eq. 1)
-int simt_center_rows(void* Z, int bf16, const int32_t* tok, const float* Tc, long long N, int r, cudaStream_t stream);
 int simt_dequant(const mapl_boundary_desc& d, const int32_t* codes, const float* C, float* Zhat,
                  cudaStream_t stream);
 int simt_scatter_add_rows(const float* gA, const int32_t* tok, float* dA, long long N, int ra,

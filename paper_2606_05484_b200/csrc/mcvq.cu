@@ -129,12 +129,8 @@ int mapl_mcvq_quantize(int64_t n_tokens, int32_t r, int32_t act_dtype, int32_t l
   if (!aligned16(X) || !aligned16(codebooks) || !aligned16(codes_out) || (Xq_out && !aligned16(Xq_out))) return MAPL_ERR_ALIGNMENT;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   const size_t smem = (size_t)kLanes * levels * k * sizeof(float2);
-  static bool attr_done = false;
-  if (!attr_done) {
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_mcvq_quantize<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLanes * kMaxLK * 8));
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_mcvq_quantize<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLanes * kMaxLK * 8));
-    attr_done = true;
-  }
+  MAPL_SMEM_OPT_IN(k_mcvq_quantize<true>, kLanes * kMaxLK * 8);
+  MAPL_SMEM_OPT_IN(k_mcvq_quantize<false>, kLanes * kMaxLK * 8);
   const unsigned blocks = (unsigned)((n_tokens + kTok - 1) / kTok);
   KernelScope ks(KID_MCVQ, st);
   if (act_dtype == MAPL_BF16) k_mcvq_quantize<true><<<blocks, kThreads, smem, st>>>(X, codebooks, codes_out, Xq_out, n_tokens, r, levels, k);

@@ -206,32 +206,6 @@ __global__ void k_scatter_add_rows(const float* __restrict__ gA, const int32_t* 
 
 }  // namespace
 
-// Z[n,:] -= T[tok_n,:]  (sender-side centring after a plain projection; Z in the activation dtype)
-template <bool kBf16>
-__global__ void k_center_rows(void* __restrict__ Zv, const int32_t* __restrict__ tok, const float* __restrict__ Tc, long long N, int r) {
-  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= N * r) return;
-  const long long n = idx / r;
-  const int j = (int)(idx % r);
-  const float t = Tc[(long long)tok[n] * r + j];
-  if (kBf16) {
-    __nv_bfloat16* Z = reinterpret_cast<__nv_bfloat16*>(Zv);
-    Z[idx] = __float2bfloat16_rn(__bfloat162float(Z[idx]) - t);
-  } else {
-    reinterpret_cast<float*>(Zv)[idx] -= t;
-  }
-}
-
-int simt_center_rows(void* Z, int bf16, const int32_t* tok, const float* Tc, long long N, int r, cudaStream_t stream) {
-  if (N <= 0) return MAPL_OK;
-  KernelScope ks(KID_SCATTER_ROWS, stream);
-  const unsigned blocks = (unsigned)((N * r + 255) / 256);
-  if (bf16) k_center_rows<true><<<blocks, 256, 0, stream>>>(Z, tok, Tc, N, r);
-  else k_center_rows<false><<<blocks, 256, 0, stream>>>(Z, tok, Tc, N, r);
-  MAPL_CUDA_CHECK(cudaGetLastError());
-  return MAPL_OK;
-}
-
 // D[tok_n, :] += X[n, :]: one warp per token row, fp32 atomics (reds)
 template <bool kBf16>
 __global__ void k_scatter_act_rows(const void* __restrict__ Xv, const int32_t* __restrict__ tok, float* __restrict__ D,
@@ -292,12 +266,8 @@ int simt_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* U, 
   if (smem > 227 * 1024) return MAPL_ERR_UNSUPPORTED;
   const long long blocks = (d.n_tokens + TOK - 1) / TOK;
   KernelScope ks(KID_SIMT_ENCODE_RVQ, stream);
-  static bool attr_done = false;   // once per process (not a stream operation; keeps graph capture clean)
-  if (!attr_done) {
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_simt_encode_rvq<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_simt_encode_rvq<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    attr_done = true;
-  }
+  MAPL_SMEM_OPT_IN(k_simt_encode_rvq<true>, 227 * 1024);
+  MAPL_SMEM_OPT_IN(k_simt_encode_rvq<false>, 227 * 1024);
   if (d.act_dtype == MAPL_BF16) {
     k_simt_encode_rvq<true><<<(unsigned)blocks, NT, smem, stream>>>(H, U, C, half_norm, Zq_out, codes, d.n_tokens, d.d, d.r, d.rvq_levels, d.rvq_k, tok, Tc);
   } else {

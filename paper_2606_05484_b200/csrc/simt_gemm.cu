@@ -22,7 +22,7 @@ struct DevGemm {
   int K[2];
   void* C; int c_bf16; long long ldc, sbc;
   int splits, atomic;
-  float alpha; const float* E; long long lde, sbe; float beta;
+  float alpha; const float* E; long long lde, sbe; float beta; const int32_t* e_gather;
   long long sbA[2], sbB[2];
 };
 
@@ -114,7 +114,7 @@ __global__ void __launch_bounds__(NT) k_simt_gemm(const DevGemm g) {
       if (g.atomic) {
         atomicAdd(reinterpret_cast<float*>(g.C) + ci, v);
       } else {
-        if (g.E) v += g.beta * g.E[offE + (long long)m * g.lde + n];
+        if (g.E) v += g.beta * g.E[offE + (long long)(g.e_gather ? g.e_gather[m] : m) * g.lde + n];
         st_from_f32(g.C, ci, g.c_bf16, v);
       }
     }
@@ -137,7 +137,7 @@ int simt_gemm(const GemmArgs& a, cudaStream_t stream) {
   }
   g.C = a.C; g.c_bf16 = a.c_bf16; g.ldc = a.ldc; g.sbc = a.sbc;
   g.splits = a.splits < 1 ? 1 : a.splits; g.atomic = a.atomic;
-  g.alpha = a.alpha; g.E = a.E; g.lde = a.lde; g.sbe = a.sbe; g.beta = a.beta;
+  g.alpha = a.alpha; g.E = a.E; g.lde = a.lde; g.sbe = a.sbe; g.beta = a.beta; g.e_gather = a.e_gather;
   const int tiles = ((a.M + BM - 1) / BM) * ((a.N + BN - 1) / BN);
   dim3 grid(tiles, g.splits, a.batch);
   { KernelScope ks(KID_SIMT_GEMM, stream); k_simt_gemm<<<grid, NT, 0, stream>>>(g); }

@@ -480,13 +480,9 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
   if (!tc_shape_ok(d)) return MAPL_ERR_UNSUPPORTED;
   const int ra = tok ? d.anchor_rank : 0, kc = d.r + ra;
 
-  static bool attr_done = false;
-  if (!attr_done) {
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_bwd_gz, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_bwd_du<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_bwd_du<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    attr_done = true;
-  }
+  MAPL_SMEM_OPT_IN(k_tc_bwd_gz, 227 * 1024);
+  MAPL_SMEM_OPT_IN(k_tc_bwd_du<true>, 227 * 1024);
+  MAPL_SMEM_OPT_IN(k_tc_bwd_du<false>, 227 * 1024);
   const uint64_t N = (uint64_t)d.n_tokens, dd = (uint64_t)d.d, rr = (uint64_t)d.r;
 
   // zhat operand for dU

@@ -32,11 +32,12 @@ TcPack tc_pack_layout(const mapl_boundary_desc& d, char* base) {
   if (d.rvq_levels > 0) {
     const size_t LK = (size_t)d.rvq_levels * d.rvq_k;
     p.WBlo = reinterpret_cast<__nv_bfloat16*>(seg((size_t)d.r * d.d * 2));
+    if (d.rvq_levels >= 3) p.WBlo2 = reinterpret_cast<__nv_bfloat16*>(seg((size_t)d.r * d.d * 2));
     p.Cb = reinterpret_cast<__nv_bfloat16*>(seg(LK * d.r * 2));
+    p.hnb = reinterpret_cast<__nv_bfloat16*>(seg(LK * 16 * 2));
     p.hn = reinterpret_cast<float*>(seg(LK * 4));
     p.rowamax = reinterpret_cast<float*>(seg(LK * 4));
-    p.cmax = reinterpret_cast<float*>(seg(8 * 4));
-    p.cscale = reinterpret_cast<float*>(seg(2 * 8 * 4));
+    p.lvl = reinterpret_cast<float*>(seg(8 * 8 * 4));
   }
   p.bytes = off;
   return p;
@@ -64,10 +65,11 @@ struct PackJob {
   __nv_bfloat16* dst; long long pitch;     // dst element (i,j) -> dst[i*pitch + j] (after optional transpose)
   int transpose;
   int mode;                                // 0: bf16(x)   1: bf16(x - float(bf16(x))), the second split term
-                                           // 2: fp16(x * scale[src_row / rows_per_scale])  (16-bit store)
+                                           // 2: fp16(x * scale[8 * (src_row / rows_per_scale) + 3])  (16-bit store)
+                                           // 3: the third split term bf16(x - hi - lo)
   const float* scale; int rows_per_scale;
 };
-struct PackArgs { PackJob job[6]; int njobs; };
+struct PackArgs { PackJob job[7]; int njobs; };
 
 __device__ __forceinline__ __nv_bfloat16 pack_term(float x, int mode, float sc) {
   if (mode == 2) {
@@ -75,7 +77,10 @@ __device__ __forceinline__ __nv_bfloat16 pack_term(float x, int mode, float sc) 
     return *reinterpret_cast<const __nv_bfloat16*>(&h);
   }
   const __nv_bfloat16 hi = __float2bfloat16_rn(x);
-  return mode == 1 ? __float2bfloat16_rn(x - __bfloat162float(hi)) : hi;
+  if (mode == 0) return hi;
+  const float r1 = x - __bfloat162float(hi);          // exact
+  const __nv_bfloat16 lo = __float2bfloat16_rn(r1);
+  return mode == 1 ? lo : __float2bfloat16_rn(r1 - __bfloat162float(lo));
 }
 
 // 32x32 tiles; blockIdx.y = job
@@ -100,7 +105,7 @@ __global__ void __launch_bounds__(256) k_tc_pack(const PackArgs a) {
     } else {
       for (int i = ty; i < 32; i += 8) {
         const int r = r0 + i, c = c0 + tx;
-        const float sc = (j.mode == 2 && r < j.rows) ? j.scale[r / j.rows_per_scale] : 1.f;
+        const float sc = (j.mode == 2 && r < j.rows) ? j.scale[8 * (r / j.rows_per_scale) + 3] : 1.f;
         if (r < j.rows && c < j.cols) j.dst[(long long)r * j.pitch + c] = pack_term(tile[i][tx], j.mode, sc);
       }
     }
@@ -120,10 +125,11 @@ __global__ void __launch_bounds__(256) k_tc_cb_stats(const float* __restrict__ C
   if (lane == 0) { hn[row] = 0.5f * s; rowamax[row] = m; }
 }
 
-// one block per level: cmax[l] = max_k ||c_k||;  cscale[l] = 2^-e with max|c| * 2^-e in [0.5, 1),
-// cscale[8 + l] = 2^e  (the fp16 codebook copy is C * cscale[l]; powers of two, so exact)
+// one block per level: lvl[8 l + ...] = {cmax sc, qmax, 2^g, sc, 2^e, cmax}: sc = 2^-e with max|c| * sc in [0.5, 1)
+// (powers of two: the fp16 codebook copy C * sc is exact up to the fp16 rounding), cmax = max_k ||c_k||,
+// q_k = hn_k sc 2^-g with g >= 0 the smallest integer that brings max_k q_k to <= 2^15 (fp16 range)
 __global__ void __launch_bounds__(256) k_tc_cmax(const float* __restrict__ hn, const float* __restrict__ rowamax,
-                                                 float* __restrict__ cmax, float* __restrict__ cscale, int K) {
+                                                 float* __restrict__ lvl, int K) {
   __shared__ float red[8], red2[8];
   float m = 0.f, a = 0.f;
   for (int k = threadIdx.x; k < K; k += 256) {
@@ -136,12 +142,38 @@ __global__ void __launch_bounds__(256) k_tc_cmax(const float* __restrict__ hn, c
   __syncthreads();
   if (threadIdx.x == 0) {
     for (int i = 1; i < 8; ++i) { m = fmaxf(m, red[i]); a = fmaxf(a, red2[i]); }
-    cmax[blockIdx.x] = sqrtf(2.f * m);
+    const float cmax = sqrtf(2.f * m);
     int eb = (int)((__float_as_uint(a) >> 23) & 0xffu);
     eb = eb < 2 ? 126 : (eb > 250 ? 250 : eb);             // all-zero / denormal codebook: scale 1
-    cscale[blockIdx.x] = __uint_as_float((uint32_t)(253 - eb) << 23);
-    cscale[8 + blockIdx.x] = __uint_as_float((uint32_t)(eb + 1) << 23);
+    const float sc = __uint_as_float((uint32_t)(253 - eb) << 23);
+    float q = m * sc, pg = 1.f;
+    while (q > 32768.f && pg < 1e30f) { q *= 0.5f; pg *= 2.f; }
+    float* o = lvl + 8 * blockIdx.x;
+    o[0] = cmax * sc; o[1] = q; o[2] = pg; o[3] = sc; o[4] = __uint_as_float((uint32_t)(eb + 1) << 23); o[5] = cmax;
+    o[6] = 0.f; o[7] = 0.f;
   }
+}
+
+// hnb[row, 0..2] = -(fp16 three-term split of q = hn[row] sc / 2^g), hnb[row, 3..15] = 0.  The split is exact up to
+// 2^-33 q + 2^-25 (each remainder is exact in fp32; the last one is dropped).
+__global__ void __launch_bounds__(256) k_tc_hnb(const float* __restrict__ hn, const float* __restrict__ lvl,
+                                                __nv_bfloat16* __restrict__ hnb, int rows, int K) {
+  const int row = blockIdx.x * blockDim.x + threadIdx.x;
+  if (row >= rows) return;
+  const float* o = lvl + 8 * (row / K);
+  float q = hn[row] * o[3] / o[2];
+  unsigned short h[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) h[i] = 0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    const __half p = __float2half_rn(q);
+    q -= __half2float(p);
+    h[i] = __half_as_ushort(__float2half_rn(-__half2float(p)));
+  }
+  uint4* dst = reinterpret_cast<uint4*>(hnb + (long long)row * 16);
+  dst[0] = make_uint4(h[0] | ((uint32_t)h[1] << 16), h[2] | ((uint32_t)h[3] << 16), 0u, 0u);
+  dst[1] = make_uint4(0u, 0u, 0u, 0u);
 }
 
 }  // namespace
@@ -156,8 +188,13 @@ int tc_pack_build(const mapl_boundary_desc& d, const float* U, const float* B, c
       k_tc_cb_stats<<<(rows + 7) / 8, 256, 0, st>>>(codebooks, p.hn, p.rowamax, rows, d.r);
       MAPL_CUDA_CHECK(cudaGetLastError());
     }
+    {
+      KernelScope ks(KID_TC_PACK, st);
+      k_tc_cmax<<<d.rvq_levels, 256, 0, st>>>(p.hn, p.rowamax, p.lvl, d.rvq_k);
+      MAPL_CUDA_CHECK(cudaGetLastError());
+    }
     KernelScope ks(KID_TC_PACK, st);
-    k_tc_cmax<<<d.rvq_levels, 256, 0, st>>>(p.hn, p.rowamax, p.cmax, p.cscale, d.rvq_k);
+    k_tc_hnb<<<(rows + 255) / 256, 256, 0, st>>>(p.hn, p.lvl, p.hnb, rows, d.rvq_k);
     MAPL_CUDA_CHECK(cudaGetLastError());
   }
   PackArgs a;
@@ -171,7 +208,8 @@ int tc_pack_build(const mapl_boundary_desc& d, const float* U, const float* B, c
   }
   if (d.rvq_levels > 0 && p.WBlo) {
     a.job[a.njobs++] = PackJob{U, d.d, d.r, p.WBlo, d.d, 1, 1, nullptr, 1};
-    if (rvq) a.job[a.njobs++] = PackJob{codebooks, d.rvq_levels * d.rvq_k, d.r, p.Cb, d.r, 0, 2, p.cscale, d.rvq_k};
+    if (p.WBlo2) a.job[a.njobs++] = PackJob{U, d.d, d.r, p.WBlo2, d.d, 1, 3, nullptr, 1};
+    if (rvq) a.job[a.njobs++] = PackJob{codebooks, d.rvq_levels * d.rvq_k, d.r, p.Cb, d.r, 0, 2, p.lvl, d.rvq_k};
   }
   {
     KernelScope ks(KID_TC_PACK, st);

@@ -8,9 +8,14 @@
 // Parameter pack (bf16 operand copies of the fp32 masters, see mapl_pack_params in mapl.h):
 //   WB   [(r+ra), d] = [U^T ; B]    K-major over d     (encode / backward-gz B operand)
 //   Wd   [d, (r+ra)] = [U | B^T]    K-major over r+ra  (decode / backward-dH B operand)
-//   WBlo [r, d]      = (U - bf16(U))^T                 (second split term: fp32-accurate z for RVQ)
-//   Cb   [L*K, r]    fp16 codebooks scaled per level by cscale[l] = 2^-e (max|c| 2^-e in [0.5,1));
-//                    hn [L*K] = 0.5 ||C_k||^2 (fp32);  cmax [L] = max_k ||C_l,k||;  cscale[8+l] = 2^e
+//   WBlo [r, d]      = bf16(U - bf16(U))^T             (second split term: z to 2^-17 for RVQ)
+//   WBlo2 [r, d]     = bf16(U - hi - lo)^T             (third split term, L >= 3 only: z fp32-accurate, so that the deep
+//                    levels, whose residual is small against the absolute error of z, stay inside rule S5)
+//   Cb   [L*K, r]    fp16 codebooks scaled per level by sc_l = 2^-e (max|c| 2^-e in [0.5,1))
+//   hnb  [L*K, 16]   fp16: -(three-term fp16 split of q_k = 0.5 ||C_k||^2 sc_l 2^-g_l), zero padded: the extra K = 16
+//                    step of the score MMA that folds the half norms in (tc_encode_rvq.cu)
+//   lvl  [8 x 8]     per level: {cmax sc_l, max_k q_k, 2^g_l, sc_l, 2^e, cmax, -, -}, cmax = max_k ||C_l,k||
+//   hn   [L*K]       0.5 ||C_k||^2 (fp32), rowamax [L*K]: scratch of the pack kernels
 #pragma once
 #include "common.cuh"
 
@@ -23,11 +28,12 @@ struct TcPack {
   __nv_bfloat16* WB = nullptr;
   __nv_bfloat16* Wd = nullptr;
   __nv_bfloat16* WBlo = nullptr;
+  __nv_bfloat16* WBlo2 = nullptr;
   __nv_bfloat16* Cb = nullptr;
+  __nv_bfloat16* hnb = nullptr;
   float* hn = nullptr;
   float* rowamax = nullptr;
-  float* cmax = nullptr;
-  float* cscale = nullptr;
+  float* lvl = nullptr;
   int kc = 0;          // r + ra
   size_t bytes = 0;
 };

@@ -149,11 +149,7 @@ int tc_decode(const mapl_boundary_desc& d, const void* Z, const int32_t* codes, 
                          codes ? (uint64_t)kc : (uint64_t)d.r, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
   if (!make_tmap_bf16_2d(&tmW, pk.Wd, (uint64_t)d.d, (uint64_t)kc, (uint64_t)kc, 64, kChunkN / 2)) return MAPL_ERR_CUDA;
   if (!make_tmap_bf16_2d(&tmO, Hhat_out, (uint64_t)d.n_tokens, (uint64_t)d.d, (uint64_t)d.d, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
-  static bool attr_done = false;
-  if (!attr_done) {
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    attr_done = true;
-  }
+  MAPL_SMEM_OPT_IN(k_tc_decode, 227 * 1024);
   const unsigned tiles = ((unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m) + 1u) & ~1u;   // whole CTA pairs
   KernelScope ks(KID_TC_DECODE, st);
   MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_decode, dim3(tiles), dim3(kThreads), smem, st, tmZ, tmW, tmO, p));

@@ -173,11 +173,7 @@ int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks
   if (stages > 8) stages = 8;
   if (stages > d.d / BK) stages = d.d / BK;
   const size_t smem = (size_t)stages * stage_bytes + 1024 + 256;
-  static bool attr_done = false;
-  if (!attr_done) {
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_encode, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    attr_done = true;
-  }
+  MAPL_SMEM_OPT_IN(k_tc_encode, 227 * 1024);
   const unsigned tiles = ((unsigned)((d.n_tokens + tile_m - 1) / tile_m) + 1u) & ~1u;   // whole CTA pairs
   KernelScope ks(KID_TC_ENCODE, st);
   MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_encode, dim3(tiles), dim3(kThreads), smem, st, tmH, tmW,

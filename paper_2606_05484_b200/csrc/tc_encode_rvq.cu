@@ -558,11 +558,7 @@ int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codeb
   if (!make_tmap_bf16_2d(&tmWhi, pk.WB, rr, dd, dd, 64, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
   if (!make_tmap_bf16_2d(&tmWlo, pk.WBlo, rr, dd, dd, 64, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
   if (!make_tmap_bf16_2d(&tmC, pk.Cb, (uint64_t)d.rvq_levels * d.rvq_k, rr, rr, 64, kChunk / 2)) return MAPL_ERR_CUDA;
-  static bool attr_done = false;
-  if (!attr_done) {
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_encode_rvq, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    attr_done = true;
-  }
+  MAPL_SMEM_OPT_IN(k_tc_encode_rvq, 227 * 1024);
   const unsigned tiles = ((unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m) + 1u) & ~1u;   // whole CTA pairs
   KernelScope ks(KID_TC_ENCODE_RVQ, st);
   MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_encode_rvq, dim3(tiles), dim3(kThreads), smem, st, tmH, tmWhi, tmWlo, tmC, p));

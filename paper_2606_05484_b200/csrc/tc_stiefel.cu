@@ -325,12 +325,8 @@ int tc_st_gemm3(const __nv_bfloat16* Ap, const __nv_bfloat16* Bp, int M, int N, 
   p.nsplit = (nkb + p.kb_per_split - 1) / p.kb_per_split;
   p.atomic = p.nsplit > 1 ? 1 : 0;
   p.sC = (long long)M * N;
-  static bool attr_done = false;
   const size_t smem = (size_t)kStages * kStageBytes + 1024 + 256;
-  if (!attr_done) {
-    MAPL_CUDA_CHECK(cudaFuncSetAttribute(k_tc_gemm3, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    attr_done = true;
-  }
+  MAPL_SMEM_OPT_IN(k_tc_gemm3, 227 * 1024);
   KernelScope ks(KID_ST_GEMM3, st);
   MAPL_CUDA_CHECK(tc::launch_pdl(k_tc_gemm3, dim3(M / 128, N / 128, batch * p.nsplit), dim3(192), smem, st, tmA, tmB, p));
   return MAPL_OK;
