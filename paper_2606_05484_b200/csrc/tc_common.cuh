@@ -27,6 +27,10 @@ bool make_tmap_bf16_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64
 bool make_tmap_f32_2d(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols, uint64_t pitch_elems,
                       uint32_t box_cols, uint32_t box_rows);
 
+// 2-D 16-bit row-major tensor [rows, 16] (row pitch 32 B), box = {16, box_rows}, 32B swizzle: rows land densely at a
+// 32-byte pitch, the layout of a K-major SWIZZLE_32B UMMA operand whose K extent is one UMMA_K = 16 step
+bool make_tmap_b16_k16_sw32(CUtensorMap* map, const void* base, uint64_t rows, uint32_t box_rows);
+
 #ifdef __CUDACC__
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -169,6 +173,16 @@ __device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr, uint32_t lbo_
   return d;
 }
 __device__ __forceinline__ uint64_t desc_kmajor_sw128(uint32_t saddr) { return make_smem_desc(saddr, 16, 1024); }
+// K-major operand of ONE UMMA_K = 16 step (16-bit elements), SWIZZLE_32B: rows of 32 B, 8 rows = one 256 B atom (SBO)
+__device__ __forceinline__ uint64_t desc_kmajor_sw32_k16(uint32_t saddr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+  d |= (uint64_t)1 << 16;             // LBO: unused for a swizzled K-major tile of one atom in K
+  d |= (uint64_t)(256 >> 4) << 32;    // SBO
+  d |= (uint64_t)1 << 46;             // descriptor version (Blackwell)
+  d |= (uint64_t)6 << 61;             // SWIZZLE_32B
+  return d;
+}
 __device__ __forceinline__ uint64_t desc_mnmajor_sw128(uint32_t saddr, uint32_t lbo_bytes) {
   return make_smem_desc(saddr, lbo_bytes, 1024);
 }

@@ -1,28 +1,33 @@
 // tc_encode_rvq.cu -- mapl_encode with residual VQ on the tensor cores: projection and all RVQ
 // levels in ONE kernel, z never leaves the chip (Eq. 1; Sec. 3.5;
-// readings S3-S5 of DESIGN.md).
+// readings S3-S5, S18 of DESIGN.md).
 //
 // One CTA per token tile (<= 128 tokens; one TMEM lane = one token); CTAs work in pairs (cluster of 2,
 // cta_group::2 MMAs of M = 256): each CTA loads half of every parameter / codebook tile.
-//   phase 1   z = H (U_hi + U_lo)      H tiles by TMA (HBM, evict-first), the two bf16 split terms
-//             of U^T from the L2-resident pack; fp32 accumulator [128 x r] in TMEM columns [0,r).
-//             bf16 H is exact and U_hi + U_lo carries 16 mantissa bits, so z is fp32-accurate.
-//   level l   rho (fp32) stays in TMEM columns [0,r); its fp16 rounding, scaled per token by a power
-//             of two so that max|rho_j| lies in [0.5,1), is the resident A operand (the codebook
-//             copy is fp16 too, scaled per level: 11 significant bits instead of bf16's 8).
-//             Codebook tiles [128 codewords x 64] stream through a TMA ring; per 128-codeword
-//             chunk one accumulator stage S = rho_f16 . C_f16^T  (2 stages, TMEM cols 256..511).
-//             Epilogue (thread = token): coarse score s_k = 0.5||c_k||^2 - S_k, running minimum,
-//             and every k with  s_k <= running min + margin  is recorded as a candidate, where
-//               margin = 2 E,   E = 2^-10 * 1.05 * ||rho|| * max_k ||c_k||  >=  |s_coarse - s_exact|
-//             (fp16 rounding of both operands, Cauchy-Schwarz).  The true minimiser is therefore
-//             always among the candidates; they are re-scored in exact fp32 (rho from TMEM, the
-//             fp32 codeword from L2), lowest index winning ties (S4).  Then rho -= C[l, k*].
-//             A thread's candidate list holds kNE 32-codeword pieces; when it is full it keeps the
-//             pieces with the lowest minima, and only a left-out piece whose minimum is within the
-//             FINAL threshold (the threshold only tightens during the scan) sends the warp to the
-//             exhaustive fp32 pass over all K codewords (duplicate-heavy codebooks).
-// Roofline: tensor at config 3 (K r = 1M per level), HBM/ALU at config 2.
+//   phase 1   z = H (U_hi + U_lo [+ U_lo2])   H tiles by TMA (HBM, evict-first), the bf16 split terms of U^T from the
+//             L2-resident pack; fp32 accumulator [128 x r] in TMEM columns [0,r).  bf16 H is exact; two terms carry 16
+//             mantissa bits of U, three (L >= 3) all 24, so that the deep levels stay inside rule S5.
+//   level l   rho (fp32) stays in TMEM columns [0,r); its fp16 rounding, scaled per token by a power of two inv, is the
+//             resident A operand (the codebook copy is fp16 too, scaled per level by sc_l).  Codebook tiles
+//             [128 codewords x 64] stream through a TMA ring; per 128-codeword chunk one accumulator stage
+//                 T_k = rho_s . c_s,k  -  a' q_k        (2 stages, TMEM cols 256..511)
+//             where the second term is ONE extra K = 16 MMA step: the A side holds a' = inv 2^g in all 16 columns, the
+//             B side the three-term fp16 split of -q_k, q_k = 0.5 ||c_k||^2 sc_l 2^-g (SWIZZLE_32B tiles; a constant A
+//             row makes the column order irrelevant).  T_k = inv sc_l (rho.c_k - 0.5||c_k||^2) up to the coarse error
+//                 E = E_op + E_acc + E_hn   (fp16 operand rounding, tensor-core accumulation, the split of q)
+//             so argmax_k T_k is the nearest codeword up to E.  Epilogue (2 threads per token, 64 scores per thread and
+//             chunk): a max3 tree per 16-codeword group (0.5 instruction per score) and the running maximum; a group
+//             whose maximum is within 2E of the running maximum is STASHED raw (four 16-byte stores) in a per-thread
+//             list in shared memory.  After the scan the final threshold best - 2E prunes the list; the surviving
+//             groups are re-read, their scores >= the threshold are the candidates (the true minimiser is always
+//             among them); a token with a single candidate is done, the others are re-scored in exact fp32 in the
+//             DIRECT form sum_j (rho_j - c_kj)^2 (rho from TMEM, the fp32 codeword from L2), lowest index winning
+//             ties (S4).  Then rho -= C[l, k*], fused with the fp16 conversion for the next level (the scale comes
+//             from the bound max|rho| + max|c|: fp16 precision does not depend on it).
+//             A list holds kne groups; when it is full a stale entry (below the current threshold) is reused, else the
+//             lowest maximum is dropped and remembered: only if that value is within the FINAL threshold does the
+//             thread fall back to the exhaustive fp32 pass over its codewords (duplicate-heavy codebooks).
+// Roofline: tensor at config 3 (K r = 1M per level), HBM at config 2.
 #include <float.h>
 
 #include "profile.cuh"
@@ -33,70 +38,75 @@ namespace mapl {
 namespace {
 using namespace tc;
 
-// scan / re-score threads per token (warps per TMEM lane quarter): 2 or 4.  Measured: 4 (16 scan warps, 96 registers)
-// is SLOWER -- c2 encode 59.7 -> 62.2 us, c3 239 -> 271 us: the per-warp cost of a chunk (TMEM load, wait, barrier
-// arrive, list bookkeeping) does not shrink with the piece count and the 512-thread exchanges cost more.
-#ifndef MAPL_RVQ_PARTS
-#define MAPL_RVQ_PARTS 2
-#endif
-constexpr int kParts = MAPL_RVQ_PARTS;
+constexpr int kParts = 2;                // scan / re-score threads per token (warps per TMEM lane quarter)
 constexpr int kEpi = 128 * kParts;       // epilogue threads
-constexpr int kThreads = 64 + kEpi;      // warp 0 TMA, warp 1 MMA, then kParts x 4 scan / re-score warps
-constexpr int kChunk = 128;        // codewords per accumulator stage (UMMA N)
-constexpr int kAccCol0 = 256;      // TMEM column of score stage 0
-constexpr int kNE = 8;             // candidate-list entries per thread (one entry = one 32-codeword piece)
+constexpr int kProducers = 3;            // TMA producer warps: warp 0 and the two warps after the epilogue warps.  A producer
+                                         // thread pays ~560 cycles per loop iteration plus ~135 per 8 KB box whatever the ring depth
+                                         // (measured: _work microbenchmark); the cost is per THREAD, so
+                                         // several producer warps taking the items in turn multiply the issue rate
+constexpr int kThreads = 64 + kEpi + 64; // warp 0 TMA, warp 1 MMA, kParts x 4 scan / re-score warps, 2 more TMA warps
+constexpr int kChunk = 128;              // codewords per accumulator stage (UMMA N)
+constexpr int kAccCol0 = 256;            // TMEM column of score stage 0
+constexpr int kXStages = 8;              // ring of the norm tiles (one per chunk)
+constexpr int kXBytes = 64 * 32;         // a CTA's half of a norm tile: 64 codewords x 16 fp16
+constexpr int kAxBytes = 128 * 32;       // A side of the norm step: 128 tokens x 16 fp16
 
 struct RvqParams {
   const float* C;        // [L,K,r] fp32 codebooks (exact re-scoring, residual update)
-  const float* hn;       // [L*K] 0.5 ||c||^2
-  const float* cmax;     // [L] max_k ||c_k||
-  const float* cscale;   // [8+l] = 2^e_l: the fp16 codebook copy is C * 2^-e_l
+  const float* lvl;      // [8 x 8] per-level constants (tc_codec.cuh)
   const int32_t* tok; const float* Tc;   // optional sender-side centring (Eq. 1): z -= Tc[tok], Tc [V,r] fp32
   __nv_bfloat16* Zq;     // optional [N,r]
   int32_t* codes;        // [N,L]
   long long N;
   int d, r, L, K, tile_m;
-  int stages1, stage1_bytes, ring_tiles;
+  int stages1, stage1_bytes, ring_tiles, nsplit, kne, p1, p2;
 };
 
 // smem carve-up (after 1024-byte alignment):
-//   region R  = max(phase-1 ring, rho operand tiles + codebook ring)
-//   sHn [K] fp32 | candidate lists [kNE][kEpi] x (m32, piece, mask) | exchange [5][kParts][128] | barriers | tmem slot
+//   region R = max(phase-1 ring,  rho operand tiles | norm A tile | codebook ring | norm ring | stash)
+//   eM [kne][kEpi] f32 | eId [kne][kEpi] i32 | exchange [6][kEpi] | barriers | tmem slot
 struct Smem {
-  uint8_t* ring1; uint8_t* sRho; uint8_t* ringC;
-  float* sHn; float* eM; int* eP; uint32_t* eMask;
-  float* xch;            // [5][kParts][128]: per (part, token) best / score / k / n2 / amax exchanged by the warps of a quarter
+  uint8_t* ring1; uint8_t* sRho; uint8_t* sAx; uint8_t* ringC; uint8_t* ringX; uint8_t* stash;
+  float* eM; int* eId;
+  float* xch;            // [6][kEpi]: best / dist / k / n2 / amax / count exchanged by the threads of a token
   uint64_t* s1_full; uint64_t* s1_empty; uint64_t* z_full;
-  uint64_t* c_full; uint64_t* c_empty; uint64_t* acc_full; uint64_t* acc_empty; uint64_t* rho_ready;
+  uint64_t* c_full; uint64_t* c_empty; uint64_t* x_full; uint64_t* x_empty;
+  uint64_t* acc_full; uint64_t* acc_empty; uint64_t* rho_ready;
   uint32_t* tmem_slot;
 };
 
+__host__ __device__ inline size_t rvq_level_bytes(const RvqParams& p) {
+  return (size_t)(p.r / 64) * kTileBytes + kAxBytes + (size_t)p.ring_tiles * kHalfTileBytes + (size_t)kXStages * kXBytes +
+         (size_t)p.kne * 4 * kEpi * 16;
+}
 __host__ __device__ inline size_t rvq_regionR(const RvqParams& p) {
-  const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes;
-  const size_t lvl = (size_t)(p.r / 64) * kTileBytes + (size_t)p.ring_tiles * kHalfTileBytes;
+  const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes, lvl = rvq_level_bytes(p);
   return ring1 > lvl ? ring1 : lvl;
 }
-__host__ __device__ inline size_t rvq_tail_bytes(const RvqParams& p) {
-  return (size_t)p.K * 4 + (size_t)kNE * kEpi * 12 + 5 * kEpi * 4 + 1024;
+__host__ __device__ inline size_t rvq_tail_bytes(int kne) {
+  return (size_t)kne * kEpi * 8 + 6 * kEpi * 4 + 1024;
 }
 
 __device__ __forceinline__ Smem carve_smem(uint8_t* base, const RvqParams& p) {
   Smem s;
   s.ring1 = base;
   s.sRho = base;
-  s.ringC = base + (size_t)(p.r / 64) * kTileBytes;
+  s.sAx = s.sRho + (size_t)(p.r / 64) * kTileBytes;
+  s.ringC = s.sAx + kAxBytes;
+  s.ringX = s.ringC + (size_t)p.ring_tiles * kHalfTileBytes;
+  s.stash = s.ringX + (size_t)kXStages * kXBytes;
   uint8_t* t = base + rvq_regionR(p);
-  s.sHn = reinterpret_cast<float*>(t); t += (size_t)p.K * 4;
-  s.eM = reinterpret_cast<float*>(t); t += kNE * kEpi * 4;
-  s.eP = reinterpret_cast<int*>(t); t += kNE * kEpi * 4;
-  s.eMask = reinterpret_cast<uint32_t*>(t); t += kNE * kEpi * 4;
-  s.xch = reinterpret_cast<float*>(t); t += 5 * kEpi * 4;
+  s.eM = reinterpret_cast<float*>(t); t += (size_t)p.kne * kEpi * 4;
+  s.eId = reinterpret_cast<int*>(t); t += (size_t)p.kne * kEpi * 4;
+  s.xch = reinterpret_cast<float*>(t); t += 6 * kEpi * 4;
   uint64_t* b = reinterpret_cast<uint64_t*>(t);
   s.s1_full = b; b += p.stages1;
   s.s1_empty = b; b += p.stages1;
   s.z_full = b; b += 1;
   s.c_full = b; b += p.ring_tiles;
   s.c_empty = b; b += p.ring_tiles;
+  s.x_full = b; b += kXStages;
+  s.x_empty = b; b += kXStages;
   s.acc_full = b; b += 2;
   s.acc_empty = b; b += 2;
   s.rho_ready = b; b += 1;
@@ -104,13 +114,13 @@ __device__ __forceinline__ Smem carve_smem(uint8_t* base, const RvqParams& p) {
   return s;
 }
 
-// exact fp32 score of codeword row `crow` against this thread's residual (TMEM columns [0,r)):
-// 0.5||c||^2 - rho.c.  Warp-convergent (tcgen05.ld is .sync.aligned); lanes without work pass any
-// valid row and ignore the result.
-__device__ __forceinline__ float exact_score(uint32_t tmem_row, const float* __restrict__ crow, float hn, int r) {
+// exact fp32 squared distance of codeword row `crow` to this thread's residual (TMEM columns [0,r)), in the DIRECT
+// form sum_j (rho_j - c_j)^2 the oracle uses (no cancellation when D << ||c||^2).  Warp-convergent (tcgen05.ld is
+// .sync.aligned); lanes without work pass any valid row and ignore the result.
+__device__ __forceinline__ float exact_dist(uint32_t tmem_row, const float* __restrict__ crow, int r) {
   // the row loads (L2 latency) of TWO 32-column pieces are in flight together (r is a multiple of 64); the residual
   // pieces are read from TMEM one at a time to keep the register count down
-  float dot = 0.f;
+  float acc = 0.f;
   for (int pc = 0; pc < r / 32; pc += 2) {
     const float4* c4 = reinterpret_cast<const float4*>(crow + pc * 32);
     float4 c[16];
@@ -123,27 +133,55 @@ __device__ __forceinline__ float exact_score(uint32_t tmem_row, const float* __r
       tmem_ld_wait();
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
-        dot = fmaf(__uint_as_float(v[4 * i + 0]), c[8 * u + i].x, dot);
-        dot = fmaf(__uint_as_float(v[4 * i + 1]), c[8 * u + i].y, dot);
-        dot = fmaf(__uint_as_float(v[4 * i + 2]), c[8 * u + i].z, dot);
-        dot = fmaf(__uint_as_float(v[4 * i + 3]), c[8 * u + i].w, dot);
+        const float d0 = __uint_as_float(v[4 * i + 0]) - c[8 * u + i].x, d1 = __uint_as_float(v[4 * i + 1]) - c[8 * u + i].y;
+        const float d2 = __uint_as_float(v[4 * i + 2]) - c[8 * u + i].z, d3 = __uint_as_float(v[4 * i + 3]) - c[8 * u + i].w;
+        acc = fmaf(d0, d0, acc); acc = fmaf(d1, d1, acc); acc = fmaf(d2, d2, acc); acc = fmaf(d3, d3, acc);
       }
     }
   }
-  return hn - dot;
+  return acc;
 }
 
-// The kParts warps of a TMEM lane quarter split the residual by 32-column pieces: part h owns the
-// pieces pc with pc % kParts == h.
-// Step 1 of a residual update: rho <- rho - sub on the own pieces (sub == nullptr: rho unchanged);
-// returns the partial ||rho||^2 and max|rho_j| of those pieces.  Warp-convergent.
-__device__ __forceinline__ void rho_subtract(uint32_t tmem_row, const float* __restrict__ sub, int r, int h, float* n2_out,
-                                             float* amax_out) {
+// power of two inv with A * inv in [0.5, 1) for the bound A >= max|rho_j| (A == 0 / denormal: inv = 1)
+__device__ __forceinline__ float inv_scale_of(float A) {
+  int eb = (int)((__float_as_uint(A) >> 23) & 0xffu);
+  eb = eb < 2 ? 126 : (eb > 250 ? 250 : eb);
+  return __uint_as_float((uint32_t)(253 - eb) << 23);
+}
+
+__device__ __forceinline__ void store_operand_piece(uint8_t* sRho, int row, int pc, const uint32_t (&v)[32], float inv) {
+  uint8_t* tile = sRho + (size_t)(pc / 2) * kTileBytes;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    uint4 o;
+    o.x = pack_f16x2(__uint_as_float(v[8 * i + 0]) * inv, __uint_as_float(v[8 * i + 1]) * inv);
+    o.y = pack_f16x2(__uint_as_float(v[8 * i + 2]) * inv, __uint_as_float(v[8 * i + 3]) * inv);
+    o.z = pack_f16x2(__uint_as_float(v[8 * i + 4]) * inv, __uint_as_float(v[8 * i + 5]) * inv);
+    o.w = pack_f16x2(__uint_as_float(v[8 * i + 6]) * inv, __uint_as_float(v[8 * i + 7]) * inv);
+    *reinterpret_cast<uint4*>(tile + sw128_offset(row, (pc & 1) * 4 + i)) = o;
+  }
+}
+
+// The kParts threads of a token split the residual by 32-column pieces: part h owns the pieces pc with pc % kParts == h.
+// rho <- rho (+ second accumulator: the two halves of the projection chain) (- sub) on the own pieces; partial
+// ||rho||^2 and max|rho_j| of those pieces; with kConvert the fp16 rounding of rho * inv goes to the swizzled
+// A-operand tiles in the same pass.  Warp-convergent.
+template <bool kConvert>
+__device__ __forceinline__ void rho_update(uint32_t tmem_row, const float* __restrict__ sub, bool add_second, uint8_t* sRho,
+                                           int row, int r, int h, float inv, float* n2_out, float* amax_out) {
   float n2 = 0.f, amax = 0.f;
   for (int pc = h; pc < r / 32; pc += kParts) {
     uint32_t v[32];
     tmem_ld32(tmem_row + pc * 32, v);
-    tmem_ld_wait();
+    if (add_second) {
+      uint32_t w[32];
+      tmem_ld32(tmem_row + kAccCol0 + pc * 32, w);
+      tmem_ld_wait();
+#pragma unroll
+      for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(__uint_as_float(v[i]) + __uint_as_float(w[i]));
+    } else {
+      tmem_ld_wait();
+    }
     if (sub != nullptr) {
       const float4* c4 = reinterpret_cast<const float4*>(sub + pc * 32);
 #pragma unroll
@@ -154,50 +192,115 @@ __device__ __forceinline__ void rho_subtract(uint32_t tmem_row, const float* __r
         v[4 * i + 2] = __float_as_uint(__uint_as_float(v[4 * i + 2]) - c.z);
         v[4 * i + 3] = __float_as_uint(__uint_as_float(v[4 * i + 3]) - c.w);
       }
-      tmem_st32(tmem_row + pc * 32, v);
     }
+    if (sub != nullptr || add_second) tmem_st32(tmem_row + pc * 32, v);
 #pragma unroll
     for (int i = 0; i < 32; ++i) {
       const float x = __uint_as_float(v[i]);
       n2 = fmaf(x, x, n2);
       amax = fmaxf(amax, fabsf(x));
     }
+    if (kConvert) store_operand_piece(sRho, row, pc, v, inv);
   }
-  if (sub != nullptr) tmem_st_wait();
+  if (sub != nullptr || add_second) tmem_st_wait();
   *n2_out = n2; *amax_out = amax;
 }
 
-// Step 2: fp16(rho * 2^-e) of the own pieces into the swizzled A-operand tiles, 2^-e chosen from the
-// row's max|rho_j| so that it lands in [0.5,1); returns 2^e.  Warp-convergent.
-__device__ __forceinline__ float rho_to_operand(uint32_t tmem_row, uint8_t* sRho, int row, int r, int h, float amax) {
-  int eb = (int)((__float_as_uint(amax) >> 23) & 0xffu);
-  eb = eb < 2 ? 126 : (eb > 250 ? 250 : eb);
-  const float inv = __uint_as_float((uint32_t)(253 - eb) << 23);
+// fp16 conversion alone (level 0, once the exact max|z_j| of the token is known)
+__device__ __forceinline__ void rho_to_operand(uint32_t tmem_row, uint8_t* sRho, int row, int r, int h, float inv) {
   for (int pc = h; pc < r / 32; pc += kParts) {
     uint32_t v[32];
     tmem_ld32(tmem_row + pc * 32, v);
     tmem_ld_wait();
-    uint8_t* tile = sRho + (size_t)(pc / 2) * kTileBytes;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      uint4 o;
-      o.x = pack_f16x2(__uint_as_float(v[8 * i + 0]) * inv, __uint_as_float(v[8 * i + 1]) * inv);
-      o.y = pack_f16x2(__uint_as_float(v[8 * i + 2]) * inv, __uint_as_float(v[8 * i + 3]) * inv);
-      o.z = pack_f16x2(__uint_as_float(v[8 * i + 4]) * inv, __uint_as_float(v[8 * i + 5]) * inv);
-      o.w = pack_f16x2(__uint_as_float(v[8 * i + 6]) * inv, __uint_as_float(v[8 * i + 7]) * inv);
-      *reinterpret_cast<uint4*>(tile + sw128_offset(row, (pc & 1) * 4 + i)) = o;
-    }
+    store_operand_piece(sRho, row, pc, v, inv);
   }
-  return __uint_as_float((uint32_t)(eb + 1) << 23);
 }
 
 // named barrier 1 over the epilogue warps
 __device__ __forceinline__ void epi_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kEpi) : "memory"); }
 
+// maximum of 16 scores: 8 three-input maxima
+__device__ __forceinline__ float max16(const uint32_t* v) {
+#define MAPL_F(i) __uint_as_float(v[i])
+  const float a = fmaxf(fmaxf(MAPL_F(0), MAPL_F(1)), MAPL_F(2)), b = fmaxf(fmaxf(MAPL_F(3), MAPL_F(4)), MAPL_F(5));
+  const float c = fmaxf(fmaxf(MAPL_F(6), MAPL_F(7)), MAPL_F(8)), d = fmaxf(fmaxf(MAPL_F(9), MAPL_F(10)), MAPL_F(11));
+  const float e = fmaxf(fmaxf(MAPL_F(12), MAPL_F(13)), MAPL_F(14));
+  const float f = MAPL_F(15);
+#undef MAPL_F
+  return fmaxf(fmaxf(fmaxf(a, b), c), fmaxf(fmaxf(d, e), f));
+}
+
+// explicit shared-space accesses (pointers carved from the dynamic buffer compile to generic LD / ST otherwise)
+__device__ __forceinline__ float lds_f32(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
+__device__ __forceinline__ int lds_s32(uint32_t a) { int v; asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ uint4 lds_v4(uint32_t a) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ void sts_f32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ void sts_s32(uint32_t a, int v) { asm volatile("st.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ void sts_v4(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+  asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+
+// per-thread candidate list (shared memory): entry e of thread t has its maximum at eM[e * kEpi + t], its group id
+// (codeword index / 16) at eId[...], its 16 raw scores as four 16-byte units at stash[((e * 4 + i) * kEpi + t) * 16]
+// (consecutive lanes -> consecutive 16-byte units: conflict-free).
+struct CandList {
+  uint32_t eM, eId, stash;   // shared-space byte addresses, already offset by the thread index
+  int cnt;             // entries in use (high-water mark)
+  float dropped;       // highest maximum that found no room (-FLT_MAX: none)
+};
+
+// record the group `gid` (maximum m, scores v[0..16)); thr = current threshold.  Lane-divergent.  While the list has
+// room the group is appended; when it is full, a stale entry (below the current threshold, which only rises during a
+// scan) is reused, else the list keeps the kne highest maxima and remembers the highest maximum it let go: only if
+// that value is within the FINAL threshold does the thread need the exhaustive pass.  (A plain FIFO is cheaper but
+// overflows at r = 256, where many group maxima lie within the margin of each other: measured 3.2 ms instead of
+// 0.2 ms per config-3 encode.  The scan is bound by the TMEM read-out, not by these instructions.)
+__device__ __forceinline__ void stash_group(CandList& cl, int kne, float m, int gid, const uint32_t* v, float thr) {
+  int slot = -1;
+  if (cl.cnt < kne) {
+    slot = cl.cnt++;
+  } else {
+    int w = 0;
+    float wm = lds_f32(cl.eM);
+    for (int e = 1; e < kne; ++e) {
+      const float em = lds_f32(cl.eM + e * kEpi * 4);
+      if (em < wm) { wm = em; w = e; }
+    }
+    if (wm < thr) slot = w;                                           // stale entry: the threshold has passed it
+    else if (m > wm) { cl.dropped = fmaxf(cl.dropped, wm); slot = w; }   // keep the kne highest maxima
+    else cl.dropped = fmaxf(cl.dropped, m);
+  }
+  if (slot >= 0) {
+    sts_f32(cl.eM + slot * kEpi * 4, m);
+    sts_s32(cl.eId + slot * kEpi * 4, gid);
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+      sts_v4(cl.stash + (uint32_t)(slot * 4 + i) * kEpi * 16, v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+  }
+}
+
+// 16-bit mask of the scores >= thr in entry e
+__device__ __forceinline__ uint32_t entry_mask(const CandList& cl, int e, float thr) {
+  uint32_t mk = 0;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const uint4 q = lds_v4(cl.stash + (uint32_t)(e * 4 + i) * kEpi * 16);
+    mk |= (__uint_as_float(q.x) >= thr ? 1u : 0u) << (4 * i);
+    mk |= (__uint_as_float(q.y) >= thr ? 1u : 0u) << (4 * i + 1);
+    mk |= (__uint_as_float(q.z) >= thr ? 1u : 0u) << (4 * i + 2);
+    mk |= (__uint_as_float(q.w) >= thr ? 1u : 0u) << (4 * i + 3);
+  }
+  return mk;
+}
+
 __global__ void __launch_bounds__(kThreads, 1)
 k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmWhi,
-                const __grid_constant__ CUtensorMap tmWlo, const __grid_constant__ CUtensorMap tmC,
-                const RvqParams p) {
+                const __grid_constant__ CUtensorMap tmWlo, const __grid_constant__ CUtensorMap tmWlo2,
+                const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmX, const RvqParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const Smem s = carve_smem(smem, p);
@@ -206,12 +309,20 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
   const uint32_t rank = cluster_ctarank();
   const long long m0 = (long long)blockIdx.x * p.tile_m;
   const int nkb1 = p.d / 64, nkb = p.r / 64, nchunks = p.K / kChunk;
+  // Every CTA pair walks the codebook chunks (and the k-blocks of the projection) in its own rotation.  With one common
+  // order all 74 pairs request the SAME L2 lines at the same moment and the requests serialise in the L2 slices that
+  // hold them (measured at config 2: 2 us from TMA issue to arrival for an 8 KB L2-resident tile).  The arg-min does not
+  // depend on the scan order (ties are decided on the codeword index in the exact pass).
+  const int pair = blockIdx.x >> 1;
+  const int rot_c = (int)(((unsigned)pair * 5u) % (unsigned)nchunks), rot_k = (int)(((unsigned)pair * 7u) % (unsigned)nkb1);
 
   if (warp == 0 && lane == 0) {
-    tma_prefetch_desc(&tmH); tma_prefetch_desc(&tmWhi); tma_prefetch_desc(&tmWlo); tma_prefetch_desc(&tmC);
+    tma_prefetch_desc(&tmH); tma_prefetch_desc(&tmWhi); tma_prefetch_desc(&tmWlo); tma_prefetch_desc(&tmWlo2);
+    tma_prefetch_desc(&tmC); tma_prefetch_desc(&tmX);
     for (int i = 0; i < p.stages1; ++i) { mbar_init(&s.s1_full[i], 1); mbar_init(&s.s1_empty[i], 1); }
     mbar_init(s.z_full, 1);
     for (int i = 0; i < p.ring_tiles; ++i) { mbar_init(&s.c_full[i], 1); mbar_init(&s.c_empty[i], 1); }
+    for (int i = 0; i < kXStages; ++i) { mbar_init(&s.x_full[i], 1); mbar_init(&s.x_empty[i], 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(&s.acc_full[i], 1); mbar_init(&s.acc_empty[i], 8 * kParts); }
     mbar_init(s.rho_ready, 8 * kParts);               // leader's barriers collect the epilogue warps of both CTAs
     fence_barrier_init();
@@ -225,261 +336,289 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
   asm volatile("griddepcontrol.wait;" ::: "memory");       // everything below touches global memory
   if (warp == 0) { DBG(0) }
 
-  if (warp == 0) {
-    // ------------------------------------------------------------ TMA producer
+  if (warp == 0 || warp >= 2 + 4 * kParts) {
+    // ------------------------------------------------------------ TMA producers: items (stages) in turn
+    const int pi = warp == 0 ? 0 : warp - (1 + 4 * kParts);
     if (elect_one()) {
       const uint32_t w_tile = (uint32_t)p.r * 64;          // this CTA's half (r/2 rows) of a U^T tile
-      for (int kb = 0; kb < nkb1; ++kb) {
-        const int st = kb % p.stages1;
-        mbar_wait(&s.s1_empty[st], ((kb / p.stages1) & 1) ^ 1);
-        if (rank == 0) mbar_arrive_expect_tx(&s.s1_full[st], 2u * ((uint32_t)(p.tile_m * 128) + 2 * w_tile));
-        uint8_t* a = s.ring1 + (size_t)st * p.stage1_bytes;
-        tma_load_2d_pair(a, &tmH, &s.s1_full[st], kb * 64, (int)m0, kEvictFirst);
-        tma_load_2d_pair(a + kTileBytes, &tmWhi, &s.s1_full[st], kb * 64, (int)rank * (p.r / 2), kEvictLast);
-        tma_load_2d_pair(a + kTileBytes + w_tile, &tmWlo, &s.s1_full[st], kb * 64, (int)rank * (p.r / 2), kEvictLast);
+      const uint32_t tx1 = 2u * ((uint32_t)(p.tile_m * 128) + (uint32_t)p.nsplit * w_tile);
+      const int wrow = (int)rank * (p.r / 2);
+      // producers in use per phase: a producer may run at most ONE use of a ring slot ahead of the consumer (the
+      // barriers carry one phase bit), which holds when the producers' items together fit the ring
+      const int kP1 = p.p1, kP2 = p.p2;
+      RingPos r1;
+      r1.advance(pi, p.stages1);
+      int kr = pi + rot_k;
+      if (kr >= nkb1) kr -= nkb1;
+      for (int kb = pi < kP1 ? pi : nkb1; kb < nkb1; kb += kP1) {
+        mbar_wait(&s.s1_empty[r1.st], r1.ph ^ 1u);
+        if (rank == 0) mbar_arrive_expect_tx(&s.s1_full[r1.st], tx1);
+        uint8_t* a = s.ring1 + (size_t)r1.st * p.stage1_bytes;
+        tma_load_2d_pair(a, &tmH, &s.s1_full[r1.st], kr * 64, (int)m0, kEvictFirst);
+        tma_load_2d_pair(a + kTileBytes, &tmWhi, &s.s1_full[r1.st], kr * 64, wrow, kEvictLast);
+        tma_load_2d_pair(a + kTileBytes + w_tile, &tmWlo, &s.s1_full[r1.st], kr * 64, wrow, kEvictLast);
+        if (p.nsplit == 3) tma_load_2d_pair(a + kTileBytes + 2 * w_tile, &tmWlo2, &s.s1_full[r1.st], kr * 64, wrow, kEvictLast);
+        r1.advance(kP1, p.stages1);
+        kr += kP1;
+        if (kr >= nkb1) kr -= nkb1;
       }
       mbar_wait(s.z_full, 0);             // phase-1 MMAs have consumed region R: it may be reused
-      int it = 0;
-      for (int l = 0; l < p.L; ++l)
-        for (int c = 0; c < nchunks; ++c)
-          for (int kb = 0; kb < nkb; ++kb, ++it) {
-            const int st = it % p.ring_tiles;
-            mbar_wait(&s.c_empty[st], ((it / p.ring_tiles) & 1) ^ 1);
-            if (rank == 0) mbar_arrive_expect_tx(&s.c_full[st], 2 * kHalfTileBytes);
-            tma_load_2d_pair(s.ringC + (size_t)st * kHalfTileBytes, &tmC, &s.c_full[st], kb * 64,
-                             l * p.K + c * kChunk + (int)rank * (kChunk / 2), kEvictLast);
-          }
+      // level phase: producer pi takes the chunks pi, pi + kProducers, ... (counted over all levels): the chunk's nkb
+      // codebook tiles and its norm tile
+      RingPos rc, rx;
+      rc.advance(pi * nkb, p.ring_tiles);
+      rx.advance(pi, kXStages);
+      int c = pi, l = pi < kP2 ? 0 : p.L;
+      while (c >= nchunks) { c -= nchunks; ++l; }
+      while (l < p.L) {
+        int cr = c + rot_c;
+        if (cr >= nchunks) cr -= nchunks;
+        const int row0 = l * p.K + cr * kChunk + (int)rank * (kChunk / 2);
+        RingPos t = rc;
+        for (int j = 0; j < nkb; ++j) {
+          mbar_wait(&s.c_empty[t.st], t.ph ^ 1u);
+          if (rank == 0) mbar_arrive_expect_tx(&s.c_full[t.st], 2 * kHalfTileBytes);
+          tma_load_2d_pair(s.ringC + (size_t)t.st * kHalfTileBytes, &tmC, &s.c_full[t.st], j * 64, row0, kEvictLast);
+          t.next(p.ring_tiles);
+        }
+        mbar_wait(&s.x_empty[rx.st], rx.ph ^ 1u);
+        if (rank == 0) mbar_arrive_expect_tx(&s.x_full[rx.st], 2 * kXBytes);
+        tma_load_2d_pair(s.ringX + (size_t)rx.st * kXBytes, &tmX, &s.x_full[rx.st], 0, row0, kEvictLast);
+        rc.advance(kP2 * nkb, p.ring_tiles);
+        rx.advance(kP2, kXStages);
+        c += kP2;
+        while (c >= nchunks) { c -= nchunks; ++l; }
+      }
     }
   } else if (warp == 1) {
     // ------------------------------------------------------------ MMA issuer
     if (rank == 0 && elect_one()) {
       const uint32_t idesc1 = make_idesc_bf16(256, (uint32_t)p.r, false, false);
+      RingPos r1;
       for (int kb = 0; kb < nkb1; ++kb) {
-        const int st = kb % p.stages1;
-        mbar_wait(&s.s1_full[st], (kb / p.stages1) & 1);
+        mbar_wait(&s.s1_full[r1.st], r1.ph);
         tc_fence_after_sync();
-        const uint32_t a = smem_u32(s.ring1 + (size_t)st * p.stage1_bytes);
-        const uint32_t bh = a + kTileBytes, bl = bh + p.r * 64;
+        const uint32_t a = smem_u32(s.ring1 + (size_t)r1.st * p.stage1_bytes);
+        const uint32_t bh = a + kTileBytes, bl = bh + p.r * 64, bl2 = bl + p.r * 64;
+        // even / odd k-blocks accumulate into two TMEM regions ([0,r) and the still unused score stages at
+        // [256,256+r)): the tensor core truncates when it adds into its accumulator, and halving the chain of
+        // MMAs halves that one-sided error of z (tc_stiefel.cu measures it); the epilogue adds the two halves
+        const uint32_t acc = tmem_base + (uint32_t)(kb & 1) * kAccCol0;
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           const uint64_t da = desc_kmajor_sw128(a + k * 32);
-          // even / odd k-blocks accumulate into two TMEM regions ([0,r) and the still unused score stages at
-          // [256,256+r)): the tensor core truncates when it adds into its accumulator, and halving the chain of
-          // MMAs halves that one-sided error of z (tc_stiefel.cu measures it); the epilogue adds the two halves
-          const uint32_t acc = tmem_base + (uint32_t)(kb & 1) * kAccCol0;
           umma_bf16_pair(acc, da, desc_kmajor_sw128(bh + k * 32), idesc1, (kb >= 2) || k != 0);
           umma_bf16_pair(acc, da, desc_kmajor_sw128(bl + k * 32), idesc1, 1);
+          if (p.nsplit == 3) umma_bf16_pair(acc, da, desc_kmajor_sw128(bl2 + k * 32), idesc1, 1);
         }
-        umma_commit_pair(&s.s1_empty[st]);
+        umma_commit_pair(&s.s1_empty[r1.st]);
+        r1.next(p.stages1);
       }
       umma_commit_pair(s.z_full);
       const uint32_t idesc2 = make_idesc_f16(256, kChunk);
-      int it = 0, cg = 0;
+      const uint64_t dax = desc_kmajor_sw32_k16(smem_u32(s.sAx));
+      const uint32_t sRho0 = smem_u32(s.sRho), ringC0 = smem_u32(s.ringC), ringX0 = smem_u32(s.ringX);
+      RingPos rc, rx;
+      uint32_t as = 0, aph = 0;            // accumulator stage and its use parity
+      int cg = 0;
       for (int l = 0; l < p.L; ++l) {
-        mbar_wait_cluster(s.rho_ready, l & 1);    // fp16 residuals of level l are in sRho of both CTAs
+        mbar_wait_cluster(s.rho_ready, l & 1);    // fp16 residuals of level l are in sRho / sAx of both CTAs
         tc_fence_after_sync();
         for (int c = 0; c < nchunks; ++c, ++cg) {
-          const int as = cg & 1;
-          mbar_wait_cluster(&s.acc_empty[as], ((cg >> 1) & 1) ^ 1);
+          mbar_wait_cluster(&s.acc_empty[as], aph ^ 1u);
           if (cg < 8) DBGT(24 + cg)
           tc_fence_after_sync();
           const uint32_t tmem_d = tmem_base + kAccCol0 + as * kChunk;
-          for (int kb = 0; kb < nkb; ++kb, ++it) {
-            const int st = it % p.ring_tiles;
-            mbar_wait(&s.c_full[st], (it / p.ring_tiles) & 1);
+          for (int kb = 0; kb < nkb; ++kb) {
+            mbar_wait(&s.c_full[rc.st], rc.ph);
             tc_fence_after_sync();
-            const uint32_t a = smem_u32(s.sRho + (size_t)kb * kTileBytes), b = smem_u32(s.ringC + (size_t)st * kHalfTileBytes);
+            const uint32_t a = sRho0 + (uint32_t)kb * kTileBytes, b = ringC0 + (uint32_t)rc.st * kHalfTileBytes;
 #pragma unroll
             for (int k = 0; k < 4; ++k)
               umma_bf16_pair(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc2, (kb | k) != 0);
-            umma_commit_pair(&s.c_empty[st]);
+            umma_commit_pair(&s.c_empty[rc.st]);
+            rc.next(p.ring_tiles);
           }
+          mbar_wait(&s.x_full[rx.st], rx.ph);       // + a' * (-q_k): the half norms, one K = 16 step
+          tc_fence_after_sync();
+          umma_bf16_pair(tmem_d, dax, desc_kmajor_sw32_k16(ringX0 + (uint32_t)rx.st * kXBytes), idesc2, 1);
+          umma_commit_pair(&s.x_empty[rx.st]);
           umma_commit_pair(&s.acc_full[as]);
+          rx.next(kXStages);
           if (cg < 8) DBGT(32 + cg)
+          as ^= 1u;
+          if (as == 0) aph ^= 1u;
         }
       }
     }
   } else {
     // ------------------------------------------------------------ epilogue: 4 kParts warps, kParts threads per token
     // q = TMEM lane quarter, h = which part of the 32-codeword pieces / 32-column pieces this warp owns
-    const int q = warp & 3, h = (warp - 2) >> 2, row = q * 32 + lane, et = threadIdx.x - 64;
+    const int q = warp & 3, h = (warp - 2) >> 2, row = q * 32 + lane;
     const long long m = m0 + row;
     const bool live = row < p.tile_m && m < p.N;
     const uint32_t tmem_row = tmem_base + ((uint32_t)(q * 32) << 16);
     const unsigned full = 0xffffffffu;
-    float* xBest = s.xch; float* xScore = s.xch + kEpi; int* xK = reinterpret_cast<int*>(s.xch + 2 * kEpi);
-    float* xN2 = s.xch + 3 * kEpi; float* xAmax = s.xch + 4 * kEpi;
+    float* xBest = s.xch; float* xDist = s.xch + kEpi; int* xK = reinterpret_cast<int*>(s.xch + 2 * kEpi);
+    float* xN2 = s.xch + 3 * kEpi; float* xAmax = s.xch + 4 * kEpi; int* xCnt = reinterpret_cast<int*>(s.xch + 5 * kEpi);
     const int mine = h * 128 + row;
-    float* eM = s.eM + mine; int* eP = s.eP + mine; uint32_t* eMask = s.eMask + mine;   // entry e at [e * kEpi]
+    CandList cl;
+    cl.eM = smem_u32(s.eM + mine); cl.eId = smem_u32(s.eId + mine); cl.stash = smem_u32(s.stash) + (uint32_t)mine * 16;
     int code_l[8];
 #pragma unroll
     for (int l = 0; l < 8; ++l) code_l[l] = 0;
-    const uint32_t sHn_u32 = smem_u32(s.sHn);
+    const float sqrt_r = sqrtf((float)p.r), n_steps = (float)(p.r / 16 + 1);
+
+    // the norm step's A row of this token: a' in all 16 columns (0 when a' is not an fp16 power of two: `hard` token)
+    auto write_ax = [&](float ax, bool& hard) {
+      hard = !(ax >= 5.9604645e-8f && ax <= 32768.f);
+      if (h == 0) {
+        const uint32_t w = pack_f16x2(hard ? 0.f : ax, hard ? 0.f : ax);
+        uint4* dst = reinterpret_cast<uint4*>(s.sAx + (size_t)row * 32);
+        dst[0] = make_uint4(w, w, w, w);
+        dst[1] = make_uint4(w, w, w, w);
+      }
+    };
+    auto publish_operand = [&]() {     // sRho / sAx rows of this warp are written: hand them to the MMA issuer
+      fence_proxy_async_smem();
+      tc_fence_before_sync();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_leader(s.rho_ready);
+    };
 
     mbar_wait(s.z_full, 0);
     if (warp == 2) { DBG(1) }
     tc_fence_after_sync();
-    float n2, amax;
-    if (nkb1 >= 2) {                     // z = even-k-block half + odd-k-block half (see the MMA issuer)
-      for (int pc = h; pc < p.r / 32; pc += kParts) {
-        uint32_t v[32], w[32];
-        tmem_ld32(tmem_row + pc * 32, v);
-        tmem_ld32(tmem_row + kAccCol0 + pc * 32, w);
-        tmem_ld_wait();
+    float n2, amax, inv;
+    bool hard;
+    {
+      // z = even-k-block half + odd-k-block half (see the MMA issuer), minus the centring row: the first residual is
+      // z - Tc[tok] (dead rows subtract row 0: any valid row keeps the warp convergent)
+      const float* csub = p.Tc != nullptr ? p.Tc + (live ? (long long)__ldg(p.tok + m) * p.r : 0) : nullptr;
+      float n2p, amaxp;
+      rho_update<false>(tmem_row, csub, nkb1 >= 2, s.sRho, row, p.r, h, 0.f, &n2p, &amaxp);
+      xN2[mine] = n2p; xAmax[mine] = amaxp;
+      epi_sync();
+      n2 = 0.f; amax = 0.f;
 #pragma unroll
-        for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(__uint_as_float(v[i]) + __uint_as_float(w[i]));
-        tmem_st32(tmem_row + pc * 32, v);
-      }
-      tmem_st_wait();
+      for (int hh = 0; hh < kParts; ++hh) { n2 += xN2[hh * 128 + row]; amax = fmaxf(amax, xAmax[hh * 128 + row]); }
+      inv = inv_scale_of(amax);
+      rho_to_operand(tmem_row, s.sRho, row, p.r, h, inv);
+      write_ax(inv * __ldg(p.lvl + 2), hard);
+      publish_operand();
     }
-    // centring: the first residual is z - Tc[tok] (dead rows subtract row 0: any valid row keeps the warp convergent)
-    const float* csub = p.Tc != nullptr ? p.Tc + (live ? (long long)__ldg(p.tok + m) * p.r : 0) : nullptr;
-    rho_subtract(tmem_row, csub, p.r, h, &n2, &amax);
-    xN2[mine] = n2; xAmax[mine] = amax;
-    epi_sync();
-    n2 = 0.f; amax = 0.f;
-#pragma unroll
-    for (int hh = 0; hh < kParts; ++hh) { n2 += xN2[hh * 128 + row]; amax = fmaxf(amax, xAmax[hh * 128 + row]); }
-    float unscale = rho_to_operand(tmem_row, s.sRho, row, p.r, h, amax);
-    fence_proxy_async_smem();
-    tc_fence_before_sync();
-    __syncwarp();
-    if (lane == 0) mbar_arrive_leader(s.rho_ready);
 
     int cg = 0;
 #pragma unroll 1
     for (int l = 0; l < p.L; ++l) {
       const float* Cl = p.C + (long long)l * p.K * p.r;
-      for (int i = et; i < p.K / 4; i += kEpi)
-        reinterpret_cast<float4*>(s.sHn)[i] = __ldg(reinterpret_cast<const float4*>(p.hn + (long long)l * p.K) + i);
-      epi_sync();
+      const float* lv = p.lvl + 8 * l;
       if (warp == 2 && l < 4) { DBG(4 + l * 4) }
-      const float margin = 0.001953125f * 1.05f * sqrtf(n2) * __ldg(p.cmax + l);
-      const float nsc = -unscale * __ldg(p.cscale + 8 + l);     // coarse S -> rho.c
+      // 2E in the scaled units of T (file header): operand rounding, accumulation, the split of q
+      float margin;
+      {
+        const float cmax_s = __ldg(lv), qmax = __ldg(lv + 1), ax = inv * __ldg(lv + 2);
+        const float rs = sqrtf(n2) * inv;
+        const float smax = rs * cmax_s + ax * qmax;
+        const float e_op = 9.765625e-4f * 1.002f * rs * cmax_s + 2.9802322e-8f * sqrt_r * (cmax_s + rs);
+        const float e_acc = n_steps * 1.9073486e-6f * (smax + 1.f);
+        const float e_hn = ax * (1.1641532e-10f * qmax + 2.9802322e-8f);
+        margin = 2.02f * (e_op + e_acc + e_hn);
+      }
 
-      float best = FLT_MAX;
-      int cnt = 0;
-      float dropped = FLT_MAX;           // lowest piece minimum that found no room in the list
+      float best = -FLT_MAX;
+      cl.cnt = 0; cl.dropped = -FLT_MAX;
+      int cr = rot_c;
       for (int c = 0; c < nchunks; ++c, ++cg) {
         const int as = cg & 1;
         mbar_wait(&s.acc_full[as], (cg >> 1) & 1);
         if (threadIdx.x == 64 && cg < 8) DBGT(40 + cg)
         tc_fence_after_sync();
-        uint32_t v[4 / kParts][32];            // this warp's pieces of the chunk: h, h + kParts, ...
-#pragma unroll
-        for (int pp = 0; pp < 4 / kParts; ++pp) tmem_ld32(tmem_row + kAccCol0 + as * kChunk + (h + kParts * pp) * 32, v[pp]);
+        uint32_t v[2][32];            // this warp's pieces of the chunk: h and h + kParts
+        tmem_ld32(tmem_row + kAccCol0 + as * kChunk + h * 32, v[0]);
+        tmem_ld32(tmem_row + kAccCol0 + as * kChunk + (h + kParts) * 32, v[1]);
         tmem_ld_wait();
         tc_fence_before_sync();
         __syncwarp();
         if (lane == 0) mbar_arrive_leader(&s.acc_empty[as]);     // scores are in registers: the stage is free
         if (threadIdx.x == 64 && cg < 8) DBGT(48 + cg)
-#pragma unroll
-        for (int pp = 0; pp < 4 / kParts; ++pp) {
-          const int piece = c * (kChunk / 32) + h + kParts * pp;
-#ifdef MAPL_DBG
-          if (threadIdx.x == 64 && cg < 8 && pp == 1) DBGT(56 + cg)      // piece 0 of the chunk done
-#endif
-          const uint32_t h4 = sHn_u32 + piece * 128;      // explicit ld.shared: the carved pointers compile to generic loads
-          float sc[32];
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            float4 hh;
-            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(hh.x), "=f"(hh.y), "=f"(hh.z), "=f"(hh.w) : "r"(h4 + 16 * i));
-            sc[4 * i + 0] = fmaf(__uint_as_float(v[pp][4 * i + 0]), nsc, hh.x);
-            sc[4 * i + 1] = fmaf(__uint_as_float(v[pp][4 * i + 1]), nsc, hh.y);
-            sc[4 * i + 2] = fmaf(__uint_as_float(v[pp][4 * i + 2]), nsc, hh.z);
-            sc[4 * i + 3] = fmaf(__uint_as_float(v[pp][4 * i + 3]), nsc, hh.w);
-          }
-          // The min / compare instructions run on the half-rate ALU pipe, which bounds this loop at r = 64: three-input
-          // minima, and the candidate mask from the sign bits of thr - sc (an FADD on the FMA pipe and one funnel
-          // shift per codeword instead of FSETP + SEL + OR).
-          float mn[4];
-#pragma unroll
-          for (int g = 0; g < 4; ++g) {
-            const float a = fminf(fminf(sc[8 * g], sc[8 * g + 1]), sc[8 * g + 2]);
-            const float b = fminf(fminf(sc[8 * g + 3], sc[8 * g + 4]), sc[8 * g + 5]);
-            mn[g] = fminf(fminf(a, b), fminf(sc[8 * g + 6], sc[8 * g + 7]));
-          }
-          const float m32 = fminf(fminf(mn[0], mn[1]), fminf(mn[2], mn[3]));
-          best = fminf(best, m32);
-          const float thr = best + margin;
-          if (__any_sync(full, live && m32 <= thr)) {      // dead rows hold stale smem: never candidates
-            // bit i of mask <=> sc[i] <= thr <=> sign(thr - sc[i]) clear (thr - sc == +0 when equal)
-            uint32_t mk[4] = {0u, 0u, 0u, 0u};
-#pragma unroll
-            for (int g = 0; g < 4; ++g)
-#pragma unroll
-              for (int i = 7; i >= 0; --i) mk[g] = __funnelshift_l(__float_as_uint(thr - sc[8 * g + i]), mk[g], 1);
-            const uint32_t mask = ~(mk[0] | (mk[1] << 8) | (mk[2] << 16) | (mk[3] << 24));
-            if (live && mask != 0) {
-              if (cnt == kNE) {                 // list full: drop entries the tighter threshold excludes
-                int j = 0;
-                for (int e = 0; e < kNE; ++e) {
-                  const float em = eM[e * kEpi];
-                  if (em <= thr) { eM[j * kEpi] = em; eP[j * kEpi] = eP[e * kEpi]; eMask[j * kEpi] = eMask[e * kEpi]; ++j; }
-                }
-                cnt = j;
-              }
-              if (cnt == kNE) {
-                // still full: the list keeps the kNE pieces with the lowest minima.  A piece left out matters only if
-                // its minimum is within the FINAL threshold (checked after the scan; the threshold only tightens), so a
-                // list that is full for a moment under the early, loose threshold no longer forces the exhaustive pass.
-                int w = 0;
-                float wm = eM[0];
-                for (int e = 1; e < kNE; ++e) {
-                  const float em = eM[e * kEpi];
-                  if (em > wm) { wm = em; w = e; }
-                }
-                if (m32 < wm) {
-                  dropped = fminf(dropped, wm);
-                  eM[w * kEpi] = m32; eP[w * kEpi] = piece; eMask[w * kEpi] = mask;     // entries no longer ascend in k
-                } else {
-                  dropped = fminf(dropped, m32);
-                }
-              } else {
-                eM[cnt * kEpi] = m32; eP[cnt * kEpi] = piece; eMask[cnt * kEpi] = mask; ++cnt;
-              }
-            }
-          }
+        const float g0 = max16(&v[0][0]), g1 = max16(&v[0][16]), g2 = max16(&v[1][0]), g3 = max16(&v[1][16]);
+        const float m64 = fmaxf(fmaxf(g0, g1), fmaxf(g2, g3));
+        best = fmaxf(best, m64);
+        const float thr = best - margin;
+        // dead rows hold stale data: never candidates.  (With 32 tokens per warp some lane qualifies in nearly every
+        // chunk -- a token's running maximum is beaten ~ln(groups) times per level -- so there is no warp vote.)
+        if (live && m64 >= thr) {
+          const int gid = (cr * 4 + h) * 2;                // 16-codeword group of v[0][0]; v[1] is kParts pieces further
+          if (g0 >= thr) stash_group(cl, p.kne, g0, gid, &v[0][0], thr);
+          if (g1 >= thr) stash_group(cl, p.kne, g1, gid + 1, &v[0][16], thr);
+          if (g2 >= thr) stash_group(cl, p.kne, g2, gid + 2 * kParts, &v[1][0], thr);
+          if (g3 >= thr) stash_group(cl, p.kne, g3, gid + 2 * kParts + 1, &v[1][16], thr);
         }
+        if (++cr == nchunks) cr = 0;
+        if (threadIdx.x == 64 && cg < 8) DBGT(56 + cg)
       }
       xBest[mine] = best;
       epi_sync();
 #pragma unroll
-      for (int hh = 0; hh < kParts; ++hh) best = fminf(best, xBest[hh * 128 + row]);
+      for (int hh = 0; hh < kParts; ++hh) best = fmaxf(best, xBest[hh * 128 + row]);
       if (warp == 2 && l < 4) { DBG(5 + l * 4) }
 
-      // ---- exact fp32 re-scoring of this thread's candidates: lowest score, lowest index on ties
-      const float thr = best + margin;
-      const bool overflow = live && dropped <= thr;     // pathological (e.g. many duplicate codewords): exhaustive below
-      float bestx = FLT_MAX;
-      int bestk = 0x7fffffff, e = 0, piece = 0;
-      uint32_t mrem = 0;
-      while (true) {
-        while (mrem == 0 && e < cnt) {
-          if (eM[e * kEpi] <= thr) { mrem = eMask[e * kEpi]; piece = eP[e * kEpi]; }
-          ++e;
+      // ---- candidates: every stashed score within the final threshold
+      const float thr = best - margin;
+      const bool overflow = live && (hard || cl.dropped >= thr);     // pathological (e.g. many duplicate codewords)
+      int ncand = 0, firstk = 0;
+      const int n_ent = cl.cnt;
+      for (int e = 0; e < n_ent; ++e) {
+        if (lds_f32(cl.eM + e * kEpi * 4) >= thr) {
+          const uint32_t mk = entry_mask(cl, e, thr);
+          if (mk != 0 && ncand == 0) firstk = lds_s32(cl.eId + e * kEpi * 4) * 16 + __ffs(mk) - 1;
+          ncand += __popc(mk);
         }
-        const bool have = mrem != 0 && !overflow;
-        if (!__any_sync(full, have)) break;
-        int k = 0;
-        if (have) { k = piece * 32 + __ffs(mrem) - 1; mrem &= mrem - 1; }
-        const float sx = exact_score(tmem_row, Cl + (long long)k * p.r, s.sHn[k], p.r);
-        if (have && (sx < bestx || (sx == bestx && k < bestk))) { bestx = sx; bestk = k; }
       }
-      if (__any_sync(full, overflow)) {         // exhaustive over the pieces this warp owns
+      if (!live) ncand = 0;
+      xCnt[mine] = overflow ? 1000 : ncand;
+      epi_sync();
+      if (warp == 2 && l < 4) { DBG(7 + l * 4) }
+      int tot = 0;
+#pragma unroll
+      for (int hh = 0; hh < kParts; ++hh) tot += xCnt[hh * 128 + row];
+      // a single candidate is the minimiser (it is always among the candidates); else exact fp32 re-scoring,
+      // lowest distance, lowest index on ties
+      const bool rescore = tot >= 2;
+      float bestx = FLT_MAX;
+      int bestk = 0x7fffffff;
+      if (!rescore && ncand == 1) { bestx = -1.f; bestk = firstk; }
+      {
+        int e = 0, gid = 0;
+        uint32_t mrem = 0;
+        while (true) {
+          while (mrem == 0 && e < n_ent) {
+            if (lds_f32(cl.eM + e * kEpi * 4) >= thr) { mrem = entry_mask(cl, e, thr); gid = lds_s32(cl.eId + e * kEpi * 4); }
+            ++e;
+          }
+          const bool have = rescore && !overflow && live && mrem != 0;
+          if (!__any_sync(full, have)) break;
+          int k = 0;
+          if (have) { k = gid * 16 + __ffs(mrem) - 1; mrem &= mrem - 1; }
+          const float dx = exact_dist(tmem_row, Cl + (long long)k * p.r, p.r);
+          if (have && (dx < bestx || (dx == bestx && k < bestk))) { bestx = dx; bestk = k; }
+        }
+      }
+      if (__any_sync(full, overflow)) {         // exhaustive over the pieces this thread owns
         for (int pc = h; pc < p.K / 32; pc += kParts)
           for (int i = 0; i < 32; ++i) {
             const int k = pc * 32 + i;
-            const float sx = exact_score(tmem_row, Cl + (long long)k * p.r, s.sHn[k], p.r);
-            if (overflow && sx < bestx) { bestx = sx; bestk = k; }
+            const float dx = exact_dist(tmem_row, Cl + (long long)k * p.r, p.r);
+            if (overflow && dx < bestx) { bestx = dx; bestk = k; }
           }
       }
-      xScore[mine] = bestx; xK[mine] = bestk;
+      if (warp == 2 && l == 1) { DBG(20) }
+      xDist[mine] = bestx; xK[mine] = bestk;
       epi_sync();
 #pragma unroll
       for (int hh = 0; hh < kParts; ++hh) {
-        const float ox = xScore[hh * 128 + row];
+        const float ox = xDist[hh * 128 + row];
         const int ok = xK[hh * 128 + row];
         if (ox < bestx || (ox == bestx && ok < bestk)) { bestx = ox; bestk = ok; }
       }
@@ -489,17 +628,20 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       if (warp == 2 && l < 4) { DBG(6 + l * 4) }
       if (live && h == 0) p.codes[m * p.L + l] = bestk;
       if (l + 1 < p.L) {
-        rho_subtract(tmem_row, Cl + (long long)bestk * p.r, p.r, h, &n2, &amax);
-        xN2[mine] = n2; xAmax[mine] = amax;
+        // rho -= C[l, k*] and, in the same pass, its fp16 operand for level l+1.  The scale only has to keep fp16 in
+        // its normal range, so it comes from the bound max|rho_new| <= max|rho| + max|c| (no second pass for the exact
+        // maximum); the exact ||rho_new||^2 and max|rho_new| are exchanged behind the hand-off.
+        inv = inv_scale_of(amax + __ldg(lv + 4));
+        float n2p, amaxp;
+        rho_update<true>(tmem_row, Cl + (long long)bestk * p.r, false, s.sRho, row, p.r, h, inv, &n2p, &amaxp);
+        xN2[mine] = n2p; xAmax[mine] = amaxp;
+        write_ax(inv * __ldg(lv + 8 + 2), hard);
+        if (warp == 2 && l == 1) { DBG(21) }
+        publish_operand();
         epi_sync();
         n2 = 0.f; amax = 0.f;
 #pragma unroll
         for (int hh = 0; hh < kParts; ++hh) { n2 += xN2[hh * 128 + row]; amax = fmaxf(amax, xAmax[hh * 128 + row]); }
-        unscale = rho_to_operand(tmem_row, s.sRho, row, p.r, h, amax);
-        fence_proxy_async_smem();
-        tc_fence_before_sync();
-        __syncwarp();
-        if (lane == 0) mbar_arrive_leader(s.rho_ready);
       }
     }
 
@@ -535,33 +677,50 @@ namespace mapl {
 
 int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
                   int32_t* codes_out, cudaStream_t st, const int32_t* tok, const float* Tc) {
-  if (!tc_rvq_ok(d) || !pk.WBlo || !pk.Cb) return MAPL_ERR_UNSUPPORTED;
+  if (!tc_rvq_ok(d) || !pk.WBlo || !pk.Cb || !pk.hnb) return MAPL_ERR_UNSUPPORTED;
   RvqParams p;
-  p.C = codebooks; p.hn = pk.hn; p.cmax = pk.cmax; p.cscale = pk.cscale; p.tok = tok; p.Tc = Tc;
+  p.C = codebooks; p.lvl = pk.lvl; p.tok = tok; p.Tc = Tc;
   p.Zq = reinterpret_cast<__nv_bfloat16*>(Zq_out); p.codes = codes_out;
   p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.L = d.rvq_levels; p.K = d.rvq_k;
   p.tile_m = tc_tile_m(d.n_tokens);
-  p.stage1_bytes = kTileBytes + 2 * d.r * 64;
-  p.stages1 = 2; p.ring_tiles = 2;
-  const size_t avail = (size_t)227 * 1024 - 1024 - rvq_tail_bytes(p);
-  if (avail < (size_t)2 * p.stage1_bytes || avail < (size_t)(d.r / 64 + 1) * kTileBytes) return MAPL_ERR_UNSUPPORTED;
-  p.stages1 = (int)(avail / p.stage1_bytes);
+  p.nsplit = pk.WBlo2 ? 3 : 2;
+  p.stage1_bytes = kTileBytes + p.nsplit * d.r * 64;
+  // shared memory: the candidate lists take what the codebook ring can spare -- at least two chunks of codebook tiles
+  // in flight, then as many list entries (16-codeword groups) per thread as fit, 8 at most, 3 at least
+  const int nkb = d.r / 64;
+  const size_t cap = (size_t)227 * 1024 - 1024;
+  p.kne = 0; p.ring_tiles = 0;
+  for (int kne = 8; kne >= 3 && p.kne == 0; --kne)
+    for (int want = 2 * nkb; want >= nkb + 1 && p.kne == 0; --want) {
+      p.kne = kne; p.ring_tiles = want; p.stages1 = 0;
+      if (rvq_level_bytes(p) + rvq_tail_bytes(kne) > cap) p.kne = 0;
+    }
+  if (p.kne == 0) return MAPL_ERR_UNSUPPORTED;
+  {   // the rest of the level region goes to the ring
+    const size_t spare = cap - rvq_tail_bytes(p.kne) - rvq_level_bytes(p);
+    p.ring_tiles += (int)(spare / kHalfTileBytes);
+    if (p.ring_tiles > 16) p.ring_tiles = 16;
+  }
+  p.stages1 = (int)((cap - rvq_tail_bytes(p.kne)) / p.stage1_bytes);
   if (p.stages1 > 8) p.stages1 = 8;
   if (p.stages1 > d.d / 64) p.stages1 = d.d / 64;
-  p.ring_tiles = (int)((avail - (size_t)(d.r / 64) * kTileBytes) / kHalfTileBytes);
-  if (p.ring_tiles > 16) p.ring_tiles = 16;
-  if (p.stages1 < 2 || p.ring_tiles < 2) return MAPL_ERR_UNSUPPORTED;
-  const size_t smem = 1024 + rvq_regionR(p) + rvq_tail_bytes(p);
-  CUtensorMap tmH, tmWhi, tmWlo, tmC;
-  const uint64_t dd = (uint64_t)d.d, rr = (uint64_t)d.r;
+  if (p.stages1 < 2) return MAPL_ERR_UNSUPPORTED;
+  const size_t smem = 1024 + rvq_regionR(p) + rvq_tail_bytes(p.kne);
+  if (smem > (size_t)227 * 1024) return MAPL_ERR_UNSUPPORTED;
+  p.p1 = p.stages1 < kProducers ? p.stages1 : kProducers;
+  p.p2 = p.ring_tiles / nkb < kProducers ? p.ring_tiles / nkb : kProducers;
+  CUtensorMap tmH, tmWhi, tmWlo, tmWlo2, tmC, tmX;
+  const uint64_t dd = (uint64_t)d.d, rr = (uint64_t)d.r, LK = (uint64_t)d.rvq_levels * d.rvq_k;
   if (!make_tmap_bf16_2d(&tmH, H, (uint64_t)d.n_tokens, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
   if (!make_tmap_bf16_2d(&tmWhi, pk.WB, rr, dd, dd, 64, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
   if (!make_tmap_bf16_2d(&tmWlo, pk.WBlo, rr, dd, dd, 64, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
-  if (!make_tmap_bf16_2d(&tmC, pk.Cb, (uint64_t)d.rvq_levels * d.rvq_k, rr, rr, 64, kChunk / 2)) return MAPL_ERR_CUDA;
+  if (!make_tmap_bf16_2d(&tmWlo2, pk.WBlo2 ? pk.WBlo2 : pk.WBlo, rr, dd, dd, 64, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
+  if (!make_tmap_bf16_2d(&tmC, pk.Cb, LK, rr, rr, 64, kChunk / 2)) return MAPL_ERR_CUDA;
+  if (!make_tmap_b16_k16_sw32(&tmX, pk.hnb, LK, kChunk / 2)) return MAPL_ERR_CUDA;
   MAPL_SMEM_OPT_IN(k_tc_encode_rvq, 227 * 1024);
   const unsigned tiles = ((unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m) + 1u) & ~1u;   // whole CTA pairs
   KernelScope ks(KID_TC_ENCODE_RVQ, st);
-  MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_encode_rvq, dim3(tiles), dim3(kThreads), smem, st, tmH, tmWhi, tmWlo, tmC, p));
+  MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_encode_rvq, dim3(tiles), dim3(kThreads), smem, st, tmH, tmWhi, tmWlo, tmWlo2, tmC, tmX, p));
   return MAPL_OK;
 }
 

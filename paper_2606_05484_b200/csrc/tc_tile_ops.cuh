@@ -34,6 +34,22 @@ constexpr int kOutBufs = MAPL_OUT_BUFS;      // [128 x 64] staging boxes: kOutBu
 constexpr int kBoxesPerHalf = kOutBufs / 2;
 constexpr int kPipeThreads = 320;            // warp 0 TMA, warp 1 MMA, warps 2-9 epilogue
 
+// Position in a ring of `size` stages, advanced without divisions: the TMA producer and MMA issuer loops run on ONE
+// thread each, every instruction waits for the one before it (no other warp hides the latency), and an integer
+// division by a run-time ring size is ~30 dependent instructions -- measured, the loops ran at ~600 cycles per
+// iteration with `it % stages` / `it / stages`, against ~50 for the barrier + TMA instructions themselves.
+struct RingPos {
+  int st; uint32_t ph;       // stage, phase parity of the stage's current use (0 for the first pass)
+  __device__ __forceinline__ RingPos() : st(0), ph(0) {}
+  __device__ __forceinline__ void advance(int n, int size) {
+    st += n;
+    while (st >= size) { st -= size; ph ^= 1u; }
+  }
+  __device__ __forceinline__ void next(int size) {
+    if (++st == size) { st = 0; ph ^= 1u; }
+  }
+};
+
 struct ChunkPipe {
   uint8_t* sA;        // resident A operand (nkb tiles)
   uint8_t* sB;        // ring (b_stages half tiles)
