@@ -58,7 +58,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   const int kc = p.r + p.ra, nkb1 = p.d / 64;
   // region R: phase 1 ring  |aliased with|  phase 2 gz operand + W ring
   const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes;
-  const size_t ring2 = (size_t)(p.r / 64) * kTileBytes + (size_t)p.b_stages * kHalfTileBytes;
+  const size_t ring2 = (size_t)(p.r / 64) * kTileBytes + (size_t)p.b_stages * kTileBytes;
   const size_t regionR = ring1 > ring2 ? ring1 : ring2;
   ChunkPipe c;
   c.nkb = p.r / 64; c.nchunks = p.d / kChunkN; c.b_stages = p.b_stages;
@@ -100,9 +100,10 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   if (warp == 0) {
     if (elect_one()) {
       const uint32_t bytes = (uint32_t)(p.tile_m * 128 + kc * 64);   // per CTA: g tile + half of the [U^T;B] rows
-      for (int kb = 0; kb < nkb1; ++kb) {
-        const int s = kb % p.stages1;
-        mbar_wait(&s1_empty[s], ((kb / p.stages1) & 1) ^ 1);
+      RingPos rp;                                    // no divisions in this one-thread loop (tc_tile_ops.cuh)
+      for (int kb = 0; kb < nkb1; ++kb, rp.next(p.stages1)) {
+        const int s = rp.st;
+        mbar_wait(&s1_empty[s], rp.ph ^ 1u);
         if (c.rank == 0) mbar_arrive_expect_tx(&s1_full[s], 2 * bytes);
         uint8_t* a = smem + (size_t)s * p.stage1_bytes;
         tma_load_2d_pair(a, &tmG, &s1_full[s], kb * 64, (int)m0, kEvictLast);   // g is read again by k_tc_bwd_du
@@ -118,11 +119,13 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
     if (c.rank == 0 && elect_one()) {
       const uint32_t idesc_u = make_idesc_bf16(256, (uint32_t)p.r, false, false);
       const uint32_t idesc_b = make_idesc_bf16(256, (uint32_t)(p.ra ? p.ra : 64), false, false);
-      for (int kb = 0; kb < nkb1; ++kb) {
-        const int s = kb % p.stages1;
-        mbar_wait(&s1_full[s], (kb / p.stages1) & 1);
+      const uint32_t smem0 = smem_u32(smem);
+      RingPos rp;
+      for (int kb = 0; kb < nkb1; ++kb, rp.next(p.stages1)) {
+        const int s = rp.st;
+        mbar_wait(&s1_full[s], rp.ph);
         tc_fence_after_sync();
-        const uint32_t a = smem_u32(smem + (size_t)s * p.stage1_bytes);
+        const uint32_t a = smem0 + (uint32_t)s * (uint32_t)p.stage1_bytes;
         const uint32_t bu = a + kTileBytes, bb = bu + p.r * 64;
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
@@ -391,9 +394,11 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   if (n_items > 0) {
     if (warp == 0) {
       if (elect_one()) {
-        for (int it = 0; it < n_items; ++it) {
-          const int s = it % p.stages, tb = tb0 + it / p.n_src, src = it % p.n_src;
-          mbar_wait(&empty[s], ((it / p.stages) & 1) ^ 1);
+        RingPos rp;
+        int tb = tb0, src = 0;
+        for (int it = 0; it < n_items; ++it, rp.next(p.stages)) {
+          const int s = rp.st;
+          mbar_wait(&empty[s], rp.ph ^ 1u);
           uint8_t* a = smem + (size_t)s * p.item_bytes;
           const CUtensorMap* ma = src ? &tmH : &tmG;
           const CUtensorMap* mb = src ? &tmGz : &tmZ;
@@ -409,18 +414,21 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
             tma_load_2d(a + kBox, ma, &full[s], dt * 128 + 64, tb * 64, kEvictFirst);
             for (int j = 0; j < nb_boxes; ++j) tma_load_2d(a + 2 * kBox + j * kBox, mb, &full[s], j * 64, tb * 64, kEvictLast);
           }
+          if (++src == p.n_src) { src = 0; ++tb; }
         }
       }
     } else if (warp == 1) {
       if (rank == 0 && elect_one()) {
         const uint32_t idesc = make_idesc_bf16(kPair ? 256 : 128, (uint32_t)p.r, true, true);
-        for (int it = 0; it < n_items; ++it) {
-          const int s = it % p.stages;
-          mbar_wait(&full[s], (it / p.stages) & 1);
+        const uint32_t smem0 = smem_u32(smem);
+        RingPos rp;
+        for (int it = 0; it < n_items; ++it, rp.next(p.stages)) {
+          const int s = rp.st;
+          mbar_wait(&full[s], rp.ph);
           if (it == 0) DU_DBG(2)
           if (it == n_items - 1) DU_DBG(3)
           tc_fence_after_sync();
-          const uint32_t a = smem_u32(smem + (size_t)s * p.item_bytes), b = a + 2 * kBox;
+          const uint32_t a = smem0 + (uint32_t)s * (uint32_t)p.item_bytes, b = a + 2 * kBox;
 #pragma unroll
           for (int k = 0; k < 4; ++k) {     // 16 tokens (= 2 swizzle atoms of 8 rows) per UMMA
             const uint64_t da = desc_mnmajor_sw128(a + k * 2048, kBox), db = desc_mnmajor_sw128(b + k * 2048, kBox);
@@ -506,11 +514,11 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     if (p.stages1 > 8) p.stages1 = 8;
     if (p.stages1 > d.d / 64) p.stages1 = d.d / 64;
     if (p.stages1 < 2) return MAPL_ERR_UNSUPPORTED;
-    p.b_stages = (int)((budget - (size_t)(d.r / 64) * kTileBytes) / kHalfTileBytes);
+    p.b_stages = (int)((budget - (size_t)(d.r / 64) * kTileBytes) / kTileBytes);
     if (p.b_stages > 16) p.b_stages = 16;
     if (p.b_stages < 2) return MAPL_ERR_UNSUPPORTED;
     const size_t ring1 = (size_t)p.stages1 * p.stage1_bytes,
-                 ring2 = (size_t)(d.r / 64) * kTileBytes + (size_t)p.b_stages * kHalfTileBytes;
+                 ring2 = (size_t)(d.r / 64) * kTileBytes + (size_t)p.b_stages * kTileBytes;
     const size_t smem = (ring1 > ring2 ? ring1 : ring2) + (size_t)kOutBufs * kTileBytes + 1024 + 1024;
     static_assert(kOutBufs == 4, "gA staging: ra / 32 pieces over four boxes");
     p.ga_tma = (ra == 64 || ra == 128) ? 1 : 0;

@@ -10,7 +10,7 @@ namespace mapl {
 
 bool tc_shape_ok(const mapl_boundary_desc& d) {
   if (d.act_dtype != MAPL_BF16) return false;
-  if (d.d % 128 != 0 || d.d < 128) return false;
+  if (d.d % 256 != 0 || d.d < 256) return false;      // the decode / dH chunk pipeline works in 256-column chunks
   if (d.r != 64 && d.r != 128 && d.r != 256) return false;
   if (d.anchor_rank != 0 && d.anchor_rank != 64 && d.anchor_rank != 128) return false;
   if (d.n_tokens < 1) return false;

@@ -2,7 +2,7 @@
 // MAPL_ERR_UNSUPPORTED when the boundary is outside its envelope (the caller then runs the fp32
 // SIMT kernels), MAPL_OK once everything is enqueued, or an error.
 //
-// Envelope: bf16 activations, d % 128 == 0, r in {64,128,256}, anchor_rank in {0,64,128};
+// Envelope: bf16 activations, d % 256 == 0, r in {64,128,256}, anchor_rank in {0,64,128};
 // RVQ on the tensor cores additionally needs K % 128 == 0.
 //
 // Parameter pack (bf16 operand copies of the fp32 masters, see mapl_pack_params in mapl.h):

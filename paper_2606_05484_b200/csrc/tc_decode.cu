@@ -39,7 +39,7 @@ k_tc_decode(const __grid_constant__ CUtensorMap tmZ, const __grid_constant__ CUt
   c.sA = smem;
   c.sOut = c.sA + (size_t)c.nkb * kTileBytes;
   c.sB = c.sOut + (size_t)kOutBufs * kTileBytes;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(c.sB + (size_t)p.b_stages * kHalfTileBytes);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(c.sB + (size_t)p.b_stages * kTileBytes);
   c.b_full = bars; c.b_empty = c.b_full + p.b_stages;
   c.acc_full = c.b_empty + p.b_stages; c.acc_empty = c.acc_full + kAccStages;
   uint64_t* a_full = c.acc_empty + kAccStages;         // leader's: A operands of both CTAs are in place
@@ -138,10 +138,10 @@ int tc_decode(const mapl_boundary_desc& d, const void* Z, const int32_t* codes, 
   p.tile_m = tc_tile_m(d.n_tokens);
   p.z_from_tma = codes ? 0 : 1;
   const size_t fixed = (size_t)(nkb + kOutBufs) * kTileBytes + 1024 + 512;
-  p.b_stages = (int)((227 * 1024 - fixed) / kHalfTileBytes);
+  p.b_stages = (int)((227 * 1024 - fixed) / kTileBytes);
   if (p.b_stages > 16) p.b_stages = 16;
   if (p.b_stages < 2) return MAPL_ERR_UNSUPPORTED;
-  const size_t smem = fixed + (size_t)p.b_stages * kHalfTileBytes;
+  const size_t smem = fixed + (size_t)p.b_stages * kTileBytes;
   CUtensorMap tmZ, tmW, tmO;
   // Z: [N, r]; when zhat comes from codes the map is unused but must be valid: point it at the pack
   const void* zbase = codes ? (const void*)pk.Wd : Z;

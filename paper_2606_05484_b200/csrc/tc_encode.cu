@@ -65,32 +65,37 @@ k_tc_encode(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUt
 
   if (warp == 0) {
     if (elect_one()) {
+      const uint32_t tx = 2u * (uint32_t)(tile_m * 128 + b_tile);
+      const int wrow = (int)rank * (r / 2);
+      RingPos rp;                                    // no divisions in this one-thread loop (tc_tile_ops.cuh)
       for (int kb = 0; kb < nkb; ++kb) {
-        const int s = kb % stages;
-        mbar_wait(&empty[s], ((kb / stages) & 1) ^ 1);
-        if (rank == 0) mbar_arrive_expect_tx(&full[s], 2u * (uint32_t)(tile_m * 128 + b_tile));
-        uint8_t* a = smem + (size_t)s * stage_bytes;
-        tma_load_2d_pair(a, &tmH, &full[s], kb * BK, (int)m0, kEvictFirst);
-        tma_load_2d_pair(a + kATile, &tmW, &full[s], kb * BK, (int)rank * (r / 2), kEvictLast);
+        mbar_wait(&empty[rp.st], rp.ph ^ 1u);
+        if (rank == 0) mbar_arrive_expect_tx(&full[rp.st], tx);
+        uint8_t* a = smem + (size_t)rp.st * stage_bytes;
+        tma_load_2d_pair(a, &tmH, &full[rp.st], kb * BK, (int)m0, kEvictFirst);
+        tma_load_2d_pair(a + kATile, &tmW, &full[rp.st], kb * BK, wrow, kEvictLast);
+        rp.next(stages);
       }
     }
   } else if (warp == 1) {
     if (rank == 0 && elect_one()) {
       const uint32_t idesc = make_idesc_bf16(2 * BM, (uint32_t)r, false, false);
+      const uint32_t smem0 = smem_u32(smem);
+      RingPos rp;
       for (int kb = 0; kb < nkb; ++kb) {
-        const int s = kb % stages;
-        mbar_wait(&full[s], (kb / stages) & 1);
+        mbar_wait(&full[rp.st], rp.ph);
 #ifdef MAPL_DBG
         if (kb == 0) DBGT(2)
         if (kb == nkb - 1) DBGT(3)
 #endif
         tc_fence_after_sync();
-        const uint32_t a = smem_u32(smem + (size_t)s * stage_bytes);
+        const uint32_t a = smem0 + (uint32_t)rp.st * (uint32_t)stage_bytes;
         const uint32_t b = a + kATile;
 #pragma unroll
         for (int k = 0; k < BK / 16; ++k)
           umma_bf16_pair(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc, (kb | k) != 0);
-        umma_commit_pair(&empty[s]);
+        umma_commit_pair(&empty[rp.st]);
+        rp.next(stages);
       }
       umma_commit_pair(accum_full);
     }

@@ -23,14 +23,14 @@
 namespace mapl {
 namespace tc {
 
-constexpr int kChunkN = 128;                 // d-chunk width == UMMA N
+constexpr int kChunkN = 256;                 // d-chunk width == UMMA N
 constexpr int kTileBytes = 128 * 64 * 2;     // one [128 x 64] bf16 tile
 constexpr int kHalfTileBytes = 64 * 64 * 2;  // the half of a W tile one CTA of the pair holds
-constexpr int kAccStages = 4;
+constexpr int kAccStages = 2;
 #ifndef MAPL_OUT_BUFS
 #define MAPL_OUT_BUFS 4
 #endif
-constexpr int kOutBufs = MAPL_OUT_BUFS;      // [128 x 64] staging boxes: kOutBufs / 2 per column half of a chunk, used in turn
+constexpr int kOutBufs = MAPL_OUT_BUFS;      // [128 x 64] staging boxes: kOutBufs / 2 per column half (128 columns) of a chunk
 constexpr int kBoxesPerHalf = kOutBufs / 2;
 constexpr int kPipeThreads = 320;            // warp 0 TMA, warp 1 MMA, warps 2-9 epilogue
 
@@ -60,15 +60,15 @@ struct ChunkPipe {
   uint32_t tmem_base, rank;
 };
 
-// producer: one thread in each CTA; tmW box = [64 rows x 64 cols]
+// producer: one thread in each CTA; tmW box = [128 rows x 64 cols]
 __device__ __forceinline__ void chunk_produce(const ChunkPipe& c, const CUtensorMap* tmW) {
-  int it = 0;
+  RingPos rp;
   for (int j = 0; j < c.nchunks; ++j)
-    for (int kb = 0; kb < c.nkb; ++kb, ++it) {
-      const int s = it % c.b_stages;
-      mbar_wait(&c.b_empty[s], ((it / c.b_stages) & 1) ^ 1);
-      if (c.rank == 0) mbar_arrive_expect_tx(&c.b_full[s], 2 * kHalfTileBytes);
-      tma_load_2d_pair(c.sB + (size_t)s * kHalfTileBytes, tmW, &c.b_full[s], kb * 64, j * kChunkN + (int)c.rank * 64, kEvictLast);
+    for (int kb = 0; kb < c.nkb; ++kb) {
+      mbar_wait(&c.b_empty[rp.st], rp.ph ^ 1u);
+      if (c.rank == 0) mbar_arrive_expect_tx(&c.b_full[rp.st], 2 * kTileBytes);
+      tma_load_2d_pair(c.sB + (size_t)rp.st * kTileBytes, tmW, &c.b_full[rp.st], kb * 64, j * kChunkN + (int)c.rank * (kChunkN / 2), kEvictLast);
+      rp.next(c.b_stages);
     }
 }
 
@@ -76,22 +76,23 @@ __device__ __forceinline__ void chunk_produce(const ChunkPipe& c, const CUtensor
 // the async proxy
 __device__ __forceinline__ void chunk_mma(const ChunkPipe& c) {
   const uint32_t idesc = make_idesc_bf16(256, kChunkN, false, false);
-  int it = 0;
+  const uint32_t sA0 = smem_u32(c.sA), sB0 = smem_u32(c.sB);
+  RingPos rp;
   for (int j = 0; j < c.nchunks; ++j) {
     const int as = j % kAccStages;
     mbar_wait_cluster(&c.acc_empty[as], ((j / kAccStages) & 1) ^ 1);
     if (j < 16) DBGT(8 + j)
     tc_fence_after_sync();
     const uint32_t tmem_d = c.tmem_base + as * kChunkN;
-    for (int kb = 0; kb < c.nkb; ++kb, ++it) {
-      const int s = it % c.b_stages;
-      mbar_wait(&c.b_full[s], (it / c.b_stages) & 1);
+    for (int kb = 0; kb < c.nkb; ++kb) {
+      mbar_wait(&c.b_full[rp.st], rp.ph);
       tc_fence_after_sync();
-      const uint32_t a = smem_u32(c.sA + (size_t)kb * kTileBytes), b = smem_u32(c.sB + (size_t)s * kHalfTileBytes);
+      const uint32_t a = sA0 + (uint32_t)kb * kTileBytes, b = sB0 + (uint32_t)rp.st * kTileBytes;
 #pragma unroll
       for (int k = 0; k < 4; ++k)
         umma_bf16_pair(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc, (kb | k) != 0);
-      umma_commit_pair(&c.b_empty[s]);
+      umma_commit_pair(&c.b_empty[rp.st]);
+      rp.next(c.b_stages);
     }
     umma_commit_pair(&c.acc_full[as]);
     if (j < 16) DBGT(24 + j)
@@ -99,45 +100,51 @@ __device__ __forceinline__ void chunk_mma(const ChunkPipe& c) {
 }
 
 // epilogue: the 8 warps with threadIdx.x in [64,320) of each CTA.  Warp w reads TMEM lane quarter
-// q = w & 3 (row = token row in the tile) and column half h = (w - 2) / 4 of the chunk, i.e. exactly one
-// [128 x 64] staging box; the two halves run independently (named barriers 1 and 2, 128 threads
-// each; threads 64 and 192 issue the TMA stores of their box).
+// q = w & 3 (row = token row in the tile) and column half h = (w - 2) / 4 of the chunk (128 columns), in two
+// rounds of 64 columns = one [128 x 64] staging box each; the two halves run independently (named barriers 1
+// and 2, 128 threads each; threads 64 and 192 issue the TMA stores of their boxes).
 __device__ __forceinline__ void chunk_epilogue(const ChunkPipe& c, const CUtensorMap* tmO, int m0) {
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32, q = warp & 3, h = (warp - 2) >> 2, row = q * 32 + lane;
   const bool issuer = threadIdx.x == 64 + h * 128;
   for (int j = 0; j < c.nchunks; ++j) {
-    uint8_t* box = c.sOut + (size_t)(h * kBoxesPerHalf + j % kBoxesPerHalf) * kTileBytes;
     const int as = j % kAccStages;
     mbar_wait(&c.acc_full[as], (j / kAccStages) & 1);
     if (threadIdx.x == 64 && j < 16) DBGT(40 + j)
     tc_fence_after_sync();
-    uint32_t v[2][32];
-    const uint32_t taddr = c.tmem_base + ((uint32_t)(q * 32) << 16) + as * kChunkN + h * 64;
-    tmem_ld32(taddr, v[0]);
-    tmem_ld32(taddr + 32, v[1]);
-    tmem_ld_wait();
-    tc_fence_before_sync();
-    __syncwarp();
-    if (lane == 0) mbar_arrive_leader(&c.acc_empty[as]);     // the TMEM stage may be overwritten
-    // the store that last used this box (chunk j - kBoxesPerHalf; in the first round whatever the caller staged
-    // there) must have read it before it is rewritten
-    if (issuer) { if (j < kBoxesPerHalf) tma_store_wait_read<0>(); else tma_store_wait_read<kBoxesPerHalf - 1>(); }
-    if (h == 0) asm volatile("bar.sync 1, 128;" ::: "memory"); else asm volatile("bar.sync 2, 128;" ::: "memory");
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const uint32_t* w = &v[i / 4][8 * (i % 4)];
-      uint4 o;
-      o.x = pack_bf16x2(__uint_as_float(w[0]), __uint_as_float(w[1]));
-      o.y = pack_bf16x2(__uint_as_float(w[2]), __uint_as_float(w[3]));
-      o.z = pack_bf16x2(__uint_as_float(w[4]), __uint_as_float(w[5]));
-      o.w = pack_bf16x2(__uint_as_float(w[6]), __uint_as_float(w[7]));
-      *reinterpret_cast<uint4*>(box + sw128_offset(row, i)) = o;
-    }
-    fence_proxy_async_smem();
-    if (h == 0) asm volatile("bar.sync 1, 128;" ::: "memory"); else asm volatile("bar.sync 2, 128;" ::: "memory");
-    if (issuer) {
-      tma_store_2d_hint(tmO, box, j * kChunkN + h * 64, m0, kEvictFirst);     // Hhat / dH: not read again by the codec
-      tma_store_commit();
+    for (int i = 0; i < kBoxesPerHalf; ++i) {
+      uint8_t* box = c.sOut + (size_t)(h * kBoxesPerHalf + i) * kTileBytes;
+      uint32_t v[2][32];
+      const uint32_t taddr = c.tmem_base + ((uint32_t)(q * 32) << 16) + as * kChunkN + h * (kChunkN / 2) + i * 64;
+      tmem_ld32(taddr, v[0]);
+      tmem_ld32(taddr + 32, v[1]);
+      tmem_ld_wait();
+      if (i == kBoxesPerHalf - 1) {          // the whole stage is in registers / staged: it may be overwritten
+        tc_fence_before_sync();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_leader(&c.acc_empty[as]);
+      }
+      // the store that last used this box (the same round of chunk j - 1; in the first chunk whatever the caller
+      // staged there) must have read it before it is rewritten: of this thread's bulk groups only the one committed
+      // after it (the other round) may still be pending
+      if (issuer) { if (j == 0) tma_store_wait_read<0>(); else tma_store_wait_read<kBoxesPerHalf - 1>(); }
+      if (h == 0) asm volatile("bar.sync 1, 128;" ::: "memory"); else asm volatile("bar.sync 2, 128;" ::: "memory");
+#pragma unroll
+      for (int t = 0; t < 8; ++t) {
+        const uint32_t* w = &v[t / 4][8 * (t % 4)];
+        uint4 o;
+        o.x = pack_bf16x2(__uint_as_float(w[0]), __uint_as_float(w[1]));
+        o.y = pack_bf16x2(__uint_as_float(w[2]), __uint_as_float(w[3]));
+        o.z = pack_bf16x2(__uint_as_float(w[4]), __uint_as_float(w[5]));
+        o.w = pack_bf16x2(__uint_as_float(w[6]), __uint_as_float(w[7]));
+        *reinterpret_cast<uint4*>(box + sw128_offset(row, t)) = o;
+      }
+      fence_proxy_async_smem();
+      if (h == 0) asm volatile("bar.sync 1, 128;" ::: "memory"); else asm volatile("bar.sync 2, 128;" ::: "memory");
+      if (issuer) {
+        tma_store_2d_hint(tmO, box, j * kChunkN + h * (kChunkN / 2) + i * 64, m0, kEvictFirst);     // Hhat / dH: not read again by the codec
+        tma_store_commit();
+      }
     }
   }
   if (issuer) tma_store_wait_all<0>();
