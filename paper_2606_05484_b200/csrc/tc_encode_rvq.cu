@@ -163,12 +163,10 @@ __device__ __forceinline__ void store_operand_piece(uint8_t* sRho, int row, int 
 }
 
 // The kParts threads of a token split the residual by 32-column pieces: part h owns the pieces pc with pc % kParts == h.
-// rho <- rho (+ second accumulator: the two halves of the projection chain) (- sub) on the own pieces; partial
-// ||rho||^2 and max|rho_j| of those pieces; with kConvert the fp16 rounding of rho * inv goes to the swizzled
-// A-operand tiles in the same pass.  Warp-convergent.
-template <bool kConvert>
-__device__ __forceinline__ void rho_update(uint32_t tmem_row, const float* __restrict__ sub, bool add_second, uint8_t* sRho,
-                                           int row, int r, int h, float inv, float* n2_out, float* amax_out) {
+// Level 0: rho <- z (+ second accumulator: the two halves of the projection chain) (- sub: the centring row) on the own
+// pieces; partial ||rho||^2 and max|rho_j| of those pieces.  Warp-convergent.
+__device__ __forceinline__ void rho_first(uint32_t tmem_row, const float* __restrict__ sub, bool add_second, int r, int h,
+                                          float* n2_out, float* amax_out) {
   float n2 = 0.f, amax = 0.f;
   for (int pc = h; pc < r / 32; pc += kParts) {
     uint32_t v[32];
@@ -200,9 +198,57 @@ __device__ __forceinline__ void rho_update(uint32_t tmem_row, const float* __res
       n2 = fmaf(x, x, n2);
       amax = fmaxf(amax, fabsf(x));
     }
-    if (kConvert) store_operand_piece(sRho, row, pc, v, inv);
   }
   if (sub != nullptr || add_second) tmem_st_wait();
+  *n2_out = n2; *amax_out = amax;
+}
+
+// Levels >= 1: rho <- rho - sub on the own pieces and, in the same pass, the fp16 rounding of rho * inv into the
+// swizzled A-operand tiles.  Two own pieces per round: the row loads of both (16 float4, L2 latency) are in flight
+// together; r / 32 / kParts is 1 (r = 64), 2 or 4.  Warp-convergent.
+__device__ __forceinline__ void rho_update(uint32_t tmem_row, const float* __restrict__ sub, uint8_t* sRho, int row, int r,
+                                           int h, float inv, float* n2_out, float* amax_out) {
+  float n2 = 0.f, amax = 0.f;
+  const int npc = r / 32 / kParts;
+#pragma unroll 1
+  for (int i0 = 0; i0 < npc; i0 += 2) {
+    const bool two = i0 + 1 < npc;
+    const int pc0 = h + i0 * kParts, pc1 = pc0 + kParts;
+    float4 c0[8], c1[8];
+    {
+      const float4* a4 = reinterpret_cast<const float4*>(sub + pc0 * 32);
+      const float4* b4 = reinterpret_cast<const float4*>(sub + (two ? pc1 : pc0) * 32);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) c0[i] = __ldg(a4 + i);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) c1[i] = __ldg(b4 + i);
+    }
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      if (u == 1 && !two) break;
+      const int pc = u ? pc1 : pc0;
+      uint32_t v[32];
+      tmem_ld32(tmem_row + pc * 32, v);
+      tmem_ld_wait();
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const float4 c = u ? c1[i] : c0[i];
+        v[4 * i + 0] = __float_as_uint(__uint_as_float(v[4 * i + 0]) - c.x);
+        v[4 * i + 1] = __float_as_uint(__uint_as_float(v[4 * i + 1]) - c.y);
+        v[4 * i + 2] = __float_as_uint(__uint_as_float(v[4 * i + 2]) - c.z);
+        v[4 * i + 3] = __float_as_uint(__uint_as_float(v[4 * i + 3]) - c.w);
+      }
+      tmem_st32(tmem_row + pc * 32, v);
+#pragma unroll
+      for (int i = 0; i < 32; ++i) {
+        const float x = __uint_as_float(v[i]);
+        n2 = fmaf(x, x, n2);
+        amax = fmaxf(amax, fabsf(x));
+      }
+      store_operand_piece(sRho, row, pc, v, inv);
+    }
+  }
+  tmem_st_wait();
   *n2_out = n2; *amax_out = amax;
 }
 
@@ -496,7 +542,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       // z - Tc[tok] (dead rows subtract row 0: any valid row keeps the warp convergent)
       const float* csub = p.Tc != nullptr ? p.Tc + (live ? (long long)__ldg(p.tok + m) * p.r : 0) : nullptr;
       float n2p, amaxp;
-      rho_update<false>(tmem_row, csub, nkb1 >= 2, s.sRho, row, p.r, h, 0.f, &n2p, &amaxp);
+      rho_first(tmem_row, csub, nkb1 >= 2, p.r, h, &n2p, &amaxp);
       xN2[mine] = n2p; xAmax[mine] = amaxp;
       epi_sync();
       n2 = 0.f; amax = 0.f;
@@ -633,7 +679,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         // maximum); the exact ||rho_new||^2 and max|rho_new| are exchanged behind the hand-off.
         inv = inv_scale_of(amax + __ldg(lv + 4));
         float n2p, amaxp;
-        rho_update<true>(tmem_row, Cl + (long long)bestk * p.r, false, s.sRho, row, p.r, h, inv, &n2p, &amaxp);
+        rho_update(tmem_row, Cl + (long long)bestk * p.r, s.sRho, row, p.r, h, inv, &n2p, &amaxp);
         xN2[mine] = n2p; xAmax[mine] = amaxp;
         write_ax(inv * __ldg(lv + 8 + 2), hard);
         if (warp == 2 && l == 1) { DBG(21) }
