@@ -34,6 +34,7 @@ struct Ws {
   size_t gA = 0;          // [N*ra] fp32
   size_t pack = 0;        // tensor-core parameter pack, used when desc.param_pack == NULL
   size_t tc = 0;          // tensor-core path scratch (bf16 zhat)
+  size_t rvq_ovf = 0;     // overflow area of the RVQ candidate lists (tensor-core encode)
   size_t total = 0;
 };
 
@@ -46,6 +47,7 @@ Ws carve(const mapl_boundary_desc& d) {
   w.gA = seg((size_t)d.n_tokens * d.anchor_rank * 4);
   w.pack = seg(tc_pack_layout(d, nullptr).bytes);
   w.tc = seg(tc_scratch_bytes(d));
+  w.rvq_ovf = seg(tc_rvq_overflow_bytes(d));
   w.total = off + 256;
   return w;
 }
@@ -133,7 +135,7 @@ static int encode_impl(const mapl_boundary_desc* desc, const void* H, const floa
   if (tc_shape_ok(d) && (L == 0 || tc_rvq_ok(d))) {
     TcPack pk;
     MAPL_RETURN_IF(resolve_pack(d, U, nullptr, codebooks, ws, w, st, &pk));
-    int s = tc_encode(d, H, codebooks, pk, Zq_out, codes_out, st, tok, Tc);
+    int s = tc_encode(d, H, codebooks, pk, Zq_out, codes_out, st, tok, Tc, ws + w.rvq_ovf);
     if (s != MAPL_ERR_UNSUPPORTED) return s;
   }
 

@@ -48,6 +48,13 @@ size_t tc_scratch_bytes(const mapl_boundary_desc& d) {
   return d.rvq_levels > 0 ? align_up((size_t)d.n_tokens * d.r * 2, 256) : 0;
 }
 
+size_t tc_rvq_overflow_bytes(const mapl_boundary_desc& d) {
+  if (!tc_rvq_ok(d)) return 0;
+  const long long tm = tc_tile_m(d.n_tokens);
+  const long long tiles = ((d.n_tokens + tm - 1) / tm + 1) & ~1ll;
+  return (size_t)tiles * 256 * kRvqOverflowEntries * kRvqOverflowBytes;
+}
+
 int tc_tile_m(long long N) {
   const long long per_wave = 148ll * 128;
   const long long waves = (N + per_wave - 1) / per_wave;

@@ -45,12 +45,20 @@ int tc_pack_build(const mapl_boundary_desc& d, const float* U, const float* B, c
 // scratch of the tc path besides the pack: bf16 zhat [N,r] (RVQ codes -> dU operand)
 size_t tc_scratch_bytes(const mapl_boundary_desc& d);
 
+// global overflow area of the RVQ candidate lists (tc_encode_rvq.cu): kRvqOverflowEntries entries of kRvqOverflowBytes
+// per scan thread (256 per CTA); entries are touched only by the rare token whose list in shared memory is full
+constexpr int kRvqOverflowEntries = 8;
+constexpr int kRvqOverflowBytes = 80;      // m, group id, 2 pad words, 16 raw scores
+size_t tc_rvq_overflow_bytes(const mapl_boundary_desc& d);
+
 // tokens per CTA (<= 128, multiple of 8) such that the grid covers the 148 SMs in whole, even waves
 int tc_tile_m(long long N);
 
 // tok / Tc (both or neither): sender-side centring z -= Tc[tok], Tc [V,r] fp32 (mapl_center_table)
+// ovf_ws: tc_rvq_overflow_bytes(d) bytes of scratch (RVQ only; nullptr: lists limited to shared memory)
 int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
-              int32_t* codes_out, cudaStream_t st, const int32_t* tok = nullptr, const float* Tc = nullptr);
+              int32_t* codes_out, cudaStream_t st, const int32_t* tok = nullptr, const float* Tc = nullptr,
+              void* ovf_ws = nullptr);
 
 int tc_decode(const mapl_boundary_desc& d, const void* Z, const int32_t* codes, const float* codebooks,
               const int32_t* tok, const float* A, const TcPack& pk, void* Hhat_out, cudaStream_t st);

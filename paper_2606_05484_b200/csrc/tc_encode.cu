@@ -163,12 +163,12 @@ MAPL_DBG_READER(mapl_debug_read_encode)
 namespace mapl {
 
 int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
-                  int32_t* codes_out, cudaStream_t st, const int32_t* tok, const float* Tc);   // tc_encode_rvq.cu
+                  int32_t* codes_out, cudaStream_t st, const int32_t* tok, const float* Tc, void* ovf_ws);   // tc_encode_rvq.cu
 
 int tc_encode(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
-              int32_t* codes_out, cudaStream_t st, const int32_t* tok, const float* Tc) {
+              int32_t* codes_out, cudaStream_t st, const int32_t* tok, const float* Tc, void* ovf_ws) {
   if (!tc_shape_ok(d)) return MAPL_ERR_UNSUPPORTED;
-  if (d.rvq_levels != 0) return tc_encode_rvq(d, H, codebooks, pk, Zq_out, codes_out, st, tok, Tc);
+  if (d.rvq_levels != 0) return tc_encode_rvq(d, H, codebooks, pk, Zq_out, codes_out, st, tok, Tc, ovf_ws);
   const int tile_m = tc_tile_m(d.n_tokens);
   CUtensorMap tmH, tmW;
   if (!make_tmap_bf16_2d(&tmH, H, (uint64_t)d.n_tokens, (uint64_t)d.d, (uint64_t)d.d, BK, (uint32_t)tile_m)) return MAPL_ERR_CUDA;

@@ -60,6 +60,7 @@ struct RvqParams {
   long long N;
   int d, r, L, K, tile_m;
   int stages1, stage1_bytes, ring_tiles, nsplit, kne, p1, p2;
+  uint8_t* ovf; int kovf;   // global overflow entries per scan thread (tc_codec.cuh); kovf == 0: none
 };
 
 // smem carve-up (after 1024-byte alignment):
@@ -290,35 +291,65 @@ __device__ __forceinline__ void sts_v4(uint32_t a, uint32_t x, uint32_t y, uint3
   asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
 
-// per-thread candidate list (shared memory): entry e of thread t has its maximum at eM[e * kEpi + t], its group id
-// (codeword index / 16) at eId[...], its 16 raw scores as four 16-byte units at stash[((e * 4 + i) * kEpi + t) * 16]
-// (consecutive lanes -> consecutive 16-byte units: conflict-free).
+// per-thread candidate list.  Entries [0, kne) live in shared memory: entry e of thread t has its maximum at
+// eM[e * kEpi + t], its group id (codeword index / 16) at eId[...], its 16 raw scores as four 16-byte units at
+// stash[((e * 4 + i) * kEpi + t) * 16] (consecutive lanes -> consecutive 16-byte units: conflict-free).  Entries
+// [kne, kne + kovf) live in the thread's slice of a global overflow area (80 bytes each: m, id, pad, pad, 16 scores),
+// written only by the rare token with more than kne groups within its margin (measured at config 3: at most 7
+// candidates per token, i.e. a handful of tokens per launch -- which cost 4 ms each when the list simply overflowed
+// into the exhaustive pass).
 struct CandList {
   uint32_t eM, eId, stash;   // shared-space byte addresses, already offset by the thread index
-  int cnt;             // entries in use (high-water mark)
-  float dropped;       // highest maximum that found no room (-FLT_MAX: none)
+  uint8_t* ovf;              // this thread's global overflow entries (nullptr: none)
+  int kne, kovf;
+  int cnt;             // shared-memory entries in use (high-water mark)
+  int novf;            // overflow entries in use
+  float dropped;       // highest maximum that found no room anywhere (-FLT_MAX: none)
 };
+
+__device__ __forceinline__ void ovf_put(CandList& cl, float m, int gid, const uint4 (&q)[4]) {
+  if (cl.novf < cl.kovf) {
+    uint4* e = reinterpret_cast<uint4*>(cl.ovf + (size_t)cl.novf * kRvqOverflowBytes);
+    e[0] = make_uint4(__float_as_uint(m), (uint32_t)gid, 0u, 0u);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) e[1 + i] = q[i];
+    ++cl.novf;
+  } else {
+    cl.dropped = fmaxf(cl.dropped, m);
+  }
+}
 
 // record the group `gid` (maximum m, scores v[0..16)); thr = current threshold.  Lane-divergent.  While the list has
 // room the group is appended; when it is full, a stale entry (below the current threshold, which only rises during a
-// scan) is reused, else the list keeps the kne highest maxima and remembers the highest maximum it let go: only if
-// that value is within the FINAL threshold does the thread need the exhaustive pass.  (A plain FIFO is cheaper but
-// overflows at r = 256, where many group maxima lie within the margin of each other: measured 3.2 ms instead of
-// 0.2 ms per config-3 encode.  The scan is bound by the TMEM read-out, not by these instructions.)
-__device__ __forceinline__ void stash_group(CandList& cl, int kne, float m, int gid, const uint32_t* v, float thr) {
+// scan) is reused, else the shared-memory list keeps the kne highest maxima and the lowest one moves to the global
+// overflow entries; only what finds no room there either is remembered in `dropped`, and only if that value is within
+// the FINAL threshold does the thread need the exhaustive pass.  (A plain FIFO is cheaper but overflows at r = 256,
+// where many group maxima lie within the margin of each other.  The scan is bound by the TMEM read-out, not by these
+// instructions.)
+__device__ __forceinline__ void stash_group(CandList& cl, float m, int gid, const uint32_t* v, float thr) {
   int slot = -1;
-  if (cl.cnt < kne) {
+  if (cl.cnt < cl.kne) {
     slot = cl.cnt++;
   } else {
     int w = 0;
     float wm = lds_f32(cl.eM);
-    for (int e = 1; e < kne; ++e) {
+    for (int e = 1; e < cl.kne; ++e) {
       const float em = lds_f32(cl.eM + e * kEpi * 4);
       if (em < wm) { wm = em; w = e; }
     }
-    if (wm < thr) slot = w;                                           // stale entry: the threshold has passed it
-    else if (m > wm) { cl.dropped = fmaxf(cl.dropped, wm); slot = w; }   // keep the kne highest maxima
-    else cl.dropped = fmaxf(cl.dropped, m);
+    if (wm < thr) {
+      slot = w;                                           // stale entry: the threshold has passed it
+    } else if (m > wm) {                                  // the lowest entry makes room
+      uint4 q[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) q[i] = lds_v4(cl.stash + (uint32_t)(w * 4 + i) * kEpi * 16);
+      ovf_put(cl, wm, lds_s32(cl.eId + w * kEpi * 4), q);
+      slot = w;
+    } else {
+      const uint4 q[4] = {make_uint4(v[0], v[1], v[2], v[3]), make_uint4(v[4], v[5], v[6], v[7]),
+                          make_uint4(v[8], v[9], v[10], v[11]), make_uint4(v[12], v[13], v[14], v[15])};
+      ovf_put(cl, m, gid, q);
+    }
   }
   if (slot >= 0) {
     sts_f32(cl.eM + slot * kEpi * 4, m);
@@ -329,12 +360,22 @@ __device__ __forceinline__ void stash_group(CandList& cl, int kne, float m, int 
   }
 }
 
-// 16-bit mask of the scores >= thr in entry e
+// entry e of the whole list (shared memory first, then the overflow entries): its maximum, group id, and the 16-bit
+// mask of its scores >= thr
+__device__ __forceinline__ float entry_max(const CandList& cl, int e) {
+  if (e < cl.kne) return lds_f32(cl.eM + e * kEpi * 4);
+  return __uint_as_float(reinterpret_cast<const uint4*>(cl.ovf + (size_t)(e - cl.kne) * kRvqOverflowBytes)[0].x);
+}
+__device__ __forceinline__ int entry_gid(const CandList& cl, int e) {
+  if (e < cl.kne) return lds_s32(cl.eId + e * kEpi * 4);
+  return (int)reinterpret_cast<const uint4*>(cl.ovf + (size_t)(e - cl.kne) * kRvqOverflowBytes)[0].y;
+}
 __device__ __forceinline__ uint32_t entry_mask(const CandList& cl, int e, float thr) {
   uint32_t mk = 0;
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
-    const uint4 q = lds_v4(cl.stash + (uint32_t)(e * 4 + i) * kEpi * 16);
+    const uint4 q = e < cl.kne ? lds_v4(cl.stash + (uint32_t)(e * 4 + i) * kEpi * 16)
+                               : reinterpret_cast<const uint4*>(cl.ovf + (size_t)(e - cl.kne) * kRvqOverflowBytes)[1 + i];
     mk |= (__uint_as_float(q.x) >= thr ? 1u : 0u) << (4 * i);
     mk |= (__uint_as_float(q.y) >= thr ? 1u : 0u) << (4 * i + 1);
     mk |= (__uint_as_float(q.z) >= thr ? 1u : 0u) << (4 * i + 2);
@@ -342,6 +383,8 @@ __device__ __forceinline__ uint32_t entry_mask(const CandList& cl, int e, float 
   }
   return mk;
 }
+// number of list positions to visit: all kne shared-memory positions once the overflow entries are in use
+__device__ __forceinline__ int entry_count(const CandList& cl) { return cl.novf > 0 ? cl.kne + cl.novf : cl.cnt; }
 
 __global__ void __launch_bounds__(kThreads, 1)
 k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmWhi,
@@ -510,6 +553,8 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
     const int mine = h * 128 + row;
     CandList cl;
     cl.eM = smem_u32(s.eM + mine); cl.eId = smem_u32(s.eId + mine); cl.stash = smem_u32(s.stash) + (uint32_t)mine * 16;
+    cl.kne = p.kne; cl.kovf = p.ovf != nullptr ? p.kovf : 0;
+    cl.ovf = p.ovf != nullptr ? p.ovf + ((size_t)blockIdx.x * kEpi + mine) * (size_t)p.kovf * kRvqOverflowBytes : nullptr;
     int code_l[8];
 #pragma unroll
     for (int l = 0; l < 8; ++l) code_l[l] = 0;
@@ -573,7 +618,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       }
 
       float best = -FLT_MAX;
-      cl.cnt = 0; cl.dropped = -FLT_MAX;
+      cl.cnt = 0; cl.novf = 0; cl.dropped = -FLT_MAX;
       int cr = rot_c;
       for (int c = 0; c < nchunks; ++c, ++cg) {
         const int as = cg & 1;
@@ -596,10 +641,10 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         // chunk -- a token's running maximum is beaten ~ln(groups) times per level -- so there is no warp vote.)
         if (live && m64 >= thr) {
           const int gid = (cr * 4 + h) * 2;                // 16-codeword group of v[0][0]; v[1] is kParts pieces further
-          if (g0 >= thr) stash_group(cl, p.kne, g0, gid, &v[0][0], thr);
-          if (g1 >= thr) stash_group(cl, p.kne, g1, gid + 1, &v[0][16], thr);
-          if (g2 >= thr) stash_group(cl, p.kne, g2, gid + 2 * kParts, &v[1][0], thr);
-          if (g3 >= thr) stash_group(cl, p.kne, g3, gid + 2 * kParts + 1, &v[1][16], thr);
+          if (g0 >= thr) stash_group(cl, g0, gid, &v[0][0], thr);
+          if (g1 >= thr) stash_group(cl, g1, gid + 1, &v[0][16], thr);
+          if (g2 >= thr) stash_group(cl, g2, gid + 2 * kParts, &v[1][0], thr);
+          if (g3 >= thr) stash_group(cl, g3, gid + 2 * kParts + 1, &v[1][16], thr);
         }
         if (++cr == nchunks) cr = 0;
         if (threadIdx.x == 64 && cg < 8) DBGT(56 + cg)
@@ -614,11 +659,11 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       const float thr = best - margin;
       const bool overflow = live && (hard || cl.dropped >= thr);     // pathological (e.g. many duplicate codewords)
       int ncand = 0, firstk = 0;
-      const int n_ent = cl.cnt;
+      const int n_ent = entry_count(cl);
       for (int e = 0; e < n_ent; ++e) {
-        if (lds_f32(cl.eM + e * kEpi * 4) >= thr) {
+        if (entry_max(cl, e) >= thr) {
           const uint32_t mk = entry_mask(cl, e, thr);
-          if (mk != 0 && ncand == 0) firstk = lds_s32(cl.eId + e * kEpi * 4) * 16 + __ffs(mk) - 1;
+          if (mk != 0 && ncand == 0) firstk = entry_gid(cl, e) * 16 + __ffs(mk) - 1;
           ncand += __popc(mk);
         }
       }
@@ -640,7 +685,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         uint32_t mrem = 0;
         while (true) {
           while (mrem == 0 && e < n_ent) {
-            if (lds_f32(cl.eM + e * kEpi * 4) >= thr) { mrem = entry_mask(cl, e, thr); gid = lds_s32(cl.eId + e * kEpi * 4); }
+            if (entry_max(cl, e) >= thr) { mrem = entry_mask(cl, e, thr); gid = entry_gid(cl, e); }
             ++e;
           }
           const bool have = rescore && !overflow && live && mrem != 0;
@@ -722,13 +767,14 @@ MAPL_DBG_READER(mapl_debug_read_rvq)
 namespace mapl {
 
 int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codebooks, const TcPack& pk, void* Zq_out,
-                  int32_t* codes_out, cudaStream_t st, const int32_t* tok, const float* Tc) {
+                  int32_t* codes_out, cudaStream_t st, const int32_t* tok, const float* Tc, void* ovf_ws) {
   if (!tc_rvq_ok(d) || !pk.WBlo || !pk.Cb || !pk.hnb) return MAPL_ERR_UNSUPPORTED;
   RvqParams p;
   p.C = codebooks; p.lvl = pk.lvl; p.tok = tok; p.Tc = Tc;
   p.Zq = reinterpret_cast<__nv_bfloat16*>(Zq_out); p.codes = codes_out;
   p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.L = d.rvq_levels; p.K = d.rvq_k;
   p.tile_m = tc_tile_m(d.n_tokens);
+  p.ovf = reinterpret_cast<uint8_t*>(ovf_ws); p.kovf = kRvqOverflowEntries;
   p.nsplit = pk.WBlo2 ? 3 : 2;
   p.stage1_bytes = kTileBytes + p.nsplit * d.r * 64;
   // shared memory: the candidate lists take what the codebook ring can spare -- at least two chunks of codebook tiles
