@@ -44,7 +44,7 @@ struct BwdGzParams {
   float* z2; long long n2;
   long long N;
   int d, r, ra, tile_m;
-  int stages1, stage1_bytes, b_stages, do_dh, ga_tma;
+  int stages1, stage1_bytes, b_stages, do_dh, ga_tma, nq;
   const int32_t* codes; const float* codebooks; __nv_bfloat16* zhat_out; int L, K;   // RVQ: zhat for k_tc_bwd_du
 };
 
@@ -62,7 +62,8 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   const size_t regionR = ring1 > ring2 ? ring1 : ring2;
   ChunkPipe c;
   c.nkb = p.r / 64; c.nchunks = p.d / kChunkN; c.b_stages = p.b_stages;
-  c.rank = cluster_ctarank();
+  c.pp = pair_pos((uint32_t)p.nq);
+  c.rank = c.pp.pr;
   c.sA = smem;
   c.sB = smem + (size_t)(p.r / 64) * kTileBytes;
   c.sOut = smem + regionR;
@@ -83,7 +84,7 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
     tma_prefetch_desc(&tmG); tma_prefetch_desc(&tmWu); tma_prefetch_desc(&tmWb);
     tma_prefetch_desc(&tmWd); tma_prefetch_desc(&tmO); tma_prefetch_desc(&tmGz); tma_prefetch_desc(&tmGA);
     chunk_init_barriers(c);
-    for (int s = 0; s < p.stages1; ++s) { mbar_init(&s1_full[s], 1); mbar_init(&s1_empty[s], 1); }
+    for (int s = 0; s < p.stages1; ++s) { mbar_init(&s1_full[s], 1); mbar_init(&s1_empty[s], p.nq); }
     mbar_init(acc1_full, 1);
     mbar_init(gz_full, 16);                   // leader's: the epilogue warps of both CTAs
     fence_barrier_init();
@@ -107,8 +108,17 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
         if (c.rank == 0) mbar_arrive_expect_tx(&s1_full[s], 2 * bytes);
         uint8_t* a = smem + (size_t)s * p.stage1_bytes;
         tma_load_2d_pair(a, &tmG, &s1_full[s], kb * 64, (int)m0, kEvictLast);   // g is read again by k_tc_bwd_du
-        tma_load_2d_pair(a + kTileBytes, &tmWu, &s1_full[s], kb * 64, (int)c.rank * (p.r / 2), kEvictLast);
-        if (p.ra) tma_load_2d_pair(a + kTileBytes + p.r * 64, &tmWb, &s1_full[s], kb * 64, p.r + (int)c.rank * (p.ra / 2), kEvictLast);
+        if (p.nq == 1) {
+          tma_load_2d_pair(a + kTileBytes, &tmWu, &s1_full[s], kb * 64, (int)c.rank * (p.r / 2), kEvictLast);
+          if (p.ra) tma_load_2d_pair(a + kTileBytes + p.r * 64, &tmWb, &s1_full[s], kb * 64, p.r + (int)c.rank * (p.ra / 2), kEvictLast);
+        } else {   // the parameter rows this CTA holds: half loaded here, half by the twin CTA of the other pair (multicast)
+          const int q = (int)c.pp.q;
+          tma_load_2d_pair_mc(a + kTileBytes + q * (p.r * 32), &tmWu, &s1_full[s], kb * 64, (int)c.rank * (p.r / 2) + q * (p.r / 4),
+                              c.pp.twin_mask, kEvictLast);
+          if (p.ra)
+            tma_load_2d_pair_mc(a + kTileBytes + p.r * 64 + q * (p.ra * 32), &tmWb, &s1_full[s], kb * 64,
+                                p.r + (int)c.rank * (p.ra / 2) + q * (p.ra / 4), c.pp.twin_mask, kEvictLast);
+        }
       }
       if (p.do_dh) {
         mbar_wait(acc1_full, 0);        // phase 1 MMAs have consumed the ring: region R may be reused
@@ -133,9 +143,9 @@ k_tc_bwd_gz(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
           umma_bf16_pair(c.tmem_base, da, desc_kmajor_sw128(bu + k * 32), idesc_u, (kb | k) != 0);
           if (p.ra) umma_bf16_pair(c.tmem_base + p.r, da, desc_kmajor_sw128(bb + k * 32), idesc_b, (kb | k) != 0);
         }
-        umma_commit_pair(&s1_empty[s]);
+        umma_commit_mask(&s1_empty[s], c.pp.all_mask);
       }
-      umma_commit_pair(acc1_full);
+      umma_commit_mask(acc1_full, c.pp.pair_mask);
       if (p.do_dh) {
         mbar_wait_cluster(gz_full, 0);          // gz operand written and the phase 1 accumulator drained
         tc_fence_after_sync();
@@ -506,7 +516,8 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
       if (ra) { p.z1 = dA_out; p.n1 = (long long)d.vocab * ra; }
       if (ra && dB_out) { p.z2 = dB_out; p.n2 = (long long)ra * d.d; }
     }
-    p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.ra = ra; p.tile_m = tc_tile_m(d.n_tokens);
+    p.nq = tc_pairs_per_cluster();
+    p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.ra = ra; p.tile_m = p.nq == 2 ? tc_tile_m4(d.n_tokens) : tc_tile_m(d.n_tokens);
     p.do_dh = dH_out ? 1 : 0;
     p.stage1_bytes = kTileBytes + kc * 64;
     const size_t budget = 227 * 1024 - (size_t)kOutBufs * kTileBytes - 1024 - 1024;   // region R
@@ -531,12 +542,13 @@ int tc_backward(const mapl_boundary_desc& d, const void* g, const void* H, const
     // dH map: when dH is skipped the map is unused but must be valid
     if (!make_tmap_bf16_2d(&tmO, dH_out ? dH_out : g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
     if (!make_tmap_bf16_2d(&tmG, g, N, dd, dd, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
-    if (!make_tmap_bf16_2d(&tmWu, pk.WB, (uint64_t)pk.kc, dd, dd, 64, (uint32_t)d.r / 2)) return MAPL_ERR_CUDA;
-    if (!make_tmap_bf16_2d(&tmWb, pk.WB, (uint64_t)pk.kc, dd, dd, 64, (uint32_t)(ra ? ra : 64) / 2)) return MAPL_ERR_CUDA;
-    if (!make_tmap_bf16_2d(&tmWd, pk.Wd, dd, (uint64_t)pk.kc, (uint64_t)pk.kc, 64, kChunkN / 2)) return MAPL_ERR_CUDA;
-    const unsigned tiles = ((unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m) + 1u) & ~1u;   // whole CTA pairs
+    if (!make_tmap_bf16_2d(&tmWu, pk.WB, (uint64_t)pk.kc, dd, dd, 64, (uint32_t)(d.r / 2 / p.nq))) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmWb, pk.WB, (uint64_t)pk.kc, dd, dd, 64, (uint32_t)((ra ? ra : 64) / 2 / p.nq))) return MAPL_ERR_CUDA;
+    if (!make_tmap_bf16_2d(&tmWd, pk.Wd, dd, (uint64_t)pk.kc, (uint64_t)pk.kc, 64, (uint32_t)(kChunkN / 2 / p.nq))) return MAPL_ERR_CUDA;
+    const unsigned cl = 2u * (unsigned)p.nq;
+    const unsigned tiles = ((unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m) + cl - 1u) / cl * cl;   // whole clusters
     KernelScope ks(KID_TC_BWD_GZ, st);
-    MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_bwd_gz, dim3(tiles), dim3(kThreads), smem, st, tmG, tmWu, tmWb, tmWd, tmO, tmGz, tmGA, p));
+    MAPL_CUDA_CHECK(launch_pdl_cluster(k_tc_bwd_gz, dim3(tiles), dim3(kThreads), smem, st, cl, tmG, tmWu, tmWb, tmWd, tmO, tmGz, tmGA, p));
   }
   {  // ---- dU (+ dA scatter)
     BwdDuParams p;

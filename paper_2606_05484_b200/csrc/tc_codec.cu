@@ -3,6 +3,7 @@
 #include "tc_codec.cuh"
 
 #include <cuda_fp16.h>
+#include <stdlib.h>
 
 #include "profile.cuh"
 
@@ -63,6 +64,21 @@ int tc_tile_m(long long N) {
   if (t > 128) t = 128;
   if (t < 8) t = 8;
   return (int)t;
+}
+
+int tc_tile_m4(long long N) {
+  const long long ctas = 132, per_wave = ctas * 128;
+  const long long waves = (N + per_wave - 1) / per_wave;
+  long long t = (N + ctas * waves - 1) / (ctas * waves);
+  t = (t + 7) / 8 * 8;
+  if (t > 128) t = 128;
+  if (t < 8) t = 8;
+  return (int)t;
+}
+
+int tc_pairs_per_cluster() {
+  static const int nq = (getenv("MAPL_NQ") && getenv("MAPL_NQ")[0] == '2') ? 2 : 1;
+  return nq;
 }
 
 namespace {

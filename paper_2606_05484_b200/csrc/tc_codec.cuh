@@ -53,6 +53,13 @@ size_t tc_rvq_overflow_bytes(const mapl_boundary_desc& d);
 
 // tokens per CTA (<= 128, multiple of 8) such that the grid covers the 148 SMs in whole, even waves
 int tc_tile_m(long long N);
+// the same for kernels launched as clusters of two CTA pairs: only 33 such clusters (132 CTAs) are resident at a time
+// (cudaOccupancyMaxActiveClusters on B200: the GPCs do not all hold a multiple of 4 SMs)
+int tc_tile_m4(long long N);
+// pairs per cluster for decode / backward-gz: 1, or 2 with MAPL_NQ=2 in the environment -- then the two pairs of a
+// cluster share every parameter tile by TMA multicast (half the L2 -> SM parameter traffic).  Measured at config 3: no
+// gain (decode 59.4 vs 58.9 us, backward 161 vs 163 us) while only 132 CTAs are resident, so it stays opt-in.
+int tc_pairs_per_cluster();
 
 // tok / Tc (both or neither): sender-side centring z -= Tc[tok], Tc [V,r] fp32 (mapl_center_table)
 // ovf_ws: tc_rvq_overflow_bytes(d) bytes of scratch (RVQ only; nullptr: lists limited to shared memory)

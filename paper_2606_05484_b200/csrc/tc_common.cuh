@@ -98,6 +98,19 @@ __device__ __forceinline__ void tma_load_2d_pair(void* smem_dst, const CUtensorM
       ::"r"(smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(m)), "r"(smem_u32(bar) & kPeerBitMask), "r"(c0), "r"(c1), "l"(policy)
       : "memory");
 }
+// the same, multicast: the box lands at the same CTA-relative offset in every CTA of `cta_mask` (cluster ranks), and each
+// destination credits the bytes to the barrier at this offset in the leader of ITS pair.  Used by clusters of two pairs
+// whose CTAs of equal pair rank hold identical parameter tiles: each loads half and sends it to both, which halves the
+// L2 -> SM traffic of the parameter stream.
+__device__ __forceinline__ void tma_load_2d_pair_mc(void* smem_dst, const CUtensorMap* m, uint64_t* bar, int c0, int c1,
+                                                    uint16_t cta_mask, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster.L2::cache_hint"
+      " [%0], [%1, {%4, %5}], [%2], %3, %6;"
+      ::"r"(smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(m)), "r"(smem_u32(bar) & kPeerBitMask), "h"(cta_mask), "r"(c0), "r"(c1),
+        "l"(policy)
+      : "memory");
+}
 __device__ __forceinline__ void tma_store_2d(const CUtensorMap* m, const void* smem_src, int c0, int c1) {
   asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
                ::"l"(reinterpret_cast<uint64_t>(m)), "r"(smem_u32(smem_src)), "r"(c0), "r"(c1) : "memory");
@@ -232,6 +245,26 @@ __device__ __forceinline__ void umma_bf16_pair(uint32_t tmem_d, uint64_t desc_a,
 __device__ __forceinline__ void umma_commit_pair(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
                ::"r"(smem_u32(bar)), "h"((uint16_t)3) : "memory");
+}
+// the same with an explicit mask of cluster ranks (clusters of more than one pair)
+__device__ __forceinline__ void umma_commit_mask(uint64_t* bar, uint16_t cta_mask) {
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(smem_u32(bar)), "h"(cta_mask) : "memory");
+}
+// Position of a CTA in a cluster of nq CTA pairs (nq = 1 or 2; cluster ranks 2q, 2q+1 form pair q)
+struct PairPos {
+  uint32_t pr, q, nq;            // rank inside the pair (0 = leader, issues the MMAs), pair number, pairs in the cluster
+  uint16_t pair_mask, all_mask, twin_mask;   // this pair / every CTA / the CTAs with this pair rank (they hold equal parameter tiles)
+};
+__device__ __forceinline__ PairPos pair_pos(uint32_t nq) {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  PairPos p;
+  p.pr = r & 1u; p.q = r >> 1; p.nq = nq;
+  p.pair_mask = (uint16_t)(3u << (r & ~1u));
+  p.all_mask = (uint16_t)((1u << (2u * nq)) - 1u);
+  p.twin_mask = (uint16_t)(nq == 2 ? (5u << p.pr) : (1u << p.pr));
+  return p;
 }
 template <uint32_t kCols>
 __device__ __forceinline__ void tmem_alloc_pair(uint32_t* smem_result) {   // one full warp in each CTA, same warp id

@@ -25,7 +25,7 @@ struct DecodeParams {
   const int32_t* tok; const float* A;             // anchor gather (tok != nullptr)
   long long N;
   int d, r, ra, L, K;
-  int tile_m, b_stages, z_from_tma;
+  int tile_m, b_stages, z_from_tma, nq;
 };
 
 __global__ void __launch_bounds__(kThreads, 1)
@@ -35,7 +35,8 @@ k_tc_decode(const __grid_constant__ CUtensorMap tmZ, const __grid_constant__ CUt
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   ChunkPipe c;
   c.nkb = (p.r + p.ra) / 64; c.nchunks = p.d / kChunkN; c.b_stages = p.b_stages;
-  c.rank = cluster_ctarank();
+  c.pp = pair_pos((uint32_t)p.nq);
+  c.rank = c.pp.pr;
   c.sA = smem;
   c.sOut = c.sA + (size_t)c.nkb * kTileBytes;
   c.sB = c.sOut + (size_t)kOutBufs * kTileBytes;
@@ -135,7 +136,8 @@ int tc_decode(const mapl_boundary_desc& d, const void* Z, const int32_t* codes, 
   DecodeParams p;
   p.codes = codes; p.codebooks = codebooks; p.tok = ra ? tok : nullptr; p.A = A;
   p.N = d.n_tokens; p.d = d.d; p.r = d.r; p.ra = ra; p.L = d.rvq_levels; p.K = d.rvq_k;
-  p.tile_m = tc_tile_m(d.n_tokens);
+  p.nq = tc_pairs_per_cluster();
+  p.tile_m = p.nq == 2 ? tc_tile_m4(d.n_tokens) : tc_tile_m(d.n_tokens);
   p.z_from_tma = codes ? 0 : 1;
   const size_t fixed = (size_t)(nkb + kOutBufs) * kTileBytes + 1024 + 512;
   p.b_stages = (int)((227 * 1024 - fixed) / kTileBytes);
@@ -147,12 +149,13 @@ int tc_decode(const mapl_boundary_desc& d, const void* Z, const int32_t* codes, 
   const void* zbase = codes ? (const void*)pk.Wd : Z;
   if (!make_tmap_bf16_2d(&tmZ, zbase, codes ? (uint64_t)d.d : (uint64_t)d.n_tokens, codes ? (uint64_t)kc : (uint64_t)d.r,
                          codes ? (uint64_t)kc : (uint64_t)d.r, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
-  if (!make_tmap_bf16_2d(&tmW, pk.Wd, (uint64_t)d.d, (uint64_t)kc, (uint64_t)kc, 64, kChunkN / 2)) return MAPL_ERR_CUDA;
+  if (!make_tmap_bf16_2d(&tmW, pk.Wd, (uint64_t)d.d, (uint64_t)kc, (uint64_t)kc, 64, (uint32_t)(kChunkN / 2 / p.nq))) return MAPL_ERR_CUDA;
   if (!make_tmap_bf16_2d(&tmO, Hhat_out, (uint64_t)d.n_tokens, (uint64_t)d.d, (uint64_t)d.d, 64, (uint32_t)p.tile_m)) return MAPL_ERR_CUDA;
   MAPL_SMEM_OPT_IN(k_tc_decode, 227 * 1024);
-  const unsigned tiles = ((unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m) + 1u) & ~1u;   // whole CTA pairs
+  const unsigned cl = 2u * (unsigned)p.nq;
+  const unsigned tiles = ((unsigned)((d.n_tokens + p.tile_m - 1) / p.tile_m) + cl - 1u) / cl * cl;   // whole clusters
   KernelScope ks(KID_TC_DECODE, st);
-  MAPL_CUDA_CHECK(launch_pdl_pair(k_tc_decode, dim3(tiles), dim3(kThreads), smem, st, tmZ, tmW, tmO, p));
+  MAPL_CUDA_CHECK(launch_pdl_cluster(k_tc_decode, dim3(tiles), dim3(kThreads), smem, st, cl, tmZ, tmW, tmO, p));
   return MAPL_OK;
 }
 

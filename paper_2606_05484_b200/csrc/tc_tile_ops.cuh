@@ -57,19 +57,37 @@ struct ChunkPipe {
   uint64_t* b_full; uint64_t* b_empty;       // [b_stages]
   uint64_t* acc_full; uint64_t* acc_empty;   // [kAccStages]
   int nkb, nchunks, b_stages;
-  uint32_t tmem_base, rank;
+  uint32_t tmem_base, rank;   // rank = rank inside the pair
+  PairPos pp;                 // pp.nq == 2: the W tiles are shared with the twin CTA of the other pair (multicast)
 };
 
-// producer: one thread in each CTA; tmW box = [128 rows x 64 cols]
+// producer: one thread in each CTA; tmW box = [128 / nq rows x 64 cols]
 __device__ __forceinline__ void chunk_produce(const ChunkPipe& c, const CUtensorMap* tmW) {
   RingPos rp;
+#ifdef MAPL_DBG
+  long long w_empty = 0;
+#endif
   for (int j = 0; j < c.nchunks; ++j)
     for (int kb = 0; kb < c.nkb; ++kb) {
+#ifdef MAPL_DBG
+      const long long t_a = clock64();
+#endif
       mbar_wait(&c.b_empty[rp.st], rp.ph ^ 1u);
+#ifdef MAPL_DBG
+      w_empty += clock64() - t_a;
+#endif
       if (c.rank == 0) mbar_arrive_expect_tx(&c.b_full[rp.st], 2 * kTileBytes);
-      tma_load_2d_pair(c.sB + (size_t)rp.st * kTileBytes, tmW, &c.b_full[rp.st], kb * 64, j * kChunkN + (int)c.rank * (kChunkN / 2), kEvictLast);
+      uint8_t* dst = c.sB + (size_t)rp.st * kTileBytes;
+      const int row = j * kChunkN + (int)c.rank * (kChunkN / 2);
+      if (c.pp.nq == 1) tma_load_2d_pair(dst, tmW, &c.b_full[rp.st], kb * 64, row, kEvictLast);
+      else   // this CTA's half of the rows it holds, sent to itself and to its twin (tmW box: kChunkN / 4 rows)
+        tma_load_2d_pair_mc(dst + (size_t)c.pp.q * (kTileBytes / 2), tmW, &c.b_full[rp.st], kb * 64, row + (int)c.pp.q * (kChunkN / 4),
+                            c.pp.twin_mask, kEvictLast);
       rp.next(c.b_stages);
     }
+#ifdef MAPL_DBG
+  g_dbg[blockIdx.x * 64 + 62] = (unsigned long long)w_empty;      // cycles the producer waited for free ring slots
+#endif
 }
 
 // MMA issuer: one thread of the LEADER CTA; the A operands of both CTAs must already be visible to
@@ -78,25 +96,44 @@ __device__ __forceinline__ void chunk_mma(const ChunkPipe& c) {
   const uint32_t idesc = make_idesc_bf16(256, kChunkN, false, false);
   const uint32_t sA0 = smem_u32(c.sA), sB0 = smem_u32(c.sB);
   RingPos rp;
+#ifdef MAPL_DBG
+  long long w_acc = 0, w_full = 0, t_b;
+#endif
   for (int j = 0; j < c.nchunks; ++j) {
     const int as = j % kAccStages;
+#ifdef MAPL_DBG
+    t_b = clock64();
+#endif
     mbar_wait_cluster(&c.acc_empty[as], ((j / kAccStages) & 1) ^ 1);
+#ifdef MAPL_DBG
+    w_acc += clock64() - t_b;
+#endif
     if (j < 16) DBGT(8 + j)
     tc_fence_after_sync();
     const uint32_t tmem_d = c.tmem_base + as * kChunkN;
     for (int kb = 0; kb < c.nkb; ++kb) {
+#ifdef MAPL_DBG
+      t_b = clock64();
+#endif
       mbar_wait(&c.b_full[rp.st], rp.ph);
+#ifdef MAPL_DBG
+      w_full += clock64() - t_b;
+#endif
       tc_fence_after_sync();
       const uint32_t a = sA0 + (uint32_t)kb * kTileBytes, b = sB0 + (uint32_t)rp.st * kTileBytes;
 #pragma unroll
       for (int k = 0; k < 4; ++k)
         umma_bf16_pair(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc, (kb | k) != 0);
-      umma_commit_pair(&c.b_empty[rp.st]);
+      umma_commit_mask(&c.b_empty[rp.st], c.pp.all_mask);      // every CTA that writes into this stage (own pair + twins)
       rp.next(c.b_stages);
     }
-    umma_commit_pair(&c.acc_full[as]);
+    umma_commit_mask(&c.acc_full[as], c.pp.pair_mask);
     if (j < 16) DBGT(24 + j)
   }
+#ifdef MAPL_DBG
+  g_dbg[blockIdx.x * 64 + 60] = (unsigned long long)w_acc;       // cycles the MMA issuer waited for a free accumulator stage
+  g_dbg[blockIdx.x * 64 + 61] = (unsigned long long)w_full;      // ... and for W tiles
+#endif
 }
 
 // epilogue: the 8 warps with threadIdx.x in [64,320) of each CTA.  Warp w reads TMEM lane quarter
@@ -151,7 +188,7 @@ __device__ __forceinline__ void chunk_epilogue(const ChunkPipe& c, const CUtenso
 }
 
 __device__ __forceinline__ void chunk_init_barriers(const ChunkPipe& c) {
-  for (int s = 0; s < c.b_stages; ++s) { mbar_init(&c.b_full[s], 1); mbar_init(&c.b_empty[s], 1); }
+  for (int s = 0; s < c.b_stages; ++s) { mbar_init(&c.b_full[s], 1); mbar_init(&c.b_empty[s], c.pp.nq); }
   for (int s = 0; s < kAccStages; ++s) { mbar_init(&c.acc_full[s], 1); mbar_init(&c.acc_empty[s], 16); }
 }
 
@@ -219,7 +256,23 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
   return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
 }
 
-// same, as clusters of two CTAs (CTA pairs for cta_group::2); grid.x must be even
+// same, as clusters of `cluster_x` CTAs (2: one CTA pair for cta_group::2; 4: two pairs sharing parameter tiles by
+// multicast); grid.x must be a multiple of cluster_x
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl_cluster(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                      unsigned cluster_x, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  static const bool pdl = getenv("MAPL_NO_PDL") == nullptr;
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+  attr[1].id = cudaLaunchAttributeClusterDimension;
+  attr[1].val.clusterDim.x = cluster_x; attr[1].val.clusterDim.y = 1; attr[1].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 2;
+  return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_pdl_pair(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
                                    Args&&... args) {

@@ -382,3 +382,16 @@ def test_repeatability_of_atomic_free_outputs(name, n):
         # the atomically accumulated gradients may differ in the last bits only
         for k in ("dU", "dA"):
             assert rel_fro(out[k], ref[k]) <= 1e-5
+
+
+def test_cluster_of_two_pairs_multicast_path():
+    """MAPL_NQ=2: decode and backward-gz run as clusters of two CTA pairs that share every parameter tile by TMA
+    multicast (opt-in).  The switch is read once per process, so this runs in a subprocess:
+    reduced c1 / c3 against the oracle."""
+    import os, subprocess, sys
+    code = ("import sys; sys.path.insert(0, 'tests'); import test_parity_codec as T; "
+            "T.test_reduced_configs('c1', 2125); T.test_reduced_configs('c3', 517); T.test_anchor_visible('c2', 300); print('ok')")
+    env = dict(os.environ, MAPL_NQ="2")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0 and "ok" in out.stdout, out.stdout[-2000:] + out.stderr[-2000:]
