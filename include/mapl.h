@@ -158,8 +158,8 @@ int mapl_codec_backward(const mapl_boundary_desc* desc, const void* g_Hhat, cons
  *     dA_s = - D (B_s U)^T   [V,ra];    dB_s = - Q U^T   [ra,d] (optional, NULL = skipped);
  *     dU  += - B_s^T Q       [d,r]      (always ADDED: it completes the H^T gz that mapl_codec_backward formed
  *                                        with the uncentred H to (H - A_s[tok] B_s)^T gz).
- * accumulate 0 / 1 applies to dA_s and dB_s as in mapl_codec_backward.  fp32 arithmetic; work is O(N r ra): only the
- * rows of dA_s that tok touches are formed (the others are zeroed / left alone).  workspace: mapl_center_backward_workspace_bytes(desc).   */
+ * accumulate 0 / 1 applies to dA_s and dB_s as in mapl_codec_backward.  fp32 arithmetic; work is O(V r ra),
+ * independent of N apart from the scatter.  workspace: mapl_center_backward_workspace_bytes(desc).   */
 size_t mapl_center_workspace_bytes(const mapl_boundary_desc* desc);
 size_t mapl_center_backward_workspace_bytes(const mapl_boundary_desc* desc);
 int mapl_center_table(const mapl_boundary_desc* desc, const float* A_s, const float* B_s, const float* U,

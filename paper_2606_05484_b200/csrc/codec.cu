@@ -189,14 +189,15 @@ int mapl_center_table(const mapl_boundary_desc* desc, const float* A_s, const fl
 }
 
 namespace {
-struct CenterWs { size_t T, Q, Wc, Ut, total; };
+struct CenterWs { size_t D, Q, Wc, Wct, Ut, total; };
 CenterWs center_carve(const mapl_boundary_desc& d) {
   CenterWs w;
   size_t off = 0;
   auto seg = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
-  w.T = seg((size_t)(d.n_tokens > 0 ? d.n_tokens : 1) * d.anchor_rank * 4);
+  w.D = seg((size_t)d.vocab * d.r * 4);
   w.Q = seg((size_t)d.anchor_rank * d.r * 4);
   w.Wc = seg((size_t)d.anchor_rank * d.r * 4);
+  w.Wct = seg((size_t)d.anchor_rank * d.r * 4);
   w.Ut = seg((size_t)d.d * d.r * 4);
   w.total = off + 256;
   return w;
@@ -221,32 +222,19 @@ int mapl_center_backward(const mapl_boundary_desc* desc, const void* gz, const i
   if (!workspace || workspace_bytes < w.total) return MAPL_ERR_WORKSPACE;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   char* ws = reinterpret_cast<char*>(workspace);
-  // Work proportional to the tokens, not to the vocabulary (only rows that tok touches change):
-  //   T = -gz (B_s U)^T [N,ra];  dA_s[tok_n] += T_n;  Q = A_s[tok]^T gz [ra,r];  dU += -B_s^T Q;  dB_s = -Q U^T
-  float* T = reinterpret_cast<float*>(ws + w.T);       // [N,ra]
-  float* Q = reinterpret_cast<float*>(ws + w.Q);       // [ra,r] sum_n A_s[tok_n] (outer) gz_n
+  float* D = reinterpret_cast<float*>(ws + w.D);       // [V,r]  D[v] = sum_{n: tok_n = v} gz_n
+  float* Q = reinterpret_cast<float*>(ws + w.Q);       // [ra,r] A_s^T D = sum_n A_s[tok_n] (outer) gz_n
   float* Wc = reinterpret_cast<float*>(ws + w.Wc);     // [ra,r] B_s U
+  float* Wct = reinterpret_cast<float*>(ws + w.Wct);   // [r,ra]
   float* Ut = reinterpret_cast<float*>(ws + w.Ut);     // [r,d]
   const int V = d.vocab, ra = d.anchor_rank, r = d.r, dd = d.d;
-  const int bf = d.act_dtype == MAPL_BF16;
+  { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(D, 0, (size_t)V * r * 4, st)); }
   { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(Q, 0, (size_t)ra * r * 4, st)); }
-  if (!accumulate) { KernelScope ks(KID_MEMSET, st); MAPL_CUDA_CHECK(cudaMemsetAsync(dA_s_out, 0, (size_t)V * ra * 4, st)); }
+  MAPL_RETURN_IF(simt_scatter_add_act_rows(gz, d.act_dtype == MAPL_BF16, tok, D, d.n_tokens, r, st));
   MAPL_RETURN_IF(st_gemm_nn(B_s, U, Wc, ra, r, dd, st));
-  if (d.n_tokens > 0) {
-    GemmArgs t;                                        // T = -gz Wc^T
-    t.M = (int)d.n_tokens; t.N = ra; t.K[0] = r;
-    t.A[0].p = gz; t.A[0].bf16 = bf; t.A[0].so = r; t.A[0].sk = 1;
-    t.B[0].p = Wc; t.B[0].so = r; t.B[0].sk = 1;
-    t.C = T; t.ldc = ra; t.alpha = -1.f;
-    MAPL_RETURN_IF(simt_gemm(t, st));
-    MAPL_RETURN_IF(simt_scatter_add_rows(T, tok, dA_s_out, d.n_tokens, ra, st));
-    GemmArgs q;                                        // Q += A_s[tok]^T gz  (split over the tokens, atomic)
-    q.M = ra; q.N = r; q.K[0] = (int)d.n_tokens;
-    q.A[0].p = A_s; q.A[0].so = 1; q.A[0].sk = ra; q.A[0].gather = tok; q.A[0].gmode = 2;
-    q.B[0].p = gz; q.B[0].bf16 = bf; q.B[0].so = 1; q.B[0].sk = r;
-    q.C = Q; q.ldc = r; q.atomic = 1; q.splits = (int)((d.n_tokens + 127) / 128);     // 2 tiles only: parallelism comes from the token split
-    MAPL_RETURN_IF(simt_gemm(q, st));
-  }
+  MAPL_RETURN_IF(simt_transpose(Wc, Wct, ra, r, st));
+  MAPL_RETURN_IF(st_gemm_tn(A_s, D, Q, ra, r, V, st));                                        // Q = A_s^T D
+  MAPL_RETURN_IF(st_gemm_nn(D, Wct, dA_s_out, V, ra, r, st, -1.f, accumulate ? dA_s_out : nullptr, 1.f));   // dA_s = -D Wc^T
   MAPL_RETURN_IF(st_gemm_tn(B_s, Q, dU_inout, dd, r, ra, st, -1.f));                         // dU += -B_s^T Q
   if (dB_s_out) {
     MAPL_RETURN_IF(simt_transpose(U, Ut, dd, r, st));
