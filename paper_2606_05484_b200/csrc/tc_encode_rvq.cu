@@ -439,8 +439,17 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       r1.advance(pi, p.stages1);
       int kr = pi + rot_k;
       if (kr >= nkb1) kr -= nkb1;
+#ifdef MAPL_DBG
+      long long w_empty1 = 0;
+#endif
       for (int kb = pi < kP1 ? pi : nkb1; kb < nkb1; kb += kP1) {
+#ifdef MAPL_DBG
+        const long long t_w = clock64();
+#endif
         mbar_wait(&s.s1_empty[r1.st], r1.ph ^ 1u);
+#ifdef MAPL_DBG
+        w_empty1 += clock64() - t_w;
+#endif
         if (rank == 0) mbar_arrive_expect_tx(&s.s1_full[r1.st], tx1);
         uint8_t* a = s.ring1 + (size_t)r1.st * p.stage1_bytes;
         tma_load_2d_pair(a, &tmH, &s.s1_full[r1.st], kr * 64, (int)m0, kEvictFirst);
@@ -451,6 +460,9 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         kr += kP1;
         if (kr >= nkb1) kr -= nkb1;
       }
+#ifdef MAPL_DBG
+      if (pi == 0) g_dbg[blockIdx.x * 64 + 23] = (unsigned long long)w_empty1;   // producer 0: cycles waiting for free stages
+#endif
       mbar_wait(s.z_full, 0);             // phase-1 MMAs have consumed region R: it may be reused
       // level phase: producer pi takes the chunks pi, pi + kProducers, ... (counted over all levels): the chunk's nkb
       // codebook tiles and its norm tile
@@ -484,8 +496,17 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
     if (rank == 0 && elect_one()) {
       const uint32_t idesc1 = make_idesc_bf16(256, (uint32_t)p.r, false, false);
       RingPos r1;
+#ifdef MAPL_DBG
+      long long w_full1 = 0;
+#endif
       for (int kb = 0; kb < nkb1; ++kb) {
+#ifdef MAPL_DBG
+        const long long t_w = clock64();
+#endif
         mbar_wait(&s.s1_full[r1.st], r1.ph);
+#ifdef MAPL_DBG
+        w_full1 += clock64() - t_w;
+#endif
         tc_fence_after_sync();
         const uint32_t a = smem_u32(s.ring1 + (size_t)r1.st * p.stage1_bytes);
         const uint32_t bh = a + kTileBytes, bl = bh + p.r * 64, bl2 = bl + p.r * 64;
@@ -504,6 +525,9 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         r1.next(p.stages1);
       }
       umma_commit_pair(s.z_full);
+#ifdef MAPL_DBG
+      g_dbg[blockIdx.x * 64 + 22] = (unsigned long long)w_full1;      // cycles the projection MMAs waited for their stages
+#endif
       const uint32_t idesc2 = make_idesc_f16(256, kChunk);
       const uint64_t dax = desc_kmajor_sw32_k16(smem_u32(s.sAx));
       const uint32_t sRho0 = smem_u32(s.sRho), ringC0 = smem_u32(s.ringC), ringX0 = smem_u32(s.ringX);

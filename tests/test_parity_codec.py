@@ -395,3 +395,36 @@ def test_cluster_of_two_pairs_multicast_path():
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     out = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=300)
     assert out.returncode == 0 and "ok" in out.stdout, out.stdout[-2000:] + out.stderr[-2000:]
+
+
+def test_tc_rvq_candidate_list_spills_to_the_overflow_area():
+    """12 near-copies of w in 12 different 32-codeword pieces of ONE scan thread's share (even pieces): more groups
+    inside the final margin than the shared-memory list holds (8 at r = 64), fewer than list + overflow area (16), so
+    the answer comes from the overflow entries without the exhaustive pass.  Codes against the oracle under S5; the
+    true nearest copy is decided by the exact pass."""
+    K, r, n = 2048, 64, 336
+    bi = I.make_generic(36, n, 256, r, 1, K, 100, 0, "bf16", cb_std=(1.0,))
+    rng = np.random.default_rng(13)
+    C = bi.C.f64.copy()
+    w = rng.standard_normal(r) * 1.5
+    spots = [64 * j + 5 for j in range(3, 15)]                 # pieces 6, 8, ..., 28: all even
+    for k in spots:
+        C[0, k] = w + 2e-3 * rng.standard_normal(r)            # spread far below the margin (~0.1), far above fp32 noise
+    Z = w[None, :] + 0.02 * rng.standard_normal((n, r))
+    bi = dataclasses.replace(_with_codebook(bi, C), H=I.store(Z @ bi.U.f64.T, "bf16"))
+    gpu, ora, stats, errs = _roundtrip(bi)
+    assert np.isin(gpu["codes"][:, 0], spots).all()
+
+
+@pytest.mark.parametrize("scale", [1e-6, 3e3])
+def test_tc_rvq_extreme_activation_scale(scale):
+    """Residuals far smaller / larger than the codebook: the per-token power-of-two scale of the fp16 operand leaves the
+    range in which the norm step's a' is an fp16 power of two (tiny h: `hard` tokens, exhaustive exact pass) or sits at
+    its other end (large h).  Codes must still be the oracle's."""
+    bi = I.make_generic(37, 200, 256, 64, 2, 256, 100, 0, "bf16", cb_std=(1.0, 0.5))
+    H = I.store(bi.H.f64 * scale, "bf16")
+    bi = dataclasses.replace(bi, H=H)
+    gpu = run_gpu(bi)
+    ora, stats = run_oracle(bi, gpu_codes=gpu["codes"])
+    assert stats["bad"] == 0, stats
+    assert np.array_equal(gpu["codes"], ora["codes"])
