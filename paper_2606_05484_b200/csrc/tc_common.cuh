@@ -246,6 +246,24 @@ __device__ __forceinline__ void umma_commit_pair(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
                ::"r"(smem_u32(bar)), "h"((uint16_t)3) : "memory");
 }
+// Descriptor arithmetic for issue loops.  The single thread that issues the MMAs pays every instruction's latency in
+// full (microbench/umma_a_tmem.cu: a tcgen05.mma costs ~52 cycles to issue, an N = 128 MMA runs 64), so a descriptor is
+// not rebuilt from an address per MMA (four dependent uniform-datapath operations): its low word advances by
+// bytes >> 4 (shared-memory addresses are < 256 KB: no carry out of the 14-bit address field), the high word is a constant.
+__device__ __forceinline__ uint32_t desc_lo_kmajor_sw128(uint32_t saddr) { return ((saddr & 0x3FFFFu) >> 4) | (1u << 16); }
+constexpr uint32_t kDescHiSw128 = (1024u >> 4) | (1u << 14) | (2u << 29);      // SBO 1024, version 1, SWIZZLE_128B
+__device__ __forceinline__ void umma_bf16_pair_lo(uint32_t tmem_d, uint32_t lo_a, uint32_t lo_b, uint32_t idesc,
+                                                  uint32_t accumulate) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      ".reg .b64 da, db;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "mov.b64 da, {%1, %5};\n"
+      "mov.b64 db, {%2, %5};\n"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], da, db, %3, p;\n"
+      "}\n" ::"r"(tmem_d), "r"(lo_a), "r"(lo_b), "r"(idesc), "r"(accumulate), "n"(kDescHiSw128) : "memory");
+}
 // the same with an explicit mask of cluster ranks (clusters of more than one pair)
 __device__ __forceinline__ void umma_commit_mask(uint64_t* bar, uint16_t cta_mask) {
   asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"

@@ -24,9 +24,10 @@
 //             DIRECT form sum_j (rho_j - c_kj)^2 (rho from TMEM, the fp32 codeword from L2), lowest index winning
 //             ties (S4).  Then rho -= C[l, k*], fused with the fp16 conversion for the next level (the scale comes
 //             from the bound max|rho| + max|c|: fp16 precision does not depend on it).
-//             A list holds kne groups; when it is full a stale entry (below the current threshold) is reused, else the
-//             lowest maximum is dropped and remembered: only if that value is within the FINAL threshold does the
-//             thread fall back to the exhaustive fp32 pass over its codewords (duplicate-heavy codebooks).
+//             A list holds kne groups in shared memory, written without branches as a FIFO (the threshold only rises,
+//             so the oldest entry is the likeliest to be stale); a live entry that must make room moves to a global
+//             overflow area, and only a maximum that finds no room there either and is within the FINAL threshold
+//             sends the thread to the exhaustive fp32 pass over its codewords (duplicate-heavy codebooks).
 // Roofline: tensor at config 3 (K r = 1M per level), HBM at config 2.
 #include <float.h>
 
@@ -303,6 +304,7 @@ struct CandList {
   uint8_t* ovf;              // this thread's global overflow entries (nullptr: none)
   int kne, kovf;
   int cnt;             // shared-memory entries in use (high-water mark)
+  int slot;            // next slot of the FIFO
   int novf;            // overflow entries in use
   float dropped;       // highest maximum that found no room anywhere (-FLT_MAX: none)
 };
@@ -319,45 +321,73 @@ __device__ __forceinline__ void ovf_put(CandList& cl, float m, int gid, const ui
   }
 }
 
-// record the group `gid` (maximum m, scores v[0..16)); thr = current threshold.  Lane-divergent.  While the list has
-// room the group is appended; when it is full, a stale entry (below the current threshold, which only rises during a
-// scan) is reused, else the shared-memory list keeps the kne highest maxima and the lowest one moves to the global
-// overflow entries; only what finds no room there either is remembered in `dropped`, and only if that value is within
-// the FINAL threshold does the thread need the exhaustive pass.  (A plain FIFO is cheaper but overflows at r = 256,
-// where many group maxima lie within the margin of each other.  The scan is bound by the TMEM read-out, not by these
-// instructions.)
-__device__ __forceinline__ void stash_group(CandList& cl, float m, int gid, const uint32_t* v, float thr) {
-  int slot = -1;
-  if (cl.cnt < cl.kne) {
-    slot = cl.cnt++;
-  } else {
-    int w = 0;
-    float wm = lds_f32(cl.eM);
-    for (int e = 1; e < cl.kne; ++e) {
-      const float em = lds_f32(cl.eM + e * kEpi * 4);
-      if (em < wm) { wm = em; w = e; }
-    }
-    if (wm < thr) {
-      slot = w;                                           // stale entry: the threshold has passed it
-    } else if (m > wm) {                                  // the lowest entry makes room
-      uint4 q[4];
+// predicated shared-memory accesses: the scan appends to its list WITHOUT branches.  With one token per lane nearly
+// every chunk has some lane whose group is within the margin (a running maximum is beaten ~ln(groups) times per level,
+// times 32 lanes), so a branchy append ran its whole body for every group of every chunk: 130 of the loop's 162
+// warp-instructions, each paying its full latency with two warps per scheduler (ncu source page, config 2: 12 % of
+// the loop's samples issue, the rest are `wait` / `branch_resolving`) -- the scan was bound by this code, not by the
+// TMEM read-out (the earlier 57 B/cycle read-out figure was an artefact of a microbenchmark that spilled to local memory).
+__device__ __forceinline__ float lds_f32_if(bool pr, uint32_t a, float other) {
+  float v;
+  asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\nmov.f32 %0, %3;\n@q ld.shared.f32 %0, [%1];\n}"
+               : "=f"(v) : "r"(a), "r"((int)pr), "f"(other));
+  return v;
+}
+// entry `slot` := (m, gid, 16 raw scores v[0..16)) if pr
+__device__ __forceinline__ void sts_entry_if(bool pr, const CandList& cl, int slot, float m, int gid, const uint32_t* v) {
+  const uint32_t aM = cl.eM + (uint32_t)slot * kEpi * 4, aId = cl.eId + (uint32_t)slot * kEpi * 4;
+  const uint32_t aS = cl.stash + (uint32_t)slot * 4 * kEpi * 16;
+  asm volatile(
+      "{\n.reg .pred q;\nsetp.ne.b32 q, %0, 0;\n"
+      "@q st.shared.f32 [%1], %2;\n"
+      "@q st.shared.s32 [%3], %4;\n"
+      "@q st.shared.v4.u32 [%5], {%6, %7, %8, %9};\n"
+      "@q st.shared.v4.u32 [%5 + 4096], {%10, %11, %12, %13};\n"
+      "@q st.shared.v4.u32 [%5 + 8192], {%14, %15, %16, %17};\n"
+      "@q st.shared.v4.u32 [%5 + 12288], {%18, %19, %20, %21};\n}"
+      ::"r"((int)pr), "r"(aM), "f"(m), "r"(aId), "r"(gid), "r"(aS),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+        "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+      : "memory");
+}
+static_assert(kEpi * 16 == 4096, "sts_entry_if hard-codes the stride between the 16-byte units of an entry");
+
+// The four 16-codeword groups of one chunk (maxima g[], ids gid[], raw scores v[i]) join the list where they are within
+// the current threshold.  The shared-memory entries are a FIFO over kne >= 4 slots: the threshold only rises during a
+// scan, so the oldest entry is the likeliest to be stale (below the threshold: droppable); if it is not, it moves to the
+// global overflow entries first -- the one rare, divergent path, entered on a warp vote.  What finds no room there
+// either is remembered in `dropped`, and only if that value is within the FINAL threshold does the thread need the
+// exhaustive pass.
+__device__ __forceinline__ void stash_chunk(CandList& cl, const float (&g)[4], const int (&gid)[4],
+                                            const uint32_t* const (&v)[4], float thr, bool live) {
+  bool pr[4], spill[4];
+  int sl[4];
+  bool any_spill = false;
 #pragma unroll
-      for (int i = 0; i < 4; ++i) q[i] = lds_v4(cl.stash + (uint32_t)(w * 4 + i) * kEpi * 16);
-      ovf_put(cl, wm, lds_s32(cl.eId + w * kEpi * 4), q);
-      slot = w;
-    } else {
-      const uint4 q[4] = {make_uint4(v[0], v[1], v[2], v[3]), make_uint4(v[4], v[5], v[6], v[7]),
-                          make_uint4(v[8], v[9], v[10], v[11]), make_uint4(v[12], v[13], v[14], v[15])};
-      ovf_put(cl, m, gid, q);
+  for (int i = 0; i < 4; ++i) {
+    pr[i] = live && g[i] >= thr;
+    sl[i] = cl.slot;
+    const bool full = pr[i] && cl.cnt >= cl.kne;          // the slot holds an older entry
+    const float m_old = lds_f32_if(full, cl.eM + (uint32_t)cl.slot * kEpi * 4, -FLT_MAX);
+    spill[i] = full && m_old >= thr;
+    any_spill |= spill[i];
+    if (pr[i]) {
+      cl.slot = cl.slot + 1 == cl.kne ? 0 : cl.slot + 1;
+      cl.cnt = min(cl.cnt + 1, cl.kne);
     }
   }
-  if (slot >= 0) {
-    sts_f32(cl.eM + slot * kEpi * 4, m);
-    sts_s32(cl.eId + slot * kEpi * 4, gid);
+  if (__any_sync(0xffffffffu, any_spill)) {
 #pragma unroll
     for (int i = 0; i < 4; ++i)
-      sts_v4(cl.stash + (uint32_t)(slot * 4 + i) * kEpi * 16, v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+      if (spill[i]) {
+        uint4 q[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) q[u] = lds_v4(cl.stash + (uint32_t)(sl[i] * 4 + u) * kEpi * 16);
+        ovf_put(cl, lds_f32(cl.eM + (uint32_t)sl[i] * kEpi * 4), lds_s32(cl.eId + (uint32_t)sl[i] * kEpi * 4), q);
+      }
   }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) sts_entry_if(pr[i], cl, sl[i], g[i], gid[i], v[i]);
 }
 
 // entry e of the whole list (shared memory first, then the overflow entries): its maximum, group id, and the 16-bit
@@ -530,7 +560,8 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 #endif
       const uint32_t idesc2 = make_idesc_f16(256, kChunk);
       const uint64_t dax = desc_kmajor_sw32_k16(smem_u32(s.sAx));
-      const uint32_t sRho0 = smem_u32(s.sRho), ringC0 = smem_u32(s.ringC), ringX0 = smem_u32(s.ringX);
+      const uint32_t ringX0 = smem_u32(s.ringX);
+      const uint32_t la0 = desc_lo_kmajor_sw128(smem_u32(s.sRho)), lb0 = desc_lo_kmajor_sw128(smem_u32(s.ringC));
       RingPos rc, rx;
       uint32_t as = 0, aph = 0;            // accumulator stage and its use parity
       int cg = 0;
@@ -545,10 +576,9 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
           for (int kb = 0; kb < nkb; ++kb) {
             mbar_wait(&s.c_full[rc.st], rc.ph);
             tc_fence_after_sync();
-            const uint32_t a = sRho0 + (uint32_t)kb * kTileBytes, b = ringC0 + (uint32_t)rc.st * kHalfTileBytes;
+            const uint32_t a = la0 + (uint32_t)kb * (kTileBytes >> 4), b = lb0 + (uint32_t)rc.st * (kHalfTileBytes >> 4);
 #pragma unroll
-            for (int k = 0; k < 4; ++k)
-              umma_bf16_pair(tmem_d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc2, (kb | k) != 0);
+            for (int k = 0; k < 4; ++k) umma_bf16_pair_lo(tmem_d, a + 2 * k, b + 2 * k, idesc2, (kb | k) != 0);
             umma_commit_pair(&s.c_empty[rc.st]);
             rc.next(p.ring_tiles);
           }
@@ -642,7 +672,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       }
 
       float best = -FLT_MAX;
-      cl.cnt = 0; cl.novf = 0; cl.dropped = -FLT_MAX;
+      cl.cnt = 0; cl.slot = 0; cl.novf = 0; cl.dropped = -FLT_MAX;
       int cr = rot_c;
       for (int c = 0; c < nchunks; ++c, ++cg) {
         const int as = cg & 1;
@@ -661,17 +691,18 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         const float m64 = fmaxf(fmaxf(g0, g1), fmaxf(g2, g3));
         best = fmaxf(best, m64);
         const float thr = best - margin;
-        // dead rows hold stale data: never candidates.  (With 32 tokens per warp some lane qualifies in nearly every
-        // chunk -- a token's running maximum is beaten ~ln(groups) times per level -- so there is no warp vote.)
-        if (live && m64 >= thr) {
-          const int gid = (cr * 4 + h) * 2;                // 16-codeword group of v[0][0]; v[1] is kParts pieces further
-          if (g0 >= thr) stash_group(cl, g0, gid, &v[0][0], thr);
-          if (g1 >= thr) stash_group(cl, g1, gid + 1, &v[0][16], thr);
-          if (g2 >= thr) stash_group(cl, g2, gid + 2 * kParts, &v[1][0], thr);
-          if (g3 >= thr) stash_group(cl, g3, gid + 2 * kParts + 1, &v[1][16], thr);
+        // dead rows hold stale data: never candidates
+        {
+          const int gid0 = (cr * 4 + h) * 2;               // 16-codeword group of v[0][0]; v[1] is kParts pieces further
+          const float g[4] = {g0, g1, g2, g3};
+          const int gid[4] = {gid0, gid0 + 1, gid0 + 2 * kParts, gid0 + 2 * kParts + 1};
+          const uint32_t* const vv[4] = {&v[0][0], &v[0][16], &v[1][0], &v[1][16]};
+          stash_chunk(cl, g, gid, vv, thr, live);
         }
         if (++cr == nchunks) cr = 0;
+#ifndef MAPL_DBG2
         if (threadIdx.x == 64 && cg < 8) DBGT(56 + cg)
+#endif
       }
       xBest[mine] = best;
       epi_sync();
@@ -693,6 +724,11 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       }
       if (!live) ncand = 0;
       xCnt[mine] = overflow ? 1000 : ncand;
+#ifdef MAPL_DBG2
+      atomicAdd(&g_dbg[blockIdx.x * 64 + 61], (unsigned long long)ncand);
+      atomicAdd(&g_dbg[blockIdx.x * 64 + 60], (unsigned long long)n_ent);
+      if (cl.novf) atomicAdd(&g_dbg[blockIdx.x * 64 + 59], (unsigned long long)cl.novf);
+#endif
       epi_sync();
       if (warp == 2 && l < 4) { DBG(7 + l * 4) }
       int tot = 0;
@@ -717,6 +753,10 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
           int k = 0;
           if (have) { k = gid * 16 + __ffs(mrem) - 1; mrem &= mrem - 1; }
           const float dx = exact_dist(tmem_row, Cl + (long long)k * p.r, p.r);
+#ifdef MAPL_DBG2
+          if (lane == 0) atomicAdd(&g_dbg[blockIdx.x * 64 + 62], 1ull);
+          if (have) atomicAdd(&g_dbg[blockIdx.x * 64 + 63], 1ull);
+#endif
           if (have && (dx < bestx || (dx == bestx && k < bestk))) { bestx = dx; bestk = k; }
         }
       }
@@ -806,7 +846,7 @@ int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codeb
   const int nkb = d.r / 64;
   const size_t cap = (size_t)227 * 1024 - 1024;
   p.kne = 0; p.ring_tiles = 0;
-  for (int kne = 8; kne >= 3 && p.kne == 0; --kne)
+  for (int kne = 8; kne >= 4 && p.kne == 0; --kne)      // >= 4: the groups of one chunk take distinct slots
     for (int want = 2 * nkb; want >= nkb + 1 && p.kne == 0; --want) {
       p.kne = kne; p.ring_tiles = want; p.stages1 = 0;
       if (rvq_level_bytes(p) + rvq_tail_bytes(kne) > cap) p.kne = 0;
