@@ -1,4 +1,7 @@
-// microbenchmark: tcgen05.ld shapes: bytes per cycle per SM with 4 and 8 warps
+// microbenchmark: tcgen05.ld shapes: bytes per cycle per SM with 4 and 8 warps (one load + wait per iteration; `depth2`:
+// two loads in flight before the wait).  The first version of this file consumed v[it & 31]: the run-time index put
+// v[] in local memory, 32 STL per load went through the same LSU path, and every shape read "57 B/cycle" -- an artefact
+// (profiles/r02_microbench.md keeps both outputs).
 #include <cstdio>
 #include "tc_common.cuh"
 using namespace mapl::tc;
@@ -30,7 +33,34 @@ __global__ void __launch_bounds__(512, 1) k_ld(int W, int iters, long long* out,
       uint32_t v[32];
       ld<V>(tmem + (it & 3) * 64, v);
       tmem_ld_wait();
-      acc += __uint_as_float(v[it & 31]);
+      acc += __uint_as_float(v[0]) + __uint_as_float(v[31]);     // constant indices: a run-time index sends v[] to local memory
+    }
+  }
+  __syncthreads();
+  long long t1 = clock64();
+  if (threadIdx.x == 0) out[0] = t1 - t0;
+  if (acc == 123.456f) sink[0] = acc;
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<512>(slot);
+}
+__global__ void __launch_bounds__(512, 1) k_ld2(int W, int iters, long long* out, float* sink) {
+  __shared__ uint32_t slot;
+  const int warp = threadIdx.x / 32;
+  if (warp == 0) tmem_alloc<512>(&slot);
+  tc_fence_before_sync();
+  __syncthreads();
+  tc_fence_after_sync();
+  const uint32_t tmem = slot + ((uint32_t)((warp & 3) * 32) << 16);
+  float acc = 0.f;
+  __syncthreads();
+  long long t0 = clock64();
+  if (warp < W) {
+    for (int it = 0; it < iters; ++it) {
+      uint32_t v[32], w[32];
+      ld<0>(tmem + (it & 3) * 64, v);
+      ld<0>(tmem + (it & 3) * 64 + 32, w);
+      tmem_ld_wait();
+      acc += __uint_as_float(v[0]) + __uint_as_float(w[31]);
     }
   }
   __syncthreads();
@@ -57,5 +87,12 @@ int main() {
   run<2>("16x128b.x16", 1024, out, sink);
   run<3>("16x64b.x32", 1024, out, sink);
   run<4>("32x32b.pack16.x32 (64c)", 2048, out, sink);
+  for (int W : {4, 8}) {
+    const int iters = 1000;
+    for (int rep = 0; rep < 2; ++rep) k_ld2<<<1, 512>>>(W, iters, out, sink);
+    if (cudaDeviceSynchronize() != cudaSuccess) { printf("depth2 err %s\n", cudaGetErrorString(cudaGetLastError())); return 1; }
+    long long h; cudaMemcpy(&h, out, 8, cudaMemcpyDeviceToHost);
+    printf("%-26s W %d: %7.1f cycles per pair of loads per warp, %6.1f TMEM cells (4 B) per cycle per SM\n", "32x32b.x32 depth2", W, (double)h / iters, W * iters * 2048.0 / h);
+  }
   return 0;
 }

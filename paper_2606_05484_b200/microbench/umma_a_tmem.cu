@@ -1,7 +1,11 @@
 // microbenchmark: tcgen05.mma cta_group::2 with the A operand in TENSOR MEMORY (packed bf16, written by tcgen05.st) against
 // A in shared memory -- (1) the layout: lane = row, 32-bit column j of a K = 16 step = elements (2j, 2j+1); checked against
 // integer arithmetic; (2) cycles per MMA for N = 128 / 256, alone, beside 4 warps of tcgen05.ld, and beside 4 warps of
-// shared-memory traffic (the decode / dH pipeline's staging stores), which is where A-from-shared loses its rate.
+// shared-memory traffic (the decode / dH pipeline's staging stores).  The operand source is a TEMPLATE parameter: the
+// first version chose it with a run-time `if` between the MMAs and measured 113 (N = 128) / 173 (N = 256, A in shared
+// memory) cycles per MMA -- the branch and the descriptor arithmetic on the one issuing thread, not the tensor pipe.
+// Measured with a clean loop: 64 / 128 cycles (the floor) for both operand sources, with or without the tcgen05.ld and
+// shared-memory traffic beside them; N = 32 / 64 show the issue cost itself, ~52 cycles per tcgen05.mma.
 #include <cstdio>
 #include "tc_common.cuh"
 using namespace mapl::tc;
@@ -23,8 +27,9 @@ __device__ __forceinline__ void umma_bf16_pair_ts(uint32_t tmem_d, uint32_t tmem
 }
 
 // mode 0: correctness (N = 128, K = 256); mode 1: timing
+template <int ts>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
-k_ts(int mode, int ts, int N, int chunks, int with_ld, int with_smem, long long* out) {
+k_ts(int mode, int N, int chunks, int with_ld, int with_smem, long long* out) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* sA = smem;                        // kNkb tiles [128 x 64] bf16 SW128 (the shared-memory A operand)
@@ -78,7 +83,7 @@ k_ts(int mode, int ts, int N, int chunks, int with_ld, int with_smem, long long*
     const uint32_t idesc = make_idesc_bf16(256, N, false, false);
     const long long t0 = clock64();
     for (int c = 0; c < chunks; ++c) {
-      const uint32_t d = tmem + (N == 128 ? (c & 1) * 128 : 0);
+      const uint32_t d = tmem + (N <= 128 ? (c & 1) * 128 : 0);
       for (int kb = 0; kb < kNkb; ++kb) {
         const uint32_t a = smem_u32(sA + kb * 16384), b = smem_u32(sB + kb * 16384);
 #pragma unroll
@@ -141,21 +146,20 @@ k_ts(int mode, int ts, int N, int chunks, int with_ld, int with_smem, long long*
   if (warp == 0) { tc_fence_after_sync(); tmem_dealloc_pair<512>(tmem); }
 }
 
-int main() {
-  long long* out; cudaMalloc(&out, 128);
-  cudaFuncSetAttribute(k_ts, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+template <int ts>
+int run(long long* out) {
+  cudaFuncSetAttribute(k_ts<ts>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   const size_t smem = 2 * kNkb * 16384 + 32768 + 1024 + 256;
-  for (int ts : {0, 1}) {
-    cudaMemset(out, 0, 128);
-    k_ts<<<2, kThreads, smem>>>(0, ts, 128, 1, 0, 0, out);
-    if (cudaDeviceSynchronize() != cudaSuccess) { printf("err %s\n", cudaGetErrorString(cudaGetLastError())); return 1; }
-    long long h[16]; cudaMemcpy(h, out, 128, cudaMemcpyDeviceToHost);
-    printf("A from %s: %lld of %d accumulator elements differ from the integer reference\n", ts ? "TMEM" : "smem", h[2], 256 * 128);
-  }
-  for (int N : {128, 256}) for (int ts : {0, 1}) for (int ld : {0, 1}) for (int sm : {0, 1}) {
+  long long h[16];
+  cudaMemset(out, 0, 128);
+  k_ts<ts><<<2, kThreads, smem>>>(0, 128, 1, 0, 0, out);
+  if (cudaDeviceSynchronize() != cudaSuccess) { printf("err %s\n", cudaGetErrorString(cudaGetLastError())); return 1; }
+  cudaMemcpy(h, out, 128, cudaMemcpyDeviceToHost);
+  printf("A from %s: %lld of %d accumulator elements differ from the integer reference\n", ts ? "TMEM" : "smem", h[2], 256 * 128);
+  for (int N : {32, 64, 128, 256}) for (int ld : {0, 1}) for (int sm : {0, 1}) {
+    if (N < 128 && (ld || sm)) continue;
     const int chunks = 200;
-    long long h[16];
-    for (int rep = 0; rep < 2; ++rep) { cudaMemset(out, 0, 128); k_ts<<<2, kThreads, smem>>>(1, ts, N, chunks, ld, sm, out); }
+    for (int rep = 0; rep < 2; ++rep) { cudaMemset(out, 0, 128); k_ts<ts><<<2, kThreads, smem>>>(1, N, chunks, ld, sm, out); }
     if (cudaDeviceSynchronize() != cudaSuccess) { printf("err %s\n", cudaGetErrorString(cudaGetLastError())); return 1; }
     cudaMemcpy(h, out, 128, cudaMemcpyDeviceToHost);
     const int n_mma = chunks * kNkb * 4;
@@ -164,4 +168,10 @@ int main() {
            N, ts ? "TMEM" : "smem", ld, ldb, sm, smb, (double)h[0] / n_mma, (double)h[1] / n_mma, N / 2);
   }
   return 0;
+}
+
+int main() {
+  long long* out; cudaMalloc(&out, 128);
+  if (run<0>(out)) return 1;
+  return run<1>(out);
 }

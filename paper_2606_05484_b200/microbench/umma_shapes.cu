@@ -1,4 +1,7 @@
-// microbenchmark: tcgen05.mma cta_group::2 throughput from shared memory for the RVQ score shape
+// microbenchmark: tcgen05.mma cta_group::2 throughput from shared memory for the RVQ score shape, with the descriptors
+// REBUILT from addresses per MMA as the library's issue loops first did: N = 128 reads 75-108 cycles against a floor of 64
+// because the one issuing thread spends that long between MMAs (umma_a_tmem.cu, with a clean loop, reaches 64); the RVQ
+// scan loop now advances the descriptors' low words instead (umma_bf16_pair_lo in tc_common.cuh).
 #include <cstdio>
 #include "tc_common.cuh"
 using namespace mapl::tc;

@@ -40,7 +40,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(320, 1) k_b(int N, i
       tmem_ld32(tr + (i & 3) * 64, v);
       tmem_ld32(tr + (i & 3) * 64 + 32, w);
       tmem_ld_wait();
-      acc += __uint_as_float(v[i & 31]) + __uint_as_float(w[i & 31]);
+      acc += __uint_as_float(v[0]) + __uint_as_float(w[31]);     // constant indices: v[i & 31] put both arrays in local memory
     }
     t_ld = clock64() - t0;
   }
