@@ -115,6 +115,26 @@ int mapl_encode(const mapl_boundary_desc* desc, const void* H, const float* U, c
                 void* Zq_out, int32_t* codes_out, void* workspace, size_t workspace_bytes,
                 void* cuda_stream);
 
+/* ENCODE WITH RVQ, NO WORKSPACE AND NO ALLOCATION (csrc/static_scratch.cu).  For callers that cannot allocate device
+ * memory and so cannot give mapl_encode a workspace (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc).  Same operation and arguments as mapl_encode with desc.rvq_levels >= 1 (S3, S4), run on
+ * the fp32 SIMT kernels whatever the shape (the kernels mapl_encode uses for fp32 activations and for shapes outside the
+ * tensor-core envelope): its results are those of that path.  Its one piece of scratch, the half squared norms of the
+ * codewords ([L*K] fp32), lives in a device array inside the library: mapl_static_scratch_rows() floats (16384 = 64 KB,
+ * held by every GPU that loads the library until the process exits).
+ *   desc.rvq_levels * desc.rvq_k > mapl_static_scratch_rows()  ->  MAPL_ERR_WORKSPACE, nothing is launched.
+ *   desc.rvq_levels == 0 -> MAPL_ERR_INVALID_ARG (there is no scratch to speak of: use mapl_encode).
+ *   desc.param_pack is ignored.  Other arguments, layouts and errors: as mapl_encode.
+ * The call and everything under it call no cudaMalloc / cudaFree / allocating library routine (with
+ * mapl_profile_enable(0), the default: launch timing creates CUDA events).  The first call on each device looks the
+ * array's address up (cudaGetSymbolAddress): make one call per device before capturing a graph.
+ * All calls on a device share the array.  A call overwrites the L*K entries it uses before reading them and nothing
+ * has to start at zero, so calls in stream order are independent of each other; calls that can OVERLAP on the GPU
+ * (different streams, concurrent graph branches) race on the array: the caller serialises them.                  */
+size_t mapl_static_scratch_rows(void);
+int mapl_encode_rvq_static(const mapl_boundary_desc* desc, const void* H, const float* U, const float* codebooks,
+                           void* Zq_out, int32_t* codes_out, void* cuda_stream);
+
 /* DECODE (receiver side).  P:75 Eq. 2 + P:106 Eq. 3: hhat_n = U zhat_n + B^T A[tok_n,:].
  *   Z / codes  exactly one non-NULL.  Z [N,r] act dtype is used as zhat; codes [N,L] int32 are
  *              dequantised (zhat_n = sum_l C[l,codes[n,l],:], needs L > 0 and codebooks).

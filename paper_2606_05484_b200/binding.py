@@ -51,6 +51,10 @@ def _load():
     lib.mapl_pack_params.restype = C.c_int
     lib.mapl_pack_params.argtypes = [dp, vp, vp, vp, vp, vp]
     lib.mapl_encode.argtypes = [dp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.mapl_static_scratch_rows.restype = sz
+    lib.mapl_static_scratch_rows.argtypes = []
+    lib.mapl_encode_rvq_static.restype = C.c_int
+    lib.mapl_encode_rvq_static.argtypes = [dp, vp, vp, vp, vp, vp, vp]
     lib.mapl_center_workspace_bytes.restype = sz
     lib.mapl_center_workspace_bytes.argtypes = [dp]
     lib.mapl_center_table.restype = C.c_int
@@ -169,6 +173,19 @@ def mapl_encode(desc: BoundaryDesc, H, U, codebooks, Zq_out, codes_out, workspac
                             _ptr(codebooks, torch.float32, "codebooks"), _ptr(Zq_out, act, "Zq_out"),
                             _ptr(codes_out, torch.int32, "codes_out"), _ptr(workspace, None, "workspace"),
                             workspace.numel() * workspace.element_size(), _stream()), "mapl_encode")
+
+
+def mapl_static_scratch_rows() -> int:
+    return int(_lib.mapl_static_scratch_rows())
+
+
+def mapl_encode_rvq_static(desc: BoundaryDesc, H, U, codebooks, Zq_out, codes_out) -> None:
+    """mapl_encode with RVQ on the fp32 SIMT kernels, scratch in a device array of the library: no workspace, no
+    allocation (include/mapl.h).  levels * K > mapl_static_scratch_rows() raises MAPL_ERR_WORKSPACE."""
+    act = act_torch_dtype(desc)
+    _check(_lib.mapl_encode_rvq_static(C.byref(desc), _ptr(H, act, "H"), _ptr(U, torch.float32, "U"),
+                                       _ptr(codebooks, torch.float32, "codebooks"), _ptr(Zq_out, act, "Zq_out"),
+                                       _ptr(codes_out, torch.int32, "codes_out"), _stream()), "mapl_encode_rvq_static")
 
 
 def mapl_center_workspace_bytes(desc: BoundaryDesc) -> int:
