@@ -120,26 +120,36 @@ __device__ __forceinline__ Smem carve_smem(uint8_t* base, const RvqParams& p) {
 // form sum_j (rho_j - c_j)^2 the oracle uses (no cancellation when D << ||c||^2).  Warp-convergent (tcgen05.ld is
 // .sync.aligned); lanes without work pass any valid row and ignore the result.
 __device__ __forceinline__ float exact_dist(uint32_t tmem_row, const float* __restrict__ crow, int r) {
-  // the row loads (L2 latency) of TWO 32-column pieces are in flight together (r is a multiple of 64); the residual
-  // pieces are read from TMEM one at a time to keep the register count down
+  // One 32-column piece of the row (8 float4, L2 latency) is in flight while the piece before it is consumed: the
+  // pass costs one L2 round trip plus r / 32 short steps, where loading two pieces per round and then consuming them
+  // cost r / 64 round trips (r is a multiple of 64: an even number of pieces).  Same summation order as before.
+  const float4* c4 = reinterpret_cast<const float4*>(crow);
   float acc = 0.f;
-  for (int pc = 0; pc < r / 32; pc += 2) {
-    const float4* c4 = reinterpret_cast<const float4*>(crow + pc * 32);
-    float4 c[16];
+  float4 ca[8], cb[8];
+  auto consume = [&](const float4 (&c)[8], int pc) {
+    uint32_t v[32];
+    tmem_ld32(tmem_row + pc * 32, v);
+    tmem_ld_wait();
 #pragma unroll
-    for (int i = 0; i < 16; ++i) c[i] = __ldg(c4 + i);
-#pragma unroll
-    for (int u = 0; u < 2; ++u) {
-      uint32_t v[32];
-      tmem_ld32(tmem_row + (pc + u) * 32, v);
-      tmem_ld_wait();
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const float d0 = __uint_as_float(v[4 * i + 0]) - c[8 * u + i].x, d1 = __uint_as_float(v[4 * i + 1]) - c[8 * u + i].y;
-        const float d2 = __uint_as_float(v[4 * i + 2]) - c[8 * u + i].z, d3 = __uint_as_float(v[4 * i + 3]) - c[8 * u + i].w;
-        acc = fmaf(d0, d0, acc); acc = fmaf(d1, d1, acc); acc = fmaf(d2, d2, acc); acc = fmaf(d3, d3, acc);
-      }
+    for (int i = 0; i < 8; ++i) {
+      const float d0 = __uint_as_float(v[4 * i + 0]) - c[i].x, d1 = __uint_as_float(v[4 * i + 1]) - c[i].y;
+      const float d2 = __uint_as_float(v[4 * i + 2]) - c[i].z, d3 = __uint_as_float(v[4 * i + 3]) - c[i].w;
+      acc = fmaf(d0, d0, acc); acc = fmaf(d1, d1, acc); acc = fmaf(d2, d2, acc); acc = fmaf(d3, d3, acc);
     }
+  };
+#pragma unroll
+  for (int i = 0; i < 8; ++i) ca[i] = __ldg(c4 + i);
+  const int np = r / 32;
+#pragma unroll 1
+  for (int pc = 0; pc < np; pc += 2) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) cb[i] = __ldg(c4 + (pc + 1) * 8 + i);
+    consume(ca, pc);
+    if (pc + 2 < np) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) ca[i] = __ldg(c4 + (pc + 2) * 8 + i);
+    }
+    consume(cb, pc + 1);
   }
   return acc;
 }

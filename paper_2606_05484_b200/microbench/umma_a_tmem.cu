@@ -27,7 +27,9 @@ __device__ __forceinline__ void umma_bf16_pair_ts(uint32_t tmem_d, uint32_t tmem
 }
 
 // mode 0: correctness (N = 128, K = 256); mode 1: timing
-template <int ts>
+// CM / WT: a tcgen05.commit / a wait on an already completed mbarrier (+ fence) after every k-block of 4 MMAs: what the
+// bookkeeping of a pipeline costs the issuing thread
+template <int ts, int CM = 0, int WT = 0>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 k_ts(int mode, int N, int chunks, int with_ld, int with_smem, long long* out) {
   extern __shared__ uint8_t smem_raw[];
@@ -59,7 +61,7 @@ k_ts(int mode, int N, int chunks, int with_ld, int with_smem, long long* out) {
     }
     *reinterpret_cast<uint4*>(sB + kb * 16384 + sw128_offset(row, ch)) = make_uint4(w[0], w[1], w[2], w[3]);
   }
-  if (threadIdx.x == 0) { mbar_init(&bar[0], 1); *done = 0; fence_barrier_init(); }
+  if (threadIdx.x == 0) { mbar_init(&bar[0], 1); mbar_init(&bar[2], 1); mbar_init(&bar[3], 1); *done = 0; fence_barrier_init(); }
   fence_proxy_async_smem();
   if (warp == 0) tmem_alloc_pair<512>(slot);
   tc_fence_before_sync();
@@ -91,6 +93,8 @@ k_ts(int mode, int N, int chunks, int with_ld, int with_smem, long long* out) {
           if (ts) umma_bf16_pair_ts(d, tmem + kACol + kb * 32 + k * 8, desc_kmajor_sw128(b + k * 32), idesc, (kb | k) != 0);
           else umma_bf16_pair(d, desc_kmajor_sw128(a + k * 32), desc_kmajor_sw128(b + k * 32), idesc, (kb | k) != 0);
         }
+        if (CM) umma_commit_pair(&bar[2]);
+        if (WT) { mbar_wait(&bar[3], 1); tc_fence_after_sync(); }
       }
     }
     const long long t1 = clock64();
@@ -170,8 +174,24 @@ int run(long long* out) {
   return 0;
 }
 
+template <int CM, int WT>
+int issue_cost(long long* out) {
+  cudaFuncSetAttribute(k_ts<0, CM, WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  const size_t smem = 2 * kNkb * 16384 + 32768 + 1024 + 256;
+  long long h[16];
+  const int chunks = 200;
+  for (int rep = 0; rep < 2; ++rep) { cudaMemset(out, 0, 128); k_ts<0, CM, WT><<<2, kThreads, smem>>>(1, 64, chunks, 0, 0, out); }
+  if (cudaDeviceSynchronize() != cudaSuccess) { printf("err %s\n", cudaGetErrorString(cudaGetLastError())); return 1; }
+  cudaMemcpy(h, out, 128, cudaMemcpyDeviceToHost);
+  printf("issuing thread, N = 64 (issue-bound): 4 MMAs%s%s: %6.1f cycles\n", CM ? " + commit" : "", WT ? " + completed wait + fence" : "",
+         (double)h[0] / (chunks * kNkb));
+  return 0;
+}
+
 int main() {
   long long* out; cudaMalloc(&out, 128);
   if (run<0>(out)) return 1;
-  return run<1>(out);
+  if (run<1>(out)) return 1;
+  if (issue_cost<0, 0>(out) || issue_cost<1, 0>(out) || issue_cost<0, 1>(out) || issue_cost<1, 1>(out)) return 1;
+  return 0;
 }
