@@ -457,6 +457,18 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc_pair<512>(s.tmem_slot);
+  // Rows tile_m .. 127 of the H tiles are never written by TMA (its box has tile_m rows) and are multiplied all the
+  // same: zero them once, and give the dead rows a zero fp16 operand in the scans too (inv = 0 below).  The chip is
+  // power-limited under tensor load and zero operands are cheap: c3 194.0 -> 192.5 us; it also
+  // keeps whatever the previous kernel left in shared memory (NaN patterns included) out of the tensor pipe.
+  if (p.tile_m < 128) {
+    const int per_stage = (128 - p.tile_m) * 8;                       // 16-byte units of the dead rows of one H tile
+    for (int i = threadIdx.x; i < p.stages1 * per_stage; i += kThreads) {
+      const int st = i / per_stage, u = i - st * per_stage;
+      *reinterpret_cast<uint4*>(s.ring1 + (size_t)st * p.stage1_bytes + (size_t)p.tile_m * 128 + (size_t)u * 16) = make_uint4(0u, 0u, 0u, 0u);
+    }
+    fence_proxy_async_smem();
+  }
   tc_fence_before_sync();
   cluster_sync_all();
   tc_fence_after_sync();
@@ -658,7 +670,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 #pragma unroll
       for (int hh = 0; hh < kParts; ++hh) { n2 += xN2[hh * 128 + row]; amax = fmaxf(amax, xAmax[hh * 128 + row]); }
       inv = inv_scale_of(amax);
-      rho_to_operand(tmem_row, s.sRho, row, p.r, h, inv);
+      rho_to_operand(tmem_row, s.sRho, row, p.r, h, live ? inv : 0.f);
       write_ax(inv * __ldg(p.lvl + 2), hard);
       publish_operand();
     }
@@ -798,7 +810,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         // maximum); the exact ||rho_new||^2 and max|rho_new| are exchanged behind the hand-off.
         inv = inv_scale_of(amax + __ldg(lv + 4));
         float n2p, amaxp;
-        rho_update(tmem_row, Cl + (long long)bestk * p.r, s.sRho, row, p.r, h, inv, &n2p, &amaxp);
+        rho_update(tmem_row, Cl + (long long)bestk * p.r, s.sRho, row, p.r, h, live ? inv : 0.f, &n2p, &amaxp);
         xN2[mine] = n2p; xAmax[mine] = amaxp;
         write_ax(inv * __ldg(lv + 8 + 2), hard);
         if (warp == 2 && l == 1) { DBG(21) }
