@@ -154,6 +154,61 @@ __device__ __forceinline__ float exact_dist(uint32_t tmem_row, const float* __re
   return acc;
 }
 
+// The exhaustive pass for ONE token (the lane `owner` of this warp) over the codewords its thread owns: the 32-codeword
+// pieces pc = h, h + kParts, ... of the level.  The owner's residual is handed to the warp piece by piece (shuffles) and
+// lane j scores codeword j of every piece, eight at a time, accumulating in exact_dist's order (so a distance has
+// the same bits whichever path computed it: duplicate codewords tie exactly); the minimum (distance, then index) goes
+// back to the owner.  ~40 us per token where the owner alone needed 2-4 ms (K / 2 serial passes with 31 lanes idle):
+// the pass is rare (a token whose candidate lists ran out of room, once in ~3000 steps of the config 3 run) but it
+// was visible as a 4 ms step.  Warp-convergent.
+__device__ __forceinline__ void exhaustive_half(uint32_t tmem_row, const float* __restrict__ Cl, int r, int K, int h,
+                                                int lane, int owner, float* bestx, int* bestk) {
+  const unsigned full = 0xffffffffu;
+  const int npieces = K / 32 / kParts;
+  float bx = FLT_MAX;
+  int bk = 0x7fffffff;
+#pragma unroll 1
+  for (int t0 = 0; t0 < npieces; t0 += 8) {
+    float acc[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) acc[u] = 0.f;
+#pragma unroll 1
+    for (int pc = 0; pc < r / 32; ++pc) {
+      uint32_t v[32];
+      tmem_ld32(tmem_row + pc * 32, v);
+      tmem_ld_wait();
+      float rb[32];
+#pragma unroll
+      for (int j = 0; j < 32; ++j) rb[j] = __shfl_sync(full, __uint_as_float(v[j]), owner);
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        if (t0 + u < npieces) {
+          const int k = (h + kParts * (t0 + u)) * 32 + lane;
+          const float4* c4 = reinterpret_cast<const float4*>(Cl + (long long)k * r + pc * 32);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const float4 c = __ldg(c4 + i);
+            const float d0 = rb[4 * i + 0] - c.x, d1 = rb[4 * i + 1] - c.y, d2 = rb[4 * i + 2] - c.z, d3 = rb[4 * i + 3] - c.w;
+            acc[u] = fmaf(d0, d0, acc[u]); acc[u] = fmaf(d1, d1, acc[u]); acc[u] = fmaf(d2, d2, acc[u]); acc[u] = fmaf(d3, d3, acc[u]);
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int k = (h + kParts * (t0 + u)) * 32 + lane;
+      if (t0 + u < npieces && (acc[u] < bx || (acc[u] == bx && k < bk))) { bx = acc[u]; bk = k; }
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const float ox = __shfl_xor_sync(full, bx, o);
+    const int ok = __shfl_xor_sync(full, bk, o);
+    if (ox < bx || (ox == bx && ok < bk)) { bx = ox; bk = ok; }
+  }
+  if (lane == owner && (bx < *bestx || (bx == *bestx && bk < *bestk))) { *bestx = bx; *bestk = bk; }
+}
+
 // power of two inv with A * inv in [0.5, 1) for the bound A >= max|rho_j| (A == 0 / denormal: inv = 1)
 __device__ __forceinline__ float inv_scale_of(float A) {
   int eb = (int)((__float_as_uint(A) >> 23) & 0xffu);
@@ -782,14 +837,9 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
           if (have && (dx < bestx || (dx == bestx && k < bestk))) { bestx = dx; bestk = k; }
         }
       }
-      if (__any_sync(full, overflow)) {         // exhaustive over the pieces this thread owns
-        for (int pc = h; pc < p.K / 32; pc += kParts)
-          for (int i = 0; i < 32; ++i) {
-            const int k = pc * 32 + i;
-            const float dx = exact_dist(tmem_row, Cl + (long long)k * p.r, p.r);
-            if (overflow && dx < bestx) { bestx = dx; bestk = k; }
-          }
-      }
+      // exhaustive pass over the codeword pieces a thread in overflow owns, done by its whole warp (below)
+      for (unsigned owners = __ballot_sync(full, overflow); owners != 0; owners &= owners - 1)
+        exhaustive_half(tmem_row, Cl, p.r, p.K, h, lane, __ffs(owners) - 1, &bestx, &bestk);
       if (warp == 2 && l == 1) { DBG(20) }
       xDist[mine] = bestx; xK[mine] = bestk;
       epi_sync();
