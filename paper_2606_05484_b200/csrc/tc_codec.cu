@@ -6,6 +6,7 @@
 #include <stdlib.h>
 
 #include "profile.cuh"
+#include "tc_tile_ops.cuh"
 
 namespace mapl {
 
@@ -106,30 +107,39 @@ __device__ __forceinline__ __nv_bfloat16 pack_term(float x, int mode, float sc) 
   return mode == 1 ? lo : __float2bfloat16_rn(r1 - __bfloat162float(lo));
 }
 
-// 32x32 tiles; blockIdx.y = job
+// 64 x 64 tiles (every dimension of a pack job is a multiple of 64 inside the tensor-core envelope); blockIdx.y = job.
+// 16-byte loads, 8-byte stores (four 16-bit values), the transposition through shared memory.  Programmatic dependent
+// launch: the next kernel's prologue may start at once, and the sources are read only after the kernels before this one
+// have completed (U may just have been written by the Stiefel step).
 __global__ void __launch_bounds__(256) k_tc_pack(const PackArgs a) {
-  __shared__ float tile[32][33];
+  __shared__ float tile[64][65];
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   const PackJob j = a.job[blockIdx.y];
-  const int tiles_c = (j.cols + 31) / 32, tiles_r = (j.rows + 31) / 32;
+  const int tiles_c = j.cols / 64, tiles_r = j.rows / 64;
+  const int q = threadIdx.x % 16, y = threadIdx.x / 16;       // q: group of 4 consecutive elements, y: 0 .. 15
   for (int t = blockIdx.x; t < tiles_c * tiles_r; t += gridDim.x) {
-    const int r0 = (t / tiles_c) * 32, c0 = (t % tiles_c) * 32;
-    const int tx = threadIdx.x % 32, ty = threadIdx.x / 32;
-    for (int i = ty; i < 32; i += 8) {
-      const int r = r0 + i, c = c0 + tx;
-      float x = (r < j.rows && c < j.cols) ? j.src[(long long)r * j.cols + c] : 0.f;
-      tile[i][tx] = x;
+    const int r0 = (t / tiles_c) * 64, c0 = (t % tiles_c) * 64;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int r = y + 16 * i;
+      const float4 x = *reinterpret_cast<const float4*>(j.src + (long long)(r0 + r) * j.cols + c0 + 4 * q);
+      tile[r][4 * q + 0] = x.x; tile[r][4 * q + 1] = x.y; tile[r][4 * q + 2] = x.z; tile[r][4 * q + 3] = x.w;
     }
     __syncthreads();
-    if (j.transpose) {
-      for (int i = ty; i < 32; i += 8) {
-        const int c = c0 + i, r = r0 + tx;           // dst row = src col
-        if (c < j.cols && r < j.rows) j.dst[(long long)c * j.pitch + r] = pack_term(tile[tx][i], j.mode, 1.f);
-      }
-    } else {
-      for (int i = ty; i < 32; i += 8) {
-        const int r = r0 + i, c = c0 + tx;
-        const float sc = (j.mode == 2 && r < j.rows) ? j.scale[8 * (r / j.rows_per_scale) + 3] : 1.f;
-        if (r < j.rows && c < j.cols) j.dst[(long long)r * j.pitch + c] = pack_term(tile[i][tx], j.mode, sc);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int u = y + 16 * i;                                // dst row inside the tile
+      __nv_bfloat16 o[4];
+      if (j.transpose) {                                       // dst[c0 + u][r0 + 4 q ..] = src[r0 + 4 q ..][c0 + u]
+#pragma unroll
+        for (int e = 0; e < 4; ++e) o[e] = pack_term(tile[4 * q + e][u], j.mode, 1.f);
+        *reinterpret_cast<uint2*>(j.dst + (long long)(c0 + u) * j.pitch + r0 + 4 * q) = *reinterpret_cast<const uint2*>(o);
+      } else {
+        const float sc = j.mode == 2 ? j.scale[8 * ((r0 + u) / j.rows_per_scale) + 3] : 1.f;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) o[e] = pack_term(tile[u][4 * q + e], j.mode, sc);
+        *reinterpret_cast<uint2*>(j.dst + (long long)(r0 + u) * j.pitch + c0 + 4 * q) = *reinterpret_cast<const uint2*>(o);
       }
     }
     __syncthreads();
@@ -236,8 +246,14 @@ int tc_pack_build(const mapl_boundary_desc& d, const float* U, const float* B, c
   }
   {
     KernelScope ks(KID_TC_PACK, st);
-    k_tc_pack<<<dim3(1024, a.njobs), 256, 0, st>>>(a);      // 32x32 tiles; blocks beyond a job's tile count exit at once
-    MAPL_CUDA_CHECK(cudaGetLastError());
+    int max_tiles = 1;
+    for (int i = 0; i < a.njobs; ++i) {
+      if (a.job[i].rows % 64 || a.job[i].cols % 64) return MAPL_ERR_UNSUPPORTED;     // cannot happen inside the envelope
+      const int t = (a.job[i].rows / 64) * (a.job[i].cols / 64);
+      if (t > max_tiles) max_tiles = t;
+    }
+    // blocks beyond a job's tile count exit at once
+    MAPL_CUDA_CHECK(tc::launch_pdl(k_tc_pack, dim3(max_tiles < 592 ? max_tiles : 592, a.njobs), dim3(256), 0, st, a));
   }
   return MAPL_OK;
 }
