@@ -538,8 +538,7 @@ struct StCtx {
 int ctx_tangent(const StCtx& c, const float* U, const float* G, float* out) {
   const int d = c.d, r = c.r, batch = c.batch;
   if (c.tc) {
-    { KernelScope ks(KID_MEMSET, c.st); MAPL_CUDA_CHECK(cudaMemsetAsync(c.S, 0, (size_t)batch * r * r * 4, c.st)); }
-    MAPL_RETURN_IF(tc_st_split(U, d, r, batch, 0, 0.f, c.Prow, c.Ptr, c.st));
+    MAPL_RETURN_IF(tc_st_split(U, d, r, batch, 0, 0.f, c.Prow, c.Ptr, c.st, c.S, (long long)r * r));   // also clears S
     MAPL_RETURN_IF(tc_st_split(G, d, r, batch, 0, 0.f, nullptr, c.Ptr2, c.st));
     MAPL_RETURN_IF(tc_st_gemm3(c.Ptr, c.Ptr2, r, r, d, batch, c.S, nullptr, 0.f, (d / 64 + 3) / 4, c.st));
     MAPL_RETURN_IF(tc_st_split(c.S, r, r, batch, 3, 0.f, c.Pm, nullptr, c.st));
@@ -645,14 +644,9 @@ int mapl_stiefel_step(int32_t d, int32_t r, int32_t batch, float* U, const float
     // accumulator shows the tensor core's truncating accumulate on diag(X^T X): d = 384 with d / 256 = 1 split ran 6
     // k-blocks in one CTA and left ||U^T U - I||_F = 1.3e-5 (3.4e-6 with two splits of 3).
     const int ksplit = (d / 64 + 3) / 4;
-    auto zero_S = [&]() -> int {
-      KernelScope ks(KID_MEMSET, st);
-      MAPL_CUDA_CHECK(cudaMemsetAsync(S, 0, (size_t)batch * r * r * 4, st));
-      return MAPL_OK;
-    };
-    // S = U^T G ;  M1 = I + lr sym(S) ;  Y = U M1 - lr G  -> X0
-    MAPL_RETURN_IF(zero_S());
-    MAPL_RETURN_IF(tc_st_split(U, d, r, batch, 0, 0.f, Prow, Ptr, st));
+    // S = U^T G ;  M1 = I + lr sym(S) ;  Y = U M1 - lr G  -> X0   (the split of U also clears S: no memset node, which
+    // would break the chain of programmatic dependent launches)
+    MAPL_RETURN_IF(tc_st_split(U, d, r, batch, 0, 0.f, Prow, Ptr, st, S, (long long)r * r));
     MAPL_RETURN_IF(tc_st_split(G, d, r, batch, 0, 0.f, nullptr, Ptr2, st));
     MAPL_RETURN_IF(tc_st_gemm3(Ptr, Ptr2, r, r, d, batch, S, nullptr, 0.f, ksplit, st));
     MAPL_RETURN_IF(tc_st_split(S, r, r, batch, 2, lr, Pm, nullptr, st));     // M1 is symmetric: its planes are B^T too
