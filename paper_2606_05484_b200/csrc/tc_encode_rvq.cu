@@ -122,9 +122,11 @@ __device__ __forceinline__ Smem carve_smem(uint8_t* base, const RvqParams& p) {
 __device__ __forceinline__ float exact_dist(uint32_t tmem_row, const float* __restrict__ crow, int r) {
   // One 32-column piece of the row (8 float4, L2 latency) is in flight while the piece before it is consumed: the
   // pass costs one L2 round trip plus r / 32 short steps, where loading two pieces per round and then consuming them
-  // cost r / 64 round trips (r is a multiple of 64: an even number of pieces).  Same summation order as before.
+  // cost r / 64 round trips (r is a multiple of 64: an even number of pieces).
+  // Four accumulators (columns j = 0, 1, 2, 3 mod 4), summed as (a0 + a1) + (a2 + a3) at the end: one chain of r
+  // dependent FMAs was ~1000 cycles of pure latency per candidate.  exhaustive_half sums in the same order.
   const float4* c4 = reinterpret_cast<const float4*>(crow);
-  float acc = 0.f;
+  float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
   float4 ca[8], cb[8];
   auto consume = [&](const float4 (&c)[8], int pc) {
     uint32_t v[32];
@@ -134,7 +136,7 @@ __device__ __forceinline__ float exact_dist(uint32_t tmem_row, const float* __re
     for (int i = 0; i < 8; ++i) {
       const float d0 = __uint_as_float(v[4 * i + 0]) - c[i].x, d1 = __uint_as_float(v[4 * i + 1]) - c[i].y;
       const float d2 = __uint_as_float(v[4 * i + 2]) - c[i].z, d3 = __uint_as_float(v[4 * i + 3]) - c[i].w;
-      acc = fmaf(d0, d0, acc); acc = fmaf(d1, d1, acc); acc = fmaf(d2, d2, acc); acc = fmaf(d3, d3, acc);
+      a0 = fmaf(d0, d0, a0); a1 = fmaf(d1, d1, a1); a2 = fmaf(d2, d2, a2); a3 = fmaf(d3, d3, a3);
     }
   };
 #pragma unroll
@@ -151,12 +153,12 @@ __device__ __forceinline__ float exact_dist(uint32_t tmem_row, const float* __re
     }
     consume(cb, pc + 1);
   }
-  return acc;
+  return (a0 + a1) + (a2 + a3);
 }
 
 // The exhaustive pass for ONE token (the lane `owner` of this warp) over the codewords its thread owns: the 32-codeword
 // pieces pc = h, h + kParts, ... of the level.  The owner's residual is handed to the warp piece by piece (shuffles) and
-// lane j scores codeword j of every piece, eight at a time, accumulating in exact_dist's order (so a distance has
+// lane j scores codeword j of every piece, four at a time, accumulating in exact_dist's order (so a distance has
 // the same bits whichever path computed it: duplicate codewords tie exactly); the minimum (distance, then index) goes
 // back to the owner.  ~40 us per token where the owner alone needed 2-4 ms (K / 2 serial passes with 31 lanes idle):
 // the pass is rare (a token whose candidate lists ran out of room, once in ~3000 steps of the config 3 run) but it
@@ -168,10 +170,10 @@ __device__ __forceinline__ void exhaustive_half(uint32_t tmem_row, const float* 
   float bx = FLT_MAX;
   int bk = 0x7fffffff;
 #pragma unroll 1
-  for (int t0 = 0; t0 < npieces; t0 += 8) {
-    float acc[8];
+  for (int t0 = 0; t0 < npieces; t0 += 4) {
+    float acc[4][4];
 #pragma unroll
-    for (int u = 0; u < 8; ++u) acc[u] = 0.f;
+    for (int u = 0; u < 4; ++u) { acc[u][0] = 0.f; acc[u][1] = 0.f; acc[u][2] = 0.f; acc[u][3] = 0.f; }
 #pragma unroll 1
     for (int pc = 0; pc < r / 32; ++pc) {
       uint32_t v[32];
@@ -181,7 +183,7 @@ __device__ __forceinline__ void exhaustive_half(uint32_t tmem_row, const float* 
 #pragma unroll
       for (int j = 0; j < 32; ++j) rb[j] = __shfl_sync(full, __uint_as_float(v[j]), owner);
 #pragma unroll
-      for (int u = 0; u < 8; ++u) {
+      for (int u = 0; u < 4; ++u) {
         if (t0 + u < npieces) {
           const int k = (h + kParts * (t0 + u)) * 32 + lane;
           const float4* c4 = reinterpret_cast<const float4*>(Cl + (long long)k * r + pc * 32);
@@ -189,15 +191,17 @@ __device__ __forceinline__ void exhaustive_half(uint32_t tmem_row, const float* 
           for (int i = 0; i < 8; ++i) {
             const float4 c = __ldg(c4 + i);
             const float d0 = rb[4 * i + 0] - c.x, d1 = rb[4 * i + 1] - c.y, d2 = rb[4 * i + 2] - c.z, d3 = rb[4 * i + 3] - c.w;
-            acc[u] = fmaf(d0, d0, acc[u]); acc[u] = fmaf(d1, d1, acc[u]); acc[u] = fmaf(d2, d2, acc[u]); acc[u] = fmaf(d3, d3, acc[u]);
+            acc[u][0] = fmaf(d0, d0, acc[u][0]); acc[u][1] = fmaf(d1, d1, acc[u][1]);
+            acc[u][2] = fmaf(d2, d2, acc[u][2]); acc[u][3] = fmaf(d3, d3, acc[u][3]);
           }
         }
       }
     }
 #pragma unroll
-    for (int u = 0; u < 8; ++u) {
+    for (int u = 0; u < 4; ++u) {
       const int k = (h + kParts * (t0 + u)) * 32 + lane;
-      if (t0 + u < npieces && (acc[u] < bx || (acc[u] == bx && k < bk))) { bx = acc[u]; bk = k; }
+      const float dx = (acc[u][0] + acc[u][1]) + (acc[u][2] + acc[u][3]);
+      if (t0 + u < npieces && (dx < bx || (dx == bx && k < bk))) { bx = dx; bk = k; }
     }
   }
 #pragma unroll
