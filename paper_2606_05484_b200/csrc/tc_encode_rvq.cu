@@ -66,11 +66,12 @@ struct RvqParams {
 
 // smem carve-up (after 1024-byte alignment):
 //   region R = max(phase-1 ring,  rho operand tiles | norm A tile | codebook ring | norm ring | stash)
-//   eM [kne][kEpi] f32 | eId [kne][kEpi] i32 | exchange [6][kEpi] | barriers | tmem slot
+//   eM [kne][kEpi] f32 | eId [kne][kEpi] i32 | exchange [6][kEpi] | xCand [kEpi][4] i32 | barriers | tmem slot
 struct Smem {
   uint8_t* ring1; uint8_t* sRho; uint8_t* sAx; uint8_t* ringC; uint8_t* ringX; uint8_t* stash;
   float* eM; int* eId;
   float* xch;            // [6][kEpi]: best / dist / k / n2 / amax / count exchanged by the threads of a token
+  int* xcand;            // [kEpi][4]: the first candidates of every thread, shared by the threads of a token
   uint64_t* s1_full; uint64_t* s1_empty; uint64_t* z_full;
   uint64_t* c_full; uint64_t* c_empty; uint64_t* x_full; uint64_t* x_empty;
   uint64_t* acc_full; uint64_t* acc_empty; uint64_t* rho_ready;
@@ -86,7 +87,7 @@ __host__ __device__ inline size_t rvq_regionR(const RvqParams& p) {
   return ring1 > lvl ? ring1 : lvl;
 }
 __host__ __device__ inline size_t rvq_tail_bytes(int kne) {
-  return (size_t)kne * kEpi * 8 + 6 * kEpi * 4 + 1024;
+  return (size_t)kne * kEpi * 8 + 6 * kEpi * 4 + kEpi * 4 * 4 + 1024;
 }
 
 __device__ __forceinline__ Smem carve_smem(uint8_t* base, const RvqParams& p) {
@@ -101,6 +102,7 @@ __device__ __forceinline__ Smem carve_smem(uint8_t* base, const RvqParams& p) {
   s.eM = reinterpret_cast<float*>(t); t += (size_t)p.kne * kEpi * 4;
   s.eId = reinterpret_cast<int*>(t); t += (size_t)p.kne * kEpi * 4;
   s.xch = reinterpret_cast<float*>(t); t += 6 * kEpi * 4;
+  s.xcand = reinterpret_cast<int*>(t); t += kEpi * 4 * 4;
   uint64_t* b = reinterpret_cast<uint64_t*>(t);
   s.s1_full = b; b += p.stages1;
   s.s1_empty = b; b += p.stages1;
@@ -798,9 +800,13 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       const int n_ent = entry_count(cl);
       for (int e = 0; e < n_ent; ++e) {
         if (entry_max(cl, e) >= thr) {
-          const uint32_t mk = entry_mask(cl, e, thr);
-          if (mk != 0 && ncand == 0) firstk = entry_gid(cl, e) * 16 + __ffs(mk) - 1;
-          ncand += __popc(mk);
+          const int k0 = entry_gid(cl, e) * 16;
+          for (uint32_t mk = entry_mask(cl, e, thr); mk != 0; mk &= mk - 1) {
+            const int k = k0 + __ffs(mk) - 1;
+            if (ncand == 0) firstk = k;
+            if (ncand < 4) s.xcand[mine * 4 + ncand] = k;     // the partner thread may take some of them (below)
+            ++ncand;
+          }
         }
       }
       if (!live) ncand = 0;
@@ -812,16 +818,27 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
 #endif
       epi_sync();
       if (warp == 2 && l < 4) { DBG(7 + l * 4) }
-      int tot = 0;
-#pragma unroll
-      for (int hh = 0; hh < kParts; ++hh) tot += xCnt[hh * 128 + row];
+      static_assert(kParts == 2, "the balanced exact pass below is written for two threads per token");
+      const int n0 = xCnt[row], n1 = xCnt[128 + row];
+      const int tot = n0 + n1;
       // a single candidate is the minimiser (it is always among the candidates); else exact fp32 re-scoring,
       // lowest distance, lowest index on ties
       const bool rescore = tot >= 2;
       float bestx = FLT_MAX;
       int bestk = 0x7fffffff;
       if (!rescore && ncand == 1) { bestx = -1.f; bestk = firstk; }
-      {
+      // The exact pass costs a warp as many serial passes as its busiest lane has candidates, so the two threads of a
+      // token share the token's candidates: thread h takes numbers h, h + 2, ... of the joint list (the first four of
+      // each thread are in shared memory).  A token with more than four in one thread keeps the per-thread pass.
+      const bool balanced = rescore && tot < 1000 && n0 <= 4 && n1 <= 4;
+      for (int i = h;; i += kParts) {
+        const bool have = balanced && live && i < tot;
+        if (!__any_sync(full, have)) break;
+        const int k = have ? (i < n0 ? s.xcand[row * 4 + i] : s.xcand[(128 + row) * 4 + (i - n0)]) : 0;
+        const float dx = exact_dist(tmem_row, Cl + (long long)k * p.r, p.r);
+        if (have && (dx < bestx || (dx == bestx && k < bestk))) { bestx = dx; bestk = k; }
+      }
+      if (__any_sync(full, rescore && !balanced && !overflow && live)) {
         int e = 0, gid = 0;
         uint32_t mrem = 0;
         while (true) {
@@ -829,7 +846,7 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
             if (entry_max(cl, e) >= thr) { mrem = entry_mask(cl, e, thr); gid = entry_gid(cl, e); }
             ++e;
           }
-          const bool have = rescore && !overflow && live && mrem != 0;
+          const bool have = rescore && !balanced && !overflow && live && mrem != 0;
           if (!__any_sync(full, have)) break;
           int k = 0;
           if (have) { k = gid * 16 + __ffs(mrem) - 1; mrem &= mrem - 1; }
