@@ -276,50 +276,54 @@ __device__ __forceinline__ void rho_first(uint32_t tmem_row, const float* __rest
   *n2_out = n2; *amax_out = amax;
 }
 
-// Levels >= 1: rho <- rho - sub on the own pieces and, in the same pass, the fp16 rounding of rho * inv into the
-// swizzled A-operand tiles.  Two own pieces per round: the row loads of both (16 float4, L2 latency) are in flight
-// together; r / 32 / kParts is 1 (r = 64), 2 or 4.  Warp-convergent.
-__device__ __forceinline__ void rho_update(uint32_t tmem_row, const float* __restrict__ sub, uint8_t* sRho, int row, int r,
-                                           int h, float inv, float* n2_out, float* amax_out) {
+// Levels >= 1: rho <- rho - C[k*] on the own pieces (pc = h, h + kParts, ...) and, in the same pass, the fp16 rounding
+// of rho * inv into the swizzled A-operand tiles.  The codeword segments are loaded CO-OPERATIVELY: eight lanes fetch the
+// 128 bytes of one token's segment, so a load instruction touches 4 full lines; every lane fetching its own token's row
+// touched 32 lines per instruction and the pass was bound by the L1 tag stage (4.6 us at config 3: ~3700 cycles for
+// each round of 16 loads).  The segments go through a per-warp staging buffer (`stage`: 32 tokens x 144 bytes, the pad
+// keeps the 16-byte accesses conflict-free) to the lane that owns the token.  k is the lane's chosen codeword (any valid
+// index on dead rows).  Warp-convergent.
+constexpr int kStagePitch = 144;
+__device__ __forceinline__ void rho_update(uint32_t tmem_row, const float* __restrict__ Cl, int k, uint8_t* sRho, uint8_t* stage,
+                                           int row, int r, int h, int lane, float inv, float* n2_out, float* amax_out) {
+  const unsigned full = 0xffffffffu;
   float n2 = 0.f, amax = 0.f;
   const int npc = r / 32 / kParts;
+  const float* rowp[8];                                  // this lane's share of the fetches: token 4 j + lane / 8, chunk lane % 8
+#pragma unroll
+  for (int j = 0; j < 8; ++j) rowp[j] = Cl + (long long)__shfl_sync(full, k, 4 * j + lane / 8) * r + (lane % 8) * 4;
 #pragma unroll 1
-  for (int i0 = 0; i0 < npc; i0 += 2) {
-    const bool two = i0 + 1 < npc;
-    const int pc0 = h + i0 * kParts, pc1 = pc0 + kParts;
-    float4 c0[8], c1[8];
-    {
-      const float4* a4 = reinterpret_cast<const float4*>(sub + pc0 * 32);
-      const float4* b4 = reinterpret_cast<const float4*>(sub + (two ? pc1 : pc0) * 32);
+  for (int i = 0; i < npc; ++i) {
+    const int pc = h + i * kParts;
+    float4 x[8];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) c0[i] = __ldg(a4 + i);
+    for (int j = 0; j < 8; ++j) x[j] = __ldg(reinterpret_cast<const float4*>(rowp[j] + pc * 32));
 #pragma unroll
-      for (int i = 0; i < 8; ++i) c1[i] = __ldg(b4 + i);
+    for (int j = 0; j < 8; ++j)
+      *reinterpret_cast<float4*>(stage + (4 * j + lane / 8) * kStagePitch + (lane % 8) * 16) = x[j];
+    __syncwarp();
+    float4 c[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) c[j] = *reinterpret_cast<const float4*>(stage + lane * kStagePitch + j * 16);
+    __syncwarp();
+    uint32_t v[32];
+    tmem_ld32(tmem_row + pc * 32, v);
+    tmem_ld_wait();
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      v[4 * j + 0] = __float_as_uint(__uint_as_float(v[4 * j + 0]) - c[j].x);
+      v[4 * j + 1] = __float_as_uint(__uint_as_float(v[4 * j + 1]) - c[j].y);
+      v[4 * j + 2] = __float_as_uint(__uint_as_float(v[4 * j + 2]) - c[j].z);
+      v[4 * j + 3] = __float_as_uint(__uint_as_float(v[4 * j + 3]) - c[j].w);
     }
+    tmem_st32(tmem_row + pc * 32, v);
 #pragma unroll
-    for (int u = 0; u < 2; ++u) {
-      if (u == 1 && !two) break;
-      const int pc = u ? pc1 : pc0;
-      uint32_t v[32];
-      tmem_ld32(tmem_row + pc * 32, v);
-      tmem_ld_wait();
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const float4 c = u ? c1[i] : c0[i];
-        v[4 * i + 0] = __float_as_uint(__uint_as_float(v[4 * i + 0]) - c.x);
-        v[4 * i + 1] = __float_as_uint(__uint_as_float(v[4 * i + 1]) - c.y);
-        v[4 * i + 2] = __float_as_uint(__uint_as_float(v[4 * i + 2]) - c.z);
-        v[4 * i + 3] = __float_as_uint(__uint_as_float(v[4 * i + 3]) - c.w);
-      }
-      tmem_st32(tmem_row + pc * 32, v);
-#pragma unroll
-      for (int i = 0; i < 32; ++i) {
-        const float x = __uint_as_float(v[i]);
-        n2 = fmaf(x, x, n2);
-        amax = fmaxf(amax, fabsf(x));
-      }
-      store_operand_piece(sRho, row, pc, v, inv);
+    for (int j = 0; j < 32; ++j) {
+      const float xv = __uint_as_float(v[j]);
+      n2 = fmaf(xv, xv, n2);
+      amax = fmaxf(amax, fabsf(xv));
     }
+    store_operand_piece(sRho, row, pc, v, inv);
   }
   tmem_st_wait();
   *n2_out = n2; *amax_out = amax;
@@ -881,7 +885,9 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         // maximum); the exact ||rho_new||^2 and max|rho_new| are exchanged behind the hand-off.
         inv = inv_scale_of(amax + __ldg(lv + 4));
         float n2p, amaxp;
-        rho_update(tmem_row, Cl + (long long)bestk * p.r, s.sRho, row, p.r, h, live ? inv : 0.f, &n2p, &amaxp);
+        // (staging buffers: the candidate lists' region is free until the next scan)
+        rho_update(tmem_row, Cl, bestk, s.sRho, s.stash + (size_t)(warp - 2) * 32 * kStagePitch, row, p.r, h, lane,
+                   live ? inv : 0.f, &n2p, &amaxp);
         xN2[mine] = n2p; xAmax[mine] = amaxp;
         write_ax(inv * __ldg(lv + 8 + 2), hard);
         if (warp == 2 && l == 1) { DBG(21) }
