@@ -863,8 +863,13 @@ k_tc_encode_rvq(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
         }
       }
       // exhaustive pass over the codeword pieces a thread in overflow owns, done by its whole warp (below)
-      for (unsigned owners = __ballot_sync(full, overflow); owners != 0; owners &= owners - 1)
+      for (unsigned owners = __ballot_sync(full, overflow); owners != 0; owners &= owners - 1) {
+#ifdef MAPL_DBG2
+        if (lane == 0) atomicAdd(&g_dbg[blockIdx.x * 64 + 58], 1ull);
+        if (lane == __ffs(owners) - 1) { atomicAdd(&g_dbg[blockIdx.x * 64 + 57], hard ? 1ull : 0ull); atomicAdd(&g_dbg[blockIdx.x * 64 + 56], (unsigned long long)cl.novf); }
+#endif
         exhaustive_half(tmem_row, Cl, p.r, p.K, h, lane, __ffs(owners) - 1, &bestx, &bestk);
+      }
       if (warp == 2 && l == 1) { DBG(20) }
       xDist[mine] = bestx; xK[mine] = bestk;
       epi_sync();
