@@ -362,9 +362,12 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
   const uint32_t rank = kPair ? cluster_ctarank() : 0u;
   const int dt = blockIdx.x;                                   // 128 rows of dU
-  const int tb0 = blockIdx.y * p.blocks_per_split;
-  const int tb1 = min(p.n_blocks, tb0 + p.blocks_per_split);
-  const int n_items = (tb1 > tb0 ? tb1 - tb0 : 0) * p.n_src;
+  // token blocks interleaved over the splits and walked from the END of the token range: all CTAs work in one window
+  // that starts where k_tc_bwd_gz finished, i.e. on the part of g that is most likely still in L2 (c1 36.6 -> 35.8 us,
+  // c3 164.8 -> 164.0 us against contiguous ranges walked forwards)
+  const int n_mine = p.n_blocks > (int)blockIdx.y ? (p.n_blocks - 1 - (int)blockIdx.y) / (int)gridDim.y + 1 : 0;
+  const int n_items = n_mine * p.n_src;
+  const int tb0 = p.n_blocks - 1 - (int)blockIdx.y;
   constexpr int kBox = 64 * 128;                               // [64 tokens x 64 cols] bf16 = 8 KB
   const int nb_boxes = kPair ? p.r / 128 : p.r / 64;           // Zhat/gz boxes this CTA loads per item
 
@@ -424,7 +427,7 @@ k_tc_bwd_du(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUt
             tma_load_2d(a + kBox, ma, &full[s], dt * 128 + 64, tb * 64, kEvictFirst);
             for (int j = 0; j < nb_boxes; ++j) tma_load_2d(a + 2 * kBox + j * kBox, mb, &full[s], j * 64, tb * 64, kEvictLast);
           }
-          if (++src == p.n_src) { src = 0; ++tb; }
+          if (++src == p.n_src) { src = 0; tb -= (int)gridDim.y; }
         }
       }
     } else if (warp == 1) {
