@@ -945,16 +945,17 @@ int tc_encode_rvq(const mapl_boundary_desc& d, const void* H, const float* codeb
   p.ovf = reinterpret_cast<uint8_t*>(ovf_ws); p.kovf = kRvqOverflowEntries;
   p.nsplit = pk.WBlo2 ? 3 : 2;
   p.stage1_bytes = kTileBytes + p.nsplit * d.r * 64;
-  // shared memory: the candidate lists take what the codebook ring can spare -- at least two chunks of codebook tiles
-  // in flight, then as many list entries (16-codeword groups) per thread as fit, 8 at most, 3 at least
+  // shared memory: four list entries (16-codeword groups) per thread -- the groups of one chunk take distinct FIFO
+  // slots, and more entries only lengthen the pass over the lists after the scan (measured at config 2: 8 entries
+  // 46.3 us, 4 entries 44.0 us, 5 spilled entries per launch) --, at least a chunk plus one codebook tile in flight,
+  // and the rest of the level region for more ring tiles
   const int nkb = d.r / 64;
   const size_t cap = (size_t)227 * 1024 - 1024;
   p.kne = 0; p.ring_tiles = 0;
-  for (int kne = 8; kne >= 4 && p.kne == 0; --kne)      // >= 4: the groups of one chunk take distinct slots
-    for (int want = 2 * nkb; want >= nkb + 1 && p.kne == 0; --want) {
-      p.kne = kne; p.ring_tiles = want; p.stages1 = 0;
-      if (rvq_level_bytes(p) + rvq_tail_bytes(kne) > cap) p.kne = 0;
-    }
+  for (int want = 2 * nkb; want >= nkb + 1 && p.kne == 0; --want) {
+    p.kne = 4; p.ring_tiles = want; p.stages1 = 0;
+    if (rvq_level_bytes(p) + rvq_tail_bytes(p.kne) > cap) p.kne = 0;
+  }
   if (p.kne == 0) return MAPL_ERR_UNSUPPORTED;
   {   // the rest of the level region goes to the ring
     const size_t spare = cap - rvq_tail_bytes(p.kne) - rvq_level_bytes(p);
